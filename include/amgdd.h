@@ -1,0 +1,163 @@
+/* amgdd.h -- C ABI of the B200-native AMG-DD local-solve hot path.
+ *
+ * Method: Mitchell, Strzodka, Falgout, "Parallel Performance of Algebraic Multigrid Domain
+ * Decomposition (AMG-DD)", arXiv 1906.10575.  "P:NNN" = line NNN of the paper text;
+ * "S1..S8" / "A1..A20" = the readings fixed in DESIGN.md.
+ *
+ * What the library computes: the paper's P "processors" become P virtual subdomains on ONE GPU.
+ *   setup  : AMG hierarchy A_l, P_l, R_l = P_l^T, A_{l+1} = R_l A_l P_l by classical
+ *            Ruge-Stueben coarsening with threshold theta, direct interpolation and Galerkin
+ *            products (S1-S5); per-subdomain composite grids D_l^p, D-bar_l^p grown by eta through
+ *            the graph of A_l with one (or more) ghost layers (eq. 1; S6-S7); local CSR
+ *            blocks uploaded to the device.  Runs once on the host.
+ *   solve  : num_cycles AMG-DD cycles (Alg. 2): global residual r_0 = b - A_0 x,
+ *            restriction r_{l+1} = P_l^T r_l to all levels, gather onto the composite grids, then
+ *            num_fac_cycles AlgFAC V(nu,nu)-cycles per subdomain (Alg. 4) with
+ *            l1-Jacobi relaxation and a dense direct solve on the coarsest level,
+ *            and the update x <- x + u_0^p on the owned dofs.  All on the device.
+ *
+ * Conventions
+ *   - All floating point is IEEE binary64; all indices are 0-based.
+ *   - "HOST" / "DEVICE" says where a pointer must point.  The library never takes ownership of a
+ *     caller's buffer: setup copies what it needs; b and x stay the caller's.
+ *   - Every call returns AMGDD_SUCCESS (0) or a negative amgdd_status; nothing is printed and no
+ *     exception crosses the boundary.  amgdd_last_error_detail() gives a one-line explanation of
+ *     the last failure on the calling thread's handle-less calls (setup) or of the handle.
+ *   - One solve at a time per handle.  Device work is enqueued on the handle's stream
+ *     (amgdd_set_stream; default: the legacy default stream).
+ *   - There is no CPU fallback: without a CUDA device every compute call returns AMGDD_ERR_CUDA.
+ */
+#ifndef AMGDD_H
+#define AMGDD_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct amgdd_handle_s* amgdd_handle_t; /* opaque; owned by the library */
+
+typedef enum amgdd_status {
+    AMGDD_SUCCESS = 0,
+    AMGDD_ERR_BAD_ARG = -1,              /* null pointer, n <= 0, P <= 0, eta < 0, num_ghost < 1, theta not in (0,1],
+                                            max_levels < 1, coarse_max < 1, num_fac_cycles < 1, relax_sweeps < 1,
+                                            num_cycles < 0, level / subdomain index out of range */
+    AMGDD_ERR_BAD_CSR = -2,              /* rowptr[0] != 0 or not monotone, column out of range, columns not strictly
+                                            ascending in a row, missing or non-positive diagonal, structurally
+                                            unsymmetric pattern */
+    AMGDD_ERR_BAD_OWNER = -3,            /* owner value outside [0,P) or a subdomain that owns no dof */
+    AMGDD_ERR_COARSE_TOO_LARGE = -4,     /* coarsening stopped (max_levels or stagnation) with n_L > 4096 */
+    AMGDD_ERR_SINGULAR_COARSE = -5,      /* zero pivot in the dense LU of A_L */
+    AMGDD_ERR_NOT_CONNECTED_UPWARD = -6, /* a P_l entry of a composite row points outside D-bar_{l+1} (P:111,
+                                            P:230: "not necessarily guaranteed"; reading A7): reported, never
+                                            silently dropped */
+    AMGDD_ERR_OUT_OF_MEMORY = -7,        /* host or device allocation failed; detail string has the byte count */
+    AMGDD_ERR_CUDA = -8,                 /* any CUDA runtime error, including "no device" */
+    AMGDD_ERR_INDEX_RANGE = -9           /* a composite level has more than 2^31-1 local nonzeros */
+} amgdd_status;
+
+/* Sizes and the traffic model of DESIGN.md §"Algorithmic bytes". */
+typedef struct amgdd_stats {
+    int32_t num_levels;              /* L + 1 */
+    int32_t num_subdomains;          /* P */
+    int64_t n_fine;                  /* N */
+    int64_t nnz_hierarchy;           /* sum_l nnz(A_l): what plain AMG stores */
+    int64_t nnz_composite_real;      /* sum_{p,l} nnz of A_l over real rows of D_l^p */
+    double overhead;                 /* nnz_composite_real / nnz_hierarchy */
+    double operator_complexity;      /* nnz_hierarchy / nnz(A_0) */
+    int64_t sum_real;                /* sum_{p,l} |D_l^p| */
+    int64_t sum_ghost;               /* sum_{p,l} |D-bar_l^p \ D_l^p| */
+    int64_t dropped_interp_entries;  /* A7 count; setup fails if nonzero */
+    int64_t device_bytes;            /* bytes held on the device by this handle */
+    int64_t shared_level_instances;  /* number of (p,l) pairs that reuse the single global copy of a level */
+    /* algorithmic bytes of one AlgFAC V(nu,nu) iteration over all subdomains with the PRIVATE
+       12 B/nnz CSR model of SURVEY.md §8(d), for nu = 1: [0] first iteration (no residual
+       recalculation), [1] every later iteration */
+    double model_bytes_fac_iter[2];
+    /* bytes of the matrix/index streams the kernel of THIS build actually requests per iteration
+       (vectors stay on chip / in L2), same two cases */
+    double stream_bytes_fac_iter[2];
+    double model_bytes_global;       /* a1+a2+a3+a10 per AMG-DD cycle: A_0 stream, R_l streams, gathers */
+    double setup_seconds_hierarchy;  /* host: S1-S5 */
+    double setup_seconds_composite;  /* host: S6-S7 + local CSR blocks + upload */
+} amgdd_stats_t;
+
+/* ---------------------------------------------------------------------------------------------
+ * amgdd_setup -- problem statement A u = f with owned partition Omega_0^p and padding eta
+ * (Alg. 2).  HOST arrays, copied.
+ *   n            N, number of fine dofs (> 0)
+ *   rowptr       n+1 entries, rowptr[0] = 0, non-decreasing
+ *   colind       rowptr[n] entries, strictly ascending inside each row; the diagonal must be stored
+ *   vals         rowptr[n] entries; an explicitly stored zero IS an edge of the graph (reading A8)
+ *   num_subdomains  P (> 0)
+ *   owner        n entries in [0,P): owner[i] = p  <=>  i in Omega_0^p
+ *   eta          padding eta_l, the same on every level l < L (>= 0; reading A6)
+ *   num_ghost    ghost layers (>= 1; the paper needs exactly 1; reading A13)
+ *   max_levels   stop coarsening at this many levels (>= 1)
+ *   theta        strength threshold in (0,1]  (S1)
+ *   coarse_max   stop coarsening when n_l <= coarse_max (>= 1); ADDED to the north_star signature,
+ *                BASELINE configs 1 and 2 state it ("coarsen to <= 16 / <= 64 dofs")
+ *   out          receives the handle; left NULL on failure
+ * Needs a CUDA device (the composite grids are uploaded).
+ * ------------------------------------------------------------------------------------------- */
+int amgdd_setup(int64_t n, const int64_t* rowptr, const int32_t* colind, const double* vals,
+                int32_t num_subdomains, const int32_t* owner, int32_t eta, int32_t num_ghost,
+                int32_t max_levels, double theta, int32_t coarse_max, amgdd_handle_t* out);
+
+/* amgdd_solve -- num_cycles AMG-DD cycles (Alg. 2 with Alg. 4 inside).
+ *   b, x          DEVICE, n doubles.  x is in/out: initial guess on entry, iterate on return.
+ *   num_cycles    >= 0 (0 only evaluates resnorm[0])
+ *   num_fac_cycles  AlgFAC iterations per cycle (>= 1; Fig. 10)
+ *   relax_sweeps  nu: l1-Jacobi sweeps before and after each coarse correction (>= 1; V(nu,nu))
+ *   resnorm_host  HOST, num_cycles+1 doubles or NULL.  resnorm[k] = || b - A_0 x_k ||_2, k = 0 is
+ *                 the initial guess.  With NULL the call only enqueues work on the handle's
+ *                 stream and returns; otherwise it synchronises the stream before returning. */
+int amgdd_solve(amgdd_handle_t h, const double* b, double* x, int32_t num_cycles,
+                int32_t num_fac_cycles, int32_t relax_sweeps, double* resnorm_host);
+
+/* Same computation with HOST b and x: copies b and x to the device, runs amgdd_solve, copies x
+ * back.  This is the end-to-end entry (host buffers in, host buffers out). */
+int amgdd_solve_host(amgdd_handle_t h, const double* b_host, double* x_host, int32_t num_cycles,
+                     int32_t num_fac_cycles, int32_t relax_sweeps, double* resnorm_host);
+
+/* || b - A_0 x ||_2 (metric of Fig. 6; reading A16).  b, x DEVICE; out HOST. Synchronises. */
+int amgdd_residual_norm(amgdd_handle_t h, const double* b, const double* x, double* out_host);
+
+/* Use this CUDA stream (a cudaStream_t passed as void*; NULL = legacy default stream). */
+int amgdd_set_stream(amgdd_handle_t h, void* cuda_stream);
+
+/* Free everything the handle owns (device and host). NULL is accepted. */
+int amgdd_destroy(amgdd_handle_t h);
+
+/* Static string for a status code. */
+const char* amgdd_strerror(int code);
+
+/* One-line detail of the most recent failure (setup failures included). Thread-local storage. */
+const char* amgdd_last_error_detail(void);
+
+/* ---- introspection: the index-exact contract (S7) and the roofline model ------------------ */
+int amgdd_num_levels(amgdd_handle_t h, int32_t* L_plus_1);
+int amgdd_level_size(amgdd_handle_t h, int32_t l, int64_t* n_l, int64_t* nnzA, int64_t* nnzP);
+/* cf_host: n_l entries, +1 C-point, -1 F-point; l < L. */
+int amgdd_get_cf(amgdd_handle_t h, int32_t l, int8_t* cf_host);
+/* which = 0: A_l (n_l x n_l), 1: P_l (n_l x n_{l+1}, l < L).  HOST outputs sized by amgdd_level_size. */
+int amgdd_get_level_matrix(amgdd_handle_t h, int32_t l, int32_t which, int64_t* rowptr, int32_t* colind,
+                           double* vals);
+int amgdd_composite_size(amgdd_handle_t h, int32_t p, int32_t l, int64_t* n_real, int64_t* n_ghost);
+/* real_gid: |D_l^p| global indices, ascending; ghost_gid: |D-bar_l^p \ D_l^p|, ascending (S7). */
+int amgdd_get_composite(amgdd_handle_t h, int32_t p, int32_t l, int32_t* real_gid, int32_t* ghost_gid);
+int amgdd_get_stats(amgdd_handle_t h, amgdd_stats_t* s);
+
+/* ---- measurement support ------------------------------------------------------------------
+ * Device time (ms, CUDA events on the handle's stream) of the phases of the most recent
+ * amgdd_solve that was given a non-NULL resnorm_host, summed over its cycles:
+ *   ms[0] global residual + norm (a1, a11)   ms[1] restriction chain (a2)
+ *   ms[2] AlgFAC kernel incl. gather and owned update (a3-a10)   ms[3] whole solve
+ * launches[0..2]: kernel launches in the same three groups. */
+int amgdd_last_solve_profile(amgdd_handle_t h, double ms[4], int64_t launches[3]);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* AMGDD_H */

@@ -1,0 +1,214 @@
+"""paper_1906_10575_b200 -- B200-native AMG-DD local-solve hot path (arXiv 1906.10575).
+
+Thin Python binding of the C ABI in include/amgdd.h (same names, argument marshalling only).
+Every step of the path runs in the hand-written CUDA kernels of libamgdd.so; PyTorch supplies
+device memory and streams.  There is no CPU fallback: if libamgdd.so cannot be loaded the import
+fails, and without a CUDA device amgdd_setup returns AMGDD_ERR_CUDA.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+from . import build as _build
+
+_vp, _i32, _i64, _f64 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_double
+
+EXPORTS = [
+    "amgdd_setup", "amgdd_solve", "amgdd_solve_host", "amgdd_residual_norm", "amgdd_set_stream", "amgdd_destroy",
+    "amgdd_strerror", "amgdd_last_error_detail", "amgdd_num_levels", "amgdd_level_size", "amgdd_get_cf",
+    "amgdd_get_level_matrix", "amgdd_composite_size", "amgdd_get_composite", "amgdd_get_stats",
+    "amgdd_last_solve_profile",
+]
+
+
+class AmgddStats(ctypes.Structure):
+    _fields_ = [
+        ("num_levels", _i32), ("num_subdomains", _i32), ("n_fine", _i64), ("nnz_hierarchy", _i64),
+        ("nnz_composite_real", _i64), ("overhead", _f64), ("operator_complexity", _f64), ("sum_real", _i64),
+        ("sum_ghost", _i64), ("dropped_interp_entries", _i64), ("device_bytes", _i64),
+        ("shared_level_instances", _i64), ("model_bytes_fac_iter", _f64 * 2), ("stream_bytes_fac_iter", _f64 * 2),
+        ("model_bytes_global", _f64), ("setup_seconds_hierarchy", _f64), ("setup_seconds_composite", _f64),
+    ]
+
+
+class AmgddError(RuntimeError):
+    def __init__(self, code, what, detail):
+        super().__init__(f"{what} (status {code}): {detail}")
+        self.code = code
+
+
+def _load():
+    lib_path = _build.LIB
+    if not os.path.exists(lib_path):
+        # building is not a fallback: it produces the same CUDA library or raises
+        _build.build()
+    L = ctypes.CDLL(lib_path)
+    L.amgdd_setup.argtypes = [_i64, _vp, _vp, _vp, _i32, _vp, _i32, _i32, _i32, _f64, _i32, ctypes.POINTER(_vp)]
+    L.amgdd_solve.argtypes = [_vp, _vp, _vp, _i32, _i32, _i32, _vp]
+    L.amgdd_solve_host.argtypes = [_vp, _vp, _vp, _i32, _i32, _i32, _vp]
+    L.amgdd_residual_norm.argtypes = [_vp, _vp, _vp, _vp]
+    L.amgdd_set_stream.argtypes = [_vp, _vp]
+    L.amgdd_destroy.argtypes = [_vp]
+    L.amgdd_strerror.restype = ctypes.c_char_p
+    L.amgdd_strerror.argtypes = [ctypes.c_int]
+    L.amgdd_last_error_detail.restype = ctypes.c_char_p
+    L.amgdd_num_levels.argtypes = [_vp, _vp]
+    L.amgdd_level_size.argtypes = [_vp, _i32, _vp, _vp, _vp]
+    L.amgdd_get_cf.argtypes = [_vp, _i32, _vp]
+    L.amgdd_get_level_matrix.argtypes = [_vp, _i32, _i32, _vp, _vp, _vp]
+    L.amgdd_composite_size.argtypes = [_vp, _i32, _i32, _vp, _vp]
+    L.amgdd_get_composite.argtypes = [_vp, _i32, _i32, _vp, _vp]
+    L.amgdd_get_stats.argtypes = [_vp, ctypes.POINTER(AmgddStats)]
+    L.amgdd_last_solve_profile.argtypes = [_vp, _vp, _vp]
+    return L
+
+
+lib = _load()
+
+
+def _check(rc):
+    if rc != 0:
+        raise AmgddError(rc, lib.amgdd_strerror(rc).decode(), lib.amgdd_last_error_detail().decode())
+
+
+def amgdd_strerror(code: int) -> str:
+    return lib.amgdd_strerror(code).decode()
+
+
+def _np(a, dt):
+    return np.ascontiguousarray(a, dtype=dt)
+
+
+class Handle:
+    """Owner of an amgdd_handle_t."""
+
+    def __init__(self, ptr):
+        self._h = ptr
+
+    def __del__(self):
+        self.destroy()
+
+    def destroy(self):
+        if getattr(self, "_h", None):
+            lib.amgdd_destroy(self._h)
+            self._h = None
+
+
+def amgdd_setup(n, rowptr, colind, vals, num_subdomains, owner, eta, num_ghost=1, max_levels=25, theta=0.25,
+                coarse_max=64) -> Handle:
+    """amgdd_setup of include/amgdd.h; numpy (host) arrays in, Handle out."""
+    rowptr = None if rowptr is None else _np(rowptr, np.int64)
+    colind = None if colind is None else _np(colind, np.int32)
+    vals = None if vals is None else _np(vals, np.float64)
+    owner = None if owner is None else _np(owner, np.int32)
+    ptr = lambda a: None if a is None else a.ctypes.data
+    out = _vp()
+    _check(lib.amgdd_setup(n, ptr(rowptr), ptr(colind), ptr(vals), num_subdomains, ptr(owner), eta, num_ghost,
+                           max_levels, theta, coarse_max, ctypes.byref(out)))
+    return Handle(out.value)
+
+
+def _dev_ptr(t, n):
+    import torch
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and t.numel() >= n):
+        raise TypeError("expected a contiguous float64 CUDA tensor of length >= n")
+    return t.data_ptr()
+
+
+def amgdd_set_stream(h: Handle, stream=None):
+    """Use a torch.cuda.Stream (default: torch's current stream)."""
+    import torch
+    s = stream if stream is not None else torch.cuda.current_stream()
+    _check(lib.amgdd_set_stream(h._h, s.cuda_stream))
+
+
+def amgdd_solve(h: Handle, b, x, num_cycles, num_fac_cycles=2, relax_sweeps=1, want_norms=True):
+    """amgdd_solve: b, x float64 CUDA tensors (x in/out).  Returns resnorm[0..num_cycles] or None."""
+    n = amgdd_level_size(h, 0)[0]
+    res = np.empty(num_cycles + 1, dtype=np.float64) if want_norms else None
+    _check(lib.amgdd_solve(h._h, _dev_ptr(b, n), _dev_ptr(x, n), num_cycles, num_fac_cycles, relax_sweeps,
+                           res.ctypes.data if want_norms else None))
+    return res
+
+
+def amgdd_solve_host(h: Handle, b_host, x_host, num_cycles, num_fac_cycles=2, relax_sweeps=1):
+    """amgdd_solve_host: numpy (or pinned torch CPU) float64 arrays, x_host updated in place."""
+    def ptr(a):
+        if isinstance(a, np.ndarray):
+            assert a.dtype == np.float64 and a.flags.c_contiguous
+            return a.ctypes.data
+        return a.data_ptr()
+    res = np.empty(num_cycles + 1, dtype=np.float64)
+    _check(lib.amgdd_solve_host(h._h, ptr(b_host), ptr(x_host), num_cycles, num_fac_cycles, relax_sweeps, res.ctypes.data))
+    return res
+
+
+def amgdd_residual_norm(h: Handle, b, x) -> float:
+    n = amgdd_level_size(h, 0)[0]
+    out = _f64()
+    _check(lib.amgdd_residual_norm(h._h, _dev_ptr(b, n), _dev_ptr(x, n), ctypes.byref(out)))
+    return out.value
+
+
+def amgdd_destroy(h: Handle):
+    h.destroy()
+
+
+def amgdd_num_levels(h: Handle) -> int:
+    out = _i32()
+    _check(lib.amgdd_num_levels(h._h, ctypes.byref(out)))
+    return out.value
+
+
+def amgdd_level_size(h: Handle, l: int):
+    n, a, p = _i64(), _i64(), _i64()
+    _check(lib.amgdd_level_size(h._h, l, ctypes.byref(n), ctypes.byref(a), ctypes.byref(p)))
+    return n.value, a.value, p.value
+
+
+def amgdd_get_cf(h: Handle, l: int) -> np.ndarray:
+    out = np.empty(amgdd_level_size(h, l)[0], dtype=np.int8)
+    _check(lib.amgdd_get_cf(h._h, l, out.ctypes.data))
+    return out
+
+
+def amgdd_get_level_matrix(h: Handle, l: int, which: int):
+    n, nnzA, nnzP = amgdd_level_size(h, l)
+    nnz = nnzA if which == 0 else nnzP
+    rp, ci, v = np.empty(n + 1, np.int64), np.empty(nnz, np.int32), np.empty(nnz, np.float64)
+    _check(lib.amgdd_get_level_matrix(h._h, l, which, rp.ctypes.data, ci.ctypes.data, v.ctypes.data))
+    return rp, ci, v
+
+
+def amgdd_composite_size(h: Handle, p: int, l: int):
+    nr, ng = _i64(), _i64()
+    _check(lib.amgdd_composite_size(h._h, p, l, ctypes.byref(nr), ctypes.byref(ng)))
+    return nr.value, ng.value
+
+
+def amgdd_get_composite(h: Handle, p: int, l: int):
+    nr, ng = amgdd_composite_size(h, p, l)
+    real, ghost = np.empty(nr, np.int32), np.empty(ng, np.int32)
+    _check(lib.amgdd_get_composite(h._h, p, l, real.ctypes.data, ghost.ctypes.data))
+    return real, ghost
+
+
+def amgdd_get_stats(h: Handle) -> dict:
+    s = AmgddStats()
+    _check(lib.amgdd_get_stats(h._h, ctypes.byref(s)))
+    d = {}
+    for name, _ in AmgddStats._fields_:
+        v = getattr(s, name)
+        d[name] = list(v) if hasattr(v, "__len__") else v
+    return d
+
+
+def amgdd_last_solve_profile(h: Handle):
+    ms = (ctypes.c_double * 4)()
+    ln = (ctypes.c_int64 * 3)()
+    _check(lib.amgdd_last_solve_profile(h._h, ms, ln))
+    return {"ms_residual": ms[0], "ms_restrict": ms[1], "ms_fac": ms[2], "ms_total": ms[3],
+            "launches": [int(ln[0]), int(ln[1]), int(ln[2])]}

@@ -1,0 +1,661 @@
+// C ABI of the AMG-DD library (include/amgdd.h): setup orchestration (host hierarchy, threaded
+// composite-grid construction streamed to the device), the solve driver, introspection.
+#include "../../include/amgdd.h"
+#include "amgdd_host.hpp"
+#include "amgdd_kernels.cuh"
+
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <chrono>
+#include <cmath>
+#include <cstring>
+#include <mutex>
+#include <new>
+#include <numeric>
+#include <string>
+
+using namespace amgdd;
+
+namespace {
+
+thread_local std::string g_detail;
+
+struct GlobalLevelDev {          // the single device copy of a whole level (int32 row pointers)
+    int* a_rp = nullptr; int* a_ci = nullptr; double* a_v = nullptr;
+    int* p_rp = nullptr; int* p_ci = nullptr; double* p_v = nullptr;
+    int* r_rp = nullptr; int* r_ci = nullptr; double* r_v = nullptr;
+    double* dinv = nullptr; int* ident = nullptr;
+    int lanes_a = 2, lanes_p = 2, lanes_r = 2;
+};
+
+struct SubMeta {                 // host-side record of one subdomain's blob
+    SubdomainBlob plan;
+    char* dev_base = nullptr;
+};
+
+}  // namespace
+
+struct amgdd_handle_s {
+    Hierarchy H;
+    int P = 0, eta = 0, nghost = 1;
+    i64 n = 0;
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    std::vector<SubMeta> subs;
+    std::vector<GlobalLevelDev> glev;
+    std::vector<void*> allocs;                  // every cudaMalloc the handle owns
+    i64 device_bytes = 0;
+    // tables
+    DevLevel* d_lev = nullptr;
+    DevSub* d_sub = nullptr;
+    int* d_order = nullptr;
+    double* d_r_all = nullptr;
+    long long* d_r_off = nullptr;
+    std::vector<long long> r_off;
+    double* d_workspace = nullptr;
+    long long slot_stride = 0, scratch_off = 0, scratch_len = 0;
+    int num_slots = 0, fac_block = 512;
+    int* d_counter = nullptr;
+    double* d_lu = nullptr; int* d_rowperm = nullptr;
+    double* d_partial = nullptr; int partial_cap = 0;
+    double* d_norms = nullptr; int norms_cap = 0;
+    double* d_b_stage = nullptr; double* d_x_stage = nullptr;   // for amgdd_solve_host
+    amgdd_stats_t stats;
+    double prof_ms[4] = {0, 0, 0, 0};
+    long long prof_launches[3] = {0, 0, 0};
+    std::string detail;
+};
+
+namespace {
+
+#define CUDA_TRY(expr)                                                                    \
+    do {                                                                                  \
+        cudaError_t e__ = (expr);                                                         \
+        if (e__ != cudaSuccess) {                                                         \
+            g_detail = std::string(#expr) + ": " + cudaGetErrorString(e__);               \
+            return e__ == cudaErrorMemoryAllocation ? AMGDD_ERR_OUT_OF_MEMORY : AMGDD_ERR_CUDA; \
+        }                                                                                 \
+    } while (0)
+
+int dev_alloc(amgdd_handle_s* h, void** p, size_t bytes) {
+    if (bytes == 0) bytes = 16;
+    cudaError_t e = cudaMalloc(p, bytes);
+    if (e != cudaSuccess) {
+        g_detail = "cudaMalloc of " + std::to_string(bytes) + " bytes failed (" + std::to_string(h->device_bytes) +
+                   " bytes already held): " + cudaGetErrorString(e);
+        cudaGetLastError();
+        return AMGDD_ERR_OUT_OF_MEMORY;
+    }
+    h->allocs.push_back(*p);
+    h->device_bytes += (i64)bytes;
+    return AMGDD_SUCCESS;
+}
+
+template <class T>
+int upload(amgdd_handle_s* h, T** dptr, const T* src, size_t count) {
+    int rc = dev_alloc(h, (void**)dptr, count * sizeof(T));
+    if (rc) return rc;
+    if (count) CUDA_TRY(cudaMemcpy(*dptr, src, count * sizeof(T), cudaMemcpyHostToDevice));
+    return AMGDD_SUCCESS;
+}
+
+int upload_csr32(amgdd_handle_s* h, const HostCsr& M, int** rp, int** ci, double** v) {
+    if (M.nnz() > (i64)INT32_MAX) { g_detail = "a level matrix has more than 2^31-1 nonzeros"; return AMGDD_ERR_INDEX_RANGE; }
+    std::vector<int> rp32(M.rp.begin(), M.rp.end());
+    int rc = upload(h, rp, rp32.data(), rp32.size());
+    if (rc) return rc;
+    if ((rc = upload(h, ci, M.ci.data(), M.ci.size()))) return rc;
+    return upload(h, v, M.v.data(), M.v.size());
+}
+
+double avg_row(const HostCsr& M) { return M.nrows ? (double)M.nnz() / (double)M.nrows : 1.0; }
+
+void free_handle(amgdd_handle_s* h) {
+    if (!h) return;
+    for (void* p : h->allocs) cudaFree(p);
+    delete h;
+}
+
+// ------------------------------------------------------------------------------------------
+// composite grids: worker threads plan + fill blobs into pinned staging and copy them into a
+// chunked device arena (SURVEY.md §7 hard part 2: stream, never hold everything on the host)
+// ------------------------------------------------------------------------------------------
+struct Arena {
+    std::mutex mu;
+    char* cur = nullptr;
+    size_t left = 0;
+    size_t chunk = (size_t)1 << 30;
+};
+
+int build_composites(amgdd_handle_s* h, const std::vector<i32>& owner, int nthreads) {
+    const int P = h->P, L = h->H.L;
+    std::vector<std::vector<i32>> owned(P);
+    for (i64 i = 0; i < h->n; ++i) owned[owner[i]].push_back((i32)i);
+    h->subs.assign(P, SubMeta());
+    Arena arena;
+    std::atomic<int> status(AMGDD_SUCCESS);
+    std::string fail_detail;
+    std::mutex fail_mu;
+    auto fail = [&](int code, const std::string& d) {
+        std::lock_guard<std::mutex> g(fail_mu);
+        if (status.load() == AMGDD_SUCCESS) { status.store(code); fail_detail = d; }
+    };
+    const int dev = h->device;
+    const int nw = std::max(1, std::min(nthreads, P));
+    std::atomic<int> next(0);
+    std::vector<std::thread> pool;
+    for (int t = 0; t < nw; ++t)
+        pool.emplace_back([&, t]() {
+            (void)t;
+            if (cudaSetDevice(dev) != cudaSuccess) { fail(AMGDD_ERR_CUDA, "cudaSetDevice failed in a setup worker"); return; }
+            cudaStream_t st;
+            if (cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking) != cudaSuccess) { fail(AMGDD_ERR_CUDA, "stream create failed"); return; }
+            char* stage = nullptr;
+            size_t stage_cap = 0;
+            CompositeBuilder cb(h->H, owner, owned, h->eta, h->nghost);
+            for (;;) {
+                const int p = next.fetch_add(1);
+                if (p >= P || status.load() != AMGDD_SUCCESS) break;
+                SubMeta& sm = h->subs[p];
+                cb.plan(p, sm.plan);
+                if (sm.plan.dropped > 0) {
+                    fail(AMGDD_ERR_NOT_CONNECTED_UPWARD, "subdomain " + std::to_string(p) + ": " + std::to_string(sm.plan.dropped) +
+                                                             " interpolation entries of composite rows fall outside D-bar_{l+1}");
+                    break;
+                }
+                bool too_big = false;
+                for (int l = 0; l <= L; ++l)
+                    if (sm.plan.lev[l].nnzA > INT32_MAX || sm.plan.lev[l].nnzP > INT32_MAX) too_big = true;
+                if (too_big) { fail(AMGDD_ERR_INDEX_RANGE, "a composite level exceeds 2^31-1 local nonzeros"); break; }
+                const size_t bytes = (size_t)std::max<i64>(sm.plan.bytes, 16);
+                {   // reserve device space
+                    std::lock_guard<std::mutex> g(arena.mu);
+                    if (arena.left < bytes) {
+                        const size_t want = std::max(arena.chunk, bytes);
+                        void* ptr = nullptr;
+                        cudaError_t e = cudaMalloc(&ptr, want);
+                        if (e != cudaSuccess) {
+                            cudaGetLastError();
+                            fail(AMGDD_ERR_OUT_OF_MEMORY, "device arena: cudaMalloc of " + std::to_string(want) + " bytes failed with " +
+                                                              std::to_string(h->device_bytes) + " bytes already held");
+                            break;
+                        }
+                        h->allocs.push_back(ptr);
+                        h->device_bytes += (i64)want;
+                        arena.cur = (char*)ptr;
+                        arena.left = want;
+                    }
+                    sm.dev_base = arena.cur;
+                    const size_t adv = (bytes + 255) & ~(size_t)255;
+                    arena.cur += std::min(adv, arena.left);
+                    arena.left -= std::min(adv, arena.left);
+                }
+                cudaStreamSynchronize(st);                         // previous copy out of `stage` finished
+                if (stage_cap < bytes) {
+                    if (stage) cudaFreeHost(stage);
+                    stage_cap = bytes + bytes / 4;
+                    if (cudaHostAlloc((void**)&stage, stage_cap, cudaHostAllocDefault) != cudaSuccess) {
+                        cudaGetLastError();
+                        stage = nullptr;
+                        fail(AMGDD_ERR_OUT_OF_MEMORY, "pinned staging buffer of " + std::to_string(stage_cap) + " bytes failed");
+                        break;
+                    }
+                }
+                cb.fill(sm.plan, stage);
+                if (cudaMemcpyAsync(sm.dev_base, stage, (size_t)sm.plan.bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) {
+                    fail(AMGDD_ERR_CUDA, "blob upload failed");
+                    break;
+                }
+            }
+            cudaStreamSynchronize(st);
+            if (stage) cudaFreeHost(stage);
+            cudaStreamDestroy(st);
+        });
+    for (auto& th : pool) th.join();
+    if (status.load() != AMGDD_SUCCESS) { g_detail = fail_detail; return status.load(); }
+    return AMGDD_SUCCESS;
+}
+
+// the SURVEY.md §8(d) traffic model, nu = 1
+void traffic_model(amgdd_handle_s* h) {
+    amgdd_stats_t& s = h->stats;
+    const int L = h->H.L;
+    double model[2] = {0, 0}, stream[2] = {0, 0};
+    for (const SubMeta& sm : h->subs) {
+        for (int l = 0; l < L; ++l) {
+            const BlockLayout& b = sm.plan.lev[l];
+            const BlockLayout& c = sm.plan.lev[l + 1];
+            const double nr = b.n_real, ng = b.n_ghost, nb = nr + ng;
+            const double nrc = c.n_real, nbc = (double)c.n_real + c.n_ghost;
+            const double Ar = 12.0 * b.nnzA_real + 4.0 * nr, Ag = 12.0 * b.nnzA_ghost + 4.0 * ng;
+            const double Pm = 12.0 * b.nnzP + 4.0 * nb, Pt = 12.0 * b.nnzP + 4.0 * nbc;
+            const double Arc = 12.0 * c.nnzA_real + 4.0 * nrc;
+            const double pre = (l == 0) ? (Ar + 8 * nb + 40 * nr) : 32 * nr;
+            const double at = Ar + Ag + 8 * nr + 16 * nb;
+            const double rs = Pt + 8 * nb + 8 * nbc;
+            const double rc = Arc + 16 * nbc + 16 * nrc;
+            const double ip = Pm + 8 * nbc + 16 * nb;
+            const double post = Ar + 8 * nb + 40 * nr;
+            model[0] += pre + at + rs + ip + post;
+            model[1] += pre + at + rs + rc + ip + post;
+            const double spre = (l == 0) ? Ar + 8 * nr : 8 * nr;
+            stream[0] += spre + (Ar + Ag) + Pt + Pm + (Ar + 8 * nr);
+            stream[1] += spre + (Ar + Ag) + Pt + Arc + Pm + (Ar + 8 * nr);
+        }
+    }
+    s.model_bytes_fac_iter[0] = model[0]; s.model_bytes_fac_iter[1] = model[1];
+    s.stream_bytes_fac_iter[0] = stream[0]; s.stream_bytes_fac_iter[1] = stream[1];
+    double g = 12.0 * h->H.lv[0].A.nnz() + 4.0 * h->n + 24.0 * h->n;            // a1: A_0, x, b, r
+    for (int l = 0; l < L; ++l) g += 12.0 * h->H.lv[l].P.nnz() + 4.0 * h->H.lv[l + 1].A.nrows + 8.0 * (h->H.lv[l].A.nrows + h->H.lv[l + 1].A.nrows);
+    g += 12.0 * (double)s.sum_real + 24.0 * h->n;                                // a3 gather, a10 update
+    s.model_bytes_global = g;
+}
+
+int finish_tables(amgdd_handle_s* h) {
+    const int P = h->P, L = h->H.L;
+    // which levels are used through the shared global copy
+    std::vector<char> need(L + 1, 0);
+    i64 shared_inst = 0;
+    for (const SubMeta& sm : h->subs)
+        for (int l = 0; l <= L; ++l)
+            if (sm.plan.lev[l].shared) { need[l] = 1; ++shared_inst; }
+    h->glev.assign(L + 1, GlobalLevelDev());
+    int rc;
+    for (int l = 0; l <= L; ++l) {
+        const HostLevel& lv = h->H.lv[l];
+        GlobalLevelDev& g = h->glev[l];
+        g.lanes_a = pick_lanes(avg_row(lv.A));
+        if (l < L) { g.lanes_p = pick_lanes(avg_row(lv.P)); g.lanes_r = pick_lanes(avg_row(lv.R)); }
+        if (l == 0 || need[l])
+            if ((rc = upload_csr32(h, lv.A, &g.a_rp, &g.a_ci, &g.a_v))) return rc;
+        if (l < L)
+            if ((rc = upload_csr32(h, lv.R, &g.r_rp, &g.r_ci, &g.r_v))) return rc;   // Alg. 2 P:473 needs every R_l
+        if (need[l]) {
+            if (l < L && (rc = upload_csr32(h, lv.P, &g.p_rp, &g.p_ci, &g.p_v))) return rc;
+            if ((rc = upload(h, &g.dinv, lv.dinv.data(), lv.dinv.size()))) return rc;
+            std::vector<int> id((size_t)lv.A.nrows);
+            std::iota(id.begin(), id.end(), 0);
+            if ((rc = upload(h, &g.ident, id.data(), id.size()))) return rc;
+        }
+    }
+    // workspace geometry: per level u | t | s | f (n_bar each), then two scratch vectors
+    long long max_sum = 0, max_nb = 0;
+    std::vector<DevLevel> lev((size_t)P * (L + 1));
+    std::vector<DevSub> sub(P);
+    amgdd_stats_t& st = h->stats;
+    for (int p = 0; p < P; ++p) {
+        const SubMeta& sm = h->subs[p];
+        long long off = 0;
+        for (int l = 0; l <= L; ++l) {
+            const BlockLayout& b = sm.plan.lev[l];
+            DevLevel& d = lev[(size_t)p * (L + 1) + l];
+            std::memset(&d, 0, sizeof(d));
+            d.n_real = b.n_real;
+            d.n_bar = b.n_real + b.n_ghost;
+            max_nb = std::max<long long>(max_nb, d.n_bar);
+            st.sum_real += b.n_real; st.sum_ghost += b.n_ghost; st.nnz_composite_real += b.nnzA_real;
+            if (b.shared) {
+                const GlobalLevelDev& g = h->glev[l];
+                d.gid = g.ident; d.dinv = g.dinv;
+                d.a_rp = g.a_rp; d.a_ci = g.a_ci; d.a_v = g.a_v;
+                d.p_rp = g.p_rp; d.p_ci = g.p_ci; d.p_v = g.p_v;
+                d.r_rp = g.r_rp; d.r_ci = g.r_ci; d.r_v = g.r_v;
+                d.lanes_a = g.lanes_a; d.lanes_p = g.lanes_p; d.lanes_r = g.lanes_r;
+            } else {
+                char* base = sm.dev_base;
+                d.gid = (const int*)(base + b.off_gid); d.dinv = (const double*)(base + b.off_dinv);
+                d.a_rp = (const int*)(base + b.off_a_rp); d.a_ci = (const int*)(base + b.off_a_ci); d.a_v = (const double*)(base + b.off_a_v);
+                d.p_rp = (const int*)(base + b.off_p_rp); d.p_ci = (const int*)(base + b.off_p_ci); d.p_v = (const double*)(base + b.off_p_v);
+                d.r_rp = (const int*)(base + b.off_r_rp); d.r_ci = (const int*)(base + b.off_r_ci); d.r_v = (const double*)(base + b.off_r_v);
+                const double nb = std::max(1, d.n_bar);
+                const double nbc = std::max(1, sm.plan.lev[l + 1].n_real + sm.plan.lev[l + 1].n_ghost);
+                d.lanes_a = pick_lanes((double)b.nnzA / nb);
+                d.lanes_p = pick_lanes((double)b.nnzP / nb);
+                d.lanes_r = pick_lanes((double)b.nnzP / nbc);
+            }
+        }
+        // vectors of a level: u | t | s | f, n_bar doubles each, consecutive; levels 16-byte aligned
+        off = 0;
+        for (int l = 0; l <= L; ++l) {
+            DevLevel& d = lev[(size_t)p * (L + 1) + l];
+            d.voff = off;
+            off += 4LL * d.n_bar;
+            off = (off + 1) & ~1LL;
+        }
+        max_sum = std::max(max_sum, off);
+        sub[p].owned = (const int*)(sm.dev_base + sm.plan.off_owned);
+        sub[p].n_owned = sm.plan.n_owned;
+    }
+    st.shared_level_instances = shared_inst;
+    h->scratch_len = (max_nb + 1) & ~1LL;
+    h->scratch_off = max_sum;
+    h->slot_stride = (max_sum + 2 * h->scratch_len + 15) & ~15LL;
+
+    cudaDeviceProp prop;
+    CUDA_TRY(cudaGetDeviceProperties(&prop, h->device));
+    h->fac_block = 512;
+    const int per_sm = 2;                                       // resident CTAs per SM (512 threads each)
+    h->num_slots = std::max(1, std::min(P, prop.multiProcessorCount * per_sm));
+    if ((rc = dev_alloc(h, (void**)&h->d_workspace, (size_t)h->num_slots * h->slot_stride * sizeof(double)))) return rc;
+    if ((rc = upload(h, &h->d_lev, lev.data(), lev.size()))) return rc;
+    if ((rc = upload(h, &h->d_sub, sub.data(), sub.size()))) return rc;
+    // largest subdomains first (longest-processing-time order for the dynamic scheduler)
+    std::vector<int> order(P);
+    std::iota(order.begin(), order.end(), 0);
+    std::vector<i64> cost(P, 0);
+    for (int p = 0; p < P; ++p) for (int l = 0; l <= L; ++l) cost[p] += h->subs[p].plan.lev[l].nnzA + h->subs[p].plan.lev[l].nnzP;
+    std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return cost[a] > cost[b]; });
+    if ((rc = upload(h, &h->d_order, order.data(), order.size()))) return rc;
+    // residual vectors of all levels, concatenated
+    h->r_off.assign(L + 2, 0);
+    for (int l = 0; l <= L; ++l) h->r_off[l + 1] = h->r_off[l] + (((long long)h->H.lv[l].A.nrows + 1) & ~1LL);
+    if ((rc = dev_alloc(h, (void**)&h->d_r_all, (size_t)h->r_off[L + 1] * sizeof(double)))) return rc;
+    if ((rc = upload(h, &h->d_r_off, h->r_off.data(), (size_t)L + 1))) return rc;
+    if ((rc = dev_alloc(h, (void**)&h->d_counter, sizeof(int)))) return rc;
+    if ((rc = upload(h, &h->d_lu, h->H.lu.data(), h->H.lu.size()))) return rc;
+    if ((rc = upload(h, &h->d_rowperm, h->H.rowperm.data(), h->H.rowperm.size()))) return rc;
+    h->partial_cap = residual_num_blocks(h->n, h->glev[0].lanes_a);
+    if ((rc = dev_alloc(h, (void**)&h->d_partial, (size_t)h->partial_cap * sizeof(double)))) return rc;
+    h->norms_cap = 1024;
+    if ((rc = dev_alloc(h, (void**)&h->d_norms, (size_t)h->norms_cap * sizeof(double)))) return rc;
+    // statistics
+    st.num_levels = L + 1; st.num_subdomains = P; st.n_fine = h->n;
+    st.nnz_hierarchy = 0;
+    for (int l = 0; l <= L; ++l) st.nnz_hierarchy += h->H.lv[l].A.nnz();
+    st.overhead = (double)st.nnz_composite_real / (double)st.nnz_hierarchy;
+    st.operator_complexity = (double)st.nnz_hierarchy / (double)h->H.lv[0].A.nnz();
+    st.dropped_interp_entries = 0;
+    traffic_model(h);
+    st.device_bytes = h->device_bytes;
+    return AMGDD_SUCCESS;
+}
+
+bool bad_handle(amgdd_handle_t h) {
+    if (!h) { g_detail = "null handle"; return true; }
+    return false;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* amgdd_strerror(int code) {
+    switch (code) {
+        case AMGDD_SUCCESS: return "success";
+        case AMGDD_ERR_BAD_ARG: return "bad argument";
+        case AMGDD_ERR_BAD_CSR: return "malformed CSR matrix";
+        case AMGDD_ERR_BAD_OWNER: return "bad owner array";
+        case AMGDD_ERR_COARSE_TOO_LARGE: return "coarsest level too large for the dense solve";
+        case AMGDD_ERR_SINGULAR_COARSE: return "coarsest-level matrix is singular";
+        case AMGDD_ERR_NOT_CONNECTED_UPWARD: return "interpolation stencil of a composite row leaves the composite grid";
+        case AMGDD_ERR_OUT_OF_MEMORY: return "out of memory";
+        case AMGDD_ERR_CUDA: return "CUDA runtime error";
+        case AMGDD_ERR_INDEX_RANGE: return "32-bit local index range exceeded";
+        default: return "unknown status";
+    }
+}
+
+const char* amgdd_last_error_detail(void) { return g_detail.c_str(); }
+
+int amgdd_setup(int64_t n, const int64_t* rowptr, const int32_t* colind, const double* vals,
+                int32_t num_subdomains, const int32_t* owner, int32_t eta, int32_t num_ghost,
+                int32_t max_levels, double theta, int32_t coarse_max, amgdd_handle_t* out) {
+    if (out) *out = nullptr;
+    g_detail.clear();
+    if (!out || !rowptr || !colind || !vals || !owner) { g_detail = "null pointer argument"; return AMGDD_ERR_BAD_ARG; }
+    if (n <= 0 || n > (i64)INT32_MAX) { g_detail = "n must be in [1, 2^31-1]"; return AMGDD_ERR_BAD_ARG; }
+    if (num_subdomains <= 0 || eta < 0 || num_ghost < 1 || max_levels < 1 || coarse_max < 1 || !(theta > 0.0 && theta <= 1.0)) {
+        g_detail = "need P > 0, eta >= 0, num_ghost >= 1, max_levels >= 1, coarse_max >= 1, 0 < theta <= 1";
+        return AMGDD_ERR_BAD_ARG;
+    }
+    int rc = validate_csr(n, rowptr, colind, vals, g_detail);
+    if (rc) return rc;
+    {
+        std::vector<char> seen((size_t)num_subdomains, 0);
+        for (i64 i = 0; i < n; ++i) {
+            if (owner[i] < 0 || owner[i] >= num_subdomains) { g_detail = "owner[" + std::to_string(i) + "] out of range"; return AMGDD_ERR_BAD_OWNER; }
+            seen[owner[i]] = 1;
+        }
+        for (int p = 0; p < num_subdomains; ++p)
+            if (!seen[p]) { g_detail = "subdomain " + std::to_string(p) + " owns no dof"; return AMGDD_ERR_BAD_OWNER; }
+    }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        g_detail = "no CUDA device: this library has no CPU fallback";
+        return AMGDD_ERR_CUDA;
+    }
+    amgdd_handle_s* h = new (std::nothrow) amgdd_handle_s();
+    if (!h) return AMGDD_ERR_OUT_OF_MEMORY;
+    std::memset(&h->stats, 0, sizeof(h->stats));
+    if (cudaGetDevice(&h->device) != cudaSuccess) { delete h; g_detail = "cudaGetDevice failed"; return AMGDD_ERR_CUDA; }
+    h->n = n; h->P = num_subdomains; h->eta = eta; h->nghost = num_ghost;
+    const int nthreads = default_threads();
+    try {
+        auto t0 = std::chrono::steady_clock::now();
+        HostCsr A0;
+        A0.nrows = A0.ncols = n;
+        A0.rp.assign(rowptr, rowptr + n + 1);
+        A0.ci.assign(colind, colind + rowptr[n]);
+        A0.v.assign(vals, vals + rowptr[n]);
+        rc = build_hierarchy(std::move(A0), theta, max_levels, coarse_max, nthreads, h->H, g_detail);
+        if (rc) { free_handle(h); return rc; }
+        auto t1 = std::chrono::steady_clock::now();
+        std::vector<i32> own(owner, owner + n);
+        rc = build_composites(h, own, std::min(nthreads, 32));
+        if (rc) { free_handle(h); return rc; }
+        rc = finish_tables(h);
+        if (rc) { free_handle(h); return rc; }
+        auto t2 = std::chrono::steady_clock::now();
+        h->stats.setup_seconds_hierarchy = std::chrono::duration<double>(t1 - t0).count();
+        h->stats.setup_seconds_composite = std::chrono::duration<double>(t2 - t1).count();
+    } catch (const std::bad_alloc&) {
+        free_handle(h);
+        g_detail = "host allocation failed during setup";
+        return AMGDD_ERR_OUT_OF_MEMORY;
+    }
+    *out = h;
+    return AMGDD_SUCCESS;
+}
+
+int amgdd_destroy(amgdd_handle_t h) {
+    free_handle(h);
+    return AMGDD_SUCCESS;
+}
+
+int amgdd_set_stream(amgdd_handle_t h, void* s) {
+    if (bad_handle(h)) return AMGDD_ERR_BAD_ARG;
+    h->stream = (cudaStream_t)s;
+    return AMGDD_SUCCESS;
+}
+
+}  // extern "C"
+
+namespace {
+
+// r_0 = b - A_0 x with ||r_0||_2 into d_norms[slot]
+int enqueue_residual(amgdd_handle_s* h, const double* b, const double* x, double* r, int norm_slot) {
+    const GlobalLevelDev& g = h->glev[0];
+    int nb = 0;
+    launch_residual(g.a_rp, g.a_ci, g.a_v, h->n, g.lanes_a, b, x, r, h->d_partial, &nb, h->stream);
+    launch_norm_finalize(h->d_partial, nb, h->d_norms + norm_slot, h->stream);
+    return AMGDD_SUCCESS;
+}
+
+}  // namespace
+
+extern "C" {
+
+int amgdd_solve(amgdd_handle_t h, const double* b, double* x, int32_t num_cycles, int32_t num_fac_cycles,
+                int32_t relax_sweeps, double* resnorm_host) {
+    if (bad_handle(h)) return AMGDD_ERR_BAD_ARG;
+    if (!b || !x || num_cycles < 0 || num_fac_cycles < 1 || relax_sweeps < 1 || num_cycles + 1 > h->norms_cap) {
+        g_detail = "need b, x non-null, 0 <= num_cycles < 1024, num_fac_cycles >= 1, relax_sweeps >= 1";
+        return AMGDD_ERR_BAD_ARG;
+    }
+    const int L = h->H.L;
+    const bool timed = resnorm_host != nullptr;
+    std::vector<cudaEvent_t> ev;
+    auto mark = [&]() {
+        if (!timed) return;
+        cudaEvent_t e;
+        cudaEventCreate(&e);
+        cudaEventRecord(e, h->stream);
+        ev.push_back(e);
+    };
+    FacParams prm;
+    prm.lev = h->d_lev; prm.sub = h->d_sub; prm.order = h->d_order;
+    prm.num_sub = h->P; prm.L = L;
+    prm.r_all = h->d_r_all; prm.r_off = h->d_r_off;
+    prm.x = x; prm.workspace = h->d_workspace;
+    prm.slot_stride = h->slot_stride; prm.scratch_off = h->scratch_off; prm.scratch_len = h->scratch_len;
+    prm.work_counter = h->d_counter;
+    prm.nfac = num_fac_cycles; prm.nu = relax_sweeps;
+    prm.lu = h->d_lu; prm.rowperm = h->d_rowperm; prm.nL = (int)h->H.nL;
+    long long launches[3] = {0, 0, 0};
+    mark();
+    for (int k = 0; k < num_cycles; ++k) {
+        enqueue_residual(h, b, x, h->d_r_all, k);                                   // Alg. 2 P:471 (+ a11)
+        launches[0] += 2;
+        mark();
+        for (int l = 0; l < L; ++l) {                                               // Alg. 2
+            const GlobalLevelDev& g = h->glev[l];
+            launch_spmv(g.r_rp, g.r_ci, g.r_v, h->H.lv[l + 1].A.nrows, g.lanes_r, h->d_r_all + h->r_off[l],
+                        h->d_r_all + h->r_off[l + 1], h->stream);
+            launches[1] += 1;
+        }
+        mark();
+        CUDA_TRY(cudaMemsetAsync(h->d_counter, 0, sizeof(int), h->stream));
+        launch_fac(prm, h->num_slots, h->fac_block, h->stream);                     // Alg. 2
+        launches[2] += 1;
+        mark();
+    }
+    enqueue_residual(h, b, x, nullptr, num_cycles);
+    launches[0] += 2;
+    mark();
+    CUDA_TRY(cudaGetLastError());
+    if (timed) {
+        CUDA_TRY(cudaMemcpyAsync(resnorm_host, h->d_norms, (size_t)(num_cycles + 1) * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+        CUDA_TRY(cudaStreamSynchronize(h->stream));
+        double ms[4] = {0, 0, 0, 0};
+        for (int k = 0; k < num_cycles; ++k) {
+            float a = 0, bb = 0, c = 0;
+            cudaEventElapsedTime(&a, ev[3 * k], ev[3 * k + 1]);
+            cudaEventElapsedTime(&bb, ev[3 * k + 1], ev[3 * k + 2]);
+            cudaEventElapsedTime(&c, ev[3 * k + 2], ev[3 * k + 3]);
+            ms[0] += a; ms[1] += bb; ms[2] += c;
+        }
+        float last = 0, tot = 0;
+        cudaEventElapsedTime(&last, ev[3 * num_cycles], ev[3 * num_cycles + 1]);
+        cudaEventElapsedTime(&tot, ev.front(), ev.back());
+        ms[0] += last; ms[3] = tot;
+        for (int i = 0; i < 4; ++i) h->prof_ms[i] = ms[i];
+        for (int i = 0; i < 3; ++i) h->prof_launches[i] = launches[i];
+        for (cudaEvent_t e : ev) cudaEventDestroy(e);
+    }
+    return AMGDD_SUCCESS;
+}
+
+int amgdd_solve_host(amgdd_handle_t h, const double* b_host, double* x_host, int32_t num_cycles,
+                     int32_t num_fac_cycles, int32_t relax_sweeps, double* resnorm_host) {
+    if (bad_handle(h)) return AMGDD_ERR_BAD_ARG;
+    if (!b_host || !x_host) { g_detail = "null host vector"; return AMGDD_ERR_BAD_ARG; }
+    int rc;
+    if (!h->d_b_stage) {
+        if ((rc = dev_alloc(h, (void**)&h->d_b_stage, (size_t)h->n * sizeof(double)))) return rc;
+        if ((rc = dev_alloc(h, (void**)&h->d_x_stage, (size_t)h->n * sizeof(double)))) return rc;
+    }
+    CUDA_TRY(cudaMemcpyAsync(h->d_b_stage, b_host, (size_t)h->n * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+    CUDA_TRY(cudaMemcpyAsync(h->d_x_stage, x_host, (size_t)h->n * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+    rc = amgdd_solve(h, h->d_b_stage, h->d_x_stage, num_cycles, num_fac_cycles, relax_sweeps, resnorm_host);
+    if (rc) return rc;
+    CUDA_TRY(cudaMemcpyAsync(x_host, h->d_x_stage, (size_t)h->n * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    return AMGDD_SUCCESS;
+}
+
+int amgdd_residual_norm(amgdd_handle_t h, const double* b, const double* x, double* out_host) {
+    if (bad_handle(h)) return AMGDD_ERR_BAD_ARG;
+    if (!b || !x || !out_host) { g_detail = "null pointer argument"; return AMGDD_ERR_BAD_ARG; }
+    enqueue_residual(h, b, x, nullptr, 0);
+    CUDA_TRY(cudaGetLastError());
+    CUDA_TRY(cudaMemcpyAsync(out_host, h->d_norms, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    return AMGDD_SUCCESS;
+}
+
+int amgdd_last_solve_profile(amgdd_handle_t h, double ms[4], int64_t launches[3]) {
+    if (bad_handle(h)) return AMGDD_ERR_BAD_ARG;
+    if (ms) for (int i = 0; i < 4; ++i) ms[i] = h->prof_ms[i];
+    if (launches) for (int i = 0; i < 3; ++i) launches[i] = h->prof_launches[i];
+    return AMGDD_SUCCESS;
+}
+
+// ---- introspection ------------------------------------------------------------------------
+int amgdd_num_levels(amgdd_handle_t h, int32_t* out) {
+    if (bad_handle(h) || !out) return AMGDD_ERR_BAD_ARG;
+    *out = h->H.L + 1;
+    return AMGDD_SUCCESS;
+}
+
+int amgdd_level_size(amgdd_handle_t h, int32_t l, int64_t* n_l, int64_t* nnzA, int64_t* nnzP) {
+    if (bad_handle(h)) return AMGDD_ERR_BAD_ARG;
+    if (l < 0 || l > h->H.L) { g_detail = "level out of range"; return AMGDD_ERR_BAD_ARG; }
+    if (n_l) *n_l = h->H.lv[l].A.nrows;
+    if (nnzA) *nnzA = h->H.lv[l].A.nnz();
+    if (nnzP) *nnzP = h->H.lv[l].P.nnz();
+    return AMGDD_SUCCESS;
+}
+
+int amgdd_get_cf(amgdd_handle_t h, int32_t l, int8_t* cf) {
+    if (bad_handle(h) || !cf) return AMGDD_ERR_BAD_ARG;
+    if (l < 0 || l >= h->H.L) { g_detail = "level out of range (cf exists for l < L)"; return AMGDD_ERR_BAD_ARG; }
+    std::copy(h->H.lv[l].cf.begin(), h->H.lv[l].cf.end(), cf);
+    return AMGDD_SUCCESS;
+}
+
+int amgdd_get_level_matrix(amgdd_handle_t h, int32_t l, int32_t which, int64_t* rp, int32_t* ci, double* v) {
+    if (bad_handle(h) || !rp || !ci || !v) return AMGDD_ERR_BAD_ARG;
+    if (l < 0 || l > h->H.L || (which != 0 && which != 1) || (which == 1 && l == h->H.L)) {
+        g_detail = "level / matrix selector out of range";
+        return AMGDD_ERR_BAD_ARG;
+    }
+    const HostCsr& M = which == 0 ? h->H.lv[l].A : h->H.lv[l].P;
+    std::copy(M.rp.begin(), M.rp.end(), rp);
+    std::copy(M.ci.begin(), M.ci.end(), ci);
+    std::copy(M.v.begin(), M.v.end(), v);
+    return AMGDD_SUCCESS;
+}
+
+int amgdd_composite_size(amgdd_handle_t h, int32_t p, int32_t l, int64_t* n_real, int64_t* n_ghost) {
+    if (bad_handle(h)) return AMGDD_ERR_BAD_ARG;
+    if (p < 0 || p >= h->P || l < 0 || l > h->H.L) { g_detail = "subdomain / level out of range"; return AMGDD_ERR_BAD_ARG; }
+    const BlockLayout& b = h->subs[p].plan.lev[l];
+    if (n_real) *n_real = b.n_real;
+    if (n_ghost) *n_ghost = b.n_ghost;
+    return AMGDD_SUCCESS;
+}
+
+int amgdd_get_composite(amgdd_handle_t h, int32_t p, int32_t l, int32_t* real_gid, int32_t* ghost_gid) {
+    if (bad_handle(h)) return AMGDD_ERR_BAD_ARG;
+    if (p < 0 || p >= h->P || l < 0 || l > h->H.L) { g_detail = "subdomain / level out of range"; return AMGDD_ERR_BAD_ARG; }
+    const BlockLayout& b = h->subs[p].plan.lev[l];
+    if (b.shared) {
+        if (real_gid) for (int i = 0; i < b.n_real; ++i) real_gid[i] = i;
+        return AMGDD_SUCCESS;
+    }
+    const char* base = h->subs[p].dev_base + b.off_gid;          // read the device copy back: what the kernels use
+    if (real_gid && b.n_real) CUDA_TRY(cudaMemcpy(real_gid, base, (size_t)b.n_real * 4, cudaMemcpyDeviceToHost));
+    if (ghost_gid && b.n_ghost) CUDA_TRY(cudaMemcpy(ghost_gid, base + (size_t)b.n_real * 4, (size_t)b.n_ghost * 4, cudaMemcpyDeviceToHost));
+    return AMGDD_SUCCESS;
+}
+
+int amgdd_get_stats(amgdd_handle_t h, amgdd_stats_t* s) {
+    if (bad_handle(h) || !s) return AMGDD_ERR_BAD_ARG;
+    h->stats.device_bytes = h->device_bytes;
+    *s = h->stats;
+    return AMGDD_SUCCESS;
+}
+
+}  // extern "C"

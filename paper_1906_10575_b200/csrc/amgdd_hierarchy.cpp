@@ -1,0 +1,284 @@
+// AMG hierarchy on the host (setup phase): classical Ruge-Stueben strength + first-pass C/F
+// colouring, direct interpolation, explicit R = P^T, Galerkin A_{l+1} = R_l A_l P_l (paper P:49),
+// l1 diagonals and the dense LU of the coarsest operator.  Follows readings S1-S5, S8 of
+// DESIGN.md.  Written independently of oracle/ (different data structures and algorithms:
+// per-entry strength flags, lazy max-heap colouring, two-stage threaded sparse products).
+#include "amgdd_host.hpp"
+
+#include <algorithm>
+#include <cmath>
+#include <queue>
+
+namespace amgdd {
+
+namespace {
+enum { ST_OK = 0, ST_BAD_CSR = -2, ST_COARSE_TOO_LARGE = -4, ST_SINGULAR = -5 };
+}
+
+int validate_csr(i64 n, const i64* rp, const i32* ci, const double* v, std::string& detail) {
+    if (rp[0] != 0) { detail = "rowptr[0] != 0"; return ST_BAD_CSR; }
+    for (i64 i = 0; i < n; ++i) {
+        if (rp[i + 1] < rp[i]) { detail = "rowptr not monotone at row " + std::to_string(i); return ST_BAD_CSR; }
+        bool diag = false;
+        for (i64 k = rp[i]; k < rp[i + 1]; ++k) {
+            if (ci[k] < 0 || ci[k] >= n) { detail = "column out of range in row " + std::to_string(i); return ST_BAD_CSR; }
+            if (k > rp[i] && ci[k] <= ci[k - 1]) { detail = "columns not strictly ascending in row " + std::to_string(i); return ST_BAD_CSR; }
+            if (ci[k] == i) {
+                diag = true;
+                if (!(v[k] > 0.0)) { detail = "non-positive diagonal in row " + std::to_string(i); return ST_BAD_CSR; }
+            }
+        }
+        if (!diag) { detail = "missing diagonal in row " + std::to_string(i); return ST_BAD_CSR; }
+    }
+    // structural symmetry: count entries per column, then check (i,j) <-> (j,i) by binary search
+    for (i64 i = 0; i < n; ++i)
+        for (i64 k = rp[i]; k < rp[i + 1]; ++k) {
+            const i32 j = ci[k];
+            if (j == i) continue;
+            const i32* b = ci + rp[j];
+            const i32* e = ci + rp[j + 1];
+            if (!std::binary_search(b, e, (i32)i)) {
+                detail = "pattern not symmetric: (" + std::to_string(i) + "," + std::to_string(j) + ") has no mirror";
+                return ST_BAD_CSR;
+            }
+        }
+    return ST_OK;
+}
+
+namespace {
+
+// S1: flag[k] = 1 iff entry k of A is a strong off-diagonal connection of its row.
+void strength_flags(const HostCsr& A, double theta, int nthreads, std::vector<uint8_t>& flag) {
+    flag.assign((size_t)A.nnz(), 0);
+    parallel_for(A.nrows, nthreads, 4096, [&](int, i64 i) {
+        const i64 b = A.rp[i], e = A.rp[i + 1];
+        double biggest = 0.0;                          // max over off-diagonals of -a_ik, if positive
+        for (i64 k = b; k < e; ++k)
+            if (A.ci[k] != i && -A.v[k] > biggest) biggest = -A.v[k];
+        if (biggest <= 0.0) return;
+        const double cut = theta * biggest * (1.0 - 1e-10);
+        for (i64 k = b; k < e; ++k)
+            if (A.ci[k] != i && A.v[k] < 0.0 && -A.v[k] >= cut) flag[k] = 1;
+    });
+}
+
+// S2: first pass of the RS colouring with a lazy max-heap keyed (lambda desc, index asc).
+void colour(const HostCsr& A, const std::vector<uint8_t>& strong, std::vector<int8_t>& cf) {
+    const i64 n = A.nrows;
+    // transpose lists of the strength graph: who strongly depends on i
+    std::vector<i64> tp(n + 1, 0);
+    for (i64 k = 0; k < A.nnz(); ++k) if (strong[k]) tp[A.ci[k] + 1]++;
+    for (i64 i = 0; i < n; ++i) tp[i + 1] += tp[i];
+    std::vector<i32> tl((size_t)tp[n]);
+    {
+        std::vector<i64> cur(tp.begin(), tp.end() - 1);
+        for (i64 i = 0; i < n; ++i)
+            for (i64 k = A.rp[i]; k < A.rp[i + 1]; ++k)
+                if (strong[k]) tl[cur[A.ci[k]]++] = (i32)i;
+    }
+    std::vector<i32> weight(n);
+    cf.assign(n, 0);
+    auto key = [](i32 w, i32 idx) { return ((uint64_t)(uint32_t)w << 32) | (uint64_t)(0xFFFFFFFFu - (uint32_t)idx); };
+    std::vector<uint64_t> init;
+    init.reserve(n);
+    for (i64 i = 0; i < n; ++i) {
+        weight[i] = (i32)(tp[i + 1] - tp[i]);
+        bool has_strong = false;
+        for (i64 k = A.rp[i]; k < A.rp[i + 1] && !has_strong; ++k) has_strong = strong[k];
+        if (!has_strong && weight[i] == 0) cf[i] = -1;
+        else init.push_back(key(weight[i], (i32)i));
+    }
+    std::priority_queue<uint64_t> heap(std::less<uint64_t>(), std::move(init));
+    while (!heap.empty()) {
+        const uint64_t top = heap.top();
+        heap.pop();
+        const i32 i = (i32)(0xFFFFFFFFu - (uint32_t)(top & 0xFFFFFFFFu));
+        if (cf[i] != 0 || (i32)(top >> 32) != weight[i]) continue;      // stale entry
+        cf[i] = 1;
+        for (i64 a = tp[i]; a < tp[i + 1]; ++a) {
+            const i32 j = tl[a];
+            if (cf[j] != 0) continue;
+            cf[j] = -1;
+            for (i64 k = A.rp[j]; k < A.rp[j + 1]; ++k) {
+                if (!strong[k]) continue;
+                const i32 m = A.ci[k];
+                if (cf[m] == 0) heap.push(key(++weight[m], m));
+            }
+        }
+    }
+}
+
+// S3: direct interpolation.
+void interpolation(const HostCsr& A, const std::vector<uint8_t>& strong, const std::vector<int8_t>& cf,
+                   int nthreads, std::vector<i32>& coarse_of, HostCsr& P) {
+    const i64 n = A.nrows;
+    coarse_of.assign(n, -1);
+    i32 nc = 0;
+    for (i64 i = 0; i < n; ++i) if (cf[i] > 0) coarse_of[i] = nc++;
+    P.nrows = n; P.ncols = nc;
+    P.rp.assign(n + 1, 0);
+    for (i64 i = 0; i < n; ++i) {
+        i64 cnt = 0;
+        if (cf[i] > 0) cnt = 1;
+        else for (i64 k = A.rp[i]; k < A.rp[i + 1]; ++k) cnt += (strong[k] && cf[A.ci[k]] > 0);
+        P.rp[i + 1] = P.rp[i] + cnt;
+    }
+    P.ci.resize((size_t)P.rp[n]);
+    P.v.resize((size_t)P.rp[n]);
+    parallel_for(n, nthreads, 4096, [&](int, i64 i) {
+        i64 q = P.rp[i];
+        if (cf[i] > 0) { P.ci[q] = coarse_of[i]; P.v[q] = 1.0; return; }
+        if (P.rp[i + 1] == q) return;                  // F-point without a strong C neighbour: empty row
+        double diag = 0.0, plus = 0.0, minus = 0.0, strongC = 0.0;
+        for (i64 k = A.rp[i]; k < A.rp[i + 1]; ++k) {
+            const double a = A.v[k];
+            if (A.ci[k] == i) diag = a;
+            else if (a > 0.0) plus += a;
+            else if (a < 0.0) minus += a;
+            if (strong[k] && cf[A.ci[k]] > 0) strongC += a;
+        }
+        const double alpha = minus / strongC, denom = diag + plus;
+        for (i64 k = A.rp[i]; k < A.rp[i + 1]; ++k)
+            if (strong[k] && cf[A.ci[k]] > 0) { P.ci[q] = coarse_of[A.ci[k]]; P.v[q] = -alpha * A.v[k] / denom; ++q; }
+    });
+}
+
+void transpose_csr(const HostCsr& M, HostCsr& T) {
+    T.nrows = M.ncols; T.ncols = M.nrows;
+    T.rp.assign(M.ncols + 1, 0);
+    const i64 nz = M.nnz();
+    for (i64 k = 0; k < nz; ++k) T.rp[M.ci[k] + 1]++;
+    for (i64 c = 0; c < M.ncols; ++c) T.rp[c + 1] += T.rp[c];
+    T.ci.resize((size_t)nz); T.v.resize((size_t)nz);
+    std::vector<i64> cur(T.rp.begin(), T.rp.end() - 1);
+    for (i64 i = 0; i < M.nrows; ++i)
+        for (i64 k = M.rp[i]; k < M.rp[i + 1]; ++k) {
+            const i64 q = cur[M.ci[k]]++;
+            T.ci[q] = (i32)i; T.v[q] = M.v[k];
+        }
+}
+
+// C = X * Y with every structural entry kept, columns ascending; threaded symbolic + numeric.
+void spgemm(const HostCsr& X, const HostCsr& Y, int nthreads, HostCsr& C) {
+    const i64 n = X.nrows, m = Y.ncols;
+    C.nrows = n; C.ncols = m;
+    C.rp.assign(n + 1, 0);
+    std::vector<std::vector<i32>> mark(nthreads);
+    std::vector<std::vector<double>> acc(nthreads);
+    std::vector<std::vector<i32>> cols(nthreads);
+    for (int t = 0; t < nthreads; ++t) mark[t].assign(m, -1);
+    parallel_for(n, nthreads, 2048, [&](int t, i64 i) {
+        std::vector<i32>& mk = mark[t];
+        i64 cnt = 0;
+        for (i64 a = X.rp[i]; a < X.rp[i + 1]; ++a) {
+            const i32 j = X.ci[a];
+            for (i64 b = Y.rp[j]; b < Y.rp[j + 1]; ++b)
+                if (mk[Y.ci[b]] != (i32)i) { mk[Y.ci[b]] = (i32)i; ++cnt; }
+        }
+        C.rp[i + 1] = cnt;
+    });
+    for (i64 i = 0; i < n; ++i) C.rp[i + 1] += C.rp[i];
+    C.ci.resize((size_t)C.rp[n]);
+    C.v.resize((size_t)C.rp[n]);
+    for (int t = 0; t < nthreads; ++t) { mark[t].assign(m, -1); acc[t].assign(m, 0.0); }
+    parallel_for(n, nthreads, 2048, [&](int t, i64 i) {
+        std::vector<i32>& mk = mark[t];
+        std::vector<double>& ac = acc[t];
+        std::vector<i32>& cl = cols[t];
+        cl.clear();
+        for (i64 a = X.rp[i]; a < X.rp[i + 1]; ++a) {
+            const i32 j = X.ci[a];
+            const double xv = X.v[a];
+            for (i64 b = Y.rp[j]; b < Y.rp[j + 1]; ++b) {
+                const i32 c = Y.ci[b];
+                if (mk[c] != (i32)i) { mk[c] = (i32)i; cl.push_back(c); ac[c] = xv * Y.v[b]; }
+                else ac[c] += xv * Y.v[b];
+            }
+        }
+        std::sort(cl.begin(), cl.end());
+        i64 q = C.rp[i];
+        for (i32 c : cl) { C.ci[q] = c; C.v[q] = ac[c]; ++q; }
+    });
+}
+
+void l1_diagonal(const HostCsr& A, int nthreads, std::vector<double>& dinv) {
+    dinv.resize((size_t)A.nrows);
+    parallel_for(A.nrows, nthreads, 8192, [&](int, i64 i) {
+        double s = 0.0;
+        for (i64 k = A.rp[i]; k < A.rp[i + 1]; ++k) s += std::fabs(A.v[k]);
+        dinv[i] = 1.0 / s;
+    });
+}
+
+// column-major right-looking LU with partial pivoting; rowperm[i] = original row now in position i
+bool factor_dense(const HostCsr& A, std::vector<double>& lu, std::vector<i32>& rowperm) {
+    const i64 n = A.nrows;
+    lu.assign((size_t)(n * n), 0.0);
+    for (i64 i = 0; i < n; ++i)
+        for (i64 k = A.rp[i]; k < A.rp[i + 1]; ++k) lu[(size_t)(i + A.ci[k] * n)] = A.v[k];
+    rowperm.resize(n);
+    for (i64 i = 0; i < n; ++i) rowperm[i] = (i32)i;
+    for (i64 c = 0; c < n; ++c) {
+        i64 piv = c;
+        double big = std::fabs(lu[(size_t)(c + c * n)]);
+        for (i64 i = c + 1; i < n; ++i) {
+            const double a = std::fabs(lu[(size_t)(i + c * n)]);
+            if (a > big) { big = a; piv = i; }
+        }
+        if (big == 0.0) return false;
+        if (piv != c) {
+            for (i64 j = 0; j < n; ++j) std::swap(lu[(size_t)(c + j * n)], lu[(size_t)(piv + j * n)]);
+            std::swap(rowperm[c], rowperm[piv]);
+        }
+        const double d = lu[(size_t)(c + c * n)];
+        for (i64 i = c + 1; i < n; ++i) lu[(size_t)(i + c * n)] /= d;
+        for (i64 j = c + 1; j < n; ++j) {
+            const double ucj = lu[(size_t)(c + j * n)];
+            if (ucj == 0.0) continue;
+            for (i64 i = c + 1; i < n; ++i) lu[(size_t)(i + j * n)] -= lu[(size_t)(i + c * n)] * ucj;
+        }
+    }
+    return true;
+}
+
+}  // namespace
+
+int build_hierarchy(HostCsr&& A0, double theta, int max_levels, int coarse_max, int nthreads, Hierarchy& H,
+                    std::string& detail) {
+    H.lv.clear();
+    H.lv.emplace_back();
+    H.lv[0].A = std::move(A0);
+    int l = 0;
+    for (;;) {
+        HostLevel& cur = H.lv[l];
+        l1_diagonal(cur.A, nthreads, cur.dinv);
+        const i64 n = cur.A.nrows;
+        if (n <= coarse_max || l + 1 >= max_levels) break;                       // S5
+        std::vector<uint8_t> strong;
+        strength_flags(cur.A, theta, nthreads, strong);
+        std::vector<int8_t> cf;
+        colour(cur.A, strong, cf);
+        i64 nc = 0;
+        for (i64 i = 0; i < n; ++i) nc += cf[i] > 0;
+        if (nc == 0 || nc == n) break;                                           // S5
+        cur.cf = std::move(cf);
+        interpolation(cur.A, strong, cur.cf, nthreads, cur.coarse_of, cur.P);
+        transpose_csr(cur.P, cur.R);
+        HostCsr AP, Ac;
+        spgemm(cur.A, cur.P, nthreads, AP);
+        spgemm(cur.R, AP, nthreads, Ac);
+        H.lv.emplace_back();
+        H.lv[l + 1].A = std::move(Ac);
+        ++l;
+    }
+    H.L = l;
+    H.nL = H.lv[l].A.nrows;
+    if (H.nL > 4096) {
+        detail = "coarsest level has " + std::to_string(H.nL) + " dofs (> 4096)";
+        return ST_COARSE_TOO_LARGE;
+    }
+    if (!factor_dense(H.lv[l].A, H.lu, H.rowperm)) { detail = "zero pivot in the coarsest-level LU"; return ST_SINGULAR; }
+    return ST_OK;
+}
+
+}  // namespace amgdd

@@ -1,0 +1,125 @@
+// Host-side data structures of the AMG-DD library (setup phase, runs once).
+// Independent of oracle/: nothing here is shared with, included by, or derived from it.
+#pragma once
+#include <atomic>
+#include <cstdint>
+#include <functional>
+#include <string>
+#include <thread>
+#include <vector>
+
+namespace amgdd {
+
+typedef int64_t i64;
+typedef int32_t i32;
+
+struct HostCsr {
+    i64 nrows = 0, ncols = 0;
+    std::vector<i64> rp;
+    std::vector<i32> ci;
+    std::vector<double> v;
+    i64 nnz() const { return rp.empty() ? 0 : rp.back(); }
+};
+
+struct HostLevel {
+    HostCsr A;                   // A_l
+    HostCsr P;                   // P_l (n_l x n_{l+1}); empty on the coarsest level
+    HostCsr R;                   // R_l = P_l^T, stored explicitly (deterministic restriction, no atomics)
+    std::vector<int8_t> cf;      // +1 C / -1 F
+    std::vector<i32> coarse_of;  // fine index -> coarse index (C-points), -1 otherwise
+    std::vector<double> dinv;    // 1 / sum_j |a_ij|   (S8)
+};
+
+struct Hierarchy {
+    std::vector<HostLevel> lv;
+    int L = 0;                   // coarsest level index
+    // dense LU of A_L: P A = L U, stored column-major (lu[i + j*nL]); rowperm[i] = source row of row i
+    std::vector<double> lu;
+    std::vector<i32> rowperm;
+    i64 nL = 0;
+};
+
+// status codes mirror include/amgdd.h (kept numeric here so this header stays free of the C ABI)
+int validate_csr(i64 n, const i64* rowptr, const i32* colind, const double* vals, std::string& detail);
+int build_hierarchy(HostCsr&& A0, double theta, int max_levels, int coarse_max, int nthreads, Hierarchy& H,
+                    std::string& detail);
+
+// ---- tiny fork-join helper: fn(thread_id, item) over items [0,n) with dynamic scheduling ----
+inline int default_threads() {
+    unsigned h = std::thread::hardware_concurrency();
+    if (h == 0) h = 4;
+    return (int)(h > 64 ? 64 : h);
+}
+
+template <class F>
+void parallel_for(i64 n, int nthreads, i64 chunk, F&& fn) {
+    if (nthreads <= 1 || n <= chunk) {
+        for (i64 i = 0; i < n; ++i) fn(0, i);
+        return;
+    }
+    std::atomic<i64> next(0);
+    std::vector<std::thread> th;
+    th.reserve(nthreads);
+    for (int t = 0; t < nthreads; ++t)
+        th.emplace_back([&, t]() {
+            for (;;) {
+                const i64 b = next.fetch_add(chunk);
+                if (b >= n) break;
+                const i64 e = b + chunk < n ? b + chunk : n;
+                for (i64 i = b; i < e; ++i) fn(t, i);
+            }
+        });
+    for (auto& x : th) x.join();
+}
+
+// ---- composite grids (S6, S7) --------------------------------------------------------------
+// Sizes of one (subdomain, level) block and where its arrays sit inside the subdomain's blob.
+struct BlockLayout {
+    i32 n_real = 0, n_ghost = 0;
+    bool shared = false;         // D_l^p = Omega_l: the single global copy of the level is used
+    i64 nnzA = 0, nnzP = 0;      // local nonzeros (ghost rows of A: real columns only)
+    i64 nnzA_real = 0;           // over real rows only (overhead statistic)
+    i64 nnzA_ghost = 0;          // ghost rows x real columns
+    // byte offsets inside the blob (all 16-byte aligned); -1 where absent
+    i64 off_gid = -1, off_dinv = -1;
+    i64 off_a_rp = -1, off_a_ci = -1, off_a_v = -1;
+    i64 off_p_rp = -1, off_p_ci = -1, off_p_v = -1;
+    i64 off_r_rp = -1, off_r_ci = -1, off_r_v = -1;
+};
+
+struct SubdomainBlob {
+    std::vector<BlockLayout> lev;     // L+1 entries
+    i64 off_owned = -1;               // int32 local indices (into level-0 real) of the owned dofs
+    i32 n_owned = 0;
+    i64 bytes = 0;                    // blob size
+    i64 dropped = 0;                  // A7 count
+};
+
+// Per-thread scratch for building composite grids; one instance per worker thread.
+class CompositeBuilder {
+public:
+    CompositeBuilder(const Hierarchy& H, const std::vector<i32>& owner, const std::vector<std::vector<i32>>& owned,
+                     int eta, int num_ghost);
+    // Phase 1: index sets and sizes of subdomain p.  Returns the layout (bytes needed).
+    void plan(int p, SubdomainBlob& out);
+    // Phase 2: write the arrays of the subdomain planned last into dst (out.bytes bytes).
+    void fill(const SubdomainBlob& plan, char* dst);
+    // index sets of the subdomain planned last
+    const std::vector<i32>& real(int l) const { return real_[l]; }
+    const std::vector<i32>& ghost(int l) const { return ghost_[l]; }
+
+private:
+    void grow(int l, const std::vector<i32>& seed, int dist, std::vector<i32>& out);
+    const Hierarchy& H_;
+    const std::vector<i32>& owner_;
+    const std::vector<std::vector<i32>>& owned_;
+    int eta_, nghost_, p_ = -1;
+    std::vector<std::vector<i32>> real_, ghost_;
+    // epoch-stamped global->local maps, one per level
+    std::vector<std::vector<i32>> loc_, stamp_;
+    std::vector<i32> epoch_;
+    std::vector<i32> frontier_, next_;
+    i32 local_of(int l, i32 g) const { return stamp_[l][g] == epoch_[l] ? loc_[l][g] : -1; }
+};
+
+}  // namespace amgdd
