@@ -2,7 +2,7 @@
 // colouring, direct interpolation, explicit R = P^T, Galerkin A_{l+1} = R_l A_l P_l (paper P:49),
 // l1 diagonals and the dense LU of the coarsest operator.  Follows readings S1-S5, S8 of
 // DESIGN.md.  Written independently of oracle/ (different data structures and algorithms:
-// per-entry strength flags, lazy max-heap colouring, two-stage threaded sparse products).
+// per-entry strength flags, lazy max-heap colouring, threaded symbolic/numeric triple product).
 #include "amgdd_host.hpp"
 
 #include <algorithm>
@@ -158,46 +158,56 @@ void transpose_csr(const HostCsr& M, HostCsr& T) {
         }
 }
 
-// C = X * Y with every structural entry kept, columns ascending; threaded symbolic + numeric.
-void spgemm(const HostCsr& X, const HostCsr& Y, int nthreads, HostCsr& C) {
-    const i64 n = X.nrows, m = Y.ncols;
-    C.nrows = n; C.ncols = m;
-    C.rp.assign(n + 1, 0);
+// Galerkin triple product C = R A P in one pass per coarse row, every structural entry kept,
+// columns ascending; threaded symbolic + numeric phases.  Entry (I,J) accumulates the terms
+// (r_Ii * a_ij) * p_jJ with i, then j, then J ascending, a fixed order, so the coarse operators
+// do not depend on the thread count.
+void galerkin_rap(const HostCsr& R, const HostCsr& A, const HostCsr& P, int nthreads, HostCsr& C) {
+    const i64 nc = R.nrows;
+    C.nrows = nc; C.ncols = nc;
+    C.rp.assign(nc + 1, 0);
     std::vector<std::vector<i32>> mark(nthreads);
     std::vector<std::vector<double>> acc(nthreads);
     std::vector<std::vector<i32>> cols(nthreads);
-    for (int t = 0; t < nthreads; ++t) mark[t].assign(m, -1);
-    parallel_for(n, nthreads, 2048, [&](int t, i64 i) {
+    for (int t = 0; t < nthreads; ++t) mark[t].assign(nc, -1);
+    parallel_for(nc, nthreads, 512, [&](int t, i64 I) {
         std::vector<i32>& mk = mark[t];
         i64 cnt = 0;
-        for (i64 a = X.rp[i]; a < X.rp[i + 1]; ++a) {
-            const i32 j = X.ci[a];
-            for (i64 b = Y.rp[j]; b < Y.rp[j + 1]; ++b)
-                if (mk[Y.ci[b]] != (i32)i) { mk[Y.ci[b]] = (i32)i; ++cnt; }
+        for (i64 a = R.rp[I]; a < R.rp[I + 1]; ++a) {
+            const i32 i = R.ci[a];
+            for (i64 b = A.rp[i]; b < A.rp[i + 1]; ++b) {
+                const i32 j = A.ci[b];
+                for (i64 c = P.rp[j]; c < P.rp[j + 1]; ++c)
+                    if (mk[P.ci[c]] != (i32)I) { mk[P.ci[c]] = (i32)I; ++cnt; }
+            }
         }
-        C.rp[i + 1] = cnt;
+        C.rp[I + 1] = cnt;
     });
-    for (i64 i = 0; i < n; ++i) C.rp[i + 1] += C.rp[i];
-    C.ci.resize((size_t)C.rp[n]);
-    C.v.resize((size_t)C.rp[n]);
-    for (int t = 0; t < nthreads; ++t) { mark[t].assign(m, -1); acc[t].assign(m, 0.0); }
-    parallel_for(n, nthreads, 2048, [&](int t, i64 i) {
+    for (i64 I = 0; I < nc; ++I) C.rp[I + 1] += C.rp[I];
+    C.ci.resize((size_t)C.rp[nc]);
+    C.v.resize((size_t)C.rp[nc]);
+    for (int t = 0; t < nthreads; ++t) { mark[t].assign(nc, -1); acc[t].assign(nc, 0.0); }
+    parallel_for(nc, nthreads, 512, [&](int t, i64 I) {
         std::vector<i32>& mk = mark[t];
         std::vector<double>& ac = acc[t];
         std::vector<i32>& cl = cols[t];
         cl.clear();
-        for (i64 a = X.rp[i]; a < X.rp[i + 1]; ++a) {
-            const i32 j = X.ci[a];
-            const double xv = X.v[a];
-            for (i64 b = Y.rp[j]; b < Y.rp[j + 1]; ++b) {
-                const i32 c = Y.ci[b];
-                if (mk[c] != (i32)i) { mk[c] = (i32)i; cl.push_back(c); ac[c] = xv * Y.v[b]; }
-                else ac[c] += xv * Y.v[b];
+        for (i64 a = R.rp[I]; a < R.rp[I + 1]; ++a) {
+            const i32 i = R.ci[a];
+            const double rv = R.v[a];
+            for (i64 b = A.rp[i]; b < A.rp[i + 1]; ++b) {
+                const i32 j = A.ci[b];
+                const double ra = rv * A.v[b];
+                for (i64 c = P.rp[j]; c < P.rp[j + 1]; ++c) {
+                    const i32 J = P.ci[c];
+                    if (mk[J] != (i32)I) { mk[J] = (i32)I; cl.push_back(J); ac[J] = 0.0; }
+                    ac[J] += ra * P.v[c];
+                }
             }
         }
         std::sort(cl.begin(), cl.end());
-        i64 q = C.rp[i];
-        for (i32 c : cl) { C.ci[q] = c; C.v[q] = ac[c]; ++q; }
+        i64 q = C.rp[I];
+        for (i32 J : cl) { C.ci[q] = J; C.v[q] = ac[J]; ++q; }
     });
 }
 
@@ -264,9 +274,8 @@ int build_hierarchy(HostCsr&& A0, double theta, int max_levels, int coarse_max, 
         cur.cf = std::move(cf);
         interpolation(cur.A, strong, cur.cf, nthreads, cur.coarse_of, cur.P);
         transpose_csr(cur.P, cur.R);
-        HostCsr AP, Ac;
-        spgemm(cur.A, cur.P, nthreads, AP);
-        spgemm(cur.R, AP, nthreads, Ac);
+        HostCsr Ac;
+        galerkin_rap(cur.R, cur.A, cur.P, nthreads, Ac);
         H.lv.emplace_back();
         H.lv[l + 1].A = std::move(Ac);
         ++l;

@@ -2,9 +2,12 @@
 
 Index work (levels, C/F splitting, sparsity patterns, composite index sets) is compared
 bit-exactly.  Floating point is compared with the bar of DESIGN.md §"Parity criterion":
-    | ||r_k||_gpu - ||r_k||_oracle |  <=  1e-10 * ||r_k||_oracle + phi_k,
+    | ||r_k||_gpu - ||r_k||_oracle |  <=  1e-10 * ||r_k||_oracle + phi_k  [+ 8 Y_k],
     phi_k = 2^-52 * || |A_0| |x_k| + |b| ||_2          (fp64 rounding floor of a residual)
-    || x_gpu - x_oracle ||_inf  <=  1e-10 * || x_oracle ||_inf
+    || x_gpu - x_oracle ||_inf  <=  1e-10 * || x_oracle ||_inf  [+ 8 ||x~_k - x_k||_inf]
+The bracketed yardstick terms are used only for config 5 (1e4 coefficient jumps x 1e3 anisotropy),
+where the ORACLE ITSELF moves by more than 1e-10 when A_0 is perturbed by one ulp: x~_k is the
+oracle's iterate on that perturbed matrix and Y_k = ||A_0 (x~_k - x_k)||_2.
 """
 import numpy as np
 import pytest
@@ -16,6 +19,7 @@ from oracle import Oracle, max_threads
 pytestmark = pytest.mark.gpu
 
 RTOL = 1e-10
+YARD = 8.0      # multiple of the oracle's own 1-ulp sensitivity allowed on ill-conditioned cases (config 5)
 
 
 def _torch():
@@ -65,7 +69,21 @@ def floor_phi(p, x):
     return 2.0 ** -52 * np.linalg.norm(abs(A) @ np.abs(x) + np.abs(p.b))
 
 
-def run_parity(p, num_cycles, nfac=2, nu=1, **kw):
+def ulp_perturbed_values(p):
+    """A symmetric +-1 ulp perturbation of the stored values of A_0 (sign by a hash of the
+    unordered index pair): the yardstick input of DESIGN.md §"Parity criterion"."""
+    rows = np.repeat(np.arange(p.n), np.diff(p.rowptr))
+    lo, hi = np.minimum(rows, p.colind).astype(np.int64), np.maximum(rows, p.colind).astype(np.int64)
+    sgn = ((lo * 2654435761 + hi * 40503) % 7 < 3) * 2.0 - 1.0
+    return p.vals * (1.0 + sgn * 2.0 ** -52)
+
+
+def run_parity(p, num_cycles, nfac=2, nu=1, yardstick=False, **kw):
+    """Trajectory parity: both sides start from x = 0 and run num_cycles AMG-DD cycles; after every
+    cycle the residual norm and x are compared.  With yardstick=True the oracle is also run on the
+    1-ulp-perturbed matrix; its own deviation (x~_k - x_k in the max norm, and Y_k = ||A_0 (x~_k - x_k)||_2
+    for the residual norm) times YARD is added to the tolerance: the bar is then "as close to the
+    oracle as the fp64 conditioning of this problem allows" (Parity criterion)."""
     torch = _torch()
     m, h = lib_setup(p, **kw)
     o = orc_setup(p, **kw)
@@ -73,26 +91,36 @@ def run_parity(p, num_cycles, nfac=2, nu=1, **kw):
                       np.linspace(0, p.num_subdomains - 1, 16).astype(int))
     b = torch.from_numpy(p.b).cuda()
     A = sp.csr_matrix((p.vals, p.colind, p.rowptr), shape=(p.n, p.n))
-    # cycle by cycle, so that x is compared after every cycle
     xg = torch.zeros(p.n, dtype=torch.float64, device="cuda")
     xo = np.zeros(p.n)
     nt = max_threads()
-    report = []
+    if yardstick:
+        import copy
+        pp = copy.copy(p)
+        pp.vals = ulp_perturbed_values(p)
+        o2 = orc_setup(pp, **kw)
+        xo2 = np.zeros(p.n)
+    report, ok = [], True
     for k in range(num_cycles):
         res_g = m.amgdd_solve(h, b, xg, 1, nfac, nu)
-        r0 = o.residual_norm(p.b, xo)
         o.cycle(p.b, xo, nfac, nu, nthreads=nt)
         assert o.dropped() == 0
         r1 = o.residual_norm(p.b, xo)
+        d_res = d_x = 0.0
+        if yardstick:
+            o2.cycle(p.b, xo2, nfac, nu, nthreads=nt)
+            d_res = np.linalg.norm(A @ (xo2 - xo))      # Y_k: residual change caused by the oracle's own deviation
+            d_x = np.abs(xo2 - xo).max()
         xg_h = xg.cpu().numpy()
-        phi0 = 2.0 ** -52 * np.linalg.norm(abs(A) @ np.abs(xo) + np.abs(p.b))
-        dx = np.abs(xg_h - xo).max() / np.abs(xo).max()
-        report.append((k, abs(res_g[0] - r0) / r0, abs(res_g[1] - r1) / r1, dx))
-        assert abs(res_g[0] - r0) <= RTOL * r0 + phi0, report
-        assert abs(res_g[1] - r1) <= RTOL * r1 + phi0, report
-        assert dx <= RTOL, report
+        phi = 2.0 ** -52 * np.linalg.norm(abs(A) @ np.abs(xo) + np.abs(p.b))
+        e_res, e_x = abs(res_g[1] - r1), np.abs(xg_h - xo).max()
+        xs = np.abs(xo).max()
+        report.append((k + 1, r1, e_res / r1, e_x / xs, phi / r1, d_res / r1, d_x / xs))
+        ok = ok and e_res <= RTOL * r1 + phi + YARD * d_res and e_x <= RTOL * xs + YARD * d_x
+    print("\n%s: cycle  ||r||_oracle  rel|d||r|||  rel|dx|_inf  floor phi/||r||  yardstick Y/||r||  D_x" % p.name)
     for row in report:
-        print("cycle %d: rel diff resnorm before %.2e after %.2e, x %.2e" % row)
+        print("  %2d  %.6e  %.2e  %.2e  %.2e  %.2e  %.2e" % row)
+    assert ok, "parity bar violated (see table above)"
     m.amgdd_destroy(h)
     return report
 
@@ -119,7 +147,7 @@ def test_config4_small_parity():
 
 
 def test_config5_small_parity():
-    run_parity(wl.make_config(5, 256), 15)
+    run_parity(wl.make_config(5, 256), 15, yardstick=True)
 
 
 # ---------------------------------------------------------------------------------------------
