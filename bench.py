@@ -1,0 +1,320 @@
+#!/usr/bin/env python
+"""bench.py -- AMG-DD cycle time on B200 (metric of BASELINE.json: "AMG-DD cycle time (ms),
+FAC-sweep HBM GB/s vs peak, residual drop/cycle").
+
+A "step" is ONE AMG-DD cycle (Alg. 2) over the whole workload: global residual and
+its norm (a1, a11), restriction to all levels (a2), and the persistent AlgFAC kernel that gathers
+the residuals, runs num_fac_cycles V(1,1) AlgFAC cycles on every subdomain and updates the owned
+dofs (a3-a10).  Default workload: BASELINE.json configs[3] (3D variable-coefficient diffusion,
+192^3, 4096 subdomains, eta = 2), the largest config that fits one B200.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config {1,2,3,4,5}] [--scale S] [--impl reference]
+
+One JSON line on stdout (rank 0).  With --impl reference the CPU oracle is timed instead (on a
+bounded sample of the same workload); see DESIGN.md §Measurement.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "amgdd_cycle_time"
+UNIT = "ms"
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4)
+    ap.add_argument("--scale", type=int, default=None, help="grid edge override (smaller instance of the recipe)")
+    ap.add_argument("--eta", type=int, default=None)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--cpu-sample", type=int, default=None, help="subdomains in the oracle's timed sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def workload_name(p, args):
+    return f"{p.name}-P{p.num_subdomains}-eta{p.eta}-fac{p.num_fac_cycles}xV({p.relax_sweeps},{p.relax_sweeps})"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md)."""
+
+    QUERY = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.rows = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.QUERY}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            if len(r) < 6:
+                continue
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, r[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def measured_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        try:
+            return float(json.load(open(path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def ncu_traffic(workload):
+    """DRAM bytes per AlgFAC launch from the committed ncu --set full capture of this workload."""
+    path = os.path.join(ROOT, "profiles", "fac_kernel_traffic.json")
+    if os.path.exists(path):
+        try:
+            d = json.load(open(path))
+            return d.get(workload)
+        except Exception:
+            return None
+    return None
+
+
+# ---------------------------------------------------------------------------------------------
+# CPU oracle leg (cpu_baseline of the b200 arm, and the whole --impl reference arm)
+# ---------------------------------------------------------------------------------------------
+def oracle_time_per_cycle(p, sample, steps, warmup):
+    """Times the oracle AS IT STANDS on a bounded sample: every step runs Alg. 2's global residual +
+    restriction over the whole problem and AlgFAC on `sample` subdomains (spread evenly over the
+    partition); the per-cycle estimate scales the AlgFAC part by P / sample."""
+    from oracle import Oracle, max_threads
+    t0 = time.time()
+    o = Oracle(p.n, p.rowptr, p.colind, p.vals, p.theta, p.max_levels, p.coarse_max)
+    o.set_partition(p.num_subdomains, p.owner, p.eta, p.num_ghost)
+    setup_s = time.time() - t0
+    nthreads = max_threads()
+    sample = max(1, min(sample, p.num_subdomains))
+    subs = np.unique(np.linspace(0, p.num_subdomains - 1, sample).astype(np.int32))
+    x = np.zeros(p.n)
+    for _ in range(max(1, warmup)):
+        o.cycle(p.b, x, p.num_fac_cycles, p.relax_sweeps, subdomains=subs, nthreads=nthreads)   # also builds the composite grids (setup)
+    times = []
+    for _ in range(steps):
+        t = time.time()
+        o.cycle(p.b, x, p.num_fac_cycles, p.relax_sweeps, subdomains=subs, nthreads=nthreads)
+        times.append(time.time() - t)
+    t_sample = float(np.mean(times))
+    est_ms = 1e3 * t_sample * p.num_subdomains / len(subs)
+    return {"value": est_ms, "unit": UNIT, "cores": nthreads, "kind": "oracle",
+            "sample": f"{len(subs)} of {p.num_subdomains} subdomains per step (AlgFAC part scaled by P/sample; "
+                      f"global residual+restriction run in full), {steps} steps, oracle setup {setup_s:.1f}s not timed",
+            "sample_seconds_per_step": t_sample}
+
+
+def default_cpu_sample(p):
+    # about 10-30 s of CPU work in total: ~0.07 core-seconds per config-4 subdomain-cycle
+    return {1: 4, 2: 64, 3: 8, 4: 64, 5: 256}.get(int(p.name[3]), 32)
+
+
+def run_reference(args, p, rank, world):
+    if rank != 0:
+        return
+    steps, warmup = args.steps, args.warmup
+    sample = args.cpu_sample or default_cpu_sample(p)
+    steps_cpu = max(1, min(steps, 3))
+    cb = oracle_time_per_cycle(p, sample, steps_cpu, 1)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus,
+        "steps": steps, "warmup": warmup, "ms_per_step": cb["value"], "higher_is_better": False,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(p, args), "note": "CPU oracle, bounded sample, timed steps capped at 3"},
+        "cpu_baseline": cb,
+        "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+# ---------------------------------------------------------------------------------------------
+# B200 arm
+# ---------------------------------------------------------------------------------------------
+def run_b200(args, p, rank, world, local_rank):
+    import torch
+    import torch.distributed as dist
+    import paper_1906_10575_b200 as m
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the B200 arm has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    distributed = world > 1
+    if distributed:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    t0 = time.time()
+    h = m.amgdd_setup(p.n, p.rowptr, p.colind, p.vals, p.num_subdomains, p.owner, p.eta, p.num_ghost,
+                      p.max_levels, p.theta, p.coarse_max)
+    setup_s = time.time() - t0
+    st = m.amgdd_get_stats(h)
+    stream = torch.cuda.current_stream()
+    m.amgdd_set_stream(h, stream)
+    b = torch.from_numpy(p.b).cuda()
+    x = torch.zeros(p.n, dtype=torch.float64, device="cuda")
+    nfac, nu = p.num_fac_cycles, p.relax_sweeps
+
+    def barrier():
+        if distributed:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- residual drop per cycle (also warms everything up) ----
+    res = m.amgdd_solve(h, b, x, p.num_cycles, nfac, nu)
+    drops = (res[1:] / res[:-1]).tolist()
+    x.zero_()
+    for _ in range(args.warmup):
+        m.amgdd_solve(h, b, x, 1, nfac, nu, want_norms=False)
+
+    # ---- timed region: exactly K steps, device-resident inputs ----
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(stream)
+    for _ in range(args.steps):
+        m.amgdd_solve(h, b, x, 1, nfac, nu, want_norms=False)
+    e1.record(stream)
+    barrier()
+    ms_total = e0.elapsed_time(e1)
+
+    # ---- the dominant kernel: per-launch duration from the library's CUDA events on its stream ----
+    x.zero_()
+    fac_ms, launches = [], None
+    for _ in range(args.steps):
+        m.amgdd_solve(h, b, x, 1, nfac, nu)
+        prof = m.amgdd_last_solve_profile(h)
+        fac_ms.append(prof["ms_fac"])
+        launches = prof["launches"]
+    clocks = sampler.stop()
+    fac_avg_ms = float(np.mean(fac_ms))
+
+    # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region ----
+    bh = torch.from_numpy(p.b).pin_memory()
+    xh = torch.zeros(p.n, dtype=torch.float64).pin_memory()
+    for _ in range(2):
+        m.amgdd_solve_host(h, bh, xh, 1, nfac, nu)
+    barrier()
+    t = time.perf_counter()
+    for _ in range(args.steps):
+        m.amgdd_solve_host(h, bh, xh, 1, nfac, nu)
+    torch.cuda.synchronize()
+    e2e_ms = 1e3 * (time.perf_counter() - t) / args.steps
+
+    ms_step = ms_total / args.steps
+    vals = torch.tensor([ms_step, e2e_ms, fac_avg_ms], dtype=torch.float64, device="cuda")
+    if distributed:
+        dist.all_reduce(vals, op=dist.ReduceOp.MAX)
+    ms_step, e2e_ms, fac_avg_ms = [float(v) for v in vals.tolist()]
+
+    if rank == 0:
+        peak, peak_src = measured_peak()
+        model_bytes = st["model_bytes_fac_iter"][0] + (nfac - 1) * st["model_bytes_fac_iter"][1]
+        stream_bytes = st["stream_bytes_fac_iter"][0] + (nfac - 1) * st["stream_bytes_fac_iter"][1]
+        achieved = model_bytes / (fac_avg_ms * 1e-3) / 1e9
+        wname = workload_name(p, args)
+        line = {
+            "metric": METRIC, "value": ms_step, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": False,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {
+                "workload": wname, "n_dofs": p.n, "nnz": p.nnz, "subdomains": p.num_subdomains, "eta": p.eta,
+                "theta": p.theta, "levels": st["num_levels"], "fac_cycles_per_step": nfac, "relax_sweeps": nu,
+                "composite_overhead": st["overhead"], "device_bytes": st["device_bytes"],
+                "l2_policy": "inputs larger than L2 (matrix streams %.1f GB per step)" % (stream_bytes / 1e9),
+                "multi_gpu": "replicas only (north_star: one GPU, no sharding, no collectives)" if args.gpus > 1 else "single GPU",
+                "setup_seconds": setup_s, "setup_seconds_hierarchy": st["setup_seconds_hierarchy"],
+                "setup_seconds_composite": st["setup_seconds_composite"],
+            },
+            "clocks": clocks,
+            "e2e": {"value": e2e_ms, "unit": UNIT, "h2d_bytes_per_step": 2 * 8 * p.n, "d2h_bytes_per_step": 8 * p.n + 16},
+            "gpu_launches": int(sum(launches)) * args.steps if launches else 0,
+            "launches_per_step": launches,
+            "residual_drop_per_cycle": drops,
+            "residual_norms": res.tolist(),
+            "phase_ms_per_step": {"fac_kernel": fac_avg_ms},
+            "roofline": {
+                "bound": "hbm", "kernel": "fac_kernel (persistent AlgFAC, a3-a10)", "achieved": achieved, "peak": peak,
+                "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": model_bytes, "stream_bytes_per_launch": stream_bytes,
+                "stream_gbs": stream_bytes / (fac_avg_ms * 1e-3) / 1e9, "launch_ms": fac_avg_ms,
+                "traffic": ncu_traffic(wname),
+            },
+        }
+        if not args.no_cpu_baseline:
+            m.amgdd_destroy(h)
+            del b, x
+            torch.cuda.empty_cache()
+            line["cpu_baseline"] = oracle_time_per_cycle(p, args.cpu_sample or default_cpu_sample(p), 1, 1)
+        print(json.dumps(line))
+    if distributed:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference" and rank != 0:
+        return
+    import workloads as wl
+    p = wl.make_config(args.config, args.scale, eta=args.eta)
+    if args.impl == "reference":
+        run_reference(args, p, rank, world)
+    else:
+        run_b200(args, p, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()
