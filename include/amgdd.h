@@ -54,7 +54,9 @@ typedef enum amgdd_status {
                                             silently dropped */
     AMGDD_ERR_OUT_OF_MEMORY = -7,        /* host or device allocation failed; detail string has the byte count */
     AMGDD_ERR_CUDA = -8,                 /* any CUDA runtime error, including "no device" */
-    AMGDD_ERR_INDEX_RANGE = -9           /* a composite level has more than 2^31-1 local nonzeros */
+    AMGDD_ERR_INDEX_RANGE = -9           /* a composite level has more than 2^31-1 local nonzeros, or a local
+                                            matrix row does not fit one stream chunk (about 1,600 nonzeros
+                                            at the default 16 KiB chunk) */
 } amgdd_status;
 
 /* Sizes and the traffic model of DESIGN.md §"Algorithmic bytes". */
@@ -75,12 +77,18 @@ typedef struct amgdd_stats {
        12 B/nnz CSR model of SURVEY.md §8(d), for nu = 1: [0] first iteration (no residual
        recalculation), [1] every later iteration */
     double model_bytes_fac_iter[2];
-    /* bytes of the matrix/index streams the kernel of THIS build actually requests per iteration
-       (vectors stay on chip / in L2), same two cases */
+    /* bytes of the packed matrix streams the kernel of THIS build actually requests from HBM per
+       iteration (chunk copies; vectors stay in shared memory / L2), same two cases */
     double stream_bytes_fac_iter[2];
     double model_bytes_global;       /* a1+a2+a3+a10 per AMG-DD cycle: A_0 stream, R_l streams, gathers */
     double setup_seconds_hierarchy;  /* host: S1-S5 */
-    double setup_seconds_composite;  /* host: S6-S7 + local CSR blocks + upload */
+    double setup_seconds_composite;  /* host: S6-S7 + local matrices + packing + upload */
+    /* launch plan of the persistent AlgFAC kernel */
+    int32_t chunk_bytes;             /* stride of a packed-stream chunk = size of a ring slot */
+    int32_t ring_stages;             /* ring slots per CTA */
+    int32_t x_cap;                   /* doubles in the shared-memory gather buffer */
+    int32_t fac_grid, fac_block, fac_smem_bytes;
+    int64_t max_n_bar;               /* largest |D-bar_l^p| over all subdomains and levels */
 } amgdd_stats_t;
 
 /* ---------------------------------------------------------------------------------------------
@@ -148,6 +156,17 @@ int amgdd_composite_size(amgdd_handle_t h, int32_t p, int32_t l, int64_t* n_real
 /* real_gid: |D_l^p| global indices, ascending; ghost_gid: |D-bar_l^p \ D_l^p|, ascending (S7). */
 int amgdd_get_composite(amgdd_handle_t h, int32_t p, int32_t l, int32_t* real_gid, int32_t* ghost_gid);
 int amgdd_get_stats(amgdd_handle_t h, amgdd_stats_t* s);
+
+/* ---- the HBM layout of the matrices, exposed for tests and tools --------------------------------
+ * Packs a CSR matrix (HOST; rowptr32 has nrows+1 int32 entries starting at 0) into the chunked
+ * stream format the AlgFAC kernel reads with bulk async copies (layout: DESIGN.md "Data layout",
+ * csrc/amgdd_stream.hpp).  wide = 0: uint16 column indices (needs every column < 65536), 1: uint32.
+ * chunk_bytes: multiple of 128 in [1024, 65536].  With out = NULL only *out_bytes / *out_nchunks
+ * are computed.  Returns AMGDD_ERR_INDEX_RANGE if a row does not fit one chunk, AMGDD_ERR_BAD_ARG
+ * on a bad argument or if out_capacity is too small.  Needs no CUDA device. */
+int amgdd_pack_stream(int32_t nrows, const int32_t* rowptr32, const int32_t* colind, const double* vals,
+                      int32_t wide, int32_t chunk_bytes, void* out, int64_t out_capacity, int64_t* out_bytes,
+                      int32_t* out_nchunks);
 
 /* ---- measurement support ------------------------------------------------------------------
  * Device time (ms, CUDA events on the handle's stream) of the phases of the most recent

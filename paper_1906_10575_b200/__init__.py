@@ -20,7 +20,7 @@ EXPORTS = [
     "amgdd_setup", "amgdd_solve", "amgdd_solve_host", "amgdd_residual_norm", "amgdd_set_stream", "amgdd_destroy",
     "amgdd_strerror", "amgdd_last_error_detail", "amgdd_num_levels", "amgdd_level_size", "amgdd_get_cf",
     "amgdd_get_level_matrix", "amgdd_composite_size", "amgdd_get_composite", "amgdd_get_stats",
-    "amgdd_last_solve_profile",
+    "amgdd_last_solve_profile", "amgdd_pack_stream",
 ]
 
 
@@ -31,6 +31,8 @@ class AmgddStats(ctypes.Structure):
         ("sum_ghost", _i64), ("dropped_interp_entries", _i64), ("device_bytes", _i64),
         ("shared_level_instances", _i64), ("model_bytes_fac_iter", _f64 * 2), ("stream_bytes_fac_iter", _f64 * 2),
         ("model_bytes_global", _f64), ("setup_seconds_hierarchy", _f64), ("setup_seconds_composite", _f64),
+        ("chunk_bytes", _i32), ("ring_stages", _i32), ("x_cap", _i32), ("fac_grid", _i32), ("fac_block", _i32),
+        ("fac_smem_bytes", _i32), ("max_n_bar", _i64),
     ]
 
 
@@ -42,8 +44,8 @@ class AmgddError(RuntimeError):
 
 def _load():
     lib_path = _build.LIB
-    if not os.path.exists(lib_path):
-        # building is not a fallback: it produces the same CUDA library or raises
+    if _build.needs_build():
+        # (re)building is not a fallback: it produces the same CUDA library or raises
         _build.build()
     L = ctypes.CDLL(lib_path)
     L.amgdd_setup.argtypes = [_i64, _vp, _vp, _vp, _i32, _vp, _i32, _i32, _i32, _f64, _i32, ctypes.POINTER(_vp)]
@@ -63,6 +65,7 @@ def _load():
     L.amgdd_get_composite.argtypes = [_vp, _i32, _i32, _vp, _vp]
     L.amgdd_get_stats.argtypes = [_vp, ctypes.POINTER(AmgddStats)]
     L.amgdd_last_solve_profile.argtypes = [_vp, _vp, _vp]
+    L.amgdd_pack_stream.argtypes = [_i32, _vp, _vp, _vp, _i32, _i32, _vp, _i64, _vp, _vp]
     return L
 
 
@@ -204,6 +207,21 @@ def amgdd_get_stats(h: Handle) -> dict:
         v = getattr(s, name)
         d[name] = list(v) if hasattr(v, "__len__") else v
     return d
+
+
+def amgdd_pack_stream(rowptr, colind, vals, wide=False, chunk_bytes=16384):
+    """amgdd_pack_stream: CSR (host) -> (bytes of the packed chunk stream as a uint8 array, nchunks)."""
+    rowptr = _np(rowptr, np.int32)
+    colind = _np(colind, np.int32)
+    vals = _np(vals, np.float64)
+    nrows = len(rowptr) - 1
+    nbytes, nchunks = _i64(), _i32()
+    _check(lib.amgdd_pack_stream(nrows, rowptr.ctypes.data, colind.ctypes.data, vals.ctypes.data, int(wide), chunk_bytes,
+                                 None, 0, ctypes.byref(nbytes), ctypes.byref(nchunks)))
+    out = np.zeros(max(nbytes.value, 1), dtype=np.uint8)
+    _check(lib.amgdd_pack_stream(nrows, rowptr.ctypes.data, colind.ctypes.data, vals.ctypes.data, int(wide), chunk_bytes,
+                                 out.ctypes.data, nbytes.value, ctypes.byref(nbytes), ctypes.byref(nchunks)))
+    return out[:nbytes.value], nchunks.value
 
 
 def amgdd_last_solve_profile(h: Handle):

@@ -3,12 +3,14 @@
 #include "../../include/amgdd.h"
 #include "amgdd_host.hpp"
 #include "amgdd_kernels.cuh"
+#include "amgdd_stream.hpp"
 
 #include <cuda_runtime.h>
 
 #include <algorithm>
 #include <chrono>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <mutex>
 #include <new>
@@ -21,12 +23,15 @@ namespace {
 
 thread_local std::string g_detail;
 
-struct GlobalLevelDev {          // the single device copy of a whole level (int32 row pointers)
+struct GlobalLevelDev {          // the single device copy of a whole level
+    // plain CSR (int32 row pointers) for the global kernels: A_0 (Alg. 2) and every R_l
     int* a_rp = nullptr; int* a_ci = nullptr; double* a_v = nullptr;
-    int* p_rp = nullptr; int* p_ci = nullptr; double* p_v = nullptr;
     int* r_rp = nullptr; int* r_ci = nullptr; double* r_v = nullptr;
+    int lanes_a = 2, lanes_r = 2;
+    // packed streams for the AlgFAC kernel, present when some subdomain covers the whole level
+    char* sA = nullptr; char* sP = nullptr; char* sR = nullptr;
+    StreamLayout layA, layP, layR;
     double* dinv = nullptr; int* ident = nullptr;
-    int lanes_a = 2, lanes_p = 2, lanes_r = 2;
 };
 
 struct SubMeta {                 // host-side record of one subdomain's blob
@@ -55,7 +60,8 @@ struct amgdd_handle_s {
     std::vector<long long> r_off;
     double* d_workspace = nullptr;
     long long slot_stride = 0, scratch_off = 0, scratch_len = 0;
-    int num_slots = 0, fac_block = 512;
+    int chunk_bytes = 16384, stages = 0, x_cap = 0;
+    FacLaunch fac_cfg = {1, 1024, 0};
     int* d_counter = nullptr;
     double* d_lu = nullptr; int* d_rowperm = nullptr;
     double* d_partial = nullptr; int partial_cap = 0;
@@ -153,7 +159,7 @@ int build_composites(amgdd_handle_s* h, const std::vector<i32>& owner, int nthre
             if (cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking) != cudaSuccess) { fail(AMGDD_ERR_CUDA, "stream create failed"); return; }
             char* stage = nullptr;
             size_t stage_cap = 0;
-            CompositeBuilder cb(h->H, owner, owned, h->eta, h->nghost);
+            CompositeBuilder cb(h->H, owner, owned, h->eta, h->nghost, h->chunk_bytes);
             for (;;) {
                 const int p = next.fetch_add(1);
                 if (p >= P || status.load() != AMGDD_SUCCESS) break;
@@ -168,6 +174,12 @@ int build_composites(amgdd_handle_s* h, const std::vector<i32>& owner, int nthre
                 for (int l = 0; l <= L; ++l)
                     if (sm.plan.lev[l].nnzA > INT32_MAX || sm.plan.lev[l].nnzP > INT32_MAX) too_big = true;
                 if (too_big) { fail(AMGDD_ERR_INDEX_RANGE, "a composite level exceeds 2^31-1 local nonzeros"); break; }
+                if (sm.plan.too_long_row >= 0) {
+                    fail(AMGDD_ERR_INDEX_RANGE, "subdomain " + std::to_string(p) + ", level " + std::to_string(sm.plan.too_long_level) +
+                                                    ": a local matrix row does not fit one " + std::to_string(h->chunk_bytes) +
+                                                    "-byte stream chunk");
+                    break;
+                }
                 const size_t bytes = (size_t)std::max<i64>(sm.plan.bytes, 16);
                 {   // reserve device space
                     std::lock_guard<std::mutex> g(arena.mu);
@@ -217,12 +229,22 @@ int build_composites(amgdd_handle_s* h, const std::vector<i32>& owner, int nthre
     return AMGDD_SUCCESS;
 }
 
-// the SURVEY.md §8(d) traffic model, nu = 1
+// bytes the kernel requests for the first `nchunks` chunks of a stream
+double chunk_bytes_of(const StreamLayout& s, int nchunks, int chunk_bytes) {
+    if (nchunks <= 0) return 0.0;
+    if (nchunks >= s.nchunks) return (double)s.bytes;
+    return (double)nchunks * chunk_bytes;
+}
+
+// the SURVEY.md §8(d) traffic model (nu = 1) and the bytes this build's kernel actually streams
 void traffic_model(amgdd_handle_s* h) {
     amgdd_stats_t& s = h->stats;
     const int L = h->H.L;
     double model[2] = {0, 0}, stream[2] = {0, 0};
     for (const SubMeta& sm : h->subs) {
+        auto layA = [&](int l) -> const StreamLayout& { return sm.plan.lev[l].shared ? h->glev[l].layA : sm.plan.lev[l].A; };
+        auto layP = [&](int l) -> const StreamLayout& { return sm.plan.lev[l].shared ? h->glev[l].layP : sm.plan.lev[l].P; };
+        auto layR = [&](int l) -> const StreamLayout& { return sm.plan.lev[l].shared ? h->glev[l].layR : sm.plan.lev[l].R; };
         for (int l = 0; l < L; ++l) {
             const BlockLayout& b = sm.plan.lev[l];
             const BlockLayout& c = sm.plan.lev[l + 1];
@@ -239,9 +261,14 @@ void traffic_model(amgdd_handle_s* h) {
             const double post = Ar + 8 * nb + 40 * nr;
             model[0] += pre + at + rs + ip + post;
             model[1] += pre + at + rs + rc + ip + post;
-            const double spre = (l == 0) ? Ar + 8 * nr : 8 * nr;
-            stream[0] += spre + (Ar + Ag) + Pt + Pm + (Ar + 8 * nr);
-            stream[1] += spre + (Ar + Ag) + Pt + Arc + Pm + (Ar + 8 * nr);
+            const StreamLayout& A = layA(l);
+            const double a_real = chunk_bytes_of(A, A.nchunks_real, h->chunk_bytes);
+            const double a_all = (double)A.bytes;
+            const StreamLayout& Ac = layA(l + 1);
+            const double ac_real = chunk_bytes_of(Ac, Ac.nchunks_real, h->chunk_bytes);
+            const double common = (l == 0 ? a_real : 0.0) + a_all + (double)layR(l).bytes + (double)layP(l).bytes + a_real;
+            stream[0] += common;
+            stream[1] += common + ac_real;
         }
     }
     s.model_bytes_fac_iter[0] = model[0]; s.model_bytes_fac_iter[1] = model[1];
@@ -250,6 +277,35 @@ void traffic_model(amgdd_handle_s* h) {
     for (int l = 0; l < L; ++l) g += 12.0 * h->H.lv[l].P.nnz() + 4.0 * h->H.lv[l + 1].A.nrows + 8.0 * (h->H.lv[l].A.nrows + h->H.lv[l + 1].A.nrows);
     g += 12.0 * (double)s.sum_real + 24.0 * h->n;                                // a3 gather, a10 update
     s.model_bytes_global = g;
+}
+
+int env_int(const char* name, int dflt) {
+    const char* v = std::getenv(name);
+    if (!v || !*v) return dflt;
+    return std::atoi(v);
+}
+
+StreamDesc make_desc(const char* base, const StreamLayout& lay) {
+    StreamDesc d;
+    d.base = base;
+    d.nchunks = lay.nchunks; d.nchunks_real = lay.nchunks_real; d.last_bytes = lay.last_bytes;
+    d.lanes = pick_lanes(lay.nrows > 0 ? (double)lay.nnz / (double)lay.nrows : 1.0);
+    d.wide = lay.wide ? 1 : 0;
+    d.pad_ = 0;
+    return d;
+}
+
+int upload_packed(amgdd_handle_s* h, const HostCsr& M, char** dptr, StreamLayout& lay, const char* what, int l) {
+    PackedLevelStream ps;
+    i64 bad = -1;
+    if (!pack_global_stream(M, h->chunk_bytes, ps, bad)) { g_detail = "a level matrix has more than 2^31-1 nonzeros"; return AMGDD_ERR_INDEX_RANGE; }
+    if (bad >= 0) {
+        g_detail = std::string("row ") + std::to_string(bad) + " of " + what + "_" + std::to_string(l) + " does not fit one " +
+                   std::to_string(h->chunk_bytes) + "-byte stream chunk";
+        return AMGDD_ERR_INDEX_RANGE;
+    }
+    lay = ps.lay;
+    return upload(h, dptr, ps.data.data(), ps.data.size());
 }
 
 int finish_tables(amgdd_handle_s* h) {
@@ -266,20 +322,24 @@ int finish_tables(amgdd_handle_s* h) {
         const HostLevel& lv = h->H.lv[l];
         GlobalLevelDev& g = h->glev[l];
         g.lanes_a = pick_lanes(avg_row(lv.A));
-        if (l < L) { g.lanes_p = pick_lanes(avg_row(lv.P)); g.lanes_r = pick_lanes(avg_row(lv.R)); }
-        if (l == 0 || need[l])
-            if ((rc = upload_csr32(h, lv.A, &g.a_rp, &g.a_ci, &g.a_v))) return rc;
+        if (l < L) g.lanes_r = pick_lanes(avg_row(lv.R));
+        if (l == 0)
+            if ((rc = upload_csr32(h, lv.A, &g.a_rp, &g.a_ci, &g.a_v))) return rc;   // Alg. 2
         if (l < L)
             if ((rc = upload_csr32(h, lv.R, &g.r_rp, &g.r_ci, &g.r_v))) return rc;   // Alg. 2 P:473 needs every R_l
         if (need[l]) {
-            if (l < L && (rc = upload_csr32(h, lv.P, &g.p_rp, &g.p_ci, &g.p_v))) return rc;
+            if ((rc = upload_packed(h, lv.A, &g.sA, g.layA, "A", l))) return rc;
+            if (l < L) {
+                if ((rc = upload_packed(h, lv.P, &g.sP, g.layP, "P", l))) return rc;
+                if ((rc = upload_packed(h, lv.R, &g.sR, g.layR, "R", l))) return rc;
+            }
             if ((rc = upload(h, &g.dinv, lv.dinv.data(), lv.dinv.size()))) return rc;
             std::vector<int> id((size_t)lv.A.nrows);
             std::iota(id.begin(), id.end(), 0);
             if ((rc = upload(h, &g.ident, id.data(), id.size()))) return rc;
         }
     }
-    // workspace geometry: per level u | t | s | f (n_bar each), then two scratch vectors
+    // workspace geometry: per level u | t | s | f (n_bar each), then one scratch vector
     long long max_sum = 0, max_nb = 0;
     std::vector<DevLevel> lev((size_t)P * (L + 1));
     std::vector<DevSub> sub(P);
@@ -298,21 +358,14 @@ int finish_tables(amgdd_handle_s* h) {
             if (b.shared) {
                 const GlobalLevelDev& g = h->glev[l];
                 d.gid = g.ident; d.dinv = g.dinv;
-                d.a_rp = g.a_rp; d.a_ci = g.a_ci; d.a_v = g.a_v;
-                d.p_rp = g.p_rp; d.p_ci = g.p_ci; d.p_v = g.p_v;
-                d.r_rp = g.r_rp; d.r_ci = g.r_ci; d.r_v = g.r_v;
-                d.lanes_a = g.lanes_a; d.lanes_p = g.lanes_p; d.lanes_r = g.lanes_r;
+                d.A = make_desc(g.sA, g.layA);
+                if (l < L) { d.P = make_desc(g.sP, g.layP); d.R = make_desc(g.sR, g.layR); }
             } else {
                 char* base = sm.dev_base;
                 d.gid = (const int*)(base + b.off_gid); d.dinv = (const double*)(base + b.off_dinv);
-                d.a_rp = (const int*)(base + b.off_a_rp); d.a_ci = (const int*)(base + b.off_a_ci); d.a_v = (const double*)(base + b.off_a_v);
-                d.p_rp = (const int*)(base + b.off_p_rp); d.p_ci = (const int*)(base + b.off_p_ci); d.p_v = (const double*)(base + b.off_p_v);
-                d.r_rp = (const int*)(base + b.off_r_rp); d.r_ci = (const int*)(base + b.off_r_ci); d.r_v = (const double*)(base + b.off_r_v);
-                const double nb = std::max(1, d.n_bar);
-                const double nbc = std::max(1, sm.plan.lev[l + 1].n_real + sm.plan.lev[l + 1].n_ghost);
-                d.lanes_a = pick_lanes((double)b.nnzA / nb);
-                d.lanes_p = pick_lanes((double)b.nnzP / nb);
-                d.lanes_r = pick_lanes((double)b.nnzP / nbc);
+                d.A = make_desc(base + b.A.off, b.A);
+                d.P = make_desc(base + b.P.off, b.P);
+                d.R = make_desc(base + b.R.off, b.R);
             }
         }
         // vectors of a level: u | t | s | f, n_bar doubles each, consecutive; levels 16-byte aligned
@@ -330,14 +383,37 @@ int finish_tables(amgdd_handle_s* h) {
     st.shared_level_instances = shared_inst;
     h->scratch_len = (max_nb + 1) & ~1LL;
     h->scratch_off = max_sum;
-    h->slot_stride = (max_sum + 2 * h->scratch_len + 15) & ~15LL;
+    h->slot_stride = (max_sum + h->scratch_len + 15) & ~15LL;
 
+    // launch plan of the persistent AlgFAC kernel: one CTA per SM slot, the shared memory split
+    // between the gather buffer (x_cap doubles) and the chunk ring (stages x chunk_bytes)
     cudaDeviceProp prop;
     CUDA_TRY(cudaGetDeviceProperties(&prop, h->device));
-    h->fac_block = 512;
-    const int per_sm = 2;                                       // resident CTAs per SM (512 threads each)
-    h->num_slots = std::max(1, std::min(P, prop.multiProcessorCount * per_sm));
-    if ((rc = dev_alloc(h, (void**)&h->d_workspace, (size_t)h->num_slots * h->slot_stride * sizeof(double)))) return rc;
+    const int per_sm = std::max(1, std::min(4, env_int("AMGDD_CTAS_PER_SM", 1)));
+    int threads = env_int("AMGDD_THREADS", per_sm == 1 ? 1024 : 512);
+    threads = std::max(64, std::min(1024, (threads / 32) * 32));
+    const int smem_optin = (int)prop.sharedMemPerBlockOptin;
+    int smem_cta = smem_optin;
+    if (per_sm > 1) smem_cta = std::min(smem_optin, (int)(prop.sharedMemPerMultiprocessor / per_sm) - 1024);
+    const int min_stages = 3;
+    const int ctrl = fac_smem_bytes(0, 0, 0);
+    long long x_cap = (max_nb + 15) & ~15LL;
+    const long long x_cap_max = ((long long)(smem_cta - ctrl - min_stages * h->chunk_bytes) / 8) & ~15LL;
+    if (x_cap_max < 64) { g_detail = "chunk size too large for the shared memory of this device"; return AMGDD_ERR_BAD_ARG; }
+    x_cap = std::min(x_cap, x_cap_max);
+    const int x_env = env_int("AMGDD_XCAP", -1);
+    if (x_env >= 0) x_cap = std::min<long long>(x_cap_max, (x_env + 15) & ~15);
+    x_cap = std::max<long long>(x_cap, 16);
+    h->x_cap = (int)x_cap;
+    h->stages = std::min(fac_max_stages(), (int)((smem_cta - ctrl - x_cap * 8) / h->chunk_bytes));
+    const int st_env = env_int("AMGDD_STAGES", -1);
+    if (st_env >= 2) h->stages = std::min(h->stages, st_env);
+    h->fac_cfg.block = threads;
+    h->fac_cfg.smem_bytes = fac_smem_bytes(h->chunk_bytes, h->stages, h->x_cap);
+    h->fac_cfg.grid = std::max(1, std::min(P, prop.multiProcessorCount * per_sm));
+    if (fac_configure(h->device, smem_optin) != 0) { g_detail = "cudaFuncSetAttribute(max dynamic shared memory) failed"; cudaGetLastError(); return AMGDD_ERR_CUDA; }
+
+    if ((rc = dev_alloc(h, (void**)&h->d_workspace, (size_t)h->fac_cfg.grid * h->slot_stride * sizeof(double)))) return rc;
     if ((rc = upload(h, &h->d_lev, lev.data(), lev.size()))) return rc;
     if ((rc = upload(h, &h->d_sub, sub.data(), sub.size()))) return rc;
     // largest subdomains first (longest-processing-time order for the dynamic scheduler)
@@ -368,6 +444,9 @@ int finish_tables(amgdd_handle_s* h) {
     st.dropped_interp_entries = 0;
     traffic_model(h);
     st.device_bytes = h->device_bytes;
+    st.chunk_bytes = h->chunk_bytes; st.ring_stages = h->stages; st.x_cap = h->x_cap;
+    st.fac_grid = h->fac_cfg.grid; st.fac_block = h->fac_cfg.block; st.fac_smem_bytes = h->fac_cfg.smem_bytes;
+    st.max_n_bar = max_nb;
     return AMGDD_SUCCESS;
 }
 
@@ -431,6 +510,12 @@ int amgdd_setup(int64_t n, const int64_t* rowptr, const int32_t* colind, const d
     std::memset(&h->stats, 0, sizeof(h->stats));
     if (cudaGetDevice(&h->device) != cudaSuccess) { delete h; g_detail = "cudaGetDevice failed"; return AMGDD_ERR_CUDA; }
     h->n = n; h->P = num_subdomains; h->eta = eta; h->nghost = num_ghost;
+    h->chunk_bytes = env_int("AMGDD_CHUNK_BYTES", 16384);
+    if (h->chunk_bytes < MIN_CHUNK_BYTES || h->chunk_bytes > MAX_CHUNK_BYTES || (h->chunk_bytes & 127)) {
+        delete h;
+        g_detail = "AMGDD_CHUNK_BYTES must be a multiple of 128 in [1024, 65536]";
+        return AMGDD_ERR_BAD_ARG;
+    }
     const int nthreads = default_threads();
     try {
         auto t0 = std::chrono::steady_clock::now();
@@ -509,8 +594,9 @@ int amgdd_solve(amgdd_handle_t h, const double* b, double* x, int32_t num_cycles
     prm.num_sub = h->P; prm.L = L;
     prm.r_all = h->d_r_all; prm.r_off = h->d_r_off;
     prm.x = x; prm.workspace = h->d_workspace;
-    prm.slot_stride = h->slot_stride; prm.scratch_off = h->scratch_off; prm.scratch_len = h->scratch_len;
+    prm.slot_stride = h->slot_stride; prm.scratch_off = h->scratch_off;
     prm.work_counter = h->d_counter;
+    prm.chunk_bytes = h->chunk_bytes; prm.stages = h->stages; prm.x_cap = h->x_cap;
     prm.nfac = num_fac_cycles; prm.nu = relax_sweeps;
     prm.lu = h->d_lu; prm.rowperm = h->d_rowperm; prm.nL = (int)h->H.nL;
     long long launches[3] = {0, 0, 0};
@@ -527,7 +613,7 @@ int amgdd_solve(amgdd_handle_t h, const double* b, double* x, int32_t num_cycles
         }
         mark();
         CUDA_TRY(cudaMemsetAsync(h->d_counter, 0, sizeof(int), h->stream));
-        launch_fac(prm, h->num_slots, h->fac_block, h->stream);                     // Alg. 2
+        launch_fac(prm, h->fac_cfg, h->stream);                                     // Alg. 2
         launches[2] += 1;
         mark();
     }
@@ -582,6 +668,29 @@ int amgdd_residual_norm(amgdd_handle_t h, const double* b, const double* x, doub
     CUDA_TRY(cudaGetLastError());
     CUDA_TRY(cudaMemcpyAsync(out_host, h->d_norms, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
     CUDA_TRY(cudaStreamSynchronize(h->stream));
+    return AMGDD_SUCCESS;
+}
+
+int amgdd_pack_stream(int32_t nrows, const int32_t* rowptr32, const int32_t* colind, const double* vals, int32_t wide,
+                      int32_t chunk_bytes, void* out, int64_t out_capacity, int64_t* out_bytes, int32_t* out_nchunks) {
+    g_detail.clear();
+    if (nrows < 0 || !rowptr32 || (!colind && rowptr32[nrows] > 0) || (!vals && rowptr32[nrows] > 0) || rowptr32[0] != 0 ||
+        chunk_bytes < MIN_CHUNK_BYTES || chunk_bytes > MAX_CHUNK_BYTES || (chunk_bytes & 127)) {
+        g_detail = "bad argument to amgdd_pack_stream";
+        return AMGDD_ERR_BAD_ARG;
+    }
+    if (!wide)
+        for (int32_t k = 0; k < rowptr32[nrows]; ++k)
+            if (colind[k] < 0 || colind[k] >= NARROW_MAX_COLS) { g_detail = "column index needs the wide form"; return AMGDD_ERR_BAD_ARG; }
+    const PackPlan pp = plan_stream(nrows, rowptr32, wide != 0, chunk_bytes, nrows);
+    if (pp.too_long_row >= 0) { g_detail = "row " + std::to_string(pp.too_long_row) + " does not fit one chunk"; return AMGDD_ERR_INDEX_RANGE; }
+    if (out_bytes) *out_bytes = pp.bytes;
+    if (out_nchunks) *out_nchunks = pp.nchunks;
+    if (out) {
+        if (out_capacity < pp.bytes) { g_detail = "output buffer too small"; return AMGDD_ERR_BAD_ARG; }
+        std::memset(out, 0, (size_t)pp.bytes);
+        write_stream(nrows, rowptr32, colind, vals, wide != 0, chunk_bytes, (char*)out);
+    }
     return AMGDD_SUCCESS;
 }
 

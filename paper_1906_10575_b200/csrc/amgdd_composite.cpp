@@ -1,21 +1,24 @@
 // Composite grids of one subdomain (paper P:57, eq. 1; readings S6, S7, A5-A8, A12) and
-// their local CSR blocks, built on the host by worker threads and shipped to the device as one
-// contiguous "blob" per subdomain.  Independent of oracle/ (epoch-stamped maps, local matrices).
+// their local matrices, built on the host by worker threads and shipped to the device as one
+// contiguous "blob" per subdomain.  Independent of oracle/ (epoch-stamped maps, local matrices,
+// packed streams).
 //
 // Local numbering of level l (S7): real points D_l^p in ascending global index get 0..n_real-1,
 // ghost points D-bar_l^p \ D_l^p in ascending global index get n_real..n_real+n_ghost-1.
-// Blocks stored per private (subdomain, level):
+// Stored per private (subdomain, level):
 //   gid   int32[n_bar]            global index of every local point
 //   dinv  double[n_real]          l1 diagonal of the full global row (S8)
-//   A     CSR, n_bar rows: real rows hold the whole global row (all columns lie in D-bar_l by
-//         eq. 1); ghost rows hold only their real columns (t_l vanishes off D_l, A12)
-//   P     CSR, n_bar rows, columns local to level l+1 (rows over all of D-bar_l)
-//   R     CSR, n_bar(l+1) rows, columns local to level l: the explicit transpose of the local P,
-//         so restriction is a gather with a fixed summation order (no atomics)
-// A level on which D_l^p = Omega_l (always true on L, reading A5) is "shared": nothing is stored
-// for it, the single global copy of the level is used ("each processor stores the entire
-// coarsest grid ... may be true for a few of the coarsest grids").
+//   A     packed stream, n_bar rows: real rows hold the whole global row (all columns lie in
+//         D-bar_l by eq. 1); ghost rows hold only their real columns (t_l vanishes off D_l,
+//         P:230, A12)
+//   P     packed stream, n_bar rows, columns local to level l+1 (rows over all of D-bar_l)
+//   R     packed stream, n_bar(l+1) rows, columns local to level l: the explicit transpose of the
+//         local P, so restriction is a gather with a fixed summation order (no atomics)
+// (stream format: amgdd_stream.hpp).  A level on which D_l^p = Omega_l (always true on L, reading
+// A5) is "shared": nothing is stored for it, the single global copy of the level is used (P:57
+// "each processor stores the entire coarsest grid ... may be true for a few of the coarsest grids").
 #include "amgdd_host.hpp"
+#include "amgdd_stream.hpp"
 
 #include <algorithm>
 #include <cstring>
@@ -24,13 +27,24 @@ namespace amgdd {
 
 namespace {
 inline i64 align16(i64 x) { return (x + 15) & ~(i64)15; }
+
+void layout_stream(const LocalCsr& M, int nrows, int ncols, int chunk_bytes, int n_real, StreamLayout& s,
+                   i64& too_long_row) {
+    s.nrows = nrows;
+    s.nnz = M.rp[nrows];
+    s.wide = ncols > NARROW_MAX_COLS;
+    const PackPlan pp = plan_stream(nrows, M.rp.data(), s.wide, chunk_bytes, n_real);
+    s.bytes = pp.bytes; s.nchunks = pp.nchunks; s.nchunks_real = pp.nchunks_real; s.last_bytes = pp.last_bytes;
+    if (pp.too_long_row >= 0 && too_long_row < 0) too_long_row = pp.too_long_row;
 }
+}  // namespace
 
 CompositeBuilder::CompositeBuilder(const Hierarchy& H, const std::vector<i32>& owner,
-                                   const std::vector<std::vector<i32>>& owned, int eta, int num_ghost)
-    : H_(H), owner_(owner), owned_(owned), eta_(eta), nghost_(num_ghost) {
+                                   const std::vector<std::vector<i32>>& owned, int eta, int num_ghost, int chunk_bytes)
+    : H_(H), owner_(owner), owned_(owned), eta_(eta), nghost_(num_ghost), chunk_bytes_(chunk_bytes) {
     const int nl = H.L + 1;
     real_.resize(nl); ghost_.resize(nl); loc_.resize(nl); stamp_.resize(nl);
+    A_.resize(nl); P_.resize(nl); R_.resize(nl);
     epoch_.assign(nl, 0);
     for (int l = 0; l < nl; ++l) {
         loc_[l].assign((size_t)H.lv[l].A.nrows, -1);
@@ -60,6 +74,7 @@ void CompositeBuilder::plan(int p, SubdomainBlob& out) {
     p_ = p;
     out.lev.assign(L + 1, BlockLayout());
     out.dropped = 0;
+    out.too_long_row = -1; out.too_long_level = -1;
     std::vector<i32> seed = owned_[p];                                   // B_0^p = Omega_0^p
     for (int l = 0; l <= L; ++l) {
         const i64 nl = H_.lv[l].A.nrows;
@@ -89,31 +104,68 @@ void CompositeBuilder::plan(int p, SubdomainBlob& out) {
         b.n_ghost = (i32)gh.size();
         b.shared = ((i64)re.size() == nl);
     }
-    // sizes
+    // local matrices (only sizes are needed for shared levels)
     for (int l = 0; l <= L; ++l) {
         BlockLayout& b = out.lev[l];
         const HostLevel& lv = H_.lv[l];
-        const i32 nr = b.n_real;
+        const i32 nr = b.n_real, nb = b.n_real + b.n_ghost;
         for (i32 g : real_[l]) b.nnzA_real += lv.A.rp[g + 1] - lv.A.rp[g];
-        for (i32 g : ghost_[l])
+        if (b.shared) {                                                  // no ghosts, whole level
+            b.nnzA = b.nnzA_real;
+            b.nnzP = (l < L) ? lv.P.nnz() : 0;
+            continue;
+        }
+        auto gid_of = [&](i32 i) { return i < nr ? real_[l][i] : ghost_[l][i - nr]; };
+        {   // 32-bit local offsets: refuse (AMGDD_ERR_INDEX_RANGE in the caller) before anything overflows
+            i64 bound = b.nnzA_real, boundP = 0;
+            for (i32 g : ghost_[l]) bound += lv.A.rp[g + 1] - lv.A.rp[g];
+            for (i32 i = 0; i < nb; ++i) boundP += lv.P.rp[gid_of(i) + 1] - lv.P.rp[gid_of(i)];
+            if (bound > (i64)INT32_MAX || boundP > (i64)INT32_MAX) { b.nnzA = bound; b.nnzP = boundP; out.bytes = 0; return; }
+        }
+        LocalCsr& A = A_[l];
+        A.rp.assign((size_t)nb + 1, 0); A.ci.clear(); A.v.clear();
+        for (i32 i = 0; i < nb; ++i) {
+            const i32 g = gid_of(i);
             for (i64 k = lv.A.rp[g]; k < lv.A.rp[g + 1]; ++k) {
                 const i32 c = local_of(l, lv.A.ci[k]);
-                b.nnzA_ghost += (c >= 0 && c < nr);
+                if (i < nr) { A.ci.push_back(c); A.v.push_back(lv.A.v[k]); }       // real rows: always inside (eq. 1)
+                else if (c >= 0 && c < nr) { A.ci.push_back(c); A.v.push_back(lv.A.v[k]); }
             }
-        b.nnzA = b.nnzA_real + b.nnzA_ghost;
-        if (l < L) {
-            auto count_rows = [&](const std::vector<i32>& rows) {
-                for (i32 g : rows)
-                    for (i64 k = lv.P.rp[g]; k < lv.P.rp[g + 1]; ++k) {
-                        if (local_of(l + 1, lv.P.ci[k]) >= 0) ++b.nnzP;
-                        else ++out.dropped;                              // A7
-                    }
-            };
-            count_rows(real_[l]);
-            count_rows(ghost_[l]);
+            A.rp[i + 1] = (i32)A.ci.size();
         }
+        b.nnzA = A.rp[nb];
+        b.nnzA_ghost = b.nnzA - b.nnzA_real;
+        // P (columns local to level l+1) and R = local P transposed; l < L here
+        const i32 nbc = out.lev[l + 1].n_real + out.lev[l + 1].n_ghost;
+        LocalCsr& P = P_[l];
+        LocalCsr& R = R_[l];
+        P.rp.assign((size_t)nb + 1, 0); P.ci.clear(); P.v.clear();
+        R.rp.assign((size_t)nbc + 1, 0);
+        for (i32 i = 0; i < nb; ++i) {
+            const i32 g = gid_of(i);
+            for (i64 k = lv.P.rp[g]; k < lv.P.rp[g + 1]; ++k) {
+                const i32 c = local_of(l + 1, lv.P.ci[k]);
+                if (c >= 0) { P.ci.push_back(c); P.v.push_back(lv.P.v[k]); R.rp[c + 1]++; }
+                else ++out.dropped;                                      // A7
+            }
+            P.rp[i + 1] = (i32)P.ci.size();
+        }
+        b.nnzP = P.rp[nb];
+        for (i32 c = 0; c < nbc; ++c) R.rp[c + 1] += R.rp[c];            // counting sort: columns ascending
+        R.ci.resize((size_t)b.nnzP); R.v.resize((size_t)b.nnzP);
+        cursor_.assign(R.rp.begin(), R.rp.end() - 1);
+        for (i32 i = 0; i < nb; ++i)
+            for (i32 k = P.rp[i]; k < P.rp[i + 1]; ++k) {
+                const i32 pos = cursor_[P.ci[k]]++;
+                R.ci[pos] = i; R.v[pos] = P.v[k];
+            }
+        i64 bad = -1;
+        layout_stream(A, nb, nb, chunk_bytes_, nr, b.A, bad);
+        layout_stream(P, nb, nbc, chunk_bytes_, nb, b.P, bad);
+        layout_stream(R, nbc, nb, chunk_bytes_, nbc, b.R, bad);
+        if (bad >= 0 && out.too_long_row < 0) { out.too_long_row = bad; out.too_long_level = l; }
     }
-    // layout
+    // blob layout
     i64 off = 0;
     auto take = [&](i64 bytes) { const i64 o = off; off = align16(off + bytes); return o; };
     out.n_owned = (i32)owned_[p].size();
@@ -122,18 +174,11 @@ void CompositeBuilder::plan(int p, SubdomainBlob& out) {
         BlockLayout& b = out.lev[l];
         if (b.shared) continue;
         const i64 nb = (i64)b.n_real + b.n_ghost;
-        const i64 nbc = (i64)out.lev[l + 1].n_real + out.lev[l + 1].n_ghost;    // l < L here
         b.off_gid = take(nb * 4);
         b.off_dinv = take((i64)b.n_real * 8);
-        b.off_a_rp = take((nb + 1) * 4);
-        b.off_a_ci = take(b.nnzA * 4);
-        b.off_a_v = take(b.nnzA * 8);
-        b.off_p_rp = take((nb + 1) * 4);
-        b.off_p_ci = take(b.nnzP * 4);
-        b.off_p_v = take(b.nnzP * 8);
-        b.off_r_rp = take((nbc + 1) * 4);
-        b.off_r_ci = take(b.nnzP * 4);
-        b.off_r_v = take(b.nnzP * 8);
+        b.A.off = take(b.A.bytes);
+        b.P.off = take(b.P.bytes);
+        b.R.off = take(b.R.bytes);
     }
     out.bytes = off;
 }
@@ -145,7 +190,6 @@ void CompositeBuilder::fill(const SubdomainBlob& plan, char* dst) {
         const std::vector<i32>& o = owned_[p_];
         for (size_t k = 0; k < o.size(); ++k) own[k] = loc_[0][o[k]];
     }
-    std::vector<i32> cursor;
     for (int l = 0; l <= L; ++l) {
         const BlockLayout& b = plan.lev[l];
         if (b.shared) continue;
@@ -156,52 +200,24 @@ void CompositeBuilder::fill(const SubdomainBlob& plan, char* dst) {
         std::memcpy(gid + nr, ghost_[l].data(), (size_t)ng * 4);
         double* dinv = (double*)(dst + b.off_dinv);
         for (i32 i = 0; i < nr; ++i) dinv[i] = lv.dinv[gid[i]];
-        // A
-        i32* arp = (i32*)(dst + b.off_a_rp);
-        i32* aci = (i32*)(dst + b.off_a_ci);
-        double* av = (double*)(dst + b.off_a_v);
-        i32 q = 0;
-        for (i32 i = 0; i < nb; ++i) {
-            arp[i] = q;
-            const i32 g = gid[i];
-            for (i64 k = lv.A.rp[g]; k < lv.A.rp[g + 1]; ++k) {
-                const i32 c = loc_[l][lv.A.ci[k]];                       // real rows: always stamped (eq. 1)
-                if (i < nr) { aci[q] = c; av[q] = lv.A.v[k]; ++q; }
-                else {
-                    const i32 cc = local_of(l, lv.A.ci[k]);
-                    if (cc >= 0 && cc < nr) { aci[q] = cc; av[q] = lv.A.v[k]; ++q; }
-                }
-            }
-        }
-        arp[nb] = q;
-        // P (columns local to level l+1)
         const i32 nbc = plan.lev[l + 1].n_real + plan.lev[l + 1].n_ghost;
-        i32* prp = (i32*)(dst + b.off_p_rp);
-        i32* pci = (i32*)(dst + b.off_p_ci);
-        double* pv = (double*)(dst + b.off_p_v);
-        i32* rrp = (i32*)(dst + b.off_r_rp);
-        i32* rci = (i32*)(dst + b.off_r_ci);
-        double* rv = (double*)(dst + b.off_r_v);
-        std::memset(rrp, 0, (size_t)(nbc + 1) * 4);
-        q = 0;
-        for (i32 i = 0; i < nb; ++i) {
-            prp[i] = q;
-            const i32 g = gid[i];
-            for (i64 k = lv.P.rp[g]; k < lv.P.rp[g + 1]; ++k) {
-                const i32 c = local_of(l + 1, lv.P.ci[k]);
-                if (c >= 0) { pci[q] = c; pv[q] = lv.P.v[k]; ++q; rrp[c + 1]++; }
-            }
-        }
-        prp[nb] = q;
-        // R = local P transposed (counting sort: columns come out ascending)
-        for (i32 c = 0; c < nbc; ++c) rrp[c + 1] += rrp[c];
-        cursor.assign(rrp, rrp + nbc);
-        for (i32 i = 0; i < nb; ++i)
-            for (i32 k = prp[i]; k < prp[i + 1]; ++k) {
-                const i32 pos = cursor[pci[k]]++;
-                rci[pos] = i; rv[pos] = pv[k];
-            }
+        write_stream(nb, A_[l].rp.data(), A_[l].ci.data(), A_[l].v.data(), b.A.wide, chunk_bytes_, dst + b.A.off);
+        write_stream(nb, P_[l].rp.data(), P_[l].ci.data(), P_[l].v.data(), b.P.wide, chunk_bytes_, dst + b.P.off);
+        write_stream(nbc, R_[l].rp.data(), R_[l].ci.data(), R_[l].v.data(), b.R.wide, chunk_bytes_, dst + b.R.off);
     }
+}
+
+bool pack_global_stream(const HostCsr& M, int chunk_bytes, PackedLevelStream& out, i64& too_long_row) {
+    if (M.nnz() > (i64)INT32_MAX || M.nrows > (i64)INT32_MAX) return false;
+    LocalCsr T;
+    T.rp.assign(M.rp.begin(), M.rp.end());
+    i64 bad = -1;
+    layout_stream(T, (int)M.nrows, (int)M.ncols, chunk_bytes, (int)M.nrows, out.lay, bad);
+    too_long_row = bad;
+    if (bad >= 0) return true;
+    out.data.assign((size_t)out.lay.bytes, 0);
+    write_stream((int)M.nrows, T.rp.data(), M.ci.data(), M.v.data(), out.lay.wide, chunk_bytes, out.data.data());
+    return true;
 }
 
 }  // namespace amgdd

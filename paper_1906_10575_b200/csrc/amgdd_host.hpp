@@ -73,6 +73,16 @@ void parallel_for(i64 n, int nthreads, i64 chunk, F&& fn) {
 }
 
 // ---- composite grids (S6, S7) --------------------------------------------------------------
+// Where one packed CSR stream (amgdd_stream.hpp) sits inside a blob, and its chunking.
+struct StreamLayout {
+    i64 off = -1;                // byte offset inside the blob (16-byte aligned)
+    i64 bytes = 0;
+    i32 nchunks = 0, nchunks_real = 0, last_bytes = 0;
+    i32 nrows = 0;
+    i64 nnz = 0;
+    bool wide = false;           // uint32 column indices
+};
+
 // Sizes of one (subdomain, level) block and where its arrays sit inside the subdomain's blob.
 struct BlockLayout {
     i32 n_real = 0, n_ghost = 0;
@@ -80,11 +90,8 @@ struct BlockLayout {
     i64 nnzA = 0, nnzP = 0;      // local nonzeros (ghost rows of A: real columns only)
     i64 nnzA_real = 0;           // over real rows only (overhead statistic)
     i64 nnzA_ghost = 0;          // ghost rows x real columns
-    // byte offsets inside the blob (all 16-byte aligned); -1 where absent
-    i64 off_gid = -1, off_dinv = -1;
-    i64 off_a_rp = -1, off_a_ci = -1, off_a_v = -1;
-    i64 off_p_rp = -1, off_p_ci = -1, off_p_v = -1;
-    i64 off_r_rp = -1, off_r_ci = -1, off_r_v = -1;
+    i64 off_gid = -1, off_dinv = -1;     // byte offsets inside the blob; -1 where absent
+    StreamLayout A, P, R;
 };
 
 struct SubdomainBlob {
@@ -93,14 +100,22 @@ struct SubdomainBlob {
     i32 n_owned = 0;
     i64 bytes = 0;                    // blob size
     i64 dropped = 0;                  // A7 count
+    i64 too_long_row = -1;            // a local row that does not fit one stream chunk (-1: none)
+    i32 too_long_level = -1;
+};
+
+// local CSR with 32-bit offsets (what the packer takes)
+struct LocalCsr {
+    std::vector<i32> rp, ci;
+    std::vector<double> v;
 };
 
 // Per-thread scratch for building composite grids; one instance per worker thread.
 class CompositeBuilder {
 public:
     CompositeBuilder(const Hierarchy& H, const std::vector<i32>& owner, const std::vector<std::vector<i32>>& owned,
-                     int eta, int num_ghost);
-    // Phase 1: index sets and sizes of subdomain p.  Returns the layout (bytes needed).
+                     int eta, int num_ghost, int chunk_bytes);
+    // Phase 1: index sets, local matrices and the blob layout of subdomain p.
     void plan(int p, SubdomainBlob& out);
     // Phase 2: write the arrays of the subdomain planned last into dst (out.bytes bytes).
     void fill(const SubdomainBlob& plan, char* dst);
@@ -113,13 +128,21 @@ private:
     const Hierarchy& H_;
     const std::vector<i32>& owner_;
     const std::vector<std::vector<i32>>& owned_;
-    int eta_, nghost_, p_ = -1;
+    int eta_, nghost_, chunk_bytes_, p_ = -1;
     std::vector<std::vector<i32>> real_, ghost_;
+    std::vector<LocalCsr> A_, P_, R_;                 // local matrices of the subdomain planned last
     // epoch-stamped global->local maps, one per level
     std::vector<std::vector<i32>> loc_, stamp_;
     std::vector<i32> epoch_;
-    std::vector<i32> frontier_, next_;
+    std::vector<i32> frontier_, next_, cursor_;
     i32 local_of(int l, i32 g) const { return stamp_[l][g] == epoch_[l] ? loc_[l][g] : -1; }
 };
+
+// packs a whole level matrix (the shared global copy) into a host buffer
+struct PackedLevelStream {
+    std::vector<char> data;
+    StreamLayout lay;
+};
+bool pack_global_stream(const HostCsr& M, int chunk_bytes, PackedLevelStream& out, i64& too_long_row);
 
 }  // namespace amgdd

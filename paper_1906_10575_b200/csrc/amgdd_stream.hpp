@@ -96,16 +96,18 @@ struct FacLaunch {
 struct PackPlan {
     int64_t bytes;             // total stream bytes (16-aligned)
     int nchunks;
+    int nchunks_real;          // chunks that contain a row < n_real
     int last_bytes;
     int64_t too_long_row;      // -1, or a row that does not fit one chunk
 };
 // rp: nrows+1 int32 offsets (rp[0] = 0)
-PackPlan plan_stream(int nrows, const int32_t* rp, bool wide, int chunk_bytes);
-// writes plan.bytes bytes; returns the number of chunks that contain a row < n_real
-int write_stream(int nrows, const int32_t* rp, const int32_t* ci, const double* v, bool wide, int chunk_bytes,
-                 int n_real, char* dst);
+PackPlan plan_stream(int nrows, const int32_t* rp, bool wide, int chunk_bytes, int n_real);
+// writes plan.bytes bytes (the gap between a chunk's padded end and the next chunk is left untouched)
+void write_stream(int nrows, const int32_t* rp, const int32_t* ci, const double* v, bool wide, int chunk_bytes,
+                  char* dst);
 
 int fac_smem_bytes(int chunk_bytes, int stages, int x_cap);
+int fac_max_stages();
 void launch_fac(const FacParams& prm, const FacLaunch& cfg, void* stream);
 int fac_configure(int device, int max_smem_optin);   // sets the kernel's dynamic-smem attribute; 0 on success
 
