@@ -95,9 +95,9 @@ class Handle:
         self.destroy()
 
     def destroy(self):
-        if getattr(self, "_h", None):
+        if getattr(self, "_h", None) and lib is not None:       # lib is None during interpreter shutdown
             lib.amgdd_destroy(self._h)
-            self._h = None
+        self._h = None
 
 
 def amgdd_setup(n, rowptr, colind, vals, num_subdomains, owner, eta, num_ghost=1, max_levels=25, theta=0.25,

@@ -289,7 +289,13 @@ StreamDesc make_desc(const char* base, const StreamLayout& lay) {
     StreamDesc d;
     d.base = base;
     d.nchunks = lay.nchunks; d.nchunks_real = lay.nchunks_real; d.last_bytes = lay.last_bytes;
-    d.lanes = pick_lanes(lay.nrows > 0 ? (double)lay.nnz / (double)lay.nrows : 1.0);
+    {   // threads per row: the largest power of two with at least `per_lane` nonzeros per thread
+        const double avg = lay.nrows > 0 ? (double)lay.nnz / (double)lay.nrows : 1.0;
+        const int per_lane = std::max(1, env_int("AMGDD_NNZ_PER_LANE", 4));
+        int g = 1;
+        while (g < 32 && g * 2 * per_lane <= avg) g *= 2;
+        d.lanes = g;
+    }
     d.wide = lay.wide ? 1 : 0;
     d.pad_ = 0;
     return d;

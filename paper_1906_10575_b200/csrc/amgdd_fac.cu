@@ -145,23 +145,27 @@ struct Producer {
 };
 
 // ---- consumers ------------------------------------------------------------------------------
-// One chunk in shared memory: rows go to warps round-robin by global row batch (G = 32/lanes rows
-// per batch), `lanes` threads stride over a row, shuffle reduction, epi(row, sum) on the first lane.
+// One chunk in shared memory.  Rows are dealt to the consumer warps in batches of G = 32/lanes
+// consecutive rows, round-robin by GLOBAL batch index (so the deal stays balanced across chunk
+// boundaries); `bnext` is the warp's next batch and is carried from chunk to chunk, which keeps
+// the per-chunk bookkeeping free of integer division.  `lanes` threads stride over a row, the row
+// sum is reduced by shuffles and epi(row, sum) runs on the first lane of the row.
 template <bool WIDE, class X, class Epi>
-__device__ __forceinline__ void consume_chunk(const char* slot, X xs, int lanes, int cw, int ncw, int row_limit, Epi epi) {
+__device__ __forceinline__ void consume_chunk(const char* slot, X xs, int ll /*log2 lanes*/, int ncw, int& bnext, int row_limit,
+                                              Epi epi) {
     const int4 hdr = *reinterpret_cast<const int4*>(slot);
     const int rb = hdr.x, nr = hdr.y, nnz = hdr.z;
     const double* v = reinterpret_cast<const double*>(slot + CHUNK_HEADER_BYTES);
     const char* cbase = slot + CHUNK_HEADER_BYTES + (size_t)nnz * 8;
     const unsigned short* rowend = reinterpret_cast<const unsigned short*>(cbase + (size_t)nnz * (WIDE ? 4 : 2));
     const int lane = threadIdx.x & 31;
-    const int G = 32 / lanes;
+    const int lanes = 1 << ll, gl = 5 - ll;
     const int li = lane & (lanes - 1);
-    const int sub = lane / lanes;
-    const int b_first = rb / G, b_last = (rb + nr - 1) / G;
-    int b = b_first + (cw - b_first % ncw + ncw) % ncw;
+    const int sub = lane >> ll;
+    const int b_last = (rb + nr - 1) >> gl;
+    int b = bnext;
     for (; b <= b_last; b += ncw) {
-        const int row = b * G + sub;
+        const int row = (b << gl) + sub;
         const int lr = row - rb;
         const bool valid = (lr >= 0) && (lr < nr) && (row < row_limit);
         double sum = 0.0;
@@ -178,6 +182,9 @@ __device__ __forceinline__ void consume_chunk(const char* slot, X xs, int lanes,
         for (int o = lanes >> 1; o > 0; o >>= 1) sum += __shfl_down_sync(0xffffffffu, sum, o, lanes);
         if (valid && li == 0) epi(row, sum);
     }
+    // a batch cut by the end of the chunk continues in the next chunk
+    if (b - ncw == b_last && ((rb + nr) & ((1 << gl) - 1)) != 0) b -= ncw;
+    bnext = b;
 }
 
 struct Consumer {
@@ -286,16 +293,18 @@ struct Consumer {
     template <class Epi>
     __device__ __forceinline__ void run_chunks(const StreamDesc& d, int nchunks, bool staged, const double* xg, int row_limit, Epi epi) {
         extern __shared__ __align__(128) unsigned char smem_dyn[];      // same base as in fac_kernel: keeps LDS addressing
+        const int ll = __ffs(d.lanes) - 1;
+        int bnext = cw;                                                  // batches cw, cw + ncw, ... are this warp's
         for (int c = 0; c < nchunks; ++c) {
             mbar_wait(&ctrl->full[slot], phase);
             const char* sl = reinterpret_cast<const char*>(smem_dyn + CTRL_BYTES + (size_t)x_cap * 8 + (size_t)slot * chunk_bytes);
             if (staged) {
                 const double* xs = reinterpret_cast<const double*>(smem_dyn + CTRL_BYTES);
-                if (d.wide) consume_chunk<true>(sl, xs, d.lanes, cw, ncw, row_limit, epi);
-                else consume_chunk<false>(sl, xs, d.lanes, cw, ncw, row_limit, epi);
+                if (d.wide) consume_chunk<true>(sl, xs, ll, ncw, bnext, row_limit, epi);
+                else consume_chunk<false>(sl, xs, ll, ncw, bnext, row_limit, epi);
             } else {
-                if (d.wide) consume_chunk<true>(sl, xg, d.lanes, cw, ncw, row_limit, epi);
-                else consume_chunk<false>(sl, xg, d.lanes, cw, ncw, row_limit, epi);
+                if (d.wide) consume_chunk<true>(sl, xg, ll, ncw, bnext, row_limit, epi);
+                else consume_chunk<false>(sl, xg, ll, ncw, bnext, row_limit, epi);
             }
             release();
         }
