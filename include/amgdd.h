@@ -54,9 +54,8 @@ typedef enum amgdd_status {
                                             silently dropped */
     AMGDD_ERR_OUT_OF_MEMORY = -7,        /* host or device allocation failed; detail string has the byte count */
     AMGDD_ERR_CUDA = -8,                 /* any CUDA runtime error, including "no device" */
-    AMGDD_ERR_INDEX_RANGE = -9           /* a composite level has more than 2^31-1 local nonzeros, or a local
-                                            matrix row does not fit one stream chunk (about 1,600 nonzeros
-                                            at the default 16 KiB chunk) */
+    AMGDD_ERR_INDEX_RANGE = -9           /* a composite level has more than 2^31-1 local nonzeros, or a matrix
+                                            row has more than 65535 entries */
 } amgdd_status;
 
 /* Sizes and the traffic model of DESIGN.md §"Algorithmic bytes". */
@@ -85,6 +84,7 @@ typedef struct amgdd_stats {
     double setup_seconds_composite;  /* host: S6-S7 + local matrices + packing + upload */
     /* launch plan of the persistent AlgFAC kernel */
     int32_t chunk_bytes;             /* stride of a packed-stream chunk = size of a ring slot */
+    int32_t window;                  /* rows per sort window of the slice-JDS streams */
     int32_t ring_stages;             /* ring slots per CTA */
     int32_t x_cap;                   /* doubles in the shared-memory gather buffer */
     int32_t fac_grid, fac_block, fac_smem_bytes;
@@ -158,15 +158,21 @@ int amgdd_get_composite(amgdd_handle_t h, int32_t p, int32_t l, int32_t* real_gi
 int amgdd_get_stats(amgdd_handle_t h, amgdd_stats_t* s);
 
 /* ---- the HBM layout of the matrices, exposed for tests and tools --------------------------------
- * Packs a CSR matrix (HOST; rowptr32 has nrows+1 int32 entries starting at 0) into the chunked
- * stream format the AlgFAC kernel reads with bulk async copies (layout: DESIGN.md "Data layout",
- * csrc/amgdd_stream.hpp).  wide = 0: uint16 column indices (needs every column < 65536), 1: uint32.
- * chunk_bytes: multiple of 128 in [1024, 65536].  With out = NULL only *out_bytes / *out_nchunks
- * are computed.  Returns AMGDD_ERR_INDEX_RANGE if a row does not fit one chunk, AMGDD_ERR_BAD_ARG
- * on a bad argument or if out_capacity is too small.  Needs no CUDA device. */
-int amgdd_pack_stream(int32_t nrows, const int32_t* rowptr32, const int32_t* colind, const double* vals,
-                      int32_t wide, int32_t chunk_bytes, void* out, int64_t out_capacity, int64_t* out_bytes,
-                      int32_t* out_nchunks);
+ * Packs a CSR matrix (HOST; rowptr32 has nrows+1 int32 entries starting at 0, at most 65535
+ * entries per row) into the chunked "slice-JDS" stream the AlgFAC kernel reads with bulk async
+ * copies (layout: DESIGN.md "Data layout", csrc/amgdd_stream.hpp): rows [0, n_real) and
+ * [n_real, nrows) are two groups (real / ghost rows of a composite A_l); inside windows of
+ * `window` rows (multiple of 32 in [32, 32768]) rows are sorted by length and cut into slices of 32
+ * rows, one warp lane per row, stored step by step without padding.
+ *   aux      HOST, nrows doubles stored with each slice (the l1 diagonal inverse for A_l), or NULL
+ *   wide     0: uint16 column indices (needs every column < 65536), 1: uint32
+ *   chunk_bytes  multiple of 128 in [1024, 65536]
+ * With out = NULL only *out_bytes / *out_nchunks / *out_nchunks_real (chunks that hold the first
+ * group) are computed.  Returns AMGDD_ERR_INDEX_RANGE for a row with more than 65535 entries,
+ * AMGDD_ERR_BAD_ARG on a bad argument or if out_capacity is too small.  Needs no CUDA device. */
+int amgdd_pack_stream(int32_t nrows, int32_t n_real, const int32_t* rowptr32, const int32_t* colind, const double* vals,
+                      const double* aux, int32_t wide, int32_t chunk_bytes, int32_t window, void* out, int64_t out_capacity,
+                      int64_t* out_bytes, int32_t* out_nchunks, int32_t* out_nchunks_real);
 
 /* ---- measurement support ------------------------------------------------------------------
  * Device time (ms, CUDA events on the handle's stream) of the phases of the most recent
@@ -175,6 +181,17 @@ int amgdd_pack_stream(int32_t nrows, const int32_t* rowptr32, const int32_t* col
  *   ms[2] AlgFAC kernel incl. gather and owned update (a3-a10)   ms[3] whole solve
  * launches[0..2]: kernel launches in the same three groups. */
 int amgdd_last_solve_profile(amgdd_handle_t h, double ms[4], int64_t launches[3]);
+
+/* Debugging aid.  If the environment variable AMGDD_FAC_PROFILE=1 was set when amgdd_setup ran,
+ * the AlgFAC kernel adds SM clock cycles to per-CTA counters; this call sums them over the CTAs
+ * into out[16] (HOST) and, with reset != 0, clears them:
+ *   [0] consumer barrier waits  [1] waits for a matrix chunk  [2] chunk processing  [3] staging the
+ *   gather vector  [4] producer waits for a free ring slot  [5] residual gather (a3)  [6] owned
+ *   update (a10)  [7] matrix-free first sweep  [8] coarse solve  [9] whole kernel
+ *   [10..14] whole mat-vec steps: relax, A t, restrict, recalculate, interpolate.
+ * Counters [0..3], [5..14] are taken by ONE consumer thread per CTA.  Returns AMGDD_ERR_BAD_ARG
+ * if profiling was not enabled.  Timed runs must not enable it. */
+int amgdd_debug_fac_cycles(amgdd_handle_t h, int64_t out[16], int32_t reset);
 
 #ifdef __cplusplus
 }

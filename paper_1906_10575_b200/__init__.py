@@ -20,7 +20,7 @@ EXPORTS = [
     "amgdd_setup", "amgdd_solve", "amgdd_solve_host", "amgdd_residual_norm", "amgdd_set_stream", "amgdd_destroy",
     "amgdd_strerror", "amgdd_last_error_detail", "amgdd_num_levels", "amgdd_level_size", "amgdd_get_cf",
     "amgdd_get_level_matrix", "amgdd_composite_size", "amgdd_get_composite", "amgdd_get_stats",
-    "amgdd_last_solve_profile", "amgdd_pack_stream",
+    "amgdd_last_solve_profile", "amgdd_pack_stream", "amgdd_debug_fac_cycles",
 ]
 
 
@@ -31,7 +31,7 @@ class AmgddStats(ctypes.Structure):
         ("sum_ghost", _i64), ("dropped_interp_entries", _i64), ("device_bytes", _i64),
         ("shared_level_instances", _i64), ("model_bytes_fac_iter", _f64 * 2), ("stream_bytes_fac_iter", _f64 * 2),
         ("model_bytes_global", _f64), ("setup_seconds_hierarchy", _f64), ("setup_seconds_composite", _f64),
-        ("chunk_bytes", _i32), ("ring_stages", _i32), ("x_cap", _i32), ("fac_grid", _i32), ("fac_block", _i32),
+        ("chunk_bytes", _i32), ("window", _i32), ("ring_stages", _i32), ("x_cap", _i32), ("fac_grid", _i32), ("fac_block", _i32),
         ("fac_smem_bytes", _i32), ("max_n_bar", _i64),
     ]
 
@@ -65,7 +65,8 @@ def _load():
     L.amgdd_get_composite.argtypes = [_vp, _i32, _i32, _vp, _vp]
     L.amgdd_get_stats.argtypes = [_vp, ctypes.POINTER(AmgddStats)]
     L.amgdd_last_solve_profile.argtypes = [_vp, _vp, _vp]
-    L.amgdd_pack_stream.argtypes = [_i32, _vp, _vp, _vp, _i32, _i32, _vp, _i64, _vp, _vp]
+    L.amgdd_debug_fac_cycles.argtypes = [_vp, _vp, _i32]
+    L.amgdd_pack_stream.argtypes = [_i32, _i32, _vp, _vp, _vp, _vp, _i32, _i32, _i32, _vp, _i64, _vp, _vp, _vp]
     return L
 
 
@@ -209,19 +210,34 @@ def amgdd_get_stats(h: Handle) -> dict:
     return d
 
 
-def amgdd_pack_stream(rowptr, colind, vals, wide=False, chunk_bytes=16384):
-    """amgdd_pack_stream: CSR (host) -> (bytes of the packed chunk stream as a uint8 array, nchunks)."""
+def amgdd_pack_stream(rowptr, colind, vals, wide=False, chunk_bytes=16384, n_real=None, aux=None, window=256):
+    """amgdd_pack_stream: CSR (host) -> (bytes of the packed slice-JDS chunk stream as a uint8 array,
+    nchunks, nchunks_real)."""
     rowptr = _np(rowptr, np.int32)
     colind = _np(colind, np.int32)
     vals = _np(vals, np.float64)
+    aux = None if aux is None else _np(aux, np.float64)
     nrows = len(rowptr) - 1
-    nbytes, nchunks = _i64(), _i32()
-    _check(lib.amgdd_pack_stream(nrows, rowptr.ctypes.data, colind.ctypes.data, vals.ctypes.data, int(wide), chunk_bytes,
-                                 None, 0, ctypes.byref(nbytes), ctypes.byref(nchunks)))
+    n_real = nrows if n_real is None else n_real
+    nbytes, nchunks, nreal = _i64(), _i32(), _i32()
+    args = (nrows, n_real, rowptr.ctypes.data, colind.ctypes.data, vals.ctypes.data, None if aux is None else aux.ctypes.data,
+            int(wide), chunk_bytes, window)
+    _check(lib.amgdd_pack_stream(*args, None, 0, ctypes.byref(nbytes), ctypes.byref(nchunks), ctypes.byref(nreal)))
     out = np.zeros(max(nbytes.value, 1), dtype=np.uint8)
-    _check(lib.amgdd_pack_stream(nrows, rowptr.ctypes.data, colind.ctypes.data, vals.ctypes.data, int(wide), chunk_bytes,
-                                 out.ctypes.data, nbytes.value, ctypes.byref(nbytes), ctypes.byref(nchunks)))
-    return out[:nbytes.value], nchunks.value
+    _check(lib.amgdd_pack_stream(*args, out.ctypes.data, nbytes.value, ctypes.byref(nbytes), ctypes.byref(nchunks),
+                                 ctypes.byref(nreal)))
+    return out[:nbytes.value], nchunks.value, nreal.value
+
+
+FAC_CYCLE_NAMES = ["sync", "wait_full", "consume", "stage", "producer_wait_empty", "gather_a3", "update_a10", "first_sweep",
+                   "coarse", "total", "op_relax", "op_At", "op_restrict", "op_recalc", "op_interp", "unused"]
+
+
+def amgdd_debug_fac_cycles(h: Handle, reset=True) -> dict:
+    """Per-phase SM cycles of the AlgFAC kernel summed over its CTAs (needs AMGDD_FAC_PROFILE=1 at setup)."""
+    out = (ctypes.c_int64 * 16)()
+    _check(lib.amgdd_debug_fac_cycles(h._h, out, int(reset)))
+    return dict(zip(FAC_CYCLE_NAMES, [int(v) for v in out]))
 
 
 def amgdd_last_solve_profile(h: Handle):

@@ -60,9 +60,10 @@ struct amgdd_handle_s {
     std::vector<long long> r_off;
     double* d_workspace = nullptr;
     long long slot_stride = 0, scratch_off = 0, scratch_len = 0;
-    int chunk_bytes = 16384, stages = 0, x_cap = 0;
+    int chunk_bytes = 16384, window = DEFAULT_WINDOW, stages = 0, x_cap = 0;
     FacLaunch fac_cfg = {1, 1024, 0};
     int* d_counter = nullptr;
+    long long* d_prof = nullptr;                // AMGDD_FAC_PROFILE=1: per-CTA cycle counters of the AlgFAC kernel
     double* d_lu = nullptr; int* d_rowperm = nullptr;
     double* d_partial = nullptr; int partial_cap = 0;
     double* d_norms = nullptr; int norms_cap = 0;
@@ -159,7 +160,7 @@ int build_composites(amgdd_handle_s* h, const std::vector<i32>& owner, int nthre
             if (cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking) != cudaSuccess) { fail(AMGDD_ERR_CUDA, "stream create failed"); return; }
             char* stage = nullptr;
             size_t stage_cap = 0;
-            CompositeBuilder cb(h->H, owner, owned, h->eta, h->nghost, h->chunk_bytes);
+            CompositeBuilder cb(h->H, owner, owned, h->eta, h->nghost, h->chunk_bytes, h->window);
             for (;;) {
                 const int p = next.fetch_add(1);
                 if (p >= P || status.load() != AMGDD_SUCCESS) break;
@@ -176,8 +177,7 @@ int build_composites(amgdd_handle_s* h, const std::vector<i32>& owner, int nthre
                 if (too_big) { fail(AMGDD_ERR_INDEX_RANGE, "a composite level exceeds 2^31-1 local nonzeros"); break; }
                 if (sm.plan.too_long_row >= 0) {
                     fail(AMGDD_ERR_INDEX_RANGE, "subdomain " + std::to_string(p) + ", level " + std::to_string(sm.plan.too_long_level) +
-                                                    ": a local matrix row does not fit one " + std::to_string(h->chunk_bytes) +
-                                                    "-byte stream chunk");
+                                                    ": a local matrix row has more than 65535 entries");
                     break;
                 }
                 const size_t bytes = (size_t)std::max<i64>(sm.plan.bytes, 16);
@@ -289,25 +289,18 @@ StreamDesc make_desc(const char* base, const StreamLayout& lay) {
     StreamDesc d;
     d.base = base;
     d.nchunks = lay.nchunks; d.nchunks_real = lay.nchunks_real; d.last_bytes = lay.last_bytes;
-    {   // threads per row: the largest power of two with at least `per_lane` nonzeros per thread
-        const double avg = lay.nrows > 0 ? (double)lay.nnz / (double)lay.nrows : 1.0;
-        const int per_lane = std::max(1, env_int("AMGDD_NNZ_PER_LANE", 4));
-        int g = 1;
-        while (g < 32 && g * 2 * per_lane <= avg) g *= 2;
-        d.lanes = g;
-    }
+    d.nslices_real = lay.nslices_real;
     d.wide = lay.wide ? 1 : 0;
-    d.pad_ = 0;
+    d.has_aux = lay.has_aux ? 1 : 0;
     return d;
 }
 
-int upload_packed(amgdd_handle_s* h, const HostCsr& M, char** dptr, StreamLayout& lay, const char* what, int l) {
+int upload_packed(amgdd_handle_s* h, const HostCsr& M, const double* aux, char** dptr, StreamLayout& lay, const char* what, int l) {
     PackedLevelStream ps;
     i64 bad = -1;
-    if (!pack_global_stream(M, h->chunk_bytes, ps, bad)) { g_detail = "a level matrix has more than 2^31-1 nonzeros"; return AMGDD_ERR_INDEX_RANGE; }
+    if (!pack_global_stream(M, aux, h->chunk_bytes, h->window, ps, bad)) { g_detail = "a level matrix has more than 2^31-1 nonzeros"; return AMGDD_ERR_INDEX_RANGE; }
     if (bad >= 0) {
-        g_detail = std::string("row ") + std::to_string(bad) + " of " + what + "_" + std::to_string(l) + " does not fit one " +
-                   std::to_string(h->chunk_bytes) + "-byte stream chunk";
+        g_detail = std::string("row ") + std::to_string(bad) + " of " + what + "_" + std::to_string(l) + " has more than 65535 entries";
         return AMGDD_ERR_INDEX_RANGE;
     }
     lay = ps.lay;
@@ -334,10 +327,10 @@ int finish_tables(amgdd_handle_s* h) {
         if (l < L)
             if ((rc = upload_csr32(h, lv.R, &g.r_rp, &g.r_ci, &g.r_v))) return rc;   // Alg. 2 P:473 needs every R_l
         if (need[l]) {
-            if ((rc = upload_packed(h, lv.A, &g.sA, g.layA, "A", l))) return rc;
+            if ((rc = upload_packed(h, lv.A, lv.dinv.data(), &g.sA, g.layA, "A", l))) return rc;
             if (l < L) {
-                if ((rc = upload_packed(h, lv.P, &g.sP, g.layP, "P", l))) return rc;
-                if ((rc = upload_packed(h, lv.R, &g.sR, g.layR, "R", l))) return rc;
+                if ((rc = upload_packed(h, lv.P, nullptr, &g.sP, g.layP, "P", l))) return rc;
+                if ((rc = upload_packed(h, lv.R, nullptr, &g.sR, g.layR, "R", l))) return rc;
             }
             if ((rc = upload(h, &g.dinv, lv.dinv.data(), lv.dinv.size()))) return rc;
             std::vector<int> id((size_t)lv.A.nrows);
@@ -435,6 +428,11 @@ int finish_tables(amgdd_handle_s* h) {
     if ((rc = dev_alloc(h, (void**)&h->d_r_all, (size_t)h->r_off[L + 1] * sizeof(double)))) return rc;
     if ((rc = upload(h, &h->d_r_off, h->r_off.data(), (size_t)L + 1))) return rc;
     if ((rc = dev_alloc(h, (void**)&h->d_counter, sizeof(int)))) return rc;
+    if (env_int("AMGDD_FAC_PROFILE", 0) > 0) {
+        const size_t bytes = (size_t)h->fac_cfg.grid * FAC_PROF_SLOTS * sizeof(long long);
+        if ((rc = dev_alloc(h, (void**)&h->d_prof, bytes))) return rc;
+        CUDA_TRY(cudaMemset(h->d_prof, 0, bytes));
+    }
     if ((rc = upload(h, &h->d_lu, h->H.lu.data(), h->H.lu.size()))) return rc;
     if ((rc = upload(h, &h->d_rowperm, h->H.rowperm.data(), h->H.rowperm.size()))) return rc;
     h->partial_cap = residual_num_blocks(h->n, h->glev[0].lanes_a);
@@ -450,7 +448,7 @@ int finish_tables(amgdd_handle_s* h) {
     st.dropped_interp_entries = 0;
     traffic_model(h);
     st.device_bytes = h->device_bytes;
-    st.chunk_bytes = h->chunk_bytes; st.ring_stages = h->stages; st.x_cap = h->x_cap;
+    st.chunk_bytes = h->chunk_bytes; st.window = h->window; st.ring_stages = h->stages; st.x_cap = h->x_cap;
     st.fac_grid = h->fac_cfg.grid; st.fac_block = h->fac_cfg.block; st.fac_smem_bytes = h->fac_cfg.smem_bytes;
     st.max_n_bar = max_nb;
     return AMGDD_SUCCESS;
@@ -520,6 +518,12 @@ int amgdd_setup(int64_t n, const int64_t* rowptr, const int32_t* colind, const d
     if (h->chunk_bytes < MIN_CHUNK_BYTES || h->chunk_bytes > MAX_CHUNK_BYTES || (h->chunk_bytes & 127)) {
         delete h;
         g_detail = "AMGDD_CHUNK_BYTES must be a multiple of 128 in [1024, 65536]";
+        return AMGDD_ERR_BAD_ARG;
+    }
+    h->window = env_int("AMGDD_WINDOW", DEFAULT_WINDOW);
+    if (h->window < SLICE_ROWS || h->window > MAX_WINDOW || (h->window % SLICE_ROWS)) {
+        delete h;
+        g_detail = "AMGDD_WINDOW must be a multiple of 32 in [32, 32768]";
         return AMGDD_ERR_BAD_ARG;
     }
     const int nthreads = default_threads();
@@ -605,6 +609,7 @@ int amgdd_solve(amgdd_handle_t h, const double* b, double* x, int32_t num_cycles
     prm.chunk_bytes = h->chunk_bytes; prm.stages = h->stages; prm.x_cap = h->x_cap;
     prm.nfac = num_fac_cycles; prm.nu = relax_sweeps;
     prm.lu = h->d_lu; prm.rowperm = h->d_rowperm; prm.nL = (int)h->H.nL;
+    prm.prof = h->d_prof;
     long long launches[3] = {0, 0, 0};
     mark();
     for (int k = 0; k < num_cycles; ++k) {
@@ -677,25 +682,31 @@ int amgdd_residual_norm(amgdd_handle_t h, const double* b, const double* x, doub
     return AMGDD_SUCCESS;
 }
 
-int amgdd_pack_stream(int32_t nrows, const int32_t* rowptr32, const int32_t* colind, const double* vals, int32_t wide,
-                      int32_t chunk_bytes, void* out, int64_t out_capacity, int64_t* out_bytes, int32_t* out_nchunks) {
+int amgdd_pack_stream(int32_t nrows, int32_t n_real, const int32_t* rowptr32, const int32_t* colind, const double* vals,
+                      const double* aux, int32_t wide, int32_t chunk_bytes, int32_t window, void* out, int64_t out_capacity,
+                      int64_t* out_bytes, int32_t* out_nchunks, int32_t* out_nchunks_real) {
     g_detail.clear();
-    if (nrows < 0 || !rowptr32 || (!colind && rowptr32[nrows] > 0) || (!vals && rowptr32[nrows] > 0) || rowptr32[0] != 0 ||
-        chunk_bytes < MIN_CHUNK_BYTES || chunk_bytes > MAX_CHUNK_BYTES || (chunk_bytes & 127)) {
+    if (nrows < 0 || n_real < 0 || n_real > nrows || !rowptr32 || (!colind && rowptr32[nrows] > 0) ||
+        (!vals && rowptr32[nrows] > 0) || rowptr32[0] != 0 || chunk_bytes < MIN_CHUNK_BYTES || chunk_bytes > MAX_CHUNK_BYTES ||
+        (chunk_bytes & 127) || window < SLICE_ROWS || window > MAX_WINDOW || (window % SLICE_ROWS)) {
         g_detail = "bad argument to amgdd_pack_stream";
         return AMGDD_ERR_BAD_ARG;
+    }
+    for (int32_t i = 0; i < nrows; ++i) {
+        if (rowptr32[i + 1] < rowptr32[i]) { g_detail = "row pointers not monotone"; return AMGDD_ERR_BAD_ARG; }
+        if (rowptr32[i + 1] - rowptr32[i] > 65535) { g_detail = "row " + std::to_string(i) + " has more than 65535 entries"; return AMGDD_ERR_INDEX_RANGE; }
     }
     if (!wide)
         for (int32_t k = 0; k < rowptr32[nrows]; ++k)
             if (colind[k] < 0 || colind[k] >= NARROW_MAX_COLS) { g_detail = "column index needs the wide form"; return AMGDD_ERR_BAD_ARG; }
-    const PackPlan pp = plan_stream(nrows, rowptr32, wide != 0, chunk_bytes, nrows);
-    if (pp.too_long_row >= 0) { g_detail = "row " + std::to_string(pp.too_long_row) + " does not fit one chunk"; return AMGDD_ERR_INDEX_RANGE; }
+    const PackPlan pp = plan_stream(nrows, rowptr32, wide != 0, aux != nullptr, chunk_bytes, n_real, window);
     if (out_bytes) *out_bytes = pp.bytes;
     if (out_nchunks) *out_nchunks = pp.nchunks;
+    if (out_nchunks_real) *out_nchunks_real = pp.nchunks_real;
     if (out) {
         if (out_capacity < pp.bytes) { g_detail = "output buffer too small"; return AMGDD_ERR_BAD_ARG; }
         std::memset(out, 0, (size_t)pp.bytes);
-        write_stream(nrows, rowptr32, colind, vals, wide != 0, chunk_bytes, (char*)out);
+        write_stream(nrows, rowptr32, colind, vals, aux, wide != 0, chunk_bytes, n_real, window, (char*)out);
     }
     return AMGDD_SUCCESS;
 }
@@ -704,6 +715,19 @@ int amgdd_last_solve_profile(amgdd_handle_t h, double ms[4], int64_t launches[3]
     if (bad_handle(h)) return AMGDD_ERR_BAD_ARG;
     if (ms) for (int i = 0; i < 4; ++i) ms[i] = h->prof_ms[i];
     if (launches) for (int i = 0; i < 3; ++i) launches[i] = h->prof_launches[i];
+    return AMGDD_SUCCESS;
+}
+
+int amgdd_debug_fac_cycles(amgdd_handle_t h, int64_t out[16], int32_t reset) {
+    if (bad_handle(h) || !out) return AMGDD_ERR_BAD_ARG;
+    for (int i = 0; i < 16; ++i) out[i] = 0;
+    if (!h->d_prof) { g_detail = "set AMGDD_FAC_PROFILE=1 before amgdd_setup"; return AMGDD_ERR_BAD_ARG; }
+    const size_t cnt = (size_t)h->fac_cfg.grid * FAC_PROF_SLOTS;
+    std::vector<long long> host(cnt);
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    CUDA_TRY(cudaMemcpy(host.data(), h->d_prof, cnt * sizeof(long long), cudaMemcpyDeviceToHost));
+    for (size_t i = 0; i < cnt; ++i) out[i % FAC_PROF_SLOTS] += host[i];
+    if (reset) CUDA_TRY(cudaMemset(h->d_prof, 0, cnt * sizeof(long long)));
     return AMGDD_SUCCESS;
 }
 

@@ -22,6 +22,9 @@
 
 #include <cuda_runtime.h>
 
+#include <climits>
+#include <type_traits>
+
 namespace amgdd {
 
 namespace {
@@ -75,6 +78,9 @@ __device__ __forceinline__ void bar_consumers(int nthreads) {
 }
 
 enum OpKind { OP_RELAX = 0, OP_AT = 1, OP_RESTRICT = 2, OP_RECALC = 3, OP_INTERP = 4 };
+// slots of the optional per-CTA cycle counters (FAC_PROF_SLOTS each; amgdd_debug_fac_cycles)
+enum ProfSlot { PROF_SYNC = 0, PROF_WAIT_FULL = 1, PROF_CONSUME = 2, PROF_STAGE = 3, PROF_WAIT_EMPTY = 4, PROF_BEGIN = 5,
+                PROF_END = 6, PROF_FIRST = 7, PROF_COARSE = 8, PROF_TOTAL = 9, PROF_OP0 = 10 };
 
 // The static program of one subdomain: the order of the mat-vecs of num_fac_cycles AlgFAC
 // V(nu,nu)-cycles (Alg. 4).  Producer and consumers both run it, so they agree on the sequence
@@ -110,7 +116,12 @@ struct Producer {
     uint32_t phase;
     uint64_t policy;
 
-    __device__ __forceinline__ void acquire() { mbar_wait(&ctrl->empty[slot], phase ^ 1u); }
+    long long* prof;
+    __device__ __forceinline__ void acquire() {
+        const long long t0 = prof ? clock64() : 0;
+        mbar_wait(&ctrl->empty[slot], phase ^ 1u);
+        if (prof) prof[PROF_WAIT_EMPTY] += clock64() - t0;
+    }
     __device__ __forceinline__ void advance() {
         if (++slot == stages) { slot = 0; phase ^= 1u; }
     }
@@ -145,46 +156,139 @@ struct Producer {
 };
 
 // ---- consumers ------------------------------------------------------------------------------
-// One chunk in shared memory.  Rows are dealt to the consumer warps in batches of G = 32/lanes
-// consecutive rows, round-robin by GLOBAL batch index (so the deal stays balanced across chunk
-// boundaries); `bnext` is the warp's next batch and is carried from chunk to chunk, which keeps
-// the per-chunk bookkeeping free of integer division.  `lanes` threads stride over a row, the row
-// sum is reduced by shuffles and epi(row, sum) runs on the first lane of the row.
-template <bool WIDE, class X, class Epi>
-__device__ __forceinline__ void consume_chunk(const char* slot, X xs, int ll /*log2 lanes*/, int ncw, int& bnext, int row_limit,
-                                              Epi epi) {
-    const int4 hdr = *reinterpret_cast<const int4*>(slot);
-    const int rb = hdr.x, nr = hdr.y, nnz = hdr.z;
-    const double* v = reinterpret_cast<const double*>(slot + CHUNK_HEADER_BYTES);
-    const char* cbase = slot + CHUNK_HEADER_BYTES + (size_t)nnz * 8;
-    const unsigned short* rowend = reinterpret_cast<const unsigned short*>(cbase + (size_t)nnz * (WIDE ? 4 : 2));
-    const int lane = threadIdx.x & 31;
-    const int lanes = 1 << ll, gl = 5 - ll;
-    const int li = lane & (lanes - 1);
-    const int sub = lane >> ll;
-    const int b_last = (rb + nr - 1) >> gl;
-    int b = bnext;
-    for (; b <= b_last; b += ncw) {
-        const int row = (b << gl) + sub;
-        const int lr = row - rb;
-        const bool valid = (lr >= 0) && (lr < nr) && (row < row_limit);
-        double sum = 0.0;
-        if (valid) {
-            const int kb = lr > 0 ? (int)rowend[lr - 1] : 0, ke = (int)rowend[lr];
-            if (WIDE) {
-                const unsigned int* ci = reinterpret_cast<const unsigned int*>(cbase);
-                for (int k = kb + li; k < ke; k += lanes) sum += v[k] * xs[ci[k]];
-            } else {
-                const unsigned short* ci = reinterpret_cast<const unsigned short*>(cbase);
-                for (int k = kb + li; k < ke; k += lanes) sum += v[k] * xs[ci[k]];
-            }
+// What a row does with its finished sum (Alg. 4 step of the mat-vec); all pointers index the
+// current level's vectors in this CTA's workspace slot.
+struct Epilogue {
+    int kind;              // OpKind, or OP_RELAX_DELTA
+    int limit;             // OP_RESTRICT: rows below this are real rows of level l+1
+    int first;             // OP_RESTRICT: first AlgFAC iteration
+    double* a;             // RELAX u | AT w | RESTRICT s_{l+1} | RECALC f_{l+1} | INTERP u | RELAX_DELTA delta
+    double* b;             // RELAX t | RESTRICT f_{l+1}
+    const double* c;       // RELAX f | AT s | RECALC s_{l+1} | RELAX_DELTA f
+};
+constexpr int OP_RELAX_DELTA = 5;
+
+__device__ __forceinline__ void apply(const Epilogue& ep, int i, double sum, double aux) {
+    switch (ep.kind) {
+        case OP_RELAX: {                   // one l1-Jacobi update (§4.1); aux = 1 / sum_j |a_ij| (S8)
+            const double dl = aux * (ep.c[i] - sum);
+            ep.a[i] += dl;
+            ep.b[i] += dl;
+            break;
         }
-        for (int o = lanes >> 1; o > 0; o >>= 1) sum += __shfl_down_sync(0xffffffffu, sum, o, lanes);
-        if (valid && li == 0) epi(row, sum);
+        case OP_RELAX_DELTA: ep.a[i] = aux * (ep.c[i] - sum); break;
+        case OP_AT: ep.a[i] = ep.c[i] + sum; break;                        // P:509 w = s_l + A_l t_l
+        case OP_RESTRICT:                                                  // P:509 s_{l+1} = R_l w ; P:511 (first iteration)
+            ep.a[i] = sum;
+            if (ep.first && i < ep.limit) ep.b[i] -= sum;
+            break;
+        case OP_RECALC: ep.a[i] = (ep.a[i] - sum) - ep.c[i]; break;
+        default: ep.a[i] += sum; break;                                    // OP_INTERP
     }
-    // a batch cut by the end of the chunk continues in the next chunk
-    if (b - ncw == b_last && ((rb + nr) & ((1 << gl) - 1)) != 0) b -= ncw;
-    bnext = b;
+}
+
+// What a warp carries from piece to piece of the slice it is working on (a slice may span chunks).
+struct SliceState {
+    double acc, aux;
+    int row;               // row of this lane, -1: none
+    int len;               // entries of that row
+    int snext;             // next slice of this warp (slices go round-robin to the consumer warps)
+};
+
+// shared-memory loads by 32-bit shared address (no generic-address arithmetic in the inner loop)
+__device__ __forceinline__ double lds_f64(uint32_t a) {
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ uint32_t lds_u16(uint32_t a) {
+    unsigned short v;
+    asm volatile("ld.shared.u16 %0, [%1];" : "=h"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ uint32_t lds_u32(uint32_t a) {
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ uint4 lds_v4(uint32_t a) {
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a));
+    return v;
+}
+// the gather vector: staged in shared memory, or read from the workspace (global memory)
+struct SmemVec {
+    uint32_t base;
+    __device__ __forceinline__ double at(uint32_t c) const { return lds_f64(base + (c << 3)); }
+};
+struct GlobalVec {
+    const double* base;
+    __device__ __forceinline__ double at(uint32_t c) const { return base[c]; }
+};
+
+// One chunk in shared memory (layout: amgdd_stream.hpp), `slot` = its shared address.  The warp
+// takes the pieces of its own slices; lane j owns row j of the slice and adds its entries in stored
+// (= column) order, so there is no cross-lane reduction and every row sum has one fixed summation
+// order.  Lanes whose row has ended re-read entry 0 of the piece and discard it: every load is
+// unconditional, so the four steps of an unrolled block overlap.
+template <bool WIDE, class X>
+__device__ __forceinline__ void consume_chunk(uint32_t slot, X xs, int ncw, int slice_limit, int has_aux, SliceState& st,
+                                              const Epilogue& ep) {
+    constexpr int CS = WIDE ? 2 : 1;                               // log2 bytes per column index
+    const int np = (int)lds_u32(slot), slice0 = (int)lds_u32(slot + 4);
+    const int lane = threadIdx.x & 31;
+    for (;;) {
+        const int i = st.snext - slice0;
+        if (i >= np || st.snext >= slice_limit) break;
+        const uint4 raw = lds_v4(slot + CHUNK_HEADER_BYTES + i * PIECE_DESC_BYTES);
+        const int k0 = (int)(raw.z & 0xFFFFu), nk = (int)(raw.z >> 16), K = (int)(raw.w & 0xFFFFu), nnz = (int)(raw.w >> 16);
+        uint32_t q = slot + raw.x;
+        if (k0 == 0) {
+            const int rid = (int)lds_u16(q + 2 * lane);
+            st.len = (int)lds_u16(q + 2 * (SLICE_ROWS + lane));
+            st.row = rid == (int)NO_ROW ? -1 : (int)raw.y + rid;
+            st.acc = 0.0;
+            q += SLICE_ROWS * 4;
+            if (has_aux) { st.aux = lds_f64(q + 8 * lane); q += SLICE_ROWS * 8; }
+        }
+        const uint32_t vb = q, cb = q + (uint32_t)nnz * 8;
+        uint32_t e = (uint32_t)lane;
+        double acc = st.acc;
+        const int len = st.len;
+        int k = k0;
+        const int kend = k0 + nk;
+        auto col = [&](uint32_t ee) { return WIDE ? lds_u32(cb + (ee << CS)) : lds_u16(cb + (ee << CS)); };
+        for (; k + 4 <= kend; k += 4) {
+            const bool a0 = k < len, a1 = k + 1 < len, a2 = k + 2 < len, a3 = k + 3 < len;
+            const uint32_t e0 = e;
+            const uint32_t e1 = e0 + __popc(__ballot_sync(0xffffffffu, a0));
+            const uint32_t e2 = e1 + __popc(__ballot_sync(0xffffffffu, a1));
+            const uint32_t e3 = e2 + __popc(__ballot_sync(0xffffffffu, a2));
+            e = e3 + __popc(__ballot_sync(0xffffffffu, a3));
+            const uint32_t f0 = a0 ? e0 : 0u, f1 = a1 ? e1 : 0u, f2 = a2 ? e2 : 0u, f3 = a3 ? e3 : 0u;
+            const uint32_t c0 = col(f0), c1 = col(f1), c2 = col(f2), c3 = col(f3);
+            const double v0 = lds_f64(vb + (f0 << 3)), v1 = lds_f64(vb + (f1 << 3));
+            const double v2 = lds_f64(vb + (f2 << 3)), v3 = lds_f64(vb + (f3 << 3));
+            const double x0 = xs.at(c0), x1 = xs.at(c1), x2 = xs.at(c2), x3 = xs.at(c3);
+            if (a0) acc = fma(v0, x0, acc);
+            if (a1) acc = fma(v1, x1, acc);
+            if (a2) acc = fma(v2, x2, acc);
+            if (a3) acc = fma(v3, x3, acc);
+        }
+        for (; k < kend; ++k) {
+            const bool a0 = k < len;
+            const uint32_t cnt = __popc(__ballot_sync(0xffffffffu, a0));
+            const uint32_t f0 = a0 ? e : 0u;
+            const double v0 = lds_f64(vb + (f0 << 3));
+            const double x0 = xs.at(col(f0));
+            if (a0) acc = fma(v0, x0, acc);
+            e += cnt;
+        }
+        st.acc = acc;
+        if (kend != K) break;                                   // the slice continues in the next chunk
+        if (st.row >= 0) apply(ep, st.row, acc, st.aux);
+        st.snext += ncw;
+    }
 }
 
 struct Consumer {
@@ -200,12 +304,20 @@ struct Consumer {
     int slot;
     uint32_t phase;
     int ctid, nct, cw, ncw;    // consumer thread id / count, consumer warp id / count
+    long long* prof;           // this CTA's cycle counters, or nullptr
 
     __device__ __forceinline__ double* U(int l) const { return ws + lev[l].voff; }
     __device__ __forceinline__ double* T(int l) const { return ws + lev[l].voff + lev[l].n_bar; }
     __device__ __forceinline__ double* S(int l) const { return ws + lev[l].voff + 2 * (size_t)lev[l].n_bar; }
     __device__ __forceinline__ double* F(int l) const { return ws + lev[l].voff + 3 * (size_t)lev[l].n_bar; }
-    __device__ __forceinline__ void sync() { bar_consumers(nct); }
+    // optional cycle counters of this CTA (FacParams::prof), written by consumer thread 0 only
+    __device__ __forceinline__ long long tick() const { return prof ? clock64() : 0; }
+    __device__ __forceinline__ void tock(int idx, long long t0) const { if (prof && ctid == 0) prof[idx] += clock64() - t0; }
+    __device__ __forceinline__ void sync() {
+        const long long t0 = tick();
+        bar_consumers(nct);
+        tock(PROF_SYNC, t0);
+    }
     __device__ __forceinline__ void advance() {
         if (++slot == stages) { slot = 0; phase ^= 1u; }
     }
@@ -224,7 +336,8 @@ struct Consumer {
 
     // ---- Alg. 2 P:475 + Alg. 4: f_l = r_l on D_l ; u = t = s = 0 ----
     __device__ __forceinline__ void begin_subdomain() {
-        sync();                                                          // previous subdomain fully done
+        sync();
+        const long long tp0 = tick();
         const int L = prm->L;
         for (int l = 0; l <= L; ++l) {
             const int n_real = lev[l].n_real, n_bar = lev[l].n_bar;
@@ -235,10 +348,12 @@ struct Consumer {
             double* f = F(l);
             for (int i = ctid; i < n_real; i += nct) f[i] = r[__ldg(gid + i)];
         }
+        tock(PROF_BEGIN, tp0);
     }
     // ---- Alg. 2: x <- x + u_0^p on Omega_0^p (disjoint targets across subdomains) ----
     __device__ __forceinline__ void end_subdomain() {
         sync();
+        const long long tp0 = tick();
         const DevSub sb = prm->sub[p];
         const double* u0 = U(0);
         const int* gid0 = lev[0].gid;
@@ -246,10 +361,12 @@ struct Consumer {
             const int li = __ldg(sb.owned + k);
             prm->x[__ldg(gid0 + li)] += u0[li];
         }
+        tock(PROF_END, tp0);
     }
     // P:506 u_l <- 0, then the first sweep needs no matrix: delta = D^{-1} f
     __device__ __forceinline__ void first_sweep(int l) {
         sync();
+        const long long tp0 = tick();
         const int n_real = lev[l].n_real, n_bar = lev[l].n_bar;
         const double* dinv = lev[l].dinv;
         double *u = U(l), *t = T(l);
@@ -259,11 +376,13 @@ struct Consumer {
             if (i < n_real) { dl = __ldg(dinv + i) * f[i]; t[i] += dl; }
             u[i] = dl;
         }
+        tock(PROF_FIRST, tp0);
     }
     // u_L = A_L^{-1} f_L with the LU factors computed at setup (Alg. 4).  One warp; columns
     // of the unit-lower / upper factors are contiguous (column-major).
     __device__ __forceinline__ void coarse() {
         sync();
+        const long long tp0 = tick();
         const int L = prm->L, n = prm->nL;
         const double* __restrict__ lu = prm->lu;
         const double* f = F(L);
@@ -288,57 +407,67 @@ struct Consumer {
         sync();
         double* uL = U(L);
         for (int i = ctid; i < n; i += nct) uL[i] = y[i];
+        tock(PROF_COARSE, tp0);
     }
 
-    template <class Epi>
-    __device__ __forceinline__ void run_chunks(const StreamDesc& d, int nchunks, bool staged, const double* xg, int row_limit, Epi epi) {
+    // one mat-vec: every chunk of the stream prefix, in ring order; `staged`: the gather vector is in xbuf
+    __device__ __forceinline__ void run_chunks(const StreamDesc& d, int nchunks, int slice_limit, bool staged, const double* xg,
+                                               const Epilogue& ep) {
         extern __shared__ __align__(128) unsigned char smem_dyn[];      // same base as in fac_kernel: keeps LDS addressing
-        const int ll = __ffs(d.lanes) - 1;
-        int bnext = cw;                                                  // batches cw, cw + ncw, ... are this warp's
+        SliceState st;
+        st.acc = 0.0; st.aux = 0.0; st.row = -1; st.len = 0; st.snext = cw;
         for (int c = 0; c < nchunks; ++c) {
+            const long long t0 = tick();
             mbar_wait(&ctrl->full[slot], phase);
-            const char* sl = reinterpret_cast<const char*>(smem_dyn + CTRL_BYTES + (size_t)x_cap * 8 + (size_t)slot * chunk_bytes);
+            tock(PROF_WAIT_FULL, t0);
+            const long long t1 = tick();
+            const uint32_t sl = smem_addr(smem_dyn) + CTRL_BYTES + (uint32_t)x_cap * 8u + (uint32_t)slot * (uint32_t)chunk_bytes;
             if (staged) {
-                const double* xs = reinterpret_cast<const double*>(smem_dyn + CTRL_BYTES);
-                if (d.wide) consume_chunk<true>(sl, xs, ll, ncw, bnext, row_limit, epi);
-                else consume_chunk<false>(sl, xs, ll, ncw, bnext, row_limit, epi);
+                SmemVec xs;
+                xs.base = smem_addr(smem_dyn) + CTRL_BYTES;
+                consume_chunk<false>(sl, xs, ncw, slice_limit, d.has_aux, st, ep);
             } else {
-                if (d.wide) consume_chunk<true>(sl, xg, ll, ncw, bnext, row_limit, epi);
-                else consume_chunk<false>(sl, xg, ll, ncw, bnext, row_limit, epi);
+                GlobalVec xs;
+                xs.base = xg;
+                if (d.wide) consume_chunk<true>(sl, xs, ncw, slice_limit, d.has_aux, st, ep);
+                else consume_chunk<false>(sl, xs, ncw, slice_limit, d.has_aux, st, ep);
             }
+            tock(PROF_CONSUME, t1);
             release();
         }
     }
 
-    // stage the gather vector of the next mat-vec in shared memory (if it fits)
+    // stage the gather vector of the next mat-vec in shared memory (if it fits; wide streams never do)
     __device__ __forceinline__ bool stage_x(const double* x, int n) {
         if (n > x_cap) return false;
+        const long long t0 = tick();
         for (int i = ctid; i < n; i += nct) xbuf[i] = x[i];
+        tock(PROF_STAGE, t0);
         return true;
     }
 
     template <int K>
     __device__ __forceinline__ void stream(int l, int it) {
         sync();                                                          // the previous step is complete
+        const long long top0 = tick();
+        Epilogue ep;
+        ep.kind = K; ep.limit = 0; ep.first = 0; ep.a = nullptr; ep.b = nullptr; ep.c = nullptr;
         if (K == OP_RELAX) {
             // one l1-Jacobi sweep on the real points (§4.1): delta from the OLD u
             // (the staged copy), then u += delta, t += delta (P:507-508 / P:517-518)
             const StreamDesc d = lev[l].A;
             const int n_real = lev[l].n_real;
-            const double* dinv = lev[l].dinv;
             double *u = U(l), *t = T(l);
-            const double* f = F(l);
             const bool staged = stage_x(u, lev[l].n_bar);
             sync();
+            ep.c = F(l);
             if (staged) {
-                run_chunks(d, d.nchunks_real, true, u, n_real, [=](int i, double au) {
-                    const double dl = __ldg(dinv + i) * (f[i] - au);
-                    u[i] += dl;
-                    t[i] += dl;
-                });
+                ep.a = u; ep.b = t;
+                run_chunks(d, d.nchunks_real, d.nslices_real, true, u, ep);
             } else {                                                     // gather from global: two passes
                 double* delta = w;
-                run_chunks(d, d.nchunks_real, false, u, n_real, [=](int i, double au) { delta[i] = __ldg(dinv + i) * (f[i] - au); });
+                ep.kind = OP_RELAX_DELTA; ep.a = delta;
+                run_chunks(d, d.nchunks_real, d.nslices_real, false, u, ep);
                 sync();
                 for (int i = ctid; i < n_real; i += nct) {
                     const double dl = delta[i];
@@ -349,45 +478,39 @@ struct Consumer {
         } else if (K == OP_AT) {
             // P:509  w = s_l + A_l t_l on all of D-bar_l (ghost rows: real columns only)
             const StreamDesc d = lev[l].A;
-            const int n_bar = lev[l].n_bar;
-            const double *t = T(l), *s = S(l);
-            double* wv = w;
-            const bool staged = stage_x(t, n_bar);
+            const double* t = T(l);
+            const bool staged = stage_x(t, lev[l].n_bar);
             sync();
-            run_chunks(d, d.nchunks, staged, t, n_bar, [=](int i, double at) { wv[i] = s[i] + at; });
+            ep.a = w; ep.c = S(l);
+            run_chunks(d, d.nchunks, INT_MAX, staged, t, ep);
         } else if (K == OP_RESTRICT) {
             // P:509  s_{l+1} = R_l w ; P:512 reset t_l, s_l ; first iteration: P:511 f_{l+1} -= s_{l+1}
             const StreamDesc d = lev[l].R;
-            const int n_bar = lev[l].n_bar, nc_bar = lev[l + 1].n_bar, nc_real = lev[l + 1].n_real;
-            double *sc = S(l + 1), *fc = F(l + 1);
-            const bool first = (it == 0);
+            const int n_bar = lev[l].n_bar;
             const bool staged = stage_x(w, n_bar);
             double* t = T(l);
             for (int i = ctid; i < 2 * n_bar; i += nct) t[i] = 0.0;      // t and s are adjacent
             sync();
-            run_chunks(d, d.nchunks, staged, w, nc_bar, [=](int I, double rw) {
-                sc[I] = rw;
-                if (first && I < nc_real) fc[I] -= rw;
-            });
+            ep.a = S(l + 1); ep.b = F(l + 1); ep.limit = lev[l + 1].n_real; ep.first = (it == 0);
+            run_chunks(d, d.nchunks, INT_MAX, staged, w, ep);
         } else if (K == OP_RECALC) {
             // P:510-511  f_{l+1} <- f_{l+1} - A_{l+1} u_{l+1} - s_{l+1}  (u_{l+1} of the previous iteration)
             const StreamDesc d = lev[l + 1].A;
-            const int nc_real = lev[l + 1].n_real;
-            const double *uc = U(l + 1), *sc = S(l + 1);
-            double* fc = F(l + 1);
+            const double* uc = U(l + 1);
             const bool staged = stage_x(uc, lev[l + 1].n_bar);
             sync();
-            run_chunks(d, d.nchunks_real, staged, uc, nc_real, [=](int I, double au) { fc[I] = (fc[I] - au) - sc[I]; });
+            ep.a = F(l + 1); ep.c = S(l + 1);
+            run_chunks(d, d.nchunks_real, d.nslices_real, staged, uc, ep);
         } else {
             // P:516  u_l += P_l u_{l+1} on all of D-bar_l (§4.2)
             const StreamDesc d = lev[l].P;
-            const int n_bar = lev[l].n_bar;
             const double* uc = U(l + 1);
-            double* u = U(l);
             const bool staged = stage_x(uc, lev[l + 1].n_bar);
             sync();
-            run_chunks(d, d.nchunks, staged, uc, n_bar, [=](int i, double pu) { u[i] += pu; });
+            ep.a = U(l);
+            run_chunks(d, d.nchunks, INT_MAX, staged, uc, ep);
         }
+        tock(PROF_OP0 + K, top0);
     }
 };
 
@@ -415,6 +538,7 @@ __global__ void __launch_bounds__(1024, 1) fac_kernel(const FacParams prm) {
             Producer pr;
             pr.ctrl = ctrl; pr.ring = ring; pr.stages = prm.stages; pr.chunk_bytes = prm.chunk_bytes;
             pr.slot = 0; pr.phase = 0; pr.policy = policy_evict_first();
+            pr.prof = prm.prof ? prm.prof + (size_t)blockIdx.x * FAC_PROF_SLOTS : nullptr;
             for (;;) {
                 const int q = atomicAdd(prm.work_counter, 1);
                 const int p = q < prm.num_sub ? prm.order[q] : -1;
@@ -434,6 +558,8 @@ __global__ void __launch_bounds__(1024, 1) fac_kernel(const FacParams prm) {
     cs.stages = prm.stages; cs.chunk_bytes = prm.chunk_bytes; cs.x_cap = prm.x_cap;
     cs.slot = 0; cs.phase = 0;
     cs.ctid = threadIdx.x - 32; cs.nct = blockDim.x - 32; cs.cw = warp - 1; cs.ncw = ncw;
+    cs.prof = prm.prof ? prm.prof + (size_t)blockIdx.x * FAC_PROF_SLOTS : nullptr;
+    const long long tk0 = cs.tick();
     for (;;) {
         const int p = cs.next_subdomain();
         if (p < 0) break;
@@ -441,6 +567,7 @@ __global__ void __launch_bounds__(1024, 1) fac_kernel(const FacParams prm) {
         cs.lev = prm.lev + (size_t)p * (L + 1);
         fac_program(cs, L, prm.nfac, prm.nu);
     }
+    cs.tock(PROF_TOTAL, tk0);
 }
 
 }  // namespace

@@ -78,9 +78,11 @@ struct StreamLayout {
     i64 off = -1;                // byte offset inside the blob (16-byte aligned)
     i64 bytes = 0;
     i32 nchunks = 0, nchunks_real = 0, last_bytes = 0;
+    i32 nslices = 0, nslices_real = 0;
     i32 nrows = 0;
     i64 nnz = 0;
     bool wide = false;           // uint32 column indices
+    bool has_aux = false;        // first pieces carry the l1 diagonal inverse of their rows
 };
 
 // Sizes of one (subdomain, level) block and where its arrays sit inside the subdomain's blob.
@@ -100,7 +102,7 @@ struct SubdomainBlob {
     i32 n_owned = 0;
     i64 bytes = 0;                    // blob size
     i64 dropped = 0;                  // A7 count
-    i64 too_long_row = -1;            // a local row that does not fit one stream chunk (-1: none)
+    i64 too_long_row = -1;            // a local row with more than 65535 entries (-1: none)
     i32 too_long_level = -1;
 };
 
@@ -114,7 +116,7 @@ struct LocalCsr {
 class CompositeBuilder {
 public:
     CompositeBuilder(const Hierarchy& H, const std::vector<i32>& owner, const std::vector<std::vector<i32>>& owned,
-                     int eta, int num_ghost, int chunk_bytes);
+                     int eta, int num_ghost, int chunk_bytes, int window);
     // Phase 1: index sets, local matrices and the blob layout of subdomain p.
     void plan(int p, SubdomainBlob& out);
     // Phase 2: write the arrays of the subdomain planned last into dst (out.bytes bytes).
@@ -128,13 +130,14 @@ private:
     const Hierarchy& H_;
     const std::vector<i32>& owner_;
     const std::vector<std::vector<i32>>& owned_;
-    int eta_, nghost_, chunk_bytes_, p_ = -1;
+    int eta_, nghost_, chunk_bytes_, window_, p_ = -1;
     std::vector<std::vector<i32>> real_, ghost_;
     std::vector<LocalCsr> A_, P_, R_;                 // local matrices of the subdomain planned last
     // epoch-stamped global->local maps, one per level
     std::vector<std::vector<i32>> loc_, stamp_;
     std::vector<i32> epoch_;
     std::vector<i32> frontier_, next_, cursor_;
+    std::vector<double> aux_;
     i32 local_of(int l, i32 g) const { return stamp_[l][g] == epoch_[l] ? loc_[l][g] : -1; }
 };
 
@@ -143,6 +146,7 @@ struct PackedLevelStream {
     std::vector<char> data;
     StreamLayout lay;
 };
-bool pack_global_stream(const HostCsr& M, int chunk_bytes, PackedLevelStream& out, i64& too_long_row);
+// aux: M.nrows doubles (l1 diagonal inverse, A streams) or nullptr
+bool pack_global_stream(const HostCsr& M, const double* aux, int chunk_bytes, int window, PackedLevelStream& out, i64& too_long_row);
 
 }  // namespace amgdd

@@ -1,9 +1,11 @@
-// Host packer of the chunked CSR stream format (layout: amgdd_stream.hpp).  Rows are packed
-// greedily: a chunk takes consecutive whole rows while header + values + column indices + row
-// ends fit `chunk_bytes`.  Index work only; no arithmetic of the method.
+// Host packer of the slice-JDS chunk stream (layout: amgdd_stream.hpp).  Index work only; no
+// arithmetic of the method.  One walker lays the pieces down; the planner and the writer are two
+// sets of callbacks on it, so they cannot disagree.
 #include "amgdd_stream.hpp"
 
+#include <algorithm>
 #include <cstring>
+#include <vector>
 
 namespace amgdd {
 
@@ -11,65 +13,166 @@ namespace {
 
 inline int64_t align16(int64_t x) { return (x + 15) & ~(int64_t)15; }
 
-// calls emit(row_begin, row_end) for every chunk; returns a row that fits no chunk, or -1
-template <class Emit>
-int64_t for_each_chunk(int nrows, const int32_t* rp, bool wide, int chunk_bytes, Emit emit) {
-    int r = 0;
-    while (r < nrows) {
-        int e = r;
-        int64_t nnz = 0;
-        while (e < nrows) {
-            const int64_t len = rp[e + 1] - rp[e];
-            if (nnz + len > 65535) break;                                   // rowend is 16-bit
-            if (chunk_payload_bytes(e + 1 - r, nnz + len, wide) > chunk_bytes) break;
-            nnz += len;
-            ++e;
+struct Slice {
+    int row_base;                 // first row of the window
+    int nrows;                    // rows in the slice (<= 32)
+    int rows[SLICE_ROWS];         // row of lane j (sorted by descending length, stable)
+    int len[SLICE_ROWS];
+    int K;                        // longest row
+};
+
+struct Piece {
+    Slice sl;
+    int k0, nk, nnz;
+    int64_t data_bytes;           // padded to 16
+};
+
+inline int prefix_bytes(bool has_aux) { return SLICE_ROWS * 2 * 2 + (has_aux ? SLICE_ROWS * 8 : 0); }
+
+// entries of step k of a slice = rows longer than k (a prefix of the lanes)
+inline int step_count(const Slice& s, int k) {
+    int c = 0;
+    while (c < s.nrows && s.len[c] > k) ++c;
+    return c;
+}
+
+// Calls on_chunk(chunk_index, pieces) for every chunk, in order.  Returns {nslices, nslices_real,
+// chunk index holding the end of the last slice of the first group (-1 if that group is empty)}.
+struct WalkResult { int nslices, nslices_real, last_real_chunk; };
+
+template <class OnChunk>
+WalkResult walk(int nrows, const int32_t* rp, bool wide, bool has_aux, int chunk_bytes, int n_real, int window,
+                OnChunk on_chunk) {
+    const int cw = wide ? 4 : 2;
+    std::vector<Piece> pending;
+    int64_t used = CHUNK_HEADER_BYTES;
+    int chunk = 0;
+    WalkResult res = {0, 0, -1};
+    auto close = [&]() {
+        if (pending.empty()) return;
+        on_chunk(chunk, pending);
+        pending.clear();
+        used = CHUNK_HEADER_BYTES;
+        ++chunk;
+    };
+    std::vector<int> order;
+    const int gb[3] = {0, std::min(n_real, nrows), nrows};
+    for (int g = 0; g < 2; ++g) {
+        for (int w0 = gb[g]; w0 < gb[g + 1]; w0 += window) {
+            const int w1 = std::min(w0 + window, gb[g + 1]);
+            order.resize(w1 - w0);
+            for (int i = 0; i < w1 - w0; ++i) order[i] = w0 + i;
+            std::stable_sort(order.begin(), order.end(),
+                             [&](int a, int b) { return rp[a + 1] - rp[a] > rp[b + 1] - rp[b]; });
+            for (int s0 = 0; s0 < w1 - w0; s0 += SLICE_ROWS) {
+                Slice sl;
+                sl.row_base = w0;
+                sl.nrows = std::min(SLICE_ROWS, w1 - w0 - s0);
+                for (int j = 0; j < SLICE_ROWS; ++j) {
+                    sl.rows[j] = j < sl.nrows ? order[s0 + j] : -1;
+                    sl.len[j] = j < sl.nrows ? rp[sl.rows[j] + 1] - rp[sl.rows[j]] : 0;
+                }
+                sl.K = sl.len[0];
+                ++res.nslices;
+                if (g == 0) ++res.nslices_real;
+                int k = 0;
+                for (;;) {                                         // at least one piece, also for K = 0
+                    const int64_t fixed = PIECE_DESC_BYTES + (k == 0 ? prefix_bytes(has_aux) : 0);
+                    const int64_t room = chunk_bytes - used - fixed;
+                    int nk = 0, nnz = 0;
+                    if (room >= 0) {
+                        while (k + nk < sl.K && nk < 65535) {
+                            const int c = step_count(sl, k + nk);
+                            if (nnz + c > 65535 || align16((int64_t)(nnz + c) * (8 + cw)) > room) break;
+                            nnz += c;
+                            ++nk;
+                        }
+                    }
+                    if (room < 0 || (nk == 0 && sl.K > 0)) { close(); continue; }   // nothing fits: next chunk
+                    Piece pc;
+                    pc.sl = sl; pc.k0 = k; pc.nk = nk; pc.nnz = nnz;
+                    pc.data_bytes = (k == 0 ? prefix_bytes(has_aux) : 0) + align16((int64_t)nnz * (8 + cw));
+                    used += PIECE_DESC_BYTES + pc.data_bytes;
+                    pending.push_back(pc);
+                    k += nk;
+                    if (k >= sl.K) break;
+                }
+                if (g == 0) res.last_real_chunk = chunk;
+            }
         }
-        if (e == r) return r;                                               // row r alone is too long
-        emit(r, e);
-        r = e;
     }
-    return -1;
+    close();
+    return res;
+}
+
+inline int64_t chunk_used_bytes(const std::vector<Piece>& pcs) {
+    int64_t b = CHUNK_HEADER_BYTES;
+    for (const Piece& p : pcs) b += PIECE_DESC_BYTES + p.data_bytes;
+    return b;
 }
 
 }  // namespace
 
-PackPlan plan_stream(int nrows, const int32_t* rp, bool wide, int chunk_bytes, int n_real) {
+PackPlan plan_stream(int nrows, const int32_t* rp, bool wide, bool has_aux, int chunk_bytes, int n_real, int window) {
     PackPlan p;
-    p.bytes = 0; p.nchunks = 0; p.nchunks_real = 0; p.last_bytes = 0;
-    p.too_long_row = for_each_chunk(nrows, rp, wide, chunk_bytes, [&](int r, int e) {
+    p.bytes = 0; p.nchunks = 0; p.nchunks_real = 0; p.last_bytes = 0; p.nslices = 0; p.nslices_real = 0;
+    const WalkResult r = walk(nrows, rp, wide, has_aux, chunk_bytes, n_real, window, [&](int, const std::vector<Piece>& pcs) {
         ++p.nchunks;
-        if (r < n_real) p.nchunks_real = p.nchunks;
-        p.last_bytes = (int)align16(chunk_payload_bytes(e - r, rp[e] - rp[r], wide));
+        p.last_bytes = (int)chunk_used_bytes(pcs);
     });
+    p.nslices = r.nslices; p.nslices_real = r.nslices_real;
+    p.nchunks_real = r.last_real_chunk + 1;
     if (p.nchunks > 0) p.bytes = (int64_t)(p.nchunks - 1) * chunk_bytes + p.last_bytes;
     return p;
 }
 
-void write_stream(int nrows, const int32_t* rp, const int32_t* ci, const double* v, bool wide, int chunk_bytes,
-                  char* dst) {
-    int c = 0;
-    for_each_chunk(nrows, rp, wide, chunk_bytes, [&](int r, int e) {
+void write_stream(int nrows, const int32_t* rp, const int32_t* ci, const double* v, const double* aux, bool wide,
+                  int chunk_bytes, int n_real, int window, char* dst) {
+    const bool has_aux = aux != nullptr;
+    int slice_counter = 0;                                         // slices started so far
+    walk(nrows, rp, wide, has_aux, chunk_bytes, n_real, window, [&](int c, const std::vector<Piece>& pcs) {
         char* out = dst + (int64_t)c * chunk_bytes;
-        const int nnz = rp[e] - rp[r], nr = e - r;
-        const int64_t used = chunk_payload_bytes(nr, nnz, wide);
-        const int64_t padded = align16(used);
-        int32_t hdr[4] = {r, nr, nnz, 0};
+        const int64_t used = chunk_used_bytes(pcs);
+        std::memset(out, 0, (size_t)used);
+        // piece 0 continues the slice started last iff its k0 > 0
+        const uint32_t slice0 = (uint32_t)(pcs[0].k0 > 0 ? slice_counter - 1 : slice_counter);
+        uint32_t hdr[4] = {(uint32_t)pcs.size(), slice0, 0, 0};
         std::memcpy(out, hdr, 16);
-        std::memcpy(out + 16, v + rp[r], (size_t)nnz * 8);
-        char* pci = out + 16 + (int64_t)nnz * 8;
-        if (wide) {
-            std::memcpy(pci, ci + rp[r], (size_t)nnz * 4);
-            pci += (int64_t)nnz * 4;
-        } else {
-            uint16_t* c16 = (uint16_t*)pci;
-            for (int k = 0; k < nnz; ++k) c16[k] = (uint16_t)ci[rp[r] + k];
-            pci += (int64_t)nnz * 2;
+        int64_t off = CHUNK_HEADER_BYTES + (int64_t)PIECE_DESC_BYTES * (int64_t)pcs.size();
+        for (size_t i = 0; i < pcs.size(); ++i) {
+            const Piece& pc = pcs[i];
+            if (pc.k0 == 0) ++slice_counter;
+            PieceDesc d;
+            d.off = (uint32_t)off; d.row_base = (uint32_t)pc.sl.row_base;
+            d.k0 = (uint16_t)pc.k0; d.nk = (uint16_t)pc.nk; d.K = (uint16_t)pc.sl.K; d.nnz = (uint16_t)pc.nnz;
+            std::memcpy(out + CHUNK_HEADER_BYTES + i * PIECE_DESC_BYTES, &d, sizeof(d));
+            char* q = out + off;
+            if (pc.k0 == 0) {
+                uint16_t* rowid = (uint16_t*)q;
+                uint16_t* len = rowid + SLICE_ROWS;
+                for (int j = 0; j < SLICE_ROWS; ++j) {
+                    rowid[j] = pc.sl.rows[j] >= 0 ? (uint16_t)(pc.sl.rows[j] - pc.sl.row_base) : NO_ROW;
+                    len[j] = (uint16_t)pc.sl.len[j];
+                }
+                q += SLICE_ROWS * 4;
+                if (has_aux) {
+                    double* a = (double*)q;
+                    for (int j = 0; j < SLICE_ROWS; ++j) a[j] = pc.sl.rows[j] >= 0 ? aux[pc.sl.rows[j]] : 0.0;
+                    q += SLICE_ROWS * 8;
+                }
+            }
+            double* vv = (double*)q;
+            char* cc = q + (int64_t)pc.nnz * 8;
+            int e = 0;
+            for (int k = pc.k0; k < pc.k0 + pc.nk; ++k)
+                for (int j = 0; j < pc.sl.nrows && pc.sl.len[j] > k; ++j, ++e) {
+                    const int src = rp[pc.sl.rows[j]] + k;
+                    vv[e] = v[src];
+                    if (wide) ((uint32_t*)cc)[e] = (uint32_t)ci[src];
+                    else ((uint16_t*)cc)[e] = (uint16_t)ci[src];
+                }
+            off += pc.data_bytes;
         }
-        uint16_t* re = (uint16_t*)pci;
-        for (int i = 0; i < nr; ++i) re[i] = (uint16_t)(rp[r + i + 1] - rp[r]);
-        std::memset(out + used, 0, (size_t)(padded - used));
-        ++c;
     });
 }
 
