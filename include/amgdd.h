@@ -77,15 +77,16 @@ typedef struct amgdd_stats {
        recalculation), [1] every later iteration */
     double model_bytes_fac_iter[2];
     /* bytes of the packed matrix streams the kernel of THIS build actually requests from HBM per
-       iteration (chunk copies; vectors stay in shared memory / L2), same two cases */
+       iteration (block copies; vectors stay in shared memory / L2), same two cases */
     double stream_bytes_fac_iter[2];
     double model_bytes_global;       /* a1+a2+a3+a10 per AMG-DD cycle: A_0 stream, R_l streams, gathers */
     double setup_seconds_hierarchy;  /* host: S1-S5 */
     double setup_seconds_composite;  /* host: S6-S7 + local matrices + packing + upload */
     /* launch plan of the persistent AlgFAC kernel */
-    int32_t chunk_bytes;             /* stride of a packed-stream chunk = size of a ring slot */
+    int32_t block_bytes;             /* stride of a packed-stream block = size of a ring slot */
+    int32_t num_ways;                /* sub-streams per matrix = consumer warps per CTA */
     int32_t window;                  /* rows per sort window of the slice-JDS streams */
-    int32_t ring_stages;             /* ring slots per CTA */
+    int32_t ring_stages;             /* ring slots per warp */
     int32_t x_cap;                   /* doubles in the shared-memory gather buffer */
     int32_t fac_grid, fac_block, fac_smem_bytes;
     int64_t max_n_bar;               /* largest |D-bar_l^p| over all subdomains and levels */
@@ -159,20 +160,30 @@ int amgdd_get_stats(amgdd_handle_t h, amgdd_stats_t* s);
 
 /* ---- the HBM layout of the matrices, exposed for tests and tools --------------------------------
  * Packs a CSR matrix (HOST; rowptr32 has nrows+1 int32 entries starting at 0, at most 65535
- * entries per row) into the chunked "slice-JDS" stream the AlgFAC kernel reads with bulk async
- * copies (layout: DESIGN.md "Data layout", csrc/amgdd_stream.hpp): rows [0, n_real) and
- * [n_real, nrows) are two groups (real / ghost rows of a composite A_l); inside windows of
- * `window` rows (multiple of 32 in [32, 32768]) rows are sorted by length and cut into slices of 32
- * rows, one warp lane per row, stored step by step without padding.
+ * entries per row) into the "slice-JDS" streams the AlgFAC kernel reads with bulk async copies
+ * (layout: DESIGN.md "Data layout", csrc/amgdd_stream.hpp): rows [0, n_real) and [n_real, nrows)
+ * are two groups (real / ghost rows of a composite A_l); inside windows of `window` rows
+ * (multiple of 32 in [32, 32768]) rows are sorted by length and cut into slices of 32 rows, one
+ * warp lane per row, stored step by step without padding; the slices are dealt to AMGDD_NUM_WAYS
+ * sub-streams ("ways", one per consumer warp), each a sequence of blocks of `block_bytes` bytes.
  *   aux      HOST, nrows doubles stored with each slice (the l1 diagonal inverse for A_l), or NULL
  *   wide     0: uint16 column indices (needs every column < 65536), 1: uint32
- *   chunk_bytes  multiple of 128 in [1024, 65536]
- * With out = NULL only *out_bytes / *out_nchunks / *out_nchunks_real (chunks that hold the first
- * group) are computed.  Returns AMGDD_ERR_INDEX_RANGE for a row with more than 65535 entries,
- * AMGDD_ERR_BAD_ARG on a bad argument or if out_capacity is too small.  Needs no CUDA device. */
+ *   block_bytes  multiple of 128 in [1024, 32768]
+ *   out_ways HOST, AMGDD_NUM_WAYS entries, or NULL
+ * With out = NULL only *out_bytes and out_ways are computed.  Returns AMGDD_ERR_INDEX_RANGE for a
+ * row with more than 65535 entries, AMGDD_ERR_BAD_ARG on a bad argument or if out_capacity is too
+ * small.  Needs no CUDA device. */
+#define AMGDD_NUM_WAYS 16
+typedef struct amgdd_way {
+    uint32_t off16;        /* start of the way: 16 * off16 bytes from the start of the stream */
+    uint32_t nblocks;      /* blocks of the way; block j starts at 16 * off16 + j * block_bytes */
+    uint32_t nblocks_real; /* leading blocks that hold the way's slices of the first row group */
+    uint16_t last16;       /* the last block is cut at 16 * last16 bytes */
+    uint16_t nslices_real; /* slices of the first row group in this way */
+} amgdd_way_t;
 int amgdd_pack_stream(int32_t nrows, int32_t n_real, const int32_t* rowptr32, const int32_t* colind, const double* vals,
-                      const double* aux, int32_t wide, int32_t chunk_bytes, int32_t window, void* out, int64_t out_capacity,
-                      int64_t* out_bytes, int32_t* out_nchunks, int32_t* out_nchunks_real);
+                      const double* aux, int32_t wide, int32_t block_bytes, int32_t window, void* out, int64_t out_capacity,
+                      int64_t* out_bytes, amgdd_way_t* out_ways);
 
 /* ---- measurement support ------------------------------------------------------------------
  * Device time (ms, CUDA events on the handle's stream) of the phases of the most recent

@@ -31,7 +31,7 @@ class AmgddStats(ctypes.Structure):
         ("sum_ghost", _i64), ("dropped_interp_entries", _i64), ("device_bytes", _i64),
         ("shared_level_instances", _i64), ("model_bytes_fac_iter", _f64 * 2), ("stream_bytes_fac_iter", _f64 * 2),
         ("model_bytes_global", _f64), ("setup_seconds_hierarchy", _f64), ("setup_seconds_composite", _f64),
-        ("chunk_bytes", _i32), ("window", _i32), ("ring_stages", _i32), ("x_cap", _i32), ("fac_grid", _i32), ("fac_block", _i32),
+        ("block_bytes", _i32), ("num_ways", _i32), ("window", _i32), ("ring_stages", _i32), ("x_cap", _i32), ("fac_grid", _i32), ("fac_block", _i32),
         ("fac_smem_bytes", _i32), ("max_n_bar", _i64),
     ]
 
@@ -66,7 +66,7 @@ def _load():
     L.amgdd_get_stats.argtypes = [_vp, ctypes.POINTER(AmgddStats)]
     L.amgdd_last_solve_profile.argtypes = [_vp, _vp, _vp]
     L.amgdd_debug_fac_cycles.argtypes = [_vp, _vp, _i32]
-    L.amgdd_pack_stream.argtypes = [_i32, _i32, _vp, _vp, _vp, _vp, _i32, _i32, _i32, _vp, _i64, _vp, _vp, _vp]
+    L.amgdd_pack_stream.argtypes = [_i32, _i32, _vp, _vp, _vp, _vp, _i32, _i32, _i32, _vp, _i64, _vp, _vp]
     return L
 
 
@@ -210,23 +210,28 @@ def amgdd_get_stats(h: Handle) -> dict:
     return d
 
 
-def amgdd_pack_stream(rowptr, colind, vals, wide=False, chunk_bytes=16384, n_real=None, aux=None, window=256):
-    """amgdd_pack_stream: CSR (host) -> (bytes of the packed slice-JDS chunk stream as a uint8 array,
-    nchunks, nchunks_real)."""
+NUM_WAYS = 16
+WAY_DTYPE = np.dtype([("off16", np.uint32), ("nblocks", np.uint32), ("nblocks_real", np.uint32), ("last16", np.uint16),
+                      ("nslices_real", np.uint16)])
+
+
+def amgdd_pack_stream(rowptr, colind, vals, wide=False, block_bytes=2048, n_real=None, aux=None, window=256):
+    """amgdd_pack_stream: CSR (host) -> (bytes of the packed slice-JDS streams as a uint8 array, the
+    NUM_WAYS way descriptors as a structured array)."""
     rowptr = _np(rowptr, np.int32)
     colind = _np(colind, np.int32)
     vals = _np(vals, np.float64)
     aux = None if aux is None else _np(aux, np.float64)
     nrows = len(rowptr) - 1
     n_real = nrows if n_real is None else n_real
-    nbytes, nchunks, nreal = _i64(), _i32(), _i32()
+    nbytes = _i64()
+    ways = np.zeros(NUM_WAYS, dtype=WAY_DTYPE)
     args = (nrows, n_real, rowptr.ctypes.data, colind.ctypes.data, vals.ctypes.data, None if aux is None else aux.ctypes.data,
-            int(wide), chunk_bytes, window)
-    _check(lib.amgdd_pack_stream(*args, None, 0, ctypes.byref(nbytes), ctypes.byref(nchunks), ctypes.byref(nreal)))
+            int(wide), block_bytes, window)
+    _check(lib.amgdd_pack_stream(*args, None, 0, ctypes.byref(nbytes), ways.ctypes.data))
     out = np.zeros(max(nbytes.value, 1), dtype=np.uint8)
-    _check(lib.amgdd_pack_stream(*args, out.ctypes.data, nbytes.value, ctypes.byref(nbytes), ctypes.byref(nchunks),
-                                 ctypes.byref(nreal)))
-    return out[:nbytes.value], nchunks.value, nreal.value
+    _check(lib.amgdd_pack_stream(*args, out.ctypes.data, nbytes.value, ctypes.byref(nbytes), ways.ctypes.data))
+    return out[:nbytes.value], ways
 
 
 FAC_CYCLE_NAMES = ["sync", "wait_full", "consume", "stage", "producer_wait_empty", "gather_a3", "update_a10", "first_sweep",

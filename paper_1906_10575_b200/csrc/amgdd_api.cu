@@ -60,8 +60,8 @@ struct amgdd_handle_s {
     std::vector<long long> r_off;
     double* d_workspace = nullptr;
     long long slot_stride = 0, scratch_off = 0, scratch_len = 0;
-    int chunk_bytes = 16384, window = DEFAULT_WINDOW, stages = 0, x_cap = 0;
-    FacLaunch fac_cfg = {1, 1024, 0};
+    int block_bytes = DEFAULT_BLOCK_BYTES, window = DEFAULT_WINDOW, stages = 0, x_cap = 0, table_bytes = 0;
+    FacLaunch fac_cfg = {1, 32 * NUM_WAYS, 0};
     int* d_counter = nullptr;
     long long* d_prof = nullptr;                // AMGDD_FAC_PROFILE=1: per-CTA cycle counters of the AlgFAC kernel
     double* d_lu = nullptr; int* d_rowperm = nullptr;
@@ -160,7 +160,7 @@ int build_composites(amgdd_handle_s* h, const std::vector<i32>& owner, int nthre
             if (cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking) != cudaSuccess) { fail(AMGDD_ERR_CUDA, "stream create failed"); return; }
             char* stage = nullptr;
             size_t stage_cap = 0;
-            CompositeBuilder cb(h->H, owner, owned, h->eta, h->nghost, h->chunk_bytes, h->window);
+            CompositeBuilder cb(h->H, owner, owned, h->eta, h->nghost, h->block_bytes, h->window);
             for (;;) {
                 const int p = next.fetch_add(1);
                 if (p >= P || status.load() != AMGDD_SUCCESS) break;
@@ -229,13 +229,6 @@ int build_composites(amgdd_handle_s* h, const std::vector<i32>& owner, int nthre
     return AMGDD_SUCCESS;
 }
 
-// bytes the kernel requests for the first `nchunks` chunks of a stream
-double chunk_bytes_of(const StreamLayout& s, int nchunks, int chunk_bytes) {
-    if (nchunks <= 0) return 0.0;
-    if (nchunks >= s.nchunks) return (double)s.bytes;
-    return (double)nchunks * chunk_bytes;
-}
-
 // the SURVEY.md §8(d) traffic model (nu = 1) and the bytes this build's kernel actually streams
 void traffic_model(amgdd_handle_s* h) {
     amgdd_stats_t& s = h->stats;
@@ -262,10 +255,10 @@ void traffic_model(amgdd_handle_s* h) {
             model[0] += pre + at + rs + ip + post;
             model[1] += pre + at + rs + rc + ip + post;
             const StreamLayout& A = layA(l);
-            const double a_real = chunk_bytes_of(A, A.nchunks_real, h->chunk_bytes);
+            const double a_real = (double)A.bytes_real;
             const double a_all = (double)A.bytes;
             const StreamLayout& Ac = layA(l + 1);
-            const double ac_real = chunk_bytes_of(Ac, Ac.nchunks_real, h->chunk_bytes);
+            const double ac_real = (double)Ac.bytes_real;
             const double common = (l == 0 ? a_real : 0.0) + a_all + (double)layR(l).bytes + (double)layP(l).bytes + a_real;
             stream[0] += common;
             stream[1] += common + ac_real;
@@ -288,8 +281,7 @@ int env_int(const char* name, int dflt) {
 StreamDesc make_desc(const char* base, const StreamLayout& lay) {
     StreamDesc d;
     d.base = base;
-    d.nchunks = lay.nchunks; d.nchunks_real = lay.nchunks_real; d.last_bytes = lay.last_bytes;
-    d.nslices_real = lay.nslices_real;
+    for (int w = 0; w < NUM_WAYS; ++w) d.way[w] = lay.way[w];
     d.wide = lay.wide ? 1 : 0;
     d.has_aux = lay.has_aux ? 1 : 0;
     return d;
@@ -298,7 +290,7 @@ StreamDesc make_desc(const char* base, const StreamLayout& lay) {
 int upload_packed(amgdd_handle_s* h, const HostCsr& M, const double* aux, char** dptr, StreamLayout& lay, const char* what, int l) {
     PackedLevelStream ps;
     i64 bad = -1;
-    if (!pack_global_stream(M, aux, h->chunk_bytes, h->window, ps, bad)) { g_detail = "a level matrix has more than 2^31-1 nonzeros"; return AMGDD_ERR_INDEX_RANGE; }
+    if (!pack_global_stream(M, aux, h->block_bytes, h->window, ps, bad)) { g_detail = "a level matrix has more than 2^31-1 nonzeros"; return AMGDD_ERR_INDEX_RANGE; }
     if (bad >= 0) {
         g_detail = std::string("row ") + std::to_string(bad) + " of " + what + "_" + std::to_string(l) + " has more than 65535 entries";
         return AMGDD_ERR_INDEX_RANGE;
@@ -384,33 +376,34 @@ int finish_tables(amgdd_handle_s* h) {
     h->scratch_off = max_sum;
     h->slot_stride = (max_sum + h->scratch_len + 15) & ~15LL;
 
-    // launch plan of the persistent AlgFAC kernel: one CTA per SM slot, the shared memory split
-    // between the gather buffer (x_cap doubles) and the chunk ring (stages x chunk_bytes)
+    // launch plan of the persistent AlgFAC kernel: one CTA of NUM_WAYS warps per SM; the shared
+    // memory is split between two descriptor-table slots, the gather buffer (x_cap doubles) and
+    // NUM_WAYS private rings of `stages` blocks
     cudaDeviceProp prop;
     CUDA_TRY(cudaGetDeviceProperties(&prop, h->device));
-    const int per_sm = std::max(1, std::min(4, env_int("AMGDD_CTAS_PER_SM", 1)));
-    int threads = env_int("AMGDD_THREADS", per_sm == 1 ? 1024 : 512);
-    threads = std::max(64, std::min(1024, (threads / 32) * 32));
-    const int smem_optin = (int)prop.sharedMemPerBlockOptin;
-    int smem_cta = smem_optin;
-    if (per_sm > 1) smem_cta = std::min(smem_optin, (int)(prop.sharedMemPerMultiprocessor / per_sm) - 1024);
-    const int min_stages = 3;
-    const int ctrl = fac_smem_bytes(0, 0, 0);
+    const int smem_cta = (int)prop.sharedMemPerBlockOptin;
+    h->table_bytes = (int)(((size_t)(L + 1) * sizeof(DevLevel) + 127) & ~(size_t)127);
+    const int fixed = fac_smem_bytes(h->block_bytes, 0, 0, h->table_bytes);
+    const int ring1 = NUM_WAYS * h->block_bytes;                    // one stage of all rings
+    int want_stages = env_int("AMGDD_STAGES", 4);
+    want_stages = std::max(2, std::min(fac_max_stages(), want_stages));
+    const int min_stages = 2;
     long long x_cap = (max_nb + 15) & ~15LL;
-    const long long x_cap_max = ((long long)(smem_cta - ctrl - min_stages * h->chunk_bytes) / 8) & ~15LL;
-    if (x_cap_max < 64) { g_detail = "chunk size too large for the shared memory of this device"; return AMGDD_ERR_BAD_ARG; }
+    const long long x_cap_max = ((long long)(smem_cta - fixed - min_stages * ring1) / 8) & ~15LL;
+    if (x_cap_max < 64) { g_detail = "block size too large for the shared memory of this device"; return AMGDD_ERR_BAD_ARG; }
+    // prefer the wanted ring depth over staging the very largest levels: cap x_cap so that it leaves room
+    const long long x_cap_pref = ((long long)(smem_cta - fixed - want_stages * ring1) / 8) & ~15LL;
+    x_cap = std::min(x_cap, std::max<long long>(x_cap_pref, 1024));
     x_cap = std::min(x_cap, x_cap_max);
     const int x_env = env_int("AMGDD_XCAP", -1);
     if (x_env >= 0) x_cap = std::min<long long>(x_cap_max, (x_env + 15) & ~15);
     x_cap = std::max<long long>(x_cap, 16);
     h->x_cap = (int)x_cap;
-    h->stages = std::min(fac_max_stages(), (int)((smem_cta - ctrl - x_cap * 8) / h->chunk_bytes));
-    const int st_env = env_int("AMGDD_STAGES", -1);
-    if (st_env >= 2) h->stages = std::min(h->stages, st_env);
-    h->fac_cfg.block = threads;
-    h->fac_cfg.smem_bytes = fac_smem_bytes(h->chunk_bytes, h->stages, h->x_cap);
-    h->fac_cfg.grid = std::max(1, std::min(P, prop.multiProcessorCount * per_sm));
-    if (fac_configure(h->device, smem_optin) != 0) { g_detail = "cudaFuncSetAttribute(max dynamic shared memory) failed"; cudaGetLastError(); return AMGDD_ERR_CUDA; }
+    h->stages = std::min(want_stages, (int)((smem_cta - fixed - x_cap * 8) / ring1));
+    h->fac_cfg.block = 32 * NUM_WAYS;
+    h->fac_cfg.smem_bytes = fac_smem_bytes(h->block_bytes, h->stages, h->x_cap, h->table_bytes);
+    h->fac_cfg.grid = std::max(1, std::min(P, prop.multiProcessorCount));
+    if (fac_configure(h->device, smem_cta) != 0) { g_detail = "cudaFuncSetAttribute(max dynamic shared memory) failed"; cudaGetLastError(); return AMGDD_ERR_CUDA; }
 
     if ((rc = dev_alloc(h, (void**)&h->d_workspace, (size_t)h->fac_cfg.grid * h->slot_stride * sizeof(double)))) return rc;
     if ((rc = upload(h, &h->d_lev, lev.data(), lev.size()))) return rc;
@@ -448,7 +441,7 @@ int finish_tables(amgdd_handle_s* h) {
     st.dropped_interp_entries = 0;
     traffic_model(h);
     st.device_bytes = h->device_bytes;
-    st.chunk_bytes = h->chunk_bytes; st.window = h->window; st.ring_stages = h->stages; st.x_cap = h->x_cap;
+    st.block_bytes = h->block_bytes; st.num_ways = NUM_WAYS; st.window = h->window; st.ring_stages = h->stages; st.x_cap = h->x_cap;
     st.fac_grid = h->fac_cfg.grid; st.fac_block = h->fac_cfg.block; st.fac_smem_bytes = h->fac_cfg.smem_bytes;
     st.max_n_bar = max_nb;
     return AMGDD_SUCCESS;
@@ -514,10 +507,10 @@ int amgdd_setup(int64_t n, const int64_t* rowptr, const int32_t* colind, const d
     std::memset(&h->stats, 0, sizeof(h->stats));
     if (cudaGetDevice(&h->device) != cudaSuccess) { delete h; g_detail = "cudaGetDevice failed"; return AMGDD_ERR_CUDA; }
     h->n = n; h->P = num_subdomains; h->eta = eta; h->nghost = num_ghost;
-    h->chunk_bytes = env_int("AMGDD_CHUNK_BYTES", 16384);
-    if (h->chunk_bytes < MIN_CHUNK_BYTES || h->chunk_bytes > MAX_CHUNK_BYTES || (h->chunk_bytes & 127)) {
+    h->block_bytes = env_int("AMGDD_BLOCK_BYTES", DEFAULT_BLOCK_BYTES);
+    if (h->block_bytes < MIN_BLOCK_BYTES || h->block_bytes > MAX_BLOCK_BYTES || (h->block_bytes & 127)) {
         delete h;
-        g_detail = "AMGDD_CHUNK_BYTES must be a multiple of 128 in [1024, 65536]";
+        g_detail = "AMGDD_BLOCK_BYTES must be a multiple of 128 in [1024, 32768]";
         return AMGDD_ERR_BAD_ARG;
     }
     h->window = env_int("AMGDD_WINDOW", DEFAULT_WINDOW);
@@ -606,8 +599,14 @@ int amgdd_solve(amgdd_handle_t h, const double* b, double* x, int32_t num_cycles
     prm.x = x; prm.workspace = h->d_workspace;
     prm.slot_stride = h->slot_stride; prm.scratch_off = h->scratch_off;
     prm.work_counter = h->d_counter;
-    prm.chunk_bytes = h->chunk_bytes; prm.stages = h->stages; prm.x_cap = h->x_cap;
+    prm.block_bytes = h->block_bytes; prm.stages = h->stages; prm.x_cap = h->x_cap; prm.table_bytes = h->table_bytes;
     prm.nfac = num_fac_cycles; prm.nu = relax_sweeps;
+    prm.nops = fac_num_ops(L, num_fac_cycles, relax_sweeps);
+    if (prm.nops > fac_max_ops() || L > 255) {
+        g_detail = "num_fac_cycles x relax_sweeps x levels gives a program of " + std::to_string(prm.nops) + " steps; the kernel holds " +
+                   std::to_string(fac_max_ops());
+        return AMGDD_ERR_BAD_ARG;
+    }
     prm.lu = h->d_lu; prm.rowperm = h->d_rowperm; prm.nL = (int)h->H.nL;
     prm.prof = h->d_prof;
     long long launches[3] = {0, 0, 0};
@@ -683,12 +682,12 @@ int amgdd_residual_norm(amgdd_handle_t h, const double* b, const double* x, doub
 }
 
 int amgdd_pack_stream(int32_t nrows, int32_t n_real, const int32_t* rowptr32, const int32_t* colind, const double* vals,
-                      const double* aux, int32_t wide, int32_t chunk_bytes, int32_t window, void* out, int64_t out_capacity,
-                      int64_t* out_bytes, int32_t* out_nchunks, int32_t* out_nchunks_real) {
+                      const double* aux, int32_t wide, int32_t block_bytes, int32_t window, void* out, int64_t out_capacity,
+                      int64_t* out_bytes, amgdd_way_t* out_ways) {
     g_detail.clear();
     if (nrows < 0 || n_real < 0 || n_real > nrows || !rowptr32 || (!colind && rowptr32[nrows] > 0) ||
-        (!vals && rowptr32[nrows] > 0) || rowptr32[0] != 0 || chunk_bytes < MIN_CHUNK_BYTES || chunk_bytes > MAX_CHUNK_BYTES ||
-        (chunk_bytes & 127) || window < SLICE_ROWS || window > MAX_WINDOW || (window % SLICE_ROWS)) {
+        (!vals && rowptr32[nrows] > 0) || rowptr32[0] != 0 || block_bytes < MIN_BLOCK_BYTES || block_bytes > MAX_BLOCK_BYTES ||
+        (block_bytes & 127) || window < SLICE_ROWS || window > MAX_WINDOW || (window % SLICE_ROWS)) {
         g_detail = "bad argument to amgdd_pack_stream";
         return AMGDD_ERR_BAD_ARG;
     }
@@ -699,14 +698,14 @@ int amgdd_pack_stream(int32_t nrows, int32_t n_real, const int32_t* rowptr32, co
     if (!wide)
         for (int32_t k = 0; k < rowptr32[nrows]; ++k)
             if (colind[k] < 0 || colind[k] >= NARROW_MAX_COLS) { g_detail = "column index needs the wide form"; return AMGDD_ERR_BAD_ARG; }
-    const PackPlan pp = plan_stream(nrows, rowptr32, wide != 0, aux != nullptr, chunk_bytes, n_real, window);
+    const PackPlan pp = plan_stream(nrows, rowptr32, wide != 0, aux != nullptr, block_bytes, n_real, window);
     if (out_bytes) *out_bytes = pp.bytes;
-    if (out_nchunks) *out_nchunks = pp.nchunks;
-    if (out_nchunks_real) *out_nchunks_real = pp.nchunks_real;
+    static_assert(sizeof(amgdd_way_t) == sizeof(WayDesc), "amgdd_way_t mirrors WayDesc");
+    if (out_ways) std::memcpy(out_ways, pp.way, sizeof(pp.way));
     if (out) {
         if (out_capacity < pp.bytes) { g_detail = "output buffer too small"; return AMGDD_ERR_BAD_ARG; }
         std::memset(out, 0, (size_t)pp.bytes);
-        write_stream(nrows, rowptr32, colind, vals, aux, wide != 0, chunk_bytes, n_real, window, (char*)out);
+        write_stream(nrows, rowptr32, colind, vals, aux, wide != 0, block_bytes, n_real, window, (char*)out);
     }
     return AMGDD_SUCCESS;
 }

@@ -8,6 +8,8 @@
 #include <thread>
 #include <vector>
 
+#include "amgdd_stream.hpp"
+
 namespace amgdd {
 
 typedef int64_t i64;
@@ -73,12 +75,12 @@ void parallel_for(i64 n, int nthreads, i64 chunk, F&& fn) {
 }
 
 // ---- composite grids (S6, S7) --------------------------------------------------------------
-// Where one packed CSR stream (amgdd_stream.hpp) sits inside a blob, and its chunking.
+// Where one packed stream (amgdd_stream.hpp) sits inside a blob, and its ways.
 struct StreamLayout {
     i64 off = -1;                // byte offset inside the blob (16-byte aligned)
-    i64 bytes = 0;
-    i32 nchunks = 0, nchunks_real = 0, last_bytes = 0;
-    i32 nslices = 0, nslices_real = 0;
+    i64 bytes = 0;               // all ways, all blocks
+    i64 bytes_real = 0;          // bytes of the blocks that hold the first group (what a real-rows-only mat-vec copies)
+    WayDesc way[NUM_WAYS] = {};
     i32 nrows = 0;
     i64 nnz = 0;
     bool wide = false;           // uint32 column indices
@@ -116,7 +118,7 @@ struct LocalCsr {
 class CompositeBuilder {
 public:
     CompositeBuilder(const Hierarchy& H, const std::vector<i32>& owner, const std::vector<std::vector<i32>>& owned,
-                     int eta, int num_ghost, int chunk_bytes, int window);
+                     int eta, int num_ghost, int block_bytes, int window);
     // Phase 1: index sets, local matrices and the blob layout of subdomain p.
     void plan(int p, SubdomainBlob& out);
     // Phase 2: write the arrays of the subdomain planned last into dst (out.bytes bytes).
@@ -130,7 +132,7 @@ private:
     const Hierarchy& H_;
     const std::vector<i32>& owner_;
     const std::vector<std::vector<i32>>& owned_;
-    int eta_, nghost_, chunk_bytes_, window_, p_ = -1;
+    int eta_, nghost_, block_bytes_, window_, p_ = -1;
     std::vector<std::vector<i32>> real_, ghost_;
     std::vector<LocalCsr> A_, P_, R_;                 // local matrices of the subdomain planned last
     // epoch-stamped global->local maps, one per level
@@ -147,6 +149,6 @@ struct PackedLevelStream {
     StreamLayout lay;
 };
 // aux: M.nrows doubles (l1 diagonal inverse, A streams) or nullptr
-bool pack_global_stream(const HostCsr& M, const double* aux, int chunk_bytes, int window, PackedLevelStream& out, i64& too_long_row);
+bool pack_global_stream(const HostCsr& M, const double* aux, int block_bytes, int window, PackedLevelStream& out, i64& too_long_row);
 
 }  // namespace amgdd
