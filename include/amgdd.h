@@ -77,17 +77,17 @@ typedef struct amgdd_stats {
        recalculation), [1] every later iteration */
     double model_bytes_fac_iter[2];
     /* bytes of the packed matrix streams the kernel of THIS build actually requests from HBM per
-       iteration (block copies; vectors stay in shared memory / L2), same two cases */
+       iteration (groups and slice headers; vectors stay in shared memory / L2), same two cases */
     double stream_bytes_fac_iter[2];
     double model_bytes_global;       /* a1+a2+a3+a10 per AMG-DD cycle: A_0 stream, R_l streams, gathers */
     double setup_seconds_hierarchy;  /* host: S1-S5 */
     double setup_seconds_composite;  /* host: S6-S7 + local matrices + packing + upload */
     /* launch plan of the persistent AlgFAC kernel */
-    int32_t block_bytes;             /* stride of a packed-stream block = size of a ring slot */
-    int32_t num_ways;                /* sub-streams per matrix = consumer warps per CTA */
-    int32_t window;                  /* rows per sort window of the slice-JDS streams */
-    int32_t ring_stages;             /* ring slots per warp */
-    int32_t x_cap;                   /* doubles in the shared-memory gather buffer */
+    int32_t block_bytes;             /* bytes of one (narrow) group of a packed stream = one slot of a warp's register ring */
+    int32_t num_ways;                /* sub-streams per matrix = warps per CTA */
+    int32_t window;                  /* rows per sort window of the SELL-32 streams */
+    int32_t ring_stages;             /* groups a warp keeps in flight */
+    int32_t x_cap;                   /* doubles in each of the two shared-memory vector buffers (0: they live in global memory) */
     int32_t fac_grid, fac_block, fac_smem_bytes;
     int64_t max_n_bar;               /* largest |D-bar_l^p| over all subdomains and levels */
 } amgdd_stats_t;
@@ -160,30 +160,36 @@ int amgdd_get_stats(amgdd_handle_t h, amgdd_stats_t* s);
 
 /* ---- the HBM layout of the matrices, exposed for tests and tools --------------------------------
  * Packs a CSR matrix (HOST; rowptr32 has nrows+1 int32 entries starting at 0, at most 65535
- * entries per row) into the "slice-JDS" streams the AlgFAC kernel reads with bulk async copies
- * (layout: DESIGN.md "Data layout", csrc/amgdd_stream.hpp): rows [0, n_real) and [n_real, nrows)
- * are two groups (real / ghost rows of a composite A_l); inside windows of `window` rows
- * (multiple of 32 in [32, 32768]) rows are sorted by length and cut into slices of 32 rows, one
- * warp lane per row, stored step by step without padding; the slices are dealt to AMGDD_NUM_WAYS
- * sub-streams ("ways", one per consumer warp), each a sequence of blocks of `block_bytes` bytes.
- *   aux      HOST, nrows doubles stored with each slice (the l1 diagonal inverse for A_l), or NULL
+ * entries per row) into the "SELL-32 group" streams the AlgFAC kernel reads with coalesced 128-bit
+ * loads (layout: DESIGN.md "Data layout", csrc/amgdd_stream.hpp): rows [0, n_real) and
+ * [n_real, nrows) are two row groups (real / ghost rows of a composite A_l); inside
+ * windows of `window` rows (multiple of 32 in [32, 1048576]) rows are sorted by descending length
+ * and cut into slices of 32 rows, one warp lane per row; a slice is stored as K = max(1,
+ * ceil(longest row / 4)) groups of 4 steps (zero padding past the end of a row) and one 512-byte
+ * header {row, K, aux} per lane; the slices are dealt to AMGDD_NUM_WAYS sub-streams ("ways", one
+ * per warp of the kernel).
+ *   aux      HOST, nrows doubles stored in the slice headers (the l1 diagonal inverse), or NULL (0.0)
  *   wide     0: uint16 column indices (needs every column < 65536), 1: uint32
- *   block_bytes  multiple of 128 in [1024, 32768]
  *   out_ways HOST, AMGDD_NUM_WAYS entries, or NULL
  * With out = NULL only *out_bytes and out_ways are computed.  Returns AMGDD_ERR_INDEX_RANGE for a
  * row with more than 65535 entries, AMGDD_ERR_BAD_ARG on a bad argument or if out_capacity is too
  * small.  Needs no CUDA device. */
 #define AMGDD_NUM_WAYS 16
+#define AMGDD_GROUP_BYTES_NARROW 1280
+#define AMGDD_GROUP_BYTES_WIDE 1536
+#define AMGDD_HEADER_BYTES 512
 typedef struct amgdd_way {
-    uint32_t off16;        /* start of the way: 16 * off16 bytes from the start of the stream */
-    uint32_t nblocks;      /* blocks of the way; block j starts at 16 * off16 + j * block_bytes */
-    uint32_t nblocks_real; /* leading blocks that hold the way's slices of the first row group */
-    uint16_t last16;       /* the last block is cut at 16 * last16 bytes */
-    uint16_t nslices_real; /* slices of the first row group in this way */
+    uint32_t grp_off128;   /* the way's groups start 128 * grp_off128 bytes from the start of the stream */
+    uint32_t hdr_off128;   /* its slice headers start 128 * hdr_off128 bytes from the start of the stream */
+    uint32_t ngroups;      /* groups of the way, contiguous */
+    uint32_t ngroups_real; /* leading groups that belong to slices of the first row group */
+    uint32_t nslices;      /* slices (= headers) of the way */
+    uint32_t nslices_real; /* leading slices of the first row group */
+    uint32_t reserved[2];
 } amgdd_way_t;
 int amgdd_pack_stream(int32_t nrows, int32_t n_real, const int32_t* rowptr32, const int32_t* colind, const double* vals,
-                      const double* aux, int32_t wide, int32_t block_bytes, int32_t window, void* out, int64_t out_capacity,
-                      int64_t* out_bytes, amgdd_way_t* out_ways);
+                      const double* aux, int32_t wide, int32_t window, void* out, int64_t out_capacity, int64_t* out_bytes,
+                      amgdd_way_t* out_ways);
 
 /* ---- measurement support ------------------------------------------------------------------
  * Device time (ms, CUDA events on the handle's stream) of the phases of the most recent
@@ -194,14 +200,14 @@ int amgdd_pack_stream(int32_t nrows, int32_t n_real, const int32_t* rowptr32, co
 int amgdd_last_solve_profile(amgdd_handle_t h, double ms[4], int64_t launches[3]);
 
 /* Debugging aid.  If the environment variable AMGDD_FAC_PROFILE=1 was set when amgdd_setup ran,
- * the AlgFAC kernel adds SM clock cycles to per-CTA counters; this call sums them over the CTAs
- * into out[16] (HOST) and, with reset != 0, clears them:
- *   [0] consumer barrier waits  [1] waits for a matrix chunk  [2] chunk processing  [3] staging the
- *   gather vector  [4] producer waits for a free ring slot  [5] residual gather (a3)  [6] owned
- *   update (a10)  [7] matrix-free first sweep  [8] coarse solve  [9] whole kernel
- *   [10..14] whole mat-vec steps: relax, A t, restrict, recalculate, interpolate.
- * Counters [0..3], [5..14] are taken by ONE consumer thread per CTA.  Returns AMGDD_ERR_BAD_ARG
- * if profiling was not enabled.  Timed runs must not enable it. */
+ * the AlgFAC kernel adds SM clock cycles (taken by thread 0 of each CTA) to per-CTA counters; this
+ * call sums them over the CTAs into out[16] (HOST) and, with reset != 0, clears them:
+ *   [0] CTA barrier waits  [1] fetching a subdomain and its tables  [2] work outside the mat-vec
+ *   rows (ghost carry, zeroing, staging)  [3] mat-vec start-up (first groups, first header)
+ *   [4] whole kernel  [5] residual gather (a3)  [6] matrix-free first sweep of level 0
+ *   [7..11] whole mat-vec steps: relax, A t, restrict, recalculate, interpolate
+ *   [12] coarse solve  [13] owned update (a10).
+ * Returns AMGDD_ERR_BAD_ARG if profiling was not enabled.  Timed runs must not enable it. */
 int amgdd_debug_fac_cycles(amgdd_handle_t h, int64_t out[16], int32_t reset);
 
 #ifdef __cplusplus

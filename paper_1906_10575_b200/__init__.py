@@ -66,7 +66,7 @@ def _load():
     L.amgdd_get_stats.argtypes = [_vp, ctypes.POINTER(AmgddStats)]
     L.amgdd_last_solve_profile.argtypes = [_vp, _vp, _vp]
     L.amgdd_debug_fac_cycles.argtypes = [_vp, _vp, _i32]
-    L.amgdd_pack_stream.argtypes = [_i32, _i32, _vp, _vp, _vp, _vp, _i32, _i32, _i32, _vp, _i64, _vp, _vp]
+    L.amgdd_pack_stream.argtypes = [_i32, _i32, _vp, _vp, _vp, _vp, _i32, _i32, _vp, _i64, _vp, _vp]
     return L
 
 
@@ -211,12 +211,13 @@ def amgdd_get_stats(h: Handle) -> dict:
 
 
 NUM_WAYS = 16
-WAY_DTYPE = np.dtype([("off16", np.uint32), ("nblocks", np.uint32), ("nblocks_real", np.uint32), ("last16", np.uint16),
-                      ("nslices_real", np.uint16)])
+GROUP_BYTES_NARROW, GROUP_BYTES_WIDE, HEADER_BYTES = 1280, 1536, 512
+WAY_DTYPE = np.dtype([("grp_off128", np.uint32), ("hdr_off128", np.uint32), ("ngroups", np.uint32), ("ngroups_real", np.uint32),
+                      ("nslices", np.uint32), ("nslices_real", np.uint32), ("reserved", np.uint32, (2,))])
 
 
-def amgdd_pack_stream(rowptr, colind, vals, wide=False, block_bytes=2048, n_real=None, aux=None, window=256):
-    """amgdd_pack_stream: CSR (host) -> (bytes of the packed slice-JDS streams as a uint8 array, the
+def amgdd_pack_stream(rowptr, colind, vals, wide=False, n_real=None, aux=None, window=256):
+    """amgdd_pack_stream: CSR (host) -> (bytes of the packed SELL-32 group streams as a uint8 array, the
     NUM_WAYS way descriptors as a structured array)."""
     rowptr = _np(rowptr, np.int32)
     colind = _np(colind, np.int32)
@@ -227,15 +228,15 @@ def amgdd_pack_stream(rowptr, colind, vals, wide=False, block_bytes=2048, n_real
     nbytes = _i64()
     ways = np.zeros(NUM_WAYS, dtype=WAY_DTYPE)
     args = (nrows, n_real, rowptr.ctypes.data, colind.ctypes.data, vals.ctypes.data, None if aux is None else aux.ctypes.data,
-            int(wide), block_bytes, window)
+            int(wide), window)
     _check(lib.amgdd_pack_stream(*args, None, 0, ctypes.byref(nbytes), ways.ctypes.data))
     out = np.zeros(max(nbytes.value, 1), dtype=np.uint8)
     _check(lib.amgdd_pack_stream(*args, out.ctypes.data, nbytes.value, ctypes.byref(nbytes), ways.ctypes.data))
     return out[:nbytes.value], ways
 
 
-FAC_CYCLE_NAMES = ["sync", "wait_full", "consume", "stage", "producer_wait_empty", "gather_a3", "update_a10", "first_sweep",
-                   "coarse", "total", "op_relax", "op_At", "op_restrict", "op_recalc", "op_interp", "unused"]
+FAC_CYCLE_NAMES = ["sync", "fetch_subdomain", "pre_actions", "matvec_startup", "total", "gather_a3", "first0", "op_relax", "op_At",
+                   "op_restrict", "op_recalc", "op_interp", "coarse", "update_a10", "unused14", "unused15"]
 
 
 def amgdd_debug_fac_cycles(h: Handle, reset=True) -> dict:

@@ -59,9 +59,11 @@ struct amgdd_handle_s {
     long long* d_r_off = nullptr;
     std::vector<long long> r_off;
     double* d_workspace = nullptr;
-    long long slot_stride = 0, scratch_off = 0, scratch_len = 0;
-    int block_bytes = DEFAULT_BLOCK_BYTES, window = DEFAULT_WINDOW, stages = 0, x_cap = 0, table_bytes = 0;
+    long long slot_stride = 0, xg_off = -1;
+    int window = DEFAULT_WINDOW, x_cap = 0, smem_cta = 0;
     FacLaunch fac_cfg = {1, 32 * NUM_WAYS, 0};
+    FacOp* d_ops = nullptr;                     // the program of one subdomain (fac_build_program)
+    int prog_nfac = -1, prog_nu = -1, prog_nops = 0;
     int* d_counter = nullptr;
     long long* d_prof = nullptr;                // AMGDD_FAC_PROFILE=1: per-CTA cycle counters of the AlgFAC kernel
     double* d_lu = nullptr; int* d_rowperm = nullptr;
@@ -160,7 +162,7 @@ int build_composites(amgdd_handle_s* h, const std::vector<i32>& owner, int nthre
             if (cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking) != cudaSuccess) { fail(AMGDD_ERR_CUDA, "stream create failed"); return; }
             char* stage = nullptr;
             size_t stage_cap = 0;
-            CompositeBuilder cb(h->H, owner, owned, h->eta, h->nghost, h->block_bytes, h->window);
+            CompositeBuilder cb(h->H, owner, owned, h->eta, h->nghost, h->window);
             for (;;) {
                 const int p = next.fetch_add(1);
                 if (p >= P || status.load() != AMGDD_SUCCESS) break;
@@ -280,17 +282,17 @@ int env_int(const char* name, int dflt) {
 
 StreamDesc make_desc(const char* base, const StreamLayout& lay) {
     StreamDesc d;
+    std::memset(&d, 0, sizeof(d));
     d.base = base;
     for (int w = 0; w < NUM_WAYS; ++w) d.way[w] = lay.way[w];
-    d.wide = lay.wide ? 1 : 0;
-    d.has_aux = lay.has_aux ? 1 : 0;
+    d.flags = (lay.wide ? STREAM_WIDE : 0u) | (lay.has_aux ? STREAM_AUX : 0u);
     return d;
 }
 
 int upload_packed(amgdd_handle_s* h, const HostCsr& M, const double* aux, char** dptr, StreamLayout& lay, const char* what, int l) {
     PackedLevelStream ps;
     i64 bad = -1;
-    if (!pack_global_stream(M, aux, h->block_bytes, h->window, ps, bad)) { g_detail = "a level matrix has more than 2^31-1 nonzeros"; return AMGDD_ERR_INDEX_RANGE; }
+    if (!pack_global_stream(M, aux, h->window, ps, bad)) { g_detail = "a level matrix has more than 2^31-1 nonzeros"; return AMGDD_ERR_INDEX_RANGE; }
     if (bad >= 0) {
         g_detail = std::string("row ") + std::to_string(bad) + " of " + what + "_" + std::to_string(l) + " has more than 65535 entries";
         return AMGDD_ERR_INDEX_RANGE;
@@ -322,7 +324,7 @@ int finish_tables(amgdd_handle_s* h) {
             if ((rc = upload_packed(h, lv.A, lv.dinv.data(), &g.sA, g.layA, "A", l))) return rc;
             if (l < L) {
                 if ((rc = upload_packed(h, lv.P, nullptr, &g.sP, g.layP, "P", l))) return rc;
-                if ((rc = upload_packed(h, lv.R, nullptr, &g.sR, g.layR, "R", l))) return rc;
+                if ((rc = upload_packed(h, lv.R, h->H.lv[l + 1].dinv.data(), &g.sR, g.layR, "R", l))) return rc;
             }
             if ((rc = upload(h, &g.dinv, lv.dinv.data(), lv.dinv.size()))) return rc;
             std::vector<int> id((size_t)lv.A.nrows);
@@ -372,38 +374,30 @@ int finish_tables(amgdd_handle_s* h) {
         sub[p].n_owned = sm.plan.n_owned;
     }
     st.shared_level_instances = shared_inst;
-    h->scratch_len = (max_nb + 1) & ~1LL;
-    h->scratch_off = max_sum;
-    h->slot_stride = (max_sum + h->scratch_len + 15) & ~15LL;
 
-    // launch plan of the persistent AlgFAC kernel: one CTA of NUM_WAYS warps per SM; the shared
-    // memory is split between two descriptor-table slots, the gather buffer (x_cap doubles) and
-    // NUM_WAYS private rings of `stages` blocks
+    // launch plan of the persistent AlgFAC kernel: one CTA of NUM_WAYS warps per SM.  The two vector
+    // buffers (the gather vector of a step and the one the step writes for the next) live in shared
+    // memory when the largest composite level fits twice next to the tables of the longest program;
+    // otherwise they live in the workspace slot (slow path, same arithmetic).
     cudaDeviceProp prop;
     CUDA_TRY(cudaGetDeviceProperties(&prop, h->device));
-    const int smem_cta = (int)prop.sharedMemPerBlockOptin;
-    h->table_bytes = (int)(((size_t)(L + 1) * sizeof(DevLevel) + 127) & ~(size_t)127);
-    const int fixed = fac_smem_bytes(h->block_bytes, 0, 0, h->table_bytes);
-    const int ring1 = NUM_WAYS * h->block_bytes;                    // one stage of all rings
-    int want_stages = env_int("AMGDD_STAGES", 4);
-    want_stages = std::max(2, std::min(fac_max_stages(), want_stages));
-    const int min_stages = 2;
-    long long x_cap = (max_nb + 15) & ~15LL;
-    const long long x_cap_max = ((long long)(smem_cta - fixed - min_stages * ring1) / 8) & ~15LL;
-    if (x_cap_max < 64) { g_detail = "block size too large for the shared memory of this device"; return AMGDD_ERR_BAD_ARG; }
-    // prefer the wanted ring depth over staging the very largest levels: cap x_cap so that it leaves room
-    const long long x_cap_pref = ((long long)(smem_cta - fixed - want_stages * ring1) / 8) & ~15LL;
-    x_cap = std::min(x_cap, std::max<long long>(x_cap_pref, 1024));
-    x_cap = std::min(x_cap, x_cap_max);
-    const int x_env = env_int("AMGDD_XCAP", -1);
-    if (x_env >= 0) x_cap = std::min<long long>(x_cap_max, (x_env + 15) & ~15);
-    x_cap = std::max<long long>(x_cap, 16);
-    h->x_cap = (int)x_cap;
-    h->stages = std::min(want_stages, (int)((smem_cta - fixed - x_cap * 8) / ring1));
+    h->smem_cta = (int)prop.sharedMemPerBlockOptin;
+    const long long x_need = (max_nb + 15) & ~15LL;
+    const bool force_global = env_int("AMGDD_FORCE_GLOBAL_X", 0) > 0;
+    if (!force_global && (long long)fac_smem_bytes(0, L, MAX_OPS) + 16 * x_need <= (long long)h->smem_cta) {
+        h->x_cap = (int)x_need;
+        h->xg_off = -1;
+        h->slot_stride = (max_sum + 15) & ~15LL;
+    } else {
+        h->x_cap = 0;
+        h->xg_off = (max_sum + 15) & ~15LL;
+        h->slot_stride = h->xg_off + 2 * x_need;
+    }
     h->fac_cfg.block = 32 * NUM_WAYS;
-    h->fac_cfg.smem_bytes = fac_smem_bytes(h->block_bytes, h->stages, h->x_cap, h->table_bytes);
+    h->fac_cfg.smem_bytes = fac_smem_bytes(h->x_cap, L, MAX_OPS);       // refined per solve (program length)
     h->fac_cfg.grid = std::max(1, std::min(P, prop.multiProcessorCount));
-    if (fac_configure(h->device, smem_cta) != 0) { g_detail = "cudaFuncSetAttribute(max dynamic shared memory) failed"; cudaGetLastError(); return AMGDD_ERR_CUDA; }
+    if (fac_configure(h->device, h->smem_cta) != 0) { g_detail = "cudaFuncSetAttribute(max dynamic shared memory) failed"; cudaGetLastError(); return AMGDD_ERR_CUDA; }
+    if ((rc = dev_alloc(h, (void**)&h->d_ops, (size_t)MAX_OPS * sizeof(FacOp)))) return rc;
 
     if ((rc = dev_alloc(h, (void**)&h->d_workspace, (size_t)h->fac_cfg.grid * h->slot_stride * sizeof(double)))) return rc;
     if ((rc = upload(h, &h->d_lev, lev.data(), lev.size()))) return rc;
@@ -441,7 +435,7 @@ int finish_tables(amgdd_handle_s* h) {
     st.dropped_interp_entries = 0;
     traffic_model(h);
     st.device_bytes = h->device_bytes;
-    st.block_bytes = h->block_bytes; st.num_ways = NUM_WAYS; st.window = h->window; st.ring_stages = h->stages; st.x_cap = h->x_cap;
+    st.block_bytes = GROUP_BYTES_NARROW; st.num_ways = NUM_WAYS; st.window = h->window; st.ring_stages = RING_DEPTH; st.x_cap = h->x_cap;
     st.fac_grid = h->fac_cfg.grid; st.fac_block = h->fac_cfg.block; st.fac_smem_bytes = h->fac_cfg.smem_bytes;
     st.max_n_bar = max_nb;
     return AMGDD_SUCCESS;
@@ -507,16 +501,10 @@ int amgdd_setup(int64_t n, const int64_t* rowptr, const int32_t* colind, const d
     std::memset(&h->stats, 0, sizeof(h->stats));
     if (cudaGetDevice(&h->device) != cudaSuccess) { delete h; g_detail = "cudaGetDevice failed"; return AMGDD_ERR_CUDA; }
     h->n = n; h->P = num_subdomains; h->eta = eta; h->nghost = num_ghost;
-    h->block_bytes = env_int("AMGDD_BLOCK_BYTES", DEFAULT_BLOCK_BYTES);
-    if (h->block_bytes < MIN_BLOCK_BYTES || h->block_bytes > MAX_BLOCK_BYTES || (h->block_bytes & 127)) {
-        delete h;
-        g_detail = "AMGDD_BLOCK_BYTES must be a multiple of 128 in [1024, 32768]";
-        return AMGDD_ERR_BAD_ARG;
-    }
     h->window = env_int("AMGDD_WINDOW", DEFAULT_WINDOW);
     if (h->window < SLICE_ROWS || h->window > MAX_WINDOW || (h->window % SLICE_ROWS)) {
         delete h;
-        g_detail = "AMGDD_WINDOW must be a multiple of 32 in [32, 32768]";
+        g_detail = "AMGDD_WINDOW must be a multiple of 32 in [32, 1048576]";
         return AMGDD_ERR_BAD_ARG;
     }
     const int nthreads = default_threads();
@@ -592,22 +580,31 @@ int amgdd_solve(amgdd_handle_t h, const double* b, double* x, int32_t num_cycles
         cudaEventRecord(e, h->stream);
         ev.push_back(e);
     };
+    if (h->prog_nfac != num_fac_cycles || h->prog_nu != relax_sweeps) {       // (re)build the program of one subdomain
+        const int nops = fac_build_program(L, num_fac_cycles, relax_sweeps, nullptr);
+        if (nops > MAX_OPS || L > 84) {
+            g_detail = "num_fac_cycles x relax_sweeps x levels gives a program of " + std::to_string(nops) + " steps; the kernel holds " +
+                       std::to_string(MAX_OPS);
+            return AMGDD_ERR_BAD_ARG;
+        }
+        std::vector<FacOp> ops((size_t)nops);
+        fac_build_program(L, num_fac_cycles, relax_sweeps, ops.data());
+        CUDA_TRY(cudaMemcpyAsync(h->d_ops, ops.data(), ops.size() * sizeof(FacOp), cudaMemcpyHostToDevice, h->stream));
+        CUDA_TRY(cudaStreamSynchronize(h->stream));
+        h->prog_nfac = num_fac_cycles; h->prog_nu = relax_sweeps; h->prog_nops = nops;
+        h->fac_cfg.smem_bytes = fac_smem_bytes(h->x_cap, L, nops);
+        h->stats.fac_smem_bytes = h->fac_cfg.smem_bytes;
+    }
     FacParams prm;
     prm.lev = h->d_lev; prm.sub = h->d_sub; prm.order = h->d_order;
     prm.num_sub = h->P; prm.L = L;
     prm.r_all = h->d_r_all; prm.r_off = h->d_r_off;
     prm.x = x; prm.workspace = h->d_workspace;
-    prm.slot_stride = h->slot_stride; prm.scratch_off = h->scratch_off;
+    prm.slot_stride = h->slot_stride; prm.xg_off = h->xg_off;
     prm.work_counter = h->d_counter;
-    prm.block_bytes = h->block_bytes; prm.stages = h->stages; prm.x_cap = h->x_cap; prm.table_bytes = h->table_bytes;
-    prm.nfac = num_fac_cycles; prm.nu = relax_sweeps;
-    prm.nops = fac_num_ops(L, num_fac_cycles, relax_sweeps);
-    if (prm.nops > fac_max_ops() || L > 255) {
-        g_detail = "num_fac_cycles x relax_sweeps x levels gives a program of " + std::to_string(prm.nops) + " steps; the kernel holds " +
-                   std::to_string(fac_max_ops());
-        return AMGDD_ERR_BAD_ARG;
-    }
+    prm.ops = h->d_ops; prm.nops = h->prog_nops;
     prm.lu = h->d_lu; prm.rowperm = h->d_rowperm; prm.nL = (int)h->H.nL;
+    prm.x_cap = h->x_cap;
     prm.prof = h->d_prof;
     long long launches[3] = {0, 0, 0};
     mark();
@@ -682,12 +679,11 @@ int amgdd_residual_norm(amgdd_handle_t h, const double* b, const double* x, doub
 }
 
 int amgdd_pack_stream(int32_t nrows, int32_t n_real, const int32_t* rowptr32, const int32_t* colind, const double* vals,
-                      const double* aux, int32_t wide, int32_t block_bytes, int32_t window, void* out, int64_t out_capacity,
-                      int64_t* out_bytes, amgdd_way_t* out_ways) {
+                      const double* aux, int32_t wide, int32_t window, void* out, int64_t out_capacity, int64_t* out_bytes,
+                      amgdd_way_t* out_ways) {
     g_detail.clear();
     if (nrows < 0 || n_real < 0 || n_real > nrows || !rowptr32 || (!colind && rowptr32[nrows] > 0) ||
-        (!vals && rowptr32[nrows] > 0) || rowptr32[0] != 0 || block_bytes < MIN_BLOCK_BYTES || block_bytes > MAX_BLOCK_BYTES ||
-        (block_bytes & 127) || window < SLICE_ROWS || window > MAX_WINDOW || (window % SLICE_ROWS)) {
+        (!vals && rowptr32[nrows] > 0) || rowptr32[0] != 0 || window < SLICE_ROWS || window > MAX_WINDOW || (window % SLICE_ROWS)) {
         g_detail = "bad argument to amgdd_pack_stream";
         return AMGDD_ERR_BAD_ARG;
     }
@@ -698,14 +694,13 @@ int amgdd_pack_stream(int32_t nrows, int32_t n_real, const int32_t* rowptr32, co
     if (!wide)
         for (int32_t k = 0; k < rowptr32[nrows]; ++k)
             if (colind[k] < 0 || colind[k] >= NARROW_MAX_COLS) { g_detail = "column index needs the wide form"; return AMGDD_ERR_BAD_ARG; }
-    const PackPlan pp = plan_stream(nrows, rowptr32, wide != 0, aux != nullptr, block_bytes, n_real, window);
+    const PackPlan pp = plan_stream(nrows, rowptr32, wide != 0, aux != nullptr, n_real, window);
     if (out_bytes) *out_bytes = pp.bytes;
     static_assert(sizeof(amgdd_way_t) == sizeof(WayDesc), "amgdd_way_t mirrors WayDesc");
     if (out_ways) std::memcpy(out_ways, pp.way, sizeof(pp.way));
     if (out) {
         if (out_capacity < pp.bytes) { g_detail = "output buffer too small"; return AMGDD_ERR_BAD_ARG; }
-        std::memset(out, 0, (size_t)pp.bytes);
-        write_stream(nrows, rowptr32, colind, vals, aux, wide != 0, block_bytes, n_real, window, (char*)out);
+        write_stream(nrows, rowptr32, colind, vals, aux, wide != 0, n_real, window, (char*)out);
     }
     return AMGDD_SUCCESS;
 }

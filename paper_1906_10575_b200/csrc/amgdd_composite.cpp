@@ -13,7 +13,9 @@
 //         P:230, A12)
 //   P     packed stream, n_bar rows, columns local to level l+1 (rows over all of D-bar_l)
 //   R     packed stream, n_bar(l+1) rows, columns local to level l: the explicit transpose of the
-//         local P, so restriction is a gather with a fixed summation order (no atomics)
+//         local P, so restriction is a gather with a fixed summation order (no atomics); its slice
+//         headers carry the l1 diagonal of level l+1 (the restriction's epilogue starts the
+//         relaxation of level l+1)
 // (stream format: amgdd_stream.hpp).  A level on which D_l^p = Omega_l (always true on L, reading
 // A5) is "shared": nothing is stored for it, the single global copy of the level is used (P:57
 // "each processor stores the entire coarsest grid ... may be true for a few of the coarsest grids").
@@ -26,33 +28,27 @@
 namespace amgdd {
 
 namespace {
-inline i64 align16(i64 x) { return (x + 15) & ~(i64)15; }
 
-void layout_stream(const LocalCsr& M, int nrows, int ncols, bool has_aux, int block_bytes, int window, int n_real,
-                   StreamLayout& s, i64& too_long_row) {
+void layout_stream(const LocalCsr& M, int nrows, int ncols, bool has_aux, int window, int n_real, StreamLayout& s,
+                   i64& too_long_row) {
     s.nrows = nrows;
     s.nnz = M.rp[nrows];
     s.wide = ncols > NARROW_MAX_COLS;
     s.has_aux = has_aux;
     for (int i = 0; i < nrows && too_long_row < 0; ++i)
-        if (M.rp[i + 1] - M.rp[i] > 65535) too_long_row = i;             // step counts are 16-bit
+        if (M.rp[i + 1] - M.rp[i] > 65535) too_long_row = i;             // group counts of a slice stay small
     if (too_long_row >= 0) return;
-    const PackPlan pp = plan_stream(nrows, M.rp.data(), s.wide, has_aux, block_bytes, n_real, window);
+    const PackPlan pp = plan_stream(nrows, M.rp.data(), s.wide, has_aux, n_real, window);
     s.bytes = pp.bytes;
-    s.bytes_real = 0;
-    for (int w = 0; w < NUM_WAYS; ++w) {
-        s.way[w] = pp.way[w];
-        const WayDesc& d = pp.way[w];
-        s.bytes_real += d.nblocks_real == d.nblocks ? (d.nblocks ? (i64)(d.nblocks - 1) * block_bytes + 16 * (i64)d.last16 : 0)
-                                                    : (i64)d.nblocks_real * block_bytes;
-    }
+    s.bytes_real = pp.bytes_real;
+    s.padded_nnz = pp.padded_nnz;
+    for (int w = 0; w < NUM_WAYS; ++w) s.way[w] = pp.way[w];
 }
 }  // namespace
 
 CompositeBuilder::CompositeBuilder(const Hierarchy& H, const std::vector<i32>& owner,
-                                   const std::vector<std::vector<i32>>& owned, int eta, int num_ghost, int block_bytes,
-                                   int window)
-    : H_(H), owner_(owner), owned_(owned), eta_(eta), nghost_(num_ghost), block_bytes_(block_bytes), window_(window) {
+                                   const std::vector<std::vector<i32>>& owned, int eta, int num_ghost, int window)
+    : H_(H), owner_(owner), owned_(owned), eta_(eta), nghost_(num_ghost), window_(window) {
     const int nl = H.L + 1;
     real_.resize(nl); ghost_.resize(nl); loc_.resize(nl); stamp_.resize(nl);
     A_.resize(nl); P_.resize(nl); R_.resize(nl);
@@ -171,14 +167,14 @@ void CompositeBuilder::plan(int p, SubdomainBlob& out) {
                 R.ci[pos] = i; R.v[pos] = P.v[k];
             }
         i64 bad = -1;
-        layout_stream(A, nb, nb, true, block_bytes_, window_, nr, b.A, bad);
-        layout_stream(P, nb, nbc, false, block_bytes_, window_, nb, b.P, bad);
-        layout_stream(R, nbc, nb, false, block_bytes_, window_, nbc, b.R, bad);
+        layout_stream(A, nb, nb, true, window_, nr, b.A, bad);
+        layout_stream(P, nb, nbc, false, window_, nb, b.P, bad);
+        layout_stream(R, nbc, nb, true, window_, nbc, b.R, bad);
         if (bad >= 0 && out.too_long_row < 0) { out.too_long_row = bad; out.too_long_level = l; }
     }
     // blob layout
     i64 off = 0;
-    auto take = [&](i64 bytes) { const i64 o = off; off = align16(off + bytes); return o; };
+    auto take = [&](i64 bytes) { const i64 o = off; off = (off + bytes + 127) & ~(i64)127; return o; };   // streams need 128-byte alignment
     out.n_owned = (i32)owned_[p].size();
     out.off_owned = take((i64)out.n_owned * 4);
     for (int l = 0; l <= L; ++l) {
@@ -214,27 +210,28 @@ void CompositeBuilder::fill(const SubdomainBlob& plan, char* dst) {
         const i32 nbc = plan.lev[l + 1].n_real + plan.lev[l + 1].n_ghost;
         aux_.assign((size_t)nb, 0.0);                                    // ghost rows never relax (A4)
         for (i32 i = 0; i < nr; ++i) aux_[i] = dinv[i];
-        write_stream(nb, A_[l].rp.data(), A_[l].ci.data(), A_[l].v.data(), aux_.data(), b.A.wide, block_bytes_, nr, window_,
-                     dst + b.A.off);
-        write_stream(nb, P_[l].rp.data(), P_[l].ci.data(), P_[l].v.data(), nullptr, b.P.wide, block_bytes_, nb, window_,
-                     dst + b.P.off);
-        write_stream(nbc, R_[l].rp.data(), R_[l].ci.data(), R_[l].v.data(), nullptr, b.R.wide, block_bytes_, nbc, window_,
-                     dst + b.R.off);
+        write_stream(nb, A_[l].rp.data(), A_[l].ci.data(), A_[l].v.data(), aux_.data(), b.A.wide, nr, window_, dst + b.A.off);
+        write_stream(nb, P_[l].rp.data(), P_[l].ci.data(), P_[l].v.data(), nullptr, b.P.wide, nb, window_, dst + b.P.off);
+        {   // R_l rows are the points of level l+1: aux = their l1 diagonal (real points), 0 on ghosts
+            const BlockLayout& c = plan.lev[l + 1];
+            const HostLevel& lc = H_.lv[l + 1];
+            auxr_.assign((size_t)nbc, 0.0);
+            for (i32 i = 0; i < c.n_real; ++i) auxr_[i] = lc.dinv[real_[l + 1][i]];
+            write_stream(nbc, R_[l].rp.data(), R_[l].ci.data(), R_[l].v.data(), auxr_.data(), b.R.wide, nbc, window_, dst + b.R.off);
+        }
     }
 }
 
-bool pack_global_stream(const HostCsr& M, const double* aux, int block_bytes, int window, PackedLevelStream& out,
-                        i64& too_long_row) {
+bool pack_global_stream(const HostCsr& M, const double* aux, int window, PackedLevelStream& out, i64& too_long_row) {
     if (M.nnz() > (i64)INT32_MAX || M.nrows > (i64)INT32_MAX) return false;
     LocalCsr T;
     T.rp.assign(M.rp.begin(), M.rp.end());
     i64 bad = -1;
-    layout_stream(T, (int)M.nrows, (int)M.ncols, aux != nullptr, block_bytes, window, (int)M.nrows, out.lay, bad);
+    layout_stream(T, (int)M.nrows, (int)M.ncols, aux != nullptr, window, (int)M.nrows, out.lay, bad);
     too_long_row = bad;
     if (bad >= 0) return true;
     out.data.assign((size_t)out.lay.bytes, 0);
-    write_stream((int)M.nrows, T.rp.data(), M.ci.data(), M.v.data(), aux, out.lay.wide, block_bytes, (int)M.nrows, window,
-                 out.data.data());
+    write_stream((int)M.nrows, T.rp.data(), M.ci.data(), M.v.data(), aux, out.lay.wide, (int)M.nrows, window, out.data.data());
     return true;
 }
 

@@ -3,293 +3,145 @@
 // One CTA per SM takes whole subdomains from a work counter and runs ALL num_fac_cycles AlgFAC
 // V(nu,nu)-cycles of a subdomain start to finish; subdomains never communicate.
 //
-// Every warp is a consumer AND its own producer.  A matrix is stored as NUM_WAYS independent
-// sub-streams (amgdd_stream.hpp); warp w owns way w of every matrix: it streams the blocks of its
-// way HBM -> its PRIVATE shared-memory ring with cp.async.bulk (TMA, SASS UBLKCP; completion on one
-// mbarrier per ring slot) and consumes them in order.  Matrix data does not depend on computed
-// values, so the warp's issue cursor walks the same static "program" of mat-vecs as its consume
-// cursor, `stages` blocks ahead -- across mat-vec, level and subdomain boundaries -- and the only
-// synchronisation between warps is the CTA barrier between two steps of Alg. 4.
+// MATRIX DATA.  A matrix is stored as NUM_WAYS independent sub-streams of SELL-32 groups
+// (amgdd_stream.hpp); warp w owns way w of every matrix.  It reads its groups with coalesced
+// 128-bit loads (ld.global.nc, L1 no-allocate, L2 evict-first) straight into a RING OF REGISTERS
+// of two blocks of RING_DEPTH groups -- the register file is the staging buffer.  While one block
+// is consumed the other is in flight (one burst of loads per block), and the ring runs ahead of
+// the arithmetic across mat-vec boundaries: the burst after the last block of a mat-vec fetches
+// the first groups of the NEXT mat-vec of the program, so the HBM pipe does not drain at the CTA
+// barrier between two steps of Alg. 4.  All loads of the ring are unconditional (clamped
+// addresses): a predicated asm load forces the compiler to wait for it at once.
 //
-// Inside a block, lane j owns row j of a 32-row slice (slice-JDS layout): it adds the entries of
-// its row in stored (= column) order, so there is no cross-lane reduction and every row sum has
-// one fixed summation order (run-to-run identical results); a row-local epilogue applies the
-// AlgFAC update.  The gather vector of a mat-vec is staged in shared memory.
-// The level vectors u, t, s, f live in a per-CTA workspace slot in global memory that every
-// subdomain of the CTA reuses; what streams from HBM is matrix data, once per mat-vec.
+// ARITHMETIC.  Lane j owns row j of a 32-row slice: it adds the entries of its row in stored
+// (= column) order, so there is no cross-lane reduction and every row sum has one fixed summation
+// order (run-to-run identical results); a row-local epilogue applies the Alg. 4 update.
+//
+// VECTORS.  The gather vector of a mat-vec lives in one of two shared-memory buffers; the epilogue
+// writes the gather vector of the NEXT step into the other (u after interpolation for the
+// relaxation, t for the A t step, w for the restriction, ...), so no step needs a staging pass and
+// there is exactly one CTA barrier per step.  u, t, s, f of all levels are kept in a per-CTA
+// workspace slot in global memory (L2 resident); the epilogue's operands are fetched when a slice
+// starts and used when it ends.
 #include "amgdd_stream.hpp"
 
 #include <cuda_runtime.h>
-
-#include <climits>
 
 namespace amgdd {
 
 namespace {
 
-constexpr int MAX_STAGES = 8;
 constexpr int NTHREADS = 32 * NUM_WAYS;
+constexpr int D = RING_DEPTH;
+constexpr int STAGE_BYTES = 512 + 3 * 256;     // per warp: one slice header + three operand vectors of 32 doubles
 
-enum OpKind { OP_RELAX = 0, OP_AT = 1, OP_RESTRICT = 2, OP_RECALC = 3, OP_INTERP = 4, OP_RELAX_DELTA = 5,
-              OP_FIRST = 6, OP_COARSE = 7, OP_BEGIN = 8, OP_END = 9 };
 // slots of the optional per-CTA cycle counters (FAC_PROF_SLOTS each; amgdd_debug_fac_cycles)
-enum ProfSlot { PROF_SYNC = 0, PROF_WAIT_FULL = 1, PROF_CONSUME = 2, PROF_STAGE = 3, PROF_ISSUE = 4, PROF_BEGIN = 5,
-                PROF_END = 6, PROF_FIRST = 7, PROF_COARSE = 8, PROF_TOTAL = 9, PROF_OP0 = 10 };
+enum ProfSlot { PROF_SYNC = 0, PROF_SETUP = 1, PROF_PRE = 2, PROF_PRIME = 3, PROF_TOTAL = 4, PROF_OP0 = 5 };   // PROF_OP0 + OpKind
 
-// an op of the program: kind | level << 4 | (first AlgFAC iteration) << 12
-__host__ __device__ constexpr unsigned short make_op(int kind, int level, int first) {
-    return (unsigned short)(kind | (level << 4) | (first << 12));
-}
-__device__ __forceinline__ int op_kind(unsigned short op) { return op & 15; }
-__device__ __forceinline__ int op_level(unsigned short op) { return (op >> 4) & 255; }
-__device__ __forceinline__ int op_first(unsigned short op) { return (op >> 12) & 1; }
-
-// The static program of one subdomain: the steps of num_fac_cycles AlgFAC V(nu,nu)-cycles (Alg. 4)
-// in order.  emit(op) is called for each; fac_num_ops() counts with the same routine.
-struct OpSink {                       // counts the ops and, if out != nullptr, stores them
-    unsigned short* out;
-    int n;
-    __host__ __device__ void operator()(unsigned short op) {
-        if (out) out[n] = op;
-        ++n;
-    }
+struct LevInfo {           // shared-memory copy of the scalar part of DevLevel
+    int n_real, n_bar;
+    long long voff;
+    const int* gid;
+    const double* dinv;
 };
-
-__host__ __device__ inline void fac_program(int L, int nfac, int nu, OpSink& emit) {
-    emit(make_op(OP_BEGIN, 0, 0));                                         // Alg. 2, Alg. 4
-    for (int it = 0; it < nfac; ++it) {
-        const int first = it == 0;
-        for (int l = 0; l < L; ++l) {                                      // downsweep P:505-513
-            int sweeps = nu;
-            if (l != 0) { emit(make_op(OP_FIRST, l, first)); --sweeps; }   // u_l = 0, so delta = D^-1 f
-            for (int k = 0; k < sweeps; ++k) emit(make_op(OP_RELAX, l, first));
-            emit(make_op(OP_AT, l, first));                                // P:509  w = s_l + A_l t_l
-            emit(make_op(OP_RESTRICT, l, first));                          // P:509  s_{l+1} = R_l w 
-            if (!first) emit(make_op(OP_RECALC, l, first));                // P:510  (identically zero at it = 0)
-        }
-        emit(make_op(OP_COARSE, L, first));
-        for (int l = L - 1; l >= 0; --l) {                                 // upsweep P:515-519
-            emit(make_op(OP_INTERP, l, first));
-            for (int k = 0; k < nu; ++k) emit(make_op(OP_RELAX, l, first));
-        }
-    }
-    emit(make_op(OP_END, 0, 0));                                           // Alg. 2
-}
-
-struct Ctrl {
-    unsigned long long full[NUM_WAYS][MAX_STAGES];   // ring slot s of warp w holds a complete block
-    unsigned long long tbl_full[2];                  // descriptor table slot q is loaded
-    int sub_id[2];                                   // subdomain whose table sits in slot q (-1: no more work)
+struct WayEnt {            // shared memory: what warp w needs to read stream s
+    const char* grp;
+    const char* hdr;
+    uint32_t n_all, n_real, nsl_all, nsl_real;
 };
-constexpr int CTRL_BYTES = 1152;
-static_assert(sizeof(Ctrl) <= CTRL_BYTES, "control block too large");
+static_assert(sizeof(WayEnt) == 32 && sizeof(LevInfo) == 32, "shared-memory table layout");
 
-// ---- PTX wrappers ---------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t smem_addr(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+struct Grp { uint4 a, b, c; };     // values of steps 0,1 | values of steps 2,3 | column indices (narrow: c.x, c.y)
 
-__device__ __forceinline__ void mbar_init(void* bar, uint32_t count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_addr(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
-    asm volatile("{\n .reg .b64 st;\n mbarrier.arrive.shared::cta.b64 st, [%0];\n}" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
-    asm volatile("{\n .reg .b64 st;\n mbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1;\n}" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
-    uint32_t ok;
-    asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
-                 : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
-    return ok != 0;
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-    while (!mbar_try_wait(bar, parity)) {}
-}
+// ---- loads ------------------------------------------------------------------------------------
 __device__ __forceinline__ uint64_t policy_evict_first() {
     uint64_t pol;
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
     return pol;
 }
-// 1-D bulk async copy global -> shared (TMA), completion counted in bytes on `bar`
-__device__ __forceinline__ void bulk_copy_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar, uint64_t policy) {
-    asm volatile(
-        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(dst),
-        "l"(src), "r"(bytes), "r"(bar), "l"(policy)
-        : "memory");
+__device__ __forceinline__ uint4 ldg_stream128(const void* p, uint64_t pol) {
+    uint4 v;
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v4.u32 {%0,%1,%2,%3}, [%4], %5;"
+                 : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p), "l"(pol));
+    return v;
 }
-__device__ __forceinline__ void bulk_copy_g2s_plain(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src),
-                 "r"(bytes), "r"(bar)
-                 : "memory");
+__device__ __forceinline__ uint2 ldg_stream64(const void* p, uint64_t pol) {
+    uint2 v;
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v2.u32 {%0,%1}, [%2], %3;" : "=r"(v.x), "=r"(v.y) : "l"(p), "l"(pol));
+    return v;
 }
-// orders this thread's earlier generic-proxy accesses to shared memory before later async-proxy ones
-__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-
-// shared-memory loads by 32-bit shared address (no generic-address arithmetic in the inner loop)
+template <bool WIDE>
+__device__ __forceinline__ Grp load_grp(const char* p, int lane, uint64_t pol) {
+    Grp g;
+    g.a = ldg_stream128(p + 16 * lane, pol);
+    g.b = ldg_stream128(p + 512 + 16 * lane, pol);
+    if (WIDE) g.c = ldg_stream128(p + 1024 + 16 * lane, pol);
+    else { const uint2 t = ldg_stream64(p + 1024 + 8 * lane, pol); g.c.x = t.x; g.c.y = t.y; g.c.z = 0; g.c.w = 0; }
+    return g;
+}
+// asynchronous copies global -> shared (LDGSTS): they complete on their own scoreboard
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async8(uint32_t dst, const void* src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+__device__ __forceinline__ uint4 lds128(uint32_t a) {
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a));
+    return v;
+}
 __device__ __forceinline__ double lds_f64(uint32_t a) {
     double v;
     asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a));
     return v;
 }
-__device__ __forceinline__ uint32_t lds_u16(uint32_t a) {
-    unsigned short v;
-    asm volatile("ld.shared.u16 %0, [%1];" : "=h"(v) : "r"(a));
-    return v;
-}
-__device__ __forceinline__ uint32_t lds_u32(uint32_t a) {
-    uint32_t v;
-    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a));
-    return v;
-}
-__device__ __forceinline__ uint4 lds_v4(uint32_t a) {
-    uint4 v;
-    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a));
-    return v;
-}
-// the gather vector: staged in shared memory, or read from the workspace (global memory)
-struct SmemVec {
-    uint32_t base;
-    __device__ __forceinline__ double at(uint32_t c) const { return lds_f64(base + (c << 3)); }
-};
-struct GlobalVec {
-    const double* base;
-    __device__ __forceinline__ double at(uint32_t c) const { return base[c]; }
-};
+__device__ __forceinline__ double mkdouble(uint32_t lo, uint32_t hi) { return __hiloint2double((int)hi, (int)lo); }
 
-// What a row does with its finished sum (the Alg. 4 step of the mat-vec); the pointers index the
-// level vectors in this CTA's workspace slot.
-struct Epilogue {
-    int kind;              // OpKind
-    int limit;             // OP_RESTRICT: rows below this are real rows of level l+1
-    int first;             // OP_RESTRICT: first AlgFAC iteration
-    double* a;             // RELAX u | AT w | RESTRICT s_{l+1} | RECALC f_{l+1} | INTERP u | RELAX_DELTA delta
-    double* b;             // RELAX t | RESTRICT f_{l+1}
-    const double* c;       // RELAX f | AT s | RECALC s_{l+1} | RELAX_DELTA f
-};
-
-__device__ __forceinline__ void apply(const Epilogue& ep, int i, double sum, double aux) {
-    switch (ep.kind) {
-        case OP_RELAX: {                   // one l1-Jacobi update (§4.1); aux = 1 / sum_j |a_ij| (S8)
-            const double dl = aux * (ep.c[i] - sum);
-            ep.a[i] += dl;
-            ep.b[i] += dl;
-            break;
-        }
-        case OP_RELAX_DELTA: ep.a[i] = aux * (ep.c[i] - sum); break;
-        case OP_AT: ep.a[i] = ep.c[i] + sum; break;                        // P:509 w = s_l + A_l t_l
-        case OP_RESTRICT:                                                  // P:509 s_{l+1} = R_l w ; P:511 (first iteration)
-            ep.a[i] = sum;
-            if (ep.first && i < ep.limit) ep.b[i] -= sum;
-            break;
-        case OP_RECALC: ep.a[i] = (ep.a[i] - sum) - ep.c[i]; break;
-        default: ep.a[i] += sum; break;                                    // OP_INTERP
+// the two vector buffers: shared memory (XS) or the workspace slot
+template <bool XS> struct XBuf;
+template <> struct XBuf<true> {
+    uint32_t a;
+    __device__ __forceinline__ double ld(uint32_t i) const {
+        double v;
+        asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a + (i << 3)));
+        return v;
     }
-}
-
-// What a warp carries from piece to piece of the slice it is working on (a slice may span blocks).
-struct SliceState {
-    double acc, aux;
-    int row;               // row of this lane, -1: none
-    int len;               // entries of that row
-    int slices_left;       // slices still to finish in this mat-vec (real-rows-only mat-vecs stop early)
+    __device__ __forceinline__ void st(uint32_t i, double v) const { asm volatile("st.shared.f64 [%0], %1;" ::"r"(a + (i << 3)), "d"(v) : "memory"); }
+};
+template <> struct XBuf<false> {
+    double* p;
+    __device__ __forceinline__ double ld(uint32_t i) const { return p[i]; }
+    __device__ __forceinline__ void st(uint32_t i, double v) const { p[i] = v; }
 };
 
-// One block in shared memory (layout: amgdd_stream.hpp), `blk` = its shared address.  Lane j owns
-// row j of the slice and adds its entries in stored (= column) order.  Lanes whose row has ended
-// re-read entry 0 of the piece and discard it: every load is unconditional, so the four steps of
-// an unrolled block overlap.
-template <bool WIDE, class X>
-__device__ __forceinline__ void consume_block(uint32_t blk, X xs, int has_aux, SliceState& st, const Epilogue& ep) {
-    constexpr int CS = WIDE ? 2 : 1;                               // log2 bytes per column index
-    const int np = (int)lds_u32(blk);
-    const int lane = threadIdx.x & 31;
-    for (int i = 0; i < np && st.slices_left > 0; ++i) {
-        const uint4 raw = lds_v4(blk + BLOCK_HEADER_BYTES + i * PIECE_DESC_BYTES);
-        const int k0 = (int)(raw.z & 0xFFFFu), nk = (int)(raw.z >> 16), K = (int)(raw.w & 0xFFFFu), nnz = (int)(raw.w >> 16);
-        uint32_t q = blk + raw.x;
-        if (k0 == 0) {
-            const int rid = (int)lds_u16(q + 2 * lane);
-            st.len = (int)lds_u16(q + 2 * (SLICE_ROWS + lane));
-            st.row = rid == (int)NO_ROW ? -1 : (int)raw.y + rid;
-            st.acc = 0.0;
-            q += SLICE_ROWS * 4;
-            if (has_aux) { st.aux = lds_f64(q + 8 * lane); q += SLICE_ROWS * 8; }
-        }
-        const uint32_t vb = q, cb = q + (uint32_t)nnz * 8;
-        uint32_t e = (uint32_t)lane;
-        double acc = st.acc;
-        const int len = st.len;
-        int k = k0;
-        const int kend = k0 + nk;
-        auto col = [&](uint32_t ee) { return WIDE ? lds_u32(cb + (ee << CS)) : lds_u16(cb + (ee << CS)); };
-        for (; k + 4 <= kend; k += 4) {
-            const bool a0 = k < len, a1 = k + 1 < len, a2 = k + 2 < len, a3 = k + 3 < len;
-            const uint32_t e0 = e;
-            const uint32_t e1 = e0 + __popc(__ballot_sync(0xffffffffu, a0));
-            const uint32_t e2 = e1 + __popc(__ballot_sync(0xffffffffu, a1));
-            const uint32_t e3 = e2 + __popc(__ballot_sync(0xffffffffu, a2));
-            e = e3 + __popc(__ballot_sync(0xffffffffu, a3));
-            const uint32_t f0 = a0 ? e0 : 0u, f1 = a1 ? e1 : 0u, f2 = a2 ? e2 : 0u, f3 = a3 ? e3 : 0u;
-            const uint32_t c0 = col(f0), c1 = col(f1), c2 = col(f2), c3 = col(f3);
-            const double v0 = lds_f64(vb + (f0 << 3)), v1 = lds_f64(vb + (f1 << 3));
-            const double v2 = lds_f64(vb + (f2 << 3)), v3 = lds_f64(vb + (f3 << 3));
-            const double x0 = xs.at(c0), x1 = xs.at(c1), x2 = xs.at(c2), x3 = xs.at(c3);
-            if (a0) acc = fma(v0, x0, acc);
-            if (a1) acc = fma(v1, x1, acc);
-            if (a2) acc = fma(v2, x2, acc);
-            if (a3) acc = fma(v3, x3, acc);
-        }
-        for (; k < kend; ++k) {
-            const bool a0 = k < len;
-            const uint32_t cnt = __popc(__ballot_sync(0xffffffffu, a0));
-            const uint32_t f0 = a0 ? e : 0u;
-            const double v0 = lds_f64(vb + (f0 << 3));
-            const double x0 = xs.at(col(f0));
-            if (a0) acc = fma(v0, x0, acc);
-            e += cnt;
-        }
-        st.acc = acc;
-        if (kend != K) break;                                   // the slice continues in the next block
-        if (st.row >= 0) apply(ep, st.row, acc, st.aux);
-        --st.slices_left;
-    }
+__device__ __forceinline__ int stream_of(const FacOp& op) {           // 3 * level + {0: A, 1: P, 2: R}
+    const int which = op.kind == OPK_INTERP ? 1 : op.kind == OPK_RESTRICT ? 2 : 0;
+    return 3 * op.level + which;
 }
+__device__ __forceinline__ bool real_rows_only(const FacOp& op) { return op.kind == OPK_RELAX || op.kind == OPK_RECALC; }
+__device__ __forceinline__ bool is_matvec(int kind) { return kind >= OPK_RELAX && kind <= OPK_INTERP; }
 
-// which packed stream a mat-vec reads, and whether it stops after the real rows
-__device__ __forceinline__ const StreamDesc* stream_of(const DevLevel* T, int kind, int l, bool& real_only) {
-    real_only = (kind == OP_RELAX || kind == OP_RECALC);
-    if (kind == OP_RELAX || kind == OP_AT) return &T[l].A;
-    if (kind == OP_RESTRICT) return &T[l].R;
-    if (kind == OP_RECALC) return &T[l + 1].A;
-    return &T[l].P;
-}
-
-template <bool PROF>
+template <bool XS, bool PROF>
 struct Worker {
-    // ---- constants of the launch ----
     const FacParams* prm;
-    Ctrl* ctrl;
-    const unsigned short* ops;     // the program (shared memory)
-    unsigned char* tbl_base;       // two descriptor-table slots (shared memory)
-    double* xbuf;                  // shared-memory gather buffer, x_cap doubles
-    uint32_t x_addr, ring_addr, bar_addr, tbl_bar_addr;   // shared addresses: xbuf, this warp's ring, its barriers, tbl_full[0]
+    const FacOp* ops;              // shared memory
+    const LevInfo* lev;            // shared memory, L+1
+    const WayEnt* wt;              // shared memory, [stream][way]
+    const uint32_t* sflags;        // shared memory, per stream
+    XBuf<XS> xb0, xb1;
+    __device__ __forceinline__ XBuf<XS> xbuf_of(int b) const { return b ? xb1 : xb0; }
     double* ws;                    // this CTA's workspace slot
-    double* w;                     // scratch vector inside the slot
-    long long* prof;               // this CTA's cycle counters (PROF only)
-    uint64_t policy;
-    int nops, stages, block_bytes, x_cap;
-    int tid, lane, wid;
-    // ---- consume cursor ----
-    const DevLevel* lev;           // table of the current subdomain
-    int ksub;                      // sequence number of the current subdomain of this CTA
-    int cslot;
-    uint32_t cphase;
-    int inflight;                  // blocks issued and not yet consumed (<= stages)
-    // ---- issue cursor: runs ahead of the consume cursor through the same program ----
-    int iksub, iop, islot;
-    uint32_t iblk, inb, itail, ilast;
-    const char* isrc;
-    bool idone;
+    long long* prof;
+    uint64_t pol;
+    int tid, lane, wid, L;
+    // ring state carried from mat-vec to mat-vec
+    Grp ra[D], rb[D];              // two blocks of D groups; `phase` tells which one holds the coming block
+    int phase;
+    bool ring_valid;               // the ring holds the first groups of the coming mat-vec
+    bool hdr_ready;                // the staging area holds (or is receiving) the header of its slice 0
+    uint32_t stage;                // shared address of this warp's staging area (STAGE_BYTES)
 
     __device__ __forceinline__ long long tick() const { return PROF ? clock64() : 0; }
     __device__ __forceinline__ void tock(int idx, long long t0) const { if (PROF && tid == 0) prof[idx] += clock64() - t0; }
@@ -298,62 +150,13 @@ struct Worker {
         __syncthreads();
         tock(PROF_SYNC, t0);
     }
-    __device__ __forceinline__ const DevLevel* table(int q) const { return reinterpret_cast<const DevLevel*>(tbl_base + (size_t)q * prm->table_bytes); }
     __device__ __forceinline__ double* U(int l) const { return ws + lev[l].voff; }
     __device__ __forceinline__ double* T(int l) const { return ws + lev[l].voff + lev[l].n_bar; }
     __device__ __forceinline__ double* S(int l) const { return ws + lev[l].voff + 2 * (size_t)lev[l].n_bar; }
     __device__ __forceinline__ double* F(int l) const { return ws + lev[l].voff + 3 * (size_t)lev[l].n_bar; }
 
-    // Issue the next block of this warp's way (if the ring has room the caller checked).  Returns
-    // false when there is nothing to issue: no more work, or the cursor would run two subdomains ahead.
-    __device__ __forceinline__ bool issue_one() {
-        while (iblk >= inb) {
-            if (idone) return false;
-            if (iop + 1 >= nops) {                                       // the program of subdomain iksub is issued
-                if (iksub > ksub) return false;
-                const int nk = iksub + 1, nq = nk & 1;
-                mbar_wait(tbl_bar_addr + 8 * nq, (uint32_t)(nk >> 1) & 1u);
-                if (ctrl->sub_id[nq] < 0) { idone = true; return false; }
-                iksub = nk;
-                iop = -1;
-            }
-            ++iop;
-            const unsigned short op = ops[iop];
-            const int kind = op_kind(op);
-            iblk = inb = 0;
-            if (kind <= OP_INTERP) {
-                bool real_only;
-                const StreamDesc* sd = stream_of(table(iksub & 1), kind, op_level(op), real_only);
-                const WayDesc wd = sd->way[wid];
-                inb = real_only ? wd.nblocks_real : wd.nblocks;
-                isrc = sd->base + 16ull * wd.off16;
-                itail = wd.nblocks - 1u;
-                ilast = 16u * wd.last16;
-            }
-        }
-        if (lane == 0) {
-            const uint32_t bytes = (iblk == itail) ? ilast : (uint32_t)block_bytes;
-            const uint32_t bar = bar_addr + 8 * islot;
-            fence_proxy_async();
-            mbar_arrive_expect_tx(bar, bytes);
-            bulk_copy_g2s(ring_addr + (uint32_t)islot * (uint32_t)block_bytes, isrc, bytes, bar, policy);
-        }
-        isrc += block_bytes;
-        ++iblk;
-        ++inflight;
-        if (++islot == stages) islot = 0;
-        return true;
-    }
-    __device__ __forceinline__ void top_up() {
-        const long long t0 = tick();
-        while (inflight < stages && issue_one()) {}
-        tock(PROF_ISSUE, t0);
-    }
-
     // ---- Alg. 2 P:475 + Alg. 4: f_l = r_l on D_l ; u = t = s = 0 ----
     __device__ __forceinline__ void begin_subdomain() {
-        const long long tp0 = tick();
-        const int L = prm->L;
         for (int l = 0; l <= L; ++l) {
             const int n_real = lev[l].n_real, n_bar = lev[l].n_bar;
             const int* gid = lev[l].gid;
@@ -361,13 +164,11 @@ struct Worker {
             double* u = U(l);
             for (int i = tid; i < 3 * n_bar; i += NTHREADS) u[i] = 0.0;   // u | t | s are adjacent
             double* f = F(l);
-            for (int i = tid; i < n_real; i += NTHREADS) f[i] = r[__ldg(gid + i)];
+            for (int i = tid; i < n_real; i += NTHREADS) f[i] = __ldg(r + __ldg(gid + i));
         }
-        tock(PROF_BEGIN, tp0);
     }
     // ---- Alg. 2: x <- x + u_0^p on Omega_0^p (disjoint targets across subdomains) ----
     __device__ __forceinline__ void end_subdomain(int p) {
-        const long long tp0 = tick();
         const DevSub sb = prm->sub[p];
         const double* u0 = U(0);
         const int* gid0 = lev[0].gid;
@@ -375,263 +176,419 @@ struct Worker {
             const int li = __ldg(sb.owned + k);
             prm->x[__ldg(gid0 + li)] += u0[li];
         }
-        tock(PROF_END, tp0);
     }
-    // P:506 u_l <- 0, then the first sweep needs no matrix: delta = D^{-1} f
-    __device__ __forceinline__ void first_sweep(int l) {
-        const long long tp0 = tick();
-        const int n_real = lev[l].n_real, n_bar = lev[l].n_bar;
-        const double* dinv = lev[l].dinv;
-        double *u = U(l), *t = T(l);
-        const double* f = F(l);
+    // level 0, first iteration: u_0 = 0, so the first sweep is delta = D^{-1} f (P:507 with A u = 0)
+    __device__ __forceinline__ void first0(const FacOp op) {
+        const XBuf<XS> xo = xbuf_of(op.gbuf ^ 1);
+        const int n_real = lev[0].n_real, n_bar = lev[0].n_bar;
+        const double* dinv = lev[0].dinv;
+        double *u = U(0), *t = T(0);
+        const double* f = F(0);
         for (int i = tid; i < n_bar; i += NTHREADS) {
             double dl = 0.0;
-            if (i < n_real) { dl = __ldg(dinv + i) * f[i]; t[i] += dl; }
-            u[i] = dl;
+            if (i < n_real) { dl = __ldg(dinv + i) * f[i]; u[i] = dl; t[i] += dl; }
+            xo.st(i, dl);
         }
-        tock(PROF_FIRST, tp0);
     }
     // u_L = A_L^{-1} f_L with the LU factors computed at setup (Alg. 4).  One warp; columns
-    // of the unit-lower / upper factors are contiguous (column-major).
-    __device__ __forceinline__ void coarse() {
-        const long long tp0 = tick();
-        const int L = prm->L, n = prm->nL;
+    // of the unit-lower / upper factors are contiguous (column-major).  The solve runs in place in
+    // the output vector buffer.
+    __device__ __forceinline__ void coarse(const FacOp op) {
+        const XBuf<XS> y = xbuf_of(op.gbuf ^ 1);
+        const int n = prm->nL;
         const double* __restrict__ lu = prm->lu;
         const double* f = F(L);
-        double* y = (n <= x_cap) ? xbuf : w;
-        for (int i = tid; i < n; i += NTHREADS) y[i] = f[__ldg(prm->rowperm + i)];
+        for (int i = tid; i < n; i += NTHREADS) y.st(i, f[__ldg(prm->rowperm + i)]);
         sync();
         if (wid == 0) {
             for (int c = 0; c < n; ++c) {                      // forward: L y = P f
-                const double yc = y[c];
-                for (int i = c + 1 + lane; i < n; i += 32) y[i] -= __ldg(lu + (size_t)c * n + i) * yc;
+                const double yc = y.ld(c);
+                for (int i = c + 1 + lane; i < n; i += 32) y.st(i, y.ld(i) - __ldg(lu + (size_t)c * n + i) * yc);
                 __syncwarp();
             }
             for (int c = n - 1; c >= 0; --c) {                 // backward: U u = y
-                if (lane == 0) y[c] = y[c] / __ldg(lu + (size_t)c * n + c);
+                if (lane == 0) y.st(c, y.ld(c) / __ldg(lu + (size_t)c * n + c));
                 __syncwarp();
-                const double yc = y[c];
-                for (int i = lane; i < c; i += 32) y[i] -= __ldg(lu + (size_t)c * n + i) * yc;
+                const double yc = y.ld(c);
+                for (int i = lane; i < c; i += 32) y.st(i, y.ld(i) - __ldg(lu + (size_t)c * n + i) * yc);
                 __syncwarp();
             }
         }
         sync();
         double* uL = U(L);
-        for (int i = tid; i < n; i += NTHREADS) uL[i] = y[i];
-        tock(PROF_COARSE, tp0);
+        for (int i = tid; i < n; i += NTHREADS) uL[i] = y.ld(i);
     }
 
-    // one mat-vec: the blocks of this warp's way, in order; `staged`: the gather vector is in xbuf
-    __device__ __forceinline__ void run_blocks(const StreamDesc* sd, bool real_only, bool staged, const double* xg, const Epilogue& ep) {
-        const WayDesc wd = sd->way[wid];
-        const uint32_t nb = real_only ? wd.nblocks_real : wd.nblocks;
-        const int has_aux = sd->has_aux, wide = sd->wide;
-        SliceState st;
-        st.acc = 0.0; st.aux = 0.0; st.row = -1; st.len = 0;
-        st.slices_left = real_only ? (int)wd.nslices_real : INT_MAX;
-        for (uint32_t b = 0; b < nb; ++b) {
-            top_up();                                                    // the block waited for below is issued now
-            const long long t0 = tick();
-            mbar_wait(bar_addr + 8 * cslot, cphase);
-            tock(PROF_WAIT_FULL, t0);
-            const long long t1 = tick();
-            const uint32_t blk = ring_addr + (uint32_t)cslot * (uint32_t)block_bytes;
-            if (staged) {
-                SmemVec xs;
-                xs.base = x_addr;
-                consume_block<false>(blk, xs, has_aux, st, ep);
-            } else {
-                GlobalVec xs;
-                xs.base = xg;
-                if (wide) consume_block<true>(blk, xs, has_aux, st, ep);
-                else consume_block<false>(blk, xs, has_aux, st, ep);
-            }
-            __syncwarp();
-            tock(PROF_CONSUME, t1);
-            --inflight;
-            if (++cslot == stages) { cslot = 0; cphase ^= 1u; }
-        }
-        top_up();
-    }
-
-    // stage the gather vector of the next mat-vec in shared memory (if it fits; wide streams never do)
-    __device__ __forceinline__ bool stage_x(const double* x, int n) {
-        if (n > x_cap) return false;
-        const long long t0 = tick();
-        for (int i = tid; i < n; i += NTHREADS) xbuf[i] = x[i];
-        tock(PROF_STAGE, t0);
-        return true;
-    }
-
-    __device__ __forceinline__ void matvec(int K, int l, int first) {
-        const long long top0 = tick();
-        Epilogue ep;
-        ep.kind = K; ep.limit = 0; ep.first = 0; ep.a = nullptr; ep.b = nullptr; ep.c = nullptr;
-        bool real_only;
-        const StreamDesc* sd = stream_of(lev, K, l, real_only);
-        if (K == OP_RELAX) {
-            // one l1-Jacobi sweep on the real points (§4.1): delta from the OLD u
-            // (the staged copy), then u += delta, t += delta (P:507-508 / P:517-518)
+    // work of a step that is not row-local to the mat-vec's rows (all threads; touches only data
+    // that neither the gathers nor the epilogues of THIS step use, so no barrier follows it)
+    __device__ __forceinline__ void pre_actions(const FacOp op) {
+        const XBuf<XS> xg = xbuf_of(op.gbuf), xo = xbuf_of(op.gbuf ^ 1);
+        const int l = op.level;
+        if (op.kind == OPK_RELAX) {                 // ghost values are fixed (A4): carry them (u) or clear them (t)
+            const int n_real = lev[l].n_real, n_bar = lev[l].n_bar;
+            if (op.flags & OPF_TSMEM) { for (int i = n_real + tid; i < n_bar; i += NTHREADS) xo.st(i, 0.0); }
+            else { for (int i = n_real + tid; i < n_bar; i += NTHREADS) xo.st(i, xg.ld(i)); }
+        } else if (op.kind == OPK_AT) {             // P:512 t_l <- 0 (its values are in the gather buffer)
+            double* t = T(l);
             const int n_real = lev[l].n_real;
-            double *u = U(l), *t = T(l);
-            const bool staged = stage_x(u, lev[l].n_bar);
-            sync();
-            ep.c = F(l);
-            if (staged) {
-                ep.a = u; ep.b = t;
-                run_blocks(sd, true, true, u, ep);
-            } else {                                                     // gather from global: two passes
-                double* delta = w;
-                ep.kind = OP_RELAX_DELTA; ep.a = delta;
-                run_blocks(sd, true, false, u, ep);
-                sync();
-                for (int i = tid; i < n_real; i += NTHREADS) {
-                    const double dl = delta[i];
-                    u[i] += dl;
-                    t[i] += dl;
+            for (int i = tid; i < n_real; i += NTHREADS) t[i] = 0.0;
+        } else if (op.kind == OPK_RESTRICT) {       // later iterations: stage u_{l+1} for the recalculation that follows
+            if (!(op.flags & OPF_FIRST)) {
+                const double* uc = U(l + 1);
+                const int nbc = lev[l + 1].n_bar;
+                for (int i = tid; i < nbc; i += NTHREADS) xo.st(i, uc[i]);
+            }
+        } else if (op.kind == OPK_RECALC) {         // P:506 u_{l+1} <- 0 on the ghost points too
+            if (!(op.flags & OPF_COARSEST)) {
+                const int n_real = lev[l].n_real, n_bar = lev[l].n_bar;
+                double* u = U(l);
+                for (int i = n_real + tid; i < n_bar; i += NTHREADS) { xo.st(i, 0.0); u[i] = 0.0; }
+            }
+        }
+    }
+
+    // one mat-vec of the program: the groups of this warp's way, in order
+    template <bool WIDE>
+    __device__ __forceinline__ void matvec(const FacOp op) {
+        constexpr int GB = WIDE ? GROUP_BYTES_WIDE : GROUP_BYTES_NARROW;
+        const long long tp0 = tick();
+        const int kind = op.kind, l = op.level;
+        const bool first = op.flags & OPF_FIRST, tsmem = op.flags & OPF_TSMEM, coarsest = op.flags & OPF_COARSEST;
+        const XBuf<XS> xg = xbuf_of(op.gbuf), xo = xbuf_of(op.gbuf ^ 1);
+        // ---- this warp's way of the stream, and of the next mat-vec's stream ----
+        const WayEnt we = wt[stream_of(op) * NUM_WAYS + wid];
+        const bool ronly = real_rows_only(op);
+        const int n = (int)(ronly ? we.n_real : we.n_all);
+        const int nsl = (int)(ronly ? we.nsl_real : we.nsl_all);
+        const char* const cur = we.grp;
+        const char* const dummy = reinterpret_cast<const char*>(prm->lev);     // always readable (>= 1536 bytes)
+        const char* nxt = dummy;
+        const char* nxt_hdr = dummy;
+        int n_next = 0;
+        if (XS && op.next_mat >= 0) {
+            const FacOp nop = ops[op.next_mat];
+            const WayEnt w2 = wt[stream_of(nop) * NUM_WAYS + wid];
+            n_next = (int)(real_rows_only(nop) ? w2.n_real : w2.n_all);
+            if (n_next > 0) { nxt = w2.grp; nxt_hdr = w2.hdr; }
+        }
+        const int next_last = n_next > 0 ? n_next - 1 : 0;
+        // ---- groups of this mat-vec that are not in the ring yet (first mat-vec of a subdomain, or after a short one) ----
+        if (!ring_valid && n > 0) {
+            if (phase == 0) {
+#pragma unroll
+                for (int d = 0; d < D; ++d) ra[d] = load_grp<WIDE>(cur + (long long)(d < n - 1 ? d : n - 1) * GB, lane, pol);
+            } else {
+#pragma unroll
+                for (int d = 0; d < D; ++d) rb[d] = load_grp<WIDE>(cur + (long long)(d < n - 1 ? d : n - 1) * GB, lane, pol);
+            }
+        }
+        // ---- the row-local operands of the epilogue (level vectors in the workspace slot) ----
+        double* pu = nullptr; double* pt = nullptr; double* ps = nullptr; double* pf = nullptr;
+        const double *cA = nullptr, *cB = nullptr, *cC = nullptr;
+        int nr = 0;                                                          // real rows of the epilogue's level
+        if (kind == OPK_RELAX) { pu = U(l); pt = T(l); cA = F(l); cB = pt; }
+        else if (kind == OPK_AT) { cA = S(l); }
+        else if (kind == OPK_RESTRICT) {
+            ps = S(l + 1); nr = lev[l + 1].n_real;
+            if (first) { pf = F(l + 1); pu = U(l + 1); pt = T(l + 1); cA = pf; cB = pt; }
+        } else if (kind == OPK_RECALC) { pf = F(l); pu = U(l); pt = T(l); cA = pf; cB = S(l); cC = pt; }
+        else { pu = U(l); cA = pu; nr = lev[l].n_real; }
+        // ---- slice bookkeeping ----
+        // The header of a slice and the row-local operands of its epilogue reach the warp through a
+        // small lane-private staging area in shared memory, filled by cp.async one slice ahead:
+        // asynchronous copies complete on their own scoreboard, so waiting for them does not wait
+        // for the ring's loads in flight (all ordinary global loads of a warp share one).
+        //   stage:  H  32 x 16 bytes  header of the next slice (after the last slice: slice 0 of the next mat-vec)
+        //           C  3 x 32 x 8 bytes  operands e0 | e1 | e2 of the current slice's epilogue
+        if (n == 0) { ring_valid = false; hdr_ready = false; tock(PROF_OP0 + kind, tp0); return; }
+        const char* const hdr = we.hdr + 16 * lane;
+        const uint32_t stH = stage + 16 * lane, stC = stage + 512 + 8 * lane;
+        const char* const hdr_after = nxt_hdr + 16 * lane;
+        auto fetch_ctx = [&](uint32_t r) {
+            if (r != NO_ROW) {
+                if (cA) cp_async8(stC, cA + r);
+                if (cB) cp_async8(stC + 256, cB + r);
+                if (cC) cp_async8(stC + 512, cC + r);
+            }
+        };
+        if (!hdr_ready) { cp_async_wait_all(); cp_async16(stH, hdr); }       // (never two copies in flight to one slot)
+        cp_async_wait_all();
+        uint4 h = lds128(stH);
+        uint32_t row = h.x;
+        int left = (int)h.y;
+        double aux = mkdouble(h.z, h.w);
+        fetch_ctx(row);
+        cp_async16(stH, nsl > 1 ? hdr + HEADER_BYTES : hdr_after);
+        hdr_ready = n_next > 0;
+        int sidx = 0;
+        double acc = 0.0;
+        auto consume = [&](const Grp& g) {
+            uint32_t c0, c1, c2, c3;
+            if (WIDE) { c0 = g.c.x; c1 = g.c.y; c2 = g.c.z; c3 = g.c.w; }
+            else { c0 = g.c.x & 0xffffu; c1 = g.c.x >> 16; c2 = g.c.y & 0xffffu; c3 = g.c.y >> 16; }
+#ifdef AMGDD_EXP_NOGATHER
+            const double x0 = __hiloint2double(c0, c1), x1 = __hiloint2double(c1, c2), x2 = __hiloint2double(c2, c3), x3 = __hiloint2double(c3, c0);
+#else
+            const double x0 = xg.ld(c0), x1 = xg.ld(c1), x2 = xg.ld(c2), x3 = xg.ld(c3);
+#endif
+            acc = fma(mkdouble(g.a.x, g.a.y), x0, acc);
+            acc = fma(mkdouble(g.a.z, g.a.w), x1, acc);
+            acc = fma(mkdouble(g.b.x, g.b.y), x2, acc);
+            acc = fma(mkdouble(g.b.z, g.b.w), x3, acc);
+        };
+        auto slice_end = [&]() {
+            cp_async_wait_all();
+#ifdef AMGDD_EXP_NOEPI
+            if (row == 0x7ffffff0u) {
+#else
+            if (row != NO_ROW) {
+#endif
+                const double e0 = lds_f64(stC), e1 = lds_f64(stC + 256), e2 = lds_f64(stC + 512);   // unused ones are stale, never read
+                if (kind == OPK_RELAX) {           // one l1-Jacobi update (§4.1); aux = 1 / sum_j |a_ij| (S8)
+                    const double dl = aux * (e0 - acc);
+                    const double un = xg.ld(row) + dl, tn = e1 + dl;
+                    pu[row] = un; pt[row] = tn;
+                    xo.st(row, tsmem ? tn : un);
+                } else if (kind == OPK_AT) {       // P:509 w = s_l + A_l t_l
+                    xo.st(row, e0 + acc);
+                } else if (kind == OPK_RESTRICT) { // P:509 s_{l+1} = R_l w
+                    ps[row] = acc;
+                    if (first) {                   // P:511 with A u = 0, then P:506-508 of level l+1: delta = D^-1 f
+                        if ((int)row < nr) {
+                            const double f = e0 - acc;
+                            pf[row] = f;
+                            if (!coarsest) {
+                                const double u = aux * f, tn = e1 + u;
+                                pu[row] = u; pt[row] = tn;
+                                xo.st(row, tsmem ? tn : u);
+                            }
+                        } else if (!coarsest) xo.st(row, 0.0);
+                    }
+                } else if (kind == OPK_RECALC) {   // P:510-511, then P:506-508 of the same level
+                    const double f = (e0 - acc) - e1;
+                    pf[row] = f;
+                    if (!coarsest) {
+                        const double u = aux * f, tn = e2 + u;
+                        pu[row] = u; pt[row] = tn;
+                        xo.st(row, tsmem ? tn : u);
+                    }
+                } else {                           // OPK_INTERP
+                    const double un = e0 + acc;
+                    xo.st(row, un);
+                    if ((int)row >= nr) pu[row] = un;              // ghost values are not relaxed: keep them
                 }
             }
-        } else if (K == OP_AT) {
-            // P:509  w = s_l + A_l t_l on all of D-bar_l (ghost rows: real columns only)
-            const double* t = T(l);
-            const bool staged = stage_x(t, lev[l].n_bar);
-            sync();
-            ep.a = w; ep.c = S(l);
-            run_blocks(sd, false, staged, t, ep);
-        } else if (K == OP_RESTRICT) {
-            // P:509  s_{l+1} = R_l w ; P:512 reset t_l, s_l ; first iteration: P:511 f_{l+1} -= s_{l+1}
-            const int n_bar = lev[l].n_bar;
-            const bool staged = stage_x(w, n_bar);
-            double* t = T(l);
-            for (int i = tid; i < 2 * n_bar; i += NTHREADS) t[i] = 0.0;  // t and s are adjacent
-            sync();
-            ep.a = S(l + 1); ep.b = F(l + 1); ep.limit = lev[l + 1].n_real; ep.first = first;
-            run_blocks(sd, false, staged, w, ep);
-        } else if (K == OP_RECALC) {
-            // P:510-511  f_{l+1} <- f_{l+1} - A_{l+1} u_{l+1} - s_{l+1}  (u_{l+1} of the previous iteration)
-            const double* uc = U(l + 1);
-            const bool staged = stage_x(uc, lev[l + 1].n_bar);
-            sync();
-            ep.a = F(l + 1); ep.c = S(l + 1);
-            run_blocks(sd, true, staged, uc, ep);
-        } else {
-            // P:516  u_l += P_l u_{l+1} on all of D-bar_l (§4.2)
-            const double* uc = U(l + 1);
-            const bool staged = stage_x(uc, lev[l + 1].n_bar);
-            sync();
-            ep.a = U(l);
-            run_blocks(sd, false, staged, uc, ep);
+            ++sidx;
+            acc = 0.0;
+            if (sidx < nsl) {
+                h = lds128(stH);
+                row = h.x; left = (int)h.y; aux = mkdouble(h.z, h.w);
+                fetch_ctx(row);
+                cp_async16(stH, sidx + 1 < nsl ? hdr + (long long)(sidx + 1) * HEADER_BYTES : hdr_after);
+            }
+        };
+        tock(PROF_PRIME, tp0);
+        // Blocks of D groups, double buffered in registers: WAIT for block j (buffer X), then issue
+        // the burst of block j+1 into the other buffer (the next D groups of this mat-vec or, after
+        // its last block, the first D groups of the next mat-vec), then consume block j while
+        // that burst is in flight.  All global loads of a warp share one hardware scoreboard, so
+        // a wait on any of them waits for all: the burst must not be issued before the data of
+        // block j has arrived.  That order is forced by a data dependence: the burst's base
+        // address is selected by a bit pattern of block j's first value that no finite matrix
+        // entry has (Inf/NaN exponent), so the address cannot be formed earlier.
+        auto step = [&](Grp (&X)[D], Grp (&Y)[D], int p0) {
+            const bool more = p0 + D < n;
+            const bool never = (X[0].a.y & 0x7FF00000u) == 0x7FF00000u;
+            const char* rbase = never ? dummy : (more ? cur : nxt);
+            const int r0 = more ? p0 + D : 0, rlast = never ? 0 : (more ? n - 1 : next_last);
+#pragma unroll
+            for (int d = 0; d < D; ++d) Y[d] = load_grp<WIDE>(rbase + (long long)(r0 + d < rlast ? r0 + d : rlast) * GB, lane, pol);
+            if (p0 + D <= n) {
+#pragma unroll
+                for (int d = 0; d < D; ++d) {
+                    consume(X[d]);
+                    if (--left == 0) slice_end();
+                }
+            } else {
+#pragma unroll
+                for (int d = 0; d < D - 1; ++d)
+                    if (p0 + d < n) {
+                        consume(X[d]);
+                        if (--left == 0) slice_end();
+                    }
+            }
+        };
+        int ph = phase;
+        for (int p0 = 0; p0 < n; p0 += D) {
+            if (ph == 0) step(ra, rb, p0);
+            else step(rb, ra, p0);
+            ph ^= 1;
         }
-        tock(PROF_OP0 + K, top0);
+        phase = ph;
+        ring_valid = n_next > 0;
+        tock(PROF_OP0 + kind, tp0);
     }
 };
 
-constexpr int OPS_RESERVE_BYTES = 2048;        // room for the program (2 bytes per op)
-
-template <bool PROF>
+template <bool XS, bool PROF>
 __global__ void __launch_bounds__(NTHREADS, 1) fac_kernel(const FacParams prm) {
     extern __shared__ __align__(128) unsigned char smem[];
-    Ctrl* ctrl = reinterpret_cast<Ctrl*>(smem);
-    unsigned short* ops = reinterpret_cast<unsigned short*>(smem + CTRL_BYTES);
-    unsigned char* tbl = smem + CTRL_BYTES + OPS_RESERVE_BYTES;
-    double* xbuf = reinterpret_cast<double*>(tbl + 2 * (size_t)prm.table_bytes);
-    unsigned char* rings = reinterpret_cast<unsigned char*>(xbuf + prm.x_cap);
-    const int L = prm.L;
-    const uint32_t tbl_exact = (uint32_t)((L + 1) * sizeof(DevLevel));
+    const int L = prm.L, nstreams = 3 * (L + 1);
+    // shared-memory plan (fac_smem_bytes): control | ops | LevInfo | stream flags | way table | staging areas | two vector buffers
+    int* ctrl = reinterpret_cast<int*>(smem);
+    FacOp* ops = reinterpret_cast<FacOp*>(smem + 128);
+    LevInfo* lev = reinterpret_cast<LevInfo*>(smem + 128 + (((size_t)prm.nops * sizeof(FacOp) + 127) & ~(size_t)127));
+    uint32_t* sflags = reinterpret_cast<uint32_t*>(lev + (L + 1));
+    WayEnt* wt = reinterpret_cast<WayEnt*>(reinterpret_cast<unsigned char*>(sflags) + (((size_t)nstreams * 4 + 127) & ~(size_t)127));
+    unsigned char* stage = reinterpret_cast<unsigned char*>(wt + (size_t)nstreams * NUM_WAYS);
+    double* xbuf = reinterpret_cast<double*>(stage + NUM_WAYS * STAGE_BYTES);
 
-    // thread 0: draw the next subdomain for sequence number k and start loading its descriptor table
-    auto load_table = [&](int k) {
-        const int q = k & 1;
-        const int id = atomicAdd(prm.work_counter, 1);
-        const int p = id < prm.num_sub ? prm.order[id] : -1;
-        ctrl->sub_id[q] = p;
-        const uint32_t bar = smem_addr(&ctrl->tbl_full[q]);
-        if (p >= 0) {
-            fence_proxy_async();
-            mbar_arrive_expect_tx(bar, tbl_exact);
-            bulk_copy_g2s_plain(smem_addr(tbl + (size_t)q * prm.table_bytes), prm.lev + (size_t)p * (L + 1), tbl_exact, bar);
-        } else {
-            mbar_arrive(bar);
-        }
-    };
-
-    if (threadIdx.x == 0) {
-        for (int w = 0; w < NUM_WAYS; ++w)
-            for (int s = 0; s < prm.stages; ++s) mbar_init(&ctrl->full[w][s], 1);
-        mbar_init(&ctrl->tbl_full[0], 1);
-        mbar_init(&ctrl->tbl_full[1], 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        OpSink sink = {ops, 0};
-        fac_program(L, prm.nfac, prm.nu, sink);
-        load_table(0);
-        load_table(1);
-    }
-    __syncthreads();
-
-    Worker<PROF> W;
-    W.prm = &prm; W.ctrl = ctrl; W.ops = ops; W.tbl_base = tbl; W.xbuf = xbuf;
-    W.tid = threadIdx.x; W.lane = threadIdx.x & 31; W.wid = threadIdx.x >> 5;
-    W.nops = prm.nops; W.stages = prm.stages; W.block_bytes = prm.block_bytes; W.x_cap = prm.x_cap;
-    W.x_addr = smem_addr(xbuf);
-    W.ring_addr = smem_addr(rings) + (uint32_t)W.wid * (uint32_t)(prm.stages * prm.block_bytes);
-    W.bar_addr = smem_addr(&ctrl->full[W.wid][0]);
-    W.tbl_bar_addr = smem_addr(&ctrl->tbl_full[0]);
+    Worker<XS, PROF> W;
+    W.prm = &prm; W.ops = ops; W.lev = lev; W.wt = wt; W.sflags = sflags;
+    W.tid = threadIdx.x; W.lane = threadIdx.x & 31; W.wid = threadIdx.x >> 5; W.L = L;
     W.ws = prm.workspace + (size_t)blockIdx.x * prm.slot_stride;
-    W.w = W.ws + prm.scratch_off;
+    if constexpr (XS) {
+        W.xb0.a = (uint32_t)__cvta_generic_to_shared(xbuf);
+        W.xb1.a = W.xb0.a + (uint32_t)prm.x_cap * 8u;
+    } else {
+        W.xb0.p = W.ws + prm.xg_off;
+        W.xb1.p = W.xb0.p + (prm.slot_stride - prm.xg_off) / 2;
+    }
     W.prof = PROF ? prm.prof + (size_t)blockIdx.x * FAC_PROF_SLOTS : nullptr;
-    W.policy = policy_evict_first();
-    W.ksub = 0; W.cslot = 0; W.cphase = 0; W.inflight = 0;
-    W.iksub = 0; W.iop = -1; W.islot = 0; W.iblk = 0; W.inb = 0; W.itail = 0; W.ilast = 0; W.isrc = nullptr; W.idone = false;
+    W.pol = policy_evict_first();
+    W.ring_valid = false; W.hdr_ready = false;
+    W.stage = (uint32_t)__cvta_generic_to_shared(stage) + (uint32_t)W.wid * STAGE_BYTES;
+#pragma unroll
+    for (int d = 0; d < D; ++d) W.ra[d].a = W.ra[d].b = W.ra[d].c = W.rb[d].a = W.rb[d].b = W.rb[d].c = make_uint4(0, 0, 0, 0);
+    W.phase = 0;
 
+    for (int j = threadIdx.x; j < prm.nops; j += NTHREADS) ops[j] = prm.ops[j];
     const long long tk0 = W.tick();
     for (;;) {
-        const int q = W.ksub & 1;
-        mbar_wait(W.tbl_bar_addr + 8 * q, (uint32_t)(W.ksub >> 1) & 1u);
-        const int p = ctrl->sub_id[q];
-        if (p < 0) break;
-        W.lev = W.table(q);
-        for (int j = 0; j < W.nops; ++j) {
-            const unsigned short op = ops[j];
-            const int kind = op_kind(op), l = op_level(op);
-            W.sync();                                                    // the previous step is complete
-            if (kind == OP_BEGIN) W.begin_subdomain();
-            else if (kind == OP_FIRST) W.first_sweep(l);
-            else if (kind == OP_COARSE) W.coarse();
-            else if (kind == OP_END) W.end_subdomain(p);
-            else W.matvec(kind, l, op_first(op));
+        const long long ts0 = W.tick();
+        if (threadIdx.x == 0) {
+            const int id = atomicAdd(prm.work_counter, 1);
+            ctrl[0] = id < prm.num_sub ? prm.order[id] : -1;
         }
-        W.sync();                                   // every warp is done with table slot q and with the workspace
-        if (threadIdx.x == 0) load_table(W.ksub + 2);
-        ++W.ksub;
+        __syncthreads();
+        const int p = ctrl[0];
+        if (p < 0) break;
+        const DevLevel* tbl = prm.lev + (size_t)p * (L + 1);
+        for (int l = threadIdx.x; l <= L; l += NTHREADS) {
+            LevInfo li;
+            li.n_real = tbl[l].n_real; li.n_bar = tbl[l].n_bar; li.voff = tbl[l].voff; li.gid = tbl[l].gid; li.dinv = tbl[l].dinv;
+            lev[l] = li;
+        }
+        for (int idx = threadIdx.x; idx < nstreams * NUM_WAYS; idx += NTHREADS) {
+            const int s = idx / NUM_WAYS, w = idx % NUM_WAYS;
+            const StreamDesc* sd = &tbl[s / 3].A + (s % 3);                  // A, P, R are consecutive members
+            const char* base = sd->base;
+            const WayDesc wd = sd->way[w];
+            WayEnt e;
+            e.grp = base + 128ull * wd.grp_off128; e.hdr = base + 128ull * wd.hdr_off128;
+            e.n_all = wd.ngroups; e.n_real = wd.ngroups_real; e.nsl_all = wd.nslices; e.nsl_real = wd.nslices_real;
+            wt[idx] = e;
+            if (w == 0) sflags[s] = sd->flags;
+        }
+        __syncthreads();
+        W.tock(PROF_SETUP, ts0);
+        W.ring_valid = false; W.hdr_ready = false;
+        for (int j = 0; j < prm.nops; ++j) {
+            const FacOp op = ops[j];
+            const long long tp0 = W.tick();
+            if (op.kind == OPK_BEGIN) W.begin_subdomain();
+            else if (op.kind == OPK_FIRST0) W.first0(op);
+            else if (op.kind == OPK_COARSE) W.coarse(op);
+            else if (op.kind == OPK_END) W.end_subdomain(p);
+            else {
+                W.pre_actions(op);
+                W.tock(PROF_PRE, tp0);
+                if (!XS && (sflags[stream_of(op)] & STREAM_WIDE)) W.template matvec<true>(op);
+                else W.template matvec<false>(op);
+            }
+            if (!is_matvec(op.kind)) W.tock(PROF_OP0 + op.kind, tp0);
+            W.sync();                                                    // the step is complete
+        }
     }
     W.tock(PROF_TOTAL, tk0);
 }
 
 }  // namespace
 
-int fac_smem_bytes(int block_bytes, int stages, int x_cap, int table_bytes) {
-    return CTRL_BYTES + OPS_RESERVE_BYTES + 2 * table_bytes + x_cap * 8 + NUM_WAYS * stages * block_bytes;
+// The static program of one subdomain: the steps of num_fac_cycles AlgFAC V(nu,nu)-cycles (Alg. 4)
+// in order, with the shared-memory buffer each mat-vec gathers from (it writes the other one).
+int fac_build_program(int L, int nfac, int nu, FacOp* ops) {
+    int n = 0;
+    auto emit = [&](int kind, int level, int gbuf, int flags) {
+        if (ops && n < MAX_OPS) {
+            FacOp o;
+            o.kind = (uint8_t)kind; o.level = (uint8_t)level; o.gbuf = (uint8_t)gbuf; o.flags = (uint8_t)flags;
+            o.next_mat = -1; o.next_mat2 = -1;
+            ops[n] = o;
+        }
+        ++n;
+    };
+    int cur = 0;                                                             // buffer that holds the live gather vector
+    emit(OPK_BEGIN, 0, 0, 0);                                                // Alg. 2, Alg. 4
+    for (int it = 0; it < nfac; ++it) {
+        const int first = it == 0 ? OPF_FIRST : 0;
+        for (int l = 0; l < L; ++l) {                                        // downsweep P:505-513
+            const int coarsest = (l + 1 == L) ? OPF_COARSEST : 0;
+            int k = 0;
+            if (l == 0 && first) { emit(OPK_FIRST0, 0, cur, first | (nu == 1 ? OPF_TSMEM : 0)); cur ^= 1; k = 1; }
+            if (l != 0) k = 1;                                               // the first sweep was fused into the step before
+            for (; k < nu; ++k) { emit(OPK_RELAX, l, cur, first | (k == nu - 1 ? OPF_TSMEM : 0)); cur ^= 1; }
+            emit(OPK_AT, l, cur, first); cur ^= 1;                           // P:509  w = s_l + A_l t_l
+            const int fl = first | coarsest | (nu == 1 ? OPF_TSMEM : 0);
+            emit(OPK_RESTRICT, l, cur, fl); cur ^= 1;                        // P:509  s_{l+1} = R_l w 
+            if (!first) { emit(OPK_RECALC, l + 1, cur, fl); cur ^= 1; }      // P:510  (identically zero at it = 0)
+        }
+        emit(OPK_COARSE, L, cur, first); cur ^= 1;
+        for (int l = L - 1; l >= 0; --l) {                                   // upsweep P:515-519
+            emit(OPK_INTERP, l, cur, first); cur ^= 1;
+            for (int k = 0; k < nu; ++k) { emit(OPK_RELAX, l, cur, first); cur ^= 1; }
+        }
+    }
+    emit(OPK_END, 0, 0, 0);                                                  // Alg. 2
+    if (ops && n <= MAX_OPS) {
+        int nm = -1, nm2 = -1;
+        for (int j = n - 1; j >= 0; --j) {
+            ops[j].next_mat = (int16_t)nm; ops[j].next_mat2 = (int16_t)nm2;
+            if (ops[j].kind >= OPK_RELAX && ops[j].kind <= OPK_INTERP) { nm2 = nm; nm = j; }
+        }
+    }
+    return n;
 }
 
-int fac_max_stages() { return MAX_STAGES; }
-
-int fac_num_ops(int L, int nfac, int nu) {
-    OpSink sink = {nullptr, 0};
-    fac_program(L, nfac, nu, sink);
-    return sink.n;
+int fac_smem_bytes(int x_cap, int L, int nops) {
+    const int nstreams = 3 * (L + 1);
+    size_t b = 128;
+    b += ((size_t)nops * sizeof(FacOp) + 127) & ~(size_t)127;
+    b += (size_t)(L + 1) * sizeof(LevInfo);
+    b += ((size_t)nstreams * 4 + 127) & ~(size_t)127;
+    b += (size_t)nstreams * NUM_WAYS * sizeof(WayEnt);
+    b += (size_t)NUM_WAYS * STAGE_BYTES;
+    b += 2 * (size_t)x_cap * 8;
+    return (int)b;
 }
-
-int fac_max_ops() { return OPS_RESERVE_BYTES / 2; }
 
 int fac_configure(int /*device*/, int max_smem_optin) {
-    cudaError_t e = cudaFuncSetAttribute(fac_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_optin);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(fac_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_optin);
+    cudaError_t e = cudaFuncSetAttribute(fac_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_optin);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fac_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_optin);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fac_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_optin);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fac_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_optin);
     return e == cudaSuccess ? 0 : (int)e;
 }
 
 void launch_fac(const FacParams& prm, const FacLaunch& cfg, void* stream) {
-    if (prm.prof) fac_kernel<true><<<cfg.grid, cfg.block, cfg.smem_bytes, (cudaStream_t)stream>>>(prm);
-    else fac_kernel<false><<<cfg.grid, cfg.block, cfg.smem_bytes, (cudaStream_t)stream>>>(prm);
+    cudaStream_t st = (cudaStream_t)stream;
+    if (prm.x_cap > 0) {
+        if (prm.prof) fac_kernel<true, true><<<cfg.grid, cfg.block, cfg.smem_bytes, st>>>(prm);
+        else fac_kernel<true, false><<<cfg.grid, cfg.block, cfg.smem_bytes, st>>>(prm);
+    } else {
+        if (prm.prof) fac_kernel<false, true><<<cfg.grid, cfg.block, cfg.smem_bytes, st>>>(prm);
+        else fac_kernel<false, false><<<cfg.grid, cfg.block, cfg.smem_bytes, st>>>(prm);
+    }
 }
 
 }  // namespace amgdd

@@ -78,13 +78,14 @@ void parallel_for(i64 n, int nthreads, i64 chunk, F&& fn) {
 // Where one packed stream (amgdd_stream.hpp) sits inside a blob, and its ways.
 struct StreamLayout {
     i64 off = -1;                // byte offset inside the blob (16-byte aligned)
-    i64 bytes = 0;               // all ways, all blocks
-    i64 bytes_real = 0;          // bytes of the blocks that hold the first group (what a real-rows-only mat-vec copies)
+    i64 bytes = 0;               // all ways: groups and slice headers
+    i64 bytes_real = 0;          // groups and headers of the first row group (what a real-rows-only mat-vec reads)
+    i64 padded_nnz = 0;          // entries stored, padding included
     WayDesc way[NUM_WAYS] = {};
     i32 nrows = 0;
     i64 nnz = 0;
     bool wide = false;           // uint32 column indices
-    bool has_aux = false;        // first pieces carry the l1 diagonal inverse of their rows
+    bool has_aux = false;        // slice headers carry a per-row value (the l1 diagonal inverse)
 };
 
 // Sizes of one (subdomain, level) block and where its arrays sit inside the subdomain's blob.
@@ -118,7 +119,7 @@ struct LocalCsr {
 class CompositeBuilder {
 public:
     CompositeBuilder(const Hierarchy& H, const std::vector<i32>& owner, const std::vector<std::vector<i32>>& owned,
-                     int eta, int num_ghost, int block_bytes, int window);
+                     int eta, int num_ghost, int window);
     // Phase 1: index sets, local matrices and the blob layout of subdomain p.
     void plan(int p, SubdomainBlob& out);
     // Phase 2: write the arrays of the subdomain planned last into dst (out.bytes bytes).
@@ -132,14 +133,14 @@ private:
     const Hierarchy& H_;
     const std::vector<i32>& owner_;
     const std::vector<std::vector<i32>>& owned_;
-    int eta_, nghost_, block_bytes_, window_, p_ = -1;
+    int eta_, nghost_, window_, p_ = -1;
     std::vector<std::vector<i32>> real_, ghost_;
     std::vector<LocalCsr> A_, P_, R_;                 // local matrices of the subdomain planned last
     // epoch-stamped global->local maps, one per level
     std::vector<std::vector<i32>> loc_, stamp_;
     std::vector<i32> epoch_;
     std::vector<i32> frontier_, next_, cursor_;
-    std::vector<double> aux_;
+    std::vector<double> aux_, auxr_;
     i32 local_of(int l, i32 g) const { return stamp_[l][g] == epoch_[l] ? loc_[l][g] : -1; }
 };
 
@@ -149,6 +150,6 @@ struct PackedLevelStream {
     StreamLayout lay;
 };
 // aux: M.nrows doubles (l1 diagonal inverse, A streams) or nullptr
-bool pack_global_stream(const HostCsr& M, const double* aux, int block_bytes, int window, PackedLevelStream& out, i64& too_long_row);
+bool pack_global_stream(const HostCsr& M, const double* aux, int window, PackedLevelStream& out, i64& too_long_row);
 
 }  // namespace amgdd

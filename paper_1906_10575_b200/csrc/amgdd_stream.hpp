@@ -1,83 +1,80 @@
-// HBM layout of the AMG-DD solve phase: packed "slice-JDS" matrix streams and the per-(subdomain,
-// level) descriptor tables.  Plain structs shared by the host packer (amgdd_pack.cpp,
-// amgdd_composite.cpp, amgdd_api.cu) and the device kernel (amgdd_fac.cu); no CUDA types, no
-// arithmetic of the method.
+// HBM layout of the AMG-DD solve phase: packed "SELL-32 group" matrix streams, the per-(subdomain,
+// level) descriptor tables and the static program of one subdomain.  Plain structs shared by the
+// host packer (amgdd_pack.cpp, amgdd_composite.cpp, amgdd_api.cu) and the device kernel
+// (amgdd_fac.cu); no CUDA types, no arithmetic of the method.
 //
 // PACKED STREAM.  Every local matrix of a composite level (A_l, P_l, R_l = P_l^T; paper P:49,
-// P:248) is stored as NUM_WAYS independent sub-streams ("ways"), one per consumer warp of the
-// AlgFAC kernel.  A way is a sequence of fixed-stride BLOCKS of `block_bytes` bytes; warp w moves
-// the blocks of way w HBM -> its own shared-memory ring with one bulk async copy each
-// (cp.async.bulk, the 1-D TMA path) and consumes them in order, so a mat-vec needs no
-// communication between warps and the matrix crosses HBM exactly once, in contiguous requests.
+// P:248) is stored as NUM_WAYS independent sub-streams ("ways"), one per warp of the AlgFAC
+// kernel.  Warp w reads way w with coalesced 128-bit loads straight into a ring of registers and
+// runs several groups ahead of its arithmetic, so a mat-vec needs no communication between warps
+// and the matrix crosses HBM exactly once, in 512-byte requests.
 //
-// Rows are grouped for a 32-wide warp with ONE LANE PER ROW:
-//   * the rows [0, n_real) and [n_real, nrows) are two GROUPS (real / ghost rows of A_l; other
-//     matrices have one group); a group is cut into WINDOWS of `window` consecutive rows; inside a
-//     window the rows are sorted by descending length (stable) and cut into SLICES of 32 rows
-//     (the last slice of a group may hold fewer).  Lane j of a slice owns its j-th longest row.
-//   * a slice with longest row K is stored as K STEPS (jagged diagonals): step k holds entry k of
-//     every row of the slice that has more than k entries -- lanes [0, cnt_k) because of the
-//     sort -- so nothing is padded: 8 + 2 (or 4) bytes per nonzero.
+// Rows are grouped for a 32-wide warp with ONE LANE PER ROW (sliced ELLPACK, slice height 32):
+//   * the rows [0, n_real) and [n_real, nrows) are two ROW GROUPS (real / ghost rows of A_l; other
+//     matrices have one); a row group is cut into WINDOWS of `window` consecutive rows; inside a
+//     window the rows are sorted by descending length (stable) and cut into SLICES of 32 rows (the
+//     last slice of a row group may hold fewer).  Lane j of a slice owns its j-th longest row.
+//   * a slice whose longest row has len entries is stored as K = max(1, ceil(len / 4)) GROUPS of
+//     4 STEPS; step k of lane j is entry k of the lane's row, in stored (= CSR) order; steps past
+//     the end of a row are padding (value 0.0, column 0).
 //   * slices are dealt to the ways in slice order, each to the way with the fewest bytes so far
-//     (ties: lowest way), first all slices of the first group, then those of the second; inside a
-//     way they keep that order.  A slice is laid down as one or more PIECES (consecutive step
-//     ranges); a piece never crosses a block, a slice may.
+//     (ties: lowest way), first all slices of the first row group, then those of the second;
+//     inside a way they keep that order, so the slices of the first row group are a prefix of
+//     every way (what a real-rows-only mat-vec reads).
 //
-//   way w:  blocks at  base + 16 * way[w].off16 + j * block_bytes,  j < way[w].nblocks; the last
-//           block of a way is cut at its 16-byte padded end (16 * way[w].last16 bytes)
-//   block:  byte 0  uint32 npieces
-//                4  uint32 reserved[3]
-//               16  PieceDesc[npieces]   16 bytes each
-//              ...  piece data, each piece 16-byte aligned
-//   piece:  [only if k0 == 0]  uint16 rowid[32]   row of lane j minus desc.row_base; 0xFFFF = no row
-//                              uint16 len[32]     entries of that row (0 for "no row")
-//                              double aux[32]     only in streams packed with an aux vector (A_l:
-//                                                 the l1 diagonal inverse of the row, S8)
-//           double v[nnz]      step after step
-//           colT   ci[nnz]     uint16 (narrow) or uint32 (wide), same order
-//           (zero padding to a multiple of 16 bytes)
+//   stream:  [groups of way 0] ... [groups of way 15] [headers of way 0] ... [headers of way 15]
+//   way w:   groups at   base + 128 * way[w].grp_off128 + g * group_bytes,   g < way[w].ngroups
+//            headers at  base + 128 * way[w].hdr_off128 + s * header_bytes,  s < way[w].nslices
+//   group (narrow, 1280 bytes):  32 x { double v[step 0], v[step 1] }     lane j at byte 16 j
+//                                32 x { double v[step 2], v[step 3] }     lane j at 512 + 16 j
+//                                32 x { uint16 col[step 0..3] }           lane j at 1024 + 8 j
+//   group (wide, 1536 bytes):    the same two value planes, then 32 x { uint32 col[step 0..3] },
+//                                lane j at 1024 + 16 j
+//   header (512 bytes):  32 x { uint32 row, uint32 ngroups, double aux }   lane j at 16 j
+//            row = the lane's row (NO_ROW: the slice has fewer than 32 rows), ngroups = K of the
+//            slice (the same in every lane), aux = a per-row value the epilogue needs (the l1
+//            diagonal inverse, S8; 0.0 in streams packed without an aux vector).  One header
+//            shape for all streams keeps every load of the kernel unconditional.
 #pragma once
 #include <cstdint>
 
 namespace amgdd {
 
-constexpr int NUM_WAYS = 16;                 // consumer warps of the AlgFAC kernel = sub-streams per matrix
-constexpr int BLOCK_HEADER_BYTES = 16;
-constexpr int PIECE_DESC_BYTES = 16;
+constexpr int NUM_WAYS = 16;                 // warps of the AlgFAC kernel = sub-streams per matrix
 constexpr int SLICE_ROWS = 32;
-constexpr int MIN_BLOCK_BYTES = 1024;
-constexpr int MAX_BLOCK_BYTES = 32768;
-constexpr int DEFAULT_BLOCK_BYTES = 2048;
+constexpr int GROUP_STEPS = 4;
+constexpr int GROUP_BYTES_NARROW = 1280;
+constexpr int GROUP_BYTES_WIDE = 1536;
+constexpr int HEADER_BYTES = 512;
 constexpr int NARROW_MAX_COLS = 65536;       // uint16 column indices
-constexpr int MAX_WINDOW = 32768;            // rowid is 16-bit relative to the window, 0xFFFF reserved
 constexpr int DEFAULT_WINDOW = 256;
-constexpr uint16_t NO_ROW = 0xFFFF;
+constexpr int MAX_WINDOW = 1 << 20;
+constexpr uint32_t NO_ROW = 0xFFFFFFFFu;
+constexpr int RING_DEPTH = 3;                // groups per register block; a warp holds two blocks (one in flight, one being consumed)
 
-struct PieceDesc {
-    uint32_t off;          // byte offset of the piece data from the start of the block (16-aligned)
-    uint32_t row_base;     // first row of the slice's window
-    uint16_t k0;           // first step of the slice held by this piece
-    uint16_t nk;           // steps in this piece
-    uint16_t K;            // steps of the whole slice (= its longest row); the piece is the last iff k0 + nk == K
-    uint16_t nnz;          // entries in this piece
-};
-static_assert(sizeof(PieceDesc) == PIECE_DESC_BYTES, "PieceDesc layout");
+inline int group_bytes(bool wide) { return wide ? GROUP_BYTES_WIDE : GROUP_BYTES_NARROW; }
 
 struct WayDesc {           // one sub-stream (same layout as amgdd_way_t of include/amgdd.h)
-    uint32_t off16;        // start of the way, in units of 16 bytes from the stream base
-    uint32_t nblocks;      // blocks of the way
-    uint32_t nblocks_real; // blocks that hold the way's slices of the first group
-    uint16_t last16;       // size of the last block in units of 16 bytes (<= block_bytes / 16)
-    uint16_t nslices_real; // the way's slices of the first group
+    uint32_t grp_off128;   // start of the way's groups, in units of 128 bytes from the stream base
+    uint32_t hdr_off128;   // start of the way's slice headers, same unit
+    uint32_t ngroups;      // groups of the way
+    uint32_t ngroups_real; // groups of the way's slices of the first row group (a prefix)
+    uint32_t nslices;      // slices of the way
+    uint32_t nslices_real; // slices of the first row group (a prefix)
+    uint32_t pad_[2];
 };
-static_assert(sizeof(WayDesc) == 16, "WayDesc layout");
+static_assert(sizeof(WayDesc) == 32, "WayDesc layout");
+
+constexpr uint32_t STREAM_WIDE = 1u;         // StreamDesc::flags
+constexpr uint32_t STREAM_AUX = 2u;
 
 struct StreamDesc {
-    const char* base;      // DEVICE, 16-byte aligned
+    const char* base;      // DEVICE, 128-byte aligned
+    uint32_t flags;        // STREAM_WIDE | STREAM_AUX
+    uint32_t pad_;
     WayDesc way[NUM_WAYS];
-    int wide;              // 1: uint32 column indices
-    int has_aux;           // 1: first pieces carry aux[32]
 };
+static_assert(sizeof(StreamDesc) == 16 + 32 * NUM_WAYS, "StreamDesc layout");
 
 // one (subdomain, level) block; pointers are device addresses (private blob or the shared global copy)
 struct DevLevel {
@@ -85,17 +82,45 @@ struct DevLevel {
     int n_bar;             // |D-bar_l^p| = real + ghost
     const int* gid;        // n_bar global indices (real ascending, then ghost ascending; S7)
     const double* dinv;    // n_real
-    StreamDesc A;          // n_bar rows: real rows complete, ghost rows restricted to real columns (A12)
-    StreamDesc P;          // n_bar rows, columns local to level l+1 (unused on L)
-    StreamDesc R;          // n_bar(l+1) rows, columns local to level l (unused on L)
     long long voff;        // offset (doubles) of this level's vectors u|t|s|f inside a workspace slot
+    StreamDesc A;          // n_bar rows: real rows complete, ghost rows restricted to real columns (A12); aux = dinv
+    StreamDesc P;          // n_bar rows, columns local to level l+1 (unused on L); no aux
+    StreamDesc R;          // n_bar(l+1) rows, columns local to level l (unused on L); aux = dinv of level l+1
 };
+static_assert(sizeof(DevLevel) % 16 == 0, "DevLevel is read with 128-bit loads");
 
 struct DevSub {
     const int* owned;      // local indices (level 0) of the owned dofs Omega_0^p
     int n_owned;
     int pad_;
 };
+
+// ---- the static program of one subdomain (built on the host by fac_build_program) ------------
+enum OpKind : uint8_t {
+    OPK_BEGIN = 0,         // Alg. 2 P:475 + Alg. 4
+    OPK_FIRST0 = 1,        // level 0, first AlgFAC iteration: u_0 = 0, so the first sweep is delta = D^-1 f (no matrix)
+    OPK_RELAX = 2,         // one l1-Jacobi sweep on the real points (P:507-508 / P:517-518), stream A_l real rows
+    OPK_AT = 3,            // w = s_l + A_l t_l on D-bar_l, stream A_l
+    OPK_RESTRICT = 4,      // s_{l+1} = R_l w [+ P:511 and the first sweep of level l+1 in the first iteration]
+    OPK_RECALC = 5,        // f_{l+1} -= A_{l+1} u_{l+1} + s_{l+1} [+ the first sweep of level l+1]
+    OPK_INTERP = 6,        // u_l += P_l u_{l+1} on D-bar_l
+    OPK_COARSE = 7,        // u_L = A_L^-1 f_L
+    OPK_END = 8            // Alg. 2
+};
+constexpr uint8_t OPF_FIRST = 1;      // first AlgFAC iteration of the cycle
+constexpr uint8_t OPF_TSMEM = 2;      // the shared-memory output is t (the gather vector of the A t step), else u
+constexpr uint8_t OPF_COARSEST = 4;   // RESTRICT / RECALC whose target level is L: no relaxation follows
+
+struct FacOp {
+    uint8_t kind;          // OpKind
+    uint8_t level;         // l of the step as written in Alg. 4 (RESTRICT: R_l; RECALC: A_{l+1} has level = l+1; INTERP: P_l)
+    uint8_t gbuf;          // shared-memory vector buffer (0/1) the mat-vec gathers from; it writes the other
+    uint8_t flags;         // OPF_*
+    int16_t next_mat;      // index of the next mat-vec op of the program (-1: none): its groups are prefetched
+    int16_t next_mat2;     // the one after that (-1: none): its way descriptor is prefetched
+};
+static_assert(sizeof(FacOp) == 8, "FacOp layout");
+constexpr int MAX_OPS = 1024;
 
 struct FacParams {
     const DevLevel* lev;       // [P][L+1]
@@ -108,19 +133,14 @@ struct FacParams {
     double* x;                 // fine iterate, updated on owned dofs
     double* workspace;         // gridDim.x * slot_stride doubles
     long long slot_stride;
-    long long scratch_off;     // offset of the scratch vector w inside a slot
+    long long xg_off;          // offset of the two global vector buffers (x_cap_global doubles each) inside a slot, or -1
     int* work_counter;
-    int nfac;
-    int nu;
-    int nops;                  // steps in the program of one subdomain = fac_num_ops(L, nfac, nu)
+    const FacOp* ops;          // DEVICE, nops entries
+    int nops;
     const double* lu;          // dense LU of A_L, column-major, unit lower
     const int* rowperm;
     int nL;
-    // shared-memory plan of one CTA
-    int block_bytes;           // ring slot size = stream block stride
-    int stages;                // ring depth of every warp
-    int x_cap;                 // doubles in the shared-memory gather buffer
-    int table_bytes;           // bytes of one descriptor table slot = (L+1) * sizeof(DevLevel), 16-aligned
+    int x_cap;                 // doubles in each of the two shared-memory vector buffers (0: vectors in global memory)
     long long* prof;           // optional: gridDim.x * FAC_PROF_SLOTS cycle counters (debugging), or nullptr
 };
 constexpr int FAC_PROF_SLOTS = 16;
@@ -133,23 +153,23 @@ struct FacLaunch {
 
 // host-side packing (amgdd_pack.cpp) ---------------------------------------------------------
 struct PackPlan {
-    int64_t bytes;             // total stream bytes (16-aligned)
+    int64_t bytes;             // total stream bytes (multiple of 128)
+    int64_t bytes_real;        // groups + headers of the first row group
     WayDesc way[NUM_WAYS];
-    int64_t nblocks;           // blocks over all ways
-    int64_t nblocks_real;
-    int nslices, nslices_real;
+    int64_t ngroups, ngroups_real;
+    int64_t nslices, nslices_real;
+    int64_t padded_nnz;        // 4 * 32 * ngroups: entries stored, padding included
 };
-// rp: nrows+1 int32 offsets (rp[0] = 0); window: rows per sort window (multiple of 32, <= MAX_WINDOW);
-// rows must have at most 65535 entries
-PackPlan plan_stream(int nrows, const int32_t* rp, bool wide, bool has_aux, int block_bytes, int n_real, int window);
+// rp: nrows+1 int32 offsets (rp[0] = 0); window: rows per sort window (multiple of 32)
+PackPlan plan_stream(int nrows, const int32_t* rp, bool wide, bool has_aux, int n_real, int window);
 // writes plan.bytes bytes; aux: nrows doubles or nullptr (must match has_aux of the plan)
 void write_stream(int nrows, const int32_t* rp, const int32_t* ci, const double* v, const double* aux, bool wide,
-                  int block_bytes, int n_real, int window, char* dst);
+                  int n_real, int window, char* dst);
 
-int fac_smem_bytes(int block_bytes, int stages, int x_cap, int table_bytes);
-int fac_max_stages();
-int fac_num_ops(int L, int nfac, int nu);   // steps in the program of one subdomain
-int fac_max_ops();                          // the longest program the kernel has room for
+// the program of one subdomain: num_fac_cycles AlgFAC V(nu,nu)-cycles (Alg. 4); returns the op count
+// (ops may be nullptr to count only)
+int fac_build_program(int L, int nfac, int nu, FacOp* ops);
+int fac_smem_bytes(int x_cap, int L, int nops);
 void launch_fac(const FacParams& prm, const FacLaunch& cfg, void* stream);
 int fac_configure(int device, int max_smem_optin);   // sets the kernel's dynamic-smem attribute; 0 on success
 

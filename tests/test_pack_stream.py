@@ -1,99 +1,78 @@
-"""Host logic, no GPU: the packed slice-JDS streams (the HBM layout the AlgFAC kernel reads with bulk
-async copies; csrc/amgdd_stream.hpp) decode back to the CSR they were
-made from, way by way and block by block, for narrow and wide column indices, ragged rows, empty
-rows, two row groups, an aux vector, and block sizes that force slices to be split across blocks."""
+"""Host logic, no GPU: the packed SELL-32 group streams (the HBM layout the AlgFAC kernel reads with
+coalesced 128-bit loads; csrc/amgdd_stream.hpp) decode back to the CSR
+they were made from, way by way and slice by slice, for narrow and wide column indices, ragged
+rows, empty rows, two row groups, an aux vector and several sort windows."""
 import numpy as np
 import pytest
 
 import paper_1906_10575_b200 as m
 
-NO_ROW = 0xFFFF
+NO_ROW = 0xFFFFFFFF
+HB = m.HEADER_BYTES
 
 
-def decode(stream, ways, block_bytes, wide, nrows, has_aux, n_real=None, window=256):
+def decode(stream, ways, wide, nrows, n_real=None, window=256):
     """Decoder written from the layout comment of amgdd_stream.hpp (independent of the packer).
-    Returns per-row lists of (column, value) in stored order and the aux vector; checks the way
-    descriptors (block counts, the real-group prefix, the cut of the last block)."""
+    Returns per-row lists of (column, value) in stored order, the aux vector and the bytes of each
+    way; checks the way descriptors (offsets, the real-group prefix) and that padding is zero."""
     raw = stream.tobytes()
     n_real = nrows if n_real is None else n_real
-    rows = [[] for _ in range(nrows)]
+    gb = m.GROUP_BYTES_WIDE if wide else m.GROUP_BYTES_NARROW
+    rows = [None] * nrows
     aux = np.full(nrows, np.nan)
-    seen = np.zeros(nrows, dtype=int)
-    cdt = np.uint32 if wide else np.uint16
-    expect_off = 0
     load = []
-    for w in range(len(ways)):
-        wd = ways[w]
-        nblocks, off = int(wd["nblocks"]), 16 * int(wd["off16"])
-        assert off == expect_off, "ways are laid back to back"
-        cur, real_slices, ghost_seen, last_real_block = None, 0, False, -1
-        end = off
-        for j in range(nblocks):
-            base = off + j * block_bytes
-            npieces, r0, r1, r2 = np.frombuffer(raw, dtype=np.uint32, count=4, offset=base)
-            assert npieces >= 1 and r0 == 0 and r1 == 0 and r2 == 0
-            end = base + 16 + 16 * int(npieces)
-            for i in range(int(npieces)):
-                poff, row_base = np.frombuffer(raw, dtype=np.uint32, count=2, offset=base + 16 + 16 * i)
-                k0, nk, K, nnz = (int(t) for t in np.frombuffer(raw, dtype=np.uint16, count=4, offset=base + 16 + 16 * i + 8))
-                assert poff % 16 == 0 and poff == end - base, "pieces are laid down back to back, 16-byte aligned"
-                q = base + int(poff)
-                if k0 == 0:
-                    assert cur is None, "a new slice starts only after the previous one is complete"
-                    rowid = np.frombuffer(raw, dtype=np.uint16, count=32, offset=q).astype(int)
-                    lens = np.frombuffer(raw, dtype=np.uint16, count=32, offset=q + 64).astype(int)
-                    q += 128
-                    a = None
-                    if has_aux:
-                        a = np.frombuffer(raw, dtype=np.float64, count=32, offset=q)
-                        q += 256
-                    assert (np.diff(lens) <= 0).all(), "rows of a slice are sorted by descending length"
-                    assert K == lens[0]
-                    valid = rowid != NO_ROW
-                    assert valid.any() and (lens[~valid] == 0).all() and valid[: valid.sum()].all(), "missing rows are the last lanes"
-                    assert row_base % window == 0 or (row_base - n_real) % window == 0
-                    grows = np.where(valid, int(row_base) + rowid, -1)
-                    assert (rowid[valid] < window).all()
-                    for jj in np.nonzero(valid)[0]:
-                        assert seen[grows[jj]] == 0
-                        seen[grows[jj]] = 1
-                        if has_aux:
-                            aux[grows[jj]] = a[jj]
-                    is_real = bool((grows[valid] < n_real).all())
-                    assert is_real or (grows[valid] >= n_real).all(), "the two groups never mix inside a slice"
-                    assert not (is_real and ghost_seen), "inside a way the first group comes first"
-                    ghost_seen = ghost_seen or not is_real
-                    cur = dict(rows=grows, lens=lens, K=K, k=0, real=is_real)
-                else:
-                    assert i == 0 and cur is not None, "only piece 0 may continue a slice"
-                    assert k0 == cur["k"] and K == cur["K"]
-                vals = np.frombuffer(raw, dtype=np.float64, count=nnz, offset=q)
-                cols = np.frombuffer(raw, dtype=cdt, count=nnz, offset=q + 8 * nnz)
-                e = 0
-                for k in range(k0, k0 + nk):
-                    cnt = int((cur["lens"] > k).sum())
-                    assert cnt >= 1
-                    for jj in range(cnt):
-                        rows[cur["rows"][jj]].append((int(cols[e + jj]), float(vals[e + jj])))
-                    e += cnt
-                assert e == nnz
-                cur["k"] = k0 + nk
-                end = q + ((nnz * (8 + cols.itemsize) + 15) // 16) * 16
-                assert end - base <= block_bytes
-                if cur["k"] == cur["K"]:
-                    if cur["real"]:
-                        real_slices += 1
-                        last_real_block = j
-                    cur = None
-                else:
-                    assert i == int(npieces) - 1, "a slice that continues must end its block"
-            if j == nblocks - 1:
-                assert end - base == 16 * int(wd["last16"]), "the last block of a way is cut at its padded end"
-        assert cur is None
-        assert int(wd["nslices_real"]) == real_slices and int(wd["nblocks_real"]) == last_real_block + 1
-        expect_off = end
-        load.append(end - off)
-    assert expect_off == len(raw) and seen.all()
+    # groups of all ways come first, back to back; then the headers, each way 128-byte aligned
+    off = 0
+    for w in ways:
+        assert 128 * int(w["grp_off128"]) == off
+        off += int(w["ngroups"]) * gb
+    for w in ways:
+        assert 128 * int(w["hdr_off128"]) == off
+        off = -(-(off + int(w["nslices"]) * HB) // 128) * 128
+    assert off == len(raw)
+    for w in ways:
+        g = 128 * int(w["grp_off128"])
+        h = 128 * int(w["hdr_off128"])
+        groups_seen = real_groups = real_slices = 0
+        ghost_seen = False
+        for s in range(int(w["nslices"])):
+            hdr = np.frombuffer(raw, dtype=np.uint32, count=128, offset=h + s * HB).reshape(32, 4)
+            a = np.frombuffer(raw, dtype=np.float64, count=64, offset=h + s * HB).reshape(32, 2)[:, 1]
+            rid, K = hdr[:, 0].astype(np.int64), hdr[:, 1]
+            assert (K == K[0]).all() and K[0] >= 1, "every lane carries the slice's group count"
+            K = int(K[0])
+            valid = rid != NO_ROW
+            assert valid.any() and valid[: valid.sum()].all(), "missing rows are the last lanes"
+            assert (a[~valid] == 0).all()
+            is_real = bool((rid[valid] < n_real).all())
+            assert is_real or (rid[valid] >= n_real).all(), "the two row groups never mix inside a slice"
+            assert not (is_real and ghost_seen), "inside a way the first row group comes first"
+            ghost_seen = ghost_seen or not is_real
+            base = 0 if is_real else n_real
+            assert len({(int(r) - base) // window for r in rid[valid]}) == 1, "a slice stays inside one sort window"
+            vals = np.empty((32, 4 * K))
+            cols = np.empty((32, 4 * K), dtype=np.int64)
+            for kg in range(K):
+                q = g + (groups_seen + kg) * gb
+                vals[:, 4 * kg: 4 * kg + 2] = np.frombuffer(raw, dtype=np.float64, count=64, offset=q).reshape(32, 2)
+                vals[:, 4 * kg + 2: 4 * kg + 4] = np.frombuffer(raw, dtype=np.float64, count=64, offset=q + 512).reshape(32, 2)
+                cdt = np.uint32 if wide else np.uint16
+                cols[:, 4 * kg: 4 * kg + 4] = np.frombuffer(raw, dtype=cdt, count=128, offset=q + 1024).reshape(32, 4)
+            groups_seen += K
+            if is_real:
+                real_groups += K
+                real_slices += 1
+            for j in range(32):
+                if not valid[j]:
+                    assert (vals[j] == 0).all() and (cols[j] == 0).all()
+                    continue
+                r = int(rid[j])
+                assert rows[r] is None, "every row is stored once"
+                rows[r] = (cols[j], vals[j])
+                aux[r] = a[j]
+        assert groups_seen == int(w["ngroups"]) and real_groups == int(w["ngroups_real"]) and real_slices == int(w["nslices_real"])
+        load.append(int(w["ngroups"]) * gb + int(w["nslices"]) * HB)
+    assert all(r is not None for r in rows)
     return rows, aux, load
 
 
@@ -107,60 +86,73 @@ def random_csr(rng, nrows, ncols, max_len, empty_frac=0.1):
 
 
 def check_rows(rows, rp, ci, v):
-    for i, r in enumerate(rows):
-        cols = [c for c, _ in r]
-        vals = [x for _, x in r]
-        assert cols == ci[rp[i]:rp[i + 1]].tolist(), f"row {i}: columns (in stored order)"
-        assert vals == v[rp[i]:rp[i + 1]].tolist(), f"row {i}: values"
+    """Stored order = CSR order; everything past the end of a row is padding (0.0, column 0)."""
+    for i, (cols, vals) in enumerate(rows):
+        n = rp[i + 1] - rp[i]
+        assert n <= len(cols), f"row {i} does not fit its slice"
+        assert cols[:n].tolist() == ci[rp[i]:rp[i + 1]].tolist(), f"row {i}: columns (in stored order)"
+        assert vals[:n].tolist() == v[rp[i]:rp[i + 1]].tolist(), f"row {i}: values"
+        assert (cols[n:] == 0).all() and (vals[n:] == 0).all(), f"row {i}: padding"
 
 
 @pytest.mark.parametrize("wide", [False, True])
-@pytest.mark.parametrize("block_bytes", [1024, 2048, 8192])
-def test_stream_round_trip(wide, block_bytes):
-    rng = np.random.default_rng(7 + block_bytes + wide)
+def test_stream_round_trip(wide):
+    rng = np.random.default_rng(7 + wide)
     ncols = 70000 if wide else 5000
     nrows, n_real = 3000, 2013
     rp, ci, v = random_csr(rng, nrows, ncols, 60)
     aux = rng.standard_normal(nrows)
-    stream, ways = m.amgdd_pack_stream(rp, ci, v, wide=wide, block_bytes=block_bytes, n_real=n_real, aux=aux)
-    assert len(ways) == m.NUM_WAYS and len(stream) % 16 == 0
-    rows, aux2, load = decode(stream, ways, block_bytes, wide, nrows, True, n_real)
+    stream, ways = m.amgdd_pack_stream(rp, ci, v, wide=wide, n_real=n_real, aux=aux)
+    assert len(ways) == m.NUM_WAYS and len(stream) % 128 == 0
+    rows, aux2, load = decode(stream, ways, wide, nrows, n_real)
     check_rows(rows, rp, ci, v)
     assert np.array_equal(aux2, aux)
-    # the ways are balanced: slices go to the lightest way, so no way exceeds the mean by more than a slice or so
-    assert max(load) <= np.mean(load) + 32 * 60 * 12 + 1024
-    # 10 (narrow) / 12 (wide) bytes per nonzero, nothing padded; per row 2 + 2 + 8 (rowid, len, aux);
-    # per block a header, per piece a descriptor and padding to 16, and at most one step (<= 32
-    # entries) that did not fit the tail of a block any more
+    # the ways are balanced: a slice goes to the lightest way, so no way exceeds the mean by more than one slice
+    gb = m.GROUP_BYTES_WIDE if wide else m.GROUP_BYTES_NARROW
+    assert max(load) <= np.mean(load) + 15 * gb + HB
+    # rows are sorted by length inside windows of 256, so a slice is padded by less than the spread
+    # of lengths over 32 consecutive sorted rows (60 / 8 here) plus the round-up to a group of 4
     per_nnz = 12 if wide else 10
-    ideal = rp[-1] * per_nnz
-    nblocks = int(ways["nblocks"].sum())
-    nslices = -(-n_real // 32) + -(-(nrows - n_real) // 32) + 30
-    assert len(stream) <= ideal + nslices * (32 * 12 + 32) + nblocks * (16 + 2 * 32 + 32 * per_nnz)
-    if block_bytes == 8192:
-        assert len(stream) <= 1.08 * ideal
+    assert int(ways["ngroups"].sum()) * 128 <= rp[-1] + nrows * (60 / 8 + 3) + 2 * 32 * 60
+    assert len(stream) <= 1.35 * rp[-1] * per_nnz + (nrows / 32 + 2) * HB + 16 * 128
+
+
+def test_uniform_rows_are_not_padded():
+    # the shape of the coarse composite levels: rows of nearly one length -> 10 bytes per nonzero + headers
+    rng = np.random.default_rng(11)
+    nrows = 4096
+    lens = np.full(nrows, 36)
+    rp = np.concatenate([[0], np.cumsum(lens)]).astype(np.int32)
+    ci = np.concatenate([np.sort(rng.choice(6000, size=k, replace=False)) for k in lens]).astype(np.int32)
+    v = rng.standard_normal(rp[-1])
+    stream, ways = m.amgdd_pack_stream(rp, ci, v)
+    assert int(ways["ngroups"].sum()) == nrows // 32 * 9
+    assert len(stream) == nrows // 32 * (9 * m.GROUP_BYTES_NARROW + HB)
+    rows, _, _ = decode(stream, ways, False, nrows)
+    check_rows(rows, rp, ci, v)
 
 
 @pytest.mark.parametrize("window", [32, 64, 1024])
 def test_windows_and_no_aux(window):
     rng = np.random.default_rng(window)
     rp, ci, v = random_csr(rng, 777, 3000, 25, empty_frac=0.3)
-    stream, ways = m.amgdd_pack_stream(rp, ci, v, block_bytes=2048, window=window)
-    rows, _, _ = decode(stream, ways, 2048, False, 777, False, window=window)
+    stream, ways = m.amgdd_pack_stream(rp, ci, v, window=window)
+    rows, aux, _ = decode(stream, ways, False, 777, window=window)
     check_rows(rows, rp, ci, v)
-    assert np.array_equal(ways["nblocks"], ways["nblocks_real"])
+    assert (aux == 0).all(), "streams packed without an aux vector carry 0.0"
+    assert np.array_equal(ways["ngroups"], ways["ngroups_real"]) and np.array_equal(ways["nslices"], ways["nslices_real"])
 
 
-def test_long_rows_are_split_across_blocks():
-    # one row of 5000 entries (50 KB) in 1 KiB blocks, next to short rows
+def test_long_rows():
+    # one row of 5000 entries next to short rows: its slice has 1250 groups
     rng = np.random.default_rng(3)
     lens = np.array([3, 5000, 0, 7, 2500] + [4] * 40)
     rp = np.concatenate([[0], np.cumsum(lens)]).astype(np.int32)
     ci = np.concatenate([np.sort(rng.choice(60000, size=k, replace=False)) for k in lens]).astype(np.int32)
     v = rng.standard_normal(rp[-1])
-    stream, ways = m.amgdd_pack_stream(rp, ci, v, block_bytes=1024)
-    assert ways["nblocks"].sum() > 50
-    rows, _, _ = decode(stream, ways, 1024, False, len(lens), False)
+    stream, ways = m.amgdd_pack_stream(rp, ci, v)
+    assert int(ways["ngroups"].max()) == 1250
+    rows, _, _ = decode(stream, ways, False, len(lens))
     check_rows(rows, rp, ci, v)
 
 
@@ -169,18 +161,18 @@ def test_few_rows_and_empty_matrix():
     ci = np.array([0, 3, 1, 2, 3], dtype=np.int32)
     v = np.arange(5, dtype=np.float64)
     stream, ways = m.amgdd_pack_stream(rp, ci, v)
-    # one slice in way 0: block header + one descriptor + rowid/len + 5 entries padded to 16
-    assert ways["nblocks"].tolist() == [1] + [0] * (m.NUM_WAYS - 1)
-    assert len(stream) == 16 + 16 + 128 + ((5 * 10 + 15) // 16) * 16
-    rows, _, _ = decode(stream, ways, 2048, False, 3, False)
+    # one slice in way 0: one group (longest row 3 <= 4 steps) and one header
+    assert ways["ngroups"].tolist() == [1] + [0] * (m.NUM_WAYS - 1)
+    assert len(stream) == m.GROUP_BYTES_NARROW + HB
+    rows, _, _ = decode(stream, ways, False, 3)
     check_rows(rows, rp, ci, v)
-    # a slice of empty rows still gets a piece (its rows still run their epilogue)
+    # a slice of empty rows still gets one (all padding) group: its rows still run their epilogue
     stream, ways = m.amgdd_pack_stream(np.zeros(4, np.int32), np.zeros(0, np.int32), np.zeros(0))
-    assert ways["nblocks"].sum() == 1 and len(stream) == 16 + 16 + 128
-    rows, _, _ = decode(stream, ways, 2048, False, 3, False)
-    assert rows == [[], [], []]
+    assert ways["ngroups"].sum() == 1 and len(stream) == m.GROUP_BYTES_NARROW + HB
+    rows, _, _ = decode(stream, ways, False, 3)
+    assert all((c == 0).all() and (x == 0).all() for c, x in rows)
     stream, ways = m.amgdd_pack_stream(np.zeros(1, np.int32), np.zeros(0, np.int32), np.zeros(0))
-    assert ways["nblocks"].sum() == 0 and len(stream) == 0
+    assert ways["ngroups"].sum() == 0 and len(stream) == 0
 
 
 def test_bad_arguments():
@@ -189,9 +181,6 @@ def test_bad_arguments():
     v = np.ones(200)
     with pytest.raises(m.AmgddError) as e:            # narrow form cannot hold column 70000
         m.amgdd_pack_stream(np.array([0, 1], np.int32), np.array([70000], np.int32), np.ones(1))
-    assert e.value.code == -1
-    with pytest.raises(m.AmgddError) as e:
-        m.amgdd_pack_stream(rp, ci, v, block_bytes=1000)
     assert e.value.code == -1
     with pytest.raises(m.AmgddError) as e:
         m.amgdd_pack_stream(rp, ci, v, window=48)
