@@ -59,7 +59,7 @@ struct amgdd_handle_s {
     long long* d_r_off = nullptr;
     std::vector<long long> r_off;
     double* d_workspace = nullptr;
-    long long slot_stride = 0, xg_off = -1;
+    long long slot_stride = 0, xg_off = -1, x_need = 0;
     int window = DEFAULT_WINDOW, x_cap = 0, smem_cta = 0;
     FacLaunch fac_cfg = {1, 32 * NUM_WAYS, 0};
     FacOp* d_ops = nullptr;                     // the program of one subdomain (fac_build_program)
@@ -381,22 +381,16 @@ int finish_tables(amgdd_handle_s* h) {
     // otherwise they live in the workspace slot (slow path, same arithmetic).
     cudaDeviceProp prop;
     CUDA_TRY(cudaGetDeviceProperties(&prop, h->device));
-    h->smem_cta = (int)prop.sharedMemPerBlockOptin;
-    const long long x_need = (max_nb + 15) & ~15LL;
-    const bool force_global = env_int("AMGDD_FORCE_GLOBAL_X", 0) > 0;
-    if (!force_global && (long long)fac_smem_bytes(0, L, MAX_OPS) + 16 * x_need <= (long long)h->smem_cta) {
-        h->x_cap = (int)x_need;
-        h->xg_off = -1;
-        h->slot_stride = (max_sum + 15) & ~15LL;
-    } else {
-        h->x_cap = 0;
-        h->xg_off = (max_sum + 15) & ~15LL;
-        h->slot_stride = h->xg_off + 2 * x_need;
-    }
+    h->smem_cta = CTAS_PER_SM == 1 ? (int)prop.sharedMemPerBlockOptin
+                                   : std::min((int)prop.sharedMemPerBlockOptin, (int)prop.sharedMemPerMultiprocessor / CTAS_PER_SM - 1024);
+    h->x_need = (max_nb + 15) & ~15LL;
+    h->xg_off = (max_sum + 15) & ~15LL;                          // the slot always has room for the slow path's buffers
+    h->slot_stride = h->xg_off + 2 * h->x_need;
+    h->x_cap = (int)h->x_need;                                   // refined per solve: the program length decides whether it fits
     h->fac_cfg.block = 32 * NUM_WAYS;
     h->fac_cfg.smem_bytes = fac_smem_bytes(h->x_cap, L, MAX_OPS);       // refined per solve (program length)
-    h->fac_cfg.grid = std::max(1, std::min(P, prop.multiProcessorCount));
-    if (fac_configure(h->device, h->smem_cta) != 0) { g_detail = "cudaFuncSetAttribute(max dynamic shared memory) failed"; cudaGetLastError(); return AMGDD_ERR_CUDA; }
+    h->fac_cfg.grid = std::max(1, std::min(P, prop.multiProcessorCount * CTAS_PER_SM));
+    if (fac_configure(h->device, (int)prop.sharedMemPerBlockOptin) != 0) { g_detail = "cudaFuncSetAttribute(max dynamic shared memory) failed"; cudaGetLastError(); return AMGDD_ERR_CUDA; }
     if ((rc = dev_alloc(h, (void**)&h->d_ops, (size_t)MAX_OPS * sizeof(FacOp)))) return rc;
 
     if ((rc = dev_alloc(h, (void**)&h->d_workspace, (size_t)h->fac_cfg.grid * h->slot_stride * sizeof(double)))) return rc;
@@ -592,7 +586,17 @@ int amgdd_solve(amgdd_handle_t h, const double* b, double* x, int32_t num_cycles
         CUDA_TRY(cudaMemcpyAsync(h->d_ops, ops.data(), ops.size() * sizeof(FacOp), cudaMemcpyHostToDevice, h->stream));
         CUDA_TRY(cudaStreamSynchronize(h->stream));
         h->prog_nfac = num_fac_cycles; h->prog_nu = relax_sweeps; h->prog_nops = nops;
-        h->fac_cfg.smem_bytes = fac_smem_bytes(h->x_cap, L, nops);
+        // shared-memory vector buffers: as large as the largest level needs, but leave the L1 (which
+        // shares the SM's 228 KB with shared memory) room for the loads in flight: with less than
+        // ~48 KB of L1 the streaming rate of this kernel drops by 15% (profiles/).  Levels that do
+        // not fit are gathered through L1 from the workspace slot instead.
+        const int budget = std::min(h->smem_cta, env_int("AMGDD_SMEM_BUDGET", 180 * 1024));
+        long long cap = ((long long)budget - fac_smem_bytes(0, L, nops)) / 16;
+        cap = std::max(0LL, std::min(cap, h->x_need)) & ~15LL;
+        if (env_int("AMGDD_FORCE_GLOBAL_X", 0) > 0) cap = 0;
+        h->x_cap = (int)cap;
+        h->stats.x_cap = h->x_cap;
+        h->fac_cfg.smem_bytes = std::min(h->smem_cta, fac_smem_bytes(h->x_cap, L, nops) + env_int("AMGDD_EXTRA_SMEM", 0));
         h->stats.fac_smem_bytes = h->fac_cfg.smem_bytes;
     }
     FacParams prm;

@@ -44,12 +44,11 @@ struct LevInfo {           // shared-memory copy of the scalar part of DevLevel
     const int* gid;
     const double* dinv;
 };
-struct WayEnt {            // shared memory: what warp w needs to read stream s
-    const char* grp;
-    const char* hdr;
+struct WayEnt {            // shared memory: what warp w needs to read stream s (offsets from the stream base, sbase[s])
+    uint32_t grp_off128, hdr_off128;
     uint32_t n_all, n_real, nsl_all, nsl_real;
 };
-static_assert(sizeof(WayEnt) == 32 && sizeof(LevInfo) == 32, "shared-memory table layout");
+static_assert(sizeof(WayEnt) == 24 && sizeof(LevInfo) == 32, "shared-memory table layout");
 
 struct Grp { uint4 a, b, c; };     // values of steps 0,1 | values of steps 2,3 | column indices (narrow: c.x, c.y)
 
@@ -99,21 +98,26 @@ __device__ __forceinline__ double lds_f64(uint32_t a) {
 }
 __device__ __forceinline__ double mkdouble(uint32_t lo, uint32_t hi) { return __hiloint2double((int)hi, (int)lo); }
 
-// the two vector buffers: shared memory (XS) or the workspace slot
-template <bool XS> struct XBuf;
-template <> struct XBuf<true> {
-    uint32_t a;
-    __device__ __forceinline__ double ld(uint32_t i) const {
-        double v;
-        asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a + (i << 3)));
-        return v;
+// One of the two vector buffers.  A vector of level l lives in shared memory when |D-bar_l| <= x_cap
+// (gathers cost a few shared-memory wavefronts), otherwise in the workspace slot (gathers go through
+// L1).  x_cap is chosen so that the L1 keeps enough room for the loads in flight (fac_pick_x_cap).
+struct XB {
+    uint32_t a;            // shared address
+    double* p;             // the same buffer's twin in the workspace slot
+    bool s;                // which one is in use for this vector
+    template <bool GS> __device__ __forceinline__ double ldt(uint32_t i) const {
+        if (GS) {
+            double v;
+            asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a + (i << 3)));
+            return v;
+        }
+        return p[i];
     }
-    __device__ __forceinline__ void st(uint32_t i, double v) const { asm volatile("st.shared.f64 [%0], %1;" ::"r"(a + (i << 3)), "d"(v) : "memory"); }
-};
-template <> struct XBuf<false> {
-    double* p;
-    __device__ __forceinline__ double ld(uint32_t i) const { return p[i]; }
-    __device__ __forceinline__ void st(uint32_t i, double v) const { p[i] = v; }
+    __device__ __forceinline__ double ld(uint32_t i) const { return s ? ldt<true>(i) : ldt<false>(i); }
+    __device__ __forceinline__ void st(uint32_t i, double v) const {
+        if (s) asm volatile("st.shared.f64 [%0], %1;" ::"r"(a + (i << 3)), "d"(v) : "memory");
+        else p[i] = v;
+    }
 };
 
 __device__ __forceinline__ int stream_of(const FacOp& op) {           // 3 * level + {0: A, 1: P, 2: R}
@@ -122,16 +126,26 @@ __device__ __forceinline__ int stream_of(const FacOp& op) {           // 3 * lev
 }
 __device__ __forceinline__ bool real_rows_only(const FacOp& op) { return op.kind == OPK_RELAX || op.kind == OPK_RECALC; }
 __device__ __forceinline__ bool is_matvec(int kind) { return kind >= OPK_RELAX && kind <= OPK_INTERP; }
+// level of the vector a step gathers from / of the vector it leaves in the other buffer
+__device__ __forceinline__ int gather_level(const FacOp& op) { return op.kind == OPK_INTERP ? op.level + 1 : op.level; }
+__device__ __forceinline__ int out_level(const FacOp& op) { return op.kind == OPK_RESTRICT ? op.level + 1 : op.level; }
 
-template <bool XS, bool PROF>
+template <bool PROF>
 struct Worker {
     const FacParams* prm;
     const FacOp* ops;              // shared memory
     const LevInfo* lev;            // shared memory, L+1
     const WayEnt* wt;              // shared memory, [stream][way]
     const uint32_t* sflags;        // shared memory, per stream
-    XBuf<XS> xb0, xb1;
-    __device__ __forceinline__ XBuf<XS> xbuf_of(int b) const { return b ? xb1 : xb0; }
+    const char* const* sbase;      // shared memory, per stream: base address of the packed stream
+    uint32_t xs0, xs1;             // the two vector buffers in shared memory (x_cap doubles each)
+    double *xg0, *xg1;             // and in the workspace slot
+    int x_cap;
+    __device__ __forceinline__ XB xbuf_of(int b, int level) const {
+        XB x;
+        x.a = b ? xs1 : xs0; x.p = b ? xg1 : xg0; x.s = lev[level].n_bar <= x_cap;
+        return x;
+    }
     double* ws;                    // this CTA's workspace slot
     long long* prof;
     uint64_t pol;
@@ -179,7 +193,7 @@ struct Worker {
     }
     // level 0, first iteration: u_0 = 0, so the first sweep is delta = D^{-1} f (P:507 with A u = 0)
     __device__ __forceinline__ void first0(const FacOp op) {
-        const XBuf<XS> xo = xbuf_of(op.gbuf ^ 1);
+        const XB xo = xbuf_of(op.gbuf ^ 1, 0);
         const int n_real = lev[0].n_real, n_bar = lev[0].n_bar;
         const double* dinv = lev[0].dinv;
         double *u = U(0), *t = T(0);
@@ -194,7 +208,7 @@ struct Worker {
     // of the unit-lower / upper factors are contiguous (column-major).  The solve runs in place in
     // the output vector buffer.
     __device__ __forceinline__ void coarse(const FacOp op) {
-        const XBuf<XS> y = xbuf_of(op.gbuf ^ 1);
+        const XB y = xbuf_of(op.gbuf ^ 1, L);
         const int n = prm->nL;
         const double* __restrict__ lu = prm->lu;
         const double* f = F(L);
@@ -222,7 +236,7 @@ struct Worker {
     // work of a step that is not row-local to the mat-vec's rows (all threads; touches only data
     // that neither the gathers nor the epilogues of THIS step use, so no barrier follows it)
     __device__ __forceinline__ void pre_actions(const FacOp op) {
-        const XBuf<XS> xg = xbuf_of(op.gbuf), xo = xbuf_of(op.gbuf ^ 1);
+        const XB xg = xbuf_of(op.gbuf, gather_level(op)), xo = xbuf_of(op.gbuf ^ 1, out_level(op));
         const int l = op.level;
         if (op.kind == OPK_RELAX) {                 // ghost values are fixed (A4): carry them (u) or clear them (t)
             const int n_real = lev[l].n_real, n_bar = lev[l].n_bar;
@@ -248,28 +262,30 @@ struct Worker {
     }
 
     // one mat-vec of the program: the groups of this warp's way, in order
-    template <bool WIDE>
+    template <bool WIDE, bool GS>
     __device__ __forceinline__ void matvec(const FacOp op) {
         constexpr int GB = WIDE ? GROUP_BYTES_WIDE : GROUP_BYTES_NARROW;
         const long long tp0 = tick();
         const int kind = op.kind, l = op.level;
         const bool first = op.flags & OPF_FIRST, tsmem = op.flags & OPF_TSMEM, coarsest = op.flags & OPF_COARSEST;
-        const XBuf<XS> xg = xbuf_of(op.gbuf), xo = xbuf_of(op.gbuf ^ 1);
+        const XB xg = xbuf_of(op.gbuf, gather_level(op)), xo = xbuf_of(op.gbuf ^ 1, out_level(op));
         // ---- this warp's way of the stream, and of the next mat-vec's stream ----
         const WayEnt we = wt[stream_of(op) * NUM_WAYS + wid];
+        const char* const sb = sbase[stream_of(op)];
+        const char* const we_hdr = sb + 128ull * we.hdr_off128;
         const bool ronly = real_rows_only(op);
         const int n = (int)(ronly ? we.n_real : we.n_all);
         const int nsl = (int)(ronly ? we.nsl_real : we.nsl_all);
-        const char* const cur = we.grp;
+        const char* const cur = sb + 128ull * we.grp_off128;
         const char* const dummy = reinterpret_cast<const char*>(prm->lev);     // always readable (>= 1536 bytes)
         const char* nxt = dummy;
         const char* nxt_hdr = dummy;
         int n_next = 0;
-        if (XS && op.next_mat >= 0) {
+        if (op.next_mat >= 0 && (bool)(sflags[stream_of(ops[op.next_mat])] & STREAM_WIDE) == WIDE) {   // (the ring holds one group shape)
             const FacOp nop = ops[op.next_mat];
             const WayEnt w2 = wt[stream_of(nop) * NUM_WAYS + wid];
             n_next = (int)(real_rows_only(nop) ? w2.n_real : w2.n_all);
-            if (n_next > 0) { nxt = w2.grp; nxt_hdr = w2.hdr; }
+            if (n_next > 0) { const char* b2 = sbase[stream_of(nop)]; nxt = b2 + 128ull * w2.grp_off128; nxt_hdr = b2 + 128ull * w2.hdr_off128; }
         }
         const int next_last = n_next > 0 ? n_next - 1 : 0;
         // ---- groups of this mat-vec that are not in the ring yet (first mat-vec of a subdomain, or after a short one) ----
@@ -301,7 +317,7 @@ struct Worker {
         //   stage:  H  32 x 16 bytes  header of the next slice (after the last slice: slice 0 of the next mat-vec)
         //           C  3 x 32 x 8 bytes  operands e0 | e1 | e2 of the current slice's epilogue
         if (n == 0) { ring_valid = false; hdr_ready = false; tock(PROF_OP0 + kind, tp0); return; }
-        const char* const hdr = we.hdr + 16 * lane;
+        const char* const hdr = we_hdr + 16 * lane;
         const uint32_t stH = stage + 16 * lane, stC = stage + 512 + 8 * lane;
         const char* const hdr_after = nxt_hdr + 16 * lane;
         auto fetch_ctx = [&](uint32_t r) {
@@ -329,7 +345,7 @@ struct Worker {
 #ifdef AMGDD_EXP_NOGATHER
             const double x0 = __hiloint2double(c0, c1), x1 = __hiloint2double(c1, c2), x2 = __hiloint2double(c2, c3), x3 = __hiloint2double(c3, c0);
 #else
-            const double x0 = xg.ld(c0), x1 = xg.ld(c1), x2 = xg.ld(c2), x3 = xg.ld(c3);
+            const double x0 = xg.template ldt<GS>(c0), x1 = xg.template ldt<GS>(c1), x2 = xg.template ldt<GS>(c2), x3 = xg.template ldt<GS>(c3);
 #endif
             acc = fma(mkdouble(g.a.x, g.a.y), x0, acc);
             acc = fma(mkdouble(g.a.z, g.a.w), x1, acc);
@@ -391,11 +407,11 @@ struct Worker {
         // Blocks of D groups, double buffered in registers: WAIT for block j (buffer X), then issue
         // the burst of block j+1 into the other buffer (the next D groups of this mat-vec or, after
         // its last block, the first D groups of the next mat-vec), then consume block j while
-        // that burst is in flight.  All global loads of a warp share one hardware scoreboard, so
-        // a wait on any of them waits for all: the burst must not be issued before the data of
-        // block j has arrived.  That order is forced by a data dependence: the burst's base
-        // address is selected by a bit pattern of block j's first value that no finite matrix
-        // entry has (Inf/NaN exponent), so the address cannot be formed earlier.
+        // that burst is in flight.  All ordinary global loads of a warp share one hardware
+        // scoreboard, so a wait on any of them waits for all: the burst must not be issued before
+        // the data of block j has arrived.  That order is forced by a data dependence: the
+        // burst's base address is selected by a bit pattern of block j's first value that no
+        // finite matrix entry has (Inf/NaN exponent), so the address cannot be formed earlier.
         auto step = [&](Grp (&X)[D], Grp (&Y)[D], int p0) {
             const bool more = p0 + D < n;
             const bool never = (X[0].a.y & 0x7FF00000u) == 0x7FF00000u;
@@ -403,7 +419,11 @@ struct Worker {
             const int r0 = more ? p0 + D : 0, rlast = never ? 0 : (more ? n - 1 : next_last);
 #pragma unroll
             for (int d = 0; d < D; ++d) Y[d] = load_grp<WIDE>(rbase + (long long)(r0 + d < rlast ? r0 + d : rlast) * GB, lane, pol);
-            if (p0 + D <= n) {
+            if (left > D && p0 + D <= n) {              // no slice ends inside this block: straight-line code
+#pragma unroll
+                for (int d = 0; d < D; ++d) consume(X[d]);
+                left -= D;
+            } else if (p0 + D <= n) {
 #pragma unroll
                 for (int d = 0; d < D; ++d) {
                     consume(X[d]);
@@ -430,30 +450,29 @@ struct Worker {
     }
 };
 
-template <bool XS, bool PROF>
-__global__ void __launch_bounds__(NTHREADS, 1) fac_kernel(const FacParams prm) {
+template <bool PROF>
+__global__ void __launch_bounds__(NTHREADS, CTAS_PER_SM) fac_kernel(const FacParams prm) {
     extern __shared__ __align__(128) unsigned char smem[];
     const int L = prm.L, nstreams = 3 * (L + 1);
-    // shared-memory plan (fac_smem_bytes): control | ops | LevInfo | stream flags | way table | staging areas | two vector buffers
+    // shared-memory plan (fac_smem_bytes): control | ops | LevInfo | stream flags | stream bases | way table | staging areas | two vector buffers
     int* ctrl = reinterpret_cast<int*>(smem);
     FacOp* ops = reinterpret_cast<FacOp*>(smem + 128);
     LevInfo* lev = reinterpret_cast<LevInfo*>(smem + 128 + (((size_t)prm.nops * sizeof(FacOp) + 127) & ~(size_t)127));
     uint32_t* sflags = reinterpret_cast<uint32_t*>(lev + (L + 1));
-    WayEnt* wt = reinterpret_cast<WayEnt*>(reinterpret_cast<unsigned char*>(sflags) + (((size_t)nstreams * 4 + 127) & ~(size_t)127));
-    unsigned char* stage = reinterpret_cast<unsigned char*>(wt + (size_t)nstreams * NUM_WAYS);
+    const char** sbase = reinterpret_cast<const char**>(reinterpret_cast<unsigned char*>(sflags) + (((size_t)nstreams * 4 + 127) & ~(size_t)127));
+    WayEnt* wt = reinterpret_cast<WayEnt*>(reinterpret_cast<unsigned char*>(sbase) + (((size_t)nstreams * 8 + 127) & ~(size_t)127));
+    unsigned char* stage = reinterpret_cast<unsigned char*>(wt) + (((size_t)nstreams * NUM_WAYS * sizeof(WayEnt) + 127) & ~(size_t)127);
     double* xbuf = reinterpret_cast<double*>(stage + NUM_WAYS * STAGE_BYTES);
 
-    Worker<XS, PROF> W;
-    W.prm = &prm; W.ops = ops; W.lev = lev; W.wt = wt; W.sflags = sflags;
+    Worker<PROF> W;
+    W.prm = &prm; W.ops = ops; W.lev = lev; W.wt = wt; W.sflags = sflags; W.sbase = sbase;
     W.tid = threadIdx.x; W.lane = threadIdx.x & 31; W.wid = threadIdx.x >> 5; W.L = L;
     W.ws = prm.workspace + (size_t)blockIdx.x * prm.slot_stride;
-    if constexpr (XS) {
-        W.xb0.a = (uint32_t)__cvta_generic_to_shared(xbuf);
-        W.xb1.a = W.xb0.a + (uint32_t)prm.x_cap * 8u;
-    } else {
-        W.xb0.p = W.ws + prm.xg_off;
-        W.xb1.p = W.xb0.p + (prm.slot_stride - prm.xg_off) / 2;
-    }
+    W.xs0 = (uint32_t)__cvta_generic_to_shared(xbuf);
+    W.xs1 = W.xs0 + (uint32_t)prm.x_cap * 8u;
+    W.xg0 = W.ws + prm.xg_off;
+    W.xg1 = W.xg0 + (prm.slot_stride - prm.xg_off) / 2;
+    W.x_cap = prm.x_cap;
     W.prof = PROF ? prm.prof + (size_t)blockIdx.x * FAC_PROF_SLOTS : nullptr;
     W.pol = policy_evict_first();
     W.ring_valid = false; W.hdr_ready = false;
@@ -485,10 +504,10 @@ __global__ void __launch_bounds__(NTHREADS, 1) fac_kernel(const FacParams prm) {
             const char* base = sd->base;
             const WayDesc wd = sd->way[w];
             WayEnt e;
-            e.grp = base + 128ull * wd.grp_off128; e.hdr = base + 128ull * wd.hdr_off128;
+            e.grp_off128 = wd.grp_off128; e.hdr_off128 = wd.hdr_off128;
             e.n_all = wd.ngroups; e.n_real = wd.ngroups_real; e.nsl_all = wd.nslices; e.nsl_real = wd.nslices_real;
             wt[idx] = e;
-            if (w == 0) sflags[s] = sd->flags;
+            if (w == 0) { sflags[s] = sd->flags; sbase[s] = base; }
         }
         __syncthreads();
         W.tock(PROF_SETUP, ts0);
@@ -503,8 +522,9 @@ __global__ void __launch_bounds__(NTHREADS, 1) fac_kernel(const FacParams prm) {
             else {
                 W.pre_actions(op);
                 W.tock(PROF_PRE, tp0);
-                if (!XS && (sflags[stream_of(op)] & STREAM_WIDE)) W.template matvec<true>(op);
-                else W.template matvec<false>(op);
+                if (sflags[stream_of(op)] & STREAM_WIDE) W.template matvec<true, false>(op);
+                else if (lev[gather_level(op)].n_bar <= prm.x_cap) W.template matvec<false, true>(op);
+                else W.template matvec<false, false>(op);
             }
             if (!is_matvec(op.kind)) W.tock(PROF_OP0 + op.kind, tp0);
             W.sync();                                                    // the step is complete
@@ -566,29 +586,23 @@ int fac_smem_bytes(int x_cap, int L, int nops) {
     b += ((size_t)nops * sizeof(FacOp) + 127) & ~(size_t)127;
     b += (size_t)(L + 1) * sizeof(LevInfo);
     b += ((size_t)nstreams * 4 + 127) & ~(size_t)127;
-    b += (size_t)nstreams * NUM_WAYS * sizeof(WayEnt);
+    b += ((size_t)nstreams * 8 + 127) & ~(size_t)127;
+    b += ((size_t)nstreams * NUM_WAYS * sizeof(WayEnt) + 127) & ~(size_t)127;
     b += (size_t)NUM_WAYS * STAGE_BYTES;
     b += 2 * (size_t)x_cap * 8;
     return (int)b;
 }
 
 int fac_configure(int /*device*/, int max_smem_optin) {
-    cudaError_t e = cudaFuncSetAttribute(fac_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_optin);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(fac_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_optin);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(fac_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_optin);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(fac_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_optin);
+    cudaError_t e = cudaFuncSetAttribute(fac_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_optin);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fac_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_optin);
     return e == cudaSuccess ? 0 : (int)e;
 }
 
 void launch_fac(const FacParams& prm, const FacLaunch& cfg, void* stream) {
     cudaStream_t st = (cudaStream_t)stream;
-    if (prm.x_cap > 0) {
-        if (prm.prof) fac_kernel<true, true><<<cfg.grid, cfg.block, cfg.smem_bytes, st>>>(prm);
-        else fac_kernel<true, false><<<cfg.grid, cfg.block, cfg.smem_bytes, st>>>(prm);
-    } else {
-        if (prm.prof) fac_kernel<false, true><<<cfg.grid, cfg.block, cfg.smem_bytes, st>>>(prm);
-        else fac_kernel<false, false><<<cfg.grid, cfg.block, cfg.smem_bytes, st>>>(prm);
-    }
+    if (prm.prof) fac_kernel<true><<<cfg.grid, cfg.block, cfg.smem_bytes, st>>>(prm);
+    else fac_kernel<false><<<cfg.grid, cfg.block, cfg.smem_bytes, st>>>(prm);
 }
 
 }  // namespace amgdd

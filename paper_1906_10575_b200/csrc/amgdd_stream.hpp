@@ -40,7 +40,17 @@
 
 namespace amgdd {
 
-constexpr int NUM_WAYS = 16;                 // warps of the AlgFAC kernel = sub-streams per matrix
+#ifndef AMGDD_RING_DEPTH
+#define AMGDD_RING_DEPTH 3
+#endif
+#ifndef AMGDD_WAYS
+#define AMGDD_WAYS 16
+#endif
+#ifndef AMGDD_CTAS_PER_SM
+#define AMGDD_CTAS_PER_SM 1
+#endif
+constexpr int NUM_WAYS = AMGDD_WAYS;          // warps of an AlgFAC CTA = sub-streams per matrix
+constexpr int CTAS_PER_SM = AMGDD_CTAS_PER_SM;   // resident AlgFAC CTAs per SM (each works on its own subdomain)
 constexpr int SLICE_ROWS = 32;
 constexpr int GROUP_STEPS = 4;
 constexpr int GROUP_BYTES_NARROW = 1280;
@@ -50,7 +60,7 @@ constexpr int NARROW_MAX_COLS = 65536;       // uint16 column indices
 constexpr int DEFAULT_WINDOW = 256;
 constexpr int MAX_WINDOW = 1 << 20;
 constexpr uint32_t NO_ROW = 0xFFFFFFFFu;
-constexpr int RING_DEPTH = 3;                // groups per register block; a warp holds two blocks (one in flight, one being consumed)
+constexpr int RING_DEPTH = AMGDD_RING_DEPTH;  // groups per register block = groups per burst of loads; a warp holds two blocks
 
 inline int group_bytes(bool wide) { return wide ? GROUP_BYTES_WIDE : GROUP_BYTES_NARROW; }
 
