@@ -20,7 +20,7 @@ EXPORTS = [
     "amgdd_setup", "amgdd_solve", "amgdd_solve_host", "amgdd_residual_norm", "amgdd_set_stream", "amgdd_destroy",
     "amgdd_strerror", "amgdd_last_error_detail", "amgdd_num_levels", "amgdd_level_size", "amgdd_get_cf",
     "amgdd_get_level_matrix", "amgdd_composite_size", "amgdd_get_composite", "amgdd_get_stats",
-    "amgdd_last_solve_profile", "amgdd_pack_stream", "amgdd_debug_fac_cycles",
+    "amgdd_last_solve_profile", "amgdd_pack_stream", "amgdd_debug_fac_cycles", "amgdd_debug_fac_op_cycles",
 ]
 
 
@@ -66,6 +66,7 @@ def _load():
     L.amgdd_get_stats.argtypes = [_vp, ctypes.POINTER(AmgddStats)]
     L.amgdd_last_solve_profile.argtypes = [_vp, _vp, _vp]
     L.amgdd_debug_fac_cycles.argtypes = [_vp, _vp, _i32]
+    L.amgdd_debug_fac_op_cycles.argtypes = [_vp, _vp, _i32, _vp]
     L.amgdd_pack_stream.argtypes = [_i32, _i32, _vp, _vp, _vp, _vp, _i32, _i32, _vp, _i64, _vp, _vp]
     return L
 
@@ -244,6 +245,18 @@ def amgdd_debug_fac_cycles(h: Handle, reset=True) -> dict:
     out = (ctypes.c_int64 * 16)()
     _check(lib.amgdd_debug_fac_cycles(h._h, out, int(reset)))
     return dict(zip(FAC_CYCLE_NAMES, [int(v) for v in out]))
+
+
+OP_KIND_NAMES = ["begin", "first0", "relax", "At", "restrict", "recalc", "interp", "coarse", "end"]
+
+
+def amgdd_debug_fac_op_cycles(h: Handle, n=256):
+    """Per-step SM cycles of the AlgFAC program (needs AMGDD_FAC_PROFILE=1 at setup): list of
+    (kind name, level, step cycles, barrier-wait cycles)."""
+    out = np.zeros(2 * n, dtype=np.int64)
+    kl = np.full(n, -1, dtype=np.int32)
+    _check(lib.amgdd_debug_fac_op_cycles(h._h, out.ctypes.data, n, kl.ctypes.data))
+    return [(OP_KIND_NAMES[k // 256], int(k % 256), int(out[j]), int(out[n + j])) for j, k in enumerate(kl) if k >= 0]
 
 
 def amgdd_last_solve_profile(h: Handle):

@@ -65,6 +65,7 @@ struct amgdd_handle_s {
     FacOp* d_ops = nullptr;                     // the program of one subdomain (fac_build_program)
     int prog_nfac = -1, prog_nu = -1, prog_nops = 0;
     int* d_counter = nullptr;
+    long long* d_prof_ops = nullptr;
     long long* d_prof = nullptr;                // AMGDD_FAC_PROFILE=1: per-CTA cycle counters of the AlgFAC kernel
     double* d_lu = nullptr; int* d_rowperm = nullptr;
     double* d_partial = nullptr; int partial_cap = 0;
@@ -413,6 +414,9 @@ int finish_tables(amgdd_handle_s* h) {
         const size_t bytes = (size_t)h->fac_cfg.grid * FAC_PROF_SLOTS * sizeof(long long);
         if ((rc = dev_alloc(h, (void**)&h->d_prof, bytes))) return rc;
         CUDA_TRY(cudaMemset(h->d_prof, 0, bytes));
+        const size_t b2 = (size_t)h->fac_cfg.grid * 2 * MAX_OPS * sizeof(long long);
+        if ((rc = dev_alloc(h, (void**)&h->d_prof_ops, b2))) return rc;
+        CUDA_TRY(cudaMemset(h->d_prof_ops, 0, b2));
     }
     if ((rc = upload(h, &h->d_lu, h->H.lu.data(), h->H.lu.size()))) return rc;
     if ((rc = upload(h, &h->d_rowperm, h->H.rowperm.data(), h->H.rowperm.size()))) return rc;
@@ -610,6 +614,7 @@ int amgdd_solve(amgdd_handle_t h, const double* b, double* x, int32_t num_cycles
     prm.lu = h->d_lu; prm.rowperm = h->d_rowperm; prm.nL = (int)h->H.nL;
     prm.x_cap = h->x_cap;
     prm.prof = h->d_prof;
+    prm.prof_ops = h->d_prof_ops;
     long long launches[3] = {0, 0, 0};
     mark();
     for (int k = 0; k < num_cycles; ++k) {
@@ -726,6 +731,28 @@ int amgdd_debug_fac_cycles(amgdd_handle_t h, int64_t out[16], int32_t reset) {
     CUDA_TRY(cudaMemcpy(host.data(), h->d_prof, cnt * sizeof(long long), cudaMemcpyDeviceToHost));
     for (size_t i = 0; i < cnt; ++i) out[i % FAC_PROF_SLOTS] += host[i];
     if (reset) CUDA_TRY(cudaMemset(h->d_prof, 0, cnt * sizeof(long long)));
+    return AMGDD_SUCCESS;
+}
+
+int amgdd_debug_fac_op_cycles(amgdd_handle_t h, int64_t* out, int32_t n, int32_t* kinds_levels) {
+    if (bad_handle(h) || !out) return AMGDD_ERR_BAD_ARG;
+    if (!h->d_prof_ops) { g_detail = "set AMGDD_FAC_PROFILE=1 before amgdd_setup"; return AMGDD_ERR_BAD_ARG; }
+    const size_t cnt = (size_t)h->fac_cfg.grid * 2 * MAX_OPS;
+    std::vector<long long> host(cnt);
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    CUDA_TRY(cudaMemcpy(host.data(), h->d_prof_ops, cnt * sizeof(long long), cudaMemcpyDeviceToHost));
+    for (int i = 0; i < 2 * n; ++i) out[i] = 0;
+    for (int b = 0; b < h->fac_cfg.grid; ++b)
+        for (int j = 0; j < n && j < MAX_OPS; ++j) {
+            out[j] += host[(size_t)b * 2 * MAX_OPS + j];
+            out[n + j] += host[(size_t)b * 2 * MAX_OPS + MAX_OPS + j];
+        }
+    if (kinds_levels) {
+        std::vector<FacOp> ops((size_t)std::max(1, h->prog_nops));
+        fac_build_program(h->H.L, h->prog_nfac, h->prog_nu, ops.data());
+        for (int j = 0; j < n && j < h->prog_nops; ++j) kinds_levels[j] = ops[j].kind * 256 + ops[j].level;
+    }
+    CUDA_TRY(cudaMemset(h->d_prof_ops, 0, cnt * sizeof(long long)));
     return AMGDD_SUCCESS;
 }
 

@@ -527,7 +527,10 @@ __global__ void __launch_bounds__(NTHREADS, CTAS_PER_SM) fac_kernel(const FacPar
                 else W.template matvec<false, false>(op);
             }
             if (!is_matvec(op.kind)) W.tock(PROF_OP0 + op.kind, tp0);
+            long long tq0 = 0;
+            if (PROF && threadIdx.x == 0 && prm.prof_ops) { tq0 = clock64(); prm.prof_ops[(size_t)blockIdx.x * 2 * MAX_OPS + j] += tq0 - tp0; }
             W.sync();                                                    // the step is complete
+            if (PROF && threadIdx.x == 0 && prm.prof_ops) prm.prof_ops[(size_t)blockIdx.x * 2 * MAX_OPS + MAX_OPS + j] += clock64() - tq0;
         }
     }
     W.tock(PROF_TOTAL, tk0);

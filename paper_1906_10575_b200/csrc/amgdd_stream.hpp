@@ -152,6 +152,7 @@ struct FacParams {
     int nL;
     int x_cap;                 // doubles in each of the two shared-memory vector buffers (0: vectors in global memory)
     long long* prof;           // optional: gridDim.x * FAC_PROF_SLOTS cycle counters (debugging), or nullptr
+    long long* prof_ops;       // optional: gridDim.x * 2 * MAX_OPS: cycles of every step of the program | barrier wait after it
 };
 constexpr int FAC_PROF_SLOTS = 16;
 

@@ -1,0 +1,61 @@
+"""Parity at BASELINE.json's full sizes, in the launch configuration bench.py times (configs 4 and
+5; configs 1 and 2 run at full size in test_gpu_parity.py).  The oracle cannot run all subdomains of
+these in a test's time, so it computes SAMPLED outputs: Alg. 2's global residual and restriction in
+full, AlgFAC on a sample of subdomains; every cycle both sides start from the same iterate (the
+library's), and x is compared on the owned dofs of the sampled subdomains.  The residual norm of
+the library's iterate is checked against the oracle's evaluation of the same vector."""
+import numpy as np
+import pytest
+
+import workloads as wl
+from oracle import Oracle, max_threads
+
+pytestmark = pytest.mark.gpu
+RTOL = 1e-10
+
+
+def _run(cfg, num_cycles, nsample):
+    import torch
+    import paper_1906_10575_b200 as m
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    p = wl.make_config(cfg)
+    h = m.amgdd_setup(p.n, p.rowptr, p.colind, p.vals, p.num_subdomains, p.owner, p.eta, p.num_ghost, p.max_levels,
+                      p.theta, p.coarse_max)
+    o = Oracle(p.n, p.rowptr, p.colind, p.vals, p.theta, p.max_levels, p.coarse_max)
+    o.set_partition(p.num_subdomains, p.owner, p.eta, p.num_ghost)
+    # index-exact hierarchy and composite grids of the sampled subdomains
+    subs = np.unique(np.linspace(0, p.num_subdomains - 1, nsample).astype(np.int32))
+    assert m.amgdd_num_levels(h) == o.num_levels
+    for l in range(o.num_levels):
+        assert m.amgdd_level_size(h, l) == o.level_size(l)
+        for q in subs[:4]:
+            real, ghost = m.amgdd_get_composite(h, int(q), l)
+            oreal, oghost = o.composite(int(q), l)
+            assert np.array_equal(real, oreal) and np.array_equal(ghost, oghost)
+    b = torch.from_numpy(p.b).cuda()
+    x = torch.zeros(p.n, dtype=torch.float64, device="cuda")
+    owned = np.isin(p.owner, subs)
+    nt = max_threads()
+    for k in range(num_cycles):
+        x_in = x.cpu().numpy().copy()
+        res = m.amgdd_solve(h, b, x, 1, p.num_fac_cycles, p.relax_sweeps)
+        x_out = x.cpu().numpy()
+        xo = x_in.copy()
+        o.cycle(p.b, xo, p.num_fac_cycles, p.relax_sweeps, subdomains=subs, nthreads=nt)
+        assert o.dropped() == 0
+        scale = np.abs(xo[owned]).max()
+        err = np.abs(x_out[owned] - xo[owned]).max()
+        r_in, r_out = o.residual_norm(p.b, x_in), o.residual_norm(p.b, x_out)
+        print(f"{p.name} cycle {k + 1}: |dx|_inf/|x|_inf on {len(subs)} subdomains = {err / scale:.2e}; "
+              f"resnorm rel diff in {abs(res[0] - r_in) / r_in:.2e} out {abs(res[1] - r_out) / r_out:.2e}")
+        assert err <= RTOL * scale
+        assert abs(res[0] - r_in) <= RTOL * r_in and abs(res[1] - r_out) <= RTOL * r_out
+    m.amgdd_destroy(h)
+
+
+def test_config4_fullsize_sampled():
+    _run(4, 2, 8)
+
+
+def test_config5_fullsize_sampled():
+    _run(5, 2, 16)

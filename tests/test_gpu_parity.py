@@ -158,6 +158,23 @@ def test_fac_cycles_and_sweeps(nfac, nu):
     run_parity(wl.make_config(2, 32), 3, nfac=nfac, nu=nu)
 
 
+@pytest.mark.parametrize("env", [{"AMGDD_FORCE_GLOBAL_X": "1"}, {"AMGDD_SMEM_BUDGET": "49152"}])
+def test_vector_buffer_placements(env, monkeypatch):
+    """The three mat-vec variants of the kernel: all level vectors gathered through L1 from the
+    workspace slot, and a small shared-memory budget under which only the coarser levels live in
+    shared memory (the default run keeps all of them there)."""
+    for k, v in env.items():
+        monkeypatch.setenv(k, v)
+    run_parity(wl.make_config(4, 48), 3)
+    run_parity(wl.make_config(2, 32), 2, nfac=2, nu=2)
+
+
+def test_wide_column_indices():
+    # one subdomain that covers a 272 x 272 grid: |D-bar_0| = 73984 > 65535, so level 0 is packed
+    # with 32-bit column indices (and gathered from the workspace slot)
+    run_parity(wl.make_config(1, 272, parts_per_dim=1), 2)
+
+
 def test_ragged_partition_and_odd_sizes():
     # 33 = 17 + 16: ragged blocks; 3 x 3 blocks of a 37 x 37 grid
     run_parity(wl.make_config(1, 37, parts_per_dim=3), 3)
