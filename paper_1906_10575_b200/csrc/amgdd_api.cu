@@ -291,9 +291,10 @@ StreamDesc make_desc(const char* base, const StreamLayout& lay) {
 }
 
 int upload_packed(amgdd_handle_s* h, const HostCsr& M, const double* aux, char** dptr, StreamLayout& lay, const char* what, int l) {
+    const int window = what[0] == 'A' ? h->window : std::min(h->window, THIN_WINDOW);
     PackedLevelStream ps;
     i64 bad = -1;
-    if (!pack_global_stream(M, aux, h->window, ps, bad)) { g_detail = "a level matrix has more than 2^31-1 nonzeros"; return AMGDD_ERR_INDEX_RANGE; }
+    if (!pack_global_stream(M, aux, window, ps, bad)) { g_detail = "a level matrix has more than 2^31-1 nonzeros"; return AMGDD_ERR_INDEX_RANGE; }
     if (bad >= 0) {
         g_detail = std::string("row ") + std::to_string(bad) + " of " + what + "_" + std::to_string(l) + " has more than 65535 entries";
         return AMGDD_ERR_INDEX_RANGE;

@@ -168,8 +168,8 @@ void CompositeBuilder::plan(int p, SubdomainBlob& out) {
             }
         i64 bad = -1;
         layout_stream(A, nb, nb, true, window_, nr, b.A, bad);
-        layout_stream(P, nb, nbc, false, window_, nb, b.P, bad);
-        layout_stream(R, nbc, nb, true, window_, nbc, b.R, bad);
+        layout_stream(P, nb, nbc, false, thin_window(), nb, b.P, bad);
+        layout_stream(R, nbc, nb, true, thin_window(), nbc, b.R, bad);
         if (bad >= 0 && out.too_long_row < 0) { out.too_long_row = bad; out.too_long_level = l; }
     }
     // blob layout
@@ -211,13 +211,13 @@ void CompositeBuilder::fill(const SubdomainBlob& plan, char* dst) {
         aux_.assign((size_t)nb, 0.0);                                    // ghost rows never relax (A4)
         for (i32 i = 0; i < nr; ++i) aux_[i] = dinv[i];
         write_stream(nb, A_[l].rp.data(), A_[l].ci.data(), A_[l].v.data(), aux_.data(), b.A.wide, nr, window_, dst + b.A.off);
-        write_stream(nb, P_[l].rp.data(), P_[l].ci.data(), P_[l].v.data(), nullptr, b.P.wide, nb, window_, dst + b.P.off);
+        write_stream(nb, P_[l].rp.data(), P_[l].ci.data(), P_[l].v.data(), nullptr, b.P.wide, nb, thin_window(), dst + b.P.off);
         {   // R_l rows are the points of level l+1: aux = their l1 diagonal (real points), 0 on ghosts
             const BlockLayout& c = plan.lev[l + 1];
             const HostLevel& lc = H_.lv[l + 1];
             auxr_.assign((size_t)nbc, 0.0);
             for (i32 i = 0; i < c.n_real; ++i) auxr_[i] = lc.dinv[real_[l + 1][i]];
-            write_stream(nbc, R_[l].rp.data(), R_[l].ci.data(), R_[l].v.data(), auxr_.data(), b.R.wide, nbc, window_, dst + b.R.off);
+            write_stream(nbc, R_[l].rp.data(), R_[l].ci.data(), R_[l].v.data(), auxr_.data(), b.R.wide, nbc, thin_window(), dst + b.R.off);
         }
     }
 }

@@ -33,6 +33,9 @@ namespace {
 
 constexpr int NTHREADS = 32 * NUM_WAYS;
 constexpr int D = RING_DEPTH;
+#ifndef AMGDD_SINGLE_BUFFER
+#define AMGDD_SINGLE_BUFFER 0
+#endif
 constexpr int STAGE_BYTES = 512 + 3 * 256;     // per warp: one slice header + three operand vectors of 32 doubles
 
 // slots of the optional per-CTA cycle counters (FAC_PROF_SLOTS each; amgdd_debug_fac_cycles)
@@ -417,32 +420,46 @@ struct Worker {
             const bool never = (X[0].a.y & 0x7FF00000u) == 0x7FF00000u;
             const char* rbase = never ? dummy : (more ? cur : nxt);
             const int r0 = more ? p0 + D : 0, rlast = never ? 0 : (more ? n - 1 : next_last);
+#if !AMGDD_SINGLE_BUFFER
 #pragma unroll
             for (int d = 0; d < D; ++d) Y[d] = load_grp<WIDE>(rbase + (long long)(r0 + d < rlast ? r0 + d : rlast) * GB, lane, pol);
-            if (left > D && p0 + D <= n) {              // no slice ends inside this block: straight-line code
+#endif
+            const int nv = n - p0 < D ? n - p0 : D;     // groups of this block (the last block of a mat-vec may be short)
+            if (left > nv && nv == D) {                 // no slice ends inside this block: straight-line code
 #pragma unroll
                 for (int d = 0; d < D; ++d) consume(X[d]);
                 left -= D;
-            } else if (p0 + D <= n) {
-#pragma unroll
-                for (int d = 0; d < D; ++d) {
-                    consume(X[d]);
-                    if (--left == 0) slice_end();
-                }
             } else {
+                // general case: consume up to the next slice end, run the epilogue (ONE copy of its code per
+                // buffer: the kernel's instruction footprint matters), resume behind it
+                int d = 0;
+                bool ended;
+                do {
+                    ended = false;
 #pragma unroll
-                for (int d = 0; d < D - 1; ++d)
-                    if (p0 + d < n) {
-                        consume(X[d]);
-                        if (--left == 0) slice_end();
-                    }
+                    for (int dd = 0; dd < D; ++dd)
+                        if (!ended && dd >= d && dd < nv) {
+                            consume(X[dd]);
+                            d = dd + 1;
+                            if (--left == 0) ended = true;
+                        }
+                    if (ended) slice_end();
+                } while (ended && d < nv);
             }
+#if AMGDD_SINGLE_BUFFER
+#pragma unroll
+            for (int d = 0; d < D; ++d) X[d] = load_grp<WIDE>(rbase + (long long)(r0 + d < rlast ? r0 + d : rlast) * GB, lane, pol);
+#endif
         };
         int ph = phase;
         for (int p0 = 0; p0 < n; p0 += D) {
+#if AMGDD_SINGLE_BUFFER
+            step(ra, ra, p0);
+#else
             if (ph == 0) step(ra, rb, p0);
             else step(rb, ra, p0);
             ph ^= 1;
+#endif
         }
         phase = ph;
         ring_valid = n_next > 0;

@@ -134,6 +134,9 @@ private:
     const std::vector<i32>& owner_;
     const std::vector<std::vector<i32>>& owned_;
     int eta_, nghost_, window_, p_ = -1;
+    // P_l and R_l have a few entries per row: their slices end after one or two groups, and every slice end
+    // touches its 32 rows' vector entries; rows of one slice are kept within a few cache lines
+    int thin_window() const { return window_ < THIN_WINDOW ? window_ : THIN_WINDOW; }
     std::vector<std::vector<i32>> real_, ghost_;
     std::vector<LocalCsr> A_, P_, R_;                 // local matrices of the subdomain planned last
     // epoch-stamped global->local maps, one per level

@@ -58,6 +58,10 @@ constexpr int GROUP_BYTES_WIDE = 1536;
 constexpr int HEADER_BYTES = 512;
 constexpr int NARROW_MAX_COLS = 65536;       // uint16 column indices
 constexpr int DEFAULT_WINDOW = 256;
+#ifndef AMGDD_THIN_WINDOW
+#define AMGDD_THIN_WINDOW 256
+#endif
+constexpr int THIN_WINDOW = AMGDD_THIN_WINDOW;    // sort window of the P_l / R_l streams
 constexpr int MAX_WINDOW = 1 << 20;
 constexpr uint32_t NO_ROW = 0xFFFFFFFFu;
 constexpr int RING_DEPTH = AMGDD_RING_DEPTH;  // groups per register block = groups per burst of loads; a warp holds two blocks
