@@ -17,12 +17,15 @@
 // (= column) order, so there is no cross-lane reduction and every row sum has one fixed summation
 // order (run-to-run identical results); a row-local epilogue applies the Alg. 4 update.
 //
-// VECTORS.  The gather vector of a mat-vec lives in one of two shared-memory buffers; the epilogue
-// writes the gather vector of the NEXT step into the other (u after interpolation for the
-// relaxation, t for the A t step, w for the restriction, ...), so no step needs a staging pass and
-// there is exactly one CTA barrier per step.  u, t, s, f of all levels are kept in a per-CTA
-// workspace slot in global memory (L2 resident); the epilogue's operands are fetched when a slice
-// starts and used when it ends.
+// VECTORS.  The gather vector of a mat-vec lives in one of two vector buffers; the epilogue writes
+// the gather vector of the NEXT step into the other (u after interpolation for the relaxation, t
+// for the A t step, w for the restriction, ...), so no step needs a staging pass and there is
+// exactly one CTA barrier per step.  A buffer is in shared memory for the levels that fit the
+// shared-memory budget (the L1 must keep ~44 KB for the loads in flight) and in the workspace
+// slot, gathered through L1, for larger ones.  u, t, s, f of all levels are kept in a per-CTA
+// workspace slot in global memory (L2 resident); a slice's header and the operands of its epilogue
+// are staged in shared memory by cp.async one slice ahead (own scoreboard: waiting for them does
+// not wait for the ring).
 #include "amgdd_stream.hpp"
 
 #include <cuda_runtime.h>
