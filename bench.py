@@ -238,6 +238,20 @@ def run_b200(args, p, rank, world, local_rank):
     clocks = sampler.stop()
     fac_avg_ms = float(np.mean(fac_ms))
 
+    # ---- context: the paper's comparison method, one AMG V(1,1)-cycle on the same hierarchy (Alg. 1; Fig. 14-15) ----
+    xv = torch.zeros(p.n, dtype=torch.float64, device="cuda")
+    res_v = m.amgdd_vcycle(h, b, xv, p.num_cycles, 1, 1)
+    for _ in range(2):
+        m.amgdd_vcycle(h, b, xv, 1, 1, 1, want_norms=False)
+    barrier()
+    e0.record(stream)
+    for _ in range(args.steps):
+        m.amgdd_vcycle(h, b, xv, 1, 1, 1, want_norms=False)
+    e1.record(stream)
+    barrier()
+    vcycle_ms = e0.elapsed_time(e1) / args.steps
+    del xv
+
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region ----
     bh = torch.from_numpy(p.b).pin_memory()
     xh = torch.zeros(p.n, dtype=torch.float64).pin_memory()
@@ -282,6 +296,13 @@ def run_b200(args, p, rank, world, local_rank):
             "residual_drop_per_cycle": drops,
             "residual_norms": res.tolist(),
             "phase_ms_per_step": {"fac_kernel": fac_avg_ms},
+            "amg_vcycle_context": {
+                "what": "one AMG V(1,1)-cycle (Alg. 1) on the same hierarchy and smoother, whole-level kernels, this GPU",
+                "ms_per_cycle": vcycle_ms, "residual_drop_per_cycle": (res_v[1:] / res_v[:-1]).tolist(),
+                "speedup_S_of_amgdd_over_amg": vcycle_ms / ms_step,
+                "amgdd_asymptotic_factor_rho": float(np.prod(drops[-3:]) ** (1.0 / 3.0)),
+                "effective_factor_rho_pow_S": float((np.prod(drops[-3:]) ** (1.0 / 3.0)) ** (vcycle_ms / ms_step)),
+            },
             "roofline": {
                 "bound": "hbm", "kernel": "fac_kernel (persistent AlgFAC, a3-a10)", "achieved": achieved, "peak": peak,
                 "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,

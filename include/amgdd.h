@@ -130,6 +130,15 @@ int amgdd_solve(amgdd_handle_t h, const double* b, double* x, int32_t num_cycles
 int amgdd_solve_host(amgdd_handle_t h, const double* b_host, double* x_host, int32_t num_cycles,
                      int32_t num_fac_cycles, int32_t relax_sweeps, double* resnorm_host);
 
+/* amgdd_vcycle -- num_cycles AMG V(nu1,nu2)-cycles on the same hierarchy (Alg. 1): the method the
+ * paper compares AMG-DD with (one V(1,1)-cycle against one AMG-DD iteration, Fig. 14).  Whole-level
+ * kernels, no subdomains: l1-Jacobi relaxation (the same as in amgdd_solve), r = f - A u, restriction with
+ * P^T, dense solve on the coarsest level, interpolation.  b, x DEVICE (x in/out); resnorm_host HOST,
+ * num_cycles+1 entries or NULL (asynchronous).  nu1, nu2 >= 0, nu1 + nu2 >= 1.  The first call uploads A_l
+ * and P_l of all levels as CSR (memory: about 12 bytes per nonzero of the hierarchy). */
+int amgdd_vcycle(amgdd_handle_t h, const double* b, double* x, int32_t num_cycles, int32_t nu1, int32_t nu2,
+                 double* resnorm_host);
+
 /* || b - A_0 x ||_2 (metric of Fig. 6; reading A16).  b, x DEVICE; out HOST. Synchronises. */
 int amgdd_residual_norm(amgdd_handle_t h, const double* b, const double* x, double* out_host);
 
@@ -206,7 +215,8 @@ int amgdd_last_solve_profile(amgdd_handle_t h, double ms[4], int64_t launches[3]
  *   rows (ghost carry, zeroing, staging)  [3] mat-vec start-up (first groups, first header)
  *   [4] whole kernel  [5] residual gather (a3)  [6] matrix-free first sweep of level 0
  *   [7..11] whole mat-vec steps: relax, A t, restrict, recalculate, interpolate
- *   [12] coarse solve  [13] owned update (a10).
+ *   [12] coarse solve  [13] owned update (a10)  [14] waits for a slice's staged header / operands
+ *   [15] waits for a block of the register ring (HBM latency).
  * Returns AMGDD_ERR_BAD_ARG if profiling was not enabled.  Timed runs must not enable it. */
 int amgdd_debug_fac_cycles(amgdd_handle_t h, int64_t out[16], int32_t reset);
 /* Same switch: SM cycles of every step of the AlgFAC program (thread 0 of each CTA, summed over CTAs and

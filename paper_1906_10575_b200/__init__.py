@@ -17,7 +17,7 @@ from . import build as _build
 _vp, _i32, _i64, _f64 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_double
 
 EXPORTS = [
-    "amgdd_setup", "amgdd_solve", "amgdd_solve_host", "amgdd_residual_norm", "amgdd_set_stream", "amgdd_destroy",
+    "amgdd_setup", "amgdd_solve", "amgdd_solve_host", "amgdd_vcycle", "amgdd_residual_norm", "amgdd_set_stream", "amgdd_destroy",
     "amgdd_strerror", "amgdd_last_error_detail", "amgdd_num_levels", "amgdd_level_size", "amgdd_get_cf",
     "amgdd_get_level_matrix", "amgdd_composite_size", "amgdd_get_composite", "amgdd_get_stats",
     "amgdd_last_solve_profile", "amgdd_pack_stream", "amgdd_debug_fac_cycles", "amgdd_debug_fac_op_cycles",
@@ -52,6 +52,7 @@ def _load():
     L.amgdd_solve.argtypes = [_vp, _vp, _vp, _i32, _i32, _i32, _vp]
     L.amgdd_solve_host.argtypes = [_vp, _vp, _vp, _i32, _i32, _i32, _vp]
     L.amgdd_residual_norm.argtypes = [_vp, _vp, _vp, _vp]
+    L.amgdd_vcycle.argtypes = [_vp, _vp, _vp, _i32, _i32, _i32, _vp]
     L.amgdd_set_stream.argtypes = [_vp, _vp]
     L.amgdd_destroy.argtypes = [_vp]
     L.amgdd_strerror.restype = ctypes.c_char_p
@@ -151,6 +152,14 @@ def amgdd_solve_host(h: Handle, b_host, x_host, num_cycles, num_fac_cycles=2, re
     return res
 
 
+def amgdd_vcycle(h: Handle, b, x, num_cycles, nu1=1, nu2=1, want_norms=True):
+    """amgdd_vcycle: AMG V(nu1,nu2)-cycles (Alg. 1) on the handle's hierarchy; b, x float64 CUDA tensors."""
+    n = amgdd_level_size(h, 0)[0]
+    res = np.empty(num_cycles + 1, dtype=np.float64) if want_norms else None
+    _check(lib.amgdd_vcycle(h._h, _dev_ptr(b, n), _dev_ptr(x, n), num_cycles, nu1, nu2, res.ctypes.data if want_norms else None))
+    return res
+
+
 def amgdd_residual_norm(h: Handle, b, x) -> float:
     n = amgdd_level_size(h, 0)[0]
     out = _f64()
@@ -237,7 +246,7 @@ def amgdd_pack_stream(rowptr, colind, vals, wide=False, n_real=None, aux=None, w
 
 
 FAC_CYCLE_NAMES = ["sync", "fetch_subdomain", "pre_actions", "matvec_startup", "total", "gather_a3", "first0", "op_relax", "op_At",
-                   "op_restrict", "op_recalc", "op_interp", "coarse", "update_a10", "unused14", "unused15"]
+                   "op_restrict", "op_recalc", "op_interp", "coarse", "update_a10", "wait_slice_operands", "wait_ring_block"]
 
 
 def amgdd_debug_fac_cycles(h: Handle, reset=True) -> dict:

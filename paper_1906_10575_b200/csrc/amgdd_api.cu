@@ -32,6 +32,10 @@ struct GlobalLevelDev {          // the single device copy of a whole level
     char* sA = nullptr; char* sP = nullptr; char* sR = nullptr;
     StreamLayout layA, layP, layR;
     double* dinv = nullptr; int* ident = nullptr;
+    // AMG V-cycle (amgdd_vcycle; uploaded on first use): A_l and P_l as plain CSR, the l1 diagonal, level vectors
+    int* p_rp = nullptr; int* p_ci = nullptr; double* p_v = nullptr;
+    int lanes_p = 2;
+    double* vdinv = nullptr; double *vu0 = nullptr, *vu1 = nullptr, *vf = nullptr, *vr = nullptr;
 };
 
 struct SubMeta {                 // host-side record of one subdomain's blob
@@ -75,6 +79,7 @@ struct amgdd_handle_s {
     double prof_ms[4] = {0, 0, 0, 0};
     long long prof_launches[3] = {0, 0, 0};
     std::string detail;
+    bool vcycle_ready = false;
 };
 
 namespace {
@@ -685,6 +690,75 @@ int amgdd_residual_norm(amgdd_handle_t h, const double* b, const double* x, doub
     CUDA_TRY(cudaGetLastError());
     CUDA_TRY(cudaMemcpyAsync(out_host, h->d_norms, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
     CUDA_TRY(cudaStreamSynchronize(h->stream));
+    return AMGDD_SUCCESS;
+}
+
+// AMG V(nu1,nu2)-cycles on the global hierarchy (Alg. 1): the paper's comparison method (Fig. 14)
+static int ensure_vcycle(amgdd_handle_s* h) {
+    if (h->vcycle_ready) return AMGDD_SUCCESS;
+    const int L = h->H.L;
+    int rc;
+    for (int l = 0; l <= L; ++l) {
+        const HostLevel& lv = h->H.lv[l];
+        GlobalLevelDev& g = h->glev[l];
+        const size_t nl = (size_t)lv.A.nrows;
+        if (!g.a_rp) { if ((rc = upload_csr32(h, lv.A, &g.a_rp, &g.a_ci, &g.a_v))) return rc; }
+        if (l < L) {
+            if ((rc = upload_csr32(h, lv.P, &g.p_rp, &g.p_ci, &g.p_v))) return rc;
+            g.lanes_p = pick_lanes(avg_row(lv.P));
+        }
+        if ((rc = upload(h, &g.vdinv, lv.dinv.data(), lv.dinv.size()))) return rc;
+        if ((rc = dev_alloc(h, (void**)&g.vu0, nl * sizeof(double)))) return rc;
+        if ((rc = dev_alloc(h, (void**)&g.vu1, nl * sizeof(double)))) return rc;
+        if ((rc = dev_alloc(h, (void**)&g.vf, nl * sizeof(double)))) return rc;
+        if ((rc = dev_alloc(h, (void**)&g.vr, nl * sizeof(double)))) return rc;
+    }
+    h->vcycle_ready = true;
+    return AMGDD_SUCCESS;
+}
+
+int amgdd_vcycle(amgdd_handle_t h, const double* b, double* x, int32_t num_cycles, int32_t nu1, int32_t nu2, double* resnorm_host) {
+    if (bad_handle(h)) return AMGDD_ERR_BAD_ARG;
+    if (!b || !x || num_cycles < 0 || nu1 < 0 || nu2 < 0 || nu1 + nu2 < 1 || num_cycles + 1 > h->norms_cap) {
+        g_detail = "need b, x non-null, 0 <= num_cycles < 1024, nu1, nu2 >= 0, nu1 + nu2 >= 1";
+        return AMGDD_ERR_BAD_ARG;
+    }
+    int rc = ensure_vcycle(h);
+    if (rc) return rc;
+    const int L = h->H.L;
+    cudaStream_t st = h->stream;
+    auto nrows = [&](int l) { return (long long)h->H.lv[l].A.nrows; };
+    for (int k = 0; k < num_cycles; ++k) {
+        enqueue_residual(h, b, x, nullptr, k);                                  // ||b - A x_k|| (metric only)
+        for (int l = 0; l < L; ++l) {                                           // downsweep P:449-455
+            GlobalLevelDev& g = h->glev[l];
+            const double* f = l == 0 ? b : g.vf;
+            bool have_u = l == 0;                                               // coarse levels start from u = 0
+            if (l == 0) CUDA_TRY(cudaMemcpyAsync(g.vu0, x, (size_t)nrows(0) * sizeof(double), cudaMemcpyDeviceToDevice, st));
+            for (int s = 0; s < nu1; ++s) {                                     // the level's iterate lives in vu0
+                launch_relax(g.a_rp, g.a_ci, g.a_v, nrows(l), g.lanes_a, g.vdinv, f, have_u ? g.vu0 : nullptr, g.vu1, st);
+                std::swap(g.vu0, g.vu1);
+                have_u = true;
+            }
+            if (!have_u) CUDA_TRY(cudaMemsetAsync(g.vu0, 0, (size_t)nrows(l) * sizeof(double), st));
+            launch_spmv_axpy(g.a_rp, g.a_ci, g.a_v, nrows(l), g.lanes_a, g.vu0, f, g.vr, 0, st);        // r = f - A u
+            launch_spmv(g.r_rp, g.r_ci, g.r_v, nrows(l + 1), g.lanes_r, g.vr, h->glev[l + 1].vf, st);   // f_{l+1} = P^T r
+        }
+        launch_coarse_solve(h->d_lu, h->d_rowperm, (int)h->H.nL, L == 0 ? b : h->glev[L].vf, L == 0 ? x : h->glev[L].vu0, st);
+        for (int l = L - 1; l >= 0; --l) {                                      // upsweep P:459-464
+            GlobalLevelDev& g = h->glev[l];
+            const double* f = l == 0 ? b : g.vf;
+            launch_spmv_axpy(g.p_rp, g.p_ci, g.p_v, nrows(l), g.lanes_p, h->glev[l + 1].vu0, nullptr, g.vu0, 1, st);   // u += P u_{l+1}
+            for (int s = 0; s < nu2; ++s) { launch_relax(g.a_rp, g.a_ci, g.a_v, nrows(l), g.lanes_a, g.vdinv, f, g.vu0, g.vu1, st); std::swap(g.vu0, g.vu1); }
+            if (l == 0) CUDA_TRY(cudaMemcpyAsync(x, g.vu0, (size_t)nrows(0) * sizeof(double), cudaMemcpyDeviceToDevice, st));
+        }
+    }
+    enqueue_residual(h, b, x, nullptr, num_cycles);
+    CUDA_TRY(cudaGetLastError());
+    if (resnorm_host) {
+        CUDA_TRY(cudaMemcpyAsync(resnorm_host, h->d_norms, (size_t)(num_cycles + 1) * sizeof(double), cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(cudaStreamSynchronize(st));
+    }
     return AMGDD_SUCCESS;
 }
 

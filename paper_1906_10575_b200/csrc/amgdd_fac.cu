@@ -322,7 +322,25 @@ struct Worker {
         // for the ring's loads in flight (all ordinary global loads of a warp share one).
         //   stage:  H  32 x 16 bytes  header of the next slice (after the last slice: slice 0 of the next mat-vec)
         //           C  3 x 32 x 8 bytes  operands e0 | e1 | e2 of the current slice's epilogue
-        if (n == 0) { ring_valid = false; hdr_ready = false; tock(PROF_OP0 + kind, tp0); return; }
+        if (n == 0) {
+            // Nothing to do for this warp in this step (a stream with fewer slices than ways): use the time
+            // to fetch the first block and the first header of the next mat-vec, so that the steps on the
+            // small coarse levels do not each start with a full round trip to memory.
+            ring_valid = hdr_ready = n_next > 0;
+            if (n_next > 0) {
+                if (phase == 0) {
+#pragma unroll
+                    for (int d = 0; d < D; ++d) ra[d] = load_grp<WIDE>(nxt + (long long)(d < next_last ? d : next_last) * GB, lane, pol);
+                } else {
+#pragma unroll
+                    for (int d = 0; d < D; ++d) rb[d] = load_grp<WIDE>(nxt + (long long)(d < next_last ? d : next_last) * GB, lane, pol);
+                }
+                cp_async_wait_all();
+                cp_async16(stage + 16 * lane, nxt_hdr + 16 * lane);
+            }
+            tock(PROF_OP0 + kind, tp0);
+            return;
+        }
         const char* const hdr = we_hdr + 16 * lane;
         const uint32_t stH = stage + 16 * lane, stC = stage + 512 + 8 * lane;
         const char* const hdr_after = nxt_hdr + 16 * lane;
@@ -359,7 +377,9 @@ struct Worker {
             acc = fma(mkdouble(g.b.z, g.b.w), x3, acc);
         };
         auto slice_end = [&]() {
+            const long long tw0 = tick();
             cp_async_wait_all();
+            tock(14, tw0);
 #ifdef AMGDD_EXP_NOEPI
             if (row == 0x7ffffff0u) {
 #else
@@ -420,7 +440,10 @@ struct Worker {
         // finite matrix entry has (Inf/NaN exponent), so the address cannot be formed earlier.
         auto step = [&](Grp (&X)[D], Grp (&Y)[D], int p0) {
             const bool more = p0 + D < n;
+            const long long tr0 = tick();
             const bool never = (X[0].a.y & 0x7FF00000u) == 0x7FF00000u;
+            if (PROF && never) prof[15] += 1;            // (keeps the read of X[0] before the second clock read)
+            tock(15, tr0);
             const char* rbase = never ? dummy : (more ? cur : nxt);
             const int r0 = more ? p0 + D : 0, rlast = never ? 0 : (more ? n - 1 : next_last);
 #if !AMGDD_SINGLE_BUFFER

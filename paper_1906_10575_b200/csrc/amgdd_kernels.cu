@@ -69,7 +69,79 @@ __global__ void __launch_bounds__(GLOBAL_BLOCK) spmv_kernel(const int* __restric
     if (row < n && lane == 0) y[row] = sum;
 }
 
+// ---------------------------------------------------------------------------------------------
+// AMG V-cycle on the global hierarchy (Alg. 1): the paper's comparison method
+// ---------------------------------------------------------------------------------------------
+// one l1-Jacobi sweep u_out = u_in + D^-1 (f - A u_in) (reading A2); u_in = nullptr means u_in = 0
+__global__ void __launch_bounds__(GLOBAL_BLOCK) relax_kernel(const int* __restrict__ rp, const int* __restrict__ ci,
+                                                             const double* __restrict__ v, long long n, int lanes,
+                                                             const double* __restrict__ dinv, const double* __restrict__ f,
+                                                             const double* __restrict__ u_in, double* __restrict__ u_out) {
+    const int lane = threadIdx.x & (lanes - 1);
+    const long long row = (long long)blockIdx.x * (GLOBAL_BLOCK / lanes) + threadIdx.x / lanes;
+    double sum = 0.0;
+    if (row < n && u_in) {
+        const int bgn = __ldg(rp + row), end = __ldg(rp + row + 1);
+        for (int k = bgn + lane; k < end; k += lanes) sum += __ldg(v + k) * __ldg(u_in + __ldg(ci + k));
+    }
+    for (int o = lanes >> 1; o > 0; o >>= 1) sum += __shfl_down_sync(0xffffffffu, sum, o, lanes);
+    if (row < n && lane == 0) u_out[row] = (u_in ? u_in[row] : 0.0) + dinv[row] * (f[row] - sum);
+}
+
+// y = f - A x (f = nullptr: y = A x); accumulate = 1: y += A x
+__global__ void __launch_bounds__(GLOBAL_BLOCK) spmv_axpy_kernel(const int* __restrict__ rp, const int* __restrict__ ci,
+                                                                 const double* __restrict__ v, long long n, int lanes,
+                                                                 const double* __restrict__ x, const double* __restrict__ f,
+                                                                 double* __restrict__ y, int accumulate) {
+    const int lane = threadIdx.x & (lanes - 1);
+    const long long row = (long long)blockIdx.x * (GLOBAL_BLOCK / lanes) + threadIdx.x / lanes;
+    double sum = 0.0;
+    if (row < n) {
+        const int bgn = __ldg(rp + row), end = __ldg(rp + row + 1);
+        for (int k = bgn + lane; k < end; k += lanes) sum += __ldg(v + k) * __ldg(x + __ldg(ci + k));
+    }
+    for (int o = lanes >> 1; o > 0; o >>= 1) sum += __shfl_down_sync(0xffffffffu, sum, o, lanes);
+    if (row < n && lane == 0) y[row] = accumulate ? y[row] + sum : (f ? f[row] - sum : sum);
+}
+
+// u = A_L^-1 f with the LU factors of setup (column-major, unit lower; rowperm[i] = source row of row i); one CTA
+__global__ void __launch_bounds__(256) coarse_solve_kernel(const double* __restrict__ lu, const int* __restrict__ rowperm, int n,
+                                                           const double* __restrict__ f, double* __restrict__ u) {
+    extern __shared__ double y[];
+    for (int i = threadIdx.x; i < n; i += blockDim.x) y[i] = f[rowperm[i]];
+    __syncthreads();
+    for (int c = 0; c < n; ++c) {                              // forward: L y = P f
+        const double yc = y[c];
+        for (int i = c + 1 + threadIdx.x; i < n; i += blockDim.x) y[i] -= lu[(size_t)c * n + i] * yc;
+        __syncthreads();
+    }
+    for (int c = n - 1; c >= 0; --c) {                         // backward: U u = y
+        if (threadIdx.x == 0) y[c] = y[c] / lu[(size_t)c * n + c];
+        __syncthreads();
+        const double yc = y[c];
+        for (int i = threadIdx.x; i < c; i += blockDim.x) y[i] -= lu[(size_t)c * n + i] * yc;
+        __syncthreads();
+    }
+    for (int i = threadIdx.x; i < n; i += blockDim.x) u[i] = y[i];
+}
+
 }  // namespace
+
+void launch_relax(const int* rp, const int* ci, const double* v, long long n, int lanes, const double* dinv, const double* f,
+                  const double* u_in, double* u_out, void* stream) {
+    if (n <= 0) return;
+    relax_kernel<<<residual_num_blocks(n, lanes), GLOBAL_BLOCK, 0, (cudaStream_t)stream>>>(rp, ci, v, n, lanes, dinv, f, u_in, u_out);
+}
+
+void launch_spmv_axpy(const int* rp, const int* ci, const double* v, long long n, int lanes, const double* x, const double* f,
+                      double* y, int accumulate, void* stream) {
+    if (n <= 0) return;
+    spmv_axpy_kernel<<<residual_num_blocks(n, lanes), GLOBAL_BLOCK, 0, (cudaStream_t)stream>>>(rp, ci, v, n, lanes, x, f, y, accumulate);
+}
+
+void launch_coarse_solve(const double* lu, const int* rowperm, int n, const double* f, double* u, void* stream) {
+    coarse_solve_kernel<<<1, 256, (size_t)n * sizeof(double), (cudaStream_t)stream>>>(lu, rowperm, n, f, u);
+}
 
 int pick_lanes(double avg) {
     int g = 2;

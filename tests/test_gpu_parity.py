@@ -175,6 +175,26 @@ def test_wide_column_indices():
     run_parity(wl.make_config(1, 272, parts_per_dim=1), 2)
 
 
+@pytest.mark.parametrize("cfg,scale,nu1,nu2", [(2, 32, 1, 1), (4, 24, 2, 1), (1, None, 1, 2), (5, 128, 1, 1)])
+def test_amg_vcycle_matches_the_oracle(cfg, scale, nu1, nu2):
+    """NEXT 2 of SURVEY.md section 8(f): the AMG V-cycle of Alg. 1 (the paper's comparison method) on the GPU
+    against the oracle's orc_vcycle (pinned to the scipy V-cycle of tests/reference_global.py)."""
+    torch = _torch()
+    p = wl.make_config(cfg, scale)
+    m, h = lib_setup(p)
+    o = orc_setup(p)
+    b = torch.from_numpy(p.b).cuda()
+    x = torch.zeros(p.n, dtype=torch.float64, device="cuda")
+    xo = np.zeros(p.n)
+    for k in range(4):
+        res = m.amgdd_vcycle(h, b, x, 1, nu1, nu2)
+        xo = o.vcycle(p.b, xo, nu1, nu2)
+        r1 = o.residual_norm(p.b, xo)
+        assert abs(res[1] - r1) <= RTOL * r1, (k, res, r1)
+        assert np.abs(x.cpu().numpy() - xo).max() <= RTOL * np.abs(xo).max()
+    m.amgdd_destroy(h)
+
+
 def test_ragged_partition_and_odd_sizes():
     # 33 = 17 + 16: ragged blocks; 3 x 3 blocks of a 37 x 37 grid
     run_parity(wl.make_config(1, 37, parts_per_dim=3), 3)
