@@ -1,5 +1,5 @@
-"""Parity at BASELINE.json's full sizes, in the launch configuration bench.py times (configs 4 and
-5; configs 1 and 2 run at full size in test_gpu_parity.py).  The oracle cannot run all subdomains of
+"""Parity at BASELINE.json's full sizes, in the launch configuration bench.py times (configs 3 at eta = 1,
+4 and 5; configs 1 and 2 run at full size in test_gpu_parity.py).  The oracle cannot run all subdomains of
 these in a test's time, so it computes SAMPLED outputs: Alg. 2's global residual and restriction in
 full, AlgFAC on a sample of subdomains; every cycle both sides start from the same iterate (the
 library's), and x is compared on the owned dofs of the sampled subdomains.  The residual norm of
@@ -14,11 +14,11 @@ pytestmark = pytest.mark.gpu
 RTOL = 1e-10
 
 
-def _run(cfg, num_cycles, nsample):
+def _run(cfg, num_cycles, nsample, eta=None):
     import torch
     import paper_1906_10575_b200 as m
     assert torch.cuda.is_available(), "GPU tests need a CUDA device"
-    p = wl.make_config(cfg)
+    p = wl.make_config(cfg, eta=eta)
     h = m.amgdd_setup(p.n, p.rowptr, p.colind, p.vals, p.num_subdomains, p.owner, p.eta, p.num_ghost, p.max_levels,
                       p.theta, p.coarse_max)
     o = Oracle(p.n, p.rowptr, p.colind, p.vals, p.theta, p.max_levels, p.coarse_max)
@@ -55,6 +55,11 @@ def _run(cfg, num_cycles, nsample):
 
 def test_config4_fullsize_sampled():
     _run(4, 2, 8)
+
+
+def test_config3_fullsize_eta1_sampled():
+    # 128^3 trilinear FE, 512 subdomains, eta = 1: 126 GB of composite matrices on the device (eta = 2, 4 do not fit)
+    _run(3, 2, 4, eta=1)
 
 
 def test_config5_fullsize_sampled():
