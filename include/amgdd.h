@@ -220,8 +220,9 @@ int amgdd_last_solve_profile(amgdd_handle_t h, double ms[4], int64_t launches[3]
  * Returns AMGDD_ERR_BAD_ARG if profiling was not enabled.  Timed runs must not enable it. */
 int amgdd_debug_fac_cycles(amgdd_handle_t h, int64_t out[16], int32_t reset);
 /* Same switch: SM cycles of every step of the AlgFAC program (thread 0 of each CTA, summed over CTAs and
- * subdomains): out[j] = step j (j < n), out[n + j] = wait at the CTA barrier after it; kinds_levels[j]
- * (HOST, n entries or NULL) = 256 * kind + level of step j.  Clears the counters. */
+ * subdomains); out has 4 n entries: out[j] = step j (j < n), out[n + j] = wait at the CTA barrier after it,
+ * out[2n + j] = its waits for blocks of the register ring, out[3n + j] = its waits for staged slice operands;
+ * kinds_levels[j] (HOST, n entries or NULL) = 256 * kind + level of step j.  Clears the counters. */
 int amgdd_debug_fac_op_cycles(amgdd_handle_t h, int64_t* out, int32_t n, int32_t* kinds_levels);
 
 #ifdef __cplusplus

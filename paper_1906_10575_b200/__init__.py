@@ -261,11 +261,12 @@ OP_KIND_NAMES = ["begin", "first0", "relax", "At", "restrict", "recalc", "interp
 
 def amgdd_debug_fac_op_cycles(h: Handle, n=256):
     """Per-step SM cycles of the AlgFAC program (needs AMGDD_FAC_PROFILE=1 at setup): list of
-    (kind name, level, step cycles, barrier-wait cycles)."""
-    out = np.zeros(2 * n, dtype=np.int64)
+    (kind name, level, step cycles, barrier-wait cycles, ring-wait cycles, slice-operand-wait cycles)."""
+    out = np.zeros(4 * n, dtype=np.int64)
     kl = np.full(n, -1, dtype=np.int32)
     _check(lib.amgdd_debug_fac_op_cycles(h._h, out.ctypes.data, n, kl.ctypes.data))
-    return [(OP_KIND_NAMES[k // 256], int(k % 256), int(out[j]), int(out[n + j])) for j, k in enumerate(kl) if k >= 0]
+    return [(OP_KIND_NAMES[k // 256], int(k % 256), int(out[j]), int(out[n + j]), int(out[2 * n + j]), int(out[3 * n + j]))
+            for j, k in enumerate(kl) if k >= 0]
 
 
 def amgdd_last_solve_profile(h: Handle):

@@ -420,7 +420,7 @@ int finish_tables(amgdd_handle_s* h) {
         const size_t bytes = (size_t)h->fac_cfg.grid * FAC_PROF_SLOTS * sizeof(long long);
         if ((rc = dev_alloc(h, (void**)&h->d_prof, bytes))) return rc;
         CUDA_TRY(cudaMemset(h->d_prof, 0, bytes));
-        const size_t b2 = (size_t)h->fac_cfg.grid * 2 * MAX_OPS * sizeof(long long);
+        const size_t b2 = (size_t)h->fac_cfg.grid * PROF_OPS_STRIDE * sizeof(long long);
         if ((rc = dev_alloc(h, (void**)&h->d_prof_ops, b2))) return rc;
         CUDA_TRY(cudaMemset(h->d_prof_ops, 0, b2));
     }
@@ -812,16 +812,14 @@ int amgdd_debug_fac_cycles(amgdd_handle_t h, int64_t out[16], int32_t reset) {
 int amgdd_debug_fac_op_cycles(amgdd_handle_t h, int64_t* out, int32_t n, int32_t* kinds_levels) {
     if (bad_handle(h) || !out) return AMGDD_ERR_BAD_ARG;
     if (!h->d_prof_ops) { g_detail = "set AMGDD_FAC_PROFILE=1 before amgdd_setup"; return AMGDD_ERR_BAD_ARG; }
-    const size_t cnt = (size_t)h->fac_cfg.grid * 2 * MAX_OPS;
+    const size_t cnt = (size_t)h->fac_cfg.grid * PROF_OPS_STRIDE;
     std::vector<long long> host(cnt);
     CUDA_TRY(cudaStreamSynchronize(h->stream));
     CUDA_TRY(cudaMemcpy(host.data(), h->d_prof_ops, cnt * sizeof(long long), cudaMemcpyDeviceToHost));
-    for (int i = 0; i < 2 * n; ++i) out[i] = 0;
+    for (int i = 0; i < 4 * n; ++i) out[i] = 0;
     for (int b = 0; b < h->fac_cfg.grid; ++b)
-        for (int j = 0; j < n && j < MAX_OPS; ++j) {
-            out[j] += host[(size_t)b * 2 * MAX_OPS + j];
-            out[n + j] += host[(size_t)b * 2 * MAX_OPS + MAX_OPS + j];
-        }
+        for (int j = 0; j < n && j < MAX_OPS; ++j)
+            for (int q = 0; q < 4; ++q) out[q * n + j] += host[(size_t)b * PROF_OPS_STRIDE + q * MAX_OPS + j];
     if (kinds_levels) {
         std::vector<FacOp> ops((size_t)std::max(1, h->prog_nops));
         fac_build_program(h->H.L, h->prog_nfac, h->prog_nu, ops.data());

@@ -162,6 +162,7 @@ struct Worker {
     bool ring_valid;               // the ring holds the first groups of the coming mat-vec
     bool hdr_ready;                // the staging area holds (or is receiving) the header of its slice 0
     uint32_t stage;                // shared address of this warp's staging area (STAGE_BYTES)
+    int opj;                       // index of the current step in the program (profiling)
 
     __device__ __forceinline__ long long tick() const { return PROF ? clock64() : 0; }
     __device__ __forceinline__ void tock(int idx, long long t0) const { if (PROF && tid == 0) prof[idx] += clock64() - t0; }
@@ -366,11 +367,7 @@ struct Worker {
             uint32_t c0, c1, c2, c3;
             if (WIDE) { c0 = g.c.x; c1 = g.c.y; c2 = g.c.z; c3 = g.c.w; }
             else { c0 = g.c.x & 0xffffu; c1 = g.c.x >> 16; c2 = g.c.y & 0xffffu; c3 = g.c.y >> 16; }
-#ifdef AMGDD_EXP_NOGATHER
-            const double x0 = __hiloint2double(c0, c1), x1 = __hiloint2double(c1, c2), x2 = __hiloint2double(c2, c3), x3 = __hiloint2double(c3, c0);
-#else
             const double x0 = xg.template ldt<GS>(c0), x1 = xg.template ldt<GS>(c1), x2 = xg.template ldt<GS>(c2), x3 = xg.template ldt<GS>(c3);
-#endif
             acc = fma(mkdouble(g.a.x, g.a.y), x0, acc);
             acc = fma(mkdouble(g.a.z, g.a.w), x1, acc);
             acc = fma(mkdouble(g.b.x, g.b.y), x2, acc);
@@ -380,11 +377,8 @@ struct Worker {
             const long long tw0 = tick();
             cp_async_wait_all();
             tock(14, tw0);
-#ifdef AMGDD_EXP_NOEPI
-            if (row == 0x7ffffff0u) {
-#else
+            if (PROF && tid == 0 && prm->prof_ops) prm->prof_ops[(size_t)blockIdx.x * PROF_OPS_STRIDE + 3 * MAX_OPS + opj] += clock64() - tw0;
             if (row != NO_ROW) {
-#endif
                 const double e0 = lds_f64(stC), e1 = lds_f64(stC + 256), e2 = lds_f64(stC + 512);   // unused ones are stale, never read
                 if (kind == OPK_RELAX) {           // one l1-Jacobi update (§4.1); aux = 1 / sum_j |a_ij| (S8)
                     const double dl = aux * (e0 - acc);
@@ -444,6 +438,7 @@ struct Worker {
             const bool never = (X[0].a.y & 0x7FF00000u) == 0x7FF00000u;
             if (PROF && never) prof[15] += 1;            // (keeps the read of X[0] before the second clock read)
             tock(15, tr0);
+            if (PROF && tid == 0 && prm->prof_ops) prm->prof_ops[(size_t)blockIdx.x * PROF_OPS_STRIDE + 2 * MAX_OPS + opj] += clock64() - tr0;
             const char* rbase = never ? dummy : (more ? cur : nxt);
             const int r0 = more ? p0 + D : 0, rlast = never ? 0 : (more ? n - 1 : next_last);
 #if !AMGDD_SINGLE_BUFFER
@@ -557,6 +552,7 @@ __global__ void __launch_bounds__(NTHREADS, CTAS_PER_SM) fac_kernel(const FacPar
         W.ring_valid = false; W.hdr_ready = false;
         for (int j = 0; j < prm.nops; ++j) {
             const FacOp op = ops[j];
+            W.opj = j;
             const long long tp0 = W.tick();
             if (op.kind == OPK_BEGIN) W.begin_subdomain();
             else if (op.kind == OPK_FIRST0) W.first0(op);
@@ -571,9 +567,9 @@ __global__ void __launch_bounds__(NTHREADS, CTAS_PER_SM) fac_kernel(const FacPar
             }
             if (!is_matvec(op.kind)) W.tock(PROF_OP0 + op.kind, tp0);
             long long tq0 = 0;
-            if (PROF && threadIdx.x == 0 && prm.prof_ops) { tq0 = clock64(); prm.prof_ops[(size_t)blockIdx.x * 2 * MAX_OPS + j] += tq0 - tp0; }
+            if (PROF && threadIdx.x == 0 && prm.prof_ops) { tq0 = clock64(); prm.prof_ops[(size_t)blockIdx.x * PROF_OPS_STRIDE + j] += tq0 - tp0; }
             W.sync();                                                    // the step is complete
-            if (PROF && threadIdx.x == 0 && prm.prof_ops) prm.prof_ops[(size_t)blockIdx.x * 2 * MAX_OPS + MAX_OPS + j] += clock64() - tq0;
+            if (PROF && threadIdx.x == 0 && prm.prof_ops) prm.prof_ops[(size_t)blockIdx.x * PROF_OPS_STRIDE + MAX_OPS + j] += clock64() - tq0;
         }
     }
     W.tock(PROF_TOTAL, tk0);

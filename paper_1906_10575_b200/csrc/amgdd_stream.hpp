@@ -156,9 +156,10 @@ struct FacParams {
     int nL;
     int x_cap;                 // doubles in each of the two shared-memory vector buffers (0: vectors in global memory)
     long long* prof;           // optional: gridDim.x * FAC_PROF_SLOTS cycle counters (debugging), or nullptr
-    long long* prof_ops;       // optional: gridDim.x * 2 * MAX_OPS: cycles of every step of the program | barrier wait after it
+    long long* prof_ops;       // optional: gridDim.x * PROF_OPS_STRIDE: per step of the program: cycles | barrier wait after it | waits for ring blocks | waits for staged slice operands
 };
 constexpr int FAC_PROF_SLOTS = 16;
+constexpr int PROF_OPS_STRIDE = 4 * MAX_OPS;
 
 struct FacLaunch {
     int grid;
