@@ -34,6 +34,7 @@ def _load():
     L.orc_create.restype = _vp
     L.orc_create.argtypes = [_i64, _vp, _vp, _vp, _f64, _i32, _i32, _vp]
     L.orc_destroy.argtypes = [_vp]
+    L.orc_set_smoother.argtypes = [_vp, _i32]
     L.orc_num_levels.argtypes = [_vp]
     L.orc_level_size.argtypes = [_vp, _i32, _vp, _vp, _vp]
     L.orc_get_cf.argtypes = [_vp, _i32, _vp]
@@ -84,6 +85,10 @@ class Oracle:
         if getattr(self, "_h", None):
             _load().orc_destroy(self._h)
             self._h = None
+
+    def set_smoother(self, kind):
+        """0: l1-Jacobi (BASELINE), 1: CF l1-Jacobi: C- then F-points before, F- then C-points after the coarse correction."""
+        _load().orc_set_smoother(self._h, int(kind))
 
     # ---- hierarchy introspection ----
     def level_size(self, l):

@@ -67,6 +67,7 @@ struct Oracle {
     std::vector<std::unique_ptr<Comp>> comp;      // built lazily, one per subdomain
     i64 dropped = 0;            // A7: P entries of composite rows that fall outside D-bar_{l+1}
     Counters cnt;               // mat-vec counters
+    int smoother = 0;           // 0: l1-Jacobi (BASELINE), 1: CF l1-Jacobi (C then F before, F then C after the coarse correction)
 };
 
 // ------------------------------------------------------------------------------------------
@@ -374,20 +375,30 @@ const Comp& get_comp(Oracle& o, int p, Scratch& sc) {
 // ------------------------------------------------------------------------------------------
 void relax_level(const Csr& A, const double* dinv_global, const std::vector<i32>& real,
                  const std::vector<i32>& g2l, std::vector<double>& u, const std::vector<double>& f,
-                 std::vector<double>* t, std::vector<double>& delta, Counters& cnt) {
+                 std::vector<double>* t, std::vector<double>& delta, Counters& cnt,
+                 const int8_t* cf = nullptr, int first_class = 0) {
+    // cf == nullptr: plain l1-Jacobi (one pass over all real points).  Otherwise "CF l1-scaled Jacobi" (P:275,
+    // reading A2b): two half-sweeps, each an l1-Jacobi update of one class of points (C: cf > 0, F: cf < 0)
+    // from the current u; first_class = +1: C-points then F-points, -1: F-points then C-points.
     const size_t nr = real.size();
     delta.resize(nr);
-    for (size_t i = 0; i < nr; ++i) {
-        const i32 g = real[i];
-        double au = 0.0;
-        for (i64 k = A.rp[g]; k < A.rp[g + 1]; ++k) {
-            const i32 lj = g2l[A.ci[k]];
-            assert(lj >= 0);                                           // eq. 1: the row stencil is in D-bar_l
-            au += A.v[k] * u[lj];
+    const int npass = cf ? 2 : 1;
+    for (int pass = 0; pass < npass; ++pass) {
+        const int cls = cf ? (pass == 0 ? first_class : -first_class) : 0;
+        for (size_t i = 0; i < nr; ++i) {
+            const i32 g = real[i];
+            delta[i] = 0.0;
+            if (cf && ((cf[g] > 0) != (cls > 0))) continue;
+            double au = 0.0;
+            for (i64 k = A.rp[g]; k < A.rp[g + 1]; ++k) {
+                const i32 lj = g2l[A.ci[k]];
+                assert(lj >= 0);                                       // eq. 1: the row stencil is in D-bar_l
+                au += A.v[k] * u[lj];
+            }
+            delta[i] = dinv_global[g] * (f[i] - au);
         }
-        delta[i] = dinv_global[g] * (f[i] - au);
+        for (size_t i = 0; i < nr; ++i) { u[i] += delta[i]; if (t) (*t)[i] += delta[i]; }
     }
-    for (size_t i = 0; i < nr; ++i) { u[i] += delta[i]; if (t) (*t)[i] += delta[i]; }
     cnt.A += 1;
 }
 
@@ -422,7 +433,8 @@ void fac_subdomain(Oracle& o, int p, const std::vector<std::vector<double>>& r, 
             const size_t nr = c.real[l].size(), nb = u[l].size();
             if (l != 0) std::fill(u[l].begin(), u[l].end(), 0.0);
             for (int k = 0; k < nu; ++k)
-                relax_level(lv.A, lv.dinv.data(), c.real[l], sc.g2l[l], u[l], f[l], &t[l], delta, cnt);
+                relax_level(lv.A, lv.dinv.data(), c.real[l], sc.g2l[l], u[l], f[l], &t[l], delta, cnt,
+                            o.smoother ? lv.cf.data() : nullptr, +1);
             // P:509  w = s_l + A_l t_l on D-bar_l ; t_l is zero off D_l (reading A12)
             w = s[l];
             for (size_t li = 0; li < nb; ++li) {
@@ -483,7 +495,8 @@ void fac_subdomain(Oracle& o, int p, const std::vector<std::vector<double>>& r, 
             }
             cnt.P += 1;
             for (int k = 0; k < nu; ++k)
-                relax_level(lv.A, lv.dinv.data(), c.real[l], sc.g2l[l], u[l], f[l], &t[l], delta, cnt);
+                relax_level(lv.A, lv.dinv.data(), c.real[l], sc.g2l[l], u[l], f[l], &t[l], delta, cnt,
+                            o.smoother ? lv.cf.data() : nullptr, -1);
         }
     }
     u0 = u[0];
@@ -595,6 +608,9 @@ void* orc_create(i64 n, const i64* rowptr, const i32* colind, const double* vals
 }
 
 void orc_destroy(void* h) { delete (Oracle*)h; }
+
+// 0: l1-Jacobi, 1: CF l1-Jacobi (relaxation of orc_cycle, orc_solve, orc_fac_local, orc_vcycle)
+void orc_set_smoother(void* h, int type) { ((Oracle*)h)->smoother = type; }
 
 int orc_num_levels(void* h) { return ((Oracle*)h)->L + 1; }
 
@@ -713,7 +729,7 @@ void orc_relax(void* h, int l, double* u, const double* f, const int8_t* mask, c
     for (size_t i = 0; i < real.size(); ++i) ff[i] = f[real[i]];
     Counters c;
     for (int k = 0; k < nsweeps; ++k)
-        relax_level(lv.A, dinv ? dinv : lv.dinv.data(), real, perm, up, ff, nullptr, delta, c);
+        relax_level(lv.A, dinv ? dinv : lv.dinv.data(), real, perm, up, ff, nullptr, delta, c, o.smoother ? lv.cf.data() : nullptr, +1);
     for (i64 i = 0; i < n; ++i) u[i] = up[perm[i]];
 }
 
@@ -730,7 +746,7 @@ void orc_vcycle(void* h, const double* b, double* x, int nu1, int nu2) {
     for (int l = 0; l <= L; ++l) { id[l].resize(o.lev[l].A.nrows); for (size_t i = 0; i < id[l].size(); ++i) id[l][i] = (i32)i; }
     for (int l = 0; l < L; ++l) {
         const Level& lv = o.lev[l];
-        for (int k = 0; k < nu1; ++k) relax_level(lv.A, lv.dinv.data(), id[l], id[l], u[l], f[l], nullptr, delta, c);
+        for (int k = 0; k < nu1; ++k) relax_level(lv.A, lv.dinv.data(), id[l], id[l], u[l], f[l], nullptr, delta, c, o.smoother ? lv.cf.data() : nullptr, +1);
         tmp.resize(lv.A.nrows);
         spmv(lv.A, u[l].data(), tmp.data());
         for (size_t i = 0; i < tmp.size(); ++i) tmp[i] = f[l][i] - tmp[i];
@@ -747,7 +763,7 @@ void orc_vcycle(void* h, const double* b, double* x, int nu1, int nu2) {
             for (i64 k = lv.P.rp[i]; k < lv.P.rp[i + 1]; ++k) pu += lv.P.v[k] * u[l + 1][lv.P.ci[k]];
             u[l][i] += pu;
         }
-        for (int k = 0; k < nu2; ++k) relax_level(lv.A, lv.dinv.data(), id[l], id[l], u[l], f[l], nullptr, delta, c);
+        for (int k = 0; k < nu2; ++k) relax_level(lv.A, lv.dinv.data(), id[l], id[l], u[l], f[l], nullptr, delta, c, o.smoother ? lv.cf.data() : nullptr, -1);
     }
     std::copy(u[0].begin(), u[0].end(), x);
 }

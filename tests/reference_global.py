@@ -13,18 +13,26 @@ def l1_dinv(A):
     return 1.0 / np.asarray(abs(A).sum(axis=1)).ravel()
 
 
-def masked_vcycles(As, Ps, masks, r0, niter, nu):
+def masked_vcycles(As, Ps, masks, r0, niter, nu, cfs=None):
     """niter global V(nu,nu)-cycles (Alg. 1) on A_0 e = r0 from e = 0 in which level l
-    relaxes only where masks[l] is True (l1-Jacobi, simultaneous update).  Returns e on level 0."""
+    relaxes only where masks[l] is True (l1-Jacobi, simultaneous update).  Returns e on level 0.
+    cfs (list of +1/-1 arrays per level < L): "CF l1-scaled Jacobi" instead: every sweep is two
+    half-sweeps, C-points then F-points before the coarse correction, F-points then C-points after it."""
     L = len(As) - 1
     dinv = [l1_dinv(A) for A in As]
     u = [np.zeros(A.shape[0]) for A in As]
     f = [np.array(r0, dtype=np.float64)] + [None] * L
     AL = As[L].toarray()
 
-    def relax(l):
-        d = dinv[l] * (f[l] - As[l] @ u[l])
-        u[l][masks[l]] += d[masks[l]]
+    def relax(l, first=+1):
+        if cfs is None:
+            d = dinv[l] * (f[l] - As[l] @ u[l])
+            u[l][masks[l]] += d[masks[l]]
+            return
+        for cls in (first, -first):
+            sel = masks[l] & ((cfs[l] > 0) == (cls > 0))
+            d = dinv[l] * (f[l] - As[l] @ u[l])
+            u[l][sel] += d[sel]
 
     for _ in range(niter):
         for l in range(L):
@@ -37,7 +45,7 @@ def masked_vcycles(As, Ps, masks, r0, niter, nu):
         for l in range(L - 1, -1, -1):
             u[l] = u[l] + Ps[l] @ u[l + 1]
             for _k in range(nu):
-                relax(l)
+                relax(l, -1)
     return u[0]
 
 

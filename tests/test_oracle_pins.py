@@ -309,6 +309,66 @@ def test_single_subdomain_is_plain_vcycle(nu):
     assert np.abs(x - u_v).max() <= 1e-13 * np.abs(u_v).max()
 
 
+# ------------------------------------------------------------------------------------------
+# CF l1-Jacobi (reading A2b)
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("cfg,scale,parts,eta,nfac,nu", [
+    (1, None, 2, 1, 2, 1), (1, 21, 3, 2, 3, 2), (2, 12, 2, 2, 2, 1), (4, 12, 2, 2, 2, 2), (5, 32, 2, 3, 2, 1), (3, 8, 2, 1, 2, 1)])
+def test_cf_jacobi_algfac_equals_masked_global_vcycle(cfg, scale, parts, eta, nfac, nu):
+    # the P:87 equivalence holds for any point-wise relaxation: here C- then F-points before, F- then
+    # C-points after the coarse correction; the global formulation is scipy code of its own
+    p = wl.make_config(cfg, scale, parts_per_dim=parts)
+    o = make_oracle(p, eta=eta, coarse_max=min(p.coarse_max, 16))
+    o.set_smoother(1)
+    As, Ps = hierarchy_from_oracle(o)
+    cfs = [o.cf(l) for l in range(o.num_levels - 1)]
+    r0 = wl.rhs(321, p.n)
+    for q in range(p.num_subdomains):
+        real, ghost = o.composite(q, 0)
+        u_fac = o.fac_local(q, r0, nfac, nu)
+        u_glob = masked_vcycles(As, Ps, _masks(o, q), r0, nfac, nu, cfs=cfs)
+        idx = np.concatenate([real, ghost])
+        tol = 1e-12 if cfg == 5 else 1e-13
+        assert np.abs(u_fac - u_glob[idx]).max() <= tol * np.abs(u_glob).max(), (q,)
+    # it is a different method from plain l1-Jacobi
+    u_cf = o.fac_local(0, r0, nfac, nu)
+    o.set_smoother(0)
+    assert np.abs(o.fac_local(0, r0, nfac, nu) - u_cf).max() > 1e-6 * np.abs(u_cf).max()
+
+
+def test_cf_jacobi_half_sweeps():
+    # one sweep = (I - M_F D^-1 A)(I - M_C D^-1 A) on the error, written with dense matrices: C-points first
+    p = wl.make_config(1, 9, parts_per_dim=1)
+    o = make_oracle(p, eta=100, coarse_max=4)
+    o.set_smoother(1)
+    A = o.scipy_matrix(0, "A").toarray()
+    cf = o.cf(0)
+    Dinv = np.diag(1.0 / np.abs(A).sum(axis=1))
+    MC, MF = np.diag((cf > 0).astype(float)), np.diag((cf < 0).astype(float))
+    rng = np.random.default_rng(0)
+    u, f = rng.standard_normal(p.n), rng.standard_normal(p.n)
+    u1 = u + MC @ Dinv @ (f - A @ u)
+    u2 = u1 + MF @ Dinv @ (f - A @ u1)
+    assert np.abs(o.relax(0, u, f) - u2).max() <= 1e-14 * np.abs(u2).max()
+    # all points in one class: plain l1-Jacobi; and the V-cycle of Alg. 1 uses the same relaxation
+    o.set_smoother(0)
+    assert np.abs(o.relax(0, u, f) - (u + Dinv @ (f - A @ u))).max() <= 1e-14 * np.abs(u).max()
+    o.set_smoother(1)
+    As, Ps = hierarchy_from_oracle(o)
+    cfs = [o.cf(l) for l in range(o.num_levels - 1)]
+    all_true = [np.ones(M.shape[0], dtype=bool) for M in As]
+    u_v = masked_vcycles(As, Ps, all_true, f, 1, 1, cfs=cfs)
+    assert np.abs(o.vcycle(f, np.zeros(p.n), 1, 1) - u_v).max() <= 1e-13 * np.abs(u_v).max()
+    # C-points are relaxed exactly once per half sweep: after the C half the residual of a C-row whose
+    # neighbours are all F-points changes only through its own update (1D-like check on the diagonal scaling)
+    r_before = f - A @ u
+    r_after = f - A @ u1
+    i = int(np.nonzero(cf > 0)[0][0])
+    nbrs = np.nonzero(A[i])[0]
+    if all(cf[j] < 0 for j in nbrs if j != i):
+        assert np.isclose(r_after[i], r_before[i] * (1.0 - A[i, i] * Dinv[i, i]), rtol=1e-12)
+
+
 def test_num_ghost_invariance():
     # A13: extra ghost layers are stored and interpolated but never read by a real row
     p = wl.make_config(1)
