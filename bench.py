@@ -44,11 +44,12 @@ def parse_args():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--cpu-sample", type=int, default=None, help="subdomains in the oracle's timed sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--smoother", type=int, default=0, choices=[0, 1], help="0: l1-Jacobi (BASELINE), 1: CF l1-Jacobi (P:275)")
     return ap.parse_args()
 
 
 def workload_name(p, args):
-    return f"{p.name}-P{p.num_subdomains}-eta{p.eta}-fac{p.num_fac_cycles}xV({p.relax_sweeps},{p.relax_sweeps})"
+    return f"{p.name}-P{p.num_subdomains}-eta{p.eta}-fac{p.num_fac_cycles}xV({p.relax_sweeps},{p.relax_sweeps})" + ("-cfjacobi" if args.smoother else "")
 
 
 class ClockSampler:
@@ -125,7 +126,7 @@ def ncu_traffic(workload):
 # ---------------------------------------------------------------------------------------------
 # CPU oracle leg (cpu_baseline of the b200 arm, and the whole --impl reference arm)
 # ---------------------------------------------------------------------------------------------
-def oracle_time_per_cycle(p, sample, steps, warmup):
+def oracle_time_per_cycle(p, sample, steps, warmup, smoother=0):
     """Times the oracle AS IT STANDS on a bounded sample: every step runs Alg. 2's global residual +
     restriction over the whole problem and AlgFAC on `sample` subdomains (spread evenly over the
     partition); the per-cycle estimate scales the AlgFAC part by P / sample."""
@@ -133,6 +134,7 @@ def oracle_time_per_cycle(p, sample, steps, warmup):
     t0 = time.time()
     o = Oracle(p.n, p.rowptr, p.colind, p.vals, p.theta, p.max_levels, p.coarse_max)
     o.set_partition(p.num_subdomains, p.owner, p.eta, p.num_ghost)
+    o.set_smoother(smoother)
     setup_s = time.time() - t0
     nthreads = max_threads()
     sample = max(1, min(sample, p.num_subdomains))
@@ -164,7 +166,7 @@ def run_reference(args, p, rank, world):
     steps, warmup = args.steps, args.warmup
     sample = args.cpu_sample or default_cpu_sample(p)
     steps_cpu = max(1, min(steps, 3))
-    cb = oracle_time_per_cycle(p, sample, steps_cpu, 1)
+    cb = oracle_time_per_cycle(p, sample, steps_cpu, 1, args.smoother)
     line = {
         "impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus,
         "steps": steps, "warmup": warmup, "ms_per_step": cb["value"], "higher_is_better": False,
@@ -197,6 +199,7 @@ def run_b200(args, p, rank, world, local_rank):
                       p.max_levels, p.theta, p.coarse_max)
     setup_s = time.time() - t0
     st = m.amgdd_get_stats(h)
+    m.amgdd_set_smoother(h, args.smoother)
     stream = torch.cuda.current_stream()
     m.amgdd_set_stream(h, stream)
     b = torch.from_numpy(p.b).cuda()
@@ -315,7 +318,7 @@ def run_b200(args, p, rank, world, local_rank):
             m.amgdd_destroy(h)
             del b, x
             torch.cuda.empty_cache()
-            line["cpu_baseline"] = oracle_time_per_cycle(p, args.cpu_sample or default_cpu_sample(p), 1, 1)
+            line["cpu_baseline"] = oracle_time_per_cycle(p, args.cpu_sample or default_cpu_sample(p), 1, 1, args.smoother)
         print(json.dumps(line))
     if distributed:
         dist.barrier()

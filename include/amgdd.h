@@ -142,6 +142,15 @@ int amgdd_vcycle(amgdd_handle_t h, const double* b, double* x, int32_t num_cycle
 /* || b - A_0 x ||_2 (metric of Fig. 6; reading A16).  b, x DEVICE; out HOST. Synchronises. */
 int amgdd_residual_norm(amgdd_handle_t h, const double* b, const double* x, double* out_host);
 
+/* Relaxation used by amgdd_solve, amgdd_solve_host and amgdd_vcycle from the next call on.
+ *   AMGDD_SMOOTHER_L1_JACOBI     (default) one l1-Jacobi sweep over the real points (reading A2, BASELINE)
+ *   AMGDD_SMOOTHER_CF_L1_JACOBI  the paper's "CF l1-scaled Jacobi" (reading A2b): every sweep is two
+ *                                half-sweeps, C-points then F-points before the coarse correction, F-points
+ *                                then C-points after it; each half-sweep is one pass over the real rows of A_l */
+#define AMGDD_SMOOTHER_L1_JACOBI 0
+#define AMGDD_SMOOTHER_CF_L1_JACOBI 1
+int amgdd_set_smoother(amgdd_handle_t h, int32_t type);
+
 /* Use this CUDA stream (a cudaStream_t passed as void*; NULL = legacy default stream). */
 int amgdd_set_stream(amgdd_handle_t h, void* cuda_stream);
 
@@ -178,6 +187,7 @@ int amgdd_get_stats(amgdd_handle_t h, amgdd_stats_t* s);
  * header {row, K, aux} per lane; the slices are dealt to AMGDD_NUM_WAYS sub-streams ("ways", one
  * per warp of the kernel).
  *   aux      HOST, nrows doubles stored in the slice headers (the l1 diagonal inverse), or NULL (0.0)
+ *   row_flags  HOST, nrows bytes (0/1) stored in bit 31 of the header's info word (C-point of the row's level), or NULL
  *   wide     0: uint16 column indices (needs every column < 65536), 1: uint32
  *   out_ways HOST, AMGDD_NUM_WAYS entries, or NULL
  * With out = NULL only *out_bytes and out_ways are computed.  Returns AMGDD_ERR_INDEX_RANGE for a
@@ -197,8 +207,8 @@ typedef struct amgdd_way {
     uint32_t reserved[2];
 } amgdd_way_t;
 int amgdd_pack_stream(int32_t nrows, int32_t n_real, const int32_t* rowptr32, const int32_t* colind, const double* vals,
-                      const double* aux, int32_t wide, int32_t window, void* out, int64_t out_capacity, int64_t* out_bytes,
-                      amgdd_way_t* out_ways);
+                      const double* aux, const uint8_t* row_flags, int32_t wide, int32_t window, void* out,
+                      int64_t out_capacity, int64_t* out_bytes, amgdd_way_t* out_ways);
 
 /* ---- measurement support ------------------------------------------------------------------
  * Device time (ms, CUDA events on the handle's stream) of the phases of the most recent

@@ -17,7 +17,7 @@ from . import build as _build
 _vp, _i32, _i64, _f64 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_double
 
 EXPORTS = [
-    "amgdd_setup", "amgdd_solve", "amgdd_solve_host", "amgdd_vcycle", "amgdd_residual_norm", "amgdd_set_stream", "amgdd_destroy",
+    "amgdd_setup", "amgdd_solve", "amgdd_solve_host", "amgdd_vcycle", "amgdd_residual_norm", "amgdd_set_smoother", "amgdd_set_stream", "amgdd_destroy",
     "amgdd_strerror", "amgdd_last_error_detail", "amgdd_num_levels", "amgdd_level_size", "amgdd_get_cf",
     "amgdd_get_level_matrix", "amgdd_composite_size", "amgdd_get_composite", "amgdd_get_stats",
     "amgdd_last_solve_profile", "amgdd_pack_stream", "amgdd_debug_fac_cycles", "amgdd_debug_fac_op_cycles",
@@ -54,6 +54,7 @@ def _load():
     L.amgdd_residual_norm.argtypes = [_vp, _vp, _vp, _vp]
     L.amgdd_vcycle.argtypes = [_vp, _vp, _vp, _i32, _i32, _i32, _vp]
     L.amgdd_set_stream.argtypes = [_vp, _vp]
+    L.amgdd_set_smoother.argtypes = [_vp, _i32]
     L.amgdd_destroy.argtypes = [_vp]
     L.amgdd_strerror.restype = ctypes.c_char_p
     L.amgdd_strerror.argtypes = [ctypes.c_int]
@@ -68,7 +69,7 @@ def _load():
     L.amgdd_last_solve_profile.argtypes = [_vp, _vp, _vp]
     L.amgdd_debug_fac_cycles.argtypes = [_vp, _vp, _i32]
     L.amgdd_debug_fac_op_cycles.argtypes = [_vp, _vp, _i32, _vp]
-    L.amgdd_pack_stream.argtypes = [_i32, _i32, _vp, _vp, _vp, _vp, _i32, _i32, _vp, _i64, _vp, _vp]
+    L.amgdd_pack_stream.argtypes = [_i32, _i32, _vp, _vp, _vp, _vp, _vp, _i32, _i32, _vp, _i64, _vp, _vp]
     return L
 
 
@@ -122,6 +123,14 @@ def _dev_ptr(t, n):
     if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and t.numel() >= n):
         raise TypeError("expected a contiguous float64 CUDA tensor of length >= n")
     return t.data_ptr()
+
+
+SMOOTHER_L1_JACOBI, SMOOTHER_CF_L1_JACOBI = 0, 1
+
+
+def amgdd_set_smoother(h: Handle, kind: int):
+    """amgdd_set_smoother: 0 l1-Jacobi (default), 1 CF l1-Jacobi."""
+    _check(lib.amgdd_set_smoother(h._h, int(kind)))
 
 
 def amgdd_set_stream(h: Handle, stream=None):
@@ -226,19 +235,20 @@ WAY_DTYPE = np.dtype([("grp_off128", np.uint32), ("hdr_off128", np.uint32), ("ng
                       ("nslices", np.uint32), ("nslices_real", np.uint32), ("reserved", np.uint32, (2,))])
 
 
-def amgdd_pack_stream(rowptr, colind, vals, wide=False, n_real=None, aux=None, window=256):
+def amgdd_pack_stream(rowptr, colind, vals, wide=False, n_real=None, aux=None, window=256, row_flags=None):
     """amgdd_pack_stream: CSR (host) -> (bytes of the packed SELL-32 group streams as a uint8 array, the
     NUM_WAYS way descriptors as a structured array)."""
     rowptr = _np(rowptr, np.int32)
     colind = _np(colind, np.int32)
     vals = _np(vals, np.float64)
     aux = None if aux is None else _np(aux, np.float64)
+    row_flags = None if row_flags is None else _np(row_flags, np.uint8)
     nrows = len(rowptr) - 1
     n_real = nrows if n_real is None else n_real
     nbytes = _i64()
     ways = np.zeros(NUM_WAYS, dtype=WAY_DTYPE)
     args = (nrows, n_real, rowptr.ctypes.data, colind.ctypes.data, vals.ctypes.data, None if aux is None else aux.ctypes.data,
-            int(wide), window)
+            None if row_flags is None else row_flags.ctypes.data, int(wide), window)
     _check(lib.amgdd_pack_stream(*args, None, 0, ctypes.byref(nbytes), ways.ctypes.data))
     out = np.zeros(max(nbytes.value, 1), dtype=np.uint8)
     _check(lib.amgdd_pack_stream(*args, out.ctypes.data, nbytes.value, ctypes.byref(nbytes), ways.ctypes.data))

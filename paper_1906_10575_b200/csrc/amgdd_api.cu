@@ -36,6 +36,7 @@ struct GlobalLevelDev {          // the single device copy of a whole level
     int* p_rp = nullptr; int* p_ci = nullptr; double* p_v = nullptr;
     int lanes_p = 2;
     double* vdinv = nullptr; double *vu0 = nullptr, *vu1 = nullptr, *vf = nullptr, *vr = nullptr;
+    int8_t* vcf = nullptr;
 };
 
 struct SubMeta {                 // host-side record of one subdomain's blob
@@ -67,11 +68,13 @@ struct amgdd_handle_s {
     int window = DEFAULT_WINDOW, x_cap = 0, smem_cta = 0;
     FacLaunch fac_cfg = {1, 32 * NUM_WAYS, 0};
     FacOp* d_ops = nullptr;                     // the program of one subdomain (fac_build_program)
-    int prog_nfac = -1, prog_nu = -1, prog_nops = 0;
+    int prog_nfac = -1, prog_nu = -1, prog_smoother = -1, prog_nops = 0;
     int* d_counter = nullptr;
     long long* d_prof_ops = nullptr;
     long long* d_prof = nullptr;                // AMGDD_FAC_PROFILE=1: per-CTA cycle counters of the AlgFAC kernel
     double* d_lu = nullptr; int* d_rowperm = nullptr;
+    int8_t* d_cf0 = nullptr;                    // C/F flags of level 0
+    int smoother = 0;                           // 0: l1-Jacobi, 1: CF l1-Jacobi (amgdd_set_smoother)
     double* d_partial = nullptr; int partial_cap = 0;
     double* d_norms = nullptr; int norms_cap = 0;
     double* d_b_stage = nullptr; double* d_x_stage = nullptr;   // for amgdd_solve_host
@@ -295,11 +298,13 @@ StreamDesc make_desc(const char* base, const StreamLayout& lay) {
     return d;
 }
 
-int upload_packed(amgdd_handle_s* h, const HostCsr& M, const double* aux, char** dptr, StreamLayout& lay, const char* what, int l) {
+int upload_packed(amgdd_handle_s* h, const HostCsr& M, const double* aux, const std::vector<int8_t>* cf, char** dptr, StreamLayout& lay, const char* what, int l) {
+    std::vector<uint8_t> flags;                                      // C-points of the rows' level (CF smoother)
+    if (cf && !cf->empty()) { flags.resize(cf->size()); for (size_t i = 0; i < cf->size(); ++i) flags[i] = (*cf)[i] > 0 ? 1 : 0; }
     const int window = what[0] == 'A' ? h->window : std::min(h->window, THIN_WINDOW);
     PackedLevelStream ps;
     i64 bad = -1;
-    if (!pack_global_stream(M, aux, window, ps, bad)) { g_detail = "a level matrix has more than 2^31-1 nonzeros"; return AMGDD_ERR_INDEX_RANGE; }
+    if (!pack_global_stream(M, aux, flags.empty() ? nullptr : flags.data(), window, ps, bad)) { g_detail = "a level matrix has more than 2^31-1 nonzeros"; return AMGDD_ERR_INDEX_RANGE; }
     if (bad >= 0) {
         g_detail = std::string("row ") + std::to_string(bad) + " of " + what + "_" + std::to_string(l) + " has more than 65535 entries";
         return AMGDD_ERR_INDEX_RANGE;
@@ -328,10 +333,10 @@ int finish_tables(amgdd_handle_s* h) {
         if (l < L)
             if ((rc = upload_csr32(h, lv.R, &g.r_rp, &g.r_ci, &g.r_v))) return rc;   // Alg. 2 P:473 needs every R_l
         if (need[l]) {
-            if ((rc = upload_packed(h, lv.A, lv.dinv.data(), &g.sA, g.layA, "A", l))) return rc;
+            if ((rc = upload_packed(h, lv.A, lv.dinv.data(), &lv.cf, &g.sA, g.layA, "A", l))) return rc;
             if (l < L) {
-                if ((rc = upload_packed(h, lv.P, nullptr, &g.sP, g.layP, "P", l))) return rc;
-                if ((rc = upload_packed(h, lv.R, h->H.lv[l + 1].dinv.data(), &g.sR, g.layR, "R", l))) return rc;
+                if ((rc = upload_packed(h, lv.P, nullptr, nullptr, &g.sP, g.layP, "P", l))) return rc;
+                if ((rc = upload_packed(h, lv.R, h->H.lv[l + 1].dinv.data(), &h->H.lv[l + 1].cf, &g.sR, g.layR, "R", l))) return rc;
             }
             if ((rc = upload(h, &g.dinv, lv.dinv.data(), lv.dinv.size()))) return rc;
             std::vector<int> id((size_t)lv.A.nrows);
@@ -426,6 +431,7 @@ int finish_tables(amgdd_handle_s* h) {
     }
     if ((rc = upload(h, &h->d_lu, h->H.lu.data(), h->H.lu.size()))) return rc;
     if ((rc = upload(h, &h->d_rowperm, h->H.rowperm.data(), h->H.rowperm.size()))) return rc;
+    if (L > 0) { if ((rc = upload(h, &h->d_cf0, h->H.lv[0].cf.data(), h->H.lv[0].cf.size()))) return rc; }
     h->partial_cap = residual_num_blocks(h->n, h->glev[0].lanes_a);
     if ((rc = dev_alloc(h, (void**)&h->d_partial, (size_t)h->partial_cap * sizeof(double)))) return rc;
     h->norms_cap = 1024;
@@ -544,6 +550,13 @@ int amgdd_destroy(amgdd_handle_t h) {
     return AMGDD_SUCCESS;
 }
 
+int amgdd_set_smoother(amgdd_handle_t h, int32_t type) {
+    if (bad_handle(h)) return AMGDD_ERR_BAD_ARG;
+    if (type != AMGDD_SMOOTHER_L1_JACOBI && type != AMGDD_SMOOTHER_CF_L1_JACOBI) { g_detail = "unknown smoother"; return AMGDD_ERR_BAD_ARG; }
+    h->smoother = type;
+    return AMGDD_SUCCESS;
+}
+
 int amgdd_set_stream(amgdd_handle_t h, void* s) {
     if (bad_handle(h)) return AMGDD_ERR_BAD_ARG;
     h->stream = (cudaStream_t)s;
@@ -584,18 +597,18 @@ int amgdd_solve(amgdd_handle_t h, const double* b, double* x, int32_t num_cycles
         cudaEventRecord(e, h->stream);
         ev.push_back(e);
     };
-    if (h->prog_nfac != num_fac_cycles || h->prog_nu != relax_sweeps) {       // (re)build the program of one subdomain
-        const int nops = fac_build_program(L, num_fac_cycles, relax_sweeps, nullptr);
+    if (h->prog_nfac != num_fac_cycles || h->prog_nu != relax_sweeps || h->prog_smoother != h->smoother) {       // (re)build the program of one subdomain
+        const int nops = fac_build_program(L, num_fac_cycles, relax_sweeps, h->smoother, nullptr);
         if (nops > MAX_OPS || L > 84) {
             g_detail = "num_fac_cycles x relax_sweeps x levels gives a program of " + std::to_string(nops) + " steps; the kernel holds " +
                        std::to_string(MAX_OPS);
             return AMGDD_ERR_BAD_ARG;
         }
         std::vector<FacOp> ops((size_t)nops);
-        fac_build_program(L, num_fac_cycles, relax_sweeps, ops.data());
+        fac_build_program(L, num_fac_cycles, relax_sweeps, h->smoother, ops.data());
         CUDA_TRY(cudaMemcpyAsync(h->d_ops, ops.data(), ops.size() * sizeof(FacOp), cudaMemcpyHostToDevice, h->stream));
         CUDA_TRY(cudaStreamSynchronize(h->stream));
-        h->prog_nfac = num_fac_cycles; h->prog_nu = relax_sweeps; h->prog_nops = nops;
+        h->prog_nfac = num_fac_cycles; h->prog_nu = relax_sweeps; h->prog_smoother = h->smoother; h->prog_nops = nops;
         // shared-memory vector buffers: as large as the largest level needs, but leave the L1 (which
         // shares the SM's 228 KB with shared memory) room for the loads in flight: with less than
         // ~48 KB of L1 the streaming rate of this kernel drops by 15% (profiles/).  Levels that do
@@ -618,6 +631,7 @@ int amgdd_solve(amgdd_handle_t h, const double* b, double* x, int32_t num_cycles
     prm.work_counter = h->d_counter;
     prm.ops = h->d_ops; prm.nops = h->prog_nops;
     prm.lu = h->d_lu; prm.rowperm = h->d_rowperm; prm.nL = (int)h->H.nL;
+    prm.cf0 = h->d_cf0;
     prm.x_cap = h->x_cap;
     prm.prof = h->d_prof;
     prm.prof_ops = h->d_prof_ops;
@@ -708,6 +722,7 @@ static int ensure_vcycle(amgdd_handle_s* h) {
             g.lanes_p = pick_lanes(avg_row(lv.P));
         }
         if ((rc = upload(h, &g.vdinv, lv.dinv.data(), lv.dinv.size()))) return rc;
+        if (l < L) { if ((rc = upload(h, &g.vcf, lv.cf.data(), lv.cf.size()))) return rc; }
         if ((rc = dev_alloc(h, (void**)&g.vu0, nl * sizeof(double)))) return rc;
         if ((rc = dev_alloc(h, (void**)&g.vu1, nl * sizeof(double)))) return rc;
         if ((rc = dev_alloc(h, (void**)&g.vf, nl * sizeof(double)))) return rc;
@@ -726,6 +741,7 @@ int amgdd_vcycle(amgdd_handle_t h, const double* b, double* x, int32_t num_cycle
     int rc = ensure_vcycle(h);
     if (rc) return rc;
     const int L = h->H.L;
+    const bool cfm = h->smoother == AMGDD_SMOOTHER_CF_L1_JACOBI;
     cudaStream_t st = h->stream;
     auto nrows = [&](int l) { return (long long)h->H.lv[l].A.nrows; };
     for (int k = 0; k < num_cycles; ++k) {
@@ -735,11 +751,13 @@ int amgdd_vcycle(amgdd_handle_t h, const double* b, double* x, int32_t num_cycle
             const double* f = l == 0 ? b : g.vf;
             bool have_u = l == 0;                                               // coarse levels start from u = 0
             if (l == 0) CUDA_TRY(cudaMemcpyAsync(g.vu0, x, (size_t)nrows(0) * sizeof(double), cudaMemcpyDeviceToDevice, st));
-            for (int s = 0; s < nu1; ++s) {                                     // the level's iterate lives in vu0
-                launch_relax(g.a_rp, g.a_ci, g.a_v, nrows(l), g.lanes_a, g.vdinv, f, have_u ? g.vu0 : nullptr, g.vu1, st);
-                std::swap(g.vu0, g.vu1);
-                have_u = true;
-            }
+            for (int s = 0; s < nu1; ++s)                                       // the level's iterate lives in vu0
+                for (int half = 0; half < (cfm ? 2 : 1); ++half) {              // CF smoother: C-points, then F-points
+                    launch_relax(g.a_rp, g.a_ci, g.a_v, nrows(l), g.lanes_a, g.vdinv, f, have_u ? g.vu0 : nullptr, g.vu1,
+                                 cfm ? (const signed char*)g.vcf : nullptr, half == 0 ? +1 : -1, st);
+                    std::swap(g.vu0, g.vu1);
+                    have_u = true;
+                }
             if (!have_u) CUDA_TRY(cudaMemsetAsync(g.vu0, 0, (size_t)nrows(l) * sizeof(double), st));
             launch_spmv_axpy(g.a_rp, g.a_ci, g.a_v, nrows(l), g.lanes_a, g.vu0, f, g.vr, 0, st);        // r = f - A u
             launch_spmv(g.r_rp, g.r_ci, g.r_v, nrows(l + 1), g.lanes_r, g.vr, h->glev[l + 1].vf, st);   // f_{l+1} = P^T r
@@ -749,7 +767,12 @@ int amgdd_vcycle(amgdd_handle_t h, const double* b, double* x, int32_t num_cycle
             GlobalLevelDev& g = h->glev[l];
             const double* f = l == 0 ? b : g.vf;
             launch_spmv_axpy(g.p_rp, g.p_ci, g.p_v, nrows(l), g.lanes_p, h->glev[l + 1].vu0, nullptr, g.vu0, 1, st);   // u += P u_{l+1}
-            for (int s = 0; s < nu2; ++s) { launch_relax(g.a_rp, g.a_ci, g.a_v, nrows(l), g.lanes_a, g.vdinv, f, g.vu0, g.vu1, st); std::swap(g.vu0, g.vu1); }
+            for (int s = 0; s < nu2; ++s)
+                for (int half = 0; half < (cfm ? 2 : 1); ++half) {              // CF smoother: F-points, then C-points
+                    launch_relax(g.a_rp, g.a_ci, g.a_v, nrows(l), g.lanes_a, g.vdinv, f, g.vu0, g.vu1,
+                                 cfm ? (const signed char*)g.vcf : nullptr, half == 0 ? -1 : +1, st);
+                    std::swap(g.vu0, g.vu1);
+                }
             if (l == 0) CUDA_TRY(cudaMemcpyAsync(x, g.vu0, (size_t)nrows(0) * sizeof(double), cudaMemcpyDeviceToDevice, st));
         }
     }
@@ -763,8 +786,8 @@ int amgdd_vcycle(amgdd_handle_t h, const double* b, double* x, int32_t num_cycle
 }
 
 int amgdd_pack_stream(int32_t nrows, int32_t n_real, const int32_t* rowptr32, const int32_t* colind, const double* vals,
-                      const double* aux, int32_t wide, int32_t window, void* out, int64_t out_capacity, int64_t* out_bytes,
-                      amgdd_way_t* out_ways) {
+                      const double* aux, const uint8_t* row_flags, int32_t wide, int32_t window, void* out, int64_t out_capacity,
+                      int64_t* out_bytes, amgdd_way_t* out_ways) {
     g_detail.clear();
     if (nrows < 0 || n_real < 0 || n_real > nrows || !rowptr32 || (!colind && rowptr32[nrows] > 0) ||
         (!vals && rowptr32[nrows] > 0) || rowptr32[0] != 0 || window < SLICE_ROWS || window > MAX_WINDOW || (window % SLICE_ROWS)) {
@@ -784,7 +807,7 @@ int amgdd_pack_stream(int32_t nrows, int32_t n_real, const int32_t* rowptr32, co
     if (out_ways) std::memcpy(out_ways, pp.way, sizeof(pp.way));
     if (out) {
         if (out_capacity < pp.bytes) { g_detail = "output buffer too small"; return AMGDD_ERR_BAD_ARG; }
-        write_stream(nrows, rowptr32, colind, vals, aux, wide != 0, n_real, window, (char*)out);
+        write_stream(nrows, rowptr32, colind, vals, aux, wide != 0, n_real, window, (char*)out, row_flags);
     }
     return AMGDD_SUCCESS;
 }
@@ -822,7 +845,7 @@ int amgdd_debug_fac_op_cycles(amgdd_handle_t h, int64_t* out, int32_t n, int32_t
             for (int q = 0; q < 4; ++q) out[q * n + j] += host[(size_t)b * PROF_OPS_STRIDE + q * MAX_OPS + j];
     if (kinds_levels) {
         std::vector<FacOp> ops((size_t)std::max(1, h->prog_nops));
-        fac_build_program(h->H.L, h->prog_nfac, h->prog_nu, ops.data());
+        fac_build_program(h->H.L, h->prog_nfac, h->prog_nu, h->prog_smoother, ops.data());
         for (int j = 0; j < n && j < h->prog_nops; ++j) kinds_levels[j] = ops[j].kind * 256 + ops[j].level;
     }
     CUDA_TRY(cudaMemset(h->d_prof_ops, 0, cnt * sizeof(long long)));

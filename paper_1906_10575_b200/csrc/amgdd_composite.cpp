@@ -210,19 +210,25 @@ void CompositeBuilder::fill(const SubdomainBlob& plan, char* dst) {
         const i32 nbc = plan.lev[l + 1].n_real + plan.lev[l + 1].n_ghost;
         aux_.assign((size_t)nb, 0.0);                                    // ghost rows never relax (A4)
         for (i32 i = 0; i < nr; ++i) aux_[i] = dinv[i];
-        write_stream(nb, A_[l].rp.data(), A_[l].ci.data(), A_[l].v.data(), aux_.data(), b.A.wide, nr, window_, dst + b.A.off);
+        flg_.assign((size_t)nb, 0);                                      // C-points among the real rows (CF smoother)
+        for (i32 i = 0; i < nr; ++i) flg_[i] = lv.cf[gid[i]] > 0 ? 1 : 0;
+        write_stream(nb, A_[l].rp.data(), A_[l].ci.data(), A_[l].v.data(), aux_.data(), b.A.wide, nr, window_, dst + b.A.off, flg_.data());
         write_stream(nb, P_[l].rp.data(), P_[l].ci.data(), P_[l].v.data(), nullptr, b.P.wide, nb, thin_window(), dst + b.P.off);
-        {   // R_l rows are the points of level l+1: aux = their l1 diagonal (real points), 0 on ghosts
+        {   // R_l rows are the points of level l+1: aux = their l1 diagonal (real points), 0 on ghosts; flag = their C/F class
             const BlockLayout& c = plan.lev[l + 1];
             const HostLevel& lc = H_.lv[l + 1];
             auxr_.assign((size_t)nbc, 0.0);
-            for (i32 i = 0; i < c.n_real; ++i) auxr_[i] = lc.dinv[real_[l + 1][i]];
-            write_stream(nbc, R_[l].rp.data(), R_[l].ci.data(), R_[l].v.data(), auxr_.data(), b.R.wide, nbc, thin_window(), dst + b.R.off);
+            flg_.assign((size_t)nbc, 0);
+            for (i32 i = 0; i < c.n_real; ++i) {
+                auxr_[i] = lc.dinv[real_[l + 1][i]];
+                if (!lc.cf.empty()) flg_[i] = lc.cf[real_[l + 1][i]] > 0 ? 1 : 0;
+            }
+            write_stream(nbc, R_[l].rp.data(), R_[l].ci.data(), R_[l].v.data(), auxr_.data(), b.R.wide, nbc, thin_window(), dst + b.R.off, flg_.data());
         }
     }
 }
 
-bool pack_global_stream(const HostCsr& M, const double* aux, int window, PackedLevelStream& out, i64& too_long_row) {
+bool pack_global_stream(const HostCsr& M, const double* aux, const uint8_t* row_flags, int window, PackedLevelStream& out, i64& too_long_row) {
     if (M.nnz() > (i64)INT32_MAX || M.nrows > (i64)INT32_MAX) return false;
     LocalCsr T;
     T.rp.assign(M.rp.begin(), M.rp.end());
@@ -231,7 +237,7 @@ bool pack_global_stream(const HostCsr& M, const double* aux, int window, PackedL
     too_long_row = bad;
     if (bad >= 0) return true;
     out.data.assign((size_t)out.lay.bytes, 0);
-    write_stream((int)M.nrows, T.rp.data(), M.ci.data(), M.v.data(), aux, out.lay.wide, (int)M.nrows, window, out.data.data());
+    write_stream((int)M.nrows, T.rp.data(), M.ci.data(), M.v.data(), aux, out.lay.wide, (int)M.nrows, window, out.data.data(), row_flags);
     return true;
 }
 

@@ -205,9 +205,11 @@ struct Worker {
         const double* dinv = lev[0].dinv;
         double *u = U(0), *t = T(0);
         const double* f = F(0);
+        const bool cfmode = op.flags & OPF_CF;                               // CF smoother: the C half of the sweep; the F half follows
+        const int* gid = lev[0].gid;
         for (int i = tid; i < n_bar; i += NTHREADS) {
             double dl = 0.0;
-            if (i < n_real) { dl = __ldg(dinv + i) * f[i]; u[i] = dl; t[i] += dl; }
+            if (i < n_real && !(cfmode && prm->cf0[__ldg(gid + i)] <= 0)) { dl = __ldg(dinv + i) * f[i]; u[i] = dl; t[i] += dl; }
             xo.st(i, dl);
         }
     }
@@ -275,6 +277,7 @@ struct Worker {
         const long long tp0 = tick();
         const int kind = op.kind, l = op.level;
         const bool first = op.flags & OPF_FIRST, tsmem = op.flags & OPF_TSMEM, coarsest = op.flags & OPF_COARSEST;
+        const bool half_c = op.flags & OPF_HALF_C, half_f = op.flags & OPF_HALF_F, cfmode = op.flags & OPF_CF;
         const XB xg = xbuf_of(op.gbuf, gather_level(op)), xo = xbuf_of(op.gbuf ^ 1, out_level(op));
         // ---- this warp's way of the stream, and of the next mat-vec's stream ----
         const WayEnt we = wt[stream_of(op) * NUM_WAYS + wid];
@@ -356,7 +359,8 @@ struct Worker {
         cp_async_wait_all();
         uint4 h = lds128(stH);
         uint32_t row = h.x;
-        int left = (int)h.y;
+        int left = (int)(h.y & HDR_GROUPS_MASK);
+        bool is_c = (h.y >> 31) != 0;                                       // the row is a C-point of its level
         double aux = mkdouble(h.z, h.w);
         fetch_ctx(row);
         cp_async16(stH, nsl > 1 ? hdr + HEADER_BYTES : hdr_after);
@@ -381,10 +385,15 @@ struct Worker {
             if (row != NO_ROW) {
                 const double e0 = lds_f64(stC), e1 = lds_f64(stC + 256), e2 = lds_f64(stC + 512);   // unused ones are stale, never read
                 if (kind == OPK_RELAX) {           // one l1-Jacobi update (§4.1); aux = 1 / sum_j |a_ij| (S8)
-                    const double dl = aux * (e0 - acc);
-                    const double un = xg.ld(row) + dl, tn = e1 + dl;
-                    pu[row] = un; pt[row] = tn;
-                    xo.st(row, tsmem ? tn : un);
+                    const double uo = xg.ld(row);
+                    if ((half_c && !is_c) || (half_f && is_c)) {   // CF smoother: not this half-sweep's class
+                        xo.st(row, tsmem ? e1 : uo);
+                    } else {
+                        const double dl = aux * (e0 - acc);
+                        const double un = uo + dl, tn = e1 + dl;
+                        pu[row] = un; pt[row] = tn;
+                        xo.st(row, tsmem ? tn : un);
+                    }
                 } else if (kind == OPK_AT) {       // P:509 w = s_l + A_l t_l
                     xo.st(row, e0 + acc);
                 } else if (kind == OPK_RESTRICT) { // P:509 s_{l+1} = R_l w
@@ -394,7 +403,7 @@ struct Worker {
                             const double f = e0 - acc;
                             pf[row] = f;
                             if (!coarsest) {
-                                const double u = aux * f, tn = e1 + u;
+                                const double u = (cfmode && !is_c) ? 0.0 : aux * f, tn = e1 + u;   // CF smoother: the C half of the sweep
                                 pu[row] = u; pt[row] = tn;
                                 xo.st(row, tsmem ? tn : u);
                             }
@@ -404,7 +413,7 @@ struct Worker {
                     const double f = (e0 - acc) - e1;
                     pf[row] = f;
                     if (!coarsest) {
-                        const double u = aux * f, tn = e2 + u;
+                        const double u = (cfmode && !is_c) ? 0.0 : aux * f, tn = e2 + u;           // CF smoother: the C half of the sweep
                         pu[row] = u; pt[row] = tn;
                         xo.st(row, tsmem ? tn : u);
                     }
@@ -418,7 +427,7 @@ struct Worker {
             acc = 0.0;
             if (sidx < nsl) {
                 h = lds128(stH);
-                row = h.x; left = (int)h.y; aux = mkdouble(h.z, h.w);
+                row = h.x; left = (int)(h.y & HDR_GROUPS_MASK); is_c = (h.y >> 31) != 0; aux = mkdouble(h.z, h.w);
                 fetch_ctx(row);
                 cp_async16(stH, sidx + 1 < nsl ? hdr + (long long)(sidx + 1) * HEADER_BYTES : hdr_after);
             }
@@ -579,7 +588,7 @@ __global__ void __launch_bounds__(NTHREADS, CTAS_PER_SM) fac_kernel(const FacPar
 
 // The static program of one subdomain: the steps of num_fac_cycles AlgFAC V(nu,nu)-cycles (Alg. 4)
 // in order, with the shared-memory buffer each mat-vec gathers from (it writes the other one).
-int fac_build_program(int L, int nfac, int nu, FacOp* ops) {
+int fac_build_program(int L, int nfac, int nu, int smoother, FacOp* ops) {
     int n = 0;
     auto emit = [&](int kind, int level, int gbuf, int flags) {
         if (ops && n < MAX_OPS) {
@@ -590,25 +599,39 @@ int fac_build_program(int L, int nfac, int nu, FacOp* ops) {
         }
         ++n;
     };
+    const bool cf = smoother == 1;                                           // CF l1-Jacobi: two half-sweeps per sweep
     int cur = 0;                                                             // buffer that holds the live gather vector
+    // one relaxation sweep on level l (P:507-508 / P:517-518); `last_pre`: the A t step follows, leave t behind;
+    // `skip_first_half`: the sweep's first half was the matrix-free sweep from u = 0 fused into the step before
+    auto sweep = [&](int l, int first, bool pre, bool last_pre, bool skip_first_half) {
+        if (!cf) { emit(OPK_RELAX, l, cur, first | (last_pre ? OPF_TSMEM : 0)); cur ^= 1; return; }
+        const int h1 = pre ? OPF_HALF_C : OPF_HALF_F, h2 = pre ? OPF_HALF_F : OPF_HALF_C;   // C then F before, F then C after the coarse correction
+        if (!skip_first_half) { emit(OPK_RELAX, l, cur, first | h1); cur ^= 1; }
+        emit(OPK_RELAX, l, cur, first | h2 | (last_pre ? OPF_TSMEM : 0)); cur ^= 1;
+    };
+    const int cff = cf ? OPF_CF : 0;
     emit(OPK_BEGIN, 0, 0, 0);                                                // Alg. 2, Alg. 4
     for (int it = 0; it < nfac; ++it) {
         const int first = it == 0 ? OPF_FIRST : 0;
+        // does the sweep from u = 0, fused into the step before, leave t (not u) in the buffer?  only if nothing follows it
+        const int fused_t = (nu == 1 && !cf) ? OPF_TSMEM : 0;
         for (int l = 0; l < L; ++l) {                                        // downsweep P:505-513
             const int coarsest = (l + 1 == L) ? OPF_COARSEST : 0;
             int k = 0;
-            if (l == 0 && first) { emit(OPK_FIRST0, 0, cur, first | (nu == 1 ? OPF_TSMEM : 0)); cur ^= 1; k = 1; }
-            if (l != 0) k = 1;                                               // the first sweep was fused into the step before
-            for (; k < nu; ++k) { emit(OPK_RELAX, l, cur, first | (k == nu - 1 ? OPF_TSMEM : 0)); cur ^= 1; }
+            bool fused = false;
+            if (l == 0 && first) { emit(OPK_FIRST0, 0, cur, first | fused_t | cff); cur ^= 1; fused = true; }
+            if (l != 0) fused = true;                                        // fused into the restriction / recalculation before
+            if (fused) { if (cf) sweep(l, first, true, nu == 1, true); k = 1; }
+            for (; k < nu; ++k) sweep(l, first, true, k == nu - 1, false);
             emit(OPK_AT, l, cur, first); cur ^= 1;                           // P:509  w = s_l + A_l t_l
-            const int fl = first | coarsest | (nu == 1 ? OPF_TSMEM : 0);
+            const int fl = first | coarsest | fused_t | cff;
             emit(OPK_RESTRICT, l, cur, fl); cur ^= 1;                        // P:509  s_{l+1} = R_l w 
             if (!first) { emit(OPK_RECALC, l + 1, cur, fl); cur ^= 1; }      // P:510  (identically zero at it = 0)
         }
         emit(OPK_COARSE, L, cur, first); cur ^= 1;
         for (int l = L - 1; l >= 0; --l) {                                   // upsweep P:515-519
             emit(OPK_INTERP, l, cur, first); cur ^= 1;
-            for (int k = 0; k < nu; ++k) { emit(OPK_RELAX, l, cur, first); cur ^= 1; }
+            for (int k = 0; k < nu; ++k) sweep(l, first, false, false, false);
         }
     }
     emit(OPK_END, 0, 0, 0);                                                  // Alg. 2

@@ -144,6 +144,7 @@ private:
     std::vector<i32> epoch_;
     std::vector<i32> frontier_, next_, cursor_;
     std::vector<double> aux_, auxr_;
+    std::vector<uint8_t> flg_;
     i32 local_of(int l, i32 g) const { return stamp_[l][g] == epoch_[l] ? loc_[l][g] : -1; }
 };
 
@@ -153,6 +154,7 @@ struct PackedLevelStream {
     StreamLayout lay;
 };
 // aux: M.nrows doubles (l1 diagonal inverse, A streams) or nullptr
-bool pack_global_stream(const HostCsr& M, const double* aux, int window, PackedLevelStream& out, i64& too_long_row);
+// row_flags: M.nrows bytes (1: C-point of the rows' level) or nullptr
+bool pack_global_stream(const HostCsr& M, const double* aux, const uint8_t* row_flags, int window, PackedLevelStream& out, i64& too_long_row);
 
 }  // namespace amgdd

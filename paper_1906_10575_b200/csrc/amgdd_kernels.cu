@@ -76,16 +76,19 @@ __global__ void __launch_bounds__(GLOBAL_BLOCK) spmv_kernel(const int* __restric
 __global__ void __launch_bounds__(GLOBAL_BLOCK) relax_kernel(const int* __restrict__ rp, const int* __restrict__ ci,
                                                              const double* __restrict__ v, long long n, int lanes,
                                                              const double* __restrict__ dinv, const double* __restrict__ f,
-                                                             const double* __restrict__ u_in, double* __restrict__ u_out) {
+                                                             const double* __restrict__ u_in, double* __restrict__ u_out,
+                                                             const signed char* __restrict__ cf, int cls) {
     const int lane = threadIdx.x & (lanes - 1);
     const long long row = (long long)blockIdx.x * (GLOBAL_BLOCK / lanes) + threadIdx.x / lanes;
+    // CF smoother: cf != nullptr restricts the update to the rows of one class (cls > 0: C-points), the others keep u
+    const bool active = row < n && (!cf || ((cf[row] > 0) == (cls > 0)));
     double sum = 0.0;
-    if (row < n && u_in) {
+    if (active && u_in) {
         const int bgn = __ldg(rp + row), end = __ldg(rp + row + 1);
         for (int k = bgn + lane; k < end; k += lanes) sum += __ldg(v + k) * __ldg(u_in + __ldg(ci + k));
     }
     for (int o = lanes >> 1; o > 0; o >>= 1) sum += __shfl_down_sync(0xffffffffu, sum, o, lanes);
-    if (row < n && lane == 0) u_out[row] = (u_in ? u_in[row] : 0.0) + dinv[row] * (f[row] - sum);
+    if (row < n && lane == 0) u_out[row] = (u_in ? u_in[row] : 0.0) + (active ? dinv[row] * (f[row] - sum) : 0.0);
 }
 
 // y = f - A x (f = nullptr: y = A x); accumulate = 1: y += A x
@@ -128,9 +131,9 @@ __global__ void __launch_bounds__(256) coarse_solve_kernel(const double* __restr
 }  // namespace
 
 void launch_relax(const int* rp, const int* ci, const double* v, long long n, int lanes, const double* dinv, const double* f,
-                  const double* u_in, double* u_out, void* stream) {
+                  const double* u_in, double* u_out, const signed char* cf, int cls, void* stream) {
     if (n <= 0) return;
-    relax_kernel<<<residual_num_blocks(n, lanes), GLOBAL_BLOCK, 0, (cudaStream_t)stream>>>(rp, ci, v, n, lanes, dinv, f, u_in, u_out);
+    relax_kernel<<<residual_num_blocks(n, lanes), GLOBAL_BLOCK, 0, (cudaStream_t)stream>>>(rp, ci, v, n, lanes, dinv, f, u_in, u_out, cf, cls);
 }
 
 void launch_spmv_axpy(const int* rp, const int* ci, const double* v, long long n, int lanes, const double* x, const double* f,

@@ -92,7 +92,7 @@ PackPlan plan_stream(int nrows, const int32_t* rp, bool wide, bool has_aux, int 
 }
 
 void write_stream(int nrows, const int32_t* rp, const int32_t* ci, const double* v, const double* aux, bool wide,
-                  int n_real, int window, char* dst) {
+                  int n_real, int window, char* dst, const uint8_t* row_flags) {
     const bool has_aux = aux != nullptr;
     const int gbytes = group_bytes(wide), hbytes = HEADER_BYTES;
     std::vector<Slice> slices;
@@ -108,7 +108,7 @@ void write_stream(int nrows, const int32_t* rp, const int32_t* ci, const double*
             const Slice& sl = slices[si];
             for (int j = 0; j < SLICE_ROWS; ++j) {
                 const uint32_t row = sl.rows[j] >= 0 ? (uint32_t)sl.rows[j] : NO_ROW;
-                const uint32_t k = (uint32_t)sl.K;
+                const uint32_t k = (uint32_t)sl.K | ((row_flags && sl.rows[j] >= 0 && row_flags[sl.rows[j]]) ? 0x80000000u : 0u);
                 char* q = h + 16 * j;
                 const double a = (has_aux && sl.rows[j] >= 0) ? aux[sl.rows[j]] : 0.0;
                 std::memcpy(q, &row, 4); std::memcpy(q + 4, &k, 4); std::memcpy(q + 8, &a, 8);

@@ -30,9 +30,10 @@
 //                                32 x { uint16 col[step 0..3] }           lane j at 1024 + 8 j
 //   group (wide, 1536 bytes):    the same two value planes, then 32 x { uint32 col[step 0..3] },
 //                                lane j at 1024 + 16 j
-//   header (512 bytes):  32 x { uint32 row, uint32 ngroups, double aux }   lane j at 16 j
-//            row = the lane's row (NO_ROW: the slice has fewer than 32 rows), ngroups = K of the
-//            slice (the same in every lane), aux = a per-row value the epilogue needs (the l1
+//   header (512 bytes):  32 x { uint32 row, uint32 info, double aux }   lane j at 16 j
+//            row = the lane's row (NO_ROW: the slice has fewer than 32 rows), info = K of the
+//            slice (the same in every lane) | the row's flag << 31 (C-point of its level: the CF
+//            smoother relaxes the two classes in turn), aux = a per-row value the epilogue needs (the l1
 //            diagonal inverse, S8; 0.0 in streams packed without an aux vector).  One header
 //            shape for all streams keeps every load of the kernel unconditional.
 #pragma once
@@ -64,6 +65,7 @@ constexpr int DEFAULT_WINDOW = 256;
 constexpr int THIN_WINDOW = AMGDD_THIN_WINDOW;    // sort window of the P_l / R_l streams
 constexpr int MAX_WINDOW = 1 << 20;
 constexpr uint32_t NO_ROW = 0xFFFFFFFFu;
+constexpr uint32_t HDR_GROUPS_MASK = 0x7FFFFFFFu;   // header info: groups of the slice; bit 31: the row's flag
 constexpr int RING_DEPTH = AMGDD_RING_DEPTH;  // groups per register block = groups per burst of loads; a warp holds two blocks
 
 inline int group_bytes(bool wide) { return wide ? GROUP_BYTES_WIDE : GROUP_BYTES_NARROW; }
@@ -124,6 +126,9 @@ enum OpKind : uint8_t {
 constexpr uint8_t OPF_FIRST = 1;      // first AlgFAC iteration of the cycle
 constexpr uint8_t OPF_TSMEM = 2;      // the shared-memory output is t (the gather vector of the A t step), else u
 constexpr uint8_t OPF_COARSEST = 4;   // RESTRICT / RECALC whose target level is L: no relaxation follows
+constexpr uint8_t OPF_HALF_C = 8;     // CF smoother: this relaxation step updates the C-points only
+constexpr uint8_t OPF_HALF_F = 16;    // ... the F-points only
+constexpr uint8_t OPF_CF = 32;        // CF smoother: a fused first sweep (u = 0) is its C half only, the F half follows as a step
 
 struct FacOp {
     uint8_t kind;          // OpKind
@@ -154,6 +159,7 @@ struct FacParams {
     const double* lu;          // dense LU of A_L, column-major, unit lower
     const int* rowperm;
     int nL;
+    const int8_t* cf0;         // C/F flags of level 0 (global numbering), for the matrix-free first sweep of the CF smoother
     int x_cap;                 // doubles in each of the two shared-memory vector buffers (0: vectors in global memory)
     long long* prof;           // optional: gridDim.x * FAC_PROF_SLOTS cycle counters (debugging), or nullptr
     long long* prof_ops;       // optional: gridDim.x * PROF_OPS_STRIDE: per step of the program: cycles | barrier wait after it | waits for ring blocks | waits for staged slice operands
@@ -178,13 +184,13 @@ struct PackPlan {
 };
 // rp: nrows+1 int32 offsets (rp[0] = 0); window: rows per sort window (multiple of 32)
 PackPlan plan_stream(int nrows, const int32_t* rp, bool wide, bool has_aux, int n_real, int window);
-// writes plan.bytes bytes; aux: nrows doubles or nullptr (must match has_aux of the plan)
+// writes plan.bytes bytes; aux: nrows doubles or nullptr (must match has_aux of the plan); row_flags: nrows bytes (0/1) or nullptr
 void write_stream(int nrows, const int32_t* rp, const int32_t* ci, const double* v, const double* aux, bool wide,
-                  int n_real, int window, char* dst);
+                  int n_real, int window, char* dst, const uint8_t* row_flags = nullptr);
 
 // the program of one subdomain: num_fac_cycles AlgFAC V(nu,nu)-cycles (Alg. 4); returns the op count
 // (ops may be nullptr to count only)
-int fac_build_program(int L, int nfac, int nu, FacOp* ops);
+int fac_build_program(int L, int nfac, int nu, int smoother, FacOp* ops);   // smoother: 0 l1-Jacobi, 1 CF l1-Jacobi
 int fac_smem_bytes(int x_cap, int L, int nops);
 void launch_fac(const FacParams& prm, const FacLaunch& cfg, void* stream);
 int fac_configure(int device, int max_smem_optin);   // sets the kernel's dynamic-smem attribute; 0 on success

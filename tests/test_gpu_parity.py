@@ -85,8 +85,11 @@ def run_parity(p, num_cycles, nfac=2, nu=1, yardstick=False, **kw):
     for the residual norm) times YARD is added to the tolerance: the bar is then "as close to the
     oracle as the fp64 conditioning of this problem allows" (Parity criterion)."""
     torch = _torch()
+    smoother = kw.pop("smoother", 0)
     m, h = lib_setup(p, **kw)
     o = orc_setup(p, **kw)
+    m.amgdd_set_smoother(h, smoother)
+    o.set_smoother(smoother)
     check_index_exact(m, h, o, p, range(p.num_subdomains) if p.num_subdomains <= 64 else
                       np.linspace(0, p.num_subdomains - 1, 16).astype(int))
     b = torch.from_numpy(p.b).cuda()
@@ -99,6 +102,7 @@ def run_parity(p, num_cycles, nfac=2, nu=1, yardstick=False, **kw):
         pp = copy.copy(p)
         pp.vals = ulp_perturbed_values(p)
         o2 = orc_setup(pp, **kw)
+        o2.set_smoother(smoother)
         xo2 = np.zeros(p.n)
     report, ok = [], True
     for k in range(num_cycles):
@@ -175,14 +179,22 @@ def test_wide_column_indices():
     run_parity(wl.make_config(1, 272, parts_per_dim=1), 2)
 
 
-@pytest.mark.parametrize("cfg,scale,nu1,nu2", [(2, 32, 1, 1), (4, 24, 2, 1), (1, None, 1, 2), (5, 128, 1, 1)])
-def test_amg_vcycle_matches_the_oracle(cfg, scale, nu1, nu2):
+@pytest.mark.parametrize("cfg,scale,nfac,nu", [(1, None, 2, 1), (2, 32, 2, 1), (2, 32, 3, 2), (4, 48, 2, 1), (3, 32, 2, 2), (5, 256, 2, 1)])
+def test_cf_l1_jacobi_smoother(cfg, scale, nfac, nu):
+    """NEXT 1 of SURVEY.md section 8(f): the paper's CF l1-scaled Jacobi (reading A2b) against the oracle."""
+    run_parity(wl.make_config(cfg, scale), 4, nfac=nfac, nu=nu, yardstick=(cfg == 5), smoother=1)
+
+
+@pytest.mark.parametrize("cfg,scale,nu1,nu2,smoother", [(2, 32, 1, 1, 0), (4, 24, 2, 1, 0), (1, None, 1, 2, 0), (5, 128, 1, 1, 0), (2, 32, 1, 1, 1), (4, 24, 2, 2, 1)])
+def test_amg_vcycle_matches_the_oracle(cfg, scale, nu1, nu2, smoother):
     """NEXT 2 of SURVEY.md section 8(f): the AMG V-cycle of Alg. 1 (the paper's comparison method) on the GPU
     against the oracle's orc_vcycle (pinned to the scipy V-cycle of tests/reference_global.py)."""
     torch = _torch()
     p = wl.make_config(cfg, scale)
     m, h = lib_setup(p)
     o = orc_setup(p)
+    m.amgdd_set_smoother(h, smoother)
+    o.set_smoother(smoother)
     b = torch.from_numpy(p.b).cuda()
     x = torch.zeros(p.n, dtype=torch.float64, device="cuda")
     xo = np.zeros(p.n)

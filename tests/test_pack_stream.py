@@ -20,6 +20,8 @@ def decode(stream, ways, wide, nrows, n_real=None, window=256):
     gb = m.GROUP_BYTES_WIDE if wide else m.GROUP_BYTES_NARROW
     rows = [None] * nrows
     aux = np.full(nrows, np.nan)
+    flags = np.zeros(nrows, dtype=np.int64)
+    decode.flags = flags
     load = []
     # groups of all ways come first, back to back; then the headers, each way 128-byte aligned
     off = 0
@@ -38,7 +40,8 @@ def decode(stream, ways, wide, nrows, n_real=None, window=256):
         for s in range(int(w["nslices"])):
             hdr = np.frombuffer(raw, dtype=np.uint32, count=128, offset=h + s * HB).reshape(32, 4)
             a = np.frombuffer(raw, dtype=np.float64, count=64, offset=h + s * HB).reshape(32, 2)[:, 1]
-            rid, K = hdr[:, 0].astype(np.int64), hdr[:, 1]
+            rid, K = hdr[:, 0].astype(np.int64), hdr[:, 1] & 0x7FFFFFFF
+            flag = hdr[:, 1] >> 31
             assert (K == K[0]).all() and K[0] >= 1, "every lane carries the slice's group count"
             K = int(K[0])
             valid = rid != NO_ROW
@@ -70,6 +73,7 @@ def decode(stream, ways, wide, nrows, n_real=None, window=256):
                 assert rows[r] is None, "every row is stored once"
                 rows[r] = (cols[j], vals[j])
                 aux[r] = a[j]
+                flags[r] = flag[j]
         assert groups_seen == int(w["ngroups"]) and real_groups == int(w["ngroups_real"]) and real_slices == int(w["nslices_real"])
         load.append(int(w["ngroups"]) * gb + int(w["nslices"]) * HB)
     assert all(r is not None for r in rows)
@@ -102,11 +106,13 @@ def test_stream_round_trip(wide):
     nrows, n_real = 3000, 2013
     rp, ci, v = random_csr(rng, nrows, ncols, 60)
     aux = rng.standard_normal(nrows)
-    stream, ways = m.amgdd_pack_stream(rp, ci, v, wide=wide, n_real=n_real, aux=aux)
+    rf = (rng.random(nrows) < 0.4).astype(np.uint8)
+    stream, ways = m.amgdd_pack_stream(rp, ci, v, wide=wide, n_real=n_real, aux=aux, row_flags=rf)
     assert len(ways) == m.NUM_WAYS and len(stream) % 128 == 0
     rows, aux2, load = decode(stream, ways, wide, nrows, n_real)
     check_rows(rows, rp, ci, v)
     assert np.array_equal(aux2, aux)
+    assert np.array_equal(decode.flags, rf), "bit 31 of the header's info word carries the row's flag"
     # the ways are balanced: a slice goes to the lightest way, so no way exceeds the mean by more than one slice
     gb = m.GROUP_BYTES_WIDE if wide else m.GROUP_BYTES_NARROW
     assert max(load) <= np.mean(load) + 15 * gb + HB
