@@ -150,6 +150,13 @@ def test_config4_small_parity():
     run_parity(wl.make_config(4, 48), 10)
 
 
+def test_config6_rotated_anisotropy_parity():
+    # the paper's Problem 2 proper (NEXT 3 of SURVEY.md section 8(f)): 9-point bilinear-FE stencil with
+    # positive off-diagonals (reading A11); padding 1 and 2
+    run_parity(wl.make_config(6, 256), 8)
+    run_parity(wl.make_config(6, 192, eta=2, parts_per_dim=4), 4)
+
+
 def test_config5_small_parity():
     run_parity(wl.make_config(5, 256), 15, yardstick=True)
 

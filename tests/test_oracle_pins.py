@@ -111,7 +111,7 @@ def _rs_first_pass_bruteforce(S):
     return cf
 
 
-@pytest.mark.parametrize("cfg,scale,theta", [(1, 9, 0.25), (4, 5, 0.5), (5, 12, 0.25), (3, 4, 0.5)])
+@pytest.mark.parametrize("cfg,scale,theta", [(1, 9, 0.25), (4, 5, 0.5), (5, 12, 0.25), (3, 4, 0.5), (6, 10, 0.25)])
 def test_strength_and_cf_split_bruteforce(cfg, scale, theta):
     p = wl.make_config(cfg, scale)
     o = Oracle(p.n, p.rowptr, p.colind, p.vals, theta, 3, 4)
@@ -154,7 +154,38 @@ def test_direct_interpolation_rows():
         assert (ratio < 0).all()          # a_ij < 0, w_ij > 0
 
 
-@pytest.mark.parametrize("cfg,scale", [(2, 8), (3, 6), (4, 6), (5, 16)])
+def test_direct_interpolation_with_positive_offdiagonals():
+    # S3 / reading A11 on the paper's Problem 2 (rotated anisotropy, bilinear FE: some off-diagonals are
+    # positive): w_ij = -alpha_i a_ij / d_i with d_i = a_ii + sum of the positive off-diagonals,
+    # alpha_i = (sum of the negative off-diagonals) / (sum over the strong C neighbours), written out with numpy
+    p = wl.make_config(6, 12)
+    theta = 0.25
+    o = Oracle(p.n, p.rowptr, p.colind, p.vals, theta, 25, 8)
+    A = o.scipy_matrix(0, "A").toarray()
+    assert ((A - np.diag(np.diag(A))) > 0).sum() > 100
+    P = o.scipy_matrix(0, "P").toarray()
+    cf = o.cf(0)
+    cidx = np.cumsum(cf == 1) - 1
+    checked = 0
+    for i in np.nonzero(cf == -1)[0]:
+        off = A[i].copy(); off[i] = 0.0
+        nz = off != 0
+        m = (-off[nz]).max() if nz.any() else 0.0
+        strong = (off != 0) & (-off > 0) & (-off >= theta * m * (1 - 1e-10))
+        Ci = np.nonzero(strong & (cf == 1))[0]
+        if len(Ci) == 0:
+            assert not P[i].any()
+            continue
+        d = A[i, i] + off[off > 0].sum()
+        alpha = off[off < 0].sum() / off[Ci].sum()
+        w = np.zeros(P.shape[1])
+        w[cidx[Ci]] = -alpha * off[Ci] / d
+        assert np.allclose(P[i], w, rtol=1e-13, atol=1e-15), i
+        checked += 1
+    assert checked > 30
+
+
+@pytest.mark.parametrize("cfg,scale", [(2, 8), (3, 6), (4, 6), (5, 16), (6, 12)])
 def test_galerkin_matches_library_triple_product(cfg, scale):
     # S4 / P:49: A_{l+1} = R_l A_l P_l with R_l = P_l^T; every structural entry kept.
     p = wl.make_config(cfg, scale)
@@ -270,7 +301,7 @@ def _masks(o, q):
 
 @pytest.mark.parametrize("cfg,scale,parts,eta,nfac,nu", [
     (1, None, 2, 1, 1, 1), (1, None, 2, 1, 2, 1), (1, None, 2, 1, 3, 2), (1, 21, 3, 2, 2, 1),
-    (2, 12, 2, 2, 2, 1), (2, 12, 2, 1, 3, 2), (4, 12, 2, 2, 2, 1), (5, 32, 2, 3, 2, 1), (3, 8, 2, 1, 2, 1)])
+    (2, 12, 2, 2, 2, 1), (2, 12, 2, 1, 3, 2), (4, 12, 2, 2, 2, 1), (5, 32, 2, 3, 2, 1), (3, 8, 2, 1, 2, 1), (6, 32, 2, 1, 2, 1)])
 def test_algfac_equals_masked_global_vcycle(cfg, scale, parts, eta, nfac, nu):
     # P:87 guiding principle; eqs. 13-30; Alg. 4
     p = wl.make_config(cfg, scale, parts_per_dim=parts)

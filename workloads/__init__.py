@@ -197,6 +197,29 @@ def aniso2d_jumps(n, seed, eps=1e-3, blocks=16, hi=1e4):
     return _fv_diffusion((n, n), kcell, (1.0, eps))
 
 
+def rotated_aniso2d_9pt(n, theta=3.0 * np.pi / 16.0, eps=1e-3):
+    """Problem 2 of the paper (eq. 33): -div(K grad u), K = Q^T D Q with the rotation angle theta and
+    D = diag(1, eps), discretised with bilinear finite elements on a uniform n x n interior grid (Dirichlet
+    boundary eliminated, no h scaling).  With K = [[a, b], [b, d]] the 9-point row is: centre 4(a+d)/3, (+-1, 0)
+    (d-2a)/3, (0, +-1) (a-2d)/3, (+1,+1) and (-1,-1) -(a+d)/6 - b/2, (+1,-1) and (-1,+1) -(a+d)/6 + b/2: some
+    off-diagonals are positive (reading A11 of DESIGN.md)."""
+    c, s_ = np.cos(theta), np.sin(theta)
+    a, b, d = c * c + eps * s_ * s_, (1.0 - eps) * c * s_, s_ * s_ + eps * c * c
+    offs, v = [], []
+    for dy in (-1, 0, 1):
+        for dx in (-1, 0, 1):
+            offs.append((dx, dy))
+            if dx == 0 and dy == 0:
+                v.append(4.0 * (a + d) / 3.0)
+            elif dy == 0:
+                v.append((d - 2.0 * a) / 3.0)
+            elif dx == 0:
+                v.append((a - 2.0 * d) / 3.0)
+            else:
+                v.append(-(a + d) / 6.0 - (b / 2.0 if dx * dy > 0 else -b / 2.0))
+    return _assemble((n, n), offs, lambda k, ok: np.full(ok.shape, v[k]))
+
+
 def block_owner(shape, parts):
     """owner[i] for regular block partitions: per dimension floor(c*parts/n)."""
     c = _coords(shape)
@@ -237,7 +260,7 @@ class Problem:
 
 
 def make_config(cfg: int, scale: int | None = None, eta: int | None = None, parts_per_dim: int | None = None) -> Problem:
-    """BASELINE.json configs 1..5.  `scale` overrides the grid edge (and keeps the subdomain block
+    """BASELINE.json configs 1..5 (and 6: the paper's Problem 2, an extra workload).  `scale` overrides the grid edge (and keeps the subdomain block
     edge of the full config where it divides) to get smaller instances of the same recipe."""
     if cfg == 1:
         n = scale or 33
@@ -279,6 +302,16 @@ def make_config(cfg: int, scale: int | None = None, eta: int | None = None, part
         own = block_owner((n, n), parts)
         return Problem(f"cfg5-aniso2d-{n}", n * n, rp, ci, v, own, pp * pp, rhs(4 + 1000, n * n),
                        eta if eta is not None else 3, 0.25, 64, 15, meta={"shape": (n, n), "parts": parts})
+    if cfg == 6:
+        # not a BASELINE.json config: the paper's Problem 2 proper (rotated anisotropic diffusion),
+        # SURVEY.md section 8(f) NEXT 3; 1024^2, 16 x 16 subdomains of 64^2, padding 1 as in the paper's GPU runs
+        n = scale or 1024
+        rp, ci, v = rotated_aniso2d_9pt(n)
+        pp = parts_per_dim or max(1, n // 64)
+        parts = (pp, pp)
+        own = block_owner((n, n), parts)
+        return Problem(f"cfg6-rotaniso2d-{n}", n * n, rp, ci, v, own, pp * pp, rhs(5 + 1000, n * n),
+                       eta if eta is not None else 1, 0.25, 64, 10, meta={"shape": (n, n), "parts": parts})
     raise ValueError(f"unknown config {cfg}")
 
 
