@@ -68,6 +68,7 @@ struct amgdd_handle_s {
     int window = DEFAULT_WINDOW, x_cap = 0, smem_cta = 0;
     FacLaunch fac_cfg = {1, 32 * NUM_WAYS, 0};
     FacOp* d_ops = nullptr;                     // the program of one subdomain (fac_build_program)
+    int prof_smem_off = 0;
     int prog_nfac = -1, prog_nu = -1, prog_smoother = -1, prog_nops = 0;
     int* d_counter = nullptr;
     long long* d_prof_ops = nullptr;
@@ -289,12 +290,12 @@ int env_int(const char* name, int dflt) {
     return std::atoi(v);
 }
 
-StreamDesc make_desc(const char* base, const StreamLayout& lay) {
+StreamDesc make_desc(const char* base, const StreamLayout& lay, bool shared = false) {
     StreamDesc d;
     std::memset(&d, 0, sizeof(d));
     d.base = base;
     for (int w = 0; w < NUM_WAYS; ++w) d.way[w] = lay.way[w];
-    d.flags = (lay.wide ? STREAM_WIDE : 0u) | (lay.has_aux ? STREAM_AUX : 0u);
+    d.flags = (lay.wide ? STREAM_WIDE : 0u) | (lay.has_aux ? STREAM_AUX : 0u) | (shared ? STREAM_SHARED : 0u);
     return d;
 }
 
@@ -363,8 +364,8 @@ int finish_tables(amgdd_handle_s* h) {
             if (b.shared) {
                 const GlobalLevelDev& g = h->glev[l];
                 d.gid = g.ident; d.dinv = g.dinv;
-                d.A = make_desc(g.sA, g.layA);
-                if (l < L) { d.P = make_desc(g.sP, g.layP); d.R = make_desc(g.sR, g.layR); }
+                d.A = make_desc(g.sA, g.layA, true);
+                if (l < L) { d.P = make_desc(g.sP, g.layP, true); d.R = make_desc(g.sR, g.layR, true); }
             } else {
                 char* base = sm.dev_base;
                 d.gid = (const int*)(base + b.off_gid); d.dinv = (const double*)(base + b.off_dinv);
@@ -614,12 +615,14 @@ int amgdd_solve(amgdd_handle_t h, const double* b, double* x, int32_t num_cycles
         // ~48 KB of L1 the streaming rate of this kernel drops by 15% (profiles/).  Levels that do
         // not fit are gathered through L1 from the workspace slot instead.
         const int budget = std::min(h->smem_cta, env_int("AMGDD_SMEM_BUDGET", 180 * 1024));
-        long long cap = ((long long)budget - fac_smem_bytes(0, L, nops)) / 16;
+        const int prof_bytes = h->d_prof ? PROF_SMEM_BYTES : 0;
+        long long cap = ((long long)budget - fac_smem_bytes(0, L, nops) - prof_bytes) / 16;
         cap = std::max(0LL, std::min(cap, h->x_need)) & ~15LL;
         if (env_int("AMGDD_FORCE_GLOBAL_X", 0) > 0) cap = 0;
         h->x_cap = (int)cap;
         h->stats.x_cap = h->x_cap;
-        h->fac_cfg.smem_bytes = std::min(h->smem_cta, fac_smem_bytes(h->x_cap, L, nops) + env_int("AMGDD_EXTRA_SMEM", 0));
+        h->prof_smem_off = fac_smem_bytes(h->x_cap, L, nops);
+        h->fac_cfg.smem_bytes = std::min(h->smem_cta, h->prof_smem_off + prof_bytes + env_int("AMGDD_EXTRA_SMEM", 0));
         h->stats.fac_smem_bytes = h->fac_cfg.smem_bytes;
     }
     FacParams prm;
@@ -634,6 +637,7 @@ int amgdd_solve(amgdd_handle_t h, const double* b, double* x, int32_t num_cycles
     prm.cf0 = h->d_cf0;
     prm.x_cap = h->x_cap;
     prm.prof = h->d_prof;
+    prm.prof_smem_off = h->prof_smem_off;
     prm.prof_ops = h->d_prof_ops;
     long long launches[3] = {0, 0, 0};
     mark();

@@ -64,6 +64,11 @@ __device__ __forceinline__ uint64_t policy_evict_first() {
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
     return pol;
 }
+__device__ __forceinline__ uint64_t policy_evict_last() {
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
 __device__ __forceinline__ uint4 ldg_stream128(const void* p, uint64_t pol) {
     uint4 v;
     asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v4.u32 {%0,%1,%2,%3}, [%4], %5;"
@@ -154,7 +159,8 @@ struct Worker {
     }
     double* ws;                    // this CTA's workspace slot
     long long* prof;
-    uint64_t pol;
+    long long* prof_s;             // shared-memory copy of the counters (PROF)
+    uint64_t pol_stream, pol_keep; // L2 policies: private streams are read once per mat-vec (evict first), shared levels by every CTA (keep)
     int tid, lane, wid, L;
     // ring state carried from mat-vec to mat-vec
     Grp ra[D], rb[D];              // two blocks of D groups; `phase` tells which one holds the coming block
@@ -165,7 +171,12 @@ struct Worker {
     int opj;                       // index of the current step in the program (profiling)
 
     __device__ __forceinline__ long long tick() const { return PROF ? clock64() : 0; }
-    __device__ __forceinline__ void tock(int idx, long long t0) const { if (PROF && tid == 0) prof[idx] += clock64() - t0; }
+    // profiling counters live in shared memory while the kernel runs (a global read-modify-write per event would
+    // cost thread 0 a round trip to L2 each time and distort what is measured); flushed once at the end
+    __device__ __forceinline__ void tock(int idx, long long t0) const { if (PROF && tid == 0) prof_s[idx] += clock64() - t0; }
+    __device__ __forceinline__ void tock_op(int which, long long t0) const {
+        if (PROF && tid == 0 && opj < PROF_OPS_SMEM) prof_s[FAC_PROF_SLOTS + which * PROF_OPS_SMEM + opj] += clock64() - t0;
+    }
     __device__ __forceinline__ void sync() {
         const long long t0 = tick();
         __syncthreads();
@@ -282,6 +293,8 @@ struct Worker {
         // ---- this warp's way of the stream, and of the next mat-vec's stream ----
         const WayEnt we = wt[stream_of(op) * NUM_WAYS + wid];
         const char* const sb = sbase[stream_of(op)];
+        const uint64_t pol = (sflags[stream_of(op)] & STREAM_SHARED) ? pol_keep : pol_stream;
+        uint64_t pol_nxt = pol_stream;
         const char* const we_hdr = sb + 128ull * we.hdr_off128;
         const bool ronly = real_rows_only(op);
         const int n = (int)(ronly ? we.n_real : we.n_all);
@@ -295,6 +308,7 @@ struct Worker {
             const FacOp nop = ops[op.next_mat];
             const WayEnt w2 = wt[stream_of(nop) * NUM_WAYS + wid];
             n_next = (int)(real_rows_only(nop) ? w2.n_real : w2.n_all);
+            if (sflags[stream_of(nop)] & STREAM_SHARED) pol_nxt = pol_keep;
             if (n_next > 0) { const char* b2 = sbase[stream_of(nop)]; nxt = b2 + 128ull * w2.grp_off128; nxt_hdr = b2 + 128ull * w2.hdr_off128; }
         }
         const int next_last = n_next > 0 ? n_next - 1 : 0;
@@ -334,10 +348,10 @@ struct Worker {
             if (n_next > 0) {
                 if (phase == 0) {
 #pragma unroll
-                    for (int d = 0; d < D; ++d) ra[d] = load_grp<WIDE>(nxt + (long long)(d < next_last ? d : next_last) * GB, lane, pol);
+                    for (int d = 0; d < D; ++d) ra[d] = load_grp<WIDE>(nxt + (long long)(d < next_last ? d : next_last) * GB, lane, pol_nxt);
                 } else {
 #pragma unroll
-                    for (int d = 0; d < D; ++d) rb[d] = load_grp<WIDE>(nxt + (long long)(d < next_last ? d : next_last) * GB, lane, pol);
+                    for (int d = 0; d < D; ++d) rb[d] = load_grp<WIDE>(nxt + (long long)(d < next_last ? d : next_last) * GB, lane, pol_nxt);
                 }
                 cp_async_wait_all();
                 cp_async16(stage + 16 * lane, nxt_hdr + 16 * lane);
@@ -381,7 +395,7 @@ struct Worker {
             const long long tw0 = tick();
             cp_async_wait_all();
             tock(14, tw0);
-            if (PROF && tid == 0 && prm->prof_ops) prm->prof_ops[(size_t)blockIdx.x * PROF_OPS_STRIDE + 3 * MAX_OPS + opj] += clock64() - tw0;
+            tock_op(3, tw0);
             if (row != NO_ROW) {
                 const double e0 = lds_f64(stC), e1 = lds_f64(stC + 256), e2 = lds_f64(stC + 512);   // unused ones are stale, never read
                 if (kind == OPK_RELAX) {           // one l1-Jacobi update (§4.1); aux = 1 / sum_j |a_ij| (S8)
@@ -445,14 +459,15 @@ struct Worker {
             const bool more = p0 + D < n;
             const long long tr0 = tick();
             const bool never = (X[0].a.y & 0x7FF00000u) == 0x7FF00000u;
-            if (PROF && never) prof[15] += 1;            // (keeps the read of X[0] before the second clock read)
+            if (PROF && never) prof_s[15] += 1;          // (keeps the read of X[0] before the second clock read)
             tock(15, tr0);
-            if (PROF && tid == 0 && prm->prof_ops) prm->prof_ops[(size_t)blockIdx.x * PROF_OPS_STRIDE + 2 * MAX_OPS + opj] += clock64() - tr0;
+            tock_op(2, tr0);
             const char* rbase = never ? dummy : (more ? cur : nxt);
             const int r0 = more ? p0 + D : 0, rlast = never ? 0 : (more ? n - 1 : next_last);
+            const uint64_t pol_b = more ? pol : pol_nxt;
 #if !AMGDD_SINGLE_BUFFER
 #pragma unroll
-            for (int d = 0; d < D; ++d) Y[d] = load_grp<WIDE>(rbase + (long long)(r0 + d < rlast ? r0 + d : rlast) * GB, lane, pol);
+            for (int d = 0; d < D; ++d) Y[d] = load_grp<WIDE>(rbase + (long long)(r0 + d < rlast ? r0 + d : rlast) * GB, lane, pol_b);
 #endif
             const int nv = n - p0 < D ? n - p0 : D;     // groups of this block (the last block of a mat-vec may be short)
             if (left > nv && nv == D) {                 // no slice ends inside this block: straight-line code
@@ -478,7 +493,7 @@ struct Worker {
             }
 #if AMGDD_SINGLE_BUFFER
 #pragma unroll
-            for (int d = 0; d < D; ++d) X[d] = load_grp<WIDE>(rbase + (long long)(r0 + d < rlast ? r0 + d : rlast) * GB, lane, pol);
+            for (int d = 0; d < D; ++d) X[d] = load_grp<WIDE>(rbase + (long long)(r0 + d < rlast ? r0 + d : rlast) * GB, lane, pol_b);
 #endif
         };
         int ph = phase;
@@ -521,7 +536,9 @@ __global__ void __launch_bounds__(NTHREADS, CTAS_PER_SM) fac_kernel(const FacPar
     W.xg1 = W.xg0 + (prm.slot_stride - prm.xg_off) / 2;
     W.x_cap = prm.x_cap;
     W.prof = PROF ? prm.prof + (size_t)blockIdx.x * FAC_PROF_SLOTS : nullptr;
-    W.pol = policy_evict_first();
+    W.prof_s = reinterpret_cast<long long*>(smem + prm.prof_smem_off);
+    if (PROF) { for (int i = threadIdx.x; i < FAC_PROF_SLOTS + 4 * PROF_OPS_SMEM; i += NTHREADS) W.prof_s[i] = 0; }
+    W.pol_stream = policy_evict_first(); W.pol_keep = policy_evict_last();
     W.ring_valid = false; W.hdr_ready = false;
     W.stage = (uint32_t)__cvta_generic_to_shared(stage) + (uint32_t)W.wid * STAGE_BYTES;
 #pragma unroll
@@ -576,12 +593,19 @@ __global__ void __launch_bounds__(NTHREADS, CTAS_PER_SM) fac_kernel(const FacPar
             }
             if (!is_matvec(op.kind)) W.tock(PROF_OP0 + op.kind, tp0);
             long long tq0 = 0;
-            if (PROF && threadIdx.x == 0 && prm.prof_ops) { tq0 = clock64(); prm.prof_ops[(size_t)blockIdx.x * PROF_OPS_STRIDE + j] += tq0 - tp0; }
+            if (PROF) { W.tock_op(0, tp0); tq0 = clock64(); }
             W.sync();                                                    // the step is complete
-            if (PROF && threadIdx.x == 0 && prm.prof_ops) prm.prof_ops[(size_t)blockIdx.x * PROF_OPS_STRIDE + MAX_OPS + j] += clock64() - tq0;
+            if (PROF) W.tock_op(1, tq0);
         }
     }
     W.tock(PROF_TOTAL, tk0);
+    if (PROF && threadIdx.x == 0) {                                          // flush the counters of this CTA
+        for (int i = 0; i < FAC_PROF_SLOTS; ++i) W.prof[i] += W.prof_s[i];
+        if (prm.prof_ops)
+            for (int q = 0; q < 4; ++q)
+                for (int j = 0; j < PROF_OPS_SMEM && j < prm.nops; ++j)
+                    prm.prof_ops[(size_t)blockIdx.x * PROF_OPS_STRIDE + q * MAX_OPS + j] += W.prof_s[FAC_PROF_SLOTS + q * PROF_OPS_SMEM + j];
+    }
 }
 
 }  // namespace

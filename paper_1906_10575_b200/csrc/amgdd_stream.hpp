@@ -83,10 +83,11 @@ static_assert(sizeof(WayDesc) == 32, "WayDesc layout");
 
 constexpr uint32_t STREAM_WIDE = 1u;         // StreamDesc::flags
 constexpr uint32_t STREAM_AUX = 2u;
+constexpr uint32_t STREAM_SHARED = 4u;       // the single copy of a fully covered level: every CTA reads it, keep it in L2
 
 struct StreamDesc {
     const char* base;      // DEVICE, 128-byte aligned
-    uint32_t flags;        // STREAM_WIDE | STREAM_AUX
+    uint32_t flags;        // STREAM_WIDE | STREAM_AUX | STREAM_SHARED
     uint32_t pad_;
     WayDesc way[NUM_WAYS];
 };
@@ -162,10 +163,13 @@ struct FacParams {
     const int8_t* cf0;         // C/F flags of level 0 (global numbering), for the matrix-free first sweep of the CF smoother
     int x_cap;                 // doubles in each of the two shared-memory vector buffers (0: vectors in global memory)
     long long* prof;           // optional: gridDim.x * FAC_PROF_SLOTS cycle counters (debugging), or nullptr
+    int prof_smem_off;         // byte offset of the profiling counters in dynamic shared memory (PROF_SMEM_BYTES), with prof != nullptr
     long long* prof_ops;       // optional: gridDim.x * PROF_OPS_STRIDE: per step of the program: cycles | barrier wait after it | waits for ring blocks | waits for staged slice operands
 };
 constexpr int FAC_PROF_SLOTS = 16;
 constexpr int PROF_OPS_STRIDE = 4 * MAX_OPS;
+constexpr int PROF_OPS_SMEM = 256;           // steps of the program that the per-step counters cover (they live in shared memory)
+constexpr int PROF_SMEM_BYTES = (FAC_PROF_SLOTS + 4 * PROF_OPS_SMEM) * 8;
 
 struct FacLaunch {
     int grid;
