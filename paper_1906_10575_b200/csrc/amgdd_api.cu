@@ -622,7 +622,7 @@ int amgdd_solve(amgdd_handle_t h, const double* b, double* x, int32_t num_cycles
         h->x_cap = (int)cap;
         h->stats.x_cap = h->x_cap;
         h->prof_smem_off = fac_smem_bytes(h->x_cap, L, nops);
-        h->fac_cfg.smem_bytes = std::min(h->smem_cta, h->prof_smem_off + prof_bytes + env_int("AMGDD_EXTRA_SMEM", 0));
+        h->fac_cfg.smem_bytes = std::min(h->smem_cta, h->prof_smem_off + prof_bytes);
         h->stats.fac_smem_bytes = h->fac_cfg.smem_bytes;
     }
     FacParams prm;

@@ -618,7 +618,7 @@ int fac_build_program(int L, int nfac, int nu, int smoother, FacOp* ops) {
         if (ops && n < MAX_OPS) {
             FacOp o;
             o.kind = (uint8_t)kind; o.level = (uint8_t)level; o.gbuf = (uint8_t)gbuf; o.flags = (uint8_t)flags;
-            o.next_mat = -1; o.next_mat2 = -1;
+            o.next_mat = -1; o.pad_ = 0;
             ops[n] = o;
         }
         ++n;
@@ -660,10 +660,10 @@ int fac_build_program(int L, int nfac, int nu, int smoother, FacOp* ops) {
     }
     emit(OPK_END, 0, 0, 0);                                                  // Alg. 2
     if (ops && n <= MAX_OPS) {
-        int nm = -1, nm2 = -1;
+        int nm = -1;
         for (int j = n - 1; j >= 0; --j) {
-            ops[j].next_mat = (int16_t)nm; ops[j].next_mat2 = (int16_t)nm2;
-            if (ops[j].kind >= OPK_RELAX && ops[j].kind <= OPK_INTERP) { nm2 = nm; nm = j; }
+            ops[j].next_mat = (int16_t)nm;
+            if (ops[j].kind >= OPK_RELAX && ops[j].kind <= OPK_INTERP) nm = j;
         }
     }
     return n;

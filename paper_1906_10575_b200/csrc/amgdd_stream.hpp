@@ -136,8 +136,8 @@ struct FacOp {
     uint8_t level;         // l of the step as written in Alg. 4 (RESTRICT: R_l; RECALC: A_{l+1} has level = l+1; INTERP: P_l)
     uint8_t gbuf;          // shared-memory vector buffer (0/1) the mat-vec gathers from; it writes the other
     uint8_t flags;         // OPF_*
-    int16_t next_mat;      // index of the next mat-vec op of the program (-1: none): its groups are prefetched
-    int16_t next_mat2;     // the one after that (-1: none): its way descriptor is prefetched
+    int16_t next_mat;      // index of the next mat-vec op of the program (-1: none): its first groups and header are prefetched
+    int16_t pad_;
 };
 static_assert(sizeof(FacOp) == 8, "FacOp layout");
 constexpr int MAX_OPS = 1024;
