@@ -214,6 +214,24 @@ def test_amg_vcycle_matches_the_oracle(cfg, scale, nu1, nu2, smoother):
     m.amgdd_destroy(h)
 
 
+@pytest.mark.parametrize("name,cfg,scale,smoother", [("config1_resnorms.txt", 1, None, 0), ("config4_scale24_resnorms.txt", 4, 24, 0),
+                                                      ("config1_cfjacobi_resnorms.txt", 1, None, 1)])
+def test_against_stored_oracle_values(name, cfg, scale, smoother):
+    """The residual norms stored under tests/golden/ (written by tests/golden/make_golden.py from oracle/ only)."""
+    import os
+    torch = _torch()
+    ref = np.array([float(ln) for ln in open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", name))
+                    if not ln.startswith("#")])
+    p = wl.make_config(cfg, scale)
+    m, h = lib_setup(p)
+    m.amgdd_set_smoother(h, smoother)
+    b = torch.from_numpy(p.b).cuda()
+    x = torch.zeros(p.n, dtype=torch.float64, device="cuda")
+    res = m.amgdd_solve(h, b, x, p.num_cycles, p.num_fac_cycles, p.relax_sweeps)
+    assert np.abs(res - ref).max() <= 0 + (RTOL * ref).max() and (np.abs(res - ref) <= RTOL * ref).all(), (res, ref)
+    m.amgdd_destroy(h)
+
+
 def test_ragged_partition_and_odd_sizes():
     # 33 = 17 + 16: ragged blocks; 3 x 3 blocks of a 37 x 37 grid
     run_parity(wl.make_config(1, 37, parts_per_dim=3), 3)

@@ -539,3 +539,25 @@ def test_overhead_definition():
     # one subdomain covering everything has overhead exactly 1
     p1 = wl.make_config(1, parts_per_dim=1)
     assert make_oracle(p1, eta=100).overhead() == 1.0
+
+
+# ------------------------------------------------------------------------------------------
+# stored values (tests/golden/, written by tests/golden/make_golden.py from oracle/ only)
+# ------------------------------------------------------------------------------------------
+def _golden(name):
+    import os
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", name)
+    return np.array([float(ln) for ln in open(path) if not ln.startswith("#")])
+
+
+@pytest.mark.parametrize("name,cfg,scale,smoother", [("config1_resnorms.txt", 1, None, 0), ("config4_scale24_resnorms.txt", 4, 24, 0),
+                                                      ("config1_cfjacobi_resnorms.txt", 1, None, 1)])
+def test_oracle_reproduces_stored_residual_norms(name, cfg, scale, smoother):
+    p = wl.make_config(cfg, scale)
+    o = make_oracle(p)
+    o.set_smoother(smoother)
+    res = o.solve(p.b, np.zeros(p.n), p.num_cycles, p.num_fac_cycles, p.relax_sweeps)
+    ref = _golden(name)
+    assert len(ref) == p.num_cycles + 1
+    assert np.allclose(res, ref, rtol=1e-12, atol=0), (res, ref)        # thread count / summation order of the oracle's host may differ in the last digits
+    assert res[0] == pytest.approx(np.linalg.norm(p.b), rel=1e-14)      # k = 0: x = 0 (reading A16, A17)
