@@ -39,7 +39,14 @@ constexpr int D = RING_DEPTH;
 #ifndef AMGDD_SINGLE_BUFFER
 #define AMGDD_SINGLE_BUFFER 0
 #endif
+#ifndef AMGDD_STAGE2
+#define AMGDD_STAGE2 0
+#endif
+#if AMGDD_STAGE2
+constexpr int STAGE_BYTES = 512 + 4 * 256 + 2 * 1024;   // per warp: slice 0's header, four {row, info} slots, two operand slots (e0 | e1 | e2 | aux)
+#else
 constexpr int STAGE_BYTES = 512 + 3 * 256;     // per warp: one slice header + three operand vectors of 32 doubles
+#endif
 
 // slots of the optional per-CTA cycle counters (FAC_PROF_SLOTS each; amgdd_debug_fac_cycles)
 enum ProfSlot { PROF_SYNC = 0, PROF_SETUP = 1, PROF_PRE = 2, PROF_PRIME = 3, PROF_TOTAL = 4, PROF_OP0 = 5 };   // PROF_OP0 + OpKind
@@ -97,6 +104,13 @@ __device__ __forceinline__ void cp_async8(uint32_t dst, const void* src) {
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_pending(int) { asm volatile("cp.async.wait_group 1;" ::: "memory"); }
+__device__ __forceinline__ uint32_t lds_u32(uint32_t a) {
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a));
+    return v;
+}
 __device__ __forceinline__ uint4 lds128(uint32_t a) {
     uint4 v;
     asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a));
@@ -359,6 +373,36 @@ struct Worker {
             tock(PROF_OP0 + kind, tp0);
             return;
         }
+#if AMGDD_STAGE2
+        // Two slices deep: a ring of four {row, info} header slots and of two operand slots (e0 | e1 | e2 | aux),
+        // ring positions by masks.  Slot 0..511 of the area holds the full header of slice 0 (of this mat-vec,
+        // then of the next one).
+        const char* const hdr = we_hdr + 16 * lane;
+        const uint32_t stN = stage + 16 * lane, stH = stage + 512 + 8 * lane, stC = stage + 1536 + 8 * lane;
+        const bool use_aux = kind == OPK_RELAX || kind == OPK_RECALC || (kind == OPK_RESTRICT && first && !coarsest);
+        auto issue_hdr = [&](int t) { if (t < nsl) cp_async8(stH + (uint32_t)(t & 3) * 256u, hdr + (long long)t * HEADER_BYTES); };
+        auto issue_ctx = [&](int t, uint32_t r) {
+            const uint32_t a = stC + (uint32_t)(t & 1) * 1024u;
+            if (r != NO_ROW) {
+                if (cA) cp_async8(a, cA + r);
+                if (cB) cp_async8(a + 256, cB + r);
+                if (cC) cp_async8(a + 512, cC + r);
+            }
+            if (use_aux) cp_async8(a + 768, hdr + (long long)t * HEADER_BYTES + 8);
+        };
+        if (!hdr_ready) { cp_async_wait_all(); cp_async16(stN, hdr); }       // (never two copies in flight to one slot)
+        cp_async_wait_all();
+        const uint4 h = lds128(stN);
+        uint32_t row = h.x;
+        int left = (int)(h.y & HDR_GROUPS_MASK);
+        bool is_c = (h.y >> 31) != 0;                                       // the row is a C-point of its level
+        double aux = mkdouble(h.z, h.w);
+        cp_async16(stN, nxt_hdr + 16 * lane);                               // static data: slice 0 of the next mat-vec
+        hdr_ready = n_next > 0;
+        issue_hdr(1); issue_hdr(2); issue_hdr(3);
+        issue_ctx(0, row);
+        cp_async_commit();
+#else
         const char* const hdr = we_hdr + 16 * lane;
         const uint32_t stH = stage + 16 * lane, stC = stage + 512 + 8 * lane;
         const char* const hdr_after = nxt_hdr + 16 * lane;
@@ -379,6 +423,7 @@ struct Worker {
         fetch_ctx(row);
         cp_async16(stH, nsl > 1 ? hdr + HEADER_BYTES : hdr_after);
         hdr_ready = n_next > 0;
+#endif
         int sidx = 0;
         double acc = 0.0;
         auto consume = [&](const Grp& g) {
@@ -393,11 +438,19 @@ struct Worker {
         };
         auto slice_end = [&]() {
             const long long tw0 = tick();
+#if AMGDD_STAGE2
+            if (sidx < 2) cp_async_wait_all();      // the rings are still filling
+            else cp_async_wait_pending(1);          // everything but the youngest group: this slice's operands, headers up to sidx + 2
+            const uint32_t stE = stC + (uint32_t)(sidx & 1) * 1024u;
+            if (use_aux && sidx > 0) aux = lds_f64(stE + 768);
+#else
             cp_async_wait_all();
+            const uint32_t stE = stC;
+#endif
             tock(14, tw0);
             tock_op(3, tw0);
             if (row != NO_ROW) {
-                const double e0 = lds_f64(stC), e1 = lds_f64(stC + 256), e2 = lds_f64(stC + 512);   // unused ones are stale, never read
+                const double e0 = lds_f64(stE), e1 = lds_f64(stE + 256), e2 = lds_f64(stE + 512);   // unused ones are stale, never read
                 if (kind == OPK_RELAX) {           // one l1-Jacobi update (§4.1); aux = 1 / sum_j |a_ij| (S8)
                     const double uo = xg.ld(row);
                     if ((half_c && !is_c) || (half_f && is_c)) {   // CF smoother: not this half-sweep's class
@@ -439,6 +492,19 @@ struct Worker {
             }
             ++sidx;
             acc = 0.0;
+#if AMGDD_STAGE2
+            if (sidx < nsl) {
+                const uint32_t hs = stH + (uint32_t)(sidx & 3) * 256u;
+                row = lds_u32(hs);
+                const uint32_t info = lds_u32(hs + 4);
+                left = (int)(info & HDR_GROUPS_MASK); is_c = (info >> 31) != 0;
+                issue_hdr(sidx + 3);                                      // into the slot of the slice just finished
+                if (sidx == 1) issue_ctx(1, row);
+                if (sidx + 1 < nsl) issue_ctx(sidx + 1, lds_u32(stH + (uint32_t)((sidx + 1) & 3) * 256u));
+                cp_async_commit();
+            }
+        };
+#else
             if (sidx < nsl) {
                 h = lds128(stH);
                 row = h.x; left = (int)(h.y & HDR_GROUPS_MASK); is_c = (h.y >> 31) != 0; aux = mkdouble(h.z, h.w);
@@ -446,6 +512,7 @@ struct Worker {
                 cp_async16(stH, sidx + 1 < nsl ? hdr + (long long)(sidx + 1) * HEADER_BYTES : hdr_after);
             }
         };
+#endif
         tock(PROF_PRIME, tp0);
         // Blocks of D groups, double buffered in registers: WAIT for block j (buffer X), then issue
         // the burst of block j+1 into the other buffer (the next D groups of this mat-vec or, after
