@@ -90,6 +90,14 @@ typedef struct amgdd_stats {
     int32_t x_cap;                   /* doubles in each of the two shared-memory vector buffers (0: they live in global memory) */
     int32_t fac_grid, fac_block, fac_smem_bytes;
     int64_t max_n_bar;               /* largest |D-bar_l^p| over all subdomains and levels */
+    /* composite-grid assembly (NEXT 3): 1 when the local matrices were cut out, renumbered and packed
+       on the device (the default), 0 for the host path (AMGDD_ASSEMBLE=host); the three parts of
+       setup_seconds_composite on the device path: host index sets, device kernels + small copies, hierarchy upload */
+    int32_t assembled_on_device;
+    int32_t reserved_;
+    double setup_seconds_index_sets;
+    double setup_seconds_assembly;
+    double setup_seconds_upload;
 } amgdd_stats_t;
 
 /* ---------------------------------------------------------------------------------------------
@@ -234,6 +242,15 @@ int amgdd_debug_fac_cycles(amgdd_handle_t h, int64_t out[16], int32_t reset);
  * out[2n + j] = its waits for blocks of the register ring, out[3n + j] = its waits for staged slice operands;
  * kinds_levels[j] (HOST, n entries or NULL) = 256 * kind + level of step j.  Clears the counters. */
 int amgdd_debug_fac_op_cycles(amgdd_handle_t h, int64_t* out, int32_t n, int32_t* kinds_levels);
+
+/* Test support for the composite-grid assembly: copies one array of the
+ * private block (subdomain p, level) out of the device blob into HOST memory `out`.
+ *   which  0 gid (int32[n_bar])   1 dinv (double[n_real])   2 / 3 / 4 the packed A_l / P_l / R_l stream
+ *          5 the owned-dof index list of the subdomain (int32[n_owned]; level ignored)
+ * *out_bytes receives the size of the array (0 for a level that uses the shared global copy); with out = NULL
+ * only the size is returned.  AMGDD_ERR_BAD_ARG on a bad index or if out_capacity is too small. */
+int amgdd_debug_read_block(amgdd_handle_t h, int32_t p, int32_t level, int32_t which, void* out, int64_t out_capacity,
+                           int64_t* out_bytes);
 
 #ifdef __cplusplus
 }

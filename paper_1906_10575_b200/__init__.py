@@ -21,6 +21,7 @@ EXPORTS = [
     "amgdd_strerror", "amgdd_last_error_detail", "amgdd_num_levels", "amgdd_level_size", "amgdd_get_cf",
     "amgdd_get_level_matrix", "amgdd_composite_size", "amgdd_get_composite", "amgdd_get_stats",
     "amgdd_last_solve_profile", "amgdd_pack_stream", "amgdd_debug_fac_cycles", "amgdd_debug_fac_op_cycles",
+    "amgdd_debug_read_block",
 ]
 
 
@@ -33,6 +34,8 @@ class AmgddStats(ctypes.Structure):
         ("model_bytes_global", _f64), ("setup_seconds_hierarchy", _f64), ("setup_seconds_composite", _f64),
         ("block_bytes", _i32), ("num_ways", _i32), ("window", _i32), ("ring_stages", _i32), ("x_cap", _i32), ("fac_grid", _i32), ("fac_block", _i32),
         ("fac_smem_bytes", _i32), ("max_n_bar", _i64),
+        ("assembled_on_device", _i32), ("reserved_", _i32), ("setup_seconds_index_sets", _f64),
+        ("setup_seconds_assembly", _f64), ("setup_seconds_upload", _f64),
     ]
 
 
@@ -69,6 +72,7 @@ def _load():
     L.amgdd_last_solve_profile.argtypes = [_vp, _vp, _vp]
     L.amgdd_debug_fac_cycles.argtypes = [_vp, _vp, _i32]
     L.amgdd_debug_fac_op_cycles.argtypes = [_vp, _vp, _i32, _vp]
+    L.amgdd_debug_read_block.argtypes = [_vp, _i32, _i32, _i32, _vp, _i64, _vp]
     L.amgdd_pack_stream.argtypes = [_i32, _i32, _vp, _vp, _vp, _vp, _vp, _i32, _i32, _vp, _i64, _vp, _vp]
     return L
 
@@ -277,6 +281,20 @@ def amgdd_debug_fac_op_cycles(h: Handle, n=256):
     _check(lib.amgdd_debug_fac_op_cycles(h._h, out.ctypes.data, n, kl.ctypes.data))
     return [(OP_KIND_NAMES[k // 256], int(k % 256), int(out[j]), int(out[n + j]), int(out[2 * n + j]), int(out[3 * n + j]))
             for j, k in enumerate(kl) if k >= 0]
+
+
+BLOCK_ARRAYS = {"gid": 0, "dinv": 1, "A": 2, "P": 3, "R": 4, "owned": 5}
+
+
+def amgdd_debug_read_block(h: Handle, p: int, level: int, which: str) -> np.ndarray:
+    """One array of a private (subdomain, level) block as the device holds it (bytes; empty for a shared level)."""
+    nbytes = _i64(0)
+    w = BLOCK_ARRAYS[which]
+    _check(lib.amgdd_debug_read_block(h._h, p, level, w, None, 0, ctypes.byref(nbytes)))
+    out = np.zeros(nbytes.value, dtype=np.uint8)
+    if nbytes.value:
+        _check(lib.amgdd_debug_read_block(h._h, p, level, w, out.ctypes.data, nbytes.value, ctypes.byref(nbytes)))
+    return out
 
 
 def amgdd_last_solve_profile(h: Handle):

@@ -1,6 +1,7 @@
 // C ABI of the AMG-DD library (include/amgdd.h): setup orchestration (host hierarchy, threaded
 // composite-grid construction streamed to the device), the solve driver, introspection.
 #include "../../include/amgdd.h"
+#include "amgdd_assemble.cuh"
 #include "amgdd_host.hpp"
 #include "amgdd_kernels.cuh"
 #include "amgdd_stream.hpp"
@@ -12,6 +13,7 @@
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
+#include <memory>
 #include <mutex>
 #include <new>
 #include <numeric>
@@ -147,6 +149,37 @@ struct Arena {
     size_t chunk = (size_t)1 << 30;
 };
 
+int env_int(const char* name, int dflt) {
+    const char* v = std::getenv(name);
+    if (!v || !*v) return dflt;
+    return std::atoi(v);
+}
+
+// reserves `bytes` of the chunked device arena (thread-safe); chunks are owned by the handle
+int arena_take(amgdd_handle_s* h, Arena& arena, size_t bytes, char** out, std::string& why) {
+    std::lock_guard<std::mutex> g(arena.mu);
+    if (arena.left < bytes) {
+        const size_t want = std::max(arena.chunk, bytes);
+        void* ptr = nullptr;
+        cudaError_t e = cudaMalloc(&ptr, want);
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            why = "device arena: cudaMalloc of " + std::to_string(want) + " bytes failed with " + std::to_string(h->device_bytes) +
+                  " bytes already held";
+            return AMGDD_ERR_OUT_OF_MEMORY;
+        }
+        h->allocs.push_back(ptr);
+        h->device_bytes += (i64)want;
+        arena.cur = (char*)ptr;
+        arena.left = want;
+    }
+    *out = arena.cur;
+    const size_t adv = (bytes + 255) & ~(size_t)255;
+    arena.cur += std::min(adv, arena.left);
+    arena.left -= std::min(adv, arena.left);
+    return AMGDD_SUCCESS;
+}
+
 int build_composites(amgdd_handle_s* h, const std::vector<i32>& owner, int nthreads) {
     const int P = h->P, L = h->H.L;
     std::vector<std::vector<i32>> owned(P);
@@ -193,27 +226,10 @@ int build_composites(amgdd_handle_s* h, const std::vector<i32>& owner, int nthre
                     break;
                 }
                 const size_t bytes = (size_t)std::max<i64>(sm.plan.bytes, 16);
-                {   // reserve device space
-                    std::lock_guard<std::mutex> g(arena.mu);
-                    if (arena.left < bytes) {
-                        const size_t want = std::max(arena.chunk, bytes);
-                        void* ptr = nullptr;
-                        cudaError_t e = cudaMalloc(&ptr, want);
-                        if (e != cudaSuccess) {
-                            cudaGetLastError();
-                            fail(AMGDD_ERR_OUT_OF_MEMORY, "device arena: cudaMalloc of " + std::to_string(want) + " bytes failed with " +
-                                                              std::to_string(h->device_bytes) + " bytes already held");
-                            break;
-                        }
-                        h->allocs.push_back(ptr);
-                        h->device_bytes += (i64)want;
-                        arena.cur = (char*)ptr;
-                        arena.left = want;
-                    }
-                    sm.dev_base = arena.cur;
-                    const size_t adv = (bytes + 255) & ~(size_t)255;
-                    arena.cur += std::min(adv, arena.left);
-                    arena.left -= std::min(adv, arena.left);
+                {
+                    std::string why;
+                    const int arc = arena_take(h, arena, bytes, &sm.dev_base, why);
+                    if (arc) { fail(arc, why); break; }
                 }
                 cudaStreamSynchronize(st);                         // previous copy out of `stage` finished
                 if (stage_cap < bytes) {
@@ -238,6 +254,264 @@ int build_composites(amgdd_handle_s* h, const std::vector<i32>& owner, int nthre
         });
     for (auto& th : pool) th.join();
     if (status.load() != AMGDD_SUCCESS) { g_detail = fail_detail; return status.load(); }
+    return AMGDD_SUCCESS;
+}
+
+// ------------------------------------------------------------------------------------------
+// Device-side assembly (NEXT 3, paper P:335): the host grows the index sets only; the local
+// matrices are cut out of the global level matrices, renumbered and packed on the device
+// (amgdd_assemble.cu), batch by batch, straight into the arena.  Same blobs, byte for byte, as
+// build_composites writes.
+// ------------------------------------------------------------------------------------------
+struct TempDev {                                    // device / pinned scratch that lives only during setup
+    std::vector<void*> dev, pinned;
+    ~TempDev() { for (void* p : dev) cudaFree(p); for (void* p : pinned) cudaFreeHost(p); }
+    template <class T> cudaError_t alloc(T** p, size_t count) {
+        cudaError_t e = cudaMalloc((void**)p, std::max<size_t>(count, 1) * sizeof(T));
+        if (e == cudaSuccess) dev.push_back(*p);
+        return e;
+    }
+    template <class T> cudaError_t put(T** p, const T* src, size_t count) {
+        cudaError_t e = alloc(p, count);
+        if (e == cudaSuccess && count) e = cudaMemcpy(*p, src, count * sizeof(T), cudaMemcpyHostToDevice);
+        return e;
+    }
+};
+
+template <class T>
+struct GrowBuf {                                    // a device array that is re-allocated when a batch needs more
+    T* p = nullptr; size_t cap = 0;
+    cudaError_t need(size_t n) {
+        if (n <= cap) return cudaSuccess;
+        if (p) cudaFree(p);
+        p = nullptr; cap = 0;
+        const size_t want = n + n / 4 + 1024;
+        cudaError_t e = cudaMalloc((void**)&p, want * sizeof(T));
+        if (e == cudaSuccess) cap = want;
+        return e;
+    }
+    ~GrowBuf() { if (p) cudaFree(p); }
+};
+
+int build_composites_device(amgdd_handle_s* h, const std::vector<i32>& owner, int nthreads) {
+    const int P = h->P, L = h->H.L;
+    std::vector<std::vector<i32>> owned(P);
+    for (i64 i = 0; i < h->n; ++i) owned[owner[i]].push_back((i32)i);
+    h->subs.assign(P, SubMeta());
+    auto tA = std::chrono::steady_clock::now();
+    // the hierarchy on the device, for the duration of the assembly
+    TempDev tmp;
+    std::vector<DevHierLevel> hier(L + 1);
+    auto put_csr = [&](const HostCsr& M, DevCsr64& d) -> cudaError_t {
+        static_assert(sizeof(long long) == sizeof(i64), "row pointers are uploaded as they are");
+        long long* rp = nullptr; int* ci = nullptr; double* v = nullptr;
+        cudaError_t e = tmp.put(&rp, (const long long*)M.rp.data(), M.rp.size());
+        if (e == cudaSuccess) e = tmp.put(&ci, M.ci.data(), M.ci.size());
+        if (e == cudaSuccess) e = tmp.put(&v, M.v.data(), M.v.size());
+        d.rp = rp; d.ci = ci; d.v = v;
+        return e;
+    };
+    for (int l = 0; l <= L; ++l) {
+        const HostLevel& lv = h->H.lv[l];
+        DevHierLevel& d = hier[l];
+        std::memset(&d, 0, sizeof(d));
+        d.n = lv.A.nrows;
+        CUDA_TRY(put_csr(lv.A, d.A));
+        if (l < L) { CUDA_TRY(put_csr(lv.P, d.P)); CUDA_TRY(put_csr(lv.R, d.R)); }
+        double* dinv = nullptr;
+        CUDA_TRY(tmp.put(&dinv, lv.dinv.data(), lv.dinv.size()));
+        d.dinv = dinv;
+        if (!lv.cf.empty()) { int8_t* cf = nullptr; CUDA_TRY(tmp.put(&cf, lv.cf.data(), lv.cf.size())); d.cf = cf; }
+    }
+    DevHierLevel* d_hier = nullptr;
+    CUDA_TRY(tmp.put(&d_hier, hier.data(), hier.size()));
+
+    const int nw = std::max(1, std::min(nthreads, P));
+    std::vector<std::unique_ptr<CompositeBuilder>> builders(nw);
+    const int batch = std::max(1, env_int("AMGDD_SETUP_BATCH", 256));
+    const int thin = std::min(h->window, THIN_WINDOW);
+    Arena arena;
+    cudaStream_t st = h->stream;
+    GrowBuf<int> d_idx, d_rows;
+    GrowBuf<AsmSlice> d_slices;
+    GrowBuf<AsmJob> d_jobs;
+    GrowBuf<AsmPlan> d_plans;
+    GrowBuf<AsmCopy> d_copies;
+    std::vector<std::vector<i32>> lists;              // per subdomain of the batch: owned local indices, then gid of every private level
+    std::vector<AsmJob> jobs;
+    std::vector<AsmPlan> plans;
+    std::vector<AsmCopy> copies;
+    std::vector<i32> flat;
+    struct JobRef { int p, l, kind; };
+    std::vector<JobRef> refs;
+    double t_sets = 0, t_dev = 0;
+    for (int p0 = 0; p0 < P; p0 += batch) {
+        const int p1 = std::min(P, p0 + batch), nb_ = p1 - p0;
+        auto t0 = std::chrono::steady_clock::now();
+        // a. index sets on the host (breadth-first growth, S6/S7), one subdomain per task
+        lists.assign(nb_, std::vector<i32>());
+        std::atomic<int> next(p0);
+        std::atomic<int> status(AMGDD_SUCCESS);
+        std::string fail_detail;
+        std::mutex fail_mu;
+        auto work = [&](int t) {
+            if (!builders[t]) builders[t].reset(new CompositeBuilder(h->H, owner, owned, h->eta, h->nghost, h->window));
+            CompositeBuilder& cb = *builders[t];
+            std::vector<i32> own;
+            for (;;) {
+                const int p = next.fetch_add(1);
+                if (p >= p1 || status.load() != AMGDD_SUCCESS) break;
+                SubMeta& sm = h->subs[p];
+                if (!cb.plan_sets(p, sm.plan)) {
+                    std::lock_guard<std::mutex> g(fail_mu);
+                    status.store(AMGDD_ERR_INDEX_RANGE);
+                    fail_detail = "a composite level exceeds 2^31-1 local nonzeros";
+                    break;
+                }
+                std::vector<i32>& out = lists[p - p0];
+                cb.owned_local(own);
+                out.insert(out.end(), own.begin(), own.end());
+                for (int l = 0; l <= L; ++l) {
+                    if (sm.plan.lev[l].shared) continue;
+                    out.insert(out.end(), cb.real(l).begin(), cb.real(l).end());
+                    out.insert(out.end(), cb.ghost(l).begin(), cb.ghost(l).end());
+                }
+            }
+        };
+        {
+            std::vector<std::thread> pool;
+            for (int t = 1; t < nw; ++t) pool.emplace_back(work, t);
+            work(0);
+            for (auto& th : pool) th.join();
+        }
+        if (status.load() != AMGDD_SUCCESS) { g_detail = fail_detail; return status.load(); }
+        auto t1 = std::chrono::steady_clock::now();
+        t_sets += std::chrono::duration<double>(t1 - t0).count();
+        // b. index lists to the device; jobs of the batch
+        size_t total = 0;
+        std::vector<size_t> base(nb_);
+        for (int k = 0; k < nb_; ++k) { base[k] = total; total += (lists[k].size() + 3) & ~(size_t)3; }
+        flat.assign(total, 0);
+        for (int k = 0; k < nb_; ++k) std::copy(lists[k].begin(), lists[k].end(), flat.begin() + base[k]);
+        CUDA_TRY(d_idx.need(total));
+        CUDA_TRY(cudaMemcpyAsync(d_idx.p, flat.data(), total * sizeof(i32), cudaMemcpyHostToDevice, st));
+        jobs.clear(); refs.clear();
+        long long row_off = 0, slice_off = 0;
+        std::vector<std::vector<const int*>> gidp(nb_, std::vector<const int*>(L + 1, nullptr));
+        for (int k = 0; k < nb_; ++k) {
+            const SubdomainBlob& sb = h->subs[p0 + k].plan;
+            size_t o = base[k] + (size_t)sb.n_owned;
+            for (int l = 0; l <= L; ++l) {
+                if (sb.lev[l].shared) continue;
+                gidp[k][l] = d_idx.p + o;
+                o += (size_t)sb.lev[l].n_real + sb.lev[l].n_ghost;
+            }
+            for (int l = 0; l < L; ++l) {
+                const BlockLayout& b = sb.lev[l];
+                if (b.shared) continue;
+                const BlockLayout& c = sb.lev[l + 1];
+                const int nb = b.n_real + b.n_ghost, nbc = c.n_real + c.n_ghost;
+                for (int kind = 0; kind < 3; ++kind) {
+                    AsmJob j;
+                    std::memset(&j, 0, sizeof(j));
+                    j.kind = kind; j.level = l;
+                    j.nrows = kind == ASM_R ? nbc : nb;
+                    j.nrows_first = kind == ASM_A ? b.n_real : j.nrows;
+                    j.nr = b.n_real; j.ng = b.n_ghost; j.nrc = c.n_real; j.ngc = c.n_ghost;
+                    j.gid = gidp[k][l]; j.gidc = gidp[k][l + 1];
+                    j.window = kind == ASM_A ? h->window : thin;
+                    j.wide = (kind == ASM_P ? nbc : nb) > NARROW_MAX_COLS;
+                    j.scratch_row = row_off; j.scratch_slice = slice_off;
+                    row_off += 2LL * j.nrows;
+                    slice_off += (j.nrows_first + SLICE_ROWS - 1) / SLICE_ROWS + (j.nrows - j.nrows_first + SLICE_ROWS - 1) / SLICE_ROWS;
+                    jobs.push_back(j);
+                    refs.push_back({p0 + k, l, kind});
+                }
+            }
+        }
+        const int njobs = (int)jobs.size();
+        CUDA_TRY(d_rows.need((size_t)row_off));
+        CUDA_TRY(d_slices.need((size_t)slice_off));
+        CUDA_TRY(d_jobs.need(jobs.size()));
+        CUDA_TRY(d_plans.need(jobs.size()));
+        // c. plan pass: row lengths, sort, slices, dealing -> sizes and way tables
+        if (njobs) {
+            CUDA_TRY(cudaMemcpyAsync(d_jobs.p, jobs.data(), jobs.size() * sizeof(AsmJob), cudaMemcpyHostToDevice, st));
+            CUDA_TRY(launch_asm_plan(d_jobs.p, njobs, d_hier, d_rows.p, d_slices.p, d_plans.p, st));
+            plans.resize(jobs.size());
+            CUDA_TRY(cudaMemcpyAsync(plans.data(), d_plans.p, jobs.size() * sizeof(AsmPlan), cudaMemcpyDeviceToHost, st));
+        }
+        CUDA_TRY(cudaStreamSynchronize(st));
+        // d. layouts, arena space, destinations
+        for (int q = 0; q < njobs; ++q) {
+            const JobRef& r = refs[q];
+            const AsmPlan& pl = plans[q];
+            SubdomainBlob& sb = h->subs[r.p].plan;
+            BlockLayout& b = sb.lev[r.l];
+            if (pl.dropped > 0) {
+                g_detail = "subdomain " + std::to_string(r.p) + ": " + std::to_string(pl.dropped) +
+                           " interpolation entries of composite rows fall outside D-bar_{l+1}";
+                return AMGDD_ERR_NOT_CONNECTED_UPWARD;
+            }
+            if (pl.too_long_row >= 0) {
+                g_detail = "subdomain " + std::to_string(r.p) + ", level " + std::to_string(r.l) + ": a local matrix row has more than 65535 entries";
+                return AMGDD_ERR_INDEX_RANGE;
+            }
+            StreamLayout& sl = r.kind == ASM_A ? b.A : (r.kind == ASM_P ? b.P : b.R);
+            sl.nrows = jobs[q].nrows; sl.nnz = pl.nnz; sl.wide = jobs[q].wide != 0; sl.has_aux = r.kind != ASM_P;
+            sl.bytes = pl.bytes; sl.bytes_real = pl.bytes_real; sl.padded_nnz = pl.padded_nnz;
+            for (int w = 0; w < NUM_WAYS; ++w) sl.way[w] = pl.way[w];
+            if (r.kind == ASM_A) { b.nnzA = pl.nnz; b.nnzA_ghost = b.nnzA - b.nnzA_real; }
+            if (r.kind == ASM_P) b.nnzP = pl.nnz;
+        }
+        copies.clear();
+        for (int k = 0; k < nb_; ++k) {
+            SubMeta& sm = h->subs[p0 + k];
+            layout_blob(sm.plan);
+            std::string why;
+            const int arc = arena_take(h, arena, (size_t)std::max<i64>(sm.plan.bytes, 16), &sm.dev_base, why);
+            if (arc) { g_detail = why; return arc; }
+            AsmCopy c;
+            std::memset(&c, 0, sizeof(c));
+            c.src = d_idx.p + base[k]; c.dst = (int*)(sm.dev_base + sm.plan.off_owned); c.n = sm.plan.n_owned;
+            copies.push_back(c);
+            for (int l = 0; l <= L; ++l) {
+                const BlockLayout& b = sm.plan.lev[l];
+                if (b.shared) continue;
+                c.src = gidp[k][l]; c.dst = (int*)(sm.dev_base + b.off_gid); c.n = b.n_real + b.n_ghost; c.gather = 0; c.dinv = nullptr;
+                copies.push_back(c);
+                c.dst = (int*)(sm.dev_base + b.off_dinv); c.n = b.n_real; c.gather = 1; c.dinv = hier[l].dinv;
+                copies.push_back(c);
+            }
+        }
+        for (int q = 0; q < njobs; ++q) {
+            const JobRef& r = refs[q];
+            const SubMeta& sm = h->subs[r.p];
+            const BlockLayout& b = sm.plan.lev[r.l];
+            jobs[q].dst = sm.dev_base + (r.kind == ASM_A ? b.A.off : (r.kind == ASM_P ? b.P.off : b.R.off));
+        }
+        // e. write pass
+        CUDA_TRY(d_copies.need(copies.size()));
+        CUDA_TRY(cudaMemcpyAsync(d_copies.p, copies.data(), copies.size() * sizeof(AsmCopy), cudaMemcpyHostToDevice, st));
+        CUDA_TRY(launch_asm_copy(d_copies.p, (int)copies.size(), st));
+        if (njobs) {
+            CUDA_TRY(cudaMemcpyAsync(d_jobs.p, jobs.data(), jobs.size() * sizeof(AsmJob), cudaMemcpyHostToDevice, st));
+            CUDA_TRY(launch_asm_write(d_jobs.p, njobs, d_hier, d_rows.p, d_slices.p, d_plans.p, st));
+            CUDA_TRY(cudaMemcpyAsync(plans.data(), d_plans.p, jobs.size() * sizeof(AsmPlan), cudaMemcpyDeviceToHost, st));
+        }
+        CUDA_TRY(cudaStreamSynchronize(st));
+        for (int q = 0; q < njobs; ++q)
+            if (plans[q].bad_col) {
+                g_detail = "subdomain " + std::to_string(refs[q].p) + ", level " + std::to_string(refs[q].l) +
+                           ": a real row of A_l leaves D-bar_l (eq. 1 violated)";
+                return AMGDD_ERR_INDEX_RANGE;
+            }
+        t_dev += std::chrono::duration<double>(std::chrono::steady_clock::now() - t1).count();
+    }
+    h->stats.setup_seconds_index_sets = t_sets;
+    h->stats.setup_seconds_assembly = t_dev;
+    h->stats.setup_seconds_upload = std::chrono::duration<double>(std::chrono::steady_clock::now() - tA).count() - t_sets - t_dev;
+    h->stats.assembled_on_device = 1;
     return AMGDD_SUCCESS;
 }
 
@@ -282,12 +556,6 @@ void traffic_model(amgdd_handle_s* h) {
     for (int l = 0; l < L; ++l) g += 12.0 * h->H.lv[l].P.nnz() + 4.0 * h->H.lv[l + 1].A.nrows + 8.0 * (h->H.lv[l].A.nrows + h->H.lv[l + 1].A.nrows);
     g += 12.0 * (double)s.sum_real + 24.0 * h->n;                                // a3 gather, a10 update
     s.model_bytes_global = g;
-}
-
-int env_int(const char* name, int dflt) {
-    const char* v = std::getenv(name);
-    if (!v || !*v) return dflt;
-    return std::atoi(v);
 }
 
 StreamDesc make_desc(const char* base, const StreamLayout& lay, bool shared = false) {
@@ -530,7 +798,11 @@ int amgdd_setup(int64_t n, const int64_t* rowptr, const int32_t* colind, const d
         if (rc) { free_handle(h); return rc; }
         auto t1 = std::chrono::steady_clock::now();
         std::vector<i32> own(owner, owner + n);
-        rc = build_composites(h, own, std::min(nthreads, 32));
+        // AMGDD_ASSEMBLE=host keeps the local matrices and the packing on the host (the reference the device
+        // assembly is tested against); windows beyond the device sort's tile also take that path
+        const char* asm_env = std::getenv("AMGDD_ASSEMBLE");
+        const bool on_host = (asm_env && std::strcmp(asm_env, "host") == 0) || h->window > ASM_MAX_WINDOW;
+        rc = on_host ? build_composites(h, own, std::min(nthreads, 32)) : build_composites_device(h, own, std::min(nthreads, 32));
         if (rc) { free_handle(h); return rc; }
         rc = finish_tables(h);
         if (rc) { free_handle(h); return rc; }
@@ -853,6 +1125,30 @@ int amgdd_debug_fac_op_cycles(amgdd_handle_t h, int64_t* out, int32_t n, int32_t
         for (int j = 0; j < n && j < h->prog_nops; ++j) kinds_levels[j] = ops[j].kind * 256 + ops[j].level;
     }
     CUDA_TRY(cudaMemset(h->d_prof_ops, 0, cnt * sizeof(long long)));
+    return AMGDD_SUCCESS;
+}
+
+int amgdd_debug_read_block(amgdd_handle_t h, int32_t p, int32_t level, int32_t which, void* out, int64_t out_capacity, int64_t* out_bytes) {
+    if (bad_handle(h) || !out_bytes) return AMGDD_ERR_BAD_ARG;
+    if (p < 0 || p >= h->P || level < 0 || level > h->H.L || which < 0 || which > 5) { g_detail = "index out of range"; return AMGDD_ERR_BAD_ARG; }
+    const SubMeta& sm = h->subs[p];
+    const BlockLayout& b = sm.plan.lev[level];
+    i64 off = -1, bytes = 0;
+    if (which == 5) { off = sm.plan.off_owned; bytes = 4LL * sm.plan.n_owned; }
+    else if (!b.shared) {
+        switch (which) {
+            case 0: off = b.off_gid; bytes = 4LL * (b.n_real + b.n_ghost); break;
+            case 1: off = b.off_dinv; bytes = 8LL * b.n_real; break;
+            case 2: off = b.A.off; bytes = b.A.bytes; break;
+            case 3: off = b.P.off; bytes = b.P.bytes; break;
+            default: off = b.R.off; bytes = b.R.bytes; break;
+        }
+    }
+    *out_bytes = bytes;
+    if (!out || bytes == 0) return AMGDD_SUCCESS;
+    if (out_capacity < bytes) { g_detail = "out_capacity too small"; return AMGDD_ERR_BAD_ARG; }
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    CUDA_TRY(cudaMemcpy(out, sm.dev_base + off, (size_t)bytes, cudaMemcpyDeviceToHost));
     return AMGDD_SUCCESS;
 }
 

@@ -1,0 +1,313 @@
+// Kernels of the device-side composite-grid assembly (amgdd_assemble.cuh).  One CTA per stream of a
+// (subdomain, level) block.  Pass 1 (plan): local row lengths, the stable sort by length inside the
+// windows, the slices and their greedy dealing to the ways -- the same rules as the host packer, so
+// both produce the same bytes.  Pass 2 (write): one warp per slice walks the global rows of its 32
+// lanes, renumbers the columns by binary search in the sorted index lists of the block and stores
+// headers and groups with coalesced 16-byte stores.
+#include "amgdd_assemble.cuh"
+
+#include <climits>
+
+namespace amgdd {
+
+namespace {
+
+constexpr int ASM_THREADS = 256;
+
+__device__ __forceinline__ int find_sorted(const int* __restrict__ a, int n, int g) {
+    int lo = 0, hi = n;
+    while (lo < hi) {
+        const int mid = (lo + hi) >> 1;
+        if (__ldg(a + mid) < g) lo = mid + 1; else hi = mid;
+    }
+    return (lo < n && __ldg(a + lo) == g) ? lo : -1;
+}
+
+// local index of global point g in a level given by its lists (real ascending, then ghost ascending; S7)
+__device__ __forceinline__ int local_of(const int* __restrict__ gid, int nr, int ng, int g) {
+    if (gid == nullptr) return g;                                    // fully covered level: identity
+    const int r = find_sorted(gid, nr, g);
+    if (r >= 0) return r;
+    const int q = find_sorted(gid + nr, ng, g);
+    return q >= 0 ? nr + q : -1;
+}
+
+// Enumerates the kept entries of local row i of a job in stored order:
+//   A, real row:  the whole global row (eq. 1: all of it lies in D-bar_l)
+//   A, ghost row: the entries whose column is a real point (A12)
+//   P:            the entries whose column lies in D-bar_{l+1} (the others are counted: A7)
+//   R:            the entries whose column (a point of level l) lies in D-bar_l, real columns first, then ghost
+//                 columns (= ascending local index: the order of the host's counting-sort transpose)
+struct RowCursor {
+    const int* ci; const double* v;
+    long long beg, cur, end;
+    int pass;
+};
+
+__device__ __forceinline__ void row_open(const AsmJob& J, const DevHierLevel& H, int i, RowCursor& c) {
+    const DevCsr64& M = J.kind == ASM_A ? H.A : (J.kind == ASM_P ? H.P : H.R);
+    const int g = J.kind == ASM_R ? (J.gidc ? __ldg(J.gidc + i) : i) : __ldg(J.gid + i);
+    c.ci = M.ci; c.v = M.v;
+    c.beg = c.cur = M.rp[g];
+    c.end = M.rp[g + 1];
+    c.pass = 0;
+}
+
+// next kept entry: returns false when the row is exhausted; *bad is raised for an impossible column
+__device__ __forceinline__ bool row_next(const AsmJob& J, int i, RowCursor& c, int& col, double& val, int& bad) {
+    for (;;) {
+        if (c.cur >= c.end) {
+            if (J.kind == ASM_R && c.pass == 0) { c.pass = 1; c.cur = c.beg; continue; }
+            return false;
+        }
+        const long long k = c.cur++;
+        const int g = __ldg(c.ci + k);
+        int loc;
+        if (J.kind == ASM_A) {
+            if (i < J.nr) { loc = local_of(J.gid, J.nr, J.ng, g); if (loc < 0) bad = 1; }
+            else { loc = find_sorted(J.gid, J.nr, g); if (loc < 0) continue; }
+        } else if (J.kind == ASM_P) {
+            loc = local_of(J.gidc, J.nrc, J.ngc, g);
+            if (loc < 0) continue;
+        } else {
+            if (c.pass == 0) { loc = find_sorted(J.gid, J.nr, g); if (loc < 0) continue; }
+            else { loc = find_sorted(J.gid + J.nr, J.ng, g); if (loc < 0) continue; loc += J.nr; }
+        }
+        col = loc; val = c.v[k];
+        return true;
+    }
+}
+
+__device__ __forceinline__ int row_length(const AsmJob& J, const DevHierLevel& H, int i, int& dropped) {
+    const DevCsr64& M = J.kind == ASM_A ? H.A : (J.kind == ASM_P ? H.P : H.R);
+    const int g = J.kind == ASM_R ? (J.gidc ? __ldg(J.gidc + i) : i) : __ldg(J.gid + i);
+    const long long b = M.rp[g], e = M.rp[g + 1];
+    if (J.kind == ASM_A && i < J.nr) return (int)(e - b);
+    int n = 0;
+    for (long long k = b; k < e; ++k) {
+        const int c = __ldg(M.ci + k);
+        if (J.kind == ASM_A) n += find_sorted(J.gid, J.nr, c) >= 0;
+        else if (J.kind == ASM_P) { const bool in = local_of(J.gidc, J.nrc, J.ngc, c) >= 0; n += in; dropped += !in; }
+        else n += local_of(J.gid, J.nr, J.ng, c) >= 0;
+    }
+    return n;
+}
+
+// first sorted position of slice s and the rows it holds
+__device__ __forceinline__ void slice_span(const AsmJob& J, int s, int& pos, int& cnt) {
+    const int n0 = J.nrows_first, s0 = (n0 + SLICE_ROWS - 1) / SLICE_ROWS;
+    if (s < s0) { pos = s * SLICE_ROWS; cnt = min(SLICE_ROWS, n0 - pos); }
+    else { pos = n0 + (s - s0) * SLICE_ROWS; cnt = min(SLICE_ROWS, J.nrows - pos); }
+}
+
+__global__ void __launch_bounds__(ASM_THREADS) asm_plan_kernel(const AsmJob* __restrict__ jobs, const DevHierLevel* __restrict__ hier,
+                                                                 int* __restrict__ row_scratch, AsmSlice* __restrict__ slice_scratch,
+                                                                 AsmPlan* __restrict__ plans) {
+    const AsmJob J = jobs[blockIdx.x];
+    const DevHierLevel H = hier[J.level];
+    int* len = row_scratch + J.scratch_row;
+    int* order = len + J.nrows;
+    AsmSlice* sl = slice_scratch + J.scratch_slice;
+    __shared__ unsigned long long s_nnz;
+    __shared__ int s_dropped, s_toolong;
+    __shared__ int tile[ASM_MAX_WINDOW];
+    const int tid = threadIdx.x;
+    if (tid == 0) { s_nnz = 0; s_dropped = 0; s_toolong = INT_MAX; }
+    __syncthreads();
+    // 1. local row lengths
+    {
+        unsigned long long nnz = 0;
+        int dropped = 0, toolong = INT_MAX;
+        for (int i = tid; i < J.nrows; i += ASM_THREADS) {
+            const int n = row_length(J, H, i, dropped);
+            len[i] = n;
+            nnz += (unsigned long long)n;
+            if (n > 65535 && i < toolong) toolong = i;
+        }
+        if (nnz) atomicAdd(&s_nnz, nnz);
+        if (dropped) atomicAdd(&s_dropped, dropped);
+        if (toolong != INT_MAX) atomicMin(&s_toolong, toolong);
+    }
+    __syncthreads();
+    // 2. inside every window of a row group: stable sort by descending length (rank by counting)
+    const int gb[3] = {0, J.nrows_first, J.nrows};
+    for (int g = 0; g < 2; ++g)
+        for (int w0 = gb[g]; w0 < gb[g + 1]; w0 += J.window) {
+            const int m = min(J.window, gb[g + 1] - w0);
+            for (int k = tid; k < m; k += ASM_THREADS) tile[k] = len[w0 + k];
+            __syncthreads();
+            for (int k = tid; k < m; k += ASM_THREADS) {
+                const int mine = tile[k];
+                int rank = 0;
+                for (int j = 0; j < m; ++j) { const int o = tile[j]; rank += (o > mine) || (o == mine && j < k); }
+                order[w0 + rank] = w0 + k;
+            }
+            __syncthreads();
+        }
+    // 3. groups of every slice: its first lane holds the longest row
+    const int n0 = J.nrows_first, n1 = J.nrows - n0;
+    const int S0 = (n0 + SLICE_ROWS - 1) / SLICE_ROWS, S = S0 + (n1 + SLICE_ROWS - 1) / SLICE_ROWS;
+    for (int s = tid; s < S; s += ASM_THREADS) {
+        int pos, cnt;
+        slice_span(J, s, pos, cnt);
+        const int longest = len[order[pos]];
+        sl[s].K = (uint32_t)max(1, (longest + GROUP_STEPS - 1) / GROUP_STEPS);
+    }
+    __syncthreads();
+    // 4. deal the slices to the ways in slice order, each to the way with the fewest bytes so far (ties: lowest way)
+    if (tid < 32) {
+        const int lane = tid;
+        const long long gbytes = J.wide ? GROUP_BYTES_WIDE : GROUP_BYTES_NARROW;
+        long long load = 0;
+        uint32_t ngr = 0, nsl = 0, ngr_first = 0, nsl_first = 0;
+        for (int s = 0; s < S; ++s) {
+            const uint32_t K = sl[s].K;
+            long long key = lane < NUM_WAYS ? load : LLONG_MAX;
+            int best = lane;
+#pragma unroll
+            for (int off = 16; off >= 1; off >>= 1) {
+                const long long ok = __shfl_xor_sync(0xffffffffu, key, off);
+                const int ob = __shfl_xor_sync(0xffffffffu, best, off);
+                if (ok < key || (ok == key && ob < best)) { key = ok; best = ob; }
+            }
+            if (lane == best) {
+                sl[s].way = (uint32_t)lane; sl[s].g_off = ngr; sl[s].h_idx = nsl;
+                load += (long long)K * gbytes + HEADER_BYTES;
+                ngr += K; nsl += 1;
+                if (s < S0) { ngr_first += K; nsl_first += 1; }
+            }
+        }
+        // offsets: all groups way by way, then all headers way by way (128-byte units; both sizes are multiples of 128)
+        const unsigned long long gb128 = (unsigned long long)ngr * (unsigned long long)(gbytes / 128);
+        const unsigned long long hb128 = (unsigned long long)nsl * (HEADER_BYTES / 128);
+        unsigned long long gpre = gb128, hpre = hb128;                // inclusive scans over the lanes
+#pragma unroll
+        for (int off = 1; off < 32; off <<= 1) {
+            const unsigned long long a = __shfl_up_sync(0xffffffffu, gpre, off);
+            const unsigned long long b = __shfl_up_sync(0xffffffffu, hpre, off);
+            if (lane >= off) { gpre += a; hpre += b; }
+        }
+        const unsigned long long gtot = __shfl_sync(0xffffffffu, gpre, 31);
+        const unsigned long long htot = __shfl_sync(0xffffffffu, hpre, 31);
+        unsigned long long tg = ngr, ts = nsl, tgf = ngr_first, tsf = nsl_first;
+#pragma unroll
+        for (int off = 16; off >= 1; off >>= 1) {
+            tg += __shfl_xor_sync(0xffffffffu, tg, off); ts += __shfl_xor_sync(0xffffffffu, ts, off);
+            tgf += __shfl_xor_sync(0xffffffffu, tgf, off); tsf += __shfl_xor_sync(0xffffffffu, tsf, off);
+        }
+        AsmPlan& pl = plans[blockIdx.x];
+        if (lane < NUM_WAYS) {
+            WayDesc d;
+            d.grp_off128 = (uint32_t)(gpre - gb128);
+            d.hdr_off128 = (uint32_t)(gtot + hpre - hb128);
+            d.ngroups = ngr; d.ngroups_real = ngr_first; d.nslices = nsl; d.nslices_real = nsl_first;
+            d.pad_[0] = d.pad_[1] = 0;
+            pl.way[lane] = d;
+        }
+        if (lane == 0) {
+            pl.bytes = (long long)((gtot + htot) * 128ull);
+            pl.bytes_real = (long long)tgf * gbytes + (long long)tsf * HEADER_BYTES;
+            pl.padded_nnz = (long long)tg * GROUP_STEPS * SLICE_ROWS;
+            pl.nnz = (long long)s_nnz;
+            pl.dropped = s_dropped;
+            pl.too_long_row = s_toolong == INT_MAX ? -1 : s_toolong;
+            pl.bad_col = 0; pl.pad_ = 0;
+        }
+    }
+}
+
+__global__ void __launch_bounds__(ASM_THREADS) asm_write_kernel(const AsmJob* __restrict__ jobs, const DevHierLevel* __restrict__ hier,
+                                                                  const int* __restrict__ row_scratch, const AsmSlice* __restrict__ slice_scratch,
+                                                                  AsmPlan* __restrict__ plans) {
+    const AsmJob J = jobs[blockIdx.x];
+    const DevHierLevel H = hier[J.level];
+    const int* len = row_scratch + J.scratch_row;
+    const int* order = len + J.nrows;
+    const AsmSlice* sl = slice_scratch + J.scratch_slice;
+    const AsmPlan& pl = plans[blockIdx.x];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = ASM_THREADS / 32;
+    const int n0 = J.nrows_first, n1 = J.nrows - n0;
+    const int S = (n0 + SLICE_ROWS - 1) / SLICE_ROWS + (n1 + SLICE_ROWS - 1) / SLICE_ROWS;
+    const int gbytes = J.wide ? GROUP_BYTES_WIDE : GROUP_BYTES_NARROW;
+    // aux / flag of a row: A_l rows are points of level l, R_l rows points of level l+1; ghosts never relax (A4)
+    const DevHierLevel Hr = J.kind == ASM_R ? hier[J.level + 1] : H;
+    const int* rgid = J.kind == ASM_R ? J.gidc : J.gid;
+    const int rreal = J.kind == ASM_R ? J.nrc : J.nr;
+    int bad = 0;
+    for (int s = warp; s < S; s += nwarps) {
+        const AsmSlice rec = sl[s];
+        int pos, cnt;
+        slice_span(J, s, pos, cnt);
+        const int row = lane < cnt ? order[pos + lane] : -1;
+        char* h = J.dst + 128ll * pl.way[rec.way].hdr_off128 + (long long)rec.h_idx * HEADER_BYTES;
+        char* g = J.dst + 128ll * pl.way[rec.way].grp_off128 + (long long)rec.g_off * gbytes;
+        {   // header: {row, K | flag << 31, aux}
+            double aux = 0.0;
+            uint32_t flag = 0;
+            if (J.kind != ASM_P && row >= 0 && row < rreal) {
+                const int gp = rgid ? __ldg(rgid + row) : row;
+                aux = Hr.dinv[gp];
+                if (Hr.cf != nullptr && Hr.cf[gp] > 0) flag = 0x80000000u;
+            }
+            uint4 w;
+            w.x = row >= 0 ? (uint32_t)row : NO_ROW;
+            w.y = rec.K | flag;
+            w.z = (uint32_t)__double_as_longlong(aux);
+            w.w = (uint32_t)(__double_as_longlong(aux) >> 32);
+            *reinterpret_cast<uint4*>(h + 16 * lane) = w;
+        }
+        RowCursor c;
+        int mylen = 0;
+        if (row >= 0) { mylen = len[row]; row_open(J, H, row, c); }
+        int done = 0;
+        for (uint32_t kg = 0; kg < rec.K; ++kg, g += gbytes) {
+            double v[GROUP_STEPS];
+            uint32_t col[GROUP_STEPS];
+#pragma unroll
+            for (int q = 0; q < GROUP_STEPS; ++q) {
+                v[q] = 0.0; col[q] = 0;
+                if (done < mylen) {
+                    int cc = 0; double vv = 0.0;
+                    if (row_next(J, row, c, cc, vv, bad)) { v[q] = vv; col[q] = (uint32_t)cc; }
+                    ++done;
+                }
+            }
+            *reinterpret_cast<double2*>(g + 16 * lane) = make_double2(v[0], v[1]);
+            *reinterpret_cast<double2*>(g + 512 + 16 * lane) = make_double2(v[2], v[3]);
+            if (J.wide) *reinterpret_cast<uint4*>(g + 1024 + 16 * lane) = make_uint4(col[0], col[1], col[2], col[3]);
+            else *reinterpret_cast<uint2*>(g + 1024 + 8 * lane) = make_uint2((col[0] & 0xFFFFu) | (col[1] << 16), (col[2] & 0xFFFFu) | (col[3] << 16));
+        }
+    }
+    if (bad) atomicOr(&plans[blockIdx.x].bad_col, 1);
+}
+
+__global__ void __launch_bounds__(ASM_THREADS) asm_copy_kernel(const AsmCopy* __restrict__ jobs) {
+    const AsmCopy c = jobs[blockIdx.x];
+    if (c.gather) {
+        double* d = reinterpret_cast<double*>(c.dst);
+        for (int i = threadIdx.x; i < c.n; i += ASM_THREADS) d[i] = c.dinv[c.src[i]];
+    } else {
+        for (int i = threadIdx.x; i < c.n; i += ASM_THREADS) c.dst[i] = c.src[i];
+    }
+}
+
+}  // namespace
+
+cudaError_t launch_asm_plan(const AsmJob* jobs, int njobs, const DevHierLevel* hier, int* row_scratch, AsmSlice* slice_scratch,
+                            AsmPlan* plans, cudaStream_t st) {
+    if (njobs > 0) asm_plan_kernel<<<njobs, ASM_THREADS, 0, st>>>(jobs, hier, row_scratch, slice_scratch, plans);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_asm_write(const AsmJob* jobs, int njobs, const DevHierLevel* hier, const int* row_scratch,
+                             const AsmSlice* slice_scratch, AsmPlan* plans, cudaStream_t st) {
+    if (njobs > 0) asm_write_kernel<<<njobs, ASM_THREADS, 0, st>>>(jobs, hier, row_scratch, slice_scratch, plans);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_asm_copy(const AsmCopy* jobs, int njobs, cudaStream_t st) {
+    if (njobs > 0) asm_copy_kernel<<<njobs, ASM_THREADS, 0, st>>>(jobs);
+    return cudaGetLastError();
+}
+
+}  // namespace amgdd

@@ -1,0 +1,75 @@
+// Device-side assembly of the composite-grid matrices (paper P:335: "a clear
+// dominant cost: setting up local indices ... (primarily mapping global to local column indices for the
+// matrices A_l on each level)").  The host only grows the index sets D_l^p / D-bar_l^p (breadth-first
+// search, amgdd_composite.cpp); the rows of the global A_l, P_l, R_l are then cut out, renumbered and
+// packed into the SELL-32 group streams (amgdd_stream.hpp) by two kernels, straight into the subdomain's
+// device blob.  The streams are byte-identical to the ones the host packer writes (amgdd_pack.cpp);
+// tests/test_gpu_assembly.py compares them.  Index work only: values are copied, never computed.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "amgdd_stream.hpp"
+
+namespace amgdd {
+
+struct DevCsr64 {               // a whole level matrix on the device, row pointers as the host keeps them
+    const long long* rp;
+    const int* ci;
+    const double* v;
+};
+
+struct DevHierLevel {
+    DevCsr64 A, P, R;           // P, R: null pointers on the coarsest level
+    const double* dinv;         // l1 diagonal inverse (S8)
+    const int8_t* cf;           // +1 C / -1 F; null when the level has no splitting (coarsest)
+    long long n;
+};
+
+enum AsmKind : int { ASM_A = 0, ASM_P = 1, ASM_R = 2 };
+
+// One stream of one private (subdomain, level) block.
+struct AsmJob {
+    int kind;                   // AsmKind
+    int level;                  // l: A_l, P_l, R_l
+    int nrows;                  // rows of the stream (A, P: n_bar(l); R: n_bar(l+1))
+    int nrows_first;            // rows of the first row group (A: n_real(l); P, R: nrows)
+    int nr, ng;                 // |D_l^p|, ghosts of level l
+    int nrc, ngc;               // the same of level l+1 (ngc = 0 and gidc = null when l+1 is fully covered)
+    const int* gid;             // DEVICE: global indices of level l, real ascending then ghost ascending
+    const int* gidc;            // DEVICE: the same of level l+1, or null: local index = global index
+    int window;                 // sort window of the stream (<= ASM_MAX_WINDOW)
+    int wide;                   // 32-bit column indices
+    long long scratch_row;      // offset (ints) of this job's row scratch: len[nrows], order[nrows]
+    long long scratch_slice;    // offset (AsmSlice) of its slice scratch
+    char* dst;                  // DEVICE: where the stream goes (set between the two passes)
+};
+
+struct AsmSlice { uint32_t K, way, g_off, h_idx; };   // groups; way; groups / slices of the way before it
+
+struct AsmPlan {                // what the plan pass reports per job
+    WayDesc way[NUM_WAYS];
+    long long bytes, bytes_real, padded_nnz, nnz;
+    int dropped;                // P entries that point outside D-bar_{l+1} (A7)
+    int too_long_row;           // a row with more than 65535 entries (-1: none)
+    int bad_col;                // write pass: entries of a real row of A_l outside D-bar_l (eq. 1 violated; must stay 0)
+    int pad_;
+};
+
+struct AsmCopy {                // gid / owned-index copies and the gather of the l1 diagonal of the real points
+    const int* src;             // DEVICE ints
+    int* dst;                   // DEVICE
+    int n;
+    int gather;                 // 1: dst is double*, dst[i] = dinv[src[i]]
+    const double* dinv;
+};
+
+constexpr int ASM_MAX_WINDOW = 1024;
+
+cudaError_t launch_asm_plan(const AsmJob* jobs, int njobs, const DevHierLevel* hier, int* row_scratch, AsmSlice* slice_scratch,
+                            AsmPlan* plans, cudaStream_t st);
+cudaError_t launch_asm_write(const AsmJob* jobs, int njobs, const DevHierLevel* hier, const int* row_scratch,
+                             const AsmSlice* slice_scratch, AsmPlan* plans, cudaStream_t st);
+cudaError_t launch_asm_copy(const AsmCopy* jobs, int njobs, cudaStream_t st);
+
+}  // namespace amgdd

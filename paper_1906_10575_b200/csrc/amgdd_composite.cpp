@@ -77,6 +77,14 @@ void CompositeBuilder::grow(int l, const std::vector<i32>& seed, int dist, std::
 }
 
 void CompositeBuilder::plan(int p, SubdomainBlob& out) {
+    if (!plan_sets(p, out)) return;
+    plan_matrices(out);
+    layout_blob(out);
+}
+
+// Index sets D_l^p, D-bar_l^p of every level (S6, S7, eq. 1) and the sizes that follow from them alone.
+// Returns false (out.bytes = 0, the offending counts in out.lev[l]) when a level would overflow 32-bit local offsets.
+bool CompositeBuilder::plan_sets(int p, SubdomainBlob& out) {
     const int L = H_.L;
     p_ = p;
     out.lev.assign(L + 1, BlockLayout());
@@ -111,7 +119,7 @@ void CompositeBuilder::plan(int p, SubdomainBlob& out) {
         b.n_ghost = (i32)gh.size();
         b.shared = ((i64)re.size() == nl);
     }
-    // local matrices (only sizes are needed for shared levels)
+    out.n_owned = (i32)owned_[p].size();
     for (int l = 0; l <= L; ++l) {
         BlockLayout& b = out.lev[l];
         const HostLevel& lv = H_.lv[l];
@@ -123,12 +131,30 @@ void CompositeBuilder::plan(int p, SubdomainBlob& out) {
             continue;
         }
         auto gid_of = [&](i32 i) { return i < nr ? real_[l][i] : ghost_[l][i - nr]; };
-        {   // 32-bit local offsets: refuse (AMGDD_ERR_INDEX_RANGE in the caller) before anything overflows
-            i64 bound = b.nnzA_real, boundP = 0;
-            for (i32 g : ghost_[l]) bound += lv.A.rp[g + 1] - lv.A.rp[g];
-            for (i32 i = 0; i < nb; ++i) boundP += lv.P.rp[gid_of(i) + 1] - lv.P.rp[gid_of(i)];
-            if (bound > (i64)INT32_MAX || boundP > (i64)INT32_MAX) { b.nnzA = bound; b.nnzP = boundP; out.bytes = 0; return; }
-        }
+        // 32-bit local offsets: refuse (AMGDD_ERR_INDEX_RANGE in the caller) before anything overflows
+        i64 bound = b.nnzA_real, boundP = 0;
+        for (i32 g : ghost_[l]) bound += lv.A.rp[g + 1] - lv.A.rp[g];
+        for (i32 i = 0; i < nb; ++i) boundP += lv.P.rp[gid_of(i) + 1] - lv.P.rp[gid_of(i)];
+        if (bound > (i64)INT32_MAX || boundP > (i64)INT32_MAX) { b.nnzA = bound; b.nnzP = boundP; out.bytes = 0; return false; }
+    }
+    return true;
+}
+
+void CompositeBuilder::owned_local(std::vector<i32>& out) const {
+    const std::vector<i32>& o = owned_[p_];
+    out.resize(o.size());
+    for (size_t k = 0; k < o.size(); ++k) out[k] = loc_[0][o[k]];
+}
+
+// Local matrices of the private levels (host assembly) and the plans of their streams.
+void CompositeBuilder::plan_matrices(SubdomainBlob& out) {
+    const int L = H_.L;
+    for (int l = 0; l <= L; ++l) {
+        BlockLayout& b = out.lev[l];
+        const HostLevel& lv = H_.lv[l];
+        const i32 nr = b.n_real, nb = b.n_real + b.n_ghost;
+        if (b.shared) continue;
+        auto gid_of = [&](i32 i) { return i < nr ? real_[l][i] : ghost_[l][i - nr]; };
         LocalCsr& A = A_[l];
         A.rp.assign((size_t)nb + 1, 0); A.ci.clear(); A.v.clear();
         for (i32 i = 0; i < nb; ++i) {
@@ -172,10 +198,13 @@ void CompositeBuilder::plan(int p, SubdomainBlob& out) {
         layout_stream(R, nbc, nb, true, thin_window(), nbc, b.R, bad);
         if (bad >= 0 && out.too_long_row < 0) { out.too_long_row = bad; out.too_long_level = l; }
     }
-    // blob layout
+}
+
+// Where the arrays of a subdomain sit inside its blob (sizes of all streams known).
+void layout_blob(SubdomainBlob& out) {
+    const int L = (int)out.lev.size() - 1;
     i64 off = 0;
     auto take = [&](i64 bytes) { const i64 o = off; off = (off + bytes + 127) & ~(i64)127; return o; };   // streams need 128-byte alignment
-    out.n_owned = (i32)owned_[p].size();
     out.off_owned = take((i64)out.n_owned * 4);
     for (int l = 0; l <= L; ++l) {
         BlockLayout& b = out.lev[l];

@@ -120,8 +120,14 @@ class CompositeBuilder {
 public:
     CompositeBuilder(const Hierarchy& H, const std::vector<i32>& owner, const std::vector<std::vector<i32>>& owned,
                      int eta, int num_ghost, int window);
-    // Phase 1: index sets, local matrices and the blob layout of subdomain p.
+    // Phase 1: index sets, local matrices and the blob layout of subdomain p (= plan_sets, plan_matrices, layout_blob).
     void plan(int p, SubdomainBlob& out);
+    // Phase 1 in parts (the device-side assembly runs only the first on the host)
+    bool plan_sets(int p, SubdomainBlob& out);
+    void plan_matrices(SubdomainBlob& out);
+    // local indices (level 0) of the owned dofs of the subdomain planned last
+    void owned_local(std::vector<i32>& out) const;
+    int thin_window_of() const { return thin_window(); }
     // Phase 2: write the arrays of the subdomain planned last into dst (out.bytes bytes).
     void fill(const SubdomainBlob& plan, char* dst);
     // index sets of the subdomain planned last
@@ -147,6 +153,9 @@ private:
     std::vector<uint8_t> flg_;
     i32 local_of(int l, i32 g) const { return stamp_[l][g] == epoch_[l] ? loc_[l][g] : -1; }
 };
+
+// offsets of the arrays inside a subdomain's blob, from the sizes in out.lev (out.n_owned set)
+void layout_blob(SubdomainBlob& out);
 
 // packs a whole level matrix (the shared global copy) into a host buffer
 struct PackedLevelStream {
