@@ -291,6 +291,7 @@ def run_b200(args, p, rank, world, local_rank):
                 "multi_gpu": "replicas only (north_star: one GPU, no sharding, no collectives)" if args.gpus > 1 else "single GPU",
                 "setup_seconds": setup_s, "setup_seconds_hierarchy": st["setup_seconds_hierarchy"],
                 "setup_seconds_composite": st["setup_seconds_composite"],
+                "composite_assembly": "device" if st["assembled_on_device"] else "host",
             },
             "clocks": clocks,
             "e2e": {"value": e2e_ms, "unit": UNIT, "h2d_bytes_per_step": 2 * 8 * p.n, "d2h_bytes_per_step": 8 * p.n + 16},
