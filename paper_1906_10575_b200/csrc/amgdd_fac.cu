@@ -42,6 +42,9 @@ constexpr int D = RING_DEPTH;
 #ifndef AMGDD_STAGE2
 #define AMGDD_STAGE2 0
 #endif
+#ifndef AMGDD_EARLY_COMMIT
+#define AMGDD_EARLY_COMMIT 1     // commit every batch of asynchronous copies where it is issued (0: cp.async.wait_all at the wait)
+#endif
 #if AMGDD_STAGE2
 constexpr int STAGE_BYTES = 512 + 4 * 256 + 2 * 1024;   // per warp: slice 0's header, four {row, info} slots, two operand slots (e0 | e1 | e2 | aux)
 #else
@@ -103,9 +106,17 @@ __device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
 __device__ __forceinline__ void cp_async8(uint32_t dst, const void* src) {
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
 }
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
-#if AMGDD_STAGE2
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+#if AMGDD_EARLY_COMMIT && !AMGDD_STAGE2
+// every batch of copies is committed where it is issued (cp_async_issued), so the wait does not plant a new
+// completion marker behind the ring's loads that were issued in between
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_issued() { cp_async_commit(); }
+#else
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_issued() {}
+#endif
+#if AMGDD_STAGE2
 __device__ __forceinline__ void cp_async_wait_pending(int) { asm volatile("cp.async.wait_group 1;" ::: "memory"); }
 __device__ __forceinline__ uint32_t lds_u32(uint32_t a) {
     uint32_t v;
@@ -371,6 +382,7 @@ struct Worker {
                 }
                 cp_async_wait_all();
                 cp_async16(stage + 16 * lane, nxt_hdr + 16 * lane);
+                cp_async_issued();
             }
             tock(PROF_OP0 + kind, tp0);
             return;
@@ -415,7 +427,7 @@ struct Worker {
                 if (cC) cp_async8(stC + 512, cC + r);
             }
         };
-        if (!hdr_ready) { cp_async_wait_all(); cp_async16(stH, hdr); }       // (never two copies in flight to one slot)
+        if (!hdr_ready) { cp_async_wait_all(); cp_async16(stH, hdr); cp_async_issued(); }       // (never two copies in flight to one slot)
         cp_async_wait_all();
         uint4 h = lds128(stH);
         uint32_t row = h.x;
@@ -424,6 +436,7 @@ struct Worker {
         double aux = mkdouble(h.z, h.w);
         fetch_ctx(row);
         cp_async16(stH, nsl > 1 ? hdr + HEADER_BYTES : hdr_after);
+        cp_async_issued();
         hdr_ready = n_next > 0;
 #endif
         int sidx = 0;
@@ -512,6 +525,7 @@ struct Worker {
                 row = h.x; left = (int)(h.y & HDR_GROUPS_MASK); is_c = (h.y >> 31) != 0; aux = mkdouble(h.z, h.w);
                 fetch_ctx(row);
                 cp_async16(stH, sidx + 1 < nsl ? hdr + (long long)(sidx + 1) * HEADER_BYTES : hdr_after);
+                cp_async_issued();
             }
         };
 #endif
