@@ -465,9 +465,16 @@ int build_composites_device(amgdd_handle_s* h, const std::vector<i32>& owner, in
             if (r.kind == ASM_P) b.nnzP = pl.nnz;
         }
         copies.clear();
+        {   // one arena chunk per batch instead of many 1 GB chunks (cudaMalloc is not cheap)
+            size_t total = 0;
+            for (int k = 0; k < nb_; ++k) {
+                layout_blob(h->subs[p0 + k].plan);
+                total += ((size_t)std::max<i64>(h->subs[p0 + k].plan.bytes, 16) + 255) & ~(size_t)255;
+            }
+            arena.chunk = std::max<size_t>((size_t)1 << 30, total);
+        }
         for (int k = 0; k < nb_; ++k) {
             SubMeta& sm = h->subs[p0 + k];
-            layout_blob(sm.plan);
             std::string why;
             const int arc = arena_take(h, arena, (size_t)std::max<i64>(sm.plan.bytes, 16), &sm.dev_base, why);
             if (arc) { g_detail = why; return arc; }
