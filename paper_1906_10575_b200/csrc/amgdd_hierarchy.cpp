@@ -2,12 +2,15 @@
 // colouring, direct interpolation, explicit R = P^T, Galerkin A_{l+1} = R_l A_l P_l (paper P:49),
 // l1 diagonals and the dense LU of the coarsest operator.  Follows readings S1-S5, S8 of
 // DESIGN.md.  Written independently of oracle/ (different data structures and algorithms:
-// per-entry strength flags, lazy max-heap colouring, threaded symbolic/numeric triple product).
+// per-entry strength flags, bucketed bitmap colouring, threaded symbolic/numeric triple product).
 #include "amgdd_host.hpp"
 
 #include <algorithm>
+#include <chrono>
 #include <cmath>
-#include <queue>
+#include <cstdio>
+#include <cstdlib>
+#include <memory>
 
 namespace amgdd {
 
@@ -62,7 +65,36 @@ void strength_flags(const HostCsr& A, double theta, int nthreads, std::vector<ui
     });
 }
 
-// S2: first pass of the RS colouring with a lazy max-heap keyed (lambda desc, index asc).
+// A set of indices in [0, n) with "lowest member" in a few word operations: a bitmap with two summary levels.
+struct IndexSet {
+    std::vector<uint64_t> l0, l1, l2;
+    i64 count = 0;
+    explicit IndexSet(i64 n) : l0((size_t)((n + 63) >> 6), 0), l1((l0.size() + 63) >> 6, 0), l2((l1.size() + 63) >> 6, 0) {}
+    void insert(i64 i) {
+        const i64 w0 = i >> 6, w1 = w0 >> 6;
+        l0[w0] |= 1ull << (i & 63); l1[w1] |= 1ull << (w0 & 63); l2[w1 >> 6] |= 1ull << (w1 & 63);
+        ++count;
+    }
+    void erase(i64 i) {
+        const i64 w0 = i >> 6, w1 = w0 >> 6;
+        l0[w0] &= ~(1ull << (i & 63));
+        if (!l0[w0]) { l1[w1] &= ~(1ull << (w0 & 63)); if (!l1[w1]) l2[w1 >> 6] &= ~(1ull << (w1 & 63)); }
+        --count;
+    }
+    i64 lowest() const {
+        for (size_t k = 0; k < l2.size(); ++k)
+            if (l2[k]) {
+                const i64 w1 = (i64)k * 64 + __builtin_ctzll(l2[k]);
+                const i64 w0 = w1 * 64 + __builtin_ctzll(l1[w1]);
+                return w0 * 64 + __builtin_ctzll(l0[w0]);
+            }
+        return -1;
+    }
+};
+
+// S2: first pass of the RS colouring.  The undecided points sit in one IndexSet per weight lambda; the next
+// C-point is the lowest index of the highest non-empty weight (lambda desc, index asc), a weight change moves
+// a point to the next set.
 void colour(const HostCsr& A, const std::vector<uint8_t>& strong, std::vector<int8_t>& cf) {
     const i64 n = A.nrows;
     // transpose lists of the strength graph: who strongly depends on i
@@ -78,31 +110,39 @@ void colour(const HostCsr& A, const std::vector<uint8_t>& strong, std::vector<in
     }
     std::vector<i32> weight(n);
     cf.assign(n, 0);
-    auto key = [](i32 w, i32 idx) { return ((uint64_t)(uint32_t)w << 32) | (uint64_t)(0xFFFFFFFFu - (uint32_t)idx); };
-    std::vector<uint64_t> init;
-    init.reserve(n);
+    std::vector<std::unique_ptr<IndexSet>> bucket;
+    auto set_of = [&](i32 w) -> IndexSet& {
+        if ((size_t)w >= bucket.size()) bucket.resize((size_t)w + 1);
+        if (!bucket[w]) bucket[w].reset(new IndexSet(n));
+        return *bucket[w];
+    };
+    i32 maxw = 0;
     for (i64 i = 0; i < n; ++i) {
         weight[i] = (i32)(tp[i + 1] - tp[i]);
         bool has_strong = false;
         for (i64 k = A.rp[i]; k < A.rp[i + 1] && !has_strong; ++k) has_strong = strong[k];
         if (!has_strong && weight[i] == 0) cf[i] = -1;
-        else init.push_back(key(weight[i], (i32)i));
+        else { set_of(weight[i]).insert(i); maxw = std::max(maxw, weight[i]); }
     }
-    std::priority_queue<uint64_t> heap(std::less<uint64_t>(), std::move(init));
-    while (!heap.empty()) {
-        const uint64_t top = heap.top();
-        heap.pop();
-        const i32 i = (i32)(0xFFFFFFFFu - (uint32_t)(top & 0xFFFFFFFFu));
-        if (cf[i] != 0 || (i32)(top >> 32) != weight[i]) continue;      // stale entry
+    for (;;) {
+        while (maxw >= 0 && ((size_t)maxw >= bucket.size() || !bucket[maxw] || bucket[maxw]->count == 0)) --maxw;
+        if (maxw < 0) break;
+        const i32 i = (i32)bucket[maxw]->lowest();
+        bucket[maxw]->erase(i);
         cf[i] = 1;
         for (i64 a = tp[i]; a < tp[i + 1]; ++a) {
             const i32 j = tl[a];
             if (cf[j] != 0) continue;
             cf[j] = -1;
+            bucket[weight[j]]->erase(j);
             for (i64 k = A.rp[j]; k < A.rp[j + 1]; ++k) {
                 if (!strong[k]) continue;
                 const i32 m = A.ci[k];
-                if (cf[m] == 0) heap.push(key(++weight[m], m));
+                if (cf[m] == 0) {
+                    bucket[weight[m]]->erase(m);
+                    set_of(++weight[m]).insert(m);
+                    maxw = std::max(maxw, weight[m]);
+                }
             }
         }
     }
@@ -255,6 +295,9 @@ bool factor_dense(const HostCsr& A, std::vector<double>& lu, std::vector<i32>& r
 
 int build_hierarchy(HostCsr&& A0, double theta, int max_levels, int coarse_max, int nthreads, Hierarchy& H,
                     std::string& detail) {
+    typedef std::chrono::steady_clock Clock;
+    const char* tenv = std::getenv("AMGDD_SETUP_TIMING");                        // 1: stage times per level on stderr
+    const bool timing = tenv && tenv[0] == '1';
     H.lv.clear();
     H.lv.emplace_back();
     H.lv[0].A = std::move(A0);
@@ -264,18 +307,29 @@ int build_hierarchy(HostCsr&& A0, double theta, int max_levels, int coarse_max, 
         l1_diagonal(cur.A, nthreads, cur.dinv);
         const i64 n = cur.A.nrows;
         if (n <= coarse_max || l + 1 >= max_levels) break;                       // S5
+        const auto t0 = Clock::now();
         std::vector<uint8_t> strong;
         strength_flags(cur.A, theta, nthreads, strong);
+        const auto t1 = Clock::now();
         std::vector<int8_t> cf;
         colour(cur.A, strong, cf);
+        const auto t2 = Clock::now();
         i64 nc = 0;
         for (i64 i = 0; i < n; ++i) nc += cf[i] > 0;
         if (nc == 0 || nc == n) break;                                           // S5
         cur.cf = std::move(cf);
         interpolation(cur.A, strong, cur.cf, nthreads, cur.coarse_of, cur.P);
+        const auto t3 = Clock::now();
         transpose_csr(cur.P, cur.R);
+        const auto t4 = Clock::now();
         HostCsr Ac;
         galerkin_rap(cur.R, cur.A, cur.P, nthreads, Ac);
+        if (timing) {
+            const auto t5 = Clock::now();
+            auto sec = [](Clock::time_point a, Clock::time_point b) { return std::chrono::duration<double>(b - a).count(); };
+            std::fprintf(stderr, "amgdd setup: level %d n %lld nnz %lld: strength %.3f colour %.3f interpolation %.3f transpose %.3f rap %.3f s\n",
+                         l, (long long)n, (long long)cur.A.nnz(), sec(t0, t1), sec(t1, t2), sec(t2, t3), sec(t3, t4), sec(t4, t5));
+        }
         H.lv.emplace_back();
         H.lv[l + 1].A = std::move(Ac);
         ++l;
