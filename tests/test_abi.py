@@ -112,3 +112,31 @@ def test_product_does_not_import_the_oracle():
             txt = open(os.path.join(ROOT, "oracle", f)).read()
             assert "paper_1906_10575_b200 import" not in txt and "import paper_1906_10575_b200" not in txt, f
             assert not re.search(r'#include\s+"[^"]*(csrc|amgdd\.h)', txt), f
+
+
+def test_stats_struct_layout_matches_the_header(tmp_path):
+    """The ctypes mirror of amgdd_stats_t / amgdd_way_t has the size and field offsets the C compiler gives the
+    header's structs (a silent mismatch would corrupt memory in amgdd_get_stats)."""
+    import shutil
+    import subprocess
+    import paper_1906_10575_b200 as m
+    gcc = shutil.which("gcc")
+    if gcc is None:
+        pytest.skip("no C compiler")
+    fields = [n for n, _ in m.AmgddStats._fields_]
+    src = ['#include <stdio.h>', '#include <stddef.h>', '#include "amgdd.h"', 'int main(void) {',
+           '  printf("%zu %zu\\n", sizeof(amgdd_stats_t), sizeof(amgdd_way_t));']
+    src += [f'  printf("{n} %zu\\n", offsetof(amgdd_stats_t, {n}));' for n in fields]
+    src += ['  return 0;', '}']
+    c = tmp_path / "layout.c"
+    c.write_text("\n".join(src))
+    exe = tmp_path / "layout"
+    subprocess.run([gcc, "-I", os.path.join(ROOT, "include"), str(c), "-o", str(exe)], check=True)
+    out = subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout.split("\n")
+    size_stats, size_way = map(int, out[0].split())
+    assert size_stats == ctypes.sizeof(m.AmgddStats)
+    assert size_way == m.WAY_DTYPE.itemsize
+    for line in out[1:]:
+        if line:
+            name, off = line.split()
+            assert getattr(m.AmgddStats, name).offset == int(off), name
