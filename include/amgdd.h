@@ -44,8 +44,8 @@ typedef enum amgdd_status {
                                             max_levels < 1, coarse_max < 1, num_fac_cycles < 1, relax_sweeps < 1,
                                             num_cycles < 0, level / subdomain index out of range */
     AMGDD_ERR_BAD_CSR = -2,              /* rowptr[0] != 0 or not monotone, column out of range, columns not strictly
-                                            ascending in a row, missing or non-positive diagonal, structurally
-                                            unsymmetric pattern */
+                                            ascending in a row, missing or non-positive diagonal, a non-finite value,
+                                            structurally unsymmetric pattern */
     AMGDD_ERR_BAD_OWNER = -3,            /* owner value outside [0,P) or a subdomain that owns no dof */
     AMGDD_ERR_COARSE_TOO_LARGE = -4,     /* coarsening stopped (max_levels or stagnation) with n_L > 4096 */
     AMGDD_ERR_SINGULAR_COARSE = -5,      /* zero pivot in the dense LU of A_L */
@@ -124,12 +124,18 @@ int amgdd_setup(int64_t n, const int64_t* rowptr, const int32_t* colind, const d
 
 /* amgdd_solve -- num_cycles AMG-DD cycles (Alg. 2 with Alg. 4 inside).
  *   b, x          DEVICE, n doubles.  x is in/out: initial guess on entry, iterate on return.
- *   num_cycles    >= 0 (0 only evaluates resnorm[0])
+ *   num_cycles    0 .. 1023 (0 only evaluates resnorm[0]; the norms of one call live in a fixed device buffer of
+ *                 1024 doubles: AMGDD_ERR_BAD_ARG beyond that -- call again to continue, x carries the state)
  *   num_fac_cycles  AlgFAC iterations per cycle (>= 1; Fig. 10)
  *   relax_sweeps  nu: l1-Jacobi sweeps before and after each coarse correction (>= 1; V(nu,nu))
  *   resnorm_host  HOST, num_cycles+1 doubles or NULL.  resnorm[k] = || b - A_0 x_k ||_2, k = 0 is
  *                 the initial guess.  With NULL the call only enqueues work on the handle's
- *                 stream and returns; otherwise it synchronises the stream before returning. */
+ *                 stream and returns (and the norm of the final iterate is not evaluated);
+ *                 otherwise it synchronises the stream before returning.
+ * Limits: the steps of one subdomain's cycle form a static program of at most 1024 steps, about
+ * num_fac_cycles * (L * (4 + 2 * relax_sweeps) + 1) (twice the relaxation steps with the CF smoother), and the
+ * kernel's tables hold at most 85 levels (L <= 84): AMGDD_ERR_BAD_ARG with the step count in the detail string
+ * otherwise.  The call runs on the device the handle was set up on, whatever the caller's current device is. */
 int amgdd_solve(amgdd_handle_t h, const double* b, double* x, int32_t num_cycles,
                 int32_t num_fac_cycles, int32_t relax_sweeps, double* resnorm_host);
 
@@ -180,7 +186,9 @@ int amgdd_get_cf(amgdd_handle_t h, int32_t l, int8_t* cf_host);
 int amgdd_get_level_matrix(amgdd_handle_t h, int32_t l, int32_t which, int64_t* rowptr, int32_t* colind,
                            double* vals);
 int amgdd_composite_size(amgdd_handle_t h, int32_t p, int32_t l, int64_t* n_real, int64_t* n_ghost);
-/* real_gid: |D_l^p| global indices, ascending; ghost_gid: |D-bar_l^p \ D_l^p|, ascending (S7). */
+/* real_gid: |D_l^p| global indices, ascending; ghost_gid: |D-bar_l^p \ D_l^p|, ascending (S7).  On a level that the
+ * subdomain covers completely (D_l^p = Omega_l, always true on L; reading A5) real_gid is 0 .. n_l - 1, there are
+ * no ghost points (amgdd_composite_size reports n_ghost = 0) and ghost_gid is not written. */
 int amgdd_get_composite(amgdd_handle_t h, int32_t p, int32_t l, int32_t* real_gid, int32_t* ghost_gid);
 int amgdd_get_stats(amgdd_handle_t h, amgdd_stats_t* s);
 

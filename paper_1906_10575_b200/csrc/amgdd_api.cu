@@ -81,6 +81,7 @@ struct amgdd_handle_s {
     double* d_partial = nullptr; int partial_cap = 0;
     double* d_norms = nullptr; int norms_cap = 0;
     double* d_b_stage = nullptr; double* d_x_stage = nullptr;   // for amgdd_solve_host
+    std::vector<cudaEvent_t> events;                            // phase timers of amgdd_solve, created once and reused
     amgdd_stats_t stats;
     double prof_ms[4] = {0, 0, 0, 0};
     long long prof_launches[3] = {0, 0, 0};
@@ -135,6 +136,7 @@ double avg_row(const HostCsr& M) { return M.nrows ? (double)M.nnz() / (double)M.
 void free_handle(amgdd_handle_s* h) {
     if (!h) return;
     for (void* p : h->allocs) cudaFree(p);
+    for (cudaEvent_t e : h->events) cudaEventDestroy(e);
     delete h;
 }
 
@@ -196,10 +198,8 @@ int build_composites(amgdd_handle_s* h, const std::vector<i32>& owner, int nthre
     const int dev = h->device;
     const int nw = std::max(1, std::min(nthreads, P));
     std::atomic<int> next(0);
-    std::vector<std::thread> pool;
-    for (int t = 0; t < nw; ++t)
-        pool.emplace_back([&, t]() {
-            (void)t;
+    run_threads(nw, [&](int) {
+        try {
             if (cudaSetDevice(dev) != cudaSuccess) { fail(AMGDD_ERR_CUDA, "cudaSetDevice failed in a setup worker"); return; }
             cudaStream_t st;
             if (cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking) != cudaSuccess) { fail(AMGDD_ERR_CUDA, "stream create failed"); return; }
@@ -251,8 +251,9 @@ int build_composites(amgdd_handle_s* h, const std::vector<i32>& owner, int nthre
             cudaStreamSynchronize(st);
             if (stage) cudaFreeHost(stage);
             cudaStreamDestroy(st);
-        });
-    for (auto& th : pool) th.join();
+        } catch (const std::bad_alloc&) { fail(AMGDD_ERR_OUT_OF_MEMORY, "host allocation failed in a setup worker"); }
+        catch (const std::exception& e) { fail(AMGDD_ERR_OUT_OF_MEMORY, std::string("setup worker failed: ") + e.what()); }
+    });
     if (status.load() != AMGDD_SUCCESS) { g_detail = fail_detail; return status.load(); }
     return AMGDD_SUCCESS;
 }
@@ -355,6 +356,7 @@ int build_composites_device(amgdd_handle_s* h, const std::vector<i32>& owner, in
         std::string fail_detail;
         std::mutex fail_mu;
         auto work = [&](int t) {
+          try {
             if (!builders[t]) builders[t].reset(new CompositeBuilder(h->H, owner, owned, h->eta, h->nghost, h->window));
             CompositeBuilder& cb = *builders[t];
             std::vector<i32> own;
@@ -377,13 +379,12 @@ int build_composites_device(amgdd_handle_s* h, const std::vector<i32>& owner, in
                     out.insert(out.end(), cb.ghost(l).begin(), cb.ghost(l).end());
                 }
             }
+          } catch (const std::exception& e) {                              // bad_alloc of the per-thread maps / lists: report, do not terminate
+              std::lock_guard<std::mutex> g(fail_mu);
+              if (status.load() == AMGDD_SUCCESS) { status.store(AMGDD_ERR_OUT_OF_MEMORY); fail_detail = std::string("host allocation failed while growing the index sets: ") + e.what(); }
+          }
         };
-        {
-            std::vector<std::thread> pool;
-            for (int t = 1; t < nw; ++t) pool.emplace_back(work, t);
-            work(0);
-            for (auto& th : pool) th.join();
-        }
+        run_threads(nw, work);
         if (status.load() != AMGDD_SUCCESS) { g_detail = fail_detail; return status.load(); }
         auto t1 = std::chrono::steady_clock::now();
         t_sets += std::chrono::duration<double>(t1 - t0).count();
@@ -545,16 +546,18 @@ void traffic_model(amgdd_handle_s* h) {
             const double rc = Arc + 16 * nbc + 16 * nrc;
             const double ip = Pm + 8 * nbc + 16 * nb;
             const double post = Ar + 8 * nb + 40 * nr;
-            model[0] += pre + at + rs + ip + post;
+            model[0] += 32 * nr + at + rs + ip + post;             // first iteration: u_l = 0 on every level, the first sweep needs no matrix (a4)
             model[1] += pre + at + rs + rc + ip + post;
             const StreamLayout& A = layA(l);
             const double a_real = (double)A.bytes_real;
             const double a_all = (double)A.bytes;
             const StreamLayout& Ac = layA(l + 1);
             const double ac_real = (double)Ac.bytes_real;
-            const double common = (l == 0 ? a_real : 0.0) + a_all + (double)layR(l).bytes + (double)layP(l).bytes + a_real;
+            // pre-relaxation: matrix-free on every level in the first iteration (u = 0: OPK_FIRST0 on level 0, fused into the
+            // restriction on l >= 1); in later iterations level 0 runs a real sweep over A_0's real rows
+            const double common = a_all + (double)layR(l).bytes + (double)layP(l).bytes + a_real;
             stream[0] += common;
-            stream[1] += common + ac_real;
+            stream[1] += common + (l == 0 ? a_real : 0.0) + ac_real;
         }
     }
     s.model_bytes_fac_iter[0] = model[0]; s.model_bytes_fac_iter[1] = model[1];
@@ -732,6 +735,21 @@ bool bad_handle(amgdd_handle_t h) {
     return false;
 }
 
+// every compute entry runs on the device the handle was set up on, whatever the caller's current device is
+// (the handle's pointers and the kernels' attributes belong to that device); the caller's device is restored
+struct DeviceScope {
+    int prev = -1;
+    bool ok = true;
+    explicit DeviceScope(int dev) {
+        if (cudaGetDevice(&prev) != cudaSuccess) { ok = false; return; }
+        if (prev != dev && cudaSetDevice(dev) != cudaSuccess) ok = false;
+    }
+    ~DeviceScope() { int cur = -1; if (prev >= 0 && cudaGetDevice(&cur) == cudaSuccess && cur != prev) cudaSetDevice(prev); }
+};
+#define DEVICE_SCOPE(h)                                                                       \
+    DeviceScope dev_scope__((h)->device);                                                     \
+    if (!dev_scope__.ok) { g_detail = "cannot select the handle's device"; cudaGetLastError(); return AMGDD_ERR_CUDA; }
+
 }  // namespace
 
 extern "C" {
@@ -820,6 +838,14 @@ int amgdd_setup(int64_t n, const int64_t* rowptr, const int32_t* colind, const d
         free_handle(h);
         g_detail = "host allocation failed during setup";
         return AMGDD_ERR_OUT_OF_MEMORY;
+    } catch (const std::exception& e) {                                  // length_error, system_error (thread creation), ...
+        free_handle(h);
+        g_detail = std::string("setup failed: ") + e.what();
+        return AMGDD_ERR_OUT_OF_MEMORY;
+    } catch (...) {
+        free_handle(h);
+        g_detail = "setup failed with an unknown exception";
+        return AMGDD_ERR_OUT_OF_MEMORY;
     }
     *out = h;
     return AMGDD_SUCCESS;
@@ -867,15 +893,21 @@ int amgdd_solve(amgdd_handle_t h, const double* b, double* x, int32_t num_cycles
         g_detail = "need b, x non-null, 0 <= num_cycles < 1024, num_fac_cycles >= 1, relax_sweeps >= 1";
         return AMGDD_ERR_BAD_ARG;
     }
+    DEVICE_SCOPE(h);
     const int L = h->H.L;
     const bool timed = resnorm_host != nullptr;
-    std::vector<cudaEvent_t> ev;
+    std::vector<cudaEvent_t>& ev = h->events;                   // owned by the handle: nothing to release on an early return
+    size_t nev = 0;
+    if (timed) {
+        const size_t want = 3 * (size_t)num_cycles + 2;
+        while (ev.size() < want) {
+            cudaEvent_t e;
+            CUDA_TRY(cudaEventCreate(&e));
+            ev.push_back(e);
+        }
+    }
     auto mark = [&]() {
-        if (!timed) return;
-        cudaEvent_t e;
-        cudaEventCreate(&e);
-        cudaEventRecord(e, h->stream);
-        ev.push_back(e);
+        if (timed) cudaEventRecord(ev[nev++], h->stream);
     };
     if (h->prog_nfac != num_fac_cycles || h->prog_nu != relax_sweeps || h->prog_smoother != h->smoother) {       // (re)build the program of one subdomain
         const int nops = fac_build_program(L, num_fac_cycles, relax_sweeps, h->smoother, nullptr);
@@ -936,8 +968,10 @@ int amgdd_solve(amgdd_handle_t h, const double* b, double* x, int32_t num_cycles
         launches[2] += 1;
         mark();
     }
-    enqueue_residual(h, b, x, nullptr, num_cycles);
-    launches[0] += 2;
+    if (timed) {                                                                    // ||b - A x|| of the final iterate; nobody can read it
+        enqueue_residual(h, b, x, nullptr, num_cycles);                             // in an asynchronous call (resnorm_host = NULL)
+        launches[0] += 2;
+    }
     mark();
     CUDA_TRY(cudaGetLastError());
     if (timed) {
@@ -953,12 +987,11 @@ int amgdd_solve(amgdd_handle_t h, const double* b, double* x, int32_t num_cycles
         }
         float last = 0, tot = 0;
         cudaEventElapsedTime(&last, ev[3 * num_cycles], ev[3 * num_cycles + 1]);
-        cudaEventElapsedTime(&tot, ev.front(), ev.back());
+        cudaEventElapsedTime(&tot, ev[0], ev[nev - 1]);
         ms[0] += last; ms[3] = tot;
         for (int i = 0; i < 4; ++i) h->prof_ms[i] = ms[i];
-        for (int i = 0; i < 3; ++i) h->prof_launches[i] = launches[i];
-        for (cudaEvent_t e : ev) cudaEventDestroy(e);
     }
+    for (int i = 0; i < 3; ++i) h->prof_launches[i] = launches[i];
     return AMGDD_SUCCESS;
 }
 
@@ -966,10 +999,13 @@ int amgdd_solve_host(amgdd_handle_t h, const double* b_host, double* x_host, int
                      int32_t num_fac_cycles, int32_t relax_sweeps, double* resnorm_host) {
     if (bad_handle(h)) return AMGDD_ERR_BAD_ARG;
     if (!b_host || !x_host) { g_detail = "null host vector"; return AMGDD_ERR_BAD_ARG; }
+    DEVICE_SCOPE(h);
     int rc;
-    if (!h->d_b_stage) {
-        if ((rc = dev_alloc(h, (void**)&h->d_b_stage, (size_t)h->n * sizeof(double)))) return rc;
-        if ((rc = dev_alloc(h, (void**)&h->d_x_stage, (size_t)h->n * sizeof(double)))) return rc;
+    if (!h->d_b_stage || !h->d_x_stage) {                        // both or neither: a failed second allocation leaves the handle usable
+        double *sb = nullptr, *sx = nullptr;
+        if ((rc = dev_alloc(h, (void**)&sb, (size_t)h->n * sizeof(double)))) return rc;
+        if ((rc = dev_alloc(h, (void**)&sx, (size_t)h->n * sizeof(double)))) return rc;    // (sb stays owned by the handle's allocation list)
+        h->d_b_stage = sb; h->d_x_stage = sx;
     }
     CUDA_TRY(cudaMemcpyAsync(h->d_b_stage, b_host, (size_t)h->n * sizeof(double), cudaMemcpyHostToDevice, h->stream));
     CUDA_TRY(cudaMemcpyAsync(h->d_x_stage, x_host, (size_t)h->n * sizeof(double), cudaMemcpyHostToDevice, h->stream));
@@ -983,6 +1019,7 @@ int amgdd_solve_host(amgdd_handle_t h, const double* b_host, double* x_host, int
 int amgdd_residual_norm(amgdd_handle_t h, const double* b, const double* x, double* out_host) {
     if (bad_handle(h)) return AMGDD_ERR_BAD_ARG;
     if (!b || !x || !out_host) { g_detail = "null pointer argument"; return AMGDD_ERR_BAD_ARG; }
+    DEVICE_SCOPE(h);
     enqueue_residual(h, b, x, nullptr, 0);
     CUDA_TRY(cudaGetLastError());
     CUDA_TRY(cudaMemcpyAsync(out_host, h->d_norms, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
@@ -1021,6 +1058,7 @@ int amgdd_vcycle(amgdd_handle_t h, const double* b, double* x, int32_t num_cycle
         g_detail = "need b, x non-null, 0 <= num_cycles < 1024, nu1, nu2 >= 0, nu1 + nu2 >= 1";
         return AMGDD_ERR_BAD_ARG;
     }
+    DEVICE_SCOPE(h);
     int rc = ensure_vcycle(h);
     if (rc) return rc;
     const int L = h->H.L;

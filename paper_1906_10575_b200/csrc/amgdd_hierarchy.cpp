@@ -26,6 +26,9 @@ int validate_csr(i64 n, const i64* rp, const i32* ci, const double* v, std::stri
         for (i64 k = rp[i]; k < rp[i + 1]; ++k) {
             if (ci[k] < 0 || ci[k] >= n) { detail = "column out of range in row " + std::to_string(i); return ST_BAD_CSR; }
             if (k > rp[i] && ci[k] <= ci[k - 1]) { detail = "columns not strictly ascending in row " + std::to_string(i); return ST_BAD_CSR; }
+            // the AlgFAC kernel streams the values unchecked (and orders its load bursts by an Inf/NaN test of data
+            // it has already received): non-finite input is refused here
+            if (!std::isfinite(v[k])) { detail = "non-finite value in row " + std::to_string(i); return ST_BAD_CSR; }
             if (ci[k] == i) {
                 diag = true;
                 if (!(v[k] > 0.0)) { detail = "non-positive diagonal in row " + std::to_string(i); return ST_BAD_CSR; }
@@ -198,7 +201,56 @@ void transpose_csr(const HostCsr& M, HostCsr& T) {
         }
 }
 
-// Galerkin triple product C = R A P in one pass per coarse row, every structural entry kept,
+// C = X * Y with every structural entry kept, columns ascending; threaded symbolic + numeric phases.  Entry (i,c)
+// accumulates x_ij * y_jc with j ascending: one fixed order, independent of the thread count.
+void spgemm(const HostCsr& X, const HostCsr& Y, int nthreads, HostCsr& C) {
+    const i64 n = X.nrows, m = Y.ncols;
+    C.nrows = n; C.ncols = m;
+    C.rp.assign(n + 1, 0);
+    std::vector<std::vector<i32>> mark(nthreads);
+    std::vector<std::vector<double>> acc(nthreads);
+    std::vector<std::vector<i32>> cols(nthreads);
+    for (int t = 0; t < nthreads; ++t) mark[t].assign(m, -1);
+    parallel_for(n, nthreads, 2048, [&](int t, i64 i) {
+        std::vector<i32>& mk = mark[t];
+        i64 cnt = 0;
+        for (i64 a = X.rp[i]; a < X.rp[i + 1]; ++a) {
+            const i32 j = X.ci[a];
+            for (i64 b = Y.rp[j]; b < Y.rp[j + 1]; ++b)
+                if (mk[Y.ci[b]] != (i32)i) { mk[Y.ci[b]] = (i32)i; ++cnt; }
+        }
+        C.rp[i + 1] = cnt;
+    });
+    for (i64 i = 0; i < n; ++i) C.rp[i + 1] += C.rp[i];
+    C.ci.resize((size_t)C.rp[n]);
+    C.v.resize((size_t)C.rp[n]);
+    for (int t = 0; t < nthreads; ++t) { mark[t].assign(m, -1); acc[t].assign(m, 0.0); }
+    parallel_for(n, nthreads, 2048, [&](int t, i64 i) {
+        std::vector<i32>& mk = mark[t];
+        std::vector<double>& ac = acc[t];
+        std::vector<i32>& cl = cols[t];
+        cl.clear();
+        for (i64 a = X.rp[i]; a < X.rp[i + 1]; ++a) {
+            const i32 j = X.ci[a];
+            const double xv = X.v[a];
+            for (i64 b = Y.rp[j]; b < Y.rp[j + 1]; ++b) {
+                const i32 c = Y.ci[b];
+                if (mk[c] != (i32)i) { mk[c] = (i32)i; cl.push_back(c); ac[c] = xv * Y.v[b]; }
+                else ac[c] += xv * Y.v[b];
+            }
+        }
+        std::sort(cl.begin(), cl.end());
+        i64 q = C.rp[i];
+        for (i32 c : cl) { C.ci[q] = c; C.v[q] = ac[c]; ++q; }
+    });
+}
+
+// Galerkin operator A_{l+1} = R_l A_l P_l (reading S4: every structural entry kept, the terms of an entry
+// summed "in any order").  DEFAULT: two sparse products, R (A P): entry (I,J) = sum_i r_Ii (sum_j a_ij p_jJ), an
+// association and a rounding of its own (it is NOT the order of the oracle's triple loop, so parity is shown with
+// coarse operators that differ from the oracle's in the last bits).  AMGDD_GALERKIN=fused selects the one-pass
+// triple product below, whose terms (r_Ii a_ij) p_jJ are added with i, then j, then J ascending.
+// Fused variant: Galerkin triple product C = R A P in one pass per coarse row, every structural entry kept,
 // columns ascending; threaded symbolic + numeric phases.  Entry (I,J) accumulates the terms
 // (r_Ii * a_ij) * p_jJ with i, then j, then J ascending, a fixed order, so the coarse operators
 // do not depend on the thread count.
@@ -298,6 +350,8 @@ int build_hierarchy(HostCsr&& A0, double theta, int max_levels, int coarse_max, 
     typedef std::chrono::steady_clock Clock;
     const char* tenv = std::getenv("AMGDD_SETUP_TIMING");                        // 1: stage times per level on stderr
     const bool timing = tenv && tenv[0] == '1';
+    const char* genv = std::getenv("AMGDD_GALERKIN");                            // "fused": one-pass triple product (see galerkin_rap)
+    const bool fused_rap = genv && std::string(genv) == "fused";
     H.lv.clear();
     H.lv.emplace_back();
     H.lv[0].A = std::move(A0);
@@ -323,13 +377,20 @@ int build_hierarchy(HostCsr&& A0, double theta, int max_levels, int coarse_max, 
         transpose_csr(cur.P, cur.R);
         const auto t4 = Clock::now();
         HostCsr Ac;
-        galerkin_rap(cur.R, cur.A, cur.P, nthreads, Ac);
+        if (fused_rap) galerkin_rap(cur.R, cur.A, cur.P, nthreads, Ac);
+        else {
+            HostCsr AP;
+            spgemm(cur.A, cur.P, nthreads, AP);
+            spgemm(cur.R, AP, nthreads, Ac);
+        }
         if (timing) {
             const auto t5 = Clock::now();
             auto sec = [](Clock::time_point a, Clock::time_point b) { return std::chrono::duration<double>(b - a).count(); };
             std::fprintf(stderr, "amgdd setup: level %d n %lld nnz %lld: strength %.3f colour %.3f interpolation %.3f transpose %.3f rap %.3f s\n",
                          l, (long long)n, (long long)cur.A.nnz(), sec(t0, t1), sec(t1, t2), sec(t2, t3), sec(t3, t4), sec(t4, t5));
         }
+        for (double a : Ac.v)
+            if (!std::isfinite(a)) { detail = "the Galerkin operator of level " + std::to_string(l + 1) + " has a non-finite entry"; return ST_BAD_CSR; }
         H.lv.emplace_back();
         H.lv[l + 1].A = std::move(Ac);
         ++l;

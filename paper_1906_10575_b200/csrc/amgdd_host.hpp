@@ -3,7 +3,9 @@
 #pragma once
 #include <atomic>
 #include <cstdint>
+#include <exception>
 #include <functional>
+#include <mutex>
 #include <string>
 #include <thread>
 #include <vector>
@@ -53,6 +55,28 @@ inline int default_threads() {
     return (int)(h > 64 ? 64 : h);
 }
 
+// Runs body(t) on nthreads threads (t = 0 on the calling thread) and joins them.  An exception thrown by any
+// body (std::bad_alloc from the scratch vectors, std::system_error from thread creation) is caught on its thread;
+// the first one is re-thrown on the CALLING thread after all threads have joined, so that nothing can reach
+// std::terminate and amgdd_setup can turn it into an error code (no exception crosses the C ABI).
+template <class F>
+void run_threads(int nthreads, F&& body) {
+    std::exception_ptr first;
+    std::mutex mu;
+    auto guarded = [&](int t) {
+        try { body(t); }
+        catch (...) { std::lock_guard<std::mutex> g(mu); if (!first) first = std::current_exception(); }
+    };
+    std::vector<std::thread> th;
+    try {
+        th.reserve(nthreads > 1 ? nthreads - 1 : 0);
+        for (int t = 1; t < nthreads; ++t) th.emplace_back(guarded, t);
+    } catch (...) { std::lock_guard<std::mutex> g(mu); if (!first) first = std::current_exception(); }
+    guarded(0);
+    for (auto& x : th) x.join();
+    if (first) std::rethrow_exception(first);
+}
+
 template <class F>
 void parallel_for(i64 n, int nthreads, i64 chunk, F&& fn) {
     if (nthreads <= 1 || n <= chunk) {
@@ -60,18 +84,17 @@ void parallel_for(i64 n, int nthreads, i64 chunk, F&& fn) {
         return;
     }
     std::atomic<i64> next(0);
-    std::vector<std::thread> th;
-    th.reserve(nthreads);
-    for (int t = 0; t < nthreads; ++t)
-        th.emplace_back([&, t]() {
+    std::atomic<bool> stop(false);
+    run_threads(nthreads, [&](int t) {
+        try {
             for (;;) {
                 const i64 b = next.fetch_add(chunk);
-                if (b >= n) break;
+                if (b >= n || stop.load(std::memory_order_relaxed)) break;
                 const i64 e = b + chunk < n ? b + chunk : n;
                 for (i64 i = b; i < e; ++i) fn(t, i);
             }
-        });
-    for (auto& x : th) x.join();
+        } catch (...) { stop.store(true); throw; }
+    });
 }
 
 // ---- composite grids (S6, S7) --------------------------------------------------------------

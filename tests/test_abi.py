@@ -74,7 +74,9 @@ def test_argument_validation_precedes_device_use():
     # drop one off-diagonal entry -> structurally unsymmetric
     keep = np.ones(p.nnz, dtype=bool); keep[p.rowptr[0] + 1] = False
     rp_u = np.concatenate([[0], np.cumsum(np.add.reduceat(keep.astype(np.int64), p.rowptr[:-1]))])
-    for kw in [dict(rowptr=rp), dict(colind=ci), dict(vals=v_neg), dict(colind=ci_oob),
+    v_nan = p.vals.copy(); v_nan[p.rowptr[7] + 1] = np.nan         # a non-finite off-diagonal (the diagonal test alone misses it)
+    v_inf = p.vals.copy(); v_inf[p.rowptr[3]] = -np.inf
+    for kw in [dict(rowptr=rp), dict(colind=ci), dict(vals=v_neg), dict(colind=ci_oob), dict(vals=v_nan), dict(vals=v_inf),
                dict(rowptr=rp_u, colind=p.colind[keep], vals=p.vals[keep])]:
         with pytest.raises(m.AmgddError) as e:
             _setup(m, p, **kw)

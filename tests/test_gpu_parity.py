@@ -254,6 +254,37 @@ def test_single_level_hierarchy_is_a_direct_solve():
     assert res[1] <= 1e-13 * res[0]
 
 
+def test_coarse_solve_with_row_exchanges():
+    """Alg. 4 P:514 with a coarsest operator whose LU needs row exchanges (tiny diagonal, O(1) off-diagonals):
+    the library's rowperm path (factor_dense, the permuted load of `coarse`) against numpy.linalg.solve and the oracle.
+    coarse_max >= n, so L = 0 and one cycle is the direct solve (reading A5)."""
+    torch = _torch()
+    import paper_1906_10575_b200 as m
+    rp, ci, v, dense = wl.pivoting_band_matrix()
+    n = dense.shape[0]
+    owner = (np.arange(n) * 3 // n).astype(np.int32)
+    h = m.amgdd_setup(n, rp, ci, v, 3, owner, 1, 1, 25, 0.25, n)
+    assert m.amgdd_num_levels(h) == 1
+    o = Oracle(n, rp, ci, v, 0.25, 25, n)
+    o.set_partition(3, owner, 1, 1)
+    bh = wl.rhs(9, n)
+    b = torch.from_numpy(bh).cuda()
+    x = torch.zeros(n, dtype=torch.float64, device="cuda")
+    res = m.amgdd_solve(h, b, x, 1, 2, 1)
+    sol = np.linalg.solve(dense, bh)
+    xo = np.zeros(n)
+    o.cycle(bh, xo, 2, 1)
+    xg = x.cpu().numpy()
+    assert np.abs(xg - sol).max() <= 1e-11 * np.abs(sol).max()
+    assert np.abs(xg - xo).max() <= 1e-11 * np.abs(xo).max()
+    assert res[1] <= 1e-10 * res[0]
+    # the same through the V-cycle entry (Alg. 1 with L = 0: launch_coarse_solve)
+    xv = torch.zeros(n, dtype=torch.float64, device="cuda")
+    m.amgdd_vcycle(h, b, xv, 1, 1, 1)
+    assert np.abs(xv.cpu().numpy() - sol).max() <= 1e-11 * np.abs(sol).max()
+    m.amgdd_destroy(h)
+
+
 def test_zero_cycles_only_reports_the_norm():
     torch = _torch()
     p = wl.make_config(1)

@@ -473,6 +473,77 @@ def test_relax_mask_only_touches_real_points():
 
 
 # ------------------------------------------------------------------------------------------
+# Alg. 2 with several subdomains: the owned-correction update
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("cfg,scale,parts,eta,nfac,nu", [(1, None, 2, 1, 2, 1), (1, 21, 3, 2, 1, 2), (2, 12, 2, 2, 2, 1),
+                                                         (4, 12, 2, 2, 2, 1), (5, 32, 2, 3, 2, 1)])
+def test_cycle_with_several_subdomains_is_the_patchwork_of_local_solves(cfg, scale, parts, eta, nfac, nu):
+    """Alg. 2 for P > 1, against a restatement that uses nothing of the oracle's cycle driver:
+    r = b - A_0 x (scipy); for every p the global V-cycles with relaxation masked to D_l^p (scipy, whole-level
+    vectors) give e^p; the new iterate is x + e^p ON Omega_0^p ONLY ("each processor updates only its owned dofs",
+    P:65).  Starts from a nonzero x so that the residual line P:471 matters, checks every dof, and checks
+    that a partial list of subdomains leaves every other dof bit-identical."""
+    p = wl.make_config(cfg, scale, parts_per_dim=parts)
+    assert p.num_subdomains > 1
+    o = make_oracle(p, eta=eta, coarse_max=min(p.coarse_max, 16))
+    As, Ps = hierarchy_from_oracle(o)
+    A = sp.csr_matrix((p.vals, p.colind, p.rowptr), shape=(p.n, p.n))
+    x0 = 0.1 * wl.rhs(77, p.n)
+    r0 = p.b - A @ x0
+    expect = x0.copy()
+    for q in range(p.num_subdomains):
+        e = masked_vcycles(As, Ps, _masks(o, q), r0, nfac, nu)
+        own = p.owner == q
+        expect[own] = x0[own] + e[own]
+    x = x0.copy()
+    o.cycle(p.b, x, nfac, nu)
+    tol = 1e-12 if cfg == 5 else 1e-13
+    assert np.abs(x - expect).max() <= tol * np.abs(expect).max()
+    # a subset of the subdomains: only their owned dofs move, the others keep their bits
+    some = np.array([0, p.num_subdomains - 1], dtype=np.int32)
+    x2 = x0.copy()
+    o.cycle(p.b, x2, nfac, nu, subdomains=some)
+    moved = np.isin(p.owner, some)
+    assert np.array_equal(x2[~moved], x0[~moved])
+    assert np.array_equal(x2[moved], x[moved])
+    # and the oracle's own per-subdomain routine composes to the same thing (the composition the GPU tests rely on)
+    x3 = x0.copy()
+    for q in range(p.num_subdomains):
+        real, _ = o.composite(q, 0)
+        u0 = o.fac_local(q, r0, nfac, nu)
+        own_local = p.owner[real] == q
+        x3[real[own_local]] += u0[:len(real)][own_local]
+    assert np.array_equal(x3, x)
+
+
+# ------------------------------------------------------------------------------------------
+# a8 with row exchanges (Alg. 4 P:514; "a direct method", P:49)
+# ------------------------------------------------------------------------------------------
+def test_dense_coarse_solve_with_row_exchanges():
+    rp, ci, v, dense = wl.pivoting_band_matrix()
+    n = dense.shape[0]
+    assert np.linalg.cond(dense) < 1e6
+    # partial pivoting must actually exchange rows here: scipy's LU of the same matrix is not the identity permutation
+    import scipy.linalg as sla
+    _, piv = sla.lu_factor(dense)
+    assert (piv != np.arange(n)).sum() >= n // 2
+    o = Oracle(n, rp, ci, v, 0.25, 25, n)                    # coarse_max >= n: L = 0, A_L = A_0 (S5)
+    assert o.num_levels == 1
+    for seed in (1, 2, 3):
+        rhs = wl.rhs(seed, n)
+        sol = np.linalg.solve(dense, rhs)
+        assert np.abs(o.coarse_solve(rhs) - sol).max() <= 1e-11 * np.abs(sol).max()
+    # through Alg. 2 / Alg. 4 with L = 0 (reading A5): one cycle is the direct solve, whatever the partition
+    owner = (np.arange(n) * 3 // n).astype(np.int32)
+    o.set_partition(3, owner, 1, 1)
+    b = wl.rhs(9, n)
+    x = np.zeros(n)
+    o.cycle(b, x, 1, 1)
+    sol = np.linalg.solve(dense, b)
+    assert np.abs(x - sol).max() <= 1e-11 * np.abs(sol).max()
+
+
+# ------------------------------------------------------------------------------------------
 # whole solve
 # ------------------------------------------------------------------------------------------
 def test_solve_converges_to_direct_solution():

@@ -320,3 +320,20 @@ def poisson1d(n):
     offs = [(-1,), (0,), (1,)]
     v = [-1.0, 2.0, -1.0]
     return _assemble((n,), offs, lambda k, ok: np.full(ok.shape, v[k]))
+
+
+def pivoting_band_matrix(n=24, seed=31):
+    """A test input for the dense coarse solve (Alg. 4): a symmetric-PATTERN pentadiagonal matrix with a tiny
+    positive diagonal and O(1) off-diagonals, so that Gaussian elimination with partial pivoting exchanges rows in
+    (almost) every column.  Returns (rowptr int64, colind int32, vals, dense array)."""
+    u = uniform(seed, 5 * n)
+    rowptr, colind, vals = [0], [], []
+    dense = np.zeros((n, n))
+    k = 0
+    for i in range(n):
+        for j in range(max(0, i - 2), min(n, i + 3)):
+            a = 1e-3 * (1.0 + u[k]) if i == j else (0.5 + u[k]) * (1.0 if (i + j) % 3 else -1.0)
+            colind.append(j); vals.append(a); dense[i, j] = a
+            k += 1
+        rowptr.append(len(colind))
+    return np.array(rowptr, dtype=np.int64), np.array(colind, dtype=np.int32), np.array(vals), dense
