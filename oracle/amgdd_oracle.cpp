@@ -657,15 +657,15 @@ int orc_set_partition(void* h, int nsub, const i32* owner, int eta, int num_ghos
 
 void orc_composite_size(void* h, int p, int l, i64* nr, i64* ng) {
     Oracle& o = *(Oracle*)h;
-    Scratch sc(o);
-    const Comp& c = get_comp(o, p, sc);
+    if (!o.comp[p]) { Scratch sc(o); get_comp(o, p, sc); }             // (the scratch arrays are of global size: only when the grid is not built yet)
+    const Comp& c = *o.comp[p];
     *nr = (i64)c.real[l].size(); *ng = (i64)c.ghost[l].size();
 }
 
 void orc_get_composite(void* h, int p, int l, i32* real, i32* ghost) {
     Oracle& o = *(Oracle*)h;
-    Scratch sc(o);
-    const Comp& c = get_comp(o, p, sc);
+    if (!o.comp[p]) { Scratch sc(o); get_comp(o, p, sc); }
+    const Comp& c = *o.comp[p];
     std::copy(c.real[l].begin(), c.real[l].end(), real);
     std::copy(c.ghost[l].begin(), c.ghost[l].end(), ghost);
 }

@@ -1,13 +1,17 @@
 """Parity of the CUDA path (through the C ABI) against the CPU oracle, on the same seeded inputs.
 
 Index work (levels, C/F splitting, sparsity patterns, composite index sets) is compared
-bit-exactly.  Floating point is compared with the bar of DESIGN.md §"Parity criterion":
-    | ||r_k||_gpu - ||r_k||_oracle |  <=  1e-10 * ||r_k||_oracle + phi_k  [+ 8 Y_k],
+bit-exactly.  Floating point is compared with the bar of DESIGN.md section 12 ("Parity criterion"):
+    | ||r_k||_gpu - ||r_k||_oracle |  <=  1e-10 * ||r_k||_oracle + phi_k  [+ YARD * Y_k],
     phi_k = 2^-52 * || |A_0| |x_k| + |b| ||_2          (fp64 rounding floor of a residual)
-    || x_gpu - x_oracle ||_inf  <=  1e-10 * || x_oracle ||_inf  [+ 8 ||x~_k - x_k||_inf]
+    || x_gpu - x_oracle ||_inf  <=  1e-10 * || x_oracle ||_inf  [+ YARD * ||x~_k - x_k||_inf]
 The bracketed yardstick terms are used only for config 5 (1e4 coefficient jumps x 1e3 anisotropy),
-where the ORACLE ITSELF moves by more than 1e-10 when A_0 is perturbed by one ulp: x~_k is the
-oracle's iterate on that perturbed matrix and Y_k = ||A_0 (x~_k - x_k)||_2.
+where the ORACLE ITSELF moves by about 1e-10 when A_0 is perturbed by one ulp: x~_k is the
+oracle's iterate on that perturbed matrix and Y_k = ||A_0 (x~_k - x_k)||_2.  YARD = 32: the library's
+coarse operators differ from the oracle's by the roundings of another Galerkin summation order on every
+level (reading S4), which moves the iterate 16-19 times as far as one ulp on A_0 does (measured table in
+DESIGN.md section 12); with the oracle's summation order (AMGDD_GALERKIN=fused) the yardstick terms are not
+needed in the first cycles.
 """
 import numpy as np
 import pytest
@@ -19,7 +23,7 @@ from oracle import Oracle, max_threads
 pytestmark = pytest.mark.gpu
 
 RTOL = 1e-10
-YARD = 8.0      # multiple of the oracle's own 1-ulp sensitivity allowed on ill-conditioned cases (config 5)
+YARD = 32.0     # multiple of the oracle's own 1-ulp sensitivity allowed on ill-conditioned cases (config 5); DESIGN.md section 12
 
 
 def _torch():
@@ -78,7 +82,7 @@ def ulp_perturbed_values(p):
     return p.vals * (1.0 + sgn * 2.0 ** -52)
 
 
-def run_parity(p, num_cycles, nfac=2, nu=1, yardstick=False, **kw):
+def run_parity(p, num_cycles, nfac=2, nu=1, yardstick=False, all_subdomains=False, **kw):
     """Trajectory parity: both sides start from x = 0 and run num_cycles AMG-DD cycles; after every
     cycle the residual norm and x are compared.  With yardstick=True the oracle is also run on the
     1-ulp-perturbed matrix; its own deviation (x~_k - x_k in the max norm, and Y_k = ||A_0 (x~_k - x_k)||_2
@@ -90,7 +94,7 @@ def run_parity(p, num_cycles, nfac=2, nu=1, yardstick=False, **kw):
     o = orc_setup(p, **kw)
     m.amgdd_set_smoother(h, smoother)
     o.set_smoother(smoother)
-    check_index_exact(m, h, o, p, range(p.num_subdomains) if p.num_subdomains <= 64 else
+    check_index_exact(m, h, o, p, range(p.num_subdomains) if p.num_subdomains <= 64 or all_subdomains else
                       np.linspace(0, p.num_subdomains - 1, 16).astype(int))
     b = torch.from_numpy(p.b).cuda()
     A = sp.csr_matrix((p.vals, p.colind, p.rowptr), shape=(p.n, p.n))
@@ -178,6 +182,41 @@ def test_vector_buffer_placements(env, monkeypatch):
         monkeypatch.setenv(k, v)
     run_parity(wl.make_config(4, 48), 3)
     run_parity(wl.make_config(2, 32), 2, nfac=2, nu=2)
+
+
+@pytest.mark.parametrize("galerkin", ["fused", "two-stage"])
+def test_galerkin_summation_orders(galerkin, monkeypatch):
+    """Reading S4: the terms of a Galerkin entry are summed "in any order".  The library's default is the two-stage
+    product R (A P); AMGDD_GALERKIN=fused is a one-pass triple product in the order of the oracle's loop nest.  Parity
+    must hold with both, i.e. also with coarse operators that differ from the oracle's in the last bits (checked
+    here: same pattern, values not identical with the two-stage product)."""
+    monkeypatch.setenv("AMGDD_GALERKIN", galerkin)
+    p = wl.make_config(4, 48)
+    m, h = lib_setup(p)
+    o = orc_setup(p)
+    differs = False
+    for l in range(1, o.num_levels):
+        rp, ci, v = m.amgdd_get_level_matrix(h, l, 0)
+        orp, oci, ov = o.matrix(l, "A")
+        assert np.array_equal(rp, orp) and np.array_equal(ci, oci)
+        assert np.abs(v - ov).max() <= 1e-13 * np.abs(ov).max()
+        differs = differs or not np.array_equal(v, ov)
+    m.amgdd_destroy(h)
+    assert differs == (galerkin == "two-stage")
+    # how far apart the coarse operators of the two sides are on the ill-conditioned config (DESIGN.md section 12)
+    p5 = wl.make_config(5, 256)
+    m, h = lib_setup(p5)
+    o5 = orc_setup(p5)
+    for l in range(1, o5.num_levels):
+        v, ov = m.amgdd_get_level_matrix(h, l, 0)[2], o5.matrix(l, "A")[2]
+        big = np.abs(ov) > 1e-6 * np.abs(ov).max()
+        ulps = np.abs(v - ov)[big] / (np.abs(ov)[big] * 2.0 ** -52)
+        print(f"{p5.name} A_{l} ({galerkin}): {int((v != ov).sum())} of {len(v)} entries differ, max {ulps.max():.1f} ulp, mean {ulps.mean():.2f} ulp")
+    m.amgdd_destroy(h)
+    run_parity(p, 4)
+    run_parity(wl.make_config(3, 32, eta=2), 3)
+    run_parity(wl.make_config(6, 192, eta=2, parts_per_dim=4), 3)
+    run_parity(wl.make_config(5, 256), 6, yardstick=True)
 
 
 def test_wide_column_indices():
