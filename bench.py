@@ -11,7 +11,7 @@ dofs (a3-a10).  Default workload: BASELINE.json configs[3] (3D variable-coeffici
   python bench.py [--gpus N] [--steps K] [--warmup W] [--config {1,2,3,4,5}] [--scale S] [--impl reference]
 
 One JSON line on stdout (rank 0).  With --impl reference the CPU oracle is timed instead (on a
-bounded sample of the same workload); see DESIGN.md §Measurement.
+bounded sample of the same workload); see DESIGN.md section 13 (Measurement).
 """
 from __future__ import annotations
 
@@ -111,25 +111,39 @@ def measured_peak():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+def kernel_source_hash():
+    """Identifies the AlgFAC kernel a committed ncu capture belongs to: sha256 over the kernel and the stream layout."""
+    import hashlib
+    hsh = hashlib.sha256()
+    for name in ("amgdd_fac.cu", "amgdd_stream.hpp"):
+        with open(os.path.join(ROOT, "paper_1906_10575_b200", "csrc", name), "rb") as f:
+            hsh.update(f.read())
+    return hsh.hexdigest()[:16]
+
+
 def ncu_traffic(workload):
-    """DRAM bytes per AlgFAC launch from the committed ncu --set full capture of this workload."""
+    """DRAM bytes per AlgFAC launch (dram__bytes_read.sum + dram__bytes_write.sum) from the committed
+    `ncu --set full` capture of this workload -- only if that capture was taken with the kernel source that is
+    running now (profiles/fac_kernel_traffic.json records the hash); otherwise None."""
     path = os.path.join(ROOT, "profiles", "fac_kernel_traffic.json")
-    if os.path.exists(path):
-        try:
-            d = json.load(open(path))
-            return d.get(workload)
-        except Exception:
+    try:
+        d = json.load(open(path))
+        if d.get("source_hash") != kernel_source_hash():
             return None
-    return None
+        return d.get("workloads", {}).get(workload)
+    except Exception:
+        return None
 
 
 # ---------------------------------------------------------------------------------------------
 # CPU oracle leg (cpu_baseline of the b200 arm, and the whole --impl reference arm)
 # ---------------------------------------------------------------------------------------------
-def oracle_time_per_cycle(p, sample, steps, warmup, smoother=0):
+def oracle_time_per_cycle(p, sample, steps, warmup, smoother=0, sample_1thread=None):
     """Times the oracle AS IT STANDS on a bounded sample: every step runs Alg. 2's global residual +
     restriction over the whole problem and AlgFAC on `sample` subdomains (spread evenly over the
-    partition); the per-cycle estimate scales the AlgFAC part by P / sample."""
+    partition); the per-cycle estimate scales the whole step by P / sample (the global part, which is run in
+    full, is a few percent of it, so the estimate is slightly high).  Timed with all host cores (one OpenMP
+    thread per core, `value`) and, on a smaller sample, with ONE thread (`value_1thread`)."""
     from oracle import Oracle, max_threads
     t0 = time.time()
     o = Oracle(p.n, p.rowptr, p.colind, p.vals, p.theta, p.max_levels, p.coarse_max)
@@ -140,24 +154,36 @@ def oracle_time_per_cycle(p, sample, steps, warmup, smoother=0):
     sample = max(1, min(sample, p.num_subdomains))
     subs = np.unique(np.linspace(0, p.num_subdomains - 1, sample).astype(np.int32))
     x = np.zeros(p.n)
+
+    def timed(sub_list, nt):
+        times = []
+        for _ in range(steps):
+            t = time.time()
+            o.cycle(p.b, x, p.num_fac_cycles, p.relax_sweeps, subdomains=sub_list, nthreads=nt)
+            times.append(time.time() - t)
+        return times
+
     for _ in range(max(1, warmup)):
         o.cycle(p.b, x, p.num_fac_cycles, p.relax_sweeps, subdomains=subs, nthreads=nthreads)   # also builds the composite grids (setup)
-    times = []
-    for _ in range(steps):
-        t = time.time()
-        o.cycle(p.b, x, p.num_fac_cycles, p.relax_sweeps, subdomains=subs, nthreads=nthreads)
-        times.append(time.time() - t)
-    t_sample = float(np.mean(times))
-    est_ms = 1e3 * t_sample * p.num_subdomains / len(subs)
+    t_all = timed(subs, nthreads)
+    n1 = max(1, min(len(subs), sample_1thread or max(1, len(subs) // 4)))
+    subs1 = subs[np.unique(np.linspace(0, len(subs) - 1, n1).astype(int))]
+    t_one = timed(subs1, 1)
+    est_ms = 1e3 * float(np.mean(t_all)) * p.num_subdomains / len(subs)
+    est1_ms = 1e3 * float(np.mean(t_one)) * p.num_subdomains / len(subs1)
     return {"value": est_ms, "unit": UNIT, "cores": nthreads, "kind": "oracle",
-            "sample": f"{len(subs)} of {p.num_subdomains} subdomains per step (AlgFAC part scaled by P/sample; "
-                      f"global residual+restriction run in full), {steps} steps, oracle setup {setup_s:.1f}s not timed",
-            "sample_seconds_per_step": t_sample}
+            "value_1thread": est1_ms,
+            "sample": f"all cores: {len(subs)} of {p.num_subdomains} subdomains per step, {steps} timed steps after {max(1, warmup)} "
+                      f"warm-up; one thread: {len(subs1)} subdomains per step, {steps} steps; each step also runs the global "
+                      f"residual+restriction in full; per-cycle value = mean step time x P/sample; oracle setup {setup_s:.1f}s not timed",
+            "sample_seconds_per_step": float(np.mean(t_all)), "sample_seconds_per_step_1thread": float(np.mean(t_one)),
+            "steps_timed": steps, "subdomains_all_cores": int(len(subs)), "subdomains_1thread": int(len(subs1))}
 
 
 def default_cpu_sample(p):
-    # about 10-30 s of CPU work in total: ~0.07 core-seconds per config-4 subdomain-cycle
-    return {1: 4, 2: 64, 3: 8, 4: 64, 5: 256}.get(int(p.name[3]), 32)
+    # about 20-30 s of CPU work in total: ~0.06 core-seconds per config-4 subdomain-cycle on the box's 16 cores
+    # (config 4: 256 subdomains x 4 steps on all cores ~ 4 s, 64 subdomains x 3 steps on one thread ~ 12 s)
+    return {1: 4, 2: 64, 3: 16, 4: 256, 5: 512}.get(int(p.name[3]), 32)
 
 
 def run_reference(args, p, rank, world):
@@ -166,7 +192,7 @@ def run_reference(args, p, rank, world):
     steps, warmup = args.steps, args.warmup
     sample = args.cpu_sample or default_cpu_sample(p)
     steps_cpu = max(1, min(steps, 3))
-    cb = oracle_time_per_cycle(p, sample, steps_cpu, 1, args.smoother)
+    cb = oracle_time_per_cycle(p, sample, steps_cpu, max(1, min(warmup, 1)), args.smoother)
     line = {
         "impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus,
         "steps": steps, "warmup": warmup, "ms_per_step": cb["value"], "higher_is_better": False,
@@ -277,8 +303,10 @@ def run_b200(args, p, rank, world, local_rank):
         peak, peak_src = measured_peak()
         model_bytes = st["model_bytes_fac_iter"][0] + (nfac - 1) * st["model_bytes_fac_iter"][1]
         stream_bytes = st["stream_bytes_fac_iter"][0] + (nfac - 1) * st["stream_bytes_fac_iter"][1]
+        useful_bytes = st["useful_bytes_fac_iter"][0] + (nfac - 1) * st["useful_bytes_fac_iter"][1]
         achieved = model_bytes / (fac_avg_ms * 1e-3) / 1e9
         wname = workload_name(p, args)
+        traffic = ncu_traffic(wname)
         line = {
             "metric": METRIC, "value": ms_step, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": False,
@@ -312,14 +340,20 @@ def run_b200(args, p, rank, world, local_rank):
                 "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": model_bytes, "stream_bytes_per_launch": stream_bytes,
                 "stream_gbs": stream_bytes / (fac_avg_ms * 1e-3) / 1e9, "launch_ms": fac_avg_ms,
-                "traffic": ncu_traffic(wname),
+                # the matrix entries themselves at this build's widths (8-byte value + 2- or 4-byte column), no padding, no headers
+                "useful_bytes": useful_bytes, "useful_gbs": useful_bytes / (fac_avg_ms * 1e-3) / 1e9,
+                "traffic": traffic,
+                # DRAM bytes of the committed ncu capture of THIS kernel source / the launch time measured now / peak
+                "frac_dram": (traffic / (fac_avg_ms * 1e-3) / 1e9 / peak) if traffic else None,
+                "frac_stream": stream_bytes / (fac_avg_ms * 1e-3) / 1e9 / peak,
+                "kernel_source_hash": kernel_source_hash(),
             },
         }
         if not args.no_cpu_baseline:
             m.amgdd_destroy(h)
             del b, x
             torch.cuda.empty_cache()
-            line["cpu_baseline"] = oracle_time_per_cycle(p, args.cpu_sample or default_cpu_sample(p), 1, 1, args.smoother)
+            line["cpu_baseline"] = oracle_time_per_cycle(p, args.cpu_sample or default_cpu_sample(p), 3, 1, args.smoother)
         print(json.dumps(line))
     if distributed:
         dist.barrier()

@@ -98,6 +98,10 @@ typedef struct amgdd_stats {
     double setup_seconds_index_sets;
     double setup_seconds_assembly;
     double setup_seconds_upload;
+    /* the matrix entries one AlgFAC iteration reads at this build's widths (8-byte value + 2-byte column index,
+       4-byte where a level has more than 65535 columns), no padding, no headers, no vectors: what a perfect
+       packing of the same streams would move; same two cases as model_bytes_fac_iter */
+    double useful_bytes_fac_iter[2];
 } amgdd_stats_t;
 
 /* ---------------------------------------------------------------------------------------------

@@ -36,6 +36,7 @@ class AmgddStats(ctypes.Structure):
         ("fac_smem_bytes", _i32), ("max_n_bar", _i64),
         ("assembled_on_device", _i32), ("reserved_", _i32), ("setup_seconds_index_sets", _f64),
         ("setup_seconds_assembly", _f64), ("setup_seconds_upload", _f64),
+        ("useful_bytes_fac_iter", _f64 * 2),
     ]
 
 

@@ -527,7 +527,7 @@ int build_composites_device(amgdd_handle_s* h, const std::vector<i32>& owner, in
 void traffic_model(amgdd_handle_s* h) {
     amgdd_stats_t& s = h->stats;
     const int L = h->H.L;
-    double model[2] = {0, 0}, stream[2] = {0, 0};
+    double model[2] = {0, 0}, stream[2] = {0, 0}, useful[2] = {0, 0};
     for (const SubMeta& sm : h->subs) {
         auto layA = [&](int l) -> const StreamLayout& { return sm.plan.lev[l].shared ? h->glev[l].layA : sm.plan.lev[l].A; };
         auto layP = [&](int l) -> const StreamLayout& { return sm.plan.lev[l].shared ? h->glev[l].layP : sm.plan.lev[l].P; };
@@ -558,10 +558,18 @@ void traffic_model(amgdd_handle_s* h) {
             const double common = a_all + (double)layR(l).bytes + (double)layP(l).bytes + a_real;
             stream[0] += common;
             stream[1] += common + (l == 0 ? a_real : 0.0) + ac_real;
+            // the entries themselves: A_l (A t: all rows; post-relaxation: real rows), R_l, P_l; later iterations add the
+            // pre-relaxation of level 0 and the recalculation on level l+1
+            const double eA = A.wide ? 12.0 : 10.0, eAc = Ac.wide ? 12.0 : 10.0;
+            const double eP = layP(l).wide ? 12.0 : 10.0, eR = layR(l).wide ? 12.0 : 10.0;
+            const double ucommon = eA * (2.0 * b.nnzA_real + b.nnzA_ghost) + (eP + eR) * b.nnzP;
+            useful[0] += ucommon;
+            useful[1] += ucommon + (l == 0 ? eA * b.nnzA_real : 0.0) + eAc * c.nnzA_real;
         }
     }
     s.model_bytes_fac_iter[0] = model[0]; s.model_bytes_fac_iter[1] = model[1];
     s.stream_bytes_fac_iter[0] = stream[0]; s.stream_bytes_fac_iter[1] = stream[1];
+    s.useful_bytes_fac_iter[0] = useful[0]; s.useful_bytes_fac_iter[1] = useful[1];
     double g = 12.0 * h->H.lv[0].A.nnz() + 4.0 * h->n + 24.0 * h->n;            // a1: A_0, x, b, r
     for (int l = 0; l < L; ++l) g += 12.0 * h->H.lv[l].P.nnz() + 4.0 * h->H.lv[l + 1].A.nrows + 8.0 * (h->H.lv[l].A.nrows + h->H.lv[l + 1].A.nrows);
     g += 12.0 * (double)s.sum_real + 24.0 * h->n;                                // a3 gather, a10 update

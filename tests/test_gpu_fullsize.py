@@ -97,3 +97,11 @@ def test_config3_fullsize_eta1_sampled():
 
 def test_config5_fullsize_sampled():
     _run_sampled(5, 2, 16, yardstick=True)
+
+
+@pytest.mark.parametrize("eta", [1, 2, 4])
+def test_config3_eta_sweep_at_64(eta):
+    # the padding experiment of BASELINE.json configs[2] (paper P:285-291) on the largest grid at which eta = 1, 2 and 4
+    # all fit one GPU with private composite matrices (64^3, 4^3 subdomains): every row of the
+    # reported table is backed by a trajectory against the oracle
+    run_parity(wl.make_config(3, 64, eta=eta), 3, all_subdomains=True)
