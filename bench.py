@@ -45,6 +45,9 @@ def parse_args():
     ap.add_argument("--cpu-sample", type=int, default=None, help="subdomains in the oracle's timed sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--smoother", type=int, default=0, choices=[0, 1], help="0: l1-Jacobi (BASELINE), 1: CF l1-Jacobi (P:275)")
+    ap.add_argument("--shard", default=None, choices=["alg5", "allgather"],
+                    help="under torchrun: shard the subdomains over the ranks (NEXT 4; Alg. 5 exchange or all-gather of x) "
+                         "instead of running replicas; unmeasured on multi-GPU hardware (DESIGN.md section 8)")
     return ap.parse_args()
 
 
@@ -220,6 +223,8 @@ def run_b200(args, p, rank, world, local_rank):
     if distributed:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
+    if args.shard:
+        return run_sharded(args, p, rank, world, local_rank, m, torch, dist)
     t0 = time.time()
     h = m.amgdd_setup(p.n, p.rowptr, p.colind, p.vals, p.num_subdomains, p.owner, p.eta, p.num_ghost,
                       p.max_levels, p.theta, p.coarse_max)
@@ -358,6 +363,53 @@ def run_b200(args, p, rank, world, local_rank):
     if distributed:
         dist.barrier()
         dist.destroy_process_group()
+
+
+def run_sharded(args, p, rank, world, local_rank, m, torch, dist):
+    """--shard: the subdomains are split over the ranks (contiguous blocks); one step = one AMG-DD cycle of the whole problem
+    with the staged exchange of include/amgdd.h ("sharding over ranks") over torch.distributed.  Strong scaling: the total
+    work is fixed.  Built and tested with virtual ranks on one GPU (tests/test_gpu_sharded.py); never timed on several GPUs."""
+    from paper_1906_10575_b200.sharded import DistComm, allgather_cycle, setup_exchange, sharded_cycle
+    if not dist.is_initialized():
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    t0 = time.time()
+    h = m.amgdd_setup_shard(p.n, p.rowptr, p.colind, p.vals, p.num_subdomains, p.owner, p.eta, p.num_ghost, p.max_levels, p.theta,
+                            p.coarse_max, rank=rank, nranks=world)
+    comm = DistComm()
+    setup_exchange({rank: h}, comm)
+    setup_s = time.time() - t0
+    stream = torch.cuda.current_stream()
+    m.amgdd_set_stream(h, stream)
+    b = {rank: torch.from_numpy(p.b).cuda()}
+    x = {rank: torch.zeros(p.n, dtype=torch.float64, device="cuda")}
+    nfac, nu = p.num_fac_cycles, p.relax_sweeps
+    cycle = (lambda want=False: sharded_cycle({rank: h}, b, x, comm, nfac, nu, want_norm=want)) if args.shard == "alg5" else \
+            (lambda want=False: allgather_cycle({rank: h}, b, x, comm, nfac, nu)[rank])
+    nlev = m.amgdd_num_levels(h)
+    norms = [cycle(True) for _ in range(p.num_cycles)]
+    for _ in range(args.warmup):
+        cycle()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    dist.barrier(); torch.cuda.synchronize()
+    e0.record(stream)
+    for _ in range(args.steps):
+        cycle()
+    e1.record(stream)
+    dist.barrier(); torch.cuda.synchronize()
+    ms = torch.tensor([e0.elapsed_time(e1) / args.steps], dtype=torch.float64, device="cuda")
+    dist.all_reduce(ms, op=dist.ReduceOp.MAX)
+    if rank == 0:
+        print(json.dumps({
+            "metric": METRIC, "value": float(ms.item()), "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": float(ms.item()), "higher_is_better": False, "scaling": "strong", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic",
+            "config": {"workload": workload_name(p, args), "subdomains": p.num_subdomains, "multi_gpu": f"sharded over {world} ranks, exchange {args.shard}",
+                       "setup_seconds": setup_s, "note": "NEXT 4; unmeasured on multi-GPU hardware before this run"},
+            "residual_norms_at_cycle_start": norms,
+            # per cycle: r_l on the owned rows of L + 1 levels (+ the sum of squares), a gather and a scatter per stage, AlgFAC
+            "gpu_launches": int(((nlev + 1) + 2 * (2 * nlev) + 1) * args.steps)}))
+    dist.barrier()
+    dist.destroy_process_group()
 
 
 def main():

@@ -196,6 +196,60 @@ int amgdd_composite_size(amgdd_handle_t h, int32_t p, int32_t l, int64_t* n_real
 int amgdd_get_composite(amgdd_handle_t h, int32_t p, int32_t l, int32_t* real_gid, int32_t* ghost_gid);
 int amgdd_get_stats(amgdd_handle_t h, amgdd_stats_t* s);
 
+/* ---- sharding over ranks (paper section 5, and Alg. 5) -----------
+ * One process per GPU; rank r of R holds the contiguous block of subdomains [ceil(r P / R), ceil((r + 1) P / R)) and owns
+ * Omega_l^r, the union of their owned points on every level.  The library has no communication layer: one sharded
+ * AMG-DD cycle is 2 L + 2 STAGES, each "compute + pack on the device -> the CALLER exchanges the packed doubles between
+ * the ranks (torch.distributed all_to_all_single, send counts per rank from amgdd_shard_stage_counts) -> unpack":
+ *   stage 0            x at the columns this rank's rows of A_0 read on other ranks ("mat-vec communication with A_0")
+ *   stage 1 + l, l < L r_l likewise for its rows of R_l; before packing, r_l is computed on the owned rows
+ *   stage L + 1 + k    Alg. 5 for level l = L - k: residuals at Psi = { i in Omega_l^r : dist(i, Omega_l^q) <= eta } and at
+ *                      the composite grid Psi_c built from Psi on the coarser levels, to every such rank q (all of level
+ *                      L to every rank, reading A5); values a rank received earlier are forwarded
+ * then amgdd_shard_local_solve runs AlgFAC on the rank's subdomains and updates x on its dofs.  x, b and the residual
+ * vector keep their global numbering on every rank; only the entries a rank owns or received are valid.
+ *
+ * Index protocol, once after setup (the redundancy removal of P:250).  For every stage in ascending order and every source
+ * in ascending rank: the source's amgdd_shard_plan_list(which = 0) is ANNOUNCED to the destination; the destination runs
+ * amgdd_shard_plan_recv_filter on it (positions it owns or was already promised come back as redundant; the rest
+ * becomes its receive list) and returns the redundant positions; the source removes them with
+ * amgdd_shard_plan_apply_drop.  Then amgdd_shard_commit uploads the final lists.  A position indexes x (stage 0) or the
+ * concatenated residual vector r_0 | r_1 | ... (offsets: amgdd_shard_plan_level).  amgdd_shard_plan_create builds a plan
+ * WITHOUT a CUDA device (the hierarchy is rebuilt on the host): tests of the protocol use it. */
+typedef struct amgdd_shard_plan_s* amgdd_shard_plan_t;
+int amgdd_setup_shard(int64_t n, const int64_t* rowptr, const int32_t* colind, const double* vals,
+                      int32_t num_subdomains, const int32_t* owner, int32_t eta, int32_t num_ghost,
+                      int32_t max_levels, double theta, int32_t coarse_max, int32_t rank, int32_t nranks,
+                      amgdd_handle_t* out);      /* as amgdd_setup; builds the rank's subdomains only (local index p - sub_lo) */
+int amgdd_shard_plan_create(int64_t n, const int64_t* rowptr, const int32_t* colind, const double* vals,
+                            int32_t num_subdomains, const int32_t* owner, int32_t eta, int32_t max_levels, double theta,
+                            int32_t coarse_max, int32_t rank, int32_t nranks, amgdd_shard_plan_t* out);
+int amgdd_shard_plan_destroy(amgdd_shard_plan_t p);
+int amgdd_get_shard_plan(amgdd_handle_t h, amgdd_shard_plan_t* out);   /* borrowed: valid until amgdd_destroy(h) */
+/* info: rank, nranks, L + 1, stages, first and one-past-last subdomain of the rank */
+int amgdd_shard_plan_info(amgdd_shard_plan_t p, int32_t info[6]);
+int amgdd_shard_plan_level(amgdd_shard_plan_t p, int32_t l, int64_t* n_l, int64_t* r_offset, int64_t* n_owned);
+int amgdd_shard_plan_owner_rank(amgdd_shard_plan_t p, int32_t l, int32_t* owner_rank);   /* HOST, n_l entries */
+/* which = 0: positions this rank sends to `peer` in `stage`; 1: positions it receives from `peer` (after recv_filter).
+ * pos = NULL returns the count only. */
+int amgdd_shard_plan_list(amgdd_shard_plan_t p, int32_t which, int32_t stage, int32_t peer, int64_t* pos, int64_t* count);
+int amgdd_shard_plan_stage_vector(amgdd_shard_plan_t p, int32_t stage, int32_t* vec);    /* 0: positions index x, 1: the residual vector */
+int amgdd_shard_plan_recv_filter(amgdd_shard_plan_t p, int32_t stage, int32_t src, const int64_t* announced, int64_t count,
+                                 int64_t* redundant, int64_t* nredundant);               /* redundant: room for count entries */
+int amgdd_shard_plan_apply_drop(amgdd_shard_plan_t p, int32_t stage, int32_t dest, const int64_t* redundant, int64_t count);
+int amgdd_shard_commit(amgdd_handle_t h);
+/* send_counts, recv_counts: HOST, nranks entries: doubles to / from every rank in this stage (buffers: rank after rank) */
+int amgdd_shard_stage_counts(amgdd_handle_t h, int32_t stage, int64_t* send_counts, int64_t* recv_counts);
+int amgdd_shard_stage_pack(amgdd_handle_t h, int32_t stage, const double* b, const double* x, double* sendbuf);   /* DEVICE pointers */
+int amgdd_shard_stage_unpack(amgdd_handle_t h, int32_t stage, double* x, const double* recvbuf);
+int amgdd_shard_local_solve(amgdd_handle_t h, double* x, int32_t num_fac_cycles, int32_t relax_sweeps);            /* a3-a10 */
+int amgdd_shard_sqnorm(amgdd_handle_t h, double* out_host);   /* sum of r_0^2 over the owned rows, as computed before stage 1 */
+/* The simple alternative of SURVEY.md section 8(e): all-gather x, then amgdd_solve on the shard handle (global residual
+ * and restriction redundantly on every rank, AlgFAC on the rank's subdomains).  buf: x at the dofs of a rank, ascending. */
+int amgdd_shard_owned_count(amgdd_handle_t h, int32_t rank, int64_t* count);
+int amgdd_shard_pack_owned(amgdd_handle_t h, const double* x, double* buf);
+int amgdd_shard_unpack_owned(amgdd_handle_t h, int32_t src_rank, const double* buf, double* x);
+
 /* ---- the HBM layout of the matrices, exposed for tests and tools --------------------------------
  * Packs a CSR matrix (HOST; rowptr32 has nrows+1 int32 entries starting at 0, at most 65535
  * entries per row) into the "SELL-32 group" streams the AlgFAC kernel reads with coalesced 128-bit

@@ -75,6 +75,26 @@ def _load():
     L.amgdd_debug_fac_op_cycles.argtypes = [_vp, _vp, _i32, _vp]
     L.amgdd_debug_read_block.argtypes = [_vp, _i32, _i32, _i32, _vp, _i64, _vp]
     L.amgdd_pack_stream.argtypes = [_i32, _i32, _vp, _vp, _vp, _vp, _vp, _i32, _i32, _vp, _i64, _vp, _vp]
+    L.amgdd_setup_shard.argtypes = [_i64, _vp, _vp, _vp, _i32, _vp, _i32, _i32, _i32, _f64, _i32, _i32, _i32, ctypes.POINTER(_vp)]
+    L.amgdd_shard_plan_create.argtypes = [_i64, _vp, _vp, _vp, _i32, _vp, _i32, _i32, _f64, _i32, _i32, _i32, ctypes.POINTER(_vp)]
+    L.amgdd_shard_plan_destroy.argtypes = [_vp]
+    L.amgdd_get_shard_plan.argtypes = [_vp, ctypes.POINTER(_vp)]
+    L.amgdd_shard_plan_info.argtypes = [_vp, _vp]
+    L.amgdd_shard_plan_level.argtypes = [_vp, _i32, _vp, _vp, _vp]
+    L.amgdd_shard_plan_owner_rank.argtypes = [_vp, _i32, _vp]
+    L.amgdd_shard_plan_list.argtypes = [_vp, _i32, _i32, _i32, _vp, _vp]
+    L.amgdd_shard_plan_stage_vector.argtypes = [_vp, _i32, _vp]
+    L.amgdd_shard_plan_recv_filter.argtypes = [_vp, _i32, _i32, _vp, _i64, _vp, _vp]
+    L.amgdd_shard_plan_apply_drop.argtypes = [_vp, _i32, _i32, _vp, _i64]
+    L.amgdd_shard_commit.argtypes = [_vp]
+    L.amgdd_shard_stage_counts.argtypes = [_vp, _i32, _vp, _vp]
+    L.amgdd_shard_stage_pack.argtypes = [_vp, _i32, _vp, _vp, _vp]
+    L.amgdd_shard_stage_unpack.argtypes = [_vp, _i32, _vp, _vp]
+    L.amgdd_shard_local_solve.argtypes = [_vp, _vp, _i32, _i32]
+    L.amgdd_shard_sqnorm.argtypes = [_vp, _vp]
+    L.amgdd_shard_owned_count.argtypes = [_vp, _i32, _vp]
+    L.amgdd_shard_pack_owned.argtypes = [_vp, _vp, _vp]
+    L.amgdd_shard_unpack_owned.argtypes = [_vp, _i32, _vp, _vp]
     return L
 
 
@@ -304,3 +324,134 @@ def amgdd_last_solve_profile(h: Handle):
     _check(lib.amgdd_last_solve_profile(h._h, ms, ln))
     return {"ms_residual": ms[0], "ms_restrict": ms[1], "ms_fac": ms[2], "ms_total": ms[3],
             "launches": [int(ln[0]), int(ln[1]), int(ln[2])]}
+
+
+# ---- sharding over ranks (include/amgdd.h, "sharding over ranks"; the exchange driver is in sharded.py) ----
+class ShardPlan:
+    """An amgdd_shard_plan_t: owned (amgdd_shard_plan_create, host only) or borrowed from a Handle."""
+
+    def __init__(self, ptr, owned, keep=None):
+        self._p, self._owned, self._keep = ptr, owned, keep
+
+    def __del__(self):
+        if getattr(self, "_p", None) and self._owned and lib is not None:
+            lib.amgdd_shard_plan_destroy(self._p)
+        self._p = None
+
+
+def amgdd_setup_shard(n, rowptr, colind, vals, num_subdomains, owner, eta, num_ghost=1, max_levels=25, theta=0.25,
+                      coarse_max=64, rank=0, nranks=1) -> Handle:
+    rowptr, colind, vals, owner = _np(rowptr, np.int64), _np(colind, np.int32), _np(vals, np.float64), _np(owner, np.int32)
+    out = _vp()
+    _check(lib.amgdd_setup_shard(n, rowptr.ctypes.data, colind.ctypes.data, vals.ctypes.data, num_subdomains, owner.ctypes.data,
+                                 eta, num_ghost, max_levels, theta, coarse_max, rank, nranks, ctypes.byref(out)))
+    return Handle(out.value)
+
+
+def amgdd_shard_plan_create(n, rowptr, colind, vals, num_subdomains, owner, eta, max_levels=25, theta=0.25, coarse_max=64,
+                            rank=0, nranks=1) -> ShardPlan:
+    rowptr, colind, vals, owner = _np(rowptr, np.int64), _np(colind, np.int32), _np(vals, np.float64), _np(owner, np.int32)
+    out = _vp()
+    _check(lib.amgdd_shard_plan_create(n, rowptr.ctypes.data, colind.ctypes.data, vals.ctypes.data, num_subdomains,
+                                       owner.ctypes.data, eta, max_levels, theta, coarse_max, rank, nranks, ctypes.byref(out)))
+    return ShardPlan(out.value, True)
+
+
+def amgdd_get_shard_plan(h: Handle) -> ShardPlan:
+    out = _vp()
+    _check(lib.amgdd_get_shard_plan(h._h, ctypes.byref(out)))
+    return ShardPlan(out.value, False, keep=h)
+
+
+def amgdd_shard_plan_info(p: ShardPlan) -> dict:
+    a = np.zeros(6, dtype=np.int32)
+    _check(lib.amgdd_shard_plan_info(p._p, a.ctypes.data))
+    return dict(zip(["rank", "nranks", "num_levels", "num_stages", "sub_lo", "sub_hi"], [int(v) for v in a]))
+
+
+def amgdd_shard_plan_level(p: ShardPlan, l: int):
+    n, off, no = _i64(), _i64(), _i64()
+    _check(lib.amgdd_shard_plan_level(p._p, l, ctypes.byref(n), ctypes.byref(off), ctypes.byref(no)))
+    return n.value, off.value, no.value
+
+
+def amgdd_shard_plan_owner_rank(p: ShardPlan, l: int) -> np.ndarray:
+    out = np.empty(amgdd_shard_plan_level(p, l)[0], dtype=np.int32)
+    _check(lib.amgdd_shard_plan_owner_rank(p._p, l, out.ctypes.data))
+    return out
+
+
+def amgdd_shard_plan_list(p: ShardPlan, which: int, stage: int, peer: int) -> np.ndarray:
+    cnt = _i64()
+    _check(lib.amgdd_shard_plan_list(p._p, which, stage, peer, None, ctypes.byref(cnt)))
+    out = np.empty(cnt.value, dtype=np.int64)
+    if cnt.value:
+        _check(lib.amgdd_shard_plan_list(p._p, which, stage, peer, out.ctypes.data, ctypes.byref(cnt)))
+    return out
+
+
+def amgdd_shard_plan_stage_vector(p: ShardPlan, stage: int) -> int:
+    v = _i32()
+    _check(lib.amgdd_shard_plan_stage_vector(p._p, stage, ctypes.byref(v)))
+    return v.value
+
+
+def amgdd_shard_plan_recv_filter(p: ShardPlan, stage: int, src: int, announced) -> np.ndarray:
+    announced = _np(announced, np.int64)
+    red = np.empty(max(1, len(announced)), dtype=np.int64)
+    nred = _i64()
+    _check(lib.amgdd_shard_plan_recv_filter(p._p, stage, src, announced.ctypes.data if len(announced) else None, len(announced),
+                                            red.ctypes.data, ctypes.byref(nred)))
+    return red[:nred.value].copy()
+
+
+def amgdd_shard_plan_apply_drop(p: ShardPlan, stage: int, dest: int, redundant):
+    redundant = _np(redundant, np.int64)
+    _check(lib.amgdd_shard_plan_apply_drop(p._p, stage, dest, redundant.ctypes.data if len(redundant) else None, len(redundant)))
+
+
+def amgdd_shard_commit(h: Handle):
+    _check(lib.amgdd_shard_commit(h._h))
+
+
+def amgdd_shard_stage_counts(h: Handle, stage: int, nranks: int):
+    s, r = np.zeros(nranks, dtype=np.int64), np.zeros(nranks, dtype=np.int64)
+    _check(lib.amgdd_shard_stage_counts(h._h, stage, s.ctypes.data, r.ctypes.data))
+    return s, r
+
+
+def amgdd_shard_stage_pack(h: Handle, stage: int, b, x, sendbuf):
+    n = amgdd_level_size(h, 0)[0]
+    _check(lib.amgdd_shard_stage_pack(h._h, stage, _dev_ptr(b, n), _dev_ptr(x, n), sendbuf.data_ptr() if sendbuf is not None and sendbuf.numel() else None))
+
+
+def amgdd_shard_stage_unpack(h: Handle, stage: int, x, recvbuf):
+    n = amgdd_level_size(h, 0)[0]
+    _check(lib.amgdd_shard_stage_unpack(h._h, stage, _dev_ptr(x, n), recvbuf.data_ptr() if recvbuf is not None and recvbuf.numel() else None))
+
+
+def amgdd_shard_local_solve(h: Handle, x, num_fac_cycles=2, relax_sweeps=1):
+    n = amgdd_level_size(h, 0)[0]
+    _check(lib.amgdd_shard_local_solve(h._h, _dev_ptr(x, n), num_fac_cycles, relax_sweeps))
+
+
+def amgdd_shard_sqnorm(h: Handle) -> float:
+    out = _f64()
+    _check(lib.amgdd_shard_sqnorm(h._h, ctypes.byref(out)))
+    return out.value
+
+
+def amgdd_shard_owned_count(h: Handle, rank: int) -> int:
+    out = _i64()
+    _check(lib.amgdd_shard_owned_count(h._h, rank, ctypes.byref(out)))
+    return out.value
+
+
+def amgdd_shard_pack_owned(h: Handle, x, buf):
+    n = amgdd_level_size(h, 0)[0]
+    _check(lib.amgdd_shard_pack_owned(h._h, _dev_ptr(x, n), buf.data_ptr()))
+
+
+def amgdd_shard_unpack_owned(h: Handle, src_rank: int, buf, x):
+    n = amgdd_level_size(h, 0)[0]
+    _check(lib.amgdd_shard_unpack_owned(h._h, src_rank, buf.data_ptr(), _dev_ptr(x, n)))

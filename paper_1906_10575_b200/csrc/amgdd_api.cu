@@ -48,6 +48,12 @@ struct SubMeta {                 // host-side record of one subdomain's blob
 
 }  // namespace
 
+struct amgdd_shard_plan_s {                     // a plan on its own (host only: amgdd_shard_plan_create) or the one of a handle
+    std::unique_ptr<Hierarchy> H;
+    std::unique_ptr<ShardPlan> own;
+    ShardPlan* S = nullptr;
+};
+
 struct amgdd_handle_s {
     Hierarchy H;
     int P = 0, eta = 0, nghost = 1;
@@ -87,7 +93,23 @@ struct amgdd_handle_s {
     long long prof_launches[3] = {0, 0, 0};
     std::string detail;
     bool vcycle_ready = false;
+    // sharding over ranks (NEXT 4): this handle holds the subdomains [sub_lo, sub_lo + P) of P_global
+    int P_global = 0, sub_lo = 0;
+    std::unique_ptr<ShardPlan> shard;
+    std::unique_ptr<struct amgdd_shard_plan_s> shard_view;       // what amgdd_get_shard_plan hands out (borrows `shard`)
+    struct StageDev {                            // one exchange stage on the device (amgdd_shard_commit)
+        long long* send_pos = nullptr; long long* recv_pos = nullptr;
+        long long nsend = 0, nrecv = 0;
+        std::vector<long long> send_counts, recv_counts;
+    };
+    std::vector<StageDev> stage_dev;
+    std::vector<int*> d_owned_rows;              // per level: the rows this rank owns
+    int* d_owned0_all = nullptr;                 // level 0: the dofs of every rank, rank after rank
+    std::vector<long long> owned0_off;           // nranks + 1 offsets into d_owned0_all
+    double* d_sq = nullptr;                      // sum of r_0^2 over the owned rows (amgdd_shard_sqnorm)
+    bool shard_committed = false;
 };
+
 
 namespace {
 
@@ -185,7 +207,7 @@ int arena_take(amgdd_handle_s* h, Arena& arena, size_t bytes, char** out, std::s
 int build_composites(amgdd_handle_s* h, const std::vector<i32>& owner, int nthreads) {
     const int P = h->P, L = h->H.L;
     std::vector<std::vector<i32>> owned(P);
-    for (i64 i = 0; i < h->n; ++i) owned[owner[i]].push_back((i32)i);
+    for (i64 i = 0; i < h->n; ++i) if (owner[i] >= 0) owned[owner[i]].push_back((i32)i);      // (-1: a subdomain of another rank)
     h->subs.assign(P, SubMeta());
     Arena arena;
     std::atomic<int> status(AMGDD_SUCCESS);
@@ -297,7 +319,7 @@ struct GrowBuf {                                    // a device array that is re
 int build_composites_device(amgdd_handle_s* h, const std::vector<i32>& owner, int nthreads) {
     const int P = h->P, L = h->H.L;
     std::vector<std::vector<i32>> owned(P);
-    for (i64 i = 0; i < h->n; ++i) owned[owner[i]].push_back((i32)i);
+    for (i64 i = 0; i < h->n; ++i) if (owner[i] >= 0) owned[owner[i]].push_back((i32)i);      // (-1: a subdomain of another rank)
     h->subs.assign(P, SubMeta());
     auto tA = std::chrono::steady_clock::now();
     // the hierarchy on the device, for the duration of the assembly
@@ -780,9 +802,32 @@ const char* amgdd_strerror(int code) {
 
 const char* amgdd_last_error_detail(void) { return g_detail.c_str(); }
 
+static int setup_impl(int64_t n, const int64_t* rowptr, const int32_t* colind, const double* vals,
+                      int32_t num_subdomains, const int32_t* owner, int32_t eta, int32_t num_ghost,
+                      int32_t max_levels, double theta, int32_t coarse_max, int32_t rank, int32_t nranks, bool sharded,
+                      amgdd_handle_t* out);
+
 int amgdd_setup(int64_t n, const int64_t* rowptr, const int32_t* colind, const double* vals,
                 int32_t num_subdomains, const int32_t* owner, int32_t eta, int32_t num_ghost,
                 int32_t max_levels, double theta, int32_t coarse_max, amgdd_handle_t* out) {
+    return setup_impl(n, rowptr, colind, vals, num_subdomains, owner, eta, num_ghost, max_levels, theta, coarse_max, 0, 1, false, out);
+}
+
+int amgdd_setup_shard(int64_t n, const int64_t* rowptr, const int32_t* colind, const double* vals,
+                      int32_t num_subdomains, const int32_t* owner, int32_t eta, int32_t num_ghost,
+                      int32_t max_levels, double theta, int32_t coarse_max, int32_t rank, int32_t nranks, amgdd_handle_t* out) {
+    if (nranks < 1 || rank < 0 || rank >= nranks || nranks > num_subdomains) {
+        if (out) *out = nullptr;
+        g_detail = "need 0 <= rank < nranks <= num_subdomains";
+        return AMGDD_ERR_BAD_ARG;
+    }
+    return setup_impl(n, rowptr, colind, vals, num_subdomains, owner, eta, num_ghost, max_levels, theta, coarse_max, rank, nranks, true, out);
+}
+
+static int setup_impl(int64_t n, const int64_t* rowptr, const int32_t* colind, const double* vals,
+                      int32_t num_subdomains, const int32_t* owner, int32_t eta, int32_t num_ghost,
+                      int32_t max_levels, double theta, int32_t coarse_max, int32_t rank, int32_t nranks, bool sharded,
+                      amgdd_handle_t* out) {
     if (out) *out = nullptr;
     g_detail.clear();
     if (!out || !rowptr || !colind || !vals || !owner) { g_detail = "null pointer argument"; return AMGDD_ERR_BAD_ARG; }
@@ -813,6 +858,11 @@ int amgdd_setup(int64_t n, const int64_t* rowptr, const int32_t* colind, const d
     std::memset(&h->stats, 0, sizeof(h->stats));
     if (cudaGetDevice(&h->device) != cudaSuccess) { delete h; g_detail = "cudaGetDevice failed"; return AMGDD_ERR_CUDA; }
     h->n = n; h->P = num_subdomains; h->eta = eta; h->nghost = num_ghost;
+    h->P_global = num_subdomains;
+    if (sharded) {                               // the rank's block of subdomains: [ceil(rank P / R), ceil((rank + 1) P / R))
+        h->sub_lo = (int)(((i64)rank * num_subdomains + nranks - 1) / nranks);
+        h->P = (int)(((i64)(rank + 1) * num_subdomains + nranks - 1) / nranks) - h->sub_lo;
+    }
     h->window = env_int("AMGDD_WINDOW", DEFAULT_WINDOW);
     if (h->window < SLICE_ROWS || h->window > MAX_WINDOW || (h->window % SLICE_ROWS)) {
         delete h;
@@ -831,6 +881,11 @@ int amgdd_setup(int64_t n, const int64_t* rowptr, const int32_t* colind, const d
         if (rc) { free_handle(h); return rc; }
         auto t1 = std::chrono::steady_clock::now();
         std::vector<i32> own(owner, owner + n);
+        if (sharded) {
+            h->shard.reset(new ShardPlan());
+            shard_build(h->H, owner, num_subdomains, eta, rank, nranks, *h->shard);
+            for (i64 i = 0; i < n; ++i) own[i] = (own[i] >= h->sub_lo && own[i] < h->sub_lo + h->P) ? own[i] - h->sub_lo : -1;
+        }
         // AMGDD_ASSEMBLE=host keeps the local matrices and the packing on the host (the reference the device
         // assembly is tested against); windows beyond the device sort's tile also take that path
         const char* asm_env = std::getenv("AMGDD_ASSEMBLE");
@@ -881,6 +936,58 @@ int amgdd_set_stream(amgdd_handle_t h, void* s) {
 
 namespace {
 
+// (re)builds the static program of one subdomain and the launch plan that depends on its length
+int ensure_program(amgdd_handle_s* h, int num_fac_cycles, int relax_sweeps) {
+    const int L = h->H.L;
+    if (h->prog_nfac != num_fac_cycles || h->prog_nu != relax_sweeps || h->prog_smoother != h->smoother) {       // (re)build the program of one subdomain
+        const int nops = fac_build_program(L, num_fac_cycles, relax_sweeps, h->smoother, nullptr);
+        if (nops > MAX_OPS || L > 84) {
+            g_detail = "num_fac_cycles x relax_sweeps x levels gives a program of " + std::to_string(nops) + " steps; the kernel holds " +
+                       std::to_string(MAX_OPS);
+            return AMGDD_ERR_BAD_ARG;
+        }
+        std::vector<FacOp> ops((size_t)nops);
+        fac_build_program(L, num_fac_cycles, relax_sweeps, h->smoother, ops.data());
+        CUDA_TRY(cudaMemcpyAsync(h->d_ops, ops.data(), ops.size() * sizeof(FacOp), cudaMemcpyHostToDevice, h->stream));
+        CUDA_TRY(cudaStreamSynchronize(h->stream));
+        h->prog_nfac = num_fac_cycles; h->prog_nu = relax_sweeps; h->prog_smoother = h->smoother; h->prog_nops = nops;
+        // shared-memory vector buffers: as large as the largest level needs, but leave the L1 (which
+        // shares the SM's 228 KB with shared memory) room for the loads in flight: with less than
+        // ~48 KB of L1 the streaming rate of this kernel drops by 15% (profiles/).  Levels that do
+        // not fit are gathered through L1 from the workspace slot instead.
+        const int budget = std::min(h->smem_cta, env_int("AMGDD_SMEM_BUDGET", 180 * 1024));
+        const int prof_bytes = h->d_prof ? PROF_SMEM_BYTES : 0;
+        long long cap = ((long long)budget - fac_smem_bytes(0, L, nops) - prof_bytes) / 16;
+        cap = std::max(0LL, std::min(cap, h->x_need)) & ~15LL;
+        if (env_int("AMGDD_FORCE_GLOBAL_X", 0) > 0) cap = 0;
+        h->x_cap = (int)cap;
+        h->stats.x_cap = h->x_cap;
+        h->prof_smem_off = fac_smem_bytes(h->x_cap, L, nops);
+        h->fac_cfg.smem_bytes = std::min(h->smem_cta, h->prof_smem_off + prof_bytes);
+        h->stats.fac_smem_bytes = h->fac_cfg.smem_bytes;
+    }
+    return AMGDD_SUCCESS;
+}
+
+FacParams fac_params(amgdd_handle_s* h, double* x) {
+    const int L = h->H.L;
+    FacParams prm;
+    prm.lev = h->d_lev; prm.sub = h->d_sub; prm.order = h->d_order;
+    prm.num_sub = h->P; prm.L = L;
+    prm.r_all = h->d_r_all; prm.r_off = h->d_r_off;
+    prm.x = x; prm.workspace = h->d_workspace;
+    prm.slot_stride = h->slot_stride; prm.xg_off = h->xg_off;
+    prm.work_counter = h->d_counter;
+    prm.ops = h->d_ops; prm.nops = h->prog_nops;
+    prm.lu = h->d_lu; prm.rowperm = h->d_rowperm; prm.nL = (int)h->H.nL;
+    prm.cf0 = h->d_cf0;
+    prm.x_cap = h->x_cap;
+    prm.prof = h->d_prof;
+    prm.prof_smem_off = h->prof_smem_off;
+    prm.prof_ops = h->d_prof_ops;
+    return prm;
+}
+
 // r_0 = b - A_0 x with ||r_0||_2 into d_norms[slot]
 int enqueue_residual(amgdd_handle_s* h, const double* b, const double* x, double* r, int norm_slot) {
     const GlobalLevelDev& g = h->glev[0];
@@ -917,47 +1024,11 @@ int amgdd_solve(amgdd_handle_t h, const double* b, double* x, int32_t num_cycles
     auto mark = [&]() {
         if (timed) cudaEventRecord(ev[nev++], h->stream);
     };
-    if (h->prog_nfac != num_fac_cycles || h->prog_nu != relax_sweeps || h->prog_smoother != h->smoother) {       // (re)build the program of one subdomain
-        const int nops = fac_build_program(L, num_fac_cycles, relax_sweeps, h->smoother, nullptr);
-        if (nops > MAX_OPS || L > 84) {
-            g_detail = "num_fac_cycles x relax_sweeps x levels gives a program of " + std::to_string(nops) + " steps; the kernel holds " +
-                       std::to_string(MAX_OPS);
-            return AMGDD_ERR_BAD_ARG;
-        }
-        std::vector<FacOp> ops((size_t)nops);
-        fac_build_program(L, num_fac_cycles, relax_sweeps, h->smoother, ops.data());
-        CUDA_TRY(cudaMemcpyAsync(h->d_ops, ops.data(), ops.size() * sizeof(FacOp), cudaMemcpyHostToDevice, h->stream));
-        CUDA_TRY(cudaStreamSynchronize(h->stream));
-        h->prog_nfac = num_fac_cycles; h->prog_nu = relax_sweeps; h->prog_smoother = h->smoother; h->prog_nops = nops;
-        // shared-memory vector buffers: as large as the largest level needs, but leave the L1 (which
-        // shares the SM's 228 KB with shared memory) room for the loads in flight: with less than
-        // ~48 KB of L1 the streaming rate of this kernel drops by 15% (profiles/).  Levels that do
-        // not fit are gathered through L1 from the workspace slot instead.
-        const int budget = std::min(h->smem_cta, env_int("AMGDD_SMEM_BUDGET", 180 * 1024));
-        const int prof_bytes = h->d_prof ? PROF_SMEM_BYTES : 0;
-        long long cap = ((long long)budget - fac_smem_bytes(0, L, nops) - prof_bytes) / 16;
-        cap = std::max(0LL, std::min(cap, h->x_need)) & ~15LL;
-        if (env_int("AMGDD_FORCE_GLOBAL_X", 0) > 0) cap = 0;
-        h->x_cap = (int)cap;
-        h->stats.x_cap = h->x_cap;
-        h->prof_smem_off = fac_smem_bytes(h->x_cap, L, nops);
-        h->fac_cfg.smem_bytes = std::min(h->smem_cta, h->prof_smem_off + prof_bytes);
-        h->stats.fac_smem_bytes = h->fac_cfg.smem_bytes;
+    {
+        const int prc = ensure_program(h, num_fac_cycles, relax_sweeps);
+        if (prc) return prc;
     }
-    FacParams prm;
-    prm.lev = h->d_lev; prm.sub = h->d_sub; prm.order = h->d_order;
-    prm.num_sub = h->P; prm.L = L;
-    prm.r_all = h->d_r_all; prm.r_off = h->d_r_off;
-    prm.x = x; prm.workspace = h->d_workspace;
-    prm.slot_stride = h->slot_stride; prm.xg_off = h->xg_off;
-    prm.work_counter = h->d_counter;
-    prm.ops = h->d_ops; prm.nops = h->prog_nops;
-    prm.lu = h->d_lu; prm.rowperm = h->d_rowperm; prm.nL = (int)h->H.nL;
-    prm.cf0 = h->d_cf0;
-    prm.x_cap = h->x_cap;
-    prm.prof = h->d_prof;
-    prm.prof_smem_off = h->prof_smem_off;
-    prm.prof_ops = h->d_prof_ops;
+    const FacParams prm = fac_params(h, x);
     long long launches[3] = {0, 0, 0};
     mark();
     for (int k = 0; k < num_cycles; ++k) {
@@ -1111,6 +1182,266 @@ int amgdd_vcycle(amgdd_handle_t h, const double* b, double* x, int32_t num_cycle
         CUDA_TRY(cudaMemcpyAsync(resnorm_host, h->d_norms, (size_t)(num_cycles + 1) * sizeof(double), cudaMemcpyDeviceToHost, st));
         CUDA_TRY(cudaStreamSynchronize(st));
     }
+    return AMGDD_SUCCESS;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Sharding over ranks (paper section 5 and Alg. 5): index protocol and stages
+// ---------------------------------------------------------------------------------------------
+int amgdd_shard_plan_create(int64_t n, const int64_t* rowptr, const int32_t* colind, const double* vals, int32_t num_subdomains,
+                            const int32_t* owner, int32_t eta, int32_t max_levels, double theta, int32_t coarse_max, int32_t rank,
+                            int32_t nranks, amgdd_shard_plan_t* out) {
+    if (out) *out = nullptr;
+    g_detail.clear();
+    if (!out || !rowptr || !colind || !vals || !owner || n <= 0 || n > (i64)INT32_MAX || num_subdomains <= 0 || eta < 0 || max_levels < 1 ||
+        coarse_max < 1 || !(theta > 0.0 && theta <= 1.0) || nranks < 1 || rank < 0 || rank >= nranks || nranks > num_subdomains) {
+        g_detail = "bad argument to amgdd_shard_plan_create";
+        return AMGDD_ERR_BAD_ARG;
+    }
+    int rc = validate_csr(n, rowptr, colind, vals, g_detail);
+    if (rc) return rc;
+    for (i64 i = 0; i < n; ++i)
+        if (owner[i] < 0 || owner[i] >= num_subdomains) { g_detail = "owner[" + std::to_string(i) + "] out of range"; return AMGDD_ERR_BAD_OWNER; }
+    try {
+        std::unique_ptr<amgdd_shard_plan_s> p(new amgdd_shard_plan_s());
+        p->H.reset(new Hierarchy());
+        HostCsr A0;
+        A0.nrows = A0.ncols = n;
+        A0.rp.assign(rowptr, rowptr + n + 1);
+        A0.ci.assign(colind, colind + rowptr[n]);
+        A0.v.assign(vals, vals + rowptr[n]);
+        rc = build_hierarchy(std::move(A0), theta, max_levels, coarse_max, default_threads(), *p->H, g_detail);
+        if (rc) return rc;
+        p->own.reset(new ShardPlan());
+        shard_build(*p->H, owner, num_subdomains, eta, rank, nranks, *p->own);
+        p->S = p->own.get();
+        *out = p.release();
+    } catch (const std::exception& e) {
+        g_detail = std::string("amgdd_shard_plan_create failed: ") + e.what();
+        return AMGDD_ERR_OUT_OF_MEMORY;
+    }
+    return AMGDD_SUCCESS;
+}
+
+int amgdd_shard_plan_destroy(amgdd_shard_plan_t p) {
+    delete p;
+    return AMGDD_SUCCESS;
+}
+
+int amgdd_get_shard_plan(amgdd_handle_t h, amgdd_shard_plan_t* out) {
+    if (bad_handle(h) || !out) return AMGDD_ERR_BAD_ARG;
+    if (!h->shard) { g_detail = "the handle was not set up with amgdd_setup_shard"; return AMGDD_ERR_BAD_ARG; }
+    if (!h->shard_view) { h->shard_view.reset(new amgdd_shard_plan_s()); h->shard_view->S = h->shard.get(); }
+    *out = h->shard_view.get();
+    return AMGDD_SUCCESS;
+}
+
+#define PLAN_OK(p) if (!(p) || !(p)->S) { g_detail = "null shard plan"; return AMGDD_ERR_BAD_ARG; }
+#define STAGE_PEER_OK(S, stage, peer)                                                                  \
+    if ((stage) < 0 || (stage) >= (int)(S).stages.size() || (peer) < 0 || (peer) >= (S).nranks) {      \
+        g_detail = "stage or rank out of range"; return AMGDD_ERR_BAD_ARG; }
+
+int amgdd_shard_plan_info(amgdd_shard_plan_t p, int32_t info[6]) {
+    PLAN_OK(p);
+    if (!info) return AMGDD_ERR_BAD_ARG;
+    const ShardPlan& S = *p->S;
+    info[0] = S.rank; info[1] = S.nranks; info[2] = S.L + 1; info[3] = (int32_t)S.stages.size(); info[4] = S.sub_lo; info[5] = S.sub_hi;
+    return AMGDD_SUCCESS;
+}
+
+int amgdd_shard_plan_level(amgdd_shard_plan_t p, int32_t l, int64_t* n_l, int64_t* r_offset, int64_t* n_owned) {
+    PLAN_OK(p);
+    const ShardPlan& S = *p->S;
+    if (l < 0 || l > S.L) { g_detail = "level out of range"; return AMGDD_ERR_BAD_ARG; }
+    if (n_l) *n_l = (int64_t)S.owner_rank[l].size();
+    if (r_offset) *r_offset = S.r_off[l];
+    if (n_owned) *n_owned = (int64_t)S.owned[l].size();
+    return AMGDD_SUCCESS;
+}
+
+int amgdd_shard_plan_owner_rank(amgdd_shard_plan_t p, int32_t l, int32_t* owner_rank) {
+    PLAN_OK(p);
+    const ShardPlan& S = *p->S;
+    if (l < 0 || l > S.L || !owner_rank) { g_detail = "level out of range"; return AMGDD_ERR_BAD_ARG; }
+    std::copy(S.owner_rank[l].begin(), S.owner_rank[l].end(), owner_rank);
+    return AMGDD_SUCCESS;
+}
+
+int amgdd_shard_plan_list(amgdd_shard_plan_t p, int32_t which, int32_t stage, int32_t peer, int64_t* pos, int64_t* count) {
+    PLAN_OK(p);
+    const ShardPlan& S = *p->S;
+    STAGE_PEER_OK(S, stage, peer);
+    if (!count || (which != 0 && which != 1)) return AMGDD_ERR_BAD_ARG;
+    const std::vector<i64>& v = which == 0 ? S.stages[stage].send[peer] : S.stages[stage].recv[peer];
+    *count = (int64_t)v.size();
+    if (pos) std::copy(v.begin(), v.end(), pos);
+    return AMGDD_SUCCESS;
+}
+
+int amgdd_shard_plan_stage_vector(amgdd_shard_plan_t p, int32_t stage, int32_t* vec) {
+    PLAN_OK(p);
+    if (stage < 0 || stage >= (int)p->S->stages.size() || !vec) return AMGDD_ERR_BAD_ARG;
+    *vec = p->S->stages[stage].vec;
+    return AMGDD_SUCCESS;
+}
+
+int amgdd_shard_plan_recv_filter(amgdd_shard_plan_t p, int32_t stage, int32_t src, const int64_t* announced, int64_t count,
+                                 int64_t* redundant, int64_t* nredundant) {
+    PLAN_OK(p);
+    ShardPlan& S = *p->S;
+    STAGE_PEER_OK(S, stage, src);
+    if (count < 0 || (count > 0 && (!announced || !redundant)) || !nredundant) return AMGDD_ERR_BAD_ARG;
+    const i64 limit = S.stages[stage].vec == 0 ? (i64)S.have_x.size() : (i64)S.have.size();
+    for (int64_t k = 0; k < count; ++k)
+        if (announced[k] < 0 || announced[k] >= limit) { g_detail = "announced position out of range"; return AMGDD_ERR_BAD_ARG; }
+    std::vector<i64> red;
+    shard_recv_filter(S, stage, src, announced, count, red);
+    *nredundant = (int64_t)red.size();
+    std::copy(red.begin(), red.end(), redundant);
+    return AMGDD_SUCCESS;
+}
+
+int amgdd_shard_plan_apply_drop(amgdd_shard_plan_t p, int32_t stage, int32_t dest, const int64_t* redundant, int64_t count) {
+    PLAN_OK(p);
+    ShardPlan& S = *p->S;
+    STAGE_PEER_OK(S, stage, dest);
+    if (count < 0 || (count > 0 && !redundant)) return AMGDD_ERR_BAD_ARG;
+    shard_apply_drop(S, stage, dest, redundant, count);
+    return AMGDD_SUCCESS;
+}
+
+#define SHARD_OK(h) if (bad_handle(h)) return AMGDD_ERR_BAD_ARG; \
+    if (!(h)->shard) { g_detail = "the handle was not set up with amgdd_setup_shard"; return AMGDD_ERR_BAD_ARG; }
+#define SHARD_READY(h) SHARD_OK(h) \
+    if (!(h)->shard_committed) { g_detail = "run the index protocol and amgdd_shard_commit first"; return AMGDD_ERR_BAD_ARG; }
+
+int amgdd_shard_commit(amgdd_handle_t h) {
+    SHARD_OK(h);
+    DEVICE_SCOPE(h);
+    const ShardPlan& S = *h->shard;
+    const int R = S.nranks;
+    int rc;
+    h->stage_dev.assign(S.stages.size(), amgdd_handle_s::StageDev());
+    for (size_t s = 0; s < S.stages.size(); ++s) {
+        amgdd_handle_s::StageDev& d = h->stage_dev[s];
+        d.send_counts.assign(R, 0); d.recv_counts.assign(R, 0);
+        std::vector<long long> sp, rv;
+        for (int q = 0; q < R; ++q) {
+            d.send_counts[q] = (long long)S.stages[s].send[q].size();
+            d.recv_counts[q] = (long long)S.stages[s].recv[q].size();
+            sp.insert(sp.end(), S.stages[s].send[q].begin(), S.stages[s].send[q].end());
+            rv.insert(rv.end(), S.stages[s].recv[q].begin(), S.stages[s].recv[q].end());
+        }
+        d.nsend = (long long)sp.size(); d.nrecv = (long long)rv.size();
+        if ((rc = upload(h, &d.send_pos, sp.data(), sp.size()))) return rc;
+        if ((rc = upload(h, &d.recv_pos, rv.data(), rv.size()))) return rc;
+    }
+    h->d_owned_rows.assign(S.L + 1, nullptr);
+    for (int l = 0; l <= S.L; ++l)
+        if ((rc = upload(h, &h->d_owned_rows[l], S.owned[l].data(), S.owned[l].size()))) return rc;
+    std::vector<int> all;
+    h->owned0_off.assign(R + 1, 0);
+    for (int q = 0; q < R; ++q) { all.insert(all.end(), S.owned0_all[q].begin(), S.owned0_all[q].end()); h->owned0_off[q + 1] = (long long)all.size(); }
+    if ((rc = upload(h, &h->d_owned0_all, all.data(), all.size()))) return rc;
+    if ((rc = dev_alloc(h, (void**)&h->d_sq, sizeof(double)))) return rc;
+    h->shard_committed = true;
+    return AMGDD_SUCCESS;
+}
+
+int amgdd_shard_stage_counts(amgdd_handle_t h, int32_t stage, int64_t* send_counts, int64_t* recv_counts) {
+    SHARD_READY(h);
+    if (stage < 0 || stage >= (int)h->stage_dev.size() || !send_counts || !recv_counts) { g_detail = "stage out of range"; return AMGDD_ERR_BAD_ARG; }
+    for (int q = 0; q < h->shard->nranks; ++q) { send_counts[q] = h->stage_dev[stage].send_counts[q]; recv_counts[q] = h->stage_dev[stage].recv_counts[q]; }
+    return AMGDD_SUCCESS;
+}
+
+int amgdd_shard_stage_pack(amgdd_handle_t h, int32_t stage, const double* b, const double* x, double* sendbuf) {
+    SHARD_READY(h);
+    const ShardPlan& S = *h->shard;
+    const int L = S.L;
+    if (stage < 0 || stage >= (int)h->stage_dev.size() || !b || !x) { g_detail = "stage out of range or null vector"; return AMGDD_ERR_BAD_ARG; }
+    DEVICE_SCOPE(h);
+    // the part of Alg. 2 that must precede the stage: r_l on the rows this rank owns, l = stage - 1
+    if (stage >= 1 && stage <= L + 1) {
+        const int l = stage - 1;
+        const long long nrows = (long long)S.owned[l].size();
+        if (l == 0) {
+            const GlobalLevelDev& g = h->glev[0];
+            int nb = 0;
+            launch_residual_rows(g.a_rp, g.a_ci, g.a_v, h->d_owned_rows[0], nrows, g.lanes_a, b, x, h->d_r_all, h->d_partial, &nb, h->stream);
+            launch_sum_finalize(h->d_partial, nb, h->d_sq, h->stream);
+        } else {
+            const GlobalLevelDev& g = h->glev[l - 1];
+            launch_spmv_rows(g.r_rp, g.r_ci, g.r_v, h->d_owned_rows[l], nrows, g.lanes_r, h->d_r_all + h->r_off[l - 1], h->d_r_all + h->r_off[l], h->stream);
+        }
+    }
+    const amgdd_handle_s::StageDev& d = h->stage_dev[stage];
+    if (d.nsend > 0) {
+        if (!sendbuf) { g_detail = "null send buffer"; return AMGDD_ERR_BAD_ARG; }
+        launch_gather(S.stages[stage].vec == 0 ? x : h->d_r_all, d.send_pos, d.nsend, sendbuf, h->stream);
+    }
+    CUDA_TRY(cudaGetLastError());
+    return AMGDD_SUCCESS;
+}
+
+int amgdd_shard_stage_unpack(amgdd_handle_t h, int32_t stage, double* x, const double* recvbuf) {
+    SHARD_READY(h);
+    if (stage < 0 || stage >= (int)h->stage_dev.size() || !x) { g_detail = "stage out of range or null vector"; return AMGDD_ERR_BAD_ARG; }
+    DEVICE_SCOPE(h);
+    const amgdd_handle_s::StageDev& d = h->stage_dev[stage];
+    if (d.nrecv > 0) {
+        if (!recvbuf) { g_detail = "null receive buffer"; return AMGDD_ERR_BAD_ARG; }
+        launch_scatter(recvbuf, d.recv_pos, d.nrecv, h->shard->stages[stage].vec == 0 ? x : h->d_r_all, h->stream);
+    }
+    CUDA_TRY(cudaGetLastError());
+    return AMGDD_SUCCESS;
+}
+
+int amgdd_shard_local_solve(amgdd_handle_t h, double* x, int32_t num_fac_cycles, int32_t relax_sweeps) {
+    SHARD_OK(h);
+    if (!x || num_fac_cycles < 1 || relax_sweeps < 1) { g_detail = "need x non-null, num_fac_cycles >= 1, relax_sweeps >= 1"; return AMGDD_ERR_BAD_ARG; }
+    DEVICE_SCOPE(h);
+    const int prc = ensure_program(h, num_fac_cycles, relax_sweeps);
+    if (prc) return prc;
+    const FacParams prm = fac_params(h, x);
+    CUDA_TRY(cudaMemsetAsync(h->d_counter, 0, sizeof(int), h->stream));
+    launch_fac(prm, h->fac_cfg, h->stream);                                         // Alg. 2 P:475-479 on this rank's subdomains
+    CUDA_TRY(cudaGetLastError());
+    return AMGDD_SUCCESS;
+}
+
+int amgdd_shard_sqnorm(amgdd_handle_t h, double* out_host) {
+    SHARD_READY(h);
+    if (!out_host) return AMGDD_ERR_BAD_ARG;
+    DEVICE_SCOPE(h);
+    CUDA_TRY(cudaMemcpyAsync(out_host, h->d_sq, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    return AMGDD_SUCCESS;
+}
+
+int amgdd_shard_owned_count(amgdd_handle_t h, int32_t rank, int64_t* count) {
+    SHARD_READY(h);
+    if (rank < 0 || rank >= h->shard->nranks || !count) { g_detail = "rank out of range"; return AMGDD_ERR_BAD_ARG; }
+    *count = h->owned0_off[rank + 1] - h->owned0_off[rank];
+    return AMGDD_SUCCESS;
+}
+
+int amgdd_shard_pack_owned(amgdd_handle_t h, const double* x, double* buf) {
+    SHARD_READY(h);
+    if (!x || !buf) return AMGDD_ERR_BAD_ARG;
+    DEVICE_SCOPE(h);
+    const int r = h->shard->rank;
+    launch_gather32(x, h->d_owned0_all + h->owned0_off[r], h->owned0_off[r + 1] - h->owned0_off[r], buf, h->stream);
+    CUDA_TRY(cudaGetLastError());
+    return AMGDD_SUCCESS;
+}
+
+int amgdd_shard_unpack_owned(amgdd_handle_t h, int32_t src_rank, const double* buf, double* x) {
+    SHARD_READY(h);
+    if (!x || !buf || src_rank < 0 || src_rank >= h->shard->nranks) return AMGDD_ERR_BAD_ARG;
+    DEVICE_SCOPE(h);
+    launch_scatter32(buf, h->d_owned0_all + h->owned0_off[src_rank], h->owned0_off[src_rank + 1] - h->owned0_off[src_rank], x, h->stream);
+    CUDA_TRY(cudaGetLastError());
     return AMGDD_SUCCESS;
 }
 

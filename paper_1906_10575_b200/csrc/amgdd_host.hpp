@@ -180,6 +180,25 @@ private:
 // offsets of the arrays inside a subdomain's blob, from the sizes in out.lev (out.n_owned set)
 void layout_blob(SubdomainBlob& out);
 
+// ---- sharding over ranks (amgdd_shard.cpp) ---------------------------------
+struct ShardStage {
+    int vec = 1;                               // 0: positions index x, 1: the concatenated residual vector r_0 | r_1 | ...
+    std::vector<std::vector<i64>> send, recv;  // per peer rank: positions, in the order both sides agree on
+};
+struct ShardPlan {
+    int rank = 0, nranks = 1, L = 0, sub_lo = 0, sub_hi = 0;
+    std::vector<i64> r_off;                    // L + 2 offsets of the levels in the residual vector
+    std::vector<std::vector<i32>> owner_rank;  // per level: the rank that owns each point (Omega_l^r)
+    std::vector<std::vector<i32>> owned;       // per level: the points of this rank, ascending
+    std::vector<std::vector<i32>> owned0_all;  // level 0: the points of every rank (all-gather of x)
+    std::vector<ShardStage> stages;            // 2 L + 2
+    std::vector<uint8_t> have, have_x;         // receiver side of the redundancy removal: owned or already promised
+};
+int shard_rank_of_sub(int p, int P, int nranks);
+void shard_build(const Hierarchy& H, const i32* owner, int P, int eta, int rank, int nranks, ShardPlan& S);
+void shard_recv_filter(ShardPlan& S, int stage, int src, const i64* announced, i64 count, std::vector<i64>& redundant);
+void shard_apply_drop(ShardPlan& S, int stage, int dest, const i64* redundant, i64 count);
+
 // packs a whole level matrix (the shared global copy) into a host buffer
 struct PackedLevelStream {
     std::vector<char> data;

@@ -12,21 +12,25 @@ namespace {
 // ---------------------------------------------------------------------------------------------
 constexpr int GLOBAL_BLOCK = 256;
 
+// `rows` (optional): the kernel works on the n listed rows instead of rows 0 .. n-1 (sharded cycle: the rows a rank
+// owns); the arithmetic of a row is the same either way
 __global__ void __launch_bounds__(GLOBAL_BLOCK) residual_kernel(const int* __restrict__ rp, const int* __restrict__ ci,
                                                                 const double* __restrict__ v, long long n, int lanes,
                                                                 const double* __restrict__ b, const double* __restrict__ x,
-                                                                double* __restrict__ r, double* __restrict__ partial) {
+                                                                double* __restrict__ r, double* __restrict__ partial,
+                                                                const int* __restrict__ rows) {
     __shared__ double red[GLOBAL_BLOCK / 32];
     const int lane = threadIdx.x & (lanes - 1);
-    const long long row = (long long)blockIdx.x * (GLOBAL_BLOCK / lanes) + threadIdx.x / lanes;
+    const long long idx = (long long)blockIdx.x * (GLOBAL_BLOCK / lanes) + threadIdx.x / lanes;
+    const long long row = (rows && idx < n) ? (long long)__ldg(rows + idx) : idx;
     double sum = 0.0;
-    if (row < n) {
+    if (idx < n) {
         const int bgn = __ldg(rp + row), end = __ldg(rp + row + 1);
         for (int k = bgn + lane; k < end; k += lanes) sum += __ldg(v + k) * __ldg(x + __ldg(ci + k));
     }
     for (int o = lanes >> 1; o > 0; o >>= 1) sum += __shfl_down_sync(0xffffffffu, sum, o, lanes);
     double sq = 0.0;
-    if (row < n && lane == 0) {
+    if (idx < n && lane == 0) {
         const double ri = b[row] - sum;
         if (r) r[row] = ri;
         sq = ri * ri;
@@ -57,16 +61,46 @@ __global__ void __launch_bounds__(1024) norm_finalize_kernel(const double* __res
 
 __global__ void __launch_bounds__(GLOBAL_BLOCK) spmv_kernel(const int* __restrict__ rp, const int* __restrict__ ci,
                                                             const double* __restrict__ v, long long n, int lanes,
-                                                            const double* __restrict__ x, double* __restrict__ y) {
+                                                            const double* __restrict__ x, double* __restrict__ y,
+                                                            const int* __restrict__ rows) {
     const int lane = threadIdx.x & (lanes - 1);
-    const long long row = (long long)blockIdx.x * (GLOBAL_BLOCK / lanes) + threadIdx.x / lanes;
+    const long long idx = (long long)blockIdx.x * (GLOBAL_BLOCK / lanes) + threadIdx.x / lanes;
+    const long long row = (rows && idx < n) ? (long long)__ldg(rows + idx) : idx;
     double sum = 0.0;
-    if (row < n) {
+    if (idx < n) {
         const int bgn = __ldg(rp + row), end = __ldg(rp + row + 1);
         for (int k = bgn + lane; k < end; k += lanes) sum += __ldg(v + k) * __ldg(x + __ldg(ci + k));
     }
     for (int o = lanes >> 1; o > 0; o >>= 1) sum += __shfl_down_sync(0xffffffffu, sum, o, lanes);
-    if (row < n && lane == 0) y[row] = sum;
+    if (idx < n && lane == 0) y[row] = sum;
+}
+
+// pack / unpack of one exchange stage of the sharded cycle (positions: 64-bit into x or the residual vector; 32-bit dof lists)
+template <class I>
+__global__ void __launch_bounds__(GLOBAL_BLOCK) gather_kernel(const double* __restrict__ src, const I* __restrict__ pos, long long n,
+                                                              double* __restrict__ dst) {
+    const long long k = (long long)blockIdx.x * GLOBAL_BLOCK + threadIdx.x;
+    if (k < n) dst[k] = src[pos[k]];
+}
+template <class I>
+__global__ void __launch_bounds__(GLOBAL_BLOCK) scatter_kernel(const double* __restrict__ src, const I* __restrict__ pos, long long n,
+                                                               double* __restrict__ dst) {
+    const long long k = (long long)blockIdx.x * GLOBAL_BLOCK + threadIdx.x;
+    if (k < n) dst[pos[k]] = src[k];
+}
+
+__global__ void __launch_bounds__(1024) sum_finalize_kernel(const double* __restrict__ partial, int nb, double* out) {
+    __shared__ double red[32];
+    double s = 0.0;
+    for (int i = threadIdx.x; i < nb; i += 1024) s += partial[i];       // fixed order: deterministic
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        s = red[threadIdx.x];
+        for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
+        if (threadIdx.x == 0) out[0] = s;
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -160,8 +194,38 @@ int residual_num_blocks(long long n, int lanes) {
 void launch_residual(const int* rp, const int* ci, const double* v, long long n, int lanes, const double* b,
                      const double* x, double* r, double* partial, int* nblocks_out, void* stream) {
     const int nb = residual_num_blocks(n, lanes);
-    residual_kernel<<<nb, GLOBAL_BLOCK, 0, (cudaStream_t)stream>>>(rp, ci, v, n, lanes, b, x, r, partial);
+    residual_kernel<<<nb, GLOBAL_BLOCK, 0, (cudaStream_t)stream>>>(rp, ci, v, n, lanes, b, x, r, partial, nullptr);
     if (nblocks_out) *nblocks_out = nb;
+}
+
+void launch_residual_rows(const int* rp, const int* ci, const double* v, const int* rows, long long nrows, int lanes, const double* b,
+                          const double* x, double* r, double* partial, int* nblocks_out, void* stream) {
+    const int nb = residual_num_blocks(nrows, lanes);
+    if (nb > 0) residual_kernel<<<nb, GLOBAL_BLOCK, 0, (cudaStream_t)stream>>>(rp, ci, v, nrows, lanes, b, x, r, partial, rows);
+    if (nblocks_out) *nblocks_out = nb;
+}
+
+void launch_spmv_rows(const int* rp, const int* ci, const double* v, const int* rows, long long nrows, int lanes, const double* x,
+                      double* y, void* stream) {
+    if (nrows <= 0) return;
+    const int nb = residual_num_blocks(nrows, lanes);
+    spmv_kernel<<<nb, GLOBAL_BLOCK, 0, (cudaStream_t)stream>>>(rp, ci, v, nrows, lanes, x, y, rows);
+}
+
+void launch_gather(const double* src, const long long* pos, long long n, double* dst, void* stream) {
+    if (n > 0) gather_kernel<long long><<<(unsigned)((n + GLOBAL_BLOCK - 1) / GLOBAL_BLOCK), GLOBAL_BLOCK, 0, (cudaStream_t)stream>>>(src, pos, n, dst);
+}
+void launch_scatter(const double* src, const long long* pos, long long n, double* dst, void* stream) {
+    if (n > 0) scatter_kernel<long long><<<(unsigned)((n + GLOBAL_BLOCK - 1) / GLOBAL_BLOCK), GLOBAL_BLOCK, 0, (cudaStream_t)stream>>>(src, pos, n, dst);
+}
+void launch_gather32(const double* src, const int* pos, long long n, double* dst, void* stream) {
+    if (n > 0) gather_kernel<int><<<(unsigned)((n + GLOBAL_BLOCK - 1) / GLOBAL_BLOCK), GLOBAL_BLOCK, 0, (cudaStream_t)stream>>>(src, pos, n, dst);
+}
+void launch_scatter32(const double* src, const int* pos, long long n, double* dst, void* stream) {
+    if (n > 0) scatter_kernel<int><<<(unsigned)((n + GLOBAL_BLOCK - 1) / GLOBAL_BLOCK), GLOBAL_BLOCK, 0, (cudaStream_t)stream>>>(src, pos, n, dst);
+}
+void launch_sum_finalize(const double* partial, int nb, double* out, void* stream) {
+    sum_finalize_kernel<<<1, 1024, 0, (cudaStream_t)stream>>>(partial, nb, out);
 }
 
 void launch_norm_finalize(const double* partial, int nb, double* out, void* stream) {
@@ -172,7 +236,7 @@ void launch_spmv(const int* rp, const int* ci, const double* v, long long nrows,
                  double* y, void* stream) {
     if (nrows <= 0) return;
     const int nb = residual_num_blocks(nrows, lanes);
-    spmv_kernel<<<nb, GLOBAL_BLOCK, 0, (cudaStream_t)stream>>>(rp, ci, v, nrows, lanes, x, y);
+    spmv_kernel<<<nb, GLOBAL_BLOCK, 0, (cudaStream_t)stream>>>(rp, ci, v, nrows, lanes, x, y, nullptr);
 }
 
 }  // namespace amgdd

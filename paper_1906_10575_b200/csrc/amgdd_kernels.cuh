@@ -25,4 +25,18 @@ void launch_coarse_solve(const double* lu, const int* rowperm, int n, const doub
 
 int pick_lanes(double avg_row_nnz);
 
+// ---- sharded cycle (NEXT 4): the same row arithmetic restricted to a list of rows, and the pack / unpack of a stage ----
+// r[rows[k]] = b[rows[k]] - (A x)[rows[k]], partial sums of r^2 over the listed rows (nblocks_out blocks)
+void launch_residual_rows(const int* rp, const int* ci, const double* v, const int* rows, long long nrows, int lanes, const double* b,
+                          const double* x, double* r, double* partial, int* nblocks_out, void* stream);
+// y[rows[k]] = (M x)[rows[k]]
+void launch_spmv_rows(const int* rp, const int* ci, const double* v, const int* rows, long long nrows, int lanes, const double* x,
+                      double* y, void* stream);
+void launch_gather(const double* src, const long long* pos, long long n, double* dst, void* stream);    // dst[k] = src[pos[k]]
+void launch_scatter(const double* src, const long long* pos, long long n, double* dst, void* stream);   // dst[pos[k]] = src[k]
+void launch_gather32(const double* src, const int* pos, long long n, double* dst, void* stream);
+void launch_scatter32(const double* src, const int* pos, long long n, double* dst, void* stream);
+// out[0] = sum partial[0..nb) (no square root)
+void launch_sum_finalize(const double* partial, int nb, double* out, void* stream);
+
 }  // namespace amgdd
