@@ -36,11 +36,11 @@ def test_config3_fullsize_eta1_trajectory():
     run_parity(wl.make_config(3, eta=1), 2, all_subdomains=True)
 
 
-def _run_sampled(cfg, num_cycles, nsample, eta=None, yardstick=False):
+def _run_sampled(cfg, num_cycles, nsample, eta=None, yardstick=False, scale=None):
     import torch
     import paper_1906_10575_b200 as m
     assert torch.cuda.is_available(), "GPU tests need a CUDA device"
-    p = wl.make_config(cfg, eta=eta)
+    p = wl.make_config(cfg, scale, eta=eta)
     h = m.amgdd_setup(p.n, p.rowptr, p.colind, p.vals, p.num_subdomains, p.owner, p.eta, p.num_ghost, p.max_levels,
                       p.theta, p.coarse_max)
 
@@ -105,3 +105,10 @@ def test_config3_eta_sweep_at_64(eta):
     # all fit one GPU with private composite matrices (64^3, 4^3 subdomains): every row of the
     # reported table is backed by a trajectory against the oracle
     run_parity(wl.make_config(3, 64, eta=eta), 3, all_subdomains=True)
+
+
+@pytest.mark.parametrize("eta", [1, 2, 4])
+def test_config3_eta_sweep_at_112_sampled(eta):
+    # 112^3 (343 subdomains) is the largest grid of config 3's recipe at which eta = 1, 2 and 4 all fit one B200 (61 / 123 /
+    # 147 GB): the rows of the reported sweep, sampled cycles against the oracle
+    _run_sampled(3, 2, 6, eta=eta, scale=112)
