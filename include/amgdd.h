@@ -94,7 +94,9 @@ typedef struct amgdd_stats {
        on the device (the default), 0 for the host path (AMGDD_ASSEMBLE=host); the three parts of
        setup_seconds_composite on the device path: host index sets, device kernels + small copies, hierarchy upload */
     int32_t assembled_on_device;
-    int32_t reserved_;
+    int32_t index_sets_on_device;    /* 1: the composite index sets (S6, S7) were grown on the device too (default with the device
+                                        assembly; AMGDD_INDEX_SETS=host, or a breadth-first frontier of more than 262144 points, keeps
+                                        the host search) */
     double setup_seconds_index_sets;
     double setup_seconds_assembly;
     double setup_seconds_upload;

@@ -22,6 +22,11 @@ EXPORTS = [
     "amgdd_get_level_matrix", "amgdd_composite_size", "amgdd_get_composite", "amgdd_get_stats",
     "amgdd_last_solve_profile", "amgdd_pack_stream", "amgdd_debug_fac_cycles", "amgdd_debug_fac_op_cycles",
     "amgdd_debug_read_block",
+    "amgdd_setup_shard", "amgdd_shard_plan_create", "amgdd_shard_plan_destroy", "amgdd_get_shard_plan", "amgdd_shard_plan_info",
+    "amgdd_shard_plan_level", "amgdd_shard_plan_owner_rank", "amgdd_shard_plan_list", "amgdd_shard_plan_stage_vector",
+    "amgdd_shard_plan_recv_filter", "amgdd_shard_plan_apply_drop", "amgdd_shard_commit", "amgdd_shard_stage_counts",
+    "amgdd_shard_stage_pack", "amgdd_shard_stage_unpack", "amgdd_shard_local_solve", "amgdd_shard_sqnorm",
+    "amgdd_shard_owned_count", "amgdd_shard_pack_owned", "amgdd_shard_unpack_owned",
 ]
 
 
@@ -34,7 +39,7 @@ class AmgddStats(ctypes.Structure):
         ("model_bytes_global", _f64), ("setup_seconds_hierarchy", _f64), ("setup_seconds_composite", _f64),
         ("block_bytes", _i32), ("num_ways", _i32), ("window", _i32), ("ring_stages", _i32), ("x_cap", _i32), ("fac_grid", _i32), ("fac_block", _i32),
         ("fac_smem_bytes", _i32), ("max_n_bar", _i64),
-        ("assembled_on_device", _i32), ("reserved_", _i32), ("setup_seconds_index_sets", _f64),
+        ("assembled_on_device", _i32), ("index_sets_on_device", _i32), ("setup_seconds_index_sets", _f64),
         ("setup_seconds_assembly", _f64), ("setup_seconds_upload", _f64),
         ("useful_bytes_fac_iter", _f64 * 2),
     ]
@@ -455,3 +460,10 @@ def amgdd_shard_pack_owned(h: Handle, x, buf):
 def amgdd_shard_unpack_owned(h: Handle, src_rank: int, buf, x):
     n = amgdd_level_size(h, 0)[0]
     _check(lib.amgdd_shard_unpack_owned(h._h, src_rank, buf.data_ptr(), _dev_ptr(x, n)))
+
+
+def amgdd_shard_plan_destroy(p: ShardPlan):
+    """Frees a plan made by amgdd_shard_plan_create (borrowed plans are left alone)."""
+    if p._p and p._owned:
+        lib.amgdd_shard_plan_destroy(p._p)
+    p._p = None

@@ -345,6 +345,7 @@ int build_composites_device(amgdd_handle_s* h, const std::vector<i32>& owner, in
         CUDA_TRY(tmp.put(&dinv, lv.dinv.data(), lv.dinv.size()));
         d.dinv = dinv;
         if (!lv.cf.empty()) { int8_t* cf = nullptr; CUDA_TRY(tmp.put(&cf, lv.cf.data(), lv.cf.size())); d.cf = cf; }
+        if (!lv.coarse_of.empty()) { int* co = nullptr; CUDA_TRY(tmp.put(&co, lv.coarse_of.data(), lv.coarse_of.size())); d.coarse_of = co; }
     }
     DevHierLevel* d_hier = nullptr;
     CUDA_TRY(tmp.put(&d_hier, hier.data(), hier.size()));
@@ -368,9 +369,120 @@ int build_composites_device(amgdd_handle_s* h, const std::vector<i32>& owner, in
     struct JobRef { int p, l, kind; };
     std::vector<JobRef> refs;
     double t_sets = 0, t_dev = 0;
+    // AMGDD_INDEX_SETS=host keeps the breadth-first growth of the index sets on the host (the reference the device
+    // path is tested against); the device path: amgdd_assemble.cuh, "composite index sets on the device"
+    const char* sets_env = std::getenv("AMGDD_INDEX_SETS");
+    bool dev_sets = !(sets_env && std::strcmp(sets_env, "host") == 0);
+    std::vector<long long> bm_off(L + 2, 0);
+    for (int l = 0; l <= L; ++l) bm_off[l + 1] = bm_off[l] + (h->H.lv[l].A.nrows + 31) / 32;
+    long long* d_bm_off = nullptr;
+    unsigned* d_bm = nullptr;
+    int* d_frontier = nullptr;
+    int* d_owned_all = nullptr;
+    SetLevelOut* d_set_out = nullptr;
+    int** d_list_dst = nullptr;
+    SetJob* d_set_jobs = nullptr;
+    std::vector<long long> owned_off(P + 1, 0);
+    std::vector<SetJob> set_jobs;
+    std::vector<SetLevelOut> set_out;
+    std::vector<int*> list_dst;
+    if (dev_sets) {
+        CUDA_TRY(tmp.put(&d_bm_off, bm_off.data(), bm_off.size()));
+        CUDA_TRY(tmp.alloc(&d_bm, (size_t)batch * 2 * (size_t)bm_off[L + 1]));
+        CUDA_TRY(cudaMemsetAsync(d_bm, 0, (size_t)batch * 2 * (size_t)bm_off[L + 1] * sizeof(unsigned), st));
+        CUDA_TRY(tmp.alloc(&d_frontier, (size_t)batch * 3 * SET_FRONTIER_CAP));
+        std::vector<int> flat_owned;
+        flat_owned.reserve((size_t)h->n);
+        for (int p = 0; p < P; ++p) { flat_owned.insert(flat_owned.end(), owned[p].begin(), owned[p].end()); owned_off[p + 1] = (long long)flat_owned.size(); }
+        CUDA_TRY(tmp.put(&d_owned_all, flat_owned.data(), flat_owned.size()));
+        CUDA_TRY(tmp.alloc(&d_set_out, (size_t)batch * (L + 1)));
+        CUDA_TRY(tmp.alloc(&d_list_dst, (size_t)batch * (L + 1)));
+        CUDA_TRY(tmp.alloc(&d_set_jobs, (size_t)batch));
+    }
     for (int p0 = 0; p0 < P; p0 += batch) {
         const int p1 = std::min(P, p0 + batch), nb_ = p1 - p0;
         auto t0 = std::chrono::steady_clock::now();
+        size_t total = 0;
+        std::vector<size_t> base(nb_);
+        bool sets_done = false;
+        auto t1 = t0;
+        if (dev_sets) {
+            // a'. index sets on the device: grow (sizes), lay out, extract (ascending lists, row-length sums)
+            set_jobs.assign(nb_, SetJob());
+            for (int k = 0; k < nb_; ++k) {
+                SetJob& j = set_jobs[k];
+                std::memset(&j, 0, sizeof(j));
+                j.owned = d_owned_all + owned_off[p0 + k]; j.n_owned = (int)(owned_off[p0 + k + 1] - owned_off[p0 + k]);
+                j.bm_real = d_bm + (size_t)k * 2 * (size_t)bm_off[L + 1];
+                j.bm_ghost = j.bm_real + bm_off[L + 1];
+                j.frontier = d_frontier + (size_t)k * 3 * SET_FRONTIER_CAP;
+                j.out = d_set_out + (size_t)k * (L + 1);
+                j.list_dst = d_list_dst + (size_t)k * (L + 1);
+            }
+            CUDA_TRY(cudaMemcpyAsync(d_set_jobs, set_jobs.data(), set_jobs.size() * sizeof(SetJob), cudaMemcpyHostToDevice, st));
+            CUDA_TRY(launch_sets_grow(d_set_jobs, nb_, d_hier, d_bm_off, L, h->eta, h->nghost, st));
+            set_out.resize((size_t)nb_ * (L + 1));
+            CUDA_TRY(cudaMemcpyAsync(set_out.data(), d_set_out, set_out.size() * sizeof(SetLevelOut), cudaMemcpyDeviceToHost, st));
+            CUDA_TRY(cudaMemcpyAsync(set_jobs.data(), d_set_jobs, set_jobs.size() * sizeof(SetJob), cudaMemcpyDeviceToHost, st));
+            CUDA_TRY(cudaStreamSynchronize(st));
+            bool overflow = false;
+            for (int k = 0; k < nb_; ++k) overflow = overflow || set_jobs[k].overflow != 0;
+            if (overflow) {
+                // a frontier larger than the scratch: the host grows the sets of this and all later batches (bitmaps are left dirty)
+                dev_sets = false;
+            } else {
+                for (int k = 0; k < nb_; ++k) {
+                    SubdomainBlob& sb = h->subs[p0 + k].plan;
+                    sb.lev.assign(L + 1, BlockLayout());
+                    sb.dropped = 0; sb.too_long_row = -1; sb.too_long_level = -1;
+                    sb.n_owned = set_jobs[k].n_owned;
+                    base[k] = total;
+                    size_t cnt = (size_t)sb.n_owned;
+                    for (int l = 0; l <= L; ++l) {
+                        const SetLevelOut& o = set_out[(size_t)k * (L + 1) + l];
+                        BlockLayout& b = sb.lev[l];
+                        b.n_real = o.n_real; b.n_ghost = o.n_ghost;
+                        b.shared = (i64)o.n_real == h->H.lv[l].A.nrows;
+                        if (!b.shared) cnt += (size_t)o.n_real + o.n_ghost;
+                    }
+                    total += (cnt + 3) & ~(size_t)3;
+                }
+                CUDA_TRY(d_idx.need(total));
+                list_dst.assign((size_t)nb_ * (L + 1), nullptr);
+                for (int k = 0; k < nb_; ++k) {
+                    const SubdomainBlob& sb = h->subs[p0 + k].plan;
+                    size_t o = base[k] + (size_t)sb.n_owned;
+                    set_jobs[k].owned_local_dst = d_idx.p + base[k];
+                    for (int l = 0; l <= L; ++l) {
+                        if (sb.lev[l].shared) continue;
+                        list_dst[(size_t)k * (L + 1) + l] = d_idx.p + o;
+                        o += (size_t)sb.lev[l].n_real + sb.lev[l].n_ghost;
+                    }
+                }
+                CUDA_TRY(cudaMemcpyAsync(d_list_dst, list_dst.data(), list_dst.size() * sizeof(int*), cudaMemcpyHostToDevice, st));
+                CUDA_TRY(cudaMemcpyAsync(d_set_jobs, set_jobs.data(), set_jobs.size() * sizeof(SetJob), cudaMemcpyHostToDevice, st));
+                CUDA_TRY(launch_sets_extract(d_set_jobs, nb_, d_hier, d_bm_off, L, st));
+                CUDA_TRY(cudaMemcpyAsync(set_out.data(), d_set_out, set_out.size() * sizeof(SetLevelOut), cudaMemcpyDeviceToHost, st));
+                CUDA_TRY(cudaStreamSynchronize(st));
+                for (int k = 0; k < nb_; ++k) {
+                    SubdomainBlob& sb = h->subs[p0 + k].plan;
+                    for (int l = 0; l <= L; ++l) {
+                        const SetLevelOut& o = set_out[(size_t)k * (L + 1) + l];
+                        BlockLayout& b = sb.lev[l];
+                        b.nnzA_real = o.nnzA_real;
+                        if (b.shared) { b.nnzA = b.nnzA_real; b.nnzP = (l < L) ? h->H.lv[l].P.nnz() : 0; }
+                        else if (o.nnzA_real + o.nnzA_ghost_bound > (i64)INT32_MAX || o.nnzP_bound > (i64)INT32_MAX) {
+                            g_detail = "a composite level exceeds 2^31-1 local nonzeros";
+                            return AMGDD_ERR_INDEX_RANGE;
+                        }
+                    }
+                }
+                sets_done = true;
+                t1 = std::chrono::steady_clock::now();
+                t_sets += std::chrono::duration<double>(t1 - t0).count();
+            }
+        }
+        if (!sets_done) {
         // a. index sets on the host (breadth-first growth, S6/S7), one subdomain per task
         lists.assign(nb_, std::vector<i32>());
         std::atomic<int> next(p0);
@@ -408,16 +520,16 @@ int build_composites_device(amgdd_handle_s* h, const std::vector<i32>& owner, in
         };
         run_threads(nw, work);
         if (status.load() != AMGDD_SUCCESS) { g_detail = fail_detail; return status.load(); }
-        auto t1 = std::chrono::steady_clock::now();
+        t1 = std::chrono::steady_clock::now();
         t_sets += std::chrono::duration<double>(t1 - t0).count();
         // b. index lists to the device; jobs of the batch
-        size_t total = 0;
-        std::vector<size_t> base(nb_);
+        total = 0;
         for (int k = 0; k < nb_; ++k) { base[k] = total; total += (lists[k].size() + 3) & ~(size_t)3; }
         flat.assign(total, 0);
         for (int k = 0; k < nb_; ++k) std::copy(lists[k].begin(), lists[k].end(), flat.begin() + base[k]);
         CUDA_TRY(d_idx.need(total));
         CUDA_TRY(cudaMemcpyAsync(d_idx.p, flat.data(), total * sizeof(i32), cudaMemcpyHostToDevice, st));
+        }
         jobs.clear(); refs.clear();
         long long row_off = 0, slice_off = 0;
         std::vector<std::vector<const int*>> gidp(nb_, std::vector<const int*>(L + 1, nullptr));
@@ -542,6 +654,7 @@ int build_composites_device(amgdd_handle_s* h, const std::vector<i32>& owner, in
     h->stats.setup_seconds_assembly = t_dev;
     h->stats.setup_seconds_upload = std::chrono::duration<double>(std::chrono::steady_clock::now() - tA).count() - t_sets - t_dev;
     h->stats.assembled_on_device = 1;
+    h->stats.index_sets_on_device = dev_sets ? 1 : 0;
     return AMGDD_SUCCESS;
 }
 

@@ -291,6 +291,198 @@ __global__ void __launch_bounds__(ASM_THREADS) asm_copy_kernel(const AsmCopy* __
     }
 }
 
+
+// ---- composite index sets (amgdd_assemble.cuh) ----------------------------------------------------------------------------
+constexpr int SET_THREADS = 256;
+
+// one layer of breadth-first growth: every point of `cur` marks its unmarked neighbours in `mark` (those not in `skip`)
+// and appends them to `next`; returns false when `next` overflowed
+__device__ bool grow_layer(const DevCsr64& A, const int* cur, int ncur, unsigned* mark, const unsigned* skip, int* next, int* s_count,
+                           int* s_lo, int* s_hi, int* s_over) {
+    for (int q = threadIdx.x; q < ncur; q += SET_THREADS) {
+        const int i = cur[q];
+        for (long long k = A.rp[i]; k < A.rp[i + 1]; ++k) {
+            const int j = __ldg(A.ci + k);
+            const unsigned bit = 1u << (j & 31);
+            if (skip && (skip[j >> 5] & bit)) continue;
+            const unsigned old = atomicOr(mark + (j >> 5), bit);
+            if (!(old & bit)) {
+                const int pos = atomicAdd(s_count, 1);
+                if (pos < SET_FRONTIER_CAP) next[pos] = j; else *s_over = 1;
+                atomicMin(s_lo, j >> 5);
+                atomicMax(s_hi, j >> 5);
+            }
+        }
+    }
+    __syncthreads();
+    return *s_over == 0;
+}
+
+__global__ void __launch_bounds__(SET_THREADS) asm_sets_grow_kernel(SetJob* __restrict__ jobs, const DevHierLevel* __restrict__ hier,
+                                                                      const long long* __restrict__ bm_off, int L, int eta, int num_ghost) {
+    SetJob& J = jobs[blockIdx.x];
+    __shared__ int s_count, s_lo, s_hi, s_over, s_nseed;
+    int* bufA = J.frontier;
+    int* bufB = J.frontier + SET_FRONTIER_CAP;
+    int* seeds = J.frontier + 2 * SET_FRONTIER_CAP;
+    if (threadIdx.x == 0) { s_over = 0; s_nseed = J.n_owned <= SET_FRONTIER_CAP ? J.n_owned : 0; if (J.n_owned > SET_FRONTIER_CAP) s_over = 1; }
+    __syncthreads();
+    for (int q = threadIdx.x; q < s_nseed; q += SET_THREADS) seeds[q] = J.owned[q];       // B_0^p = Omega_0^p
+    __syncthreads();
+    for (int l = 0; l <= L && s_over == 0; ++l) {
+        const DevHierLevel H = hier[l];
+        SetLevelOut& o = J.out[l];
+        if (l == L) {                                                    // reading A5: D_L^p = Omega_L, no ghosts
+            if (threadIdx.x == 0) { o.n_real = (int)H.n; o.n_ghost = 0; o.lo_word = 0; o.hi_word = -1; }
+            break;
+        }
+        unsigned* real = J.bm_real + bm_off[l];
+        unsigned* ghost = J.bm_ghost + bm_off[l];
+        const int nseed = s_nseed;
+        if (threadIdx.x == 0) { s_count = 0; s_lo = INT_MAX; s_hi = -1; }
+        __syncthreads();
+        for (int q = threadIdx.x; q < nseed; q += SET_THREADS) {         // the seeds are distinct
+            const int i = seeds[q];
+            atomicOr(real + (i >> 5), 1u << (i & 31));
+            bufA[q] = i;
+            atomicMin(&s_lo, i >> 5);
+            atomicMax(&s_hi, i >> 5);
+        }
+        __syncthreads();
+        int n_real = nseed, ncur = nseed;
+        int* cur = bufA;
+        int* nxt = bufB;
+        for (int d = 0; d < eta && ncur > 0; ++d) {                       // D_l^p: within eta of B_l^p
+            if (!grow_layer(H.A, cur, ncur, real, nullptr, nxt, &s_count, &s_lo, &s_hi, &s_over)) break;
+            ncur = s_count;
+            n_real += ncur;
+            __syncthreads();
+            if (threadIdx.x == 0) s_count = 0;
+            __syncthreads();
+            int* t = cur; cur = nxt; nxt = t;
+        }
+        if (s_over) break;
+        // ghost layers: only the points of the last real layer can have neighbours outside D_l^p
+        int n_ghost = 0;
+        for (int d = 0; d < num_ghost && ncur > 0; ++d) {
+            if (!grow_layer(H.A, cur, ncur, ghost, real, nxt, &s_count, &s_lo, &s_hi, &s_over)) break;
+            ncur = s_count;
+            n_ghost += ncur;
+            __syncthreads();
+            if (threadIdx.x == 0) s_count = 0;
+            __syncthreads();
+            int* t = cur; cur = nxt; nxt = t;
+        }
+        if (s_over) break;
+        if (threadIdx.x == 0) { o.n_real = n_real; o.n_ghost = n_ghost; o.lo_word = s_lo == INT_MAX ? 0 : s_lo; o.hi_word = s_hi; s_nseed = 0; }
+        __syncthreads();
+        // B_{l+1}^p: coarse images of the C-points of D_l^p (order does not matter)
+        const int lo = s_lo == INT_MAX ? 0 : s_lo, hi = s_hi;
+        for (int w = lo + threadIdx.x; w <= hi; w += SET_THREADS) {
+            unsigned bits = real[w];
+            while (bits) {
+                const int b = __ffs(bits) - 1;
+                bits &= bits - 1;
+                const int i = 32 * w + b;
+                if (H.cf[i] > 0) {
+                    const int pos = atomicAdd(&s_nseed, 1);
+                    if (pos < SET_FRONTIER_CAP) seeds[pos] = H.coarse_of[i]; else s_over = 1;
+                }
+            }
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) J.overflow = s_over;
+}
+
+// ascending extraction of a bitmap range into dst (returns the count); clears the words; all threads of the CTA
+__device__ int extract_sorted(unsigned* bm, int lo, int hi, int* dst, int* s_scan, const DevHierLevel& H, bool is_real,
+                              unsigned long long* s_sumA, unsigned long long* s_sumP) {
+    int base = 0;
+    unsigned long long sumA = 0, sumP = 0;
+    for (int w0 = lo; w0 <= hi; w0 += SET_THREADS) {
+        const int w = w0 + threadIdx.x;
+        unsigned bits = w <= hi ? bm[w] : 0u;
+        if (w <= hi && bits) bm[w] = 0u;
+        const int cnt = __popc(bits);
+        // block exclusive scan of cnt
+        s_scan[threadIdx.x] = cnt;
+        __syncthreads();
+        for (int off = 1; off < SET_THREADS; off <<= 1) {
+            const int v = threadIdx.x >= off ? s_scan[threadIdx.x - off] : 0;
+            __syncthreads();
+            s_scan[threadIdx.x] += v;
+            __syncthreads();
+        }
+        int pos = base + s_scan[threadIdx.x] - cnt;
+        const int total = s_scan[SET_THREADS - 1];
+        while (bits) {
+            const int b = __ffs(bits) - 1;
+            bits &= bits - 1;
+            const int i = 32 * w + b;
+            if (dst) dst[pos] = i;
+            ++pos;
+            sumA += (unsigned long long)(H.A.rp[i + 1] - H.A.rp[i]);
+            if (H.P.rp) sumP += (unsigned long long)(H.P.rp[i + 1] - H.P.rp[i]);
+        }
+        base += total;
+        __syncthreads();
+    }
+    if (sumA) atomicAdd(s_sumA, sumA);
+    if (sumP) atomicAdd(s_sumP, sumP);
+    (void)is_real;
+    return base;
+}
+
+__global__ void __launch_bounds__(SET_THREADS) asm_sets_extract_kernel(SetJob* __restrict__ jobs, const DevHierLevel* __restrict__ hier,
+                                                                         const long long* __restrict__ bm_off, int L) {
+    SetJob& J = jobs[blockIdx.x];
+    __shared__ int s_scan[SET_THREADS];
+    __shared__ unsigned long long s_sumA, s_sumP, s_sumAg;
+    for (int l = 0; l <= L; ++l) {
+        const DevHierLevel H = hier[l];
+        SetLevelOut& o = J.out[l];
+        if (threadIdx.x == 0) { s_sumA = 0; s_sumP = 0; s_sumAg = 0; }
+        __syncthreads();
+        if (l == L || o.n_real == (int)H.n) {
+            // the whole level (shared copy): nothing to extract; the sums over the whole level; bitmaps still to be cleared
+            if (l < L) {
+                unsigned* real = J.bm_real + bm_off[l];
+                unsigned* ghost = J.bm_ghost + bm_off[l];
+                for (int w = o.lo_word + threadIdx.x; w <= o.hi_word; w += SET_THREADS) { real[w] = 0u; ghost[w] = 0u; }
+            }
+            if (threadIdx.x == 0) {
+                o.nnzA_real = H.A.rp[H.n]; o.nnzA_ghost_bound = 0; o.nnzP_bound = H.P.rp ? H.P.rp[H.n] : 0;
+            }
+            __syncthreads();
+            continue;
+        }
+        int* dst = J.list_dst[l];
+        unsigned* real = J.bm_real + bm_off[l];
+        unsigned* ghost = J.bm_ghost + bm_off[l];
+        const int nr = extract_sorted(real, o.lo_word, o.hi_word, dst, s_scan, H, true, &s_sumA, &s_sumP);
+        __syncthreads();
+        extract_sorted(ghost, o.lo_word, o.hi_word, dst ? dst + nr : nullptr, s_scan, H, false, &s_sumAg, &s_sumP);
+        __syncthreads();
+        if (threadIdx.x == 0) { o.nnzA_real = (long long)s_sumA; o.nnzA_ghost_bound = (long long)s_sumAg; o.nnzP_bound = (long long)s_sumP; }
+        __syncthreads();
+    }
+    // local indices (level 0) of the owned dofs: position in the ascending real list (identity on a fully covered level)
+    const SetLevelOut& o0 = J.out[0];
+    const bool shared0 = (L == 0) || o0.n_real == (int)hier[0].n;
+    const int* real0 = shared0 ? nullptr : J.list_dst[0];
+    for (int k = threadIdx.x; k < J.n_owned; k += SET_THREADS) {
+        const int g = J.owned[k];
+        int loc = g;
+        if (!shared0) {                                                // (plain loads: the list was written by this kernel)
+            int lo = 0, hi = o0.n_real;
+            while (lo < hi) { const int mid = (lo + hi) >> 1; if (real0[mid] < g) lo = mid + 1; else hi = mid; }
+            loc = lo;
+        }
+        J.owned_local_dst[k] = loc;
+    }
+}
+
 }  // namespace
 
 cudaError_t launch_asm_plan(const AsmJob* jobs, int njobs, const DevHierLevel* hier, int* row_scratch, AsmSlice* slice_scratch,
@@ -302,6 +494,17 @@ cudaError_t launch_asm_plan(const AsmJob* jobs, int njobs, const DevHierLevel* h
 cudaError_t launch_asm_write(const AsmJob* jobs, int njobs, const DevHierLevel* hier, const int* row_scratch,
                              const AsmSlice* slice_scratch, AsmPlan* plans, cudaStream_t st) {
     if (njobs > 0) asm_write_kernel<<<njobs, ASM_THREADS, 0, st>>>(jobs, hier, row_scratch, slice_scratch, plans);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_sets_grow(SetJob* jobs, int njobs, const DevHierLevel* hier, const long long* bm_off, int L, int eta, int num_ghost,
+                             cudaStream_t st) {
+    if (njobs > 0) asm_sets_grow_kernel<<<njobs, SET_THREADS, 0, st>>>(jobs, hier, bm_off, L, eta, num_ghost);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_sets_extract(SetJob* jobs, int njobs, const DevHierLevel* hier, const long long* bm_off, int L, cudaStream_t st) {
+    if (njobs > 0) asm_sets_extract_kernel<<<njobs, SET_THREADS, 0, st>>>(jobs, hier, bm_off, L);
     return cudaGetLastError();
 }
 

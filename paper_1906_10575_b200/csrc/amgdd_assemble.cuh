@@ -23,6 +23,7 @@ struct DevHierLevel {
     DevCsr64 A, P, R;           // P, R: null pointers on the coarsest level
     const double* dinv;         // l1 diagonal inverse (S8)
     const int8_t* cf;           // +1 C / -1 F; null when the level has no splitting (coarsest)
+    const int* coarse_of;       // fine index -> coarse index of a C-point (null on the coarsest level)
     long long n;
 };
 
@@ -63,6 +64,35 @@ struct AsmCopy {                // gid / owned-index copies and the gather of th
     int gather;                 // 1: dst is double*, dst[i] = dinv[src[i]]
     const double* dinv;
 };
+
+// ---- composite index sets on the device (S6, S7; eq. 1): breadth-first growth with bitmaps -----------------
+// One CTA per subdomain.  Pass 1 (asm_sets_grow) walks the levels top down: D_l^p = points within eta of B_l^p in the graph
+// of A_l, the ghost layers around it, B_{l+1}^p = coarse images of the C-points of D_l^p; membership lives in two bitmaps
+// per (subdomain, level), the frontiers in a scratch of SET_FRONTIER_CAP indices (a larger frontier raises `overflow` and
+// the host path takes the batch).  Pass 2 (asm_sets_extract) turns the bitmaps into the ascending index lists (S7) at the
+// offsets the host laid out from the sizes, sums the row lengths the layout needs, and clears the bitmaps again.
+struct SetLevelOut {            // per (subdomain, level), written by pass 1 (sizes, range) and pass 2 (sums)
+    int n_real, n_ghost;
+    int lo_word, hi_word;       // bitmap words that hold the sets (inclusive range; hi < lo: empty)
+    long long nnzA_real;        // sum of the global row lengths of A_l over D_l^p
+    long long nnzA_ghost_bound; // the same over the ghost points (bound of the local ghost rows)
+    long long nnzP_bound;       // sum of the global row lengths of P_l over D-bar_l^p
+};
+struct SetJob {
+    const int* owned;           // DEVICE: Omega_0^p, global indices ascending
+    int n_owned;
+    int overflow;               // out: a frontier exceeded the scratch
+    unsigned* bm_real;          // DEVICE scratch: bitmaps of all levels, level l at word offset bm_off[l]
+    unsigned* bm_ghost;
+    int* frontier;              // DEVICE scratch: 3 * SET_FRONTIER_CAP ints
+    SetLevelOut* out;           // DEVICE: L + 1 records
+    int* const* list_dst;       // pass 2: DEVICE array of L + 1 pointers: where real | ghost of level l go (null: shared level)
+    int* owned_local_dst;       // pass 2: n_owned local indices (level 0) of the owned dofs
+};
+constexpr int SET_FRONTIER_CAP = 1 << 18;
+cudaError_t launch_sets_grow(SetJob* jobs, int njobs, const DevHierLevel* hier, const long long* bm_off, int L, int eta, int num_ghost,
+                             cudaStream_t st);
+cudaError_t launch_sets_extract(SetJob* jobs, int njobs, const DevHierLevel* hier, const long long* bm_off, int L, cudaStream_t st);
 
 constexpr int ASM_MAX_WINDOW = 1024;
 

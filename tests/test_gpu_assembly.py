@@ -121,3 +121,41 @@ def test_large_window_falls_back_to_the_host_packer(monkeypatch):
                       p.theta, p.coarse_max)
     assert m.amgdd_get_stats(h)["assembled_on_device"] == 0
     m.amgdd_destroy(h)
+
+
+def test_index_sets_on_the_device_and_on_the_host(monkeypatch):
+    """The rest of NEXT 3: D_l^p and the ghost layers grown on the device (bitmaps, one CTA per subdomain) against the host's
+    breadth-first search (AMGDD_INDEX_SETS=host), byte for byte; a frontier that does not fit the device scratch hands the
+    batch to the host."""
+    import paper_1906_10575_b200 as m
+    for cfg, scale, kw in ((4, 48, {}), (5, 256, {}), (3, 32, {"eta": 4}), (1, 37, {"parts_per_dim": 3, "eta": 0})):
+        p = wl.make_config(cfg, scale, **kw)
+        monkeypatch.delenv("AMGDD_INDEX_SETS", raising=False)
+        try:
+            _, hd = setup(p, monkeypatch, host=False)
+        except m.AmgddError as e:                       # eta = 0 may leave interpolation stencils outside the grid (A7): both paths refuse
+            assert e.code == -6
+            monkeypatch.setenv("AMGDD_INDEX_SETS", "host")
+            with pytest.raises(m.AmgddError):
+                setup(p, monkeypatch, host=False)
+            continue
+        assert m.amgdd_get_stats(hd)["index_sets_on_device"] == 1
+        monkeypatch.setenv("AMGDD_INDEX_SETS", "host")
+        _, hs = setup(p, monkeypatch, host=False)
+        assert m.amgdd_get_stats(hs)["index_sets_on_device"] == 0
+        assert compare_blocks(m, hd, hs, p, np.arange(p.num_subdomains)) > 0
+        sd, sh = m.amgdd_get_stats(hd), m.amgdd_get_stats(hs)
+        for k in ("nnz_composite_real", "sum_real", "sum_ghost", "shared_level_instances", "stream_bytes_fac_iter", "overhead"):
+            assert sd[k] == sh[k], k
+        m.amgdd_destroy(hd); m.amgdd_destroy(hs)
+    # one subdomain that owns 640 x 640 dofs: more seeds than the frontier scratch holds
+    monkeypatch.delenv("AMGDD_INDEX_SETS", raising=False)
+    p = wl.make_config(1, 640, parts_per_dim=1)
+    _, h = setup(p, monkeypatch, host=False)
+    assert m.amgdd_get_stats(h)["index_sets_on_device"] == 0
+    import torch
+    b = torch.from_numpy(p.b).cuda()
+    x = torch.zeros(p.n, dtype=torch.float64, device="cuda")
+    res = m.amgdd_solve(h, b, x, 2)
+    assert res[2] < res[1] < res[0]
+    m.amgdd_destroy(h)
