@@ -144,9 +144,8 @@ def ncu_traffic(workload):
 def oracle_time_per_cycle(p, sample, steps, warmup, smoother=0, sample_1thread=None):
     """Times the oracle AS IT STANDS on a bounded sample: every step runs Alg. 2's global residual +
     restriction over the whole problem and AlgFAC on `sample` subdomains (spread evenly over the
-    partition); the per-cycle estimate scales the whole step by P / sample (the global part, which is run in
-    full, is a few percent of it, so the estimate is slightly high).  Timed with all host cores (one OpenMP
-    thread per core, `value`) and, on a smaller sample, with ONE thread (`value_1thread`)."""
+    partition).  Timed with all host cores (one OpenMP thread per core, `value`) and, on a smaller sample, with ONE
+    thread (`value_1thread`)."""
     from oracle import Oracle, max_threads
     t0 = time.time()
     o = Oracle(p.n, p.rowptr, p.colind, p.vals, p.theta, p.max_levels, p.coarse_max)
@@ -168,18 +167,31 @@ def oracle_time_per_cycle(p, sample, steps, warmup, smoother=0, sample_1thread=N
 
     for _ in range(max(1, warmup)):
         o.cycle(p.b, x, p.num_fac_cycles, p.relax_sweeps, subdomains=subs, nthreads=nthreads)   # also builds the composite grids (setup)
-    t_all = timed(subs, nthreads)
     n1 = max(1, min(len(subs), sample_1thread or max(1, len(subs) // 4)))
     subs1 = subs[np.unique(np.linspace(0, len(subs) - 1, n1).astype(int))]
-    t_one = timed(subs1, 1)
-    est_ms = 1e3 * float(np.mean(t_all)) * p.num_subdomains / len(subs)
-    est1_ms = 1e3 * float(np.mean(t_one)) * p.num_subdomains / len(subs1)
+    one = subs[len(subs) // 2:len(subs) // 2 + 1]
+
+    def per_cycle(sub_list, nt):
+        """A step costs g + a * (subdomains in it): g = Alg. 2's global residual + restriction (run in full every step),
+        a = AlgFAC per subdomain.  Two sample sizes give both; the cycle of the whole workload costs g + a * P."""
+        t_s, t_1 = float(np.mean(timed(sub_list, nt))), float(np.mean(timed(one, nt)))
+        if len(sub_list) > 1:
+            a = max(0.0, (t_s - t_1) / (len(sub_list) - 1))
+            g = max(0.0, t_1 - a)
+        else:
+            a, g = t_s, 0.0
+        return 1e3 * (g + a * p.num_subdomains), t_s, g
+
+    est_ms, t_all, g_all = per_cycle(subs, nthreads)
+    est1_ms, t_one, g_one = per_cycle(subs1, 1)
     return {"value": est_ms, "unit": UNIT, "cores": nthreads, "kind": "oracle",
             "value_1thread": est1_ms,
             "sample": f"all cores: {len(subs)} of {p.num_subdomains} subdomains per step, {steps} timed steps after {max(1, warmup)} "
-                      f"warm-up; one thread: {len(subs1)} subdomains per step, {steps} steps; each step also runs the global "
-                      f"residual+restriction in full; per-cycle value = mean step time x P/sample; oracle setup {setup_s:.1f}s not timed",
-            "sample_seconds_per_step": float(np.mean(t_all)), "sample_seconds_per_step_1thread": float(np.mean(t_one)),
+                      f"warm-up; one thread: {len(subs1)} subdomains per step, {steps} steps; every step also runs the global "
+                      f"residual+restriction in full, so a second timing with ONE subdomain separates that part (g) from the cost "
+                      f"per subdomain (a); per-cycle value = g + a x P; oracle setup {setup_s:.1f}s not timed",
+            "sample_seconds_per_step": t_all, "sample_seconds_per_step_1thread": t_one,
+            "global_part_seconds": g_all, "global_part_seconds_1thread": g_one,
             "steps_timed": steps, "subdomains_all_cores": int(len(subs)), "subdomains_1thread": int(len(subs1))}
 
 
