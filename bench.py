@@ -275,6 +275,8 @@ def run_b200(args, p, rank, world, local_rank):
 
     # ---- the dominant kernel: per-launch duration from the library's CUDA events on its stream ----
     x.zero_()
+    if os.environ.get("AMGDD_FAC_PROFILE", "0") == "1":
+        m.amgdd_debug_fac_op_cycles(h)                                   # clears the per-step counters
     fac_ms, launches = [], None
     for _ in range(args.steps):
         m.amgdd_solve(h, b, x, 1, nfac, nu)
@@ -283,6 +285,7 @@ def run_b200(args, p, rank, world, local_rank):
         launches = prof["launches"]
     clocks = sampler.stop()
     fac_avg_ms = float(np.mean(fac_ms))
+    fac_ops = m.amgdd_debug_fac_op_cycles(h) if os.environ.get("AMGDD_FAC_PROFILE", "0") == "1" else None   # exactly these cycles
 
     # ---- context: the paper's comparison method, one AMG V(1,1)-cycle on the same hierarchy (Alg. 1; Fig. 14-15) ----
     xv = torch.zeros(p.n, dtype=torch.float64, device="cuda")
@@ -366,6 +369,20 @@ def run_b200(args, p, rank, world, local_rank):
                 "kernel_source_hash": kernel_source_hash(),
             },
         }
+        if os.environ.get("AMGDD_FAC_PROFILE", "0") == "1":
+            # debugging aid (never a timed run): SM cycles of every step of the AlgFAC program, thread 0 of every CTA, over the cycles
+            # of the per-launch timing loop above; shares by step kind and by level
+            ops = fac_ops
+            tot = float(sum(o[2] + o[3] for o in ops)) or 1.0
+            by_kind, by_level = {}, {}
+            for kind, lvl, cyc, bar, ring, opw in ops:
+                by_kind[kind] = by_kind.get(kind, 0.0) + (cyc + bar) / tot
+                by_level[str(lvl)] = by_level.get(str(lvl), 0.0) + (cyc + bar) / tot
+            line["fac_step_profile"] = {
+                "cycles_per_subdomain_and_cycle": tot / (args.steps * p.num_subdomains), "share_by_kind": by_kind, "share_by_level": by_level,
+                "steps": [{"kind": k, "level": l, "cycles": c / (args.steps * p.num_subdomains), "barrier": bw / (args.steps * p.num_subdomains),
+                           "ring_wait": rw / (args.steps * p.num_subdomains), "operand_wait": ow / (args.steps * p.num_subdomains)}
+                          for k, l, c, bw, rw, ow in ops]}
         if not args.no_cpu_baseline:
             m.amgdd_destroy(h)
             del b, x

@@ -107,6 +107,12 @@ struct amgdd_handle_s {
     int* d_owned0_all = nullptr;                 // level 0: the dofs of every rank, rank after rank
     std::vector<long long> owned0_off;           // nranks + 1 offsets into d_owned0_all
     double* d_sq = nullptr;                      // sum of r_0^2 over the owned rows (amgdd_shard_sqnorm)
+    // one AMG-DD cycle captured as a CUDA graph (asynchronous amgdd_solve calls: 4 + L launches become one)
+    cudaGraphExec_t cycle_graph = nullptr;
+    cudaStream_t capture_stream = nullptr;
+    const double* graph_b = nullptr; double* graph_x = nullptr;
+    int graph_nfac = -1, graph_nu = -1, graph_smoother = -1, graph_nops = -1;
+    bool graph_off = false;
     bool shard_committed = false;
 };
 
@@ -159,6 +165,8 @@ void free_handle(amgdd_handle_s* h) {
     if (!h) return;
     for (void* p : h->allocs) cudaFree(p);
     for (cudaEvent_t e : h->events) cudaEventDestroy(e);
+    if (h->cycle_graph) cudaGraphExecDestroy(h->cycle_graph);
+    if (h->capture_stream) cudaStreamDestroy(h->capture_stream);
     delete h;
 }
 
@@ -1143,6 +1151,49 @@ int amgdd_solve(amgdd_handle_t h, const double* b, double* x, int32_t num_cycles
     }
     const FacParams prm = fac_params(h, x);
     long long launches[3] = {0, 0, 0};
+    // Asynchronous calls (no norms wanted, no phase timers): the cycle is a fixed sequence of 4 + L launches on fixed
+    // pointers, so it is captured once as a CUDA graph (on a stream of the handle's own: the caller's may be the legacy
+    // default stream, which cannot capture) and replayed on the caller's stream.  AMGDD_GRAPH=0 launches kernel by kernel.
+    if (!timed && num_cycles > 0 && !h->graph_off) {
+        const bool hit = h->cycle_graph && h->graph_b == b && h->graph_x == x && h->graph_nfac == num_fac_cycles &&
+                         h->graph_nu == relax_sweeps && h->graph_smoother == h->smoother && h->graph_nops == h->prog_nops;
+        if (!hit) {
+            if (env_int("AMGDD_GRAPH", 1) <= 0) h->graph_off = true;
+            if (h->cycle_graph) { cudaGraphExecDestroy(h->cycle_graph); h->cycle_graph = nullptr; }
+            if (!h->graph_off && !h->capture_stream && cudaStreamCreateWithFlags(&h->capture_stream, cudaStreamNonBlocking) != cudaSuccess) h->graph_off = true;
+            if (!h->graph_off) {
+                cudaStream_t user = h->stream;
+                cudaGraph_t graph = nullptr;
+                bool ok = cudaStreamBeginCapture(h->capture_stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+                if (ok) {
+                    h->stream = h->capture_stream;
+                    enqueue_residual(h, b, x, h->d_r_all, 0);
+                    for (int l = 0; l < L; ++l) {
+                        const GlobalLevelDev& g = h->glev[l];
+                        launch_spmv(g.r_rp, g.r_ci, g.r_v, h->H.lv[l + 1].A.nrows, g.lanes_r, h->d_r_all + h->r_off[l],
+                                    h->d_r_all + h->r_off[l + 1], h->stream);
+                    }
+                    ok = cudaMemsetAsync(h->d_counter, 0, sizeof(int), h->stream) == cudaSuccess;
+                    launch_fac(prm, h->fac_cfg, h->stream);
+                    h->stream = user;
+                    ok = (cudaStreamEndCapture(h->capture_stream, &graph) == cudaSuccess) && ok && graph != nullptr;
+                }
+                if (ok) ok = cudaGraphInstantiate(&h->cycle_graph, graph, 0) == cudaSuccess;
+                if (graph) cudaGraphDestroy(graph);
+                if (!ok) { cudaGetLastError(); h->cycle_graph = nullptr; h->graph_off = true; }
+                else {
+                    h->graph_b = b; h->graph_x = x; h->graph_nfac = num_fac_cycles; h->graph_nu = relax_sweeps;
+                    h->graph_smoother = h->smoother; h->graph_nops = h->prog_nops;
+                }
+            }
+        }
+        if (h->cycle_graph) {
+            for (int k = 0; k < num_cycles; ++k) CUDA_TRY(cudaGraphLaunch(h->cycle_graph, h->stream));
+            launches[0] = 2LL * num_cycles; launches[1] = (long long)L * num_cycles; launches[2] = num_cycles;
+            for (int i = 0; i < 3; ++i) h->prof_launches[i] = launches[i];
+            return AMGDD_SUCCESS;
+        }
+    }
     mark();
     for (int k = 0; k < num_cycles; ++k) {
         enqueue_residual(h, b, x, h->d_r_all, k);                                   // Alg. 2 P:471 (+ a11)
