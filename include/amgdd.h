@@ -136,8 +136,11 @@ int amgdd_setup(int64_t n, const int64_t* rowptr, const int32_t* colind, const d
  *   relax_sweeps  nu: l1-Jacobi sweeps before and after each coarse correction (>= 1; V(nu,nu))
  *   resnorm_host  HOST, num_cycles+1 doubles or NULL.  resnorm[k] = || b - A_0 x_k ||_2, k = 0 is
  *                 the initial guess.  With NULL the call only enqueues work on the handle's
- *                 stream and returns (and the norm of the final iterate is not evaluated);
- *                 otherwise it synchronises the stream before returning.
+ *                 stream and returns (and the norm of the final iterate is not evaluated): the 4 + L
+ *                 launches of a cycle are captured once as a CUDA graph (per b, x, num_fac_cycles,
+ *                 relax_sweeps) and replayed, one graph launch per cycle; AMGDD_GRAPH=0 in the
+ *                 environment launches kernel by kernel.  Otherwise the call synchronises the stream
+ *                 before returning.
  * Limits: the steps of one subdomain's cycle form a static program of at most 1024 steps, about
  * num_fac_cycles * (L * (4 + 2 * relax_sweeps) + 1) (twice the relaxation steps with the CF smoother), and the
  * kernel's tables hold at most 85 levels (L <= 84): AMGDD_ERR_BAD_ARG with the step count in the detail string
