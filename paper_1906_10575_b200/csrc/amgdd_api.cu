@@ -30,6 +30,9 @@ struct GlobalLevelDev {          // the single device copy of a whole level
     int* a_rp = nullptr; int* a_ci = nullptr; double* a_v = nullptr;
     int* r_rp = nullptr; int* r_ci = nullptr; double* r_v = nullptr;
     int lanes_a = 2, lanes_r = 2;
+    // row blocks of the CSR stream kernel (amgdd_kernels.cuh) for A_0 and R_l
+    int* a_blk = nullptr; int a_nblk = 0;
+    int* r_blk = nullptr; int r_nblk = 0;
     // packed streams for the AlgFAC kernel, present when some subdomain covers the whole level
     char* sA = nullptr; char* sP = nullptr; char* sR = nullptr;
     StreamLayout layA, layP, layR;
@@ -160,6 +163,22 @@ int upload_csr32(amgdd_handle_s* h, const HostCsr& M, int** rp, int** ci, double
 }
 
 double avg_row(const HostCsr& M) { return M.nrows ? (double)M.nnz() / (double)M.nrows : 1.0; }
+
+// blocks of consecutive rows for the CSR stream kernel: at most stream_block_rows() rows and stream_block_nnz() entries
+// (a row longer than that is a block of its own); returns the nblk + 1 row offsets
+std::vector<int> stream_row_blocks(const HostCsr& M) {
+    const i64 max_rows = stream_block_rows(), max_nnz = stream_block_nnz();
+    std::vector<int> blk(1, 0);
+    i64 r = 0;
+    while (r < M.nrows) {
+        i64 e = r;
+        while (e < M.nrows && e - r < max_rows && M.rp[e + 1] - M.rp[r] <= max_nnz) ++e;
+        if (e == r) e = r + 1;
+        blk.push_back((int)e);
+        r = e;
+    }
+    return blk;
+}
 
 void free_handle(amgdd_handle_s* h) {
     if (!h) return;
@@ -758,10 +777,18 @@ int finish_tables(amgdd_handle_s* h) {
         GlobalLevelDev& g = h->glev[l];
         g.lanes_a = pick_lanes(avg_row(lv.A));
         if (l < L) g.lanes_r = pick_lanes(avg_row(lv.R));
-        if (l == 0)
+        if (l == 0) {
             if ((rc = upload_csr32(h, lv.A, &g.a_rp, &g.a_ci, &g.a_v))) return rc;   // Alg. 2
-        if (l < L)
+            const std::vector<int> blk = stream_row_blocks(lv.A);
+            g.a_nblk = (int)blk.size() - 1;
+            if ((rc = upload(h, &g.a_blk, blk.data(), blk.size()))) return rc;
+        }
+        if (l < L) {
             if ((rc = upload_csr32(h, lv.R, &g.r_rp, &g.r_ci, &g.r_v))) return rc;   // Alg. 2 P:473 needs every R_l
+            const std::vector<int> blk = stream_row_blocks(lv.R);
+            g.r_nblk = (int)blk.size() - 1;
+            if ((rc = upload(h, &g.r_blk, blk.data(), blk.size()))) return rc;
+        }
         if (need[l]) {
             if ((rc = upload_packed(h, lv.A, lv.dinv.data(), &lv.cf, &g.sA, g.layA, "A", l))) return rc;
             if (l < L) {
@@ -862,7 +889,7 @@ int finish_tables(amgdd_handle_s* h) {
     if ((rc = upload(h, &h->d_lu, h->H.lu.data(), h->H.lu.size()))) return rc;
     if ((rc = upload(h, &h->d_rowperm, h->H.rowperm.data(), h->H.rowperm.size()))) return rc;
     if (L > 0) { if ((rc = upload(h, &h->d_cf0, h->H.lv[0].cf.data(), h->H.lv[0].cf.size()))) return rc; }
-    h->partial_cap = residual_num_blocks(h->n, h->glev[0].lanes_a);
+    h->partial_cap = std::max(h->glev[0].a_nblk, residual_num_blocks(h->n, 1));          // stream blocks, or 256 listed rows per block
     if ((rc = dev_alloc(h, (void**)&h->d_partial, (size_t)h->partial_cap * sizeof(double)))) return rc;
     h->norms_cap = 1024;
     if ((rc = dev_alloc(h, (void**)&h->d_norms, (size_t)h->norms_cap * sizeof(double)))) return rc;
@@ -1113,7 +1140,8 @@ FacParams fac_params(amgdd_handle_s* h, double* x) {
 int enqueue_residual(amgdd_handle_s* h, const double* b, const double* x, double* r, int norm_slot) {
     const GlobalLevelDev& g = h->glev[0];
     int nb = 0;
-    launch_residual(g.a_rp, g.a_ci, g.a_v, h->n, g.lanes_a, b, x, r, h->d_partial, &nb, h->stream);
+    nb = g.a_nblk;
+    launch_residual(g.a_rp, g.a_ci, g.a_v, g.a_blk, g.a_nblk, b, x, r, h->d_partial, h->stream);
     launch_norm_finalize(h->d_partial, nb, h->d_norms + norm_slot, h->stream);
     return AMGDD_SUCCESS;
 }
@@ -1170,7 +1198,7 @@ int amgdd_solve(amgdd_handle_t h, const double* b, double* x, int32_t num_cycles
                     enqueue_residual(h, b, x, h->d_r_all, 0);
                     for (int l = 0; l < L; ++l) {
                         const GlobalLevelDev& g = h->glev[l];
-                        launch_spmv(g.r_rp, g.r_ci, g.r_v, h->H.lv[l + 1].A.nrows, g.lanes_r, h->d_r_all + h->r_off[l],
+                        launch_spmv(g.r_rp, g.r_ci, g.r_v, g.r_blk, g.r_nblk, h->d_r_all + h->r_off[l],
                                     h->d_r_all + h->r_off[l + 1], h->stream);
                     }
                     ok = cudaMemsetAsync(h->d_counter, 0, sizeof(int), h->stream) == cudaSuccess;
@@ -1201,7 +1229,7 @@ int amgdd_solve(amgdd_handle_t h, const double* b, double* x, int32_t num_cycles
         mark();
         for (int l = 0; l < L; ++l) {                                               // Alg. 2
             const GlobalLevelDev& g = h->glev[l];
-            launch_spmv(g.r_rp, g.r_ci, g.r_v, h->H.lv[l + 1].A.nrows, g.lanes_r, h->d_r_all + h->r_off[l],
+            launch_spmv(g.r_rp, g.r_ci, g.r_v, g.r_blk, g.r_nblk, h->d_r_all + h->r_off[l],
                         h->d_r_all + h->r_off[l + 1], h->stream);
             launches[1] += 1;
         }
@@ -1324,7 +1352,7 @@ int amgdd_vcycle(amgdd_handle_t h, const double* b, double* x, int32_t num_cycle
                 }
             if (!have_u) CUDA_TRY(cudaMemsetAsync(g.vu0, 0, (size_t)nrows(l) * sizeof(double), st));
             launch_spmv_axpy(g.a_rp, g.a_ci, g.a_v, nrows(l), g.lanes_a, g.vu0, f, g.vr, 0, st);        // r = f - A u
-            launch_spmv(g.r_rp, g.r_ci, g.r_v, nrows(l + 1), g.lanes_r, g.vr, h->glev[l + 1].vf, st);   // f_{l+1} = P^T r
+            launch_spmv(g.r_rp, g.r_ci, g.r_v, g.r_blk, g.r_nblk, g.vr, h->glev[l + 1].vf, st);         // f_{l+1} = P^T r
         }
         launch_coarse_solve(h->d_lu, h->d_rowperm, (int)h->H.nL, L == 0 ? b : h->glev[L].vf, L == 0 ? x : h->glev[L].vu0, st);
         for (int l = L - 1; l >= 0; --l) {                                      // upsweep P:459-464
@@ -1532,11 +1560,11 @@ int amgdd_shard_stage_pack(amgdd_handle_t h, int32_t stage, const double* b, con
         if (l == 0) {
             const GlobalLevelDev& g = h->glev[0];
             int nb = 0;
-            launch_residual_rows(g.a_rp, g.a_ci, g.a_v, h->d_owned_rows[0], nrows, g.lanes_a, b, x, h->d_r_all, h->d_partial, &nb, h->stream);
+            launch_residual_rows(g.a_rp, g.a_ci, g.a_v, h->d_owned_rows[0], nrows, b, x, h->d_r_all, h->d_partial, &nb, h->stream);
             launch_sum_finalize(h->d_partial, nb, h->d_sq, h->stream);
         } else {
             const GlobalLevelDev& g = h->glev[l - 1];
-            launch_spmv_rows(g.r_rp, g.r_ci, g.r_v, h->d_owned_rows[l], nrows, g.lanes_r, h->d_r_all + h->r_off[l - 1], h->d_r_all + h->r_off[l], h->stream);
+            launch_spmv_rows(g.r_rp, g.r_ci, g.r_v, h->d_owned_rows[l], nrows, h->d_r_all + h->r_off[l - 1], h->d_r_all + h->r_off[l], h->stream);
         }
     }
     const amgdd_handle_s::StageDev& d = h->stage_dev[stage];

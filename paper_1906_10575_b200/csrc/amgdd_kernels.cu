@@ -12,36 +12,91 @@ namespace {
 // ---------------------------------------------------------------------------------------------
 constexpr int GLOBAL_BLOCK = 256;
 
-// `rows` (optional): the kernel works on the n listed rows instead of rows 0 .. n-1 (sharded cycle: the rows a rank
-// owns); the arithmetic of a row is the same either way
-__global__ void __launch_bounds__(GLOBAL_BLOCK) residual_kernel(const int* __restrict__ rp, const int* __restrict__ ci,
-                                                                const double* __restrict__ v, long long n, int lanes,
-                                                                const double* __restrict__ b, const double* __restrict__ x,
-                                                                double* __restrict__ r, double* __restrict__ partial,
-                                                                const int* __restrict__ rows) {
+// Row sums of the global kernels (a1, a2): the entries of a row are multiplied and added ONE BY ONE in stored order
+// (__dmul_rn, __dadd_rn: no contraction), whichever kernel computes the row -- the whole-matrix "CSR stream" kernel below
+// or the row-list kernel of the sharded cycle -- so a row's result does not depend on who owns it.
+constexpr int STREAM_ROWS = 256;             // rows of a block of the stream kernel (one thread per row in the second phase)
+constexpr int STREAM_NNZ = 2304;             // entries of a block (their products wait in shared memory)
+
+// y = M x (MODE 0) or r = b - M x with per-block sums of r^2 (MODE 1) over consecutive rows.  Block k owns the rows
+// [blk[k], blk[k+1]) (host-built: at most STREAM_ROWS rows and STREAM_NNZ entries; a longer row is a block of its own).
+// Phase 1: all threads walk the block's contiguous entries (coalesced loads of values and columns, x gathered through
+// L2) and leave the products in shared memory; phase 2: thread t adds the products of row t in order.
+template <int MODE>
+__global__ void __launch_bounds__(GLOBAL_BLOCK) csr_stream_kernel(const int* __restrict__ rp, const int* __restrict__ ci,
+                                                                  const double* __restrict__ v, const int* __restrict__ blk,
+                                                                  const double* __restrict__ x, const double* __restrict__ b,
+                                                                  double* __restrict__ y, double* __restrict__ partial) {
+    __shared__ double prod[STREAM_NNZ];
+    __shared__ int srp[STREAM_ROWS + 1];
     __shared__ double red[GLOBAL_BLOCK / 32];
-    const int lane = threadIdx.x & (lanes - 1);
-    const long long idx = (long long)blockIdx.x * (GLOBAL_BLOCK / lanes) + threadIdx.x / lanes;
-    const long long row = (rows && idx < n) ? (long long)__ldg(rows + idx) : idx;
-    double sum = 0.0;
-    if (idx < n) {
-        const int bgn = __ldg(rp + row), end = __ldg(rp + row + 1);
-        for (int k = bgn + lane; k < end; k += lanes) sum += __ldg(v + k) * __ldg(x + __ldg(ci + k));
-    }
-    for (int o = lanes >> 1; o > 0; o >>= 1) sum += __shfl_down_sync(0xffffffffu, sum, o, lanes);
-    double sq = 0.0;
-    if (idx < n && lane == 0) {
-        const double ri = b[row] - sum;
-        if (r) r[row] = ri;
-        sq = ri * ri;
-    }
-    for (int o = 16; o > 0; o >>= 1) sq += __shfl_down_sync(0xffffffffu, sq, o);
-    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = sq;
+    const int r0 = __ldg(blk + blockIdx.x), r1 = __ldg(blk + blockIdx.x + 1), n = r1 - r0;
+    for (int t = threadIdx.x; t <= n; t += GLOBAL_BLOCK) srp[t] = __ldg(rp + r0 + t);
     __syncthreads();
-    if (threadIdx.x == 0) {
-        double tot = 0.0;
-        for (int k = 0; k < GLOBAL_BLOCK / 32; ++k) tot += red[k];
-        partial[blockIdx.x] = tot;
+    const int e0 = srp[0], e1 = srp[n];
+    double sq = 0.0;
+    if (e1 - e0 <= STREAM_NNZ) {
+        for (int e = e0 + threadIdx.x; e < e1; e += GLOBAL_BLOCK) prod[e - e0] = __dmul_rn(__ldg(v + e), __ldg(x + __ldg(ci + e)));
+        __syncthreads();
+        if (threadIdx.x < n) {
+            double sum = 0.0;
+            for (int k = srp[threadIdx.x] - e0; k < srp[threadIdx.x + 1] - e0; ++k) sum = __dadd_rn(sum, prod[k]);
+            const int row = r0 + threadIdx.x;
+            if (MODE == 1) {
+                const double ri = b[row] - sum;
+                if (y) y[row] = ri;
+                sq = ri * ri;
+            } else y[row] = sum;
+        }
+    } else if (threadIdx.x == 0) {             // one row longer than a block holds: the same order, one thread
+        double sum = 0.0;
+        for (int e = e0; e < e1; ++e) sum = __dadd_rn(sum, __dmul_rn(__ldg(v + e), __ldg(x + __ldg(ci + e))));
+        if (MODE == 1) {
+            const double ri = b[r0] - sum;
+            if (y) y[r0] = ri;
+            sq = ri * ri;
+        } else y[r0] = sum;
+    }
+    if (MODE == 1) {
+        for (int o = 16; o > 0; o >>= 1) sq += __shfl_down_sync(0xffffffffu, sq, o);
+        if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = sq;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double tot = 0.0;
+            for (int k = 0; k < GLOBAL_BLOCK / 32; ++k) tot += red[k];
+            partial[blockIdx.x] = tot;
+        }
+    }
+}
+
+// the same rows for a LIST of rows (sharded cycle: the rows a rank owns), one thread per row
+template <int MODE>
+__global__ void __launch_bounds__(GLOBAL_BLOCK) csr_rows_kernel(const int* __restrict__ rp, const int* __restrict__ ci,
+                                                                const double* __restrict__ v, const int* __restrict__ rows, long long n,
+                                                                const double* __restrict__ x, const double* __restrict__ b,
+                                                                double* __restrict__ y, double* __restrict__ partial) {
+    __shared__ double red[GLOBAL_BLOCK / 32];
+    const long long idx = (long long)blockIdx.x * GLOBAL_BLOCK + threadIdx.x;
+    double sq = 0.0;
+    if (idx < n) {
+        const int row = __ldg(rows + idx);
+        double sum = 0.0;
+        for (int k = __ldg(rp + row); k < __ldg(rp + row + 1); ++k) sum = __dadd_rn(sum, __dmul_rn(__ldg(v + k), __ldg(x + __ldg(ci + k))));
+        if (MODE == 1) {
+            const double ri = b[row] - sum;
+            if (y) y[row] = ri;
+            sq = ri * ri;
+        } else y[row] = sum;
+    }
+    if (MODE == 1) {
+        for (int o = 16; o > 0; o >>= 1) sq += __shfl_down_sync(0xffffffffu, sq, o);
+        if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = sq;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double tot = 0.0;
+            for (int k = 0; k < GLOBAL_BLOCK / 32; ++k) tot += red[k];
+            partial[blockIdx.x] = tot;
+        }
     }
 }
 
@@ -57,22 +112,6 @@ __global__ void __launch_bounds__(1024) norm_finalize_kernel(const double* __res
         for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
         if (threadIdx.x == 0) out[0] = sqrt(s);
     }
-}
-
-__global__ void __launch_bounds__(GLOBAL_BLOCK) spmv_kernel(const int* __restrict__ rp, const int* __restrict__ ci,
-                                                            const double* __restrict__ v, long long n, int lanes,
-                                                            const double* __restrict__ x, double* __restrict__ y,
-                                                            const int* __restrict__ rows) {
-    const int lane = threadIdx.x & (lanes - 1);
-    const long long idx = (long long)blockIdx.x * (GLOBAL_BLOCK / lanes) + threadIdx.x / lanes;
-    const long long row = (rows && idx < n) ? (long long)__ldg(rows + idx) : idx;
-    double sum = 0.0;
-    if (idx < n) {
-        const int bgn = __ldg(rp + row), end = __ldg(rp + row + 1);
-        for (int k = bgn + lane; k < end; k += lanes) sum += __ldg(v + k) * __ldg(x + __ldg(ci + k));
-    }
-    for (int o = lanes >> 1; o > 0; o >>= 1) sum += __shfl_down_sync(0xffffffffu, sum, o, lanes);
-    if (idx < n && lane == 0) y[row] = sum;
 }
 
 // pack / unpack of one exchange stage of the sharded cycle (positions: 64-bit into x or the residual vector; 32-bit dof lists)
@@ -191,25 +230,26 @@ int residual_num_blocks(long long n, int lanes) {
     return (int)((n + rows_per_block - 1) / rows_per_block);
 }
 
-void launch_residual(const int* rp, const int* ci, const double* v, long long n, int lanes, const double* b,
-                     const double* x, double* r, double* partial, int* nblocks_out, void* stream) {
-    const int nb = residual_num_blocks(n, lanes);
-    residual_kernel<<<nb, GLOBAL_BLOCK, 0, (cudaStream_t)stream>>>(rp, ci, v, n, lanes, b, x, r, partial, nullptr);
-    if (nblocks_out) *nblocks_out = nb;
+int stream_block_rows() { return STREAM_ROWS; }
+int stream_block_nnz() { return STREAM_NNZ; }
+
+void launch_residual(const int* rp, const int* ci, const double* v, const int* blk, int nblk, const double* b,
+                     const double* x, double* r, double* partial, void* stream) {
+    if (nblk > 0) csr_stream_kernel<1><<<nblk, GLOBAL_BLOCK, 0, (cudaStream_t)stream>>>(rp, ci, v, blk, x, b, r, partial);
 }
 
-void launch_residual_rows(const int* rp, const int* ci, const double* v, const int* rows, long long nrows, int lanes, const double* b,
+void launch_residual_rows(const int* rp, const int* ci, const double* v, const int* rows, long long nrows, const double* b,
                           const double* x, double* r, double* partial, int* nblocks_out, void* stream) {
-    const int nb = residual_num_blocks(nrows, lanes);
-    if (nb > 0) residual_kernel<<<nb, GLOBAL_BLOCK, 0, (cudaStream_t)stream>>>(rp, ci, v, nrows, lanes, b, x, r, partial, rows);
+    const int nb = (int)((nrows + GLOBAL_BLOCK - 1) / GLOBAL_BLOCK);
+    if (nb > 0) csr_rows_kernel<1><<<nb, GLOBAL_BLOCK, 0, (cudaStream_t)stream>>>(rp, ci, v, rows, nrows, x, b, r, partial);
     if (nblocks_out) *nblocks_out = nb;
 }
 
-void launch_spmv_rows(const int* rp, const int* ci, const double* v, const int* rows, long long nrows, int lanes, const double* x,
+void launch_spmv_rows(const int* rp, const int* ci, const double* v, const int* rows, long long nrows, const double* x,
                       double* y, void* stream) {
     if (nrows <= 0) return;
-    const int nb = residual_num_blocks(nrows, lanes);
-    spmv_kernel<<<nb, GLOBAL_BLOCK, 0, (cudaStream_t)stream>>>(rp, ci, v, nrows, lanes, x, y, rows);
+    const int nb = (int)((nrows + GLOBAL_BLOCK - 1) / GLOBAL_BLOCK);
+    csr_rows_kernel<0><<<nb, GLOBAL_BLOCK, 0, (cudaStream_t)stream>>>(rp, ci, v, rows, nrows, x, nullptr, y, nullptr);
 }
 
 void launch_gather(const double* src, const long long* pos, long long n, double* dst, void* stream) {
@@ -232,11 +272,9 @@ void launch_norm_finalize(const double* partial, int nb, double* out, void* stre
     norm_finalize_kernel<<<1, 1024, 0, (cudaStream_t)stream>>>(partial, nb, out);
 }
 
-void launch_spmv(const int* rp, const int* ci, const double* v, long long nrows, int lanes, const double* x,
+void launch_spmv(const int* rp, const int* ci, const double* v, const int* blk, int nblk, const double* x,
                  double* y, void* stream) {
-    if (nrows <= 0) return;
-    const int nb = residual_num_blocks(nrows, lanes);
-    spmv_kernel<<<nb, GLOBAL_BLOCK, 0, (cudaStream_t)stream>>>(rp, ci, v, nrows, lanes, x, y, nullptr);
+    if (nblk > 0) csr_stream_kernel<0><<<nblk, GLOBAL_BLOCK, 0, (cudaStream_t)stream>>>(rp, ci, v, blk, x, nullptr, y, nullptr);
 }
 
 }  // namespace amgdd
