@@ -128,6 +128,21 @@ def test_shard_index_sets_against_brute_force(cfg, scale, R, kw):
     check_everything(p, R, build_plans(p, R))
 
 
+def test_shard_degenerate_hierarchies():
+    """L = 0 (the whole problem is the coarsest level: every rank sends all it owns to every other rank, reading A5) and
+    eta = 0 (Psi = the points adjacent to nothing: only Psi_c structures and the halos move)."""
+    import copy
+    p = copy.copy(wl.make_config(1, 7, parts_per_dim=2))
+    p.coarse_max = 64
+    check_everything(p, 2, build_plans(p, 2))
+    p = wl.make_config(2, 16, parts_per_dim=2, eta=0)
+    o = oracle_of(p)
+    x = np.zeros(p.n)
+    o.cycle(p.b, x, 1, 1)
+    if o.dropped() == 0:                                  # (with eta = 0 the composite grids may not be closed under interpolation, A7)
+        check_everything(p, 2, build_plans(p, 2))
+
+
 def test_one_rank_exchanges_nothing():
     import paper_1906_10575_b200 as m
     p = wl.make_config(1)
