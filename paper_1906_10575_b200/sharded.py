@@ -106,12 +106,17 @@ def run_index_protocol(plans, comm):
                 amgdd_shard_plan_apply_drop(plans[s], stage, d, back[s][d])
 
 
+_STAGE_CACHE = {}
+
+
 def setup_exchange(handles, comm):
     """After amgdd_setup_shard on every rank: index protocol, then upload of the final lists."""
     plans = {r: amgdd_get_shard_plan(h) for r, h in handles.items()}
     run_index_protocol(plans, comm)
     for h in handles.values():
         amgdd_shard_commit(h)
+        for key in [k for k in _STAGE_CACHE if k[0] == id(h)]:
+            del _STAGE_CACHE[key]
     return plans
 
 
@@ -125,8 +130,11 @@ def sharded_cycle(handles, b, x, comm, num_fac_cycles=2, relax_sweeps=1, want_no
     for stage in range(nstages):
         sc, rc, bufs = {}, {}, {}
         for r, h in handles.items():
-            sc[r], rc[r] = amgdd_shard_stage_counts(h, stage, R)
-            bufs[r] = torch.empty(int(sc[r].sum()), dtype=torch.float64, device=x[r].device)
+            key = (id(h), stage)
+            if key not in _STAGE_CACHE:                                    # counts and the send buffer of a stage never change
+                s_cnt, r_cnt = amgdd_shard_stage_counts(h, stage, R)
+                _STAGE_CACHE[key] = (s_cnt, r_cnt, torch.empty(int(s_cnt.sum()), dtype=torch.float64, device=x[r].device))
+            sc[r], rc[r], bufs[r] = _STAGE_CACHE[key]
             amgdd_shard_stage_pack(h, stage, b[r], x[r], bufs[r])
         if want_norm and stage == 1:                                       # the owned rows' r_0 was just computed
             sq = comm.allreduce_sum({r: amgdd_shard_sqnorm(h) for r, h in handles.items()})
