@@ -398,6 +398,32 @@ def test_async_solve_on_torch_stream():
     assert np.isclose(m.amgdd_residual_norm(h, b, x2), ref[-1], rtol=1e-14)
 
 
+def test_graph_replay_matches_kernel_by_kernel_launches(monkeypatch):
+    """An asynchronous amgdd_solve replays the cycle as a CUDA graph (captured per b, x, num_fac_cycles, relax_sweeps,
+    smoother); AMGDD_GRAPH=0 launches kernel by kernel.  Same kernels, same order: the iterates must be bit-identical, also
+    when the program changes between calls (re-capture) and when x lives in another tensor."""
+    torch = _torch()
+    p = wl.make_config(4, 48)
+    out = {}
+    for graph in ("1", "0"):
+        monkeypatch.setenv("AMGDD_GRAPH", graph)
+        m, h = lib_setup(p)
+        b = torch.from_numpy(p.b).cuda()
+        x = torch.zeros(p.n, dtype=torch.float64, device="cuda")
+        m.amgdd_solve(h, b, x, 2, 2, 1, want_norms=False)
+        m.amgdd_solve(h, b, x, 1, 3, 2, want_norms=False)          # another program
+        m.amgdd_set_smoother(h, 1)
+        m.amgdd_solve(h, b, x, 1, 3, 2, want_norms=False)          # another smoother, same shape of call
+        x2 = x.clone()
+        m.amgdd_set_smoother(h, 0)
+        m.amgdd_solve(h, b, x2, 2, 2, 1, want_norms=False)         # another x
+        torch.cuda.synchronize()
+        out[graph] = (x.cpu().numpy(), x2.cpu().numpy(), m.amgdd_residual_norm(h, b, x2))
+        m.amgdd_destroy(h)
+    assert np.array_equal(out["1"][0], out["0"][0]) and np.array_equal(out["1"][1], out["0"][1])
+    assert out["1"][2] == out["0"][2] and out["1"][2] < 1e-2 * np.linalg.norm(p.b)
+
+
 def test_stats_and_overhead_definition():
     # P:293-299 overhead through the library's stats equals the oracle's
     p = wl.make_config(2, 32)

@@ -62,6 +62,28 @@ def test_sharded_cycle_is_bit_identical(cfg, scale, R, kw):
     m.amgdd_destroy(href)
 
 
+def test_sharded_cycle_with_the_cf_smoother_and_two_sweeps():
+    import torch
+    from paper_1906_10575_b200.sharded import sharded_cycle
+    p = wl.make_config(2, 32)
+    R = 4
+    m, handles, comm, plans = _setup(p, R)
+    own0 = torch.from_numpy(m.amgdd_shard_plan_owner_rank(plans[0], 0)).cuda()
+    href = m.amgdd_setup(p.n, p.rowptr, p.colind, p.vals, p.num_subdomains, p.owner, p.eta, p.num_ghost, p.max_levels, p.theta, p.coarse_max)
+    for h in list(handles.values()) + [href]:
+        m.amgdd_set_smoother(h, 1)
+    b = torch.from_numpy(p.b).cuda()
+    xr = torch.zeros(p.n, dtype=torch.float64, device="cuda")
+    x = {r: torch.zeros(p.n, dtype=torch.float64, device="cuda") for r in range(R)}
+    for k in range(2):
+        m.amgdd_solve(href, b, xr, 1, 3, 2)
+        sharded_cycle(handles, {r: b for r in range(R)}, x, comm, 3, 2)
+        xs = torch.zeros_like(xr)
+        for r in range(R):
+            xs[own0 == r] = x[r][own0 == r]
+        assert torch.equal(xs, xr)
+
+
 def test_shard_handle_reports_local_subdomains():
     import paper_1906_10575_b200 as m
     p = wl.make_config(2, 32)
