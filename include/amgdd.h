@@ -262,12 +262,12 @@ int amgdd_shard_unpack_owned(amgdd_handle_t h, int32_t src_rank, const double* b
  * [n_real, nrows) are two row groups (real / ghost rows of a composite A_l); inside
  * windows of `window` rows (multiple of 32 in [32, 1048576]) rows are sorted by descending length
  * and cut into slices of 32 rows, one warp lane per row; a slice is stored as K = max(1,
- * ceil(longest row / 4)) groups of 4 steps (zero padding past the end of a row) and one 512-byte
- * header {row, K, aux} per lane; the slices are dealt to AMGDD_NUM_WAYS sub-streams ("ways", one
- * per warp of the kernel).
- *   aux      HOST, nrows doubles stored in the slice headers (the l1 diagonal inverse), or NULL (0.0)
- *   row_flags  HOST, nrows bytes (0/1) stored in bit 31 of the header's info word (C-point of the row's level), or NULL
- *   wide     0: uint16 column indices (needs every column < 65536), 1: uint32
+ * ceil(longest row / 4)) groups of 4 steps (zero padding past the end of a row) and one header of 4 bytes
+ * per lane (narrow: row | K << 16 | flag << 31; 0xFFFF: no row) or 8 bytes per lane (wide: row, K | flag << 31);
+ * the slices are dealt to AMGDD_NUM_WAYS sub-streams ("ways", one per warp of the kernel).  The l1 diagonal
+ * a relaxing step needs is not part of the stream (the kernel fetches it like the other row-local operands).
+ *   row_flags  HOST, nrows bytes (0/1) stored in bit 31 of the header word (C-point of the row's level), or NULL
+ *   wide     0: uint16 column indices and rows (needs every column < 65536 and at most 65535 rows), 1: uint32
  *   out_ways HOST, AMGDD_NUM_WAYS entries, or NULL
  * With out = NULL only *out_bytes and out_ways are computed.  Returns AMGDD_ERR_INDEX_RANGE for a
  * row with more than 65535 entries, AMGDD_ERR_BAD_ARG on a bad argument or if out_capacity is too
@@ -275,7 +275,8 @@ int amgdd_shard_unpack_owned(amgdd_handle_t h, int32_t src_rank, const double* b
 #define AMGDD_NUM_WAYS 16
 #define AMGDD_GROUP_BYTES_NARROW 1280
 #define AMGDD_GROUP_BYTES_WIDE 1536
-#define AMGDD_HEADER_BYTES 512
+#define AMGDD_HEADER_BYTES_NARROW 128
+#define AMGDD_HEADER_BYTES_WIDE 256
 typedef struct amgdd_way {
     uint32_t grp_off128;   /* the way's groups start 128 * grp_off128 bytes from the start of the stream */
     uint32_t hdr_off128;   /* its slice headers start 128 * hdr_off128 bytes from the start of the stream */
@@ -286,7 +287,7 @@ typedef struct amgdd_way {
     uint32_t reserved[2];
 } amgdd_way_t;
 int amgdd_pack_stream(int32_t nrows, int32_t n_real, const int32_t* rowptr32, const int32_t* colind, const double* vals,
-                      const double* aux, const uint8_t* row_flags, int32_t wide, int32_t window, void* out,
+                      const uint8_t* row_flags, int32_t wide, int32_t window, void* out,
                       int64_t out_capacity, int64_t* out_bytes, amgdd_way_t* out_ways);
 
 /* ---- measurement support ------------------------------------------------------------------

@@ -79,7 +79,7 @@ def _load():
     L.amgdd_debug_fac_cycles.argtypes = [_vp, _vp, _i32]
     L.amgdd_debug_fac_op_cycles.argtypes = [_vp, _vp, _i32, _vp]
     L.amgdd_debug_read_block.argtypes = [_vp, _i32, _i32, _i32, _vp, _i64, _vp]
-    L.amgdd_pack_stream.argtypes = [_i32, _i32, _vp, _vp, _vp, _vp, _vp, _i32, _i32, _vp, _i64, _vp, _vp]
+    L.amgdd_pack_stream.argtypes = [_i32, _i32, _vp, _vp, _vp, _vp, _i32, _i32, _vp, _i64, _vp, _vp]
     L.amgdd_setup_shard.argtypes = [_i64, _vp, _vp, _vp, _i32, _vp, _i32, _i32, _i32, _f64, _i32, _i32, _i32, ctypes.POINTER(_vp)]
     L.amgdd_shard_plan_create.argtypes = [_i64, _vp, _vp, _vp, _i32, _vp, _i32, _i32, _f64, _i32, _i32, _i32, ctypes.POINTER(_vp)]
     L.amgdd_shard_plan_destroy.argtypes = [_vp]
@@ -260,24 +260,23 @@ def amgdd_get_stats(h: Handle) -> dict:
 
 
 NUM_WAYS = 16
-GROUP_BYTES_NARROW, GROUP_BYTES_WIDE, HEADER_BYTES = 1280, 1536, 512
+GROUP_BYTES_NARROW, GROUP_BYTES_WIDE, HEADER_BYTES_NARROW, HEADER_BYTES_WIDE = 1280, 1536, 128, 256
 WAY_DTYPE = np.dtype([("grp_off128", np.uint32), ("hdr_off128", np.uint32), ("ngroups", np.uint32), ("ngroups_real", np.uint32),
                       ("nslices", np.uint32), ("nslices_real", np.uint32), ("reserved", np.uint32, (2,))])
 
 
-def amgdd_pack_stream(rowptr, colind, vals, wide=False, n_real=None, aux=None, window=256, row_flags=None):
+def amgdd_pack_stream(rowptr, colind, vals, wide=False, n_real=None, window=256, row_flags=None):
     """amgdd_pack_stream: CSR (host) -> (bytes of the packed SELL-32 group streams as a uint8 array, the
     NUM_WAYS way descriptors as a structured array)."""
     rowptr = _np(rowptr, np.int32)
     colind = _np(colind, np.int32)
     vals = _np(vals, np.float64)
-    aux = None if aux is None else _np(aux, np.float64)
     row_flags = None if row_flags is None else _np(row_flags, np.uint8)
     nrows = len(rowptr) - 1
     n_real = nrows if n_real is None else n_real
     nbytes = _i64()
     ways = np.zeros(NUM_WAYS, dtype=WAY_DTYPE)
-    args = (nrows, n_real, rowptr.ctypes.data, colind.ctypes.data, vals.ctypes.data, None if aux is None else aux.ctypes.data,
+    args = (nrows, n_real, rowptr.ctypes.data, colind.ctypes.data, vals.ctypes.data,
             None if row_flags is None else row_flags.ctypes.data, int(wide), window)
     _check(lib.amgdd_pack_stream(*args, None, 0, ctypes.byref(nbytes), ways.ctypes.data))
     out = np.zeros(max(nbytes.value, 1), dtype=np.uint8)

@@ -582,7 +582,7 @@ int build_composites_device(amgdd_handle_s* h, const std::vector<i32>& owner, in
                     j.nr = b.n_real; j.ng = b.n_ghost; j.nrc = c.n_real; j.ngc = c.n_ghost;
                     j.gid = gidp[k][l]; j.gidc = gidp[k][l + 1];
                     j.window = kind == ASM_A ? h->window : thin;
-                    j.wide = (kind == ASM_P ? nbc : nb) > NARROW_MAX_COLS;
+                    j.wide = needs_wide(j.nrows, kind == ASM_P ? nbc : nb);
                     j.scratch_row = row_off; j.scratch_slice = slice_off;
                     row_off += 2LL * j.nrows;
                     slice_off += (j.nrows_first + SLICE_ROWS - 1) / SLICE_ROWS + (j.nrows - j.nrows_first + SLICE_ROWS - 1) / SLICE_ROWS;
@@ -620,7 +620,7 @@ int build_composites_device(amgdd_handle_s* h, const std::vector<i32>& owner, in
                 return AMGDD_ERR_INDEX_RANGE;
             }
             StreamLayout& sl = r.kind == ASM_A ? b.A : (r.kind == ASM_P ? b.P : b.R);
-            sl.nrows = jobs[q].nrows; sl.nnz = pl.nnz; sl.wide = jobs[q].wide != 0; sl.has_aux = r.kind != ASM_P;
+            sl.nrows = jobs[q].nrows; sl.nnz = pl.nnz; sl.wide = jobs[q].wide != 0;
             sl.bytes = pl.bytes; sl.bytes_real = pl.bytes_real; sl.padded_nnz = pl.padded_nnz;
             for (int w = 0; w < NUM_WAYS; ++w) sl.way[w] = pl.way[w];
             if (r.kind == ASM_A) { b.nnzA = pl.nnz; b.nnzA_ghost = b.nnzA - b.nnzA_real; }
@@ -649,7 +649,7 @@ int build_composites_device(amgdd_handle_s* h, const std::vector<i32>& owner, in
                 if (b.shared) continue;
                 c.src = gidp[k][l]; c.dst = (int*)(sm.dev_base + b.off_gid); c.n = b.n_real + b.n_ghost; c.gather = 0; c.dinv = nullptr;
                 copies.push_back(c);
-                c.dst = (int*)(sm.dev_base + b.off_dinv); c.n = b.n_real; c.gather = 1; c.dinv = hier[l].dinv;
+                c.dst = (int*)(sm.dev_base + b.off_dinv); c.n = b.n_real + b.n_ghost; c.n_gather = b.n_real; c.gather = 1; c.dinv = hier[l].dinv;
                 copies.push_back(c);
             }
         }
@@ -743,17 +743,17 @@ StreamDesc make_desc(const char* base, const StreamLayout& lay, bool shared = fa
     std::memset(&d, 0, sizeof(d));
     d.base = base;
     for (int w = 0; w < NUM_WAYS; ++w) d.way[w] = lay.way[w];
-    d.flags = (lay.wide ? STREAM_WIDE : 0u) | (lay.has_aux ? STREAM_AUX : 0u) | (shared ? STREAM_SHARED : 0u);
+    d.flags = (lay.wide ? STREAM_WIDE : 0u) | (shared ? STREAM_SHARED : 0u);
     return d;
 }
 
-int upload_packed(amgdd_handle_s* h, const HostCsr& M, const double* aux, const std::vector<int8_t>* cf, char** dptr, StreamLayout& lay, const char* what, int l) {
+int upload_packed(amgdd_handle_s* h, const HostCsr& M, const std::vector<int8_t>* cf, char** dptr, StreamLayout& lay, const char* what, int l) {
     std::vector<uint8_t> flags;                                      // C-points of the rows' level (CF smoother)
     if (cf && !cf->empty()) { flags.resize(cf->size()); for (size_t i = 0; i < cf->size(); ++i) flags[i] = (*cf)[i] > 0 ? 1 : 0; }
     const int window = what[0] == 'A' ? h->window : std::min(h->window, THIN_WINDOW);
     PackedLevelStream ps;
     i64 bad = -1;
-    if (!pack_global_stream(M, aux, flags.empty() ? nullptr : flags.data(), window, ps, bad)) { g_detail = "a level matrix has more than 2^31-1 nonzeros"; return AMGDD_ERR_INDEX_RANGE; }
+    if (!pack_global_stream(M, flags.empty() ? nullptr : flags.data(), window, ps, bad)) { g_detail = "a level matrix has more than 2^31-1 nonzeros"; return AMGDD_ERR_INDEX_RANGE; }
     if (bad >= 0) {
         g_detail = std::string("row ") + std::to_string(bad) + " of " + what + "_" + std::to_string(l) + " has more than 65535 entries";
         return AMGDD_ERR_INDEX_RANGE;
@@ -790,10 +790,10 @@ int finish_tables(amgdd_handle_s* h) {
             if ((rc = upload(h, &g.r_blk, blk.data(), blk.size()))) return rc;
         }
         if (need[l]) {
-            if ((rc = upload_packed(h, lv.A, lv.dinv.data(), &lv.cf, &g.sA, g.layA, "A", l))) return rc;
+            if ((rc = upload_packed(h, lv.A, &lv.cf, &g.sA, g.layA, "A", l))) return rc;
             if (l < L) {
-                if ((rc = upload_packed(h, lv.P, nullptr, nullptr, &g.sP, g.layP, "P", l))) return rc;
-                if ((rc = upload_packed(h, lv.R, h->H.lv[l + 1].dinv.data(), &h->H.lv[l + 1].cf, &g.sR, g.layR, "R", l))) return rc;
+                if ((rc = upload_packed(h, lv.P, nullptr, &g.sP, g.layP, "P", l))) return rc;
+                if ((rc = upload_packed(h, lv.R, &h->H.lv[l + 1].cf, &g.sR, g.layR, "R", l))) return rc;
             }
             if ((rc = upload(h, &g.dinv, lv.dinv.data(), lv.dinv.size()))) return rc;
             std::vector<int> id((size_t)lv.A.nrows);
@@ -1638,7 +1638,7 @@ int amgdd_shard_unpack_owned(amgdd_handle_t h, int32_t src_rank, const double* b
 }
 
 int amgdd_pack_stream(int32_t nrows, int32_t n_real, const int32_t* rowptr32, const int32_t* colind, const double* vals,
-                      const double* aux, const uint8_t* row_flags, int32_t wide, int32_t window, void* out, int64_t out_capacity,
+                      const uint8_t* row_flags, int32_t wide, int32_t window, void* out, int64_t out_capacity,
                       int64_t* out_bytes, amgdd_way_t* out_ways) {
     g_detail.clear();
     if (nrows < 0 || n_real < 0 || n_real > nrows || !rowptr32 || (!colind && rowptr32[nrows] > 0) ||
@@ -1650,16 +1650,18 @@ int amgdd_pack_stream(int32_t nrows, int32_t n_real, const int32_t* rowptr32, co
         if (rowptr32[i + 1] < rowptr32[i]) { g_detail = "row pointers not monotone"; return AMGDD_ERR_BAD_ARG; }
         if (rowptr32[i + 1] - rowptr32[i] > 65535) { g_detail = "row " + std::to_string(i) + " has more than 65535 entries"; return AMGDD_ERR_INDEX_RANGE; }
     }
-    if (!wide)
+    if (!wide) {
+        if (nrows > NARROW_MAX_ROWS) { g_detail = "more than 65535 rows need the wide form"; return AMGDD_ERR_BAD_ARG; }
         for (int32_t k = 0; k < rowptr32[nrows]; ++k)
             if (colind[k] < 0 || colind[k] >= NARROW_MAX_COLS) { g_detail = "column index needs the wide form"; return AMGDD_ERR_BAD_ARG; }
-    const PackPlan pp = plan_stream(nrows, rowptr32, wide != 0, aux != nullptr, n_real, window);
+    }
+    const PackPlan pp = plan_stream(nrows, rowptr32, wide != 0, n_real, window);
     if (out_bytes) *out_bytes = pp.bytes;
     static_assert(sizeof(amgdd_way_t) == sizeof(WayDesc), "amgdd_way_t mirrors WayDesc");
     if (out_ways) std::memcpy(out_ways, pp.way, sizeof(pp.way));
     if (out) {
         if (out_capacity < pp.bytes) { g_detail = "output buffer too small"; return AMGDD_ERR_BAD_ARG; }
-        write_stream(nrows, rowptr32, colind, vals, aux, wide != 0, n_real, window, (char*)out, row_flags);
+        write_stream(nrows, rowptr32, colind, vals, wide != 0, n_real, window, (char*)out, row_flags);
     }
     return AMGDD_SUCCESS;
 }
@@ -1714,7 +1716,7 @@ int amgdd_debug_read_block(amgdd_handle_t h, int32_t p, int32_t level, int32_t w
     else if (!b.shared) {
         switch (which) {
             case 0: off = b.off_gid; bytes = 4LL * (b.n_real + b.n_ghost); break;
-            case 1: off = b.off_dinv; bytes = 8LL * b.n_real; break;
+            case 1: off = b.off_dinv; bytes = 8LL * (b.n_real + b.n_ghost); break;
             case 2: off = b.A.off; bytes = b.A.bytes; break;
             case 3: off = b.P.off; bytes = b.P.bytes; break;
             default: off = b.R.off; bytes = b.R.bytes; break;

@@ -158,6 +158,7 @@ __global__ void __launch_bounds__(ASM_THREADS) asm_plan_kernel(const AsmJob* __r
     if (tid < 32) {
         const int lane = tid;
         const long long gbytes = J.wide ? GROUP_BYTES_WIDE : GROUP_BYTES_NARROW;
+        const long long hbytes = J.wide ? HEADER_BYTES_WIDE : HEADER_BYTES_NARROW;
         long long load = 0;
         uint32_t ngr = 0, nsl = 0, ngr_first = 0, nsl_first = 0;
         for (int s = 0; s < S; ++s) {
@@ -172,14 +173,14 @@ __global__ void __launch_bounds__(ASM_THREADS) asm_plan_kernel(const AsmJob* __r
             }
             if (lane == best) {
                 sl[s].way = (uint32_t)lane; sl[s].g_off = ngr; sl[s].h_idx = nsl;
-                load += (long long)K * gbytes + HEADER_BYTES;
+                load += (long long)K * gbytes + hbytes;
                 ngr += K; nsl += 1;
                 if (s < S0) { ngr_first += K; nsl_first += 1; }
             }
         }
         // offsets: all groups way by way, then all headers way by way (128-byte units; both sizes are multiples of 128)
         const unsigned long long gb128 = (unsigned long long)ngr * (unsigned long long)(gbytes / 128);
-        const unsigned long long hb128 = (unsigned long long)nsl * (HEADER_BYTES / 128);
+        const unsigned long long hb128 = ((unsigned long long)nsl * (unsigned long long)hbytes + 127ull) / 128ull;      // a way's headers end 128-byte aligned
         unsigned long long gpre = gb128, hpre = hb128;                // inclusive scans over the lanes
 #pragma unroll
         for (int off = 1; off < 32; off <<= 1) {
@@ -206,7 +207,7 @@ __global__ void __launch_bounds__(ASM_THREADS) asm_plan_kernel(const AsmJob* __r
         }
         if (lane == 0) {
             pl.bytes = (long long)((gtot + htot) * 128ull);
-            pl.bytes_real = (long long)tgf * gbytes + (long long)tsf * HEADER_BYTES;
+            pl.bytes_real = (long long)tgf * gbytes + (long long)tsf * hbytes;
             pl.padded_nnz = (long long)tg * GROUP_STEPS * SLICE_ROWS;
             pl.nnz = (long long)s_nnz;
             pl.dropped = s_dropped;
@@ -239,22 +240,16 @@ __global__ void __launch_bounds__(ASM_THREADS) asm_write_kernel(const AsmJob* __
         int pos, cnt;
         slice_span(J, s, pos, cnt);
         const int row = lane < cnt ? order[pos + lane] : -1;
-        char* h = J.dst + 128ll * pl.way[rec.way].hdr_off128 + (long long)rec.h_idx * HEADER_BYTES;
+        char* h = J.dst + 128ll * pl.way[rec.way].hdr_off128 + (long long)rec.h_idx * (J.wide ? HEADER_BYTES_WIDE : HEADER_BYTES_NARROW);
         char* g = J.dst + 128ll * pl.way[rec.way].grp_off128 + (long long)rec.g_off * gbytes;
-        {   // header: {row, K | flag << 31, aux}
-            double aux = 0.0;
+        {   // header: narrow row | K << 16 | flag << 31; wide { row, K | flag << 31 }
             uint32_t flag = 0;
             if (J.kind != ASM_P && row >= 0 && row < rreal) {
                 const int gp = rgid ? __ldg(rgid + row) : row;
-                aux = Hr.dinv[gp];
                 if (Hr.cf != nullptr && Hr.cf[gp] > 0) flag = 0x80000000u;
             }
-            uint4 w;
-            w.x = row >= 0 ? (uint32_t)row : NO_ROW;
-            w.y = rec.K | flag;
-            w.z = (uint32_t)__double_as_longlong(aux);
-            w.w = (uint32_t)(__double_as_longlong(aux) >> 32);
-            *reinterpret_cast<uint4*>(h + 16 * lane) = w;
+            if (J.wide) *reinterpret_cast<uint2*>(h + 8 * lane) = make_uint2(row >= 0 ? (uint32_t)row : NO_ROW, rec.K | flag);
+            else *reinterpret_cast<uint32_t*>(h + 4 * lane) = (row >= 0 ? (uint32_t)row : (uint32_t)NO_ROW16) | (rec.K << 16) | flag;
         }
         RowCursor c;
         int mylen = 0;
@@ -285,7 +280,7 @@ __global__ void __launch_bounds__(ASM_THREADS) asm_copy_kernel(const AsmCopy* __
     const AsmCopy c = jobs[blockIdx.x];
     if (c.gather) {
         double* d = reinterpret_cast<double*>(c.dst);
-        for (int i = threadIdx.x; i < c.n; i += ASM_THREADS) d[i] = c.dinv[c.src[i]];
+        for (int i = threadIdx.x; i < c.n; i += ASM_THREADS) d[i] = i < c.n_gather ? c.dinv[c.src[i]] : 0.0;
     } else {
         for (int i = threadIdx.x; i < c.n; i += ASM_THREADS) c.dst[i] = c.src[i];
     }

@@ -61,8 +61,10 @@ struct AsmCopy {                // gid / owned-index copies and the gather of th
     const int* src;             // DEVICE ints
     int* dst;                   // DEVICE
     int n;
-    int gather;                 // 1: dst is double*, dst[i] = dinv[src[i]]
+    int gather;                 // 1: dst is double*, dst[i] = dinv[src[i]] for i < n_gather, 0.0 behind (ghost points)
     const double* dinv;
+    int n_gather;
+    int pad_;
 };
 
 // ---- composite index sets on the device (S6, S7; eq. 1): breadth-first growth with bitmaps -----------------

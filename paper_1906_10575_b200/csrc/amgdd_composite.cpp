@@ -7,15 +7,13 @@
 // ghost points D-bar_l^p \ D_l^p in ascending global index get n_real..n_real+n_ghost-1.
 // Stored per private (subdomain, level):
 //   gid   int32[n_bar]            global index of every local point
-//   dinv  double[n_real]          l1 diagonal of the full global row (S8)
+//   dinv  double[n_bar]           l1 diagonal inverse of the full global row (S8); 0.0 on the ghost points
 //   A     packed stream, n_bar rows: real rows hold the whole global row (all columns lie in
 //         D-bar_l by eq. 1); ghost rows hold only their real columns (t_l vanishes off D_l,
 //         P:230, A12)
 //   P     packed stream, n_bar rows, columns local to level l+1 (rows over all of D-bar_l)
 //   R     packed stream, n_bar(l+1) rows, columns local to level l: the explicit transpose of the
-//         local P, so restriction is a gather with a fixed summation order (no atomics); its slice
-//         headers carry the l1 diagonal of level l+1 (the restriction's epilogue starts the
-//         relaxation of level l+1)
+//         local P, so restriction is a gather with a fixed summation order (no atomics)
 // (stream format: amgdd_stream.hpp).  A level on which D_l^p = Omega_l (always true on L, reading
 // A5) is "shared": nothing is stored for it, the single global copy of the level is used (P:57
 // "each processor stores the entire coarsest grid ... may be true for a few of the coarsest grids").
@@ -29,16 +27,15 @@ namespace amgdd {
 
 namespace {
 
-void layout_stream(const LocalCsr& M, int nrows, int ncols, bool has_aux, int window, int n_real, StreamLayout& s,
+void layout_stream(const LocalCsr& M, int nrows, int ncols, int window, int n_real, StreamLayout& s,
                    i64& too_long_row) {
     s.nrows = nrows;
     s.nnz = M.rp[nrows];
-    s.wide = ncols > NARROW_MAX_COLS;
-    s.has_aux = has_aux;
+    s.wide = needs_wide(nrows, ncols);
     for (int i = 0; i < nrows && too_long_row < 0; ++i)
         if (M.rp[i + 1] - M.rp[i] > 65535) too_long_row = i;             // group counts of a slice stay small
     if (too_long_row >= 0) return;
-    const PackPlan pp = plan_stream(nrows, M.rp.data(), s.wide, has_aux, n_real, window);
+    const PackPlan pp = plan_stream(nrows, M.rp.data(), s.wide, n_real, window);
     s.bytes = pp.bytes;
     s.bytes_real = pp.bytes_real;
     s.padded_nnz = pp.padded_nnz;
@@ -193,9 +190,9 @@ void CompositeBuilder::plan_matrices(SubdomainBlob& out) {
                 R.ci[pos] = i; R.v[pos] = P.v[k];
             }
         i64 bad = -1;
-        layout_stream(A, nb, nb, true, window_, nr, b.A, bad);
-        layout_stream(P, nb, nbc, false, thin_window(), nb, b.P, bad);
-        layout_stream(R, nbc, nb, true, thin_window(), nbc, b.R, bad);
+        layout_stream(A, nb, nb, window_, nr, b.A, bad);
+        layout_stream(P, nb, nbc, thin_window(), nb, b.P, bad);
+        layout_stream(R, nbc, nb, thin_window(), nbc, b.R, bad);
         if (bad >= 0 && out.too_long_row < 0) { out.too_long_row = bad; out.too_long_level = l; }
     }
 }
@@ -211,7 +208,7 @@ void layout_blob(SubdomainBlob& out) {
         if (b.shared) continue;
         const i64 nb = (i64)b.n_real + b.n_ghost;
         b.off_gid = take(nb * 4);
-        b.off_dinv = take((i64)b.n_real * 8);
+        b.off_dinv = take(nb * 8);                       // n_bar entries: 0.0 on the ghost points (they never relax, A4)
         b.A.off = take(b.A.bytes);
         b.P.off = take(b.P.bytes);
         b.R.off = take(b.R.bytes);
@@ -236,37 +233,33 @@ void CompositeBuilder::fill(const SubdomainBlob& plan, char* dst) {
         std::memcpy(gid + nr, ghost_[l].data(), (size_t)ng * 4);
         double* dinv = (double*)(dst + b.off_dinv);
         for (i32 i = 0; i < nr; ++i) dinv[i] = lv.dinv[gid[i]];
+        for (i32 i = nr; i < nb; ++i) dinv[i] = 0.0;                     // ghost rows never relax (A4)
         const i32 nbc = plan.lev[l + 1].n_real + plan.lev[l + 1].n_ghost;
-        aux_.assign((size_t)nb, 0.0);                                    // ghost rows never relax (A4)
-        for (i32 i = 0; i < nr; ++i) aux_[i] = dinv[i];
         flg_.assign((size_t)nb, 0);                                      // C-points among the real rows (CF smoother)
         for (i32 i = 0; i < nr; ++i) flg_[i] = lv.cf[gid[i]] > 0 ? 1 : 0;
-        write_stream(nb, A_[l].rp.data(), A_[l].ci.data(), A_[l].v.data(), aux_.data(), b.A.wide, nr, window_, dst + b.A.off, flg_.data());
-        write_stream(nb, P_[l].rp.data(), P_[l].ci.data(), P_[l].v.data(), nullptr, b.P.wide, nb, thin_window(), dst + b.P.off);
-        {   // R_l rows are the points of level l+1: aux = their l1 diagonal (real points), 0 on ghosts; flag = their C/F class
+        write_stream(nb, A_[l].rp.data(), A_[l].ci.data(), A_[l].v.data(), b.A.wide, nr, window_, dst + b.A.off, flg_.data());
+        write_stream(nb, P_[l].rp.data(), P_[l].ci.data(), P_[l].v.data(), b.P.wide, nb, thin_window(), dst + b.P.off);
+        {   // R_l rows are the points of level l+1: flag = their C/F class
             const BlockLayout& c = plan.lev[l + 1];
             const HostLevel& lc = H_.lv[l + 1];
-            auxr_.assign((size_t)nbc, 0.0);
             flg_.assign((size_t)nbc, 0);
-            for (i32 i = 0; i < c.n_real; ++i) {
-                auxr_[i] = lc.dinv[real_[l + 1][i]];
+            for (i32 i = 0; i < c.n_real; ++i)
                 if (!lc.cf.empty()) flg_[i] = lc.cf[real_[l + 1][i]] > 0 ? 1 : 0;
-            }
-            write_stream(nbc, R_[l].rp.data(), R_[l].ci.data(), R_[l].v.data(), auxr_.data(), b.R.wide, nbc, thin_window(), dst + b.R.off, flg_.data());
+            write_stream(nbc, R_[l].rp.data(), R_[l].ci.data(), R_[l].v.data(), b.R.wide, nbc, thin_window(), dst + b.R.off, flg_.data());
         }
     }
 }
 
-bool pack_global_stream(const HostCsr& M, const double* aux, const uint8_t* row_flags, int window, PackedLevelStream& out, i64& too_long_row) {
+bool pack_global_stream(const HostCsr& M, const uint8_t* row_flags, int window, PackedLevelStream& out, i64& too_long_row) {
     if (M.nnz() > (i64)INT32_MAX || M.nrows > (i64)INT32_MAX) return false;
     LocalCsr T;
     T.rp.assign(M.rp.begin(), M.rp.end());
     i64 bad = -1;
-    layout_stream(T, (int)M.nrows, (int)M.ncols, aux != nullptr, window, (int)M.nrows, out.lay, bad);
+    layout_stream(T, (int)M.nrows, (int)M.ncols, window, (int)M.nrows, out.lay, bad);
     too_long_row = bad;
     if (bad >= 0) return true;
     out.data.assign((size_t)out.lay.bytes, 0);
-    write_stream((int)M.nrows, T.rp.data(), M.ci.data(), M.v.data(), aux, out.lay.wide, (int)M.nrows, window, out.data.data(), row_flags);
+    write_stream((int)M.nrows, T.rp.data(), M.ci.data(), M.v.data(), out.lay.wide, (int)M.nrows, window, out.data.data(), row_flags);
     return true;
 }
 

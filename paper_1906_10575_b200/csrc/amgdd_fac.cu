@@ -39,17 +39,10 @@ constexpr int D = RING_DEPTH;
 #ifndef AMGDD_SINGLE_BUFFER
 #define AMGDD_SINGLE_BUFFER 0
 #endif
-#ifndef AMGDD_STAGE2
-#define AMGDD_STAGE2 0
-#endif
 #ifndef AMGDD_EARLY_COMMIT
 #define AMGDD_EARLY_COMMIT 1     // commit every batch of asynchronous copies where it is issued (0: cp.async.wait_all at the wait)
 #endif
-#if AMGDD_STAGE2
-constexpr int STAGE_BYTES = 512 + 4 * 256 + 2 * 1024;   // per warp: slice 0's header, four {row, info} slots, two operand slots (e0 | e1 | e2 | aux)
-#else
 constexpr int STAGE_BYTES = 512 + 3 * 256;     // per warp: one slice header + three operand vectors of 32 doubles
-#endif
 
 // slots of the optional per-CTA cycle counters (FAC_PROF_SLOTS each; amgdd_debug_fac_cycles)
 enum ProfSlot { PROF_SYNC = 0, PROF_SETUP = 1, PROF_PRE = 2, PROF_PRIME = 3, PROF_TOTAL = 4, PROF_OP0 = 5 };   // PROF_OP0 + OpKind
@@ -100,14 +93,14 @@ __device__ __forceinline__ Grp load_grp(const char* p, int lane, uint64_t pol) {
     return g;
 }
 // asynchronous copies global -> shared (LDGSTS): they complete on their own scoreboard
-__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
-}
 __device__ __forceinline__ void cp_async8(uint32_t dst, const void* src) {
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
 }
+__device__ __forceinline__ void cp_async4(uint32_t dst, const void* src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst), "l"(src) : "memory");
+}
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-#if AMGDD_EARLY_COMMIT && !AMGDD_STAGE2
+#if AMGDD_EARLY_COMMIT
 // every batch of copies is committed where it is issued (cp_async_issued), so the wait does not plant a new
 // completion marker behind the ring's loads that were issued in between
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
@@ -116,17 +109,14 @@ __device__ __forceinline__ void cp_async_issued() { cp_async_commit(); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_issued() {}
 #endif
-#if AMGDD_STAGE2
-__device__ __forceinline__ void cp_async_wait_pending(int) { asm volatile("cp.async.wait_group 1;" ::: "memory"); }
 __device__ __forceinline__ uint32_t lds_u32(uint32_t a) {
     uint32_t v;
     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a));
     return v;
 }
-#endif
-__device__ __forceinline__ uint4 lds128(uint32_t a) {
-    uint4 v;
-    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a));
+__device__ __forceinline__ uint2 lds_u64(uint32_t a) {
+    uint2 v;
+    asm volatile("ld.shared.v2.u32 {%0,%1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(a));
     return v;
 }
 __device__ __forceinline__ double lds_f64(uint32_t a) {
@@ -365,8 +355,9 @@ struct Worker {
         // small lane-private staging area in shared memory, filled by cp.async one slice ahead:
         // asynchronous copies complete on their own scoreboard, so waiting for them does not wait
         // for the ring's loads in flight (all ordinary global loads of a warp share one).
-        //   stage:  H  32 x 16 bytes  header of the next slice (after the last slice: slice 0 of the next mat-vec)
-        //           C  3 x 32 x 8 bytes  operands e0 | e1 | e2 of the current slice's epilogue
+        //   stage:  H  32 x 4 (wide: 8) bytes  header of the next slice (after the last slice: slice 0 of the next mat-vec)
+        //           D  32 x 8 bytes at 256    the l1 diagonal inverse of the current slice's rows (where the step relaxes)
+        //           C  3 x 32 x 8 bytes at 512  operands e0 | e1 | e2 of the current slice's epilogue
         if (n == 0) {
             // Nothing to do for this warp in this step (a stream with fewer slices than ways): use the time
             // to fetch the first block and the first header of the next mat-vec, so that the steps on the
@@ -381,64 +372,48 @@ struct Worker {
                     for (int d = 0; d < D; ++d) rb[d] = load_grp<WIDE>(nxt + (long long)(d < next_last ? d : next_last) * GB, lane, pol_nxt);
                 }
                 cp_async_wait_all();
-                cp_async16(stage + 16 * lane, nxt_hdr + 16 * lane);
+                if (WIDE) cp_async8(stage + 8 * lane, nxt_hdr + 8 * lane);
+                else cp_async4(stage + 4 * lane, nxt_hdr + 4 * lane);
                 cp_async_issued();
             }
             tock(PROF_OP0 + kind, tp0);
             return;
         }
-#if AMGDD_STAGE2
-        // Two slices deep: a ring of four {row, info} header slots and of two operand slots (e0 | e1 | e2 | aux),
-        // ring positions by masks.  Slot 0..511 of the area holds the full header of slice 0 (of this mat-vec,
-        // then of the next one).
-        const char* const hdr = we_hdr + 16 * lane;
-        const uint32_t stN = stage + 16 * lane, stH = stage + 512 + 8 * lane, stC = stage + 1536 + 8 * lane;
-        const bool use_aux = kind == OPK_RELAX || kind == OPK_RECALC || (kind == OPK_RESTRICT && first && !coarsest);
-        auto issue_hdr = [&](int t) { if (t < nsl) cp_async8(stH + (uint32_t)(t & 3) * 256u, hdr + (long long)t * HEADER_BYTES); };
-        auto issue_ctx = [&](int t, uint32_t r) {
-            const uint32_t a = stC + (uint32_t)(t & 1) * 1024u;
-            if (r != NO_ROW) {
-                if (cA) cp_async8(a, cA + r);
-                if (cB) cp_async8(a + 256, cB + r);
-                if (cC) cp_async8(a + 512, cC + r);
-            }
-            if (use_aux) cp_async8(a + 768, hdr + (long long)t * HEADER_BYTES + 8);
-        };
-        if (!hdr_ready) { cp_async_wait_all(); cp_async16(stN, hdr); }       // (never two copies in flight to one slot)
-        cp_async_wait_all();
-        const uint4 h = lds128(stN);
-        uint32_t row = h.x;
-        int left = (int)(h.y & HDR_GROUPS_MASK);
-        bool is_c = (h.y >> 31) != 0;                                       // the row is a C-point of its level
-        double aux = mkdouble(h.z, h.w);
-        cp_async16(stN, nxt_hdr + 16 * lane);                               // static data: slice 0 of the next mat-vec
-        hdr_ready = n_next > 0;
-        issue_hdr(1); issue_hdr(2); issue_hdr(3);
-        issue_ctx(0, row);
-        cp_async_commit();
-#else
-        const char* const hdr = we_hdr + 16 * lane;
-        const uint32_t stH = stage + 16 * lane, stC = stage + 512 + 8 * lane;
-        const char* const hdr_after = nxt_hdr + 16 * lane;
+        constexpr int HL = WIDE ? 8 : 4, HB = WIDE ? HEADER_BYTES_WIDE : HEADER_BYTES_NARROW;   // header bytes per lane / per slice
+        const char* const hdr = we_hdr + HL * lane;
+        const uint32_t stH = stage + HL * lane, stD = stage + 256 + 8 * lane, stC = stage + 512 + 8 * lane;
+        const char* const hdr_after = nxt_hdr + HL * lane;
         auto fetch_ctx = [&](uint32_t r) {
             if (r != NO_ROW) {
                 if (cA) cp_async8(stC, cA + r);
                 if (cB) cp_async8(stC + 256, cB + r);
                 if (cC) cp_async8(stC + 512, cC + r);
+                // the l1 diagonal inverse of the rows that relax (S8; the level's dinv array has n_bar entries, 0.0 on ghosts);
+                // the pointer is read from the level table where it is needed: it is not worth two registers of the ring loop
+                if (kind == OPK_RELAX || ((kind == OPK_RECALC || (kind == OPK_RESTRICT && first)) && !coarsest))
+                    cp_async8(stD, lev[kind == OPK_RESTRICT ? l + 1 : l].dinv + r);
             }
         };
-        if (!hdr_ready) { cp_async_wait_all(); cp_async16(stH, hdr); cp_async_issued(); }       // (never two copies in flight to one slot)
+        auto fetch_hdr = [&](const char* src) { if (WIDE) cp_async8(stH, src); else cp_async4(stH, src); };
+        uint32_t row;
+        int left;
+        bool is_c;                                                          // the row is a C-point of its level
+        auto read_hdr = [&]() {                                             // narrow: row | K << 16 | flag << 31; wide: row, K | flag << 31
+            if (WIDE) { const uint2 w = lds_u64(stH); row = w.x; left = (int)(w.y & HDR_GROUPS_MASK); is_c = (w.y >> 31) != 0; }
+            else {
+                const uint32_t w = lds_u32(stH);
+                row = (w & 0xFFFFu) == 0xFFFFu ? NO_ROW : (w & 0xFFFFu);
+                left = (int)((w >> 16) & 0x7FFFu); is_c = (w >> 31) != 0;
+            }
+        };
+        if (!hdr_ready) { cp_async_wait_all(); fetch_hdr(hdr); cp_async_issued(); }       // (never two copies in flight to one slot)
         cp_async_wait_all();
-        uint4 h = lds128(stH);
-        uint32_t row = h.x;
-        int left = (int)(h.y & HDR_GROUPS_MASK);
-        bool is_c = (h.y >> 31) != 0;                                       // the row is a C-point of its level
-        double aux = mkdouble(h.z, h.w);
+        read_hdr();
+        double aux = 0.0;
         fetch_ctx(row);
-        cp_async16(stH, nsl > 1 ? hdr + HEADER_BYTES : hdr_after);
+        fetch_hdr(nsl > 1 ? hdr + HB : hdr_after);
         cp_async_issued();
         hdr_ready = n_next > 0;
-#endif
         int sidx = 0;
         double acc = 0.0;
         auto consume = [&](const Grp& g) {
@@ -453,19 +428,13 @@ struct Worker {
         };
         auto slice_end = [&]() {
             const long long tw0 = tick();
-#if AMGDD_STAGE2
-            if (sidx < 2) cp_async_wait_all();      // the rings are still filling
-            else cp_async_wait_pending(1);          // everything but the youngest group: this slice's operands, headers up to sidx + 2
-            const uint32_t stE = stC + (uint32_t)(sidx & 1) * 1024u;
-            if (use_aux && sidx > 0) aux = lds_f64(stE + 768);
-#else
             cp_async_wait_all();
             const uint32_t stE = stC;
-#endif
             tock(14, tw0);
             tock_op(3, tw0);
             if (row != NO_ROW) {
                 const double e0 = lds_f64(stE), e1 = lds_f64(stE + 256), e2 = lds_f64(stE + 512);   // unused ones are stale, never read
+                aux = lds_f64(stD);
                 if (kind == OPK_RELAX) {           // one l1-Jacobi update (§4.1); aux = 1 / sum_j |a_ij| (S8)
                     const double uo = xg.ld(row);
                     if ((half_c && !is_c) || (half_f && is_c)) {   // CF smoother: not this half-sweep's class
@@ -507,28 +476,13 @@ struct Worker {
             }
             ++sidx;
             acc = 0.0;
-#if AMGDD_STAGE2
             if (sidx < nsl) {
-                const uint32_t hs = stH + (uint32_t)(sidx & 3) * 256u;
-                row = lds_u32(hs);
-                const uint32_t info = lds_u32(hs + 4);
-                left = (int)(info & HDR_GROUPS_MASK); is_c = (info >> 31) != 0;
-                issue_hdr(sidx + 3);                                      // into the slot of the slice just finished
-                if (sidx == 1) issue_ctx(1, row);
-                if (sidx + 1 < nsl) issue_ctx(sidx + 1, lds_u32(stH + (uint32_t)((sidx + 1) & 3) * 256u));
-                cp_async_commit();
-            }
-        };
-#else
-            if (sidx < nsl) {
-                h = lds128(stH);
-                row = h.x; left = (int)(h.y & HDR_GROUPS_MASK); is_c = (h.y >> 31) != 0; aux = mkdouble(h.z, h.w);
+                read_hdr();
                 fetch_ctx(row);
-                cp_async16(stH, sidx + 1 < nsl ? hdr + (long long)(sidx + 1) * HEADER_BYTES : hdr_after);
+                fetch_hdr(sidx + 1 < nsl ? hdr + (long long)(sidx + 1) * HB : hdr_after);
                 cp_async_issued();
             }
         };
-#endif
         tock(PROF_PRIME, tp0);
         // Blocks of D groups, double buffered in registers: WAIT for block j (buffer X), then issue
         // the burst of block j+1 into the other buffer (the next D groups of this mat-vec or, after

@@ -108,7 +108,6 @@ struct StreamLayout {
     i32 nrows = 0;
     i64 nnz = 0;
     bool wide = false;           // uint32 column indices
-    bool has_aux = false;        // slice headers carry a per-row value (the l1 diagonal inverse)
 };
 
 // Sizes of one (subdomain, level) block and where its arrays sit inside the subdomain's blob.
@@ -172,7 +171,6 @@ private:
     std::vector<std::vector<i32>> loc_, stamp_;
     std::vector<i32> epoch_;
     std::vector<i32> frontier_, next_, cursor_;
-    std::vector<double> aux_, auxr_;
     std::vector<uint8_t> flg_;
     i32 local_of(int l, i32 g) const { return stamp_[l][g] == epoch_[l] ? loc_[l][g] : -1; }
 };
@@ -204,8 +202,7 @@ struct PackedLevelStream {
     std::vector<char> data;
     StreamLayout lay;
 };
-// aux: M.nrows doubles (l1 diagonal inverse, A streams) or nullptr
 // row_flags: M.nrows bytes (1: C-point of the rows' level) or nullptr
-bool pack_global_stream(const HostCsr& M, const double* aux, const uint8_t* row_flags, int window, PackedLevelStream& out, i64& too_long_row);
+bool pack_global_stream(const HostCsr& M, const uint8_t* row_flags, int window, PackedLevelStream& out, i64& too_long_row);
 
 }  // namespace amgdd

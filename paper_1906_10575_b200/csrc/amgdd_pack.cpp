@@ -83,18 +83,17 @@ PackPlan make_plan(const std::vector<Slice>& slices, const std::vector<int> (&of
 
 }  // namespace
 
-PackPlan plan_stream(int nrows, const int32_t* rp, bool wide, bool has_aux, int n_real, int window) {
+PackPlan plan_stream(int nrows, const int32_t* rp, bool wide, int n_real, int window) {
     std::vector<Slice> slices;
     build_slices(nrows, rp, n_real, window, slices);
     std::vector<int> of_way[NUM_WAYS];
-    deal(slices, group_bytes(wide), HEADER_BYTES, of_way);
-    return make_plan(slices, of_way, group_bytes(wide), HEADER_BYTES);
+    deal(slices, group_bytes(wide), header_bytes(wide), of_way);
+    return make_plan(slices, of_way, group_bytes(wide), header_bytes(wide));
 }
 
-void write_stream(int nrows, const int32_t* rp, const int32_t* ci, const double* v, const double* aux, bool wide,
+void write_stream(int nrows, const int32_t* rp, const int32_t* ci, const double* v, bool wide,
                   int n_real, int window, char* dst, const uint8_t* row_flags) {
-    const bool has_aux = aux != nullptr;
-    const int gbytes = group_bytes(wide), hbytes = HEADER_BYTES;
+    const int gbytes = group_bytes(wide), hbytes = header_bytes(wide);
     std::vector<Slice> slices;
     build_slices(nrows, rp, n_real, window, slices);
     std::vector<int> of_way[NUM_WAYS];
@@ -107,11 +106,15 @@ void write_stream(int nrows, const int32_t* rp, const int32_t* ci, const double*
         for (int si : of_way[w]) {
             const Slice& sl = slices[si];
             for (int j = 0; j < SLICE_ROWS; ++j) {
-                const uint32_t row = sl.rows[j] >= 0 ? (uint32_t)sl.rows[j] : NO_ROW;
-                const uint32_t k = (uint32_t)sl.K | ((row_flags && sl.rows[j] >= 0 && row_flags[sl.rows[j]]) ? 0x80000000u : 0u);
-                char* q = h + 16 * j;
-                const double a = (has_aux && sl.rows[j] >= 0) ? aux[sl.rows[j]] : 0.0;
-                std::memcpy(q, &row, 4); std::memcpy(q + 4, &k, 4); std::memcpy(q + 8, &a, 8);
+                const uint32_t flag = (row_flags && sl.rows[j] >= 0 && row_flags[sl.rows[j]]) ? 0x80000000u : 0u;
+                if (wide) {                                                  // { row, K | flag << 31 }
+                    const uint32_t row = sl.rows[j] >= 0 ? (uint32_t)sl.rows[j] : NO_ROW;
+                    const uint32_t k = (uint32_t)sl.K | flag;
+                    std::memcpy(h + 8 * j, &row, 4); std::memcpy(h + 8 * j + 4, &k, 4);
+                } else {                                                     // row | K << 16 | flag << 31
+                    const uint32_t w = (sl.rows[j] >= 0 ? (uint32_t)sl.rows[j] : (uint32_t)NO_ROW16) | ((uint32_t)sl.K << 16) | flag;
+                    std::memcpy(h + 4 * j, &w, 4);
+                }
             }
             h += hbytes;
             for (int kg = 0; kg < sl.K; ++kg, g += gbytes)

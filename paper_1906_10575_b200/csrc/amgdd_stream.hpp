@@ -30,12 +30,14 @@
 //                                32 x { uint16 col[step 0..3] }           lane j at 1024 + 8 j
 //   group (wide, 1536 bytes):    the same two value planes, then 32 x { uint32 col[step 0..3] },
 //                                lane j at 1024 + 16 j
-//   header (512 bytes):  32 x { uint32 row, uint32 info, double aux }   lane j at 16 j
-//            row = the lane's row (NO_ROW: the slice has fewer than 32 rows), info = K of the
-//            slice (the same in every lane) | the row's flag << 31 (C-point of its level: the CF
-//            smoother relaxes the two classes in turn), aux = a per-row value the epilogue needs (the l1
-//            diagonal inverse, S8; 0.0 in streams packed without an aux vector).  One header
-//            shape for all streams keeps every load of the kernel unconditional.
+//   header (narrow, 128 bytes):  32 x uint32  row | K << 16 | flag << 31      lane j at 4 j
+//   header (wide, 256 bytes):    32 x { uint32 row, uint32 K | flag << 31 }    lane j at 8 j
+//            row = the lane's row (0xFFFF / NO_ROW: the slice has fewer than 32 rows), K = groups of the
+//            slice (the same in every lane), flag = the row is a C-point of its level (the CF smoother relaxes
+//            the two classes in turn).  The l1 diagonal inverse a relaxing epilogue needs is NOT in the
+//            stream: the kernel fetches it from the level's dinv array together with the other row-local
+//            operands (round 1 kept it in a 16-byte header per row; the headers were 4-30 % of a stream).
+//            A narrow stream has at most 65536 columns AND at most 65535 rows.
 #pragma once
 #include <cstdint>
 
@@ -56,8 +58,12 @@ constexpr int SLICE_ROWS = 32;
 constexpr int GROUP_STEPS = 4;
 constexpr int GROUP_BYTES_NARROW = 1280;
 constexpr int GROUP_BYTES_WIDE = 1536;
-constexpr int HEADER_BYTES = 512;
+constexpr int HEADER_BYTES_NARROW = 128;     // 32 x uint32 { row | K << 16 | flag << 31 }
+constexpr int HEADER_BYTES_WIDE = 256;       // 32 x { uint32 row, uint32 K | flag << 31 }
+inline int header_bytes(bool wide) { return wide ? HEADER_BYTES_WIDE : HEADER_BYTES_NARROW; }
+constexpr uint16_t NO_ROW16 = 0xFFFFu;
 constexpr int NARROW_MAX_COLS = 65536;       // uint16 column indices
+constexpr int NARROW_MAX_ROWS = 65535;       // uint16 row in the header word (0xFFFF: no row)
 constexpr int DEFAULT_WINDOW = 256;
 #ifndef AMGDD_THIN_WINDOW
 #define AMGDD_THIN_WINDOW 256
@@ -82,12 +88,11 @@ struct WayDesc {           // one sub-stream (same layout as amgdd_way_t of incl
 static_assert(sizeof(WayDesc) == 32, "WayDesc layout");
 
 constexpr uint32_t STREAM_WIDE = 1u;         // StreamDesc::flags
-constexpr uint32_t STREAM_AUX = 2u;
 constexpr uint32_t STREAM_SHARED = 4u;       // the single copy of a fully covered level: every CTA reads it, keep it in L2
 
 struct StreamDesc {
     const char* base;      // DEVICE, 128-byte aligned
-    uint32_t flags;        // STREAM_WIDE | STREAM_AUX | STREAM_SHARED
+    uint32_t flags;        // STREAM_WIDE | STREAM_SHARED
     uint32_t pad_;
     WayDesc way[NUM_WAYS];
 };
@@ -187,10 +192,12 @@ struct PackPlan {
     int64_t padded_nnz;        // 4 * 32 * ngroups: entries stored, padding included
 };
 // rp: nrows+1 int32 offsets (rp[0] = 0); window: rows per sort window (multiple of 32)
-PackPlan plan_stream(int nrows, const int32_t* rp, bool wide, bool has_aux, int n_real, int window);
-// writes plan.bytes bytes; aux: nrows doubles or nullptr (must match has_aux of the plan); row_flags: nrows bytes (0/1) or nullptr
-void write_stream(int nrows, const int32_t* rp, const int32_t* ci, const double* v, const double* aux, bool wide,
+// wide must be true when the matrix has more than NARROW_MAX_COLS columns or more than NARROW_MAX_ROWS rows
+PackPlan plan_stream(int nrows, const int32_t* rp, bool wide, int n_real, int window);
+// writes plan.bytes bytes; row_flags: nrows bytes (0/1) or nullptr
+void write_stream(int nrows, const int32_t* rp, const int32_t* ci, const double* v, bool wide,
                   int n_real, int window, char* dst, const uint8_t* row_flags = nullptr);
+inline bool needs_wide(long long nrows, long long ncols) { return ncols > NARROW_MAX_COLS || nrows > NARROW_MAX_ROWS; }
 
 // the program of one subdomain: num_fac_cycles AlgFAC V(nu,nu)-cycles (Alg. 4); returns the op count
 // (ops may be nullptr to count only)

@@ -1,25 +1,28 @@
 """Host logic, no GPU: the packed SELL-32 group streams (the HBM layout the AlgFAC kernel reads with
 coalesced 128-bit loads; csrc/amgdd_stream.hpp) decode back to the CSR
 they were made from, way by way and slice by slice, for narrow and wide column indices, ragged
-rows, empty rows, two row groups, an aux vector and several sort windows."""
+rows, empty rows, two row groups, row flags and several sort windows."""
 import numpy as np
 import pytest
 
 import paper_1906_10575_b200 as m
 
 NO_ROW = 0xFFFFFFFF
-HB = m.HEADER_BYTES
+
+
+def header_bytes(wide):
+    return m.HEADER_BYTES_WIDE if wide else m.HEADER_BYTES_NARROW
 
 
 def decode(stream, ways, wide, nrows, n_real=None, window=256):
     """Decoder written from the layout comment of amgdd_stream.hpp (independent of the packer).
-    Returns per-row lists of (column, value) in stored order, the aux vector and the bytes of each
-    way; checks the way descriptors (offsets, the real-group prefix) and that padding is zero."""
+    Returns per-row lists of (column, value) in stored order and the bytes of each way; checks the
+    way descriptors (offsets, the real-group prefix) and that padding is zero."""
     raw = stream.tobytes()
     n_real = nrows if n_real is None else n_real
     gb = m.GROUP_BYTES_WIDE if wide else m.GROUP_BYTES_NARROW
+    HB = header_bytes(wide)
     rows = [None] * nrows
-    aux = np.full(nrows, np.nan)
     flags = np.zeros(nrows, dtype=np.int64)
     decode.flags = flags
     load = []
@@ -38,15 +41,19 @@ def decode(stream, ways, wide, nrows, n_real=None, window=256):
         groups_seen = real_groups = real_slices = 0
         ghost_seen = False
         for s in range(int(w["nslices"])):
-            hdr = np.frombuffer(raw, dtype=np.uint32, count=128, offset=h + s * HB).reshape(32, 4)
-            a = np.frombuffer(raw, dtype=np.float64, count=64, offset=h + s * HB).reshape(32, 2)[:, 1]
-            rid, K = hdr[:, 0].astype(np.int64), hdr[:, 1] & 0x7FFFFFFF
-            flag = hdr[:, 1] >> 31
+            if wide:                   # 32 x { uint32 row, uint32 K | flag << 31 }
+                hdr = np.frombuffer(raw, dtype=np.uint32, count=64, offset=h + s * HB).reshape(32, 2)
+                rid, K, flag = hdr[:, 0].astype(np.int64), hdr[:, 1] & 0x7FFFFFFF, hdr[:, 1] >> 31
+            else:                      # 32 x uint32  row | K << 16 | flag << 31, row 0xFFFF: none
+                hdr = np.frombuffer(raw, dtype=np.uint32, count=32, offset=h + s * HB)
+                rid = (hdr & 0xFFFF).astype(np.int64)
+                rid[rid == 0xFFFF] = NO_ROW
+                K, flag = (hdr >> 16) & 0x7FFF, hdr >> 31
             assert (K == K[0]).all() and K[0] >= 1, "every lane carries the slice's group count"
             K = int(K[0])
             valid = rid != NO_ROW
             assert valid.any() and valid[: valid.sum()].all(), "missing rows are the last lanes"
-            assert (a[~valid] == 0).all()
+            assert (flag[~valid] == 0).all()
             is_real = bool((rid[valid] < n_real).all())
             assert is_real or (rid[valid] >= n_real).all(), "the two row groups never mix inside a slice"
             assert not (is_real and ghost_seen), "inside a way the first row group comes first"
@@ -72,12 +79,11 @@ def decode(stream, ways, wide, nrows, n_real=None, window=256):
                 r = int(rid[j])
                 assert rows[r] is None, "every row is stored once"
                 rows[r] = (cols[j], vals[j])
-                aux[r] = a[j]
                 flags[r] = flag[j]
         assert groups_seen == int(w["ngroups"]) and real_groups == int(w["ngroups_real"]) and real_slices == int(w["nslices_real"])
         load.append(int(w["ngroups"]) * gb + int(w["nslices"]) * HB)
     assert all(r is not None for r in rows)
-    return rows, aux, load
+    return rows, load
 
 
 def random_csr(rng, nrows, ncols, max_len, empty_frac=0.1):
@@ -105,14 +111,13 @@ def test_stream_round_trip(wide):
     ncols = 70000 if wide else 5000
     nrows, n_real = 3000, 2013
     rp, ci, v = random_csr(rng, nrows, ncols, 60)
-    aux = rng.standard_normal(nrows)
     rf = (rng.random(nrows) < 0.4).astype(np.uint8)
-    stream, ways = m.amgdd_pack_stream(rp, ci, v, wide=wide, n_real=n_real, aux=aux, row_flags=rf)
+    stream, ways = m.amgdd_pack_stream(rp, ci, v, wide=wide, n_real=n_real, row_flags=rf)
     assert len(ways) == m.NUM_WAYS and len(stream) % 128 == 0
-    rows, aux2, load = decode(stream, ways, wide, nrows, n_real)
+    rows, load = decode(stream, ways, wide, nrows, n_real)
     check_rows(rows, rp, ci, v)
-    assert np.array_equal(aux2, aux)
-    assert np.array_equal(decode.flags, rf), "bit 31 of the header's info word carries the row's flag"
+    assert np.array_equal(decode.flags, rf), "bit 31 of the header word carries the row's flag"
+    HB = header_bytes(wide)
     # the ways are balanced: a slice goes to the lightest way, so no way exceeds the mean by more than one slice
     gb = m.GROUP_BYTES_WIDE if wide else m.GROUP_BYTES_NARROW
     assert max(load) <= np.mean(load) + 15 * gb + HB
@@ -133,8 +138,8 @@ def test_uniform_rows_are_not_padded():
     v = rng.standard_normal(rp[-1])
     stream, ways = m.amgdd_pack_stream(rp, ci, v)
     assert int(ways["ngroups"].sum()) == nrows // 32 * 9
-    assert len(stream) == nrows // 32 * (9 * m.GROUP_BYTES_NARROW + HB)
-    rows, _, _ = decode(stream, ways, False, nrows)
+    assert len(stream) == nrows // 32 * (9 * m.GROUP_BYTES_NARROW + m.HEADER_BYTES_NARROW)
+    rows, _ = decode(stream, ways, False, nrows)
     check_rows(rows, rp, ci, v)
 
 
@@ -143,9 +148,9 @@ def test_windows_and_no_aux(window):
     rng = np.random.default_rng(window)
     rp, ci, v = random_csr(rng, 777, 3000, 25, empty_frac=0.3)
     stream, ways = m.amgdd_pack_stream(rp, ci, v, window=window)
-    rows, aux, _ = decode(stream, ways, False, 777, window=window)
+    rows, _ = decode(stream, ways, False, 777, window=window)
     check_rows(rows, rp, ci, v)
-    assert (aux == 0).all(), "streams packed without an aux vector carry 0.0"
+    assert (decode.flags == 0).all(), "streams packed without row flags carry none"
     assert np.array_equal(ways["ngroups"], ways["ngroups_real"]) and np.array_equal(ways["nslices"], ways["nslices_real"])
 
 
@@ -158,7 +163,7 @@ def test_long_rows():
     v = rng.standard_normal(rp[-1])
     stream, ways = m.amgdd_pack_stream(rp, ci, v)
     assert int(ways["ngroups"].max()) == 1250
-    rows, _, _ = decode(stream, ways, False, len(lens))
+    rows, _ = decode(stream, ways, False, len(lens))
     check_rows(rows, rp, ci, v)
 
 
@@ -169,13 +174,13 @@ def test_few_rows_and_empty_matrix():
     stream, ways = m.amgdd_pack_stream(rp, ci, v)
     # one slice in way 0: one group (longest row 3 <= 4 steps) and one header
     assert ways["ngroups"].tolist() == [1] + [0] * (m.NUM_WAYS - 1)
-    assert len(stream) == m.GROUP_BYTES_NARROW + HB
-    rows, _, _ = decode(stream, ways, False, 3)
+    assert len(stream) == m.GROUP_BYTES_NARROW + m.HEADER_BYTES_NARROW
+    rows, _ = decode(stream, ways, False, 3)
     check_rows(rows, rp, ci, v)
     # a slice of empty rows still gets one (all padding) group: its rows still run their epilogue
     stream, ways = m.amgdd_pack_stream(np.zeros(4, np.int32), np.zeros(0, np.int32), np.zeros(0))
-    assert ways["ngroups"].sum() == 1 and len(stream) == m.GROUP_BYTES_NARROW + HB
-    rows, _, _ = decode(stream, ways, False, 3)
+    assert ways["ngroups"].sum() == 1 and len(stream) == m.GROUP_BYTES_NARROW + m.HEADER_BYTES_NARROW
+    rows, _ = decode(stream, ways, False, 3)
     assert all((c == 0).all() and (x == 0).all() for c, x in rows)
     stream, ways = m.amgdd_pack_stream(np.zeros(1, np.int32), np.zeros(0, np.int32), np.zeros(0))
     assert ways["ngroups"].sum() == 0 and len(stream) == 0
