@@ -199,6 +199,11 @@ def test_bad_arguments():
     with pytest.raises(m.AmgddError) as e:
         m.amgdd_pack_stream(rp, ci, v, n_real=2)
     assert e.value.code == -1
+    with pytest.raises(m.AmgddError) as e:            # the narrow header holds a 16-bit row: 65536 rows need the wide form
+        m.amgdd_pack_stream(np.zeros(65537, np.int32), np.zeros(0, np.int32), np.zeros(0))
+    assert e.value.code == -1
+    stream, ways = m.amgdd_pack_stream(np.zeros(65537, np.int32), np.zeros(0, np.int32), np.zeros(0), wide=True)
+    assert int(ways["nslices"].sum()) == 2048 and len(stream) == 2048 * (m.GROUP_BYTES_WIDE + m.HEADER_BYTES_WIDE)
     big = np.array([0, 70000], dtype=np.int32)        # more than 65535 entries in one row
     with pytest.raises(m.AmgddError) as e:
         m.amgdd_pack_stream(big, np.zeros(70000, np.int32), np.zeros(70000), wide=True)
