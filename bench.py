@@ -212,7 +212,9 @@ def run_reference(args, p, rank, world):
         "impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus,
         "steps": steps, "warmup": warmup, "ms_per_step": cb["value"], "higher_is_better": False,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": workload_name(p, args), "note": "CPU oracle, bounded sample, timed steps capped at 3"},
+        "config": {"workload": workload_name(p, args), "n_dofs": p.n, "nnz": p.nnz, "subdomains": p.num_subdomains, "eta": p.eta,
+                   "theta": p.theta, "fac_cycles_per_step": p.num_fac_cycles, "relax_sweeps": p.relax_sweeps},
+        "note": "CPU oracle as it stands, bounded sample of the workload (cpu_baseline.sample), timed steps capped at 3",
         "cpu_baseline": cb,
         "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
