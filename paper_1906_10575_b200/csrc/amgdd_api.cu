@@ -40,6 +40,7 @@ struct GlobalLevelDev {          // the single device copy of a whole level
     // AMG V-cycle (amgdd_vcycle; uploaded on first use): A_l and P_l as plain CSR, the l1 diagonal, level vectors
     int* p_rp = nullptr; int* p_ci = nullptr; double* p_v = nullptr;
     int lanes_p = 2;
+    int* p_blk = nullptr; int p_nblk = 0;
     double* vdinv = nullptr; double *vu0 = nullptr, *vu1 = nullptr, *vf = nullptr, *vr = nullptr;
     int8_t* vcf = nullptr;
 };
@@ -1308,9 +1309,16 @@ static int ensure_vcycle(amgdd_handle_s* h) {
         GlobalLevelDev& g = h->glev[l];
         const size_t nl = (size_t)lv.A.nrows;
         if (!g.a_rp) { if ((rc = upload_csr32(h, lv.A, &g.a_rp, &g.a_ci, &g.a_v))) return rc; }
+        if (!g.a_blk) {
+            const std::vector<int> blk = stream_row_blocks(lv.A);
+            g.a_nblk = (int)blk.size() - 1;
+            if ((rc = upload(h, &g.a_blk, blk.data(), blk.size()))) return rc;
+        }
         if (l < L) {
             if ((rc = upload_csr32(h, lv.P, &g.p_rp, &g.p_ci, &g.p_v))) return rc;
-            g.lanes_p = pick_lanes(avg_row(lv.P));
+            const std::vector<int> blk = stream_row_blocks(lv.P);
+            g.p_nblk = (int)blk.size() - 1;
+            if ((rc = upload(h, &g.p_blk, blk.data(), blk.size()))) return rc;
         }
         if ((rc = upload(h, &g.vdinv, lv.dinv.data(), lv.dinv.size()))) return rc;
         if (l < L) { if ((rc = upload(h, &g.vcf, lv.cf.data(), lv.cf.size()))) return rc; }
@@ -1345,23 +1353,23 @@ int amgdd_vcycle(amgdd_handle_t h, const double* b, double* x, int32_t num_cycle
             if (l == 0) CUDA_TRY(cudaMemcpyAsync(g.vu0, x, (size_t)nrows(0) * sizeof(double), cudaMemcpyDeviceToDevice, st));
             for (int s = 0; s < nu1; ++s)                                       // the level's iterate lives in vu0
                 for (int half = 0; half < (cfm ? 2 : 1); ++half) {              // CF smoother: C-points, then F-points
-                    launch_relax(g.a_rp, g.a_ci, g.a_v, nrows(l), g.lanes_a, g.vdinv, f, have_u ? g.vu0 : nullptr, g.vu1,
+                    launch_relax(g.a_rp, g.a_ci, g.a_v, g.a_blk, g.a_nblk, g.vdinv, f, have_u ? g.vu0 : nullptr, g.vu1,
                                  cfm ? (const signed char*)g.vcf : nullptr, half == 0 ? +1 : -1, st);
                     std::swap(g.vu0, g.vu1);
                     have_u = true;
                 }
             if (!have_u) CUDA_TRY(cudaMemsetAsync(g.vu0, 0, (size_t)nrows(l) * sizeof(double), st));
-            launch_spmv_axpy(g.a_rp, g.a_ci, g.a_v, nrows(l), g.lanes_a, g.vu0, f, g.vr, 0, st);        // r = f - A u
+            launch_spmv_axpy(g.a_rp, g.a_ci, g.a_v, g.a_blk, g.a_nblk, g.vu0, f, g.vr, 0, st);          // r = f - A u
             launch_spmv(g.r_rp, g.r_ci, g.r_v, g.r_blk, g.r_nblk, g.vr, h->glev[l + 1].vf, st);         // f_{l+1} = P^T r
         }
         launch_coarse_solve(h->d_lu, h->d_rowperm, (int)h->H.nL, L == 0 ? b : h->glev[L].vf, L == 0 ? x : h->glev[L].vu0, st);
         for (int l = L - 1; l >= 0; --l) {                                      // upsweep P:459-464
             GlobalLevelDev& g = h->glev[l];
             const double* f = l == 0 ? b : g.vf;
-            launch_spmv_axpy(g.p_rp, g.p_ci, g.p_v, nrows(l), g.lanes_p, h->glev[l + 1].vu0, nullptr, g.vu0, 1, st);   // u += P u_{l+1}
+            launch_spmv_axpy(g.p_rp, g.p_ci, g.p_v, g.p_blk, g.p_nblk, h->glev[l + 1].vu0, nullptr, g.vu0, 1, st);   // u += P u_{l+1}
             for (int s = 0; s < nu2; ++s)
                 for (int half = 0; half < (cfm ? 2 : 1); ++half) {              // CF smoother: F-points, then C-points
-                    launch_relax(g.a_rp, g.a_ci, g.a_v, nrows(l), g.lanes_a, g.vdinv, f, g.vu0, g.vu1,
+                    launch_relax(g.a_rp, g.a_ci, g.a_v, g.a_blk, g.a_nblk, g.vdinv, f, g.vu0, g.vu1,
                                  cfm ? (const signed char*)g.vcf : nullptr, half == 0 ? -1 : +1, st);
                     std::swap(g.vu0, g.vu1);
                 }

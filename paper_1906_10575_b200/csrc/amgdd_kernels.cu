@@ -18,7 +18,8 @@ constexpr int GLOBAL_BLOCK = 256;
 constexpr int STREAM_ROWS = 256;             // rows of a block of the stream kernel (one thread per row in the second phase)
 constexpr int STREAM_NNZ = 2304;             // entries of a block (their products wait in shared memory)
 
-// y = M x (MODE 0) or r = b - M x with per-block sums of r^2 (MODE 1) over consecutive rows.  Block k owns the rows
+// y = M x (MODE 0), r = b - M x with per-block sums of r^2 (MODE 1), one l1-Jacobi sweep y = x + D^-1 (b - M x) on the rows
+// of one C/F class or on all rows (MODE 2; x = nullptr: from zero), y = b - M x (MODE 3) or y += M x (MODE 4) over consecutive rows.  Block k owns the rows
 // [blk[k], blk[k+1]) (host-built: at most STREAM_ROWS rows and STREAM_NNZ entries; a longer row is a block of its own).
 // Phase 1: all threads walk the block's contiguous entries (coalesced loads of values and columns, x gathered through
 // L2) and leave the products in shared memory; phase 2: thread t adds the products of row t in order.
@@ -26,7 +27,8 @@ template <int MODE>
 __global__ void __launch_bounds__(GLOBAL_BLOCK) csr_stream_kernel(const int* __restrict__ rp, const int* __restrict__ ci,
                                                                   const double* __restrict__ v, const int* __restrict__ blk,
                                                                   const double* __restrict__ x, const double* __restrict__ b,
-                                                                  double* __restrict__ y, double* __restrict__ partial) {
+                                                                  double* __restrict__ y, double* __restrict__ partial,
+                                                                  const double* __restrict__ dinv, const signed char* __restrict__ cf, int cls) {
     __shared__ double prod[STREAM_NNZ];
     __shared__ int srp[STREAM_ROWS + 1];
     __shared__ double red[GLOBAL_BLOCK / 32];
@@ -35,27 +37,34 @@ __global__ void __launch_bounds__(GLOBAL_BLOCK) csr_stream_kernel(const int* __r
     __syncthreads();
     const int e0 = srp[0], e1 = srp[n];
     double sq = 0.0;
+    auto finish = [&](int row, double sum) {
+        if (MODE == 1) {
+            const double ri = b[row] - sum;
+            if (y) y[row] = ri;
+            sq = ri * ri;
+        } else if (MODE == 2) {                // CF smoother: cf != nullptr restricts the update to one class (cls > 0: C-points)
+            const bool active = !cf || ((cf[row] > 0) == (cls > 0));
+            y[row] = (x ? x[row] : 0.0) + (active ? dinv[row] * (b[row] - sum) : 0.0);
+        } else if (MODE == 3) y[row] = b[row] - sum;
+        else if (MODE == 4) y[row] = y[row] + sum;
+        else y[row] = sum;
+    };
+    const bool have_x = MODE != 2 || x != nullptr;                      // a sweep from u = 0 needs no products
     if (e1 - e0 <= STREAM_NNZ) {
-        for (int e = e0 + threadIdx.x; e < e1; e += GLOBAL_BLOCK) prod[e - e0] = __dmul_rn(__ldg(v + e), __ldg(x + __ldg(ci + e)));
+        if (have_x)
+            for (int e = e0 + threadIdx.x; e < e1; e += GLOBAL_BLOCK) prod[e - e0] = __dmul_rn(__ldg(v + e), __ldg(x + __ldg(ci + e)));
         __syncthreads();
         if (threadIdx.x < n) {
             double sum = 0.0;
-            for (int k = srp[threadIdx.x] - e0; k < srp[threadIdx.x + 1] - e0; ++k) sum = __dadd_rn(sum, prod[k]);
-            const int row = r0 + threadIdx.x;
-            if (MODE == 1) {
-                const double ri = b[row] - sum;
-                if (y) y[row] = ri;
-                sq = ri * ri;
-            } else y[row] = sum;
+            if (have_x)
+                for (int k = srp[threadIdx.x] - e0; k < srp[threadIdx.x + 1] - e0; ++k) sum = __dadd_rn(sum, prod[k]);
+            finish(r0 + threadIdx.x, sum);
         }
     } else if (threadIdx.x == 0) {             // one row longer than a block holds: the same order, one thread
         double sum = 0.0;
-        for (int e = e0; e < e1; ++e) sum = __dadd_rn(sum, __dmul_rn(__ldg(v + e), __ldg(x + __ldg(ci + e))));
-        if (MODE == 1) {
-            const double ri = b[r0] - sum;
-            if (y) y[r0] = ri;
-            sq = ri * ri;
-        } else y[r0] = sum;
+        if (have_x)
+            for (int e = e0; e < e1; ++e) sum = __dadd_rn(sum, __dmul_rn(__ldg(v + e), __ldg(x + __ldg(ci + e))));
+        finish(r0, sum);
     }
     if (MODE == 1) {
         for (int o = 16; o > 0; o >>= 1) sq += __shfl_down_sync(0xffffffffu, sq, o);
@@ -145,41 +154,6 @@ __global__ void __launch_bounds__(1024) sum_finalize_kernel(const double* __rest
 // ---------------------------------------------------------------------------------------------
 // AMG V-cycle on the global hierarchy (Alg. 1): the paper's comparison method
 // ---------------------------------------------------------------------------------------------
-// one l1-Jacobi sweep u_out = u_in + D^-1 (f - A u_in) (reading A2); u_in = nullptr means u_in = 0
-__global__ void __launch_bounds__(GLOBAL_BLOCK) relax_kernel(const int* __restrict__ rp, const int* __restrict__ ci,
-                                                             const double* __restrict__ v, long long n, int lanes,
-                                                             const double* __restrict__ dinv, const double* __restrict__ f,
-                                                             const double* __restrict__ u_in, double* __restrict__ u_out,
-                                                             const signed char* __restrict__ cf, int cls) {
-    const int lane = threadIdx.x & (lanes - 1);
-    const long long row = (long long)blockIdx.x * (GLOBAL_BLOCK / lanes) + threadIdx.x / lanes;
-    // CF smoother: cf != nullptr restricts the update to the rows of one class (cls > 0: C-points), the others keep u
-    const bool active = row < n && (!cf || ((cf[row] > 0) == (cls > 0)));
-    double sum = 0.0;
-    if (active && u_in) {
-        const int bgn = __ldg(rp + row), end = __ldg(rp + row + 1);
-        for (int k = bgn + lane; k < end; k += lanes) sum += __ldg(v + k) * __ldg(u_in + __ldg(ci + k));
-    }
-    for (int o = lanes >> 1; o > 0; o >>= 1) sum += __shfl_down_sync(0xffffffffu, sum, o, lanes);
-    if (row < n && lane == 0) u_out[row] = (u_in ? u_in[row] : 0.0) + (active ? dinv[row] * (f[row] - sum) : 0.0);
-}
-
-// y = f - A x (f = nullptr: y = A x); accumulate = 1: y += A x
-__global__ void __launch_bounds__(GLOBAL_BLOCK) spmv_axpy_kernel(const int* __restrict__ rp, const int* __restrict__ ci,
-                                                                 const double* __restrict__ v, long long n, int lanes,
-                                                                 const double* __restrict__ x, const double* __restrict__ f,
-                                                                 double* __restrict__ y, int accumulate) {
-    const int lane = threadIdx.x & (lanes - 1);
-    const long long row = (long long)blockIdx.x * (GLOBAL_BLOCK / lanes) + threadIdx.x / lanes;
-    double sum = 0.0;
-    if (row < n) {
-        const int bgn = __ldg(rp + row), end = __ldg(rp + row + 1);
-        for (int k = bgn + lane; k < end; k += lanes) sum += __ldg(v + k) * __ldg(x + __ldg(ci + k));
-    }
-    for (int o = lanes >> 1; o > 0; o >>= 1) sum += __shfl_down_sync(0xffffffffu, sum, o, lanes);
-    if (row < n && lane == 0) y[row] = accumulate ? y[row] + sum : (f ? f[row] - sum : sum);
-}
-
 // u = A_L^-1 f with the LU factors of setup (column-major, unit lower; rowperm[i] = source row of row i); one CTA
 __global__ void __launch_bounds__(256) coarse_solve_kernel(const double* __restrict__ lu, const int* __restrict__ rowperm, int n,
                                                            const double* __restrict__ f, double* __restrict__ u) {
@@ -203,16 +177,17 @@ __global__ void __launch_bounds__(256) coarse_solve_kernel(const double* __restr
 
 }  // namespace
 
-void launch_relax(const int* rp, const int* ci, const double* v, long long n, int lanes, const double* dinv, const double* f,
+void launch_relax(const int* rp, const int* ci, const double* v, const int* blk, int nblk, const double* dinv, const double* f,
                   const double* u_in, double* u_out, const signed char* cf, int cls, void* stream) {
-    if (n <= 0) return;
-    relax_kernel<<<residual_num_blocks(n, lanes), GLOBAL_BLOCK, 0, (cudaStream_t)stream>>>(rp, ci, v, n, lanes, dinv, f, u_in, u_out, cf, cls);
+    if (nblk > 0) csr_stream_kernel<2><<<nblk, GLOBAL_BLOCK, 0, (cudaStream_t)stream>>>(rp, ci, v, blk, u_in, f, u_out, nullptr, dinv, cf, cls);
 }
 
-void launch_spmv_axpy(const int* rp, const int* ci, const double* v, long long n, int lanes, const double* x, const double* f,
+void launch_spmv_axpy(const int* rp, const int* ci, const double* v, const int* blk, int nblk, const double* x, const double* f,
                       double* y, int accumulate, void* stream) {
-    if (n <= 0) return;
-    spmv_axpy_kernel<<<residual_num_blocks(n, lanes), GLOBAL_BLOCK, 0, (cudaStream_t)stream>>>(rp, ci, v, n, lanes, x, f, y, accumulate);
+    if (nblk <= 0) return;
+    if (accumulate) csr_stream_kernel<4><<<nblk, GLOBAL_BLOCK, 0, (cudaStream_t)stream>>>(rp, ci, v, blk, x, nullptr, y, nullptr, nullptr, nullptr, 0);
+    else if (f) csr_stream_kernel<3><<<nblk, GLOBAL_BLOCK, 0, (cudaStream_t)stream>>>(rp, ci, v, blk, x, f, y, nullptr, nullptr, nullptr, 0);
+    else csr_stream_kernel<0><<<nblk, GLOBAL_BLOCK, 0, (cudaStream_t)stream>>>(rp, ci, v, blk, x, nullptr, y, nullptr, nullptr, nullptr, 0);
 }
 
 void launch_coarse_solve(const double* lu, const int* rowperm, int n, const double* f, double* u, void* stream) {
@@ -235,7 +210,7 @@ int stream_block_nnz() { return STREAM_NNZ; }
 
 void launch_residual(const int* rp, const int* ci, const double* v, const int* blk, int nblk, const double* b,
                      const double* x, double* r, double* partial, void* stream) {
-    if (nblk > 0) csr_stream_kernel<1><<<nblk, GLOBAL_BLOCK, 0, (cudaStream_t)stream>>>(rp, ci, v, blk, x, b, r, partial);
+    if (nblk > 0) csr_stream_kernel<1><<<nblk, GLOBAL_BLOCK, 0, (cudaStream_t)stream>>>(rp, ci, v, blk, x, b, r, partial, nullptr, nullptr, 0);
 }
 
 void launch_residual_rows(const int* rp, const int* ci, const double* v, const int* rows, long long nrows, const double* b,
@@ -274,7 +249,7 @@ void launch_norm_finalize(const double* partial, int nb, double* out, void* stre
 
 void launch_spmv(const int* rp, const int* ci, const double* v, const int* blk, int nblk, const double* x,
                  double* y, void* stream) {
-    if (nblk > 0) csr_stream_kernel<0><<<nblk, GLOBAL_BLOCK, 0, (cudaStream_t)stream>>>(rp, ci, v, blk, x, nullptr, y, nullptr);
+    if (nblk > 0) csr_stream_kernel<0><<<nblk, GLOBAL_BLOCK, 0, (cudaStream_t)stream>>>(rp, ci, v, blk, x, nullptr, y, nullptr, nullptr, nullptr, 0);
 }
 
 }  // namespace amgdd

@@ -21,9 +21,9 @@ void launch_spmv(const int* rp, const int* ci, const double* v, const int* blk, 
 
 // AMG V-cycle pieces (Alg. 1): one l1-Jacobi sweep (u_in = nullptr: from u = 0); y = f - A x, y = A x or
 // y += A x; dense coarse solve with the LU factors of setup (n <= 4096, one CTA)
-void launch_relax(const int* rp, const int* ci, const double* v, long long n, int lanes, const double* dinv, const double* f,
+void launch_relax(const int* rp, const int* ci, const double* v, const int* blk, int nblk, const double* dinv, const double* f,
                   const double* u_in, double* u_out, const signed char* cf, int cls, void* stream);   // cf: one class of points only (CF smoother)
-void launch_spmv_axpy(const int* rp, const int* ci, const double* v, long long n, int lanes, const double* x, const double* f,
+void launch_spmv_axpy(const int* rp, const int* ci, const double* v, const int* blk, int nblk, const double* x, const double* f,
                       double* y, int accumulate, void* stream);
 void launch_coarse_solve(const double* lu, const int* rowperm, int n, const double* f, double* u, void* stream);
 
