@@ -165,6 +165,36 @@ int amgdd_vcycle(amgdd_handle_t h, const double* b, double* x, int32_t num_cycle
 /* || b - A_0 x ||_2 (metric of Fig. 6; reading A16).  b, x DEVICE; out HOST. Synchronises. */
 int amgdd_residual_norm(amgdd_handle_t h, const double* b, const double* x, double* out_host);
 
+/* amgdd_residual_norm_static -- the same norm, || b - A x ||_2 (Fig. 6; r = b - A x as in P:471), for callers
+ * that cannot allocate device memory at the point where they need it: this call performs no cudaMalloc, no cudaFree and
+ * calls no library routine that allocates.  Typical callers: an application whose own pool (or a framework's caching
+ * allocator) already holds the GPU's memory, so that a cudaMalloc here would fail or force that pool to give memory
+ * back; a time-critical loop that must not hit the device-wide synchronisation of cudaFree; code that has no
+ * amgdd_handle_t, since amgdd_setup allocates the whole hierarchy.  Nothing is taken from a handle: the caller passes the
+ * matrix, the vectors and the result, all DEVICE pointers on the calling thread's CURRENT device:
+ *   n                 rows of A (> 0, at most AMGDD_STATIC_MAX_ROWS)
+ *   rowptr            n+1 entries (int64, rowptr[0] = 0), colind / vals: rowptr[n] entries, as amgdd_setup takes them
+ *   b, x              n doubles (read only)
+ *   r                 n doubles that receive b - A x, or NULL
+ *   out_norm          1 double that receives the norm
+ *   cuda_stream       a cudaStream_t passed as void* (NULL = legacy default stream)
+ * The call only ENQUEUES a 4-byte memset and one kernel on that stream and returns; read *out_norm after synchronising
+ * the stream.  The kernel's scratch memory -- one partial sum per 256 rows and an arrival counter -- is a fixed
+ * file-scope device array of 512.25 KiB, which every GPU that loads this library keeps until the process exits; that
+ * array is why n is limited: AMGDD_ERR_BAD_ARG with the limit in the detail string beyond AMGDD_STATIC_MAX_ROWS (use
+ * amgdd_residual_norm, whose scratch is sized by amgdd_setup, for larger systems).
+ * First call on a device: it looks the array's device address up once (cudaGetSymbolAddress, with that device
+ * current, which may make the runtime load this library's kernels there).  Make that first call at start-up, before any
+ * stream capture begins on the device.
+ * Sharing: all calls on a device use the one array.  A call clears the counter it needs and never reads partial sums of
+ * an earlier call, so calls that follow each other on one stream are independent; two calls that can be in flight at
+ * the same time (different streams, different host threads without ordering) race on it and return garbage norms.
+ * Rows are summed as in amgdd_residual_norm (stored order, no contraction): r is bit-identical to that path, the norm
+ * agrees to rounding.  Entries are not validated (a column index outside [0, n) reads out of bounds). */
+#define AMGDD_STATIC_MAX_ROWS 16777216
+int amgdd_residual_norm_static(int64_t n, const int64_t* rowptr, const int32_t* colind, const double* vals, const double* b,
+                               const double* x, double* r, double* out_norm, void* cuda_stream);
+
 /* Relaxation used by amgdd_solve, amgdd_solve_host and amgdd_vcycle from the next call on.
  *   AMGDD_SMOOTHER_L1_JACOBI     (default) one l1-Jacobi sweep over the real points (reading A2, BASELINE)
  *   AMGDD_SMOOTHER_CF_L1_JACOBI  the paper's "CF l1-scaled Jacobi" (reading A2b): every sweep is two

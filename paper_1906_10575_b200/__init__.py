@@ -17,7 +17,7 @@ from . import build as _build
 _vp, _i32, _i64, _f64 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_double
 
 EXPORTS = [
-    "amgdd_setup", "amgdd_solve", "amgdd_solve_host", "amgdd_vcycle", "amgdd_residual_norm", "amgdd_set_smoother", "amgdd_set_stream", "amgdd_destroy",
+    "amgdd_setup", "amgdd_solve", "amgdd_solve_host", "amgdd_vcycle", "amgdd_residual_norm", "amgdd_residual_norm_static", "amgdd_set_smoother", "amgdd_set_stream", "amgdd_destroy",
     "amgdd_strerror", "amgdd_last_error_detail", "amgdd_num_levels", "amgdd_level_size", "amgdd_get_cf",
     "amgdd_get_level_matrix", "amgdd_composite_size", "amgdd_get_composite", "amgdd_get_stats",
     "amgdd_last_solve_profile", "amgdd_pack_stream", "amgdd_debug_fac_cycles", "amgdd_debug_fac_op_cycles",
@@ -61,6 +61,7 @@ def _load():
     L.amgdd_solve.argtypes = [_vp, _vp, _vp, _i32, _i32, _i32, _vp]
     L.amgdd_solve_host.argtypes = [_vp, _vp, _vp, _i32, _i32, _i32, _vp]
     L.amgdd_residual_norm.argtypes = [_vp, _vp, _vp, _vp]
+    L.amgdd_residual_norm_static.argtypes = [_i64, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp]
     L.amgdd_vcycle.argtypes = [_vp, _vp, _vp, _i32, _i32, _i32, _vp]
     L.amgdd_set_stream.argtypes = [_vp, _vp]
     L.amgdd_set_smoother.argtypes = [_vp, _i32]
@@ -204,6 +205,36 @@ def amgdd_residual_norm(h: Handle, b, x) -> float:
     out = _f64()
     _check(lib.amgdd_residual_norm(h._h, _dev_ptr(b, n), _dev_ptr(x, n), ctypes.byref(out)))
     return out.value
+
+
+STATIC_MAX_ROWS = 16777216
+
+
+def amgdd_residual_norm_static(n, rowptr, colind, vals, b, x, out_norm, r=None, stream=None):
+    """amgdd_residual_norm_static: || b - A x ||_2 without any device allocation, for callers that cannot
+    allocate where they need the norm (all device memory already in a pool, no handle, no room for the
+    synchronisation of cudaFree).  Everything is a CUDA tensor on the current device that the CALLER made:
+    rowptr int64 [n+1], colind int32, vals / b / x float64, out_norm float64 [1] (written asynchronously on
+    `stream`, default torch's current stream: synchronise before reading it), r float64 [n] or None.  At most
+    STATIC_MAX_ROWS rows (the scratch is a fixed 512 KiB device array inside the library); concurrent calls on
+    one device race on that array.  The first call on a device should be made before any stream capture."""
+    import torch
+
+    def ptr(t, dt, count, name):
+        if t is None:
+            return None
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == dt and t.is_contiguous() and t.numel() >= count):
+            raise TypeError(f"{name}: expected a contiguous {dt} CUDA tensor with at least {count} entries")
+        return t.data_ptr()
+    n = int(n)
+    big = n > STATIC_MAX_ROWS or n <= 0          # the library reports these; do not touch the tensors' sizes first
+    nnz = 0 if big else int(colind.numel())
+    s = stream if stream is not None else torch.cuda.current_stream()
+    _check(lib.amgdd_residual_norm_static(
+        n, ptr(rowptr, torch.int64, 0 if big else n + 1, "rowptr"), ptr(colind, torch.int32, nnz, "colind"),
+        ptr(vals, torch.float64, nnz, "vals"), ptr(b, torch.float64, 0 if big else n, "b"),
+        ptr(x, torch.float64, 0 if big else n, "x"), ptr(r, torch.float64, 0 if big else n, "r"),
+        ptr(out_norm, torch.float64, 1, "out_norm"), s.cuda_stream))
 
 
 def amgdd_destroy(h: Handle):

@@ -7,7 +7,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-SOURCES = ["amgdd_api.cu", "amgdd_kernels.cu", "amgdd_fac.cu", "amgdd_assemble.cu", "amgdd_hierarchy.cpp", "amgdd_composite.cpp", "amgdd_pack.cpp", "amgdd_shard.cpp"]
+SOURCES = ["amgdd_api.cu", "amgdd_kernels.cu", "amgdd_fac.cu", "amgdd_assemble.cu", "amgdd_static.cu", "amgdd_hierarchy.cpp", "amgdd_composite.cpp", "amgdd_pack.cpp", "amgdd_shard.cpp"]
 HEADERS = ["amgdd_host.hpp", "amgdd_kernels.cuh", "amgdd_assemble.cuh", "amgdd_stream.hpp", os.path.join("..", "..", "include", "amgdd.h")]
 LIB = os.path.join(HERE, "libamgdd.so")
 

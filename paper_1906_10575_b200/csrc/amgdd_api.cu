@@ -52,6 +52,11 @@ struct SubMeta {                 // host-side record of one subdomain's blob
 
 }  // namespace
 
+namespace amgdd {
+// for entry points in other translation units (amgdd_static.cu): the string amgdd_last_error_detail returns
+void set_error_detail(const std::string& s) { g_detail = s; }
+}  // namespace amgdd
+
 struct amgdd_shard_plan_s {                     // a plan on its own (host only: amgdd_shard_plan_create) or the one of a handle
     std::unique_ptr<Hierarchy> H;
     std::unique_ptr<ShardPlan> own;
