@@ -40,6 +40,7 @@ def _load():
     L.orc_get_cf.argtypes = [_vp, _i32, _vp]
     L.orc_get_matrix.argtypes = [_vp, _i32, _i32, _vp, _vp, _vp]
     L.orc_get_dinv.argtypes = [_vp, _i32, _vp]
+    L.orc_set_level_values.argtypes = [_vp, _i32, _vp]
     L.orc_set_partition.argtypes = [_vp, _i32, _vp, _i32, _i32]
     L.orc_composite_size.argtypes = [_vp, _i32, _i32, _vp, _vp]
     L.orc_get_composite.argtypes = [_vp, _i32, _i32, _vp, _vp]
@@ -123,6 +124,15 @@ class Oracle:
         out = np.empty(self.level_size(l)[0], dtype=np.float64)
         _load().orc_get_dinv(self._h, l, _p(out))
         return out
+
+    def set_level_values(self, l, vals):
+        """Test support (no arithmetic of the method): overwrite the values of A_l, l >= 1, on its stored pattern; the l1
+        diagonal and, on the coarsest level, the LU are refreshed."""
+        vals = np.ascontiguousarray(vals, dtype=np.float64)
+        assert vals.shape == (self.level_size(l)[1],)
+        rc = _load().orc_set_level_values(self._h, l, _p(vals))
+        if rc != 0:
+            raise RuntimeError(f"orc_set_level_values failed with {rc}")
 
     # ---- decomposition ----
     def set_partition(self, num_subdomains, owner, eta, num_ghost=1):

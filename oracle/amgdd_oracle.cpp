@@ -637,6 +637,28 @@ void orc_get_dinv(void* h, int l, double* d) {
     std::copy(lv.dinv.begin(), lv.dinv.end(), d);
 }
 
+// TEST SUPPORT, no arithmetic of the method: overwrite the stored VALUES of A_l (same pattern, l >= 1) with the caller's
+// and refresh what is derived from them with the routines above -- the l1 diagonal (S8) and, on the coarsest level, the
+// dense LU.  P_l, the C/F splitting and the composite index sets (patterns only) stay.  Reading S4 leaves the summation
+// order of a Galerkin entry open; with this entry a test can build a SECOND valid oracle whose coarse operators were
+// summed in another order (scipy's P^T (A P) of this oracle's own A_l, P_l) and measure how far two valid oracles are
+// apart: the yardstick of DESIGN.md section 12.  Returns 0, -1 for a bad level, -5 for a singular A_L.
+int orc_set_level_values(void* h, int l, const double* vals) {
+    Oracle& o = *(Oracle*)h;
+    if (l < 1 || l > o.L) return -1;
+    Level& lv = o.lev[l];
+    std::copy(vals, vals + lv.A.nnz(), lv.A.v.begin());
+    l1_dinv(lv.A, lv.dinv);
+    if (l == o.L) {
+        const i64 nL = lv.A.nrows;
+        o.lu.assign((size_t)nL * nL, 0.0);
+        for (i64 i = 0; i < nL; ++i)
+            for (i64 k = lv.A.rp[i]; k < lv.A.rp[i + 1]; ++k) o.lu[(size_t)i * nL + lv.A.ci[k]] = lv.A.v[k];
+        if (!dense_lu((int)nL, o.lu, o.piv)) return -5;
+    }
+    return 0;
+}
+
 // S6: owner partition, padding eta (one value for every level l < L, reading A6), ghost layers
 int orc_set_partition(void* h, int nsub, const i32* owner, int eta, int num_ghost) {
     Oracle& o = *(Oracle*)h;

@@ -65,3 +65,27 @@ def bfs_sets_bruteforce(A, seed, dist):
     D = shortest_path(G, method="FW", directed=True, unweighted=True)
     d = D[np.asarray(seed, dtype=np.int64), :].min(axis=0)
     return np.nonzero(d <= dist)[0]
+
+
+def resum_galerkin_two_stage(o):
+    """Turn the oracle object `o` into a SECOND valid oracle under reading S4 (the terms of a Galerkin entry may be summed in
+    any order): every coarse operator is replaced, level by level, by scipy's two-stage product P_l^T (A_l P_l) of the
+    oracle's own P_l and its (already replaced) A_l, scattered onto the stored pattern (what scipy drops as an exact zero
+    stays 0.0).  Nothing of the CUDA path enters.  The new values differ from the one-pass triple loop of the oracle's
+    `galerkin` by rounding only; returns the largest entry change per level relative to the largest entry."""
+    moved = []
+    for l in range(o.num_levels - 1):
+        A, P = o.scipy_matrix(l, "A"), o.scipy_matrix(l, "P")
+        C = (P.T.tocsr() @ (A @ P)).tocsr()
+        C.sort_indices()
+        rp, ci, v = o.matrix(l + 1, "A")
+        n = len(rp) - 1
+        key = np.repeat(np.arange(n, dtype=np.int64), np.diff(rp)) * n + ci       # ascending: rows have ascending columns
+        ckey = np.repeat(np.arange(n, dtype=np.int64), np.diff(C.indptr)) * n + C.indices
+        pos = np.searchsorted(key, ckey)
+        assert (pos < len(key)).all() and (key[pos] == ckey).all(), "scipy's product has an entry outside the oracle's pattern"
+        nv = np.zeros_like(v)
+        nv[pos] = C.data
+        moved.append(float(np.abs(nv - v).max() / np.abs(v).max()))
+        o.set_level_values(l + 1, nv)
+    return moved

@@ -2,16 +2,17 @@
 
 Index work (levels, C/F splitting, sparsity patterns, composite index sets) is compared
 bit-exactly.  Floating point is compared with the bar of DESIGN.md section 12 ("Parity criterion"):
-    | ||r_k||_gpu - ||r_k||_oracle |  <=  1e-10 * ||r_k||_oracle + phi_k  [+ YARD * Y_k],
+    | ||r_k||_gpu - ||r_k||_oracle |  <=  1e-10 * ||r_k||_oracle + phi_k  [+ CY * Y_k],
     phi_k = 2^-52 * || |A_0| |x_k| + |b| ||_2          (fp64 rounding floor of a residual)
-    || x_gpu - x_oracle ||_inf  <=  1e-10 * || x_oracle ||_inf  [+ YARD * ||x~_k - x_k||_inf]
-The bracketed yardstick terms are used only for config 5 (1e4 coefficient jumps x 1e3 anisotropy),
-where the ORACLE ITSELF moves by about 1e-10 when A_0 is perturbed by one ulp: x~_k is the
-oracle's iterate on that perturbed matrix and Y_k = ||A_0 (x~_k - x_k)||_2.  YARD = 32: the library's
-coarse operators differ from the oracle's by the roundings of another Galerkin summation order on every
-level (reading S4), which moves the iterate 16-19 times as far as one ulp on A_0 does (measured table in
-DESIGN.md section 12); with the oracle's summation order (AMGDD_GALERKIN=fused) the yardstick terms are not
-needed in the first cycles.
+    || x_gpu - x_oracle ||_inf  <=  1e-10 * || x_oracle ||_inf  [+ CY * ||x'_k - x_k||_inf]
+The bracketed yardstick terms are used only for config 5 (1e4 coefficient jumps x 1e3 anisotropy).  Reading S4
+leaves the summation order of a Galerkin entry open (P:49 gives A_{l+1} = R_l A_l P_l, no order), and on this
+config two VALID ORACLES that differ in nothing but that order are farther apart than 1e-10: x'_k is the iterate
+of a second oracle whose coarse operators are scipy's two-stage product P_l^T (A_l P_l) of the oracle's own
+matrices on every level (tests/reference_global.py: resum_galerkin_two_stage; nothing of the CUDA path enters
+it), and Y_k = ||A_0 (x'_k - x_k)||_2.  CY = 4 was fixed before the library was compared against it.  Where the
+library is given the oracle's own summation order (AMGDD_GALERKIN=fused: coarse operators bit-identical) config 5
+is held to the PLAIN bar: x on every cycle, the residual norm on the cycles whose floor phi_k the bar still covers.
 """
 import numpy as np
 import pytest
@@ -23,7 +24,7 @@ from oracle import Oracle, max_threads
 pytestmark = pytest.mark.gpu
 
 RTOL = 1e-10
-YARD = 32.0     # multiple of the oracle's own 1-ulp sensitivity allowed on ill-conditioned cases (config 5); DESIGN.md section 12
+CY = 4.0        # multiple of the distance between two valid oracles (Galerkin sums in two orders) allowed on config 5; DESIGN.md section 12
 
 
 def _torch():
@@ -73,21 +74,25 @@ def floor_phi(p, x):
     return 2.0 ** -52 * np.linalg.norm(abs(A) @ np.abs(x) + np.abs(p.b))
 
 
-def ulp_perturbed_values(p):
-    """A symmetric +-1 ulp perturbation of the stored values of A_0 (sign by a hash of the
-    unordered index pair): the yardstick input of DESIGN.md §"Parity criterion"."""
-    rows = np.repeat(np.arange(p.n), np.diff(p.rowptr))
-    lo, hi = np.minimum(rows, p.colind).astype(np.int64), np.maximum(rows, p.colind).astype(np.int64)
-    sgn = ((lo * 2654435761 + hi * 40503) % 7 < 3) * 2.0 - 1.0
-    return p.vals * (1.0 + sgn * 2.0 ** -52)
+def second_oracle(p, **kw):
+    """The yardstick oracle of DESIGN.md section 12: the same hierarchy with every Galerkin operator summed in another
+    order (scipy's two-stage product of the oracle's own A_l, P_l)."""
+    from tests.reference_global import resum_galerkin_two_stage
+    o2 = orc_setup(p, **kw)
+    moved = resum_galerkin_two_stage(o2)
+    assert 0.0 < max(moved) < 1e-9, moved          # another rounding of the same sums, nothing else
+    return o2
 
 
-def run_parity(p, num_cycles, nfac=2, nu=1, yardstick=False, all_subdomains=False, **kw):
+def run_parity(p, num_cycles, nfac=2, nu=1, yardstick=False, all_subdomains=False, plain_x=False, plain_res_cycles=0, **kw):
     """Trajectory parity: both sides start from x = 0 and run num_cycles AMG-DD cycles; after every
-    cycle the residual norm and x are compared.  With yardstick=True the oracle is also run on the
-    1-ulp-perturbed matrix; its own deviation (x~_k - x_k in the max norm, and Y_k = ||A_0 (x~_k - x_k)||_2
-    for the residual norm) times YARD is added to the tolerance: the bar is then "as close to the
-    oracle as the fp64 conditioning of this problem allows" (Parity criterion)."""
+    cycle the residual norm and x are compared.  With yardstick=True a second valid oracle (second_oracle: Galerkin
+    sums in another order) runs alongside; its distance from the first (x'_k - x_k in the max norm, and
+    Y_k = ||A_0 (x'_k - x_k)||_2 for the residual norm) times CY is added to the tolerance: the bar is then "as
+    close to the oracle as two valid oracles are to each other" (Parity criterion).  plain_x=True
+    keeps x at the plain bar on every cycle and plain_res_cycles=n keeps the residual norm of the first n cycles
+    at the plain bar (+ phi_k) even with yardstick=True (used with AMGDD_GALERKIN=fused, where the library's
+    operators are the oracle's bit for bit)."""
     torch = _torch()
     smoother = kw.pop("smoother", 0)
     m, h = lib_setup(p, **kw)
@@ -102,10 +107,7 @@ def run_parity(p, num_cycles, nfac=2, nu=1, yardstick=False, all_subdomains=Fals
     xo = np.zeros(p.n)
     nt = max_threads()
     if yardstick:
-        import copy
-        pp = copy.copy(p)
-        pp.vals = ulp_perturbed_values(p)
-        o2 = orc_setup(pp, **kw)
+        o2 = second_oracle(p, **kw)
         o2.set_smoother(smoother)
         xo2 = np.zeros(p.n)
     report, ok = [], True
@@ -117,14 +119,15 @@ def run_parity(p, num_cycles, nfac=2, nu=1, yardstick=False, all_subdomains=Fals
         d_res = d_x = 0.0
         if yardstick:
             o2.cycle(p.b, xo2, nfac, nu, nthreads=nt)
-            d_res = np.linalg.norm(A @ (xo2 - xo))      # Y_k: residual change caused by the oracle's own deviation
+            d_res = np.linalg.norm(A @ (xo2 - xo))      # Y_k: residual change between the two valid oracles
             d_x = np.abs(xo2 - xo).max()
         xg_h = xg.cpu().numpy()
         phi = 2.0 ** -52 * np.linalg.norm(abs(A) @ np.abs(xo) + np.abs(p.b))
         e_res, e_x = abs(res_g[1] - r1), np.abs(xg_h - xo).max()
         xs = np.abs(xo).max()
         report.append((k + 1, r1, e_res / r1, e_x / xs, phi / r1, d_res / r1, d_x / xs))
-        ok = ok and e_res <= RTOL * r1 + phi + YARD * d_res and e_x <= RTOL * xs + YARD * d_x
+        ok = ok and e_res <= RTOL * r1 + phi + (0.0 if k < plain_res_cycles else CY * d_res)
+        ok = ok and e_x <= RTOL * xs + (0.0 if plain_x else CY * d_x)
     print("\n%s: cycle  ||r||_oracle  rel|d||r|||  rel|dx|_inf  floor phi/||r||  yardstick Y/||r||  D_x" % p.name)
     for row in report:
         print("  %2d  %.6e  %.2e  %.2e  %.2e  %.2e  %.2e" % row)
@@ -216,7 +219,11 @@ def test_galerkin_summation_orders(galerkin, monkeypatch):
     run_parity(p, 4)
     run_parity(wl.make_config(3, 32, eta=2), 3)
     run_parity(wl.make_config(6, 192, eta=2, parts_per_dim=4), 3)
-    run_parity(wl.make_config(5, 256), 6, yardstick=True)
+    if galerkin == "fused":
+        # the library's operators ARE the oracle's: config 5 at the plain bar, x on all cycles, ||r|| while 1e-10 covers its floor
+        run_parity(wl.make_config(5, 256), 6, yardstick=True, plain_x=True, plain_res_cycles=2)
+    else:
+        run_parity(wl.make_config(5, 256), 6, yardstick=True)
 
 
 def test_wide_column_indices():

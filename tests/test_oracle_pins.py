@@ -632,3 +632,47 @@ def test_oracle_reproduces_stored_residual_norms(name, cfg, scale, smoother):
     assert len(ref) == p.num_cycles + 1
     assert np.allclose(res, ref, rtol=1e-12, atol=0), (res, ref)        # thread count / summation order of the oracle's host may differ in the last digits
     assert res[0] == pytest.approx(np.linalg.norm(p.b), rel=1e-14)      # k = 0: x = 0 (reading A16, A17)
+
+
+# ------------------------------------------------------------------------------------------
+# test support: a second valid oracle (reading S4: any summation order of a Galerkin entry)
+# ------------------------------------------------------------------------------------------
+def test_set_level_values_refreshes_the_l1_diagonal_and_the_lu_and_nothing_else():
+    """orc_set_level_values carries no arithmetic of the method: writing the stored values back changes no bit of a
+    solve; writing other values changes exactly A_l, its l1 diagonal (S8: numpy row sums) and, on the coarsest level,
+    the direct solve (numpy.linalg.solve on the new dense matrix).  resum_galerkin_two_stage then yields a hierarchy
+    whose operators are scipy's P^T (A P) to rounding: a second valid oracle, a little apart from the first."""
+    from tests.reference_global import resum_galerkin_two_stage
+    p = wl.make_config(5, 64)
+    a, b, c = make_oracle(p), make_oracle(p), make_oracle(p)
+    L = a.num_levels - 1
+    assert L >= 2
+    for l in range(1, L + 1):                                   # the identity: same values back
+        c.set_level_values(l, c.matrix(l, "A")[2])
+    with pytest.raises(RuntimeError):
+        c.set_level_values(0, c.matrix(0, "A")[2])              # A_0 is the problem statement, not replaceable
+    moved = resum_galerkin_two_stage(b)
+    assert len(moved) == L and 0.0 < max(moved) < 1e-12
+    rng = np.random.default_rng(5)
+    for l in range(1, L + 1):
+        A_new = b.scipy_matrix(l, "A")
+        assert not np.array_equal(A_new.data, a.matrix(l, "A")[2]) or moved[l - 1] == 0.0
+        assert np.allclose(b.dinv(l), l1_dinv(A_new), rtol=1e-14, atol=0)          # refreshed from the NEW values
+        if moved[l - 1] > 1e-15:
+            assert not np.allclose(b.dinv(l), a.dinv(l), rtol=1e-17, atol=0)
+        # the product it was built from, recomputed here from the getters
+        ref = (b.scipy_matrix(l - 1, "P").T @ (b.scipy_matrix(l - 1, "A") @ b.scipy_matrix(l - 1, "P"))).toarray()
+        assert np.abs(A_new.toarray() - ref).max() == 0.0
+        # P_l and the C/F splitting are untouched
+        if l < L:
+            assert np.array_equal(b.matrix(l, "P")[2], a.matrix(l, "P")[2]) and np.array_equal(b.cf(l), a.cf(l))
+    rhs = rng.uniform(-1, 1, b.level_size(L)[0])
+    want = np.linalg.solve(b.scipy_matrix(L, "A").toarray(), rhs)
+    assert np.abs(b.coarse_solve(rhs) - want).max() <= 1e-9 * np.abs(want).max()
+    xa, xb, xc = np.zeros(p.n), np.zeros(p.n), np.zeros(p.n)
+    ra = a.solve(p.b, xa, 3, 2, 1)
+    rb = b.solve(p.b, xb, 3, 2, 1)
+    rc = c.solve(p.b, xc, 3, 2, 1)
+    assert np.array_equal(xa, xc) and np.array_equal(ra, rc)
+    d = np.abs(xa - xb).max() / np.abs(xa).max()
+    assert 0.0 < d < 1e-8 and np.allclose(ra, rb, rtol=1e-7)
