@@ -249,7 +249,10 @@ int amgdd_get_stats(amgdd_handle_t h, amgdd_stats_t* s);
  * amgdd_shard_plan_recv_filter on it (positions it owns or was already promised come back as redundant; the rest
  * becomes its receive list) and returns the redundant positions; the source removes them with
  * amgdd_shard_plan_apply_drop.  Then amgdd_shard_commit uploads the final lists.  A position indexes x (stage 0) or the
- * concatenated residual vector r_0 | r_1 | ... (offsets: amgdd_shard_plan_level).  amgdd_shard_plan_create builds a plan
+ * concatenated residual vector r_0 | r_1 | ... (offsets: amgdd_shard_plan_level).  The protocol runs ONCE per plan: a second
+ * amgdd_shard_plan_recv_filter or amgdd_shard_plan_apply_drop for the same (stage, peer) pair and a second amgdd_shard_commit
+ * return AMGDD_ERR_BAD_ARG and change nothing (the filter marks positions as held for good; repeating it would empty the
+ * send lists).  amgdd_shard_plan_create builds a plan
  * WITHOUT a CUDA device (the hierarchy is rebuilt on the host): tests of the protocol use it. */
 typedef struct amgdd_shard_plan_s* amgdd_shard_plan_t;
 int amgdd_setup_shard(int64_t n, const int64_t* rowptr, const int32_t* colind, const double* vals,

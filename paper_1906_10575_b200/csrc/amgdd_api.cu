@@ -1499,6 +1499,14 @@ int amgdd_shard_plan_recv_filter(amgdd_shard_plan_t p, int32_t stage, int32_t sr
     const i64 limit = S.stages[stage].vec == 0 ? (i64)S.have_x.size() : (i64)S.have.size();
     for (int64_t k = 0; k < count; ++k)
         if (announced[k] < 0 || announced[k] >= limit) { g_detail = "announced position out of range"; return AMGDD_ERR_BAD_ARG; }
+    std::vector<uint8_t>& done = S.stages[stage].filtered;
+    done.resize((size_t)S.nranks, 0);
+    if (done[src]) {
+        g_detail = "the index protocol already ran for stage " + std::to_string(stage) + ", source " + std::to_string(src) +
+                   " (it is not repeatable on a plan: set the handle or plan up again)";
+        return AMGDD_ERR_BAD_ARG;
+    }
+    done[src] = 1;
     std::vector<i64> red;
     shard_recv_filter(S, stage, src, announced, count, red);
     *nredundant = (int64_t)red.size();
@@ -1511,6 +1519,13 @@ int amgdd_shard_plan_apply_drop(amgdd_shard_plan_t p, int32_t stage, int32_t des
     ShardPlan& S = *p->S;
     STAGE_PEER_OK(S, stage, dest);
     if (count < 0 || (count > 0 && !redundant)) return AMGDD_ERR_BAD_ARG;
+    std::vector<uint8_t>& done = S.stages[stage].dropped;
+    done.resize((size_t)S.nranks, 0);
+    if (done[dest]) {
+        g_detail = "redundant positions were already removed for stage " + std::to_string(stage) + ", destination " + std::to_string(dest);
+        return AMGDD_ERR_BAD_ARG;
+    }
+    done[dest] = 1;
     shard_apply_drop(S, stage, dest, redundant, count);
     return AMGDD_SUCCESS;
 }
@@ -1522,6 +1537,7 @@ int amgdd_shard_plan_apply_drop(amgdd_shard_plan_t p, int32_t stage, int32_t des
 
 int amgdd_shard_commit(amgdd_handle_t h) {
     SHARD_OK(h);
+    if (h->shard_committed) { g_detail = "amgdd_shard_commit already ran on this handle (its device lists are in use)"; return AMGDD_ERR_BAD_ARG; }
     DEVICE_SCOPE(h);
     const ShardPlan& S = *h->shard;
     const int R = S.nranks;

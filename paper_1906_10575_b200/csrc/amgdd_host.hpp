@@ -182,6 +182,9 @@ void layout_blob(SubdomainBlob& out);
 struct ShardStage {
     int vec = 1;                               // 0: positions index x, 1: the concatenated residual vector r_0 | r_1 | ...
     std::vector<std::vector<i64>> send, recv;  // per peer rank: positions, in the order both sides agree on
+    // the index protocol runs ONCE: recv_filter marks positions as held for good, so a second pass over a (stage, peer)
+    // pair would report every position redundant and empty the send lists; these flags make the C ABI refuse it
+    std::vector<uint8_t> filtered, dropped;    // per peer rank, sized on first use
 };
 struct ShardPlan {
     int rank = 0, nranks = 1, L = 0, sub_lo = 0, sub_hi = 0;

@@ -159,3 +159,28 @@ def test_shard_argument_checks():
     assert e.value.code == -1
     with pytest.raises(m.AmgddError):
         m.amgdd_shard_plan_create(p.n, p.rowptr, p.colind, p.vals, p.num_subdomains, p.owner, p.eta, rank=0, nranks=5)   # more ranks than subdomains
+
+
+def test_index_protocol_is_refused_a_second_time():
+    """The redundancy removal marks positions as held for good, so a second pass would drop every send list.  The C ABI
+    refuses it (AMGDD_ERR_BAD_ARG) and leaves the lists of the first pass as they are."""
+    import paper_1906_10575_b200 as m
+    from paper_1906_10575_b200.sharded import LocalComm, run_index_protocol
+    p = wl.make_config(1, 21, parts_per_dim=2)
+    R = 2
+    plans = {r: m.amgdd_shard_plan_create(p.n, p.rowptr, p.colind, p.vals, p.num_subdomains, p.owner, p.eta, p.max_levels,
+                                          p.theta, p.coarse_max, rank=r, nranks=R) for r in range(R)}
+    run_index_protocol(plans, LocalComm(R))
+    nstages = m.amgdd_shard_plan_info(plans[0])["num_stages"]
+    before = {(r, w, s, q): m.amgdd_shard_plan_list(plans[r], w, s, q).copy()
+              for r in range(R) for w in (0, 1) for s in range(nstages) for q in range(R)}
+    assert sum(len(v) for v in before.values()) > 0
+    with pytest.raises(m.AmgddError) as e:
+        run_index_protocol(plans, LocalComm(R))
+    assert e.value.code == -1 and "already" in str(e.value)
+    with pytest.raises(m.AmgddError) as e:
+        m.amgdd_shard_plan_apply_drop(plans[0], 0, 1, before[(0, 0, 0, 1)])
+    assert e.value.code == -1 and "already" in str(e.value)
+    for key, want in before.items():
+        r, w, s, q = key
+        assert np.array_equal(m.amgdd_shard_plan_list(plans[r], w, s, q), want), key
