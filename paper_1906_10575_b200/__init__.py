@@ -169,6 +169,7 @@ def amgdd_set_stream(h: Handle, stream=None):
     import torch
     s = stream if stream is not None else torch.cuda.current_stream()
     _check(lib.amgdd_set_stream(h._h, s.cuda_stream))
+    h._stream = int(s.cuda_stream)                   # remembered for the stream check of sharded.py (0 / absent: legacy default stream)
 
 
 def amgdd_solve(h: Handle, b, x, num_cycles, num_fac_cycles=2, relax_sweeps=1, want_norms=True):

@@ -106,18 +106,25 @@ def run_index_protocol(plans, comm):
                 amgdd_shard_plan_apply_drop(plans[s], stage, d, back[s][d])
 
 
-_STAGE_CACHE = {}
-
-
 def setup_exchange(handles, comm):
     """After amgdd_setup_shard on every rank: index protocol, then upload of the final lists."""
     plans = {r: amgdd_get_shard_plan(h) for r, h in handles.items()}
     run_index_protocol(plans, comm)
     for h in handles.values():
         amgdd_shard_commit(h)
-        for key in [k for k in _STAGE_CACHE if k[0] == id(h)]:
-            del _STAGE_CACHE[key]
+        h._stage_cache = {}            # counts and send buffers per stage live ON the handle object and die with it
     return plans
+
+
+def _same_stream(h, tensor):
+    """The library enqueues pack / unpack / solve on the handle's stream; the exchange (torch.distributed, torch.cat, the
+    buffers) runs on torch's current stream.  Nothing orders the two, so they must be the same stream."""
+    import torch
+    mine = int(getattr(h, "_stream", 0) or 0)
+    cur = int(torch.cuda.current_stream(tensor.device).cuda_stream) if tensor.is_cuda else 0
+    if mine != cur:
+        raise RuntimeError(f"the handle works on CUDA stream {mine:#x} but torch's current stream is {cur:#x}: the packed buffers would "
+                           "race with the exchange; call amgdd_set_stream(h) under the stream the cycle runs on")
 
 
 def sharded_cycle(handles, b, x, comm, num_fac_cycles=2, relax_sweeps=1, want_norm=False):
@@ -125,16 +132,22 @@ def sharded_cycle(handles, b, x, comm, num_fac_cycles=2, relax_sweeps=1, want_no
     valid on the rank's dofs).  Returns ||b - A x||_2 of the iterate the cycle STARTED from if want_norm."""
     import torch
     R = comm.nranks
-    nstages = 2 * (amgdd_shard_plan_info(amgdd_get_shard_plan(next(iter(handles.values()))))["num_levels"] - 1) + 2
+    for r, h in handles.items():
+        _same_stream(h, x[r])
+        if not hasattr(h, "_stage_cache"):
+            h._stage_cache = {}
+    h0 = next(iter(handles.values()))
+    if "nstages" not in h0._stage_cache:
+        h0._stage_cache["nstages"] = 2 * (amgdd_shard_plan_info(amgdd_get_shard_plan(h0))["num_levels"] - 1) + 2
+    nstages = h0._stage_cache["nstages"]
     norm = None
     for stage in range(nstages):
         sc, rc, bufs = {}, {}, {}
         for r, h in handles.items():
-            key = (id(h), stage)
-            if key not in _STAGE_CACHE:                                    # counts and the send buffer of a stage never change
+            if stage not in h._stage_cache:                                # counts and the send buffer of a stage never change
                 s_cnt, r_cnt = amgdd_shard_stage_counts(h, stage, R)
-                _STAGE_CACHE[key] = (s_cnt, r_cnt, torch.empty(int(s_cnt.sum()), dtype=torch.float64, device=x[r].device))
-            sc[r], rc[r], bufs[r] = _STAGE_CACHE[key]
+                h._stage_cache[stage] = (s_cnt, r_cnt, torch.empty(int(s_cnt.sum()), dtype=torch.float64, device=x[r].device))
+            sc[r], rc[r], bufs[r] = h._stage_cache[stage]
             amgdd_shard_stage_pack(h, stage, b[r], x[r], bufs[r])
         if want_norm and stage == 1:                                       # the owned rows' r_0 was just computed
             sq = comm.allreduce_sum({r: amgdd_shard_sqnorm(h) for r, h in handles.items()})
@@ -154,6 +167,7 @@ def allgather_cycle(handles, b, x, comm, num_fac_cycles=2, relax_sweeps=1):
     R = comm.nranks
     bufs, counts = {}, None
     for r, h in handles.items():
+        _same_stream(h, x[r])
         counts = [amgdd_shard_owned_count(h, q) for q in range(R)]
         bufs[r] = torch.empty(counts[r], dtype=torch.float64, device=x[r].device)
         amgdd_shard_pack_owned(h, x[r], bufs[r])

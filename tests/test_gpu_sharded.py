@@ -96,3 +96,26 @@ def test_shard_handle_reports_local_subdomains():
         assert st["num_subdomains"] == info["sub_hi"] - info["sub_lo"]
         tot += st["num_subdomains"]
     assert tot == p.num_subdomains
+
+
+def test_sharded_cycle_refuses_a_handle_on_another_stream():
+    """The exchange runs on torch's current stream, the library on the handle's: the driver checks that they are one."""
+    import torch
+    from paper_1906_10575_b200.sharded import allgather_cycle, sharded_cycle
+    p = wl.make_config(1)
+    m, handles, comm, plans = _setup(p, 2)
+    b = torch.from_numpy(p.b).cuda()
+    x = {r: torch.zeros(p.n, dtype=torch.float64, device="cuda") for r in range(2)}
+    bb = {r: b for r in range(2)}
+    side = torch.cuda.Stream()
+    m.amgdd_set_stream(handles[1], side)
+    for cycle in (sharded_cycle, allgather_cycle):
+        with pytest.raises(RuntimeError, match="current stream"):
+            cycle(handles, bb, x, comm, p.num_fac_cycles, p.relax_sweeps)
+    with torch.cuda.stream(side):                      # under that stream for both handles: accepted
+        m.amgdd_set_stream(handles[0], side)
+        sharded_cycle(handles, bb, x, comm, p.num_fac_cycles, p.relax_sweeps)
+    side.synchronize()
+    assert hasattr(handles[0], "_stage_cache") and "nstages" in handles[0]._stage_cache
+    for h in handles.values():
+        m.amgdd_destroy(h)
