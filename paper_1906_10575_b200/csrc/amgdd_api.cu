@@ -385,7 +385,7 @@ int build_composites_device(amgdd_handle_s* h, const std::vector<i32>& owner, in
 
     const int nw = std::max(1, std::min(nthreads, P));
     std::vector<std::unique_ptr<CompositeBuilder>> builders(nw);
-    const int batch = std::max(1, env_int("AMGDD_SETUP_BATCH", 256));
+    const int batch = std::min(P, std::max(1, env_int("AMGDD_SETUP_BATCH", 256)));   // scratch is sized per subdomain of a batch
     const int thin = std::min(h->window, THIN_WINDOW);
     Arena arena;
     cudaStream_t st = h->stream;
@@ -411,6 +411,11 @@ int build_composites_device(amgdd_handle_s* h, const std::vector<i32>& owner, in
     long long* d_bm_off = nullptr;
     unsigned* d_bm = nullptr;
     int* d_frontier = nullptr;
+    // a frontier (or a seed list) holds distinct points of one level, so it never exceeds the largest level: the scratch of a
+    // small problem is small (it used to be 3 MiB per subdomain of the batch whatever the size)
+    long long max_nl = 1;
+    for (int l = 0; l <= L; ++l) max_nl = std::max<long long>(max_nl, h->H.lv[l].A.nrows);
+    const int frontier_cap = (int)std::min<long long>(SET_FRONTIER_CAP, max_nl);
     int* d_owned_all = nullptr;
     SetLevelOut* d_set_out = nullptr;
     int** d_list_dst = nullptr;
@@ -423,7 +428,7 @@ int build_composites_device(amgdd_handle_s* h, const std::vector<i32>& owner, in
         CUDA_TRY(tmp.put(&d_bm_off, bm_off.data(), bm_off.size()));
         CUDA_TRY(tmp.alloc(&d_bm, (size_t)batch * 2 * (size_t)bm_off[L + 1]));
         CUDA_TRY(cudaMemsetAsync(d_bm, 0, (size_t)batch * 2 * (size_t)bm_off[L + 1] * sizeof(unsigned), st));
-        CUDA_TRY(tmp.alloc(&d_frontier, (size_t)batch * 3 * SET_FRONTIER_CAP));
+        CUDA_TRY(tmp.alloc(&d_frontier, (size_t)batch * 3 * (size_t)frontier_cap));
         std::vector<int> flat_owned;
         flat_owned.reserve((size_t)h->n);
         for (int p = 0; p < P; ++p) { flat_owned.insert(flat_owned.end(), owned[p].begin(), owned[p].end()); owned_off[p + 1] = (long long)flat_owned.size(); }
@@ -448,7 +453,7 @@ int build_composites_device(amgdd_handle_s* h, const std::vector<i32>& owner, in
                 j.owned = d_owned_all + owned_off[p0 + k]; j.n_owned = (int)(owned_off[p0 + k + 1] - owned_off[p0 + k]);
                 j.bm_real = d_bm + (size_t)k * 2 * (size_t)bm_off[L + 1];
                 j.bm_ghost = j.bm_real + bm_off[L + 1];
-                j.frontier = d_frontier + (size_t)k * 3 * SET_FRONTIER_CAP;
+                j.frontier = d_frontier + (size_t)k * 3 * (size_t)frontier_cap; j.frontier_cap = frontier_cap;
                 j.out = d_set_out + (size_t)k * (L + 1);
                 j.list_dst = d_list_dst + (size_t)k * (L + 1);
             }
@@ -1198,7 +1203,9 @@ int amgdd_solve(amgdd_handle_t h, const double* b, double* x, int32_t num_cycles
             if (!h->graph_off) {
                 cudaStream_t user = h->stream;
                 cudaGraph_t graph = nullptr;
-                bool ok = cudaStreamBeginCapture(h->capture_stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+                const char* why = "cudaStreamBeginCapture";
+                cudaError_t ce = cudaStreamBeginCapture(h->capture_stream, cudaStreamCaptureModeThreadLocal);
+                bool ok = ce == cudaSuccess;
                 if (ok) {
                     h->stream = h->capture_stream;
                     enqueue_residual(h, b, x, h->d_r_all, 0);
@@ -1207,14 +1214,24 @@ int amgdd_solve(amgdd_handle_t h, const double* b, double* x, int32_t num_cycles
                         launch_spmv(g.r_rp, g.r_ci, g.r_v, g.r_blk, g.r_nblk, h->d_r_all + h->r_off[l],
                                     h->d_r_all + h->r_off[l + 1], h->stream);
                     }
-                    ok = cudaMemsetAsync(h->d_counter, 0, sizeof(int), h->stream) == cudaSuccess;
+                    ce = cudaGetLastError();                                 // a launch-configuration error of the global kernels
+                    if (ce != cudaSuccess) { ok = false; why = "a residual / restriction launch during capture"; }
+                    if (ok && (ce = cudaMemsetAsync(h->d_counter, 0, sizeof(int), h->stream)) != cudaSuccess) { ok = false; why = "cudaMemsetAsync during capture"; }
                     launch_fac(prm, h->fac_cfg, h->stream);
+                    if (ok && (ce = cudaGetLastError()) != cudaSuccess) { ok = false; why = "the fac_kernel launch during capture"; }
                     h->stream = user;
-                    ok = (cudaStreamEndCapture(h->capture_stream, &graph) == cudaSuccess) && ok && graph != nullptr;
+                    const cudaError_t ee = cudaStreamEndCapture(h->capture_stream, &graph);
+                    if (ok && (ee != cudaSuccess || !graph)) { ok = false; ce = ee; why = "cudaStreamEndCapture"; }
                 }
-                if (ok) ok = cudaGraphInstantiate(&h->cycle_graph, graph, 0) == cudaSuccess;
+                if (ok && (ce = cudaGraphInstantiate(&h->cycle_graph, graph, 0)) != cudaSuccess) { ok = false; why = "cudaGraphInstantiate"; }
                 if (graph) cudaGraphDestroy(graph);
-                if (!ok) { cudaGetLastError(); h->cycle_graph = nullptr; h->graph_off = true; }
+                if (!ok) {
+                    // fall back to kernel-by-kernel launches for the rest of the handle's life, and say why: the call itself
+                    // still succeeds if those launches do (a real launch error is reported by them below)
+                    cudaGetLastError();
+                    h->cycle_graph = nullptr; h->graph_off = true;
+                    g_detail = std::string("CUDA graph of the cycle not used (") + why + ": " + cudaGetErrorString(ce) + "); launching kernel by kernel";
+                }
                 else {
                     h->graph_b = b; h->graph_x = x; h->graph_nfac = num_fac_cycles; h->graph_nu = relax_sweeps;
                     h->graph_smoother = h->smoother; h->graph_nops = h->prog_nops;
@@ -1223,6 +1240,7 @@ int amgdd_solve(amgdd_handle_t h, const double* b, double* x, int32_t num_cycles
         }
         if (h->cycle_graph) {
             for (int k = 0; k < num_cycles; ++k) CUDA_TRY(cudaGraphLaunch(h->cycle_graph, h->stream));
+            CUDA_TRY(cudaGetLastError());
             launches[0] = 2LL * num_cycles; launches[1] = (long long)L * num_cycles; launches[2] = num_cycles;
             for (int i = 0; i < 3; ++i) h->prof_launches[i] = launches[i];
             return AMGDD_SUCCESS;

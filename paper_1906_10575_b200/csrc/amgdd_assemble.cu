@@ -292,7 +292,7 @@ constexpr int SET_THREADS = 256;
 
 // one layer of breadth-first growth: every point of `cur` marks its unmarked neighbours in `mark` (those not in `skip`)
 // and appends them to `next`; returns false when `next` overflowed
-__device__ bool grow_layer(const DevCsr64& A, const int* cur, int ncur, unsigned* mark, const unsigned* skip, int* next, int* s_count,
+__device__ bool grow_layer(const DevCsr64& A, const int* cur, int ncur, unsigned* mark, const unsigned* skip, int* next, int cap, int* s_count,
                            int* s_lo, int* s_hi, int* s_over) {
     for (int q = threadIdx.x; q < ncur; q += SET_THREADS) {
         const int i = cur[q];
@@ -303,7 +303,7 @@ __device__ bool grow_layer(const DevCsr64& A, const int* cur, int ncur, unsigned
             const unsigned old = atomicOr(mark + (j >> 5), bit);
             if (!(old & bit)) {
                 const int pos = atomicAdd(s_count, 1);
-                if (pos < SET_FRONTIER_CAP) next[pos] = j; else *s_over = 1;
+                if (pos < cap) next[pos] = j; else *s_over = 1;
                 atomicMin(s_lo, j >> 5);
                 atomicMax(s_hi, j >> 5);
             }
@@ -318,9 +318,10 @@ __global__ void __launch_bounds__(SET_THREADS) asm_sets_grow_kernel(SetJob* __re
     SetJob& J = jobs[blockIdx.x];
     __shared__ int s_count, s_lo, s_hi, s_over, s_nseed;
     int* bufA = J.frontier;
-    int* bufB = J.frontier + SET_FRONTIER_CAP;
-    int* seeds = J.frontier + 2 * SET_FRONTIER_CAP;
-    if (threadIdx.x == 0) { s_over = 0; s_nseed = J.n_owned <= SET_FRONTIER_CAP ? J.n_owned : 0; if (J.n_owned > SET_FRONTIER_CAP) s_over = 1; }
+    const int cap = J.frontier_cap;                  // min(SET_FRONTIER_CAP, n_0): no frontier holds more points than the largest level has
+    int* bufB = J.frontier + cap;
+    int* seeds = J.frontier + 2 * cap;
+    if (threadIdx.x == 0) { s_over = 0; s_nseed = J.n_owned <= cap ? J.n_owned : 0; if (J.n_owned > cap) s_over = 1; }
     __syncthreads();
     for (int q = threadIdx.x; q < s_nseed; q += SET_THREADS) seeds[q] = J.owned[q];       // B_0^p = Omega_0^p
     __syncthreads();
@@ -348,7 +349,7 @@ __global__ void __launch_bounds__(SET_THREADS) asm_sets_grow_kernel(SetJob* __re
         int* cur = bufA;
         int* nxt = bufB;
         for (int d = 0; d < eta && ncur > 0; ++d) {                       // D_l^p: within eta of B_l^p
-            if (!grow_layer(H.A, cur, ncur, real, nullptr, nxt, &s_count, &s_lo, &s_hi, &s_over)) break;
+            if (!grow_layer(H.A, cur, ncur, real, nullptr, nxt, cap, &s_count, &s_lo, &s_hi, &s_over)) break;
             ncur = s_count;
             n_real += ncur;
             __syncthreads();
@@ -360,7 +361,7 @@ __global__ void __launch_bounds__(SET_THREADS) asm_sets_grow_kernel(SetJob* __re
         // ghost layers: only the points of the last real layer can have neighbours outside D_l^p
         int n_ghost = 0;
         for (int d = 0; d < num_ghost && ncur > 0; ++d) {
-            if (!grow_layer(H.A, cur, ncur, ghost, real, nxt, &s_count, &s_lo, &s_hi, &s_over)) break;
+            if (!grow_layer(H.A, cur, ncur, ghost, real, nxt, cap, &s_count, &s_lo, &s_hi, &s_over)) break;
             ncur = s_count;
             n_ghost += ncur;
             __syncthreads();
@@ -381,7 +382,7 @@ __global__ void __launch_bounds__(SET_THREADS) asm_sets_grow_kernel(SetJob* __re
                 const int i = 32 * w + b;
                 if (H.cf[i] > 0) {
                     const int pos = atomicAdd(&s_nseed, 1);
-                    if (pos < SET_FRONTIER_CAP) seeds[pos] = H.coarse_of[i]; else s_over = 1;
+                    if (pos < cap) seeds[pos] = H.coarse_of[i]; else s_over = 1;
                 }
             }
         }

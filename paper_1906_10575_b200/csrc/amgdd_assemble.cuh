@@ -70,7 +70,7 @@ struct AsmCopy {                // gid / owned-index copies and the gather of th
 // ---- composite index sets on the device (S6, S7; eq. 1): breadth-first growth with bitmaps -----------------
 // One CTA per subdomain.  Pass 1 (asm_sets_grow) walks the levels top down: D_l^p = points within eta of B_l^p in the graph
 // of A_l, the ghost layers around it, B_{l+1}^p = coarse images of the C-points of D_l^p; membership lives in two bitmaps
-// per (subdomain, level), the frontiers in a scratch of SET_FRONTIER_CAP indices (a larger frontier raises `overflow` and
+// per (subdomain, level), the frontiers in a scratch of min(SET_FRONTIER_CAP, n_0) indices (a larger frontier raises `overflow` and
 // the host path takes the batch).  Pass 2 (asm_sets_extract) turns the bitmaps into the ascending index lists (S7) at the
 // offsets the host laid out from the sizes, sums the row lengths the layout needs, and clears the bitmaps again.
 struct SetLevelOut {            // per (subdomain, level), written by pass 1 (sizes, range) and pass 2 (sums)
@@ -86,7 +86,8 @@ struct SetJob {
     int overflow;               // out: a frontier exceeded the scratch
     unsigned* bm_real;          // DEVICE scratch: bitmaps of all levels, level l at word offset bm_off[l]
     unsigned* bm_ghost;
-    int* frontier;              // DEVICE scratch: 3 * SET_FRONTIER_CAP ints
+    int* frontier;              // DEVICE scratch: 3 * frontier_cap ints
+    int frontier_cap;           // capacity of each of the three index buffers: min(SET_FRONTIER_CAP, largest level size)
     SetLevelOut* out;           // DEVICE: L + 1 records
     int* const* list_dst;       // pass 2: DEVICE array of L + 1 pointers: where real | ghost of level l go (null: shared level)
     int* owned_local_dst;       // pass 2: n_owned local indices (level 0) of the owned dofs
