@@ -44,6 +44,8 @@ def parse_args():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--cpu-sample", type=int, default=None, help="subdomains in the oracle's timed sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the short runs of configs 1, 2, 5 after the default config-4 line")
+    ap.add_argument("--all-configs", action="store_true", help="per_config also runs config 3 at eta = 1 (112 GB on the device, long setup)")
     ap.add_argument("--smoother", type=int, default=0, choices=[0, 1], help="0: l1-Jacobi (BASELINE), 1: CF l1-Jacobi (P:275)")
     ap.add_argument("--shard", default=None, choices=["alg5", "allgather"],
                     help="under torchrun: shard the subdomains over the ranks (NEXT 4; Alg. 5 exchange or all-gather of x) "
@@ -167,7 +169,7 @@ def oracle_time_per_cycle(p, sample, steps, warmup, smoother=0, sample_1thread=N
 
     for _ in range(max(1, warmup)):
         o.cycle(p.b, x, p.num_fac_cycles, p.relax_sweeps, subdomains=subs, nthreads=nthreads)   # also builds the composite grids (setup)
-    n1 = max(1, min(len(subs), sample_1thread or max(1, len(subs) // 4)))
+    n1 = max(1, min(len(subs), sample_1thread or min(64, max(1, len(subs) // 4))))
     subs1 = subs[np.unique(np.linspace(0, len(subs) - 1, n1).astype(int))]
     one = subs[len(subs) // 2:len(subs) // 2 + 1]
 
@@ -198,7 +200,9 @@ def oracle_time_per_cycle(p, sample, steps, warmup, smoother=0, sample_1thread=N
 def default_cpu_sample(p):
     # about 20-30 s of CPU work in total: ~0.06 core-seconds per config-4 subdomain-cycle on the box's 16 cores
     # (config 4: 256 subdomains x 4 steps on all cores ~ 4 s, 64 subdomains x 3 steps on one thread ~ 12 s)
-    return {1: 4, 2: 64, 3: 16, 4: 256, 5: 512}.get(int(p.name[3]), 32)
+    # config 4: ALL 4096 subdomains on all cores (3 timed cycles of about 4.3 s each after one warm-up cycle that also builds the
+    # composite grids), so the all-cores value is a measured full cycle, not an extrapolation; the one-thread leg stays sampled
+    return {1: 4, 2: 64, 3: 16, 4: 4096, 5: 1024}.get(int(p.name[3]), 32)
 
 
 def run_reference(args, p, rank, world):
@@ -211,10 +215,10 @@ def run_reference(args, p, rank, world):
     line = {
         "impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus,
         "steps": steps, "warmup": warmup, "ms_per_step": cb["value"], "higher_is_better": False,
-        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "scaling": "weak" if args.gpus > 1 else "none", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": workload_name(p, args), "n_dofs": p.n, "nnz": p.nnz, "subdomains": p.num_subdomains, "eta": p.eta,
                    "theta": p.theta, "fac_cycles_per_step": p.num_fac_cycles, "relax_sweeps": p.relax_sweeps},
-        "note": "CPU oracle as it stands, bounded sample of the workload (cpu_baseline.sample), timed steps capped at 3",
+        "note": "CPU oracle as it stands (cpu_baseline.sample says which subdomains a step ran: all of them on config 4), timed steps capped at 3",
         "cpu_baseline": cb,
         "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -225,6 +229,53 @@ def run_reference(args, p, rank, world):
 # ---------------------------------------------------------------------------------------------
 # B200 arm
 # ---------------------------------------------------------------------------------------------
+def measure_config(m, torch, cfg, steps, warmup, eta=None):
+    """Short run of another BASELINE.json config for the `per_config` record (north_star: "report throughput on synthetic
+    Poisson and variable-coefficient diffusion systems"): the same step as the headline line -- one AMG-DD cycle, asynchronous
+    calls timed with CUDA events on the handle's stream -- plus the AlgFAC launch time from the library's own events."""
+    import workloads as wl
+    p = wl.make_config(cfg, None, eta=eta)
+    t0 = time.time()
+    h = m.amgdd_setup(p.n, p.rowptr, p.colind, p.vals, p.num_subdomains, p.owner, p.eta, p.num_ghost,
+                      p.max_levels, p.theta, p.coarse_max)
+    setup_s = time.time() - t0
+    st = m.amgdd_get_stats(h)
+    stream = torch.cuda.current_stream()
+    m.amgdd_set_stream(h, stream)
+    b = torch.from_numpy(p.b).cuda()
+    x = torch.zeros(p.n, dtype=torch.float64, device="cuda")
+    nfac, nu = p.num_fac_cycles, p.relax_sweeps
+    res = m.amgdd_solve(h, b, x, min(p.num_cycles, 5), nfac, nu)
+    x.zero_()
+    for _ in range(max(3, warmup)):
+        m.amgdd_solve(h, b, x, 1, nfac, nu, want_norms=False)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record(stream)
+    for _ in range(steps):
+        m.amgdd_solve(h, b, x, 1, nfac, nu, want_norms=False)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms_step = e0.elapsed_time(e1) / steps
+    fac_ms = []
+    for _ in range(steps):
+        m.amgdd_solve(h, b, x, 1, nfac, nu)
+        fac_ms.append(m.amgdd_last_solve_profile(h)["ms_fac"])
+    fac = float(np.mean(fac_ms))
+    peak, _ = measured_peak()
+    model_bytes = st["model_bytes_fac_iter"][0] + (nfac - 1) * st["model_bytes_fac_iter"][1]
+    stream_bytes = st["stream_bytes_fac_iter"][0] + (nfac - 1) * st["stream_bytes_fac_iter"][1]
+    out = {"ms_per_step": ms_step, "fac_ms": fac, "frac": model_bytes / (fac * 1e-3) / 1e9 / peak,
+           "frac_stream": stream_bytes / (fac * 1e-3) / 1e9 / peak, "stream_bytes_per_step": stream_bytes,
+           "l2": "inputs larger than L2" if stream_bytes > 2 * 126e6 else "matrix streams fit the 126 MB L2: an L2-resident number, no flush between steps",
+           "n_dofs": p.n, "subdomains": p.num_subdomains, "eta": p.eta, "levels": st["num_levels"], "device_bytes": st["device_bytes"],
+           "setup_seconds": setup_s, "steps": steps, "residual_drop_per_cycle": (res[1:] / res[:-1]).tolist()[:3]}
+    m.amgdd_destroy(h)
+    del b, x
+    torch.cuda.empty_cache()
+    return p.name, out
+
+
 def run_b200(args, p, rank, world, local_rank):
     import torch
     import torch.distributed as dist
@@ -332,7 +383,7 @@ def run_b200(args, p, rank, world, local_rank):
         line = {
             "metric": METRIC, "value": ms_step, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": False,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "scaling": "weak" if args.gpus > 1 else "none", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {
                 "workload": wname, "n_dofs": p.n, "nnz": p.nnz, "subdomains": p.num_subdomains, "eta": p.eta,
                 "theta": p.theta, "levels": st["num_levels"], "fac_cycles_per_step": nfac, "relax_sweeps": nu,
@@ -385,10 +436,17 @@ def run_b200(args, p, rank, world, local_rank):
                 "steps": [{"kind": k, "level": l, "cycles": c / (args.steps * p.num_subdomains), "barrier": bw / (args.steps * p.num_subdomains),
                            "ring_wait": rw / (args.steps * p.num_subdomains), "operand_wait": ow / (args.steps * p.num_subdomains)}
                           for k, l, c, bw, rw, ow in ops]}
-        if not args.no_cpu_baseline:
+        if not args.no_cpu_baseline or not args.no_per_config:
             m.amgdd_destroy(h)
             del b, x
             torch.cuda.empty_cache()
+        if not args.no_per_config and not distributed and args.config == 4 and args.scale is None and args.eta is None and not args.smoother:
+            # the other BASELINE.json configs, a few seconds each (config 3 needs 112 GB and a long setup: --all-configs)
+            line["per_config"] = {}
+            for cfg, eta in [(1, None), (2, None), (5, None)] + ([(3, 1)] if args.all_configs else []):
+                name, rec = measure_config(m, torch, cfg, max(args.steps, 10), args.warmup, eta)
+                line["per_config"][name] = rec
+        if not args.no_cpu_baseline:
             line["cpu_baseline"] = oracle_time_per_cycle(p, args.cpu_sample or default_cpu_sample(p), 3, 1, args.smoother)
         print(json.dumps(line))
     if distributed:

@@ -1,6 +1,6 @@
 """bench.py under torchrun with 2 ranks on CPU (gloo world): the reference arm runs on rank 0 alone and
-prints exactly one JSON line; the other rank exits 0 without work.  The path does not shard
-("replicas only"), so there is no data-path collective to test."""
+prints exactly one JSON line; the other rank exits 0 without work.  (The sharded cycle with its Alg. 5 exchange,
+DESIGN.md section 8, is covered by tests/test_shard_plan.py, tests/test_shard_gloo.py and tests/test_gpu_sharded.py.)"""
 import json
 import os
 import subprocess
