@@ -119,3 +119,35 @@ def test_sharded_cycle_refuses_a_handle_on_another_stream():
     assert hasattr(handles[0], "_stage_cache") and "nstages" in handles[0]._stage_cache
     for h in handles.values():
         m.amgdd_destroy(h)
+
+
+@pytest.mark.parametrize("cfg,scale,R", [(4, 24, 2), (2, 32, 3)])
+def test_sharded_cycle_against_the_oracle(cfg, scale, R):
+    """The sharded cycle (Alg. 5 exchange) compared with the ORACLE directly, not through the unsharded library
+    path: residual norms and the x assembled from the ranks' own dofs, per cycle, at the plain 1e-10 bar."""
+    import torch
+    from oracle import Oracle, max_threads
+    from paper_1906_10575_b200.sharded import sharded_cycle
+    p = wl.make_config(cfg, scale)
+    m, handles, comm, plans = _setup(p, R)
+    own0 = torch.from_numpy(m.amgdd_shard_plan_owner_rank(plans[0], 0)).cuda()
+    o = Oracle(p.n, p.rowptr, p.colind, p.vals, p.theta, p.max_levels, p.coarse_max)
+    o.set_partition(p.num_subdomains, p.owner, p.eta, p.num_ghost)
+    b = torch.from_numpy(p.b).cuda()
+    x = {r: torch.zeros(p.n, dtype=torch.float64, device="cuda") for r in range(R)}
+    bb = {r: b for r in range(R)}
+    xo = np.zeros(p.n)
+    for k in range(3):
+        r_before = o.residual_norm(p.b, xo)
+        for r in range(R):
+            x[r][own0 != r] = float("nan")
+        norm = sharded_cycle(handles, bb, x, comm, p.num_fac_cycles, p.relax_sweeps, want_norm=True)
+        o.cycle(p.b, xo, p.num_fac_cycles, p.relax_sweeps, nthreads=max_threads())
+        assert abs(norm - r_before) <= 1e-10 * r_before, (k, norm, r_before)
+        xs = torch.zeros(p.n, dtype=torch.float64, device="cuda")
+        for r in range(R):
+            xs[own0 == r] = x[r][own0 == r]
+        err = np.abs(xs.cpu().numpy() - xo).max()
+        assert err <= 1e-10 * np.abs(xo).max(), (k, err)
+    for h in handles.values():
+        m.amgdd_destroy(h)
